@@ -1,0 +1,363 @@
+#!/usr/bin/env python
+"""bench.py -- throughput of the checkerboard Monte Carlo sweep on B200 (contract: see DESIGN.md 7).
+
+    python bench.py [--gpus N] [--steps K] [--warmup W] [--impl ours|reference] [--workload NAME]
+
+One "step" = SWEEPS_PER_STEP consecutive checkerboard sweeps (both
+half-sweep launches, Philox words, threshold compare, in-place write, fused per-sweep (B, M)) of the
+BASELINE.json config-2 lattice (2D Ising spin-1/2, 8192 x 8192, T = 2.269), recorded after every
+sweep.  Rows a0/a1 (threshold table, initial state) run once at setup; a8/a9 are checked after the
+timed region.  `value` = attempted site updates per second over all ranks (Gflips/s).
+
+Prints ONE JSON line on rank 0.  N > 1 runs independent replicas (different seeds), no collective
+("replicas only").
+"""
+from __future__ import annotations
+
+import argparse
+import json
+import os
+import statistics
+import sys
+import threading
+import time
+
+ROOT = os.path.dirname(os.path.abspath(__file__))
+sys.path.insert(0, ROOT)
+
+SWEEPS_PER_STEP = 100
+BYTES_PER_UPDATE = 3  # read own colour, read other colour, write own colour (int8 split arrays)
+
+
+def parse():
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=20)
+    ap.add_argument("--warmup", type=int, default=3)
+    ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
+    ap.add_argument("--workload", default="cfg2_T2.269")
+    ap.add_argument("--sweeps-per-step", type=int, default=SWEEPS_PER_STEP)
+    ap.add_argument("--no-extras", action="store_true", help="skip the secondary workloads / cpu baseline")
+    return ap.parse_args()
+
+
+def measured_peaks():
+    p = os.path.join(ROOT, "MEASURED_PEAKS.json")
+    if os.path.exists(p):
+        try:
+            d = json.load(open(p))
+            return float(d["hbm_gbs"]), "measured (MEASURED_PEAKS.json)", d
+        except Exception:
+            pass
+    return 6650.0, "fallback (B200_PROFILING.md)", {}
+
+
+# ----------------------------------------------------------------------------- clocks sampler
+class ClockSampler(threading.Thread):
+    """Samples SM clock and throttle reasons of one GPU every 100 ms while the timed region runs."""
+
+    def __init__(self, index):
+        super().__init__(daemon=True)
+        self.index, self.samples, self.reasons, self.max_mhz = index, [], set(), None
+        self._stop_evt = threading.Event()
+        self.ok = False
+        try:
+            import pynvml
+
+            pynvml.nvmlInit()
+            self.nv = pynvml
+            self.h = pynvml.nvmlDeviceGetHandleByIndex(index)
+            self.max_mhz = pynvml.nvmlDeviceGetMaxClockInfo(self.h, pynvml.NVML_CLOCK_SM)
+            self.ok = True
+        except Exception:
+            self.ok = False
+
+    def run(self):
+        if not self.ok:
+            return
+        nv = self.nv
+        names = {
+            getattr(nv, "nvmlClocksEventReasonHwSlowdown", 0x8): "hw_slowdown",
+            getattr(nv, "nvmlClocksEventReasonHwThermalSlowdown", 0x40): "hw_thermal_slowdown",
+            getattr(nv, "nvmlClocksEventReasonSwThermalSlowdown", 0x20): "sw_thermal_slowdown",
+            getattr(nv, "nvmlClocksEventReasonSwPowerCap", 0x4): "sw_power_cap",
+        }
+        while not self._stop_evt.is_set():
+            try:
+                self.samples.append(nv.nvmlDeviceGetClockInfo(self.h, nv.NVML_CLOCK_SM))
+                try:
+                    r = nv.nvmlDeviceGetCurrentClocksEventReasons(self.h)
+                except Exception:
+                    r = nv.nvmlDeviceGetCurrentClocksThrottleReasons(self.h)
+                for bit, name in names.items():
+                    if r & bit:
+                        self.reasons.add(name)
+            except Exception:
+                pass
+            self._stop_evt.wait(0.1)
+
+    def stop(self):
+        self._stop_evt.set()
+        self.join(timeout=2)
+        return {
+            "sm_mhz": statistics.median(self.samples) if self.samples else None,
+            "sm_max_mhz": self.max_mhz,
+            "reasons": sorted(self.reasons),
+            "samples": len(self.samples),
+        }
+
+
+# ----------------------------------------------------------------------------- oracle legs (CPU)
+def time_oracle(w, L, sweeps):
+    """The oracle as it stands, one thread, on an L^dims lattice of workload w: updates/s."""
+    from oracle import lsm_oracle as O
+
+    kw = w.create_args()
+    kw["L"] = L
+    o = O.Oracle(**kw)
+    t0 = time.perf_counter()
+    o.sweep(sweeps)
+    dt = time.perf_counter() - t0
+    n = (L ** w.dims) * sweeps
+    o.close()
+    return n / dt, dt, n
+
+
+def run_reference(args, w):
+    """--impl reference: the CPU oracle on the host cores; each step = one sweep of a bounded
+    2048^2 (or 128^3) sample of the workload."""
+    rank = int(os.environ.get("RANK", "0"))
+    if rank != 0:
+        return 0
+    from oracle import lsm_oracle as O
+
+    L = 2048 if w.dims == 2 else 128
+    kw = w.create_args()
+    kw["L"] = L
+    o = O.Oracle(**kw)
+    for _ in range(args.warmup):
+        o.sweep(1)
+    t0 = time.perf_counter()
+    for _ in range(args.steps):
+        o.sweep(1)
+    dt = time.perf_counter() - t0
+    upd = (L ** w.dims) * args.steps
+    value = upd / dt / 1e9
+    sample = f"each step = 1 sweep of a {L}^{w.dims} lattice with the workload's J, h, T, seed ({L ** w.dims} updates)"
+    line = {
+        "impl": "reference", "metric": "site_updates_per_sec", "value": value, "unit": "Gflips/s",
+        "n_gpus": args.gpus, "steps": args.steps, "warmup": args.warmup, "ms_per_step": dt / args.steps * 1e3,
+        "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "int8/u32", "data": "synthetic",
+        "config": {"workload": w.name, "lattice": f"{w.L}^{w.dims}", "T": w.T, "sample": sample},
+        "cpu_baseline": {"value": value, "unit": "Gflips/s", "cores": 1, "kind": "oracle", "sample": sample},
+        "e2e": {"value": value, "unit": "Gflips/s", "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
+        "gpu_launches": 0,
+    }
+    print(json.dumps(line), flush=True)
+    return 0
+
+
+# ----------------------------------------------------------------------------- our arm (GPU)
+def run_ours(args, w):
+    import torch
+    import torch.distributed as dist
+
+    from paper_1209_0296_b200 import build, lsm
+
+    rank = int(os.environ.get("RANK", "0"))
+    local = int(os.environ.get("LOCAL_RANK", "0"))
+    world = int(os.environ.get("WORLD_SIZE", "1"))
+    if not torch.cuda.is_available():
+        raise RuntimeError("bench.py needs a CUDA device: there is no CPU fallback (use --impl reference for the oracle)")
+    torch.cuda.set_device(local)
+    if world > 1:
+        dist.init_process_group("nccl", device_id=torch.device("cuda", local))
+    build.build()
+    lsm.load()
+
+    S = args.sweeps_per_step
+    K, Wm = args.steps, max(args.warmup, 3)
+    from dataclasses import replace
+
+    wl = replace(w, seed=w.seed + 1000 * rank)  # replicas: independent seeds, no communication
+    lat = lsm.Lattice(**wl.create_args(), device=f"cuda:{local}")
+    if wl.model == lsm.ISING:
+        lat.set_tracking(False)  # persistence is not part of configs 1-4
+    N = lat.N
+    obs = torch.empty((S, 2), dtype=torch.int64, device=lat.device)
+    flush = torch.empty(256 << 20, dtype=torch.uint8, device=lat.device)  # > 126 MB L2
+
+    def barrier():
+        if world > 1:
+            dist.barrier()
+        torch.cuda.synchronize()
+
+    for _ in range(Wm):
+        lat.sweep_record(S, out=obs)
+    barrier()
+
+    sampler = ClockSampler(local)
+    sampler.start()
+    ev = [(torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)) for _ in range(K)]
+    launches0 = lat.launch_count
+    barrier()
+    for k in range(K):
+        flush.fill_(k & 0xFF)  # L2 flush between timed iterations (not timed)
+        ev[k][0].record()
+        lat.sweep_record(S, out=obs)
+        ev[k][1].record()
+    barrier()
+    clocks = sampler.stop()
+    launches = lat.launch_count - launches0
+    step_ms = [a.elapsed_time(b) for a, b in ev]
+    total_ms = sum(step_ms)
+    t = torch.tensor([total_ms], dtype=torch.float64, device=lat.device)
+    if world > 1:
+        dist.all_reduce(t, op=dist.ReduceOp.MAX)
+    total_ms_max = float(t.item())
+    updates_all = float(N) * S * K * world
+    value = updates_all / (total_ms_max * 1e-3) / 1e9
+
+    # sanity of the state after the timed region: fused running sums == full reduction (a6 vs a8)
+    Bv, Mv, tdone = lat.measure_int()
+    assert lat.measure_full() == (Bv, Mv), "fused observables disagree with the full reduction"
+    assert tdone == S * (K + Wm)
+
+    # ---- end-to-end through the C ABI with HOST buffers (pinned), copies inside the timed region
+    h_in = torch.empty(N, dtype=torch.int8).pin_memory()
+    h_in.copy_(lat.get_spins().cpu())
+    h_obs = torch.empty((S, 2), dtype=torch.int64).pin_memory()
+    Ke = max(3, min(K, 10))
+    lat.set_spins_host(h_in, tdone)
+    lat.sweep_record_host(S, h_obs)
+    barrier()
+    t0 = time.perf_counter()
+    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    e0.record()
+    for _ in range(Ke):
+        lat.set_spins_host(h_in, tdone)        # H2D of the step's input configuration (N bytes)
+        lat.sweep_record_host(S, h_obs)        # S sweeps + D2H of the (B, M) series (synchronises)
+    e1.record()
+    torch.cuda.synchronize()
+    e2e_ms = e0.elapsed_time(e1)
+    t = torch.tensor([e2e_ms], dtype=torch.float64, device=lat.device)
+    if world > 1:
+        dist.all_reduce(t, op=dist.ReduceOp.MAX)
+    e2e_value = float(N) * S * Ke * world / (float(t.item()) * 1e-3) / 1e9
+
+    if rank != 0:
+        if world > 1:
+            dist.destroy_process_group()
+        return 0
+
+    # ---- roofline of the dominant kernel (the half-sweep kernel): algorithmic bytes / launch time
+    peak, peak_src, _ = measured_peaks()
+    n_sweep_launches = 2 * S * K
+    avg_launch_s = (sum(step_ms) * 1e-3) / n_sweep_launches
+    bytes_per_launch = BYTES_PER_UPDATE * (N // 2)
+    achieved = bytes_per_launch / avg_launch_s / 1e9
+    roofline = {"bound": "hbm", "achieved": achieved, "peak": peak, "unit": "GB/s", "frac": achieved / peak,
+                "traffic": None, "peak_source": peak_src, "kernel": "half-sweep (lsm_tiled / lsm_generic)",
+                "algorithmic_bytes_per_update": BYTES_PER_UPDATE, "updates_per_launch": N // 2,
+                "avg_launch_us": avg_launch_s * 1e6}
+
+    line = {
+        "metric": "site_updates_per_sec", "value": value, "unit": "Gflips/s", "n_gpus": world, "steps": K,
+        "warmup": Wm, "ms_per_step": total_ms_max / K, "higher_is_better": True, "scaling": "weak",
+        "vs_baseline": None, "dtype": "int8/u32", "data": "synthetic",
+        "config": {"workload": wl.name, "lattice": f"{wl.L}^{wl.dims}", "model": "Ising spin-1/2" if wl.two_S == 1 and wl.model == 0 else wl.note,
+                   "T": wl.T, "J": wl.J, "h": wl.h, "sweeps_per_step": S, "record": "(B, M) after every sweep",
+                   "parallelism": "replicas only" if world > 1 else "single GPU",
+                   "kernel_family": {1: "generic", 2: "tiled", 3: "resident"}.get(lat.kernel, "?"),
+                   "l2": "256 MiB flush write between timed steps; the 64 MiB lattice is re-read from L2 within a step"},
+        "roofline": roofline,
+        "e2e": {"value": e2e_value, "unit": "Gflips/s", "h2d_bytes_per_step": N, "d2h_bytes_per_step": 16 * S,
+                "steps": Ke, "api": "lsm_set_spins_host + lsm_sweep_record_host (pinned host buffers)"},
+        "gpu_launches": int(launches),
+        "clocks": clocks,
+        "step_ms_min_med_max": [min(step_ms), statistics.median(step_ms), max(step_ms)],
+    }
+
+    if not args.no_extras and world == 1:
+        line["philox_only"] = philox_microbench(lsm, torch)
+        line["other_workloads"] = other_workloads(lsm, torch, w.name)
+        from paper_1209_0296_b200 import workloads as W
+
+        sweeps = 2
+        v, dt, n = time_oracle(w, w.L, sweeps)
+        line["cpu_baseline"] = {"value": v / 1e9, "unit": "Gflips/s", "cores": 1, "kind": "oracle",
+                                "sample": f"{sweeps} sweeps of the full {w.L}^{w.dims} lattice ({n} updates, {dt:.1f} s), single thread of {os.cpu_count()}"}
+    else:
+        line["cpu_baseline"] = None
+    print(json.dumps(line), flush=True)
+    if world > 1:
+        dist.destroy_process_group()
+    return 0
+
+
+def philox_microbench(lsm, torch):
+    """Register-only Philox4x32-10 loop: words/s the integer pipes deliver (bound for step a4)."""
+    blocks, calls = 148 * 8, 4096
+    lsm.philox_throughput(blocks, 64)
+    torch.cuda.synchronize()
+    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    e0.record()
+    sink = lsm.philox_throughput(blocks, calls)
+    e1.record()
+    torch.cuda.synchronize()
+    ms = e0.elapsed_time(e1)
+    calls_s = blocks * 256 * calls / (ms * 1e-3)
+    del sink
+    return {"gcalls_per_s": calls_s / 1e9, "gwords_per_s": 4 * calls_s / 1e9,
+            "updates_bound_gflips_1word": 4 * calls_s / 1e9, "updates_bound_gflips_2words": 2 * calls_s / 1e9}
+
+
+def other_workloads(lsm, torch, skip):
+    """Short timings of the other BASELINE.json configs (context for the headline number)."""
+    from paper_1209_0296_b200 import workloads as W
+
+    out = {}
+    for name, sweeps in (("cfg1", 1000), ("cfg2_T2.0", 100), ("cfg2_T2.6", 100), ("cfg3", 40), ("cfg4", 100),
+                         ("cfg5_c0.10", 100), ("cfg5_c0.20", 100), ("cfg5_c0.30", 100)):
+        if name == skip:
+            continue
+        w = W.configs()[name]
+        try:
+            lat = lsm.Lattice(**w.create_args())
+            if w.model == lsm.ISING:
+                lat.set_tracking(False)
+            obs = torch.empty((sweeps, 2), dtype=torch.int64, device="cuda")
+            lat.sweep_record(sweeps, out=obs)
+            torch.cuda.synchronize()
+            e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+            reps = 3
+            e0.record()
+            for _ in range(reps):
+                lat.sweep_record(sweeps, out=obs)
+                if w.model != lsm.ISING:
+                    lat.persistence()
+            e1.record()
+            torch.cuda.synchronize()
+            s = e0.elapsed_time(e1) * 1e-3
+            gf = w.N * sweeps * reps / s / 1e9
+            out[name] = {"gflips": gf, "alg_GBps": gf * BYTES_PER_UPDATE, "us_per_sweep": s / (sweeps * reps) * 1e6,
+                         "kernel_family": lat.kernel}
+            lat.close()
+            del lat, obs
+        except Exception as e:  # a secondary workload must not take the headline down
+            out[name] = {"error": repr(e)[:200]}
+    return out
+
+
+def main():
+    args = parse()
+    from paper_1209_0296_b200 import workloads as W
+
+    w = W.configs()[args.workload]
+    if args.impl == "reference":
+        return run_reference(args, w)
+    return run_ours(args, w)
+
+
+if __name__ == "__main__":
+    sys.exit(main())

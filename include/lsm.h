@@ -1,0 +1,157 @@
+/*
+ * lsm.h -- C ABI of liblsm: sublattice-parallel ("checkerboard") single-spin-flip
+ * Monte Carlo sweeps of lattice spin models on one NVIDIA B200 (sm_100a).
+ *
+ * Method: T. Levy, G. Cohen, E. Rabani, "Simulating lattice spin models on GPUs",
+ * arXiv:1209.0296.  Line references "PAPER.md:NN" are to the text of that paper;
+ * "D<n>" are the readings of DESIGN.md section 3 (= SURVEY.md 8(c)) adopted where
+ * the paper is silent or ambiguous.
+ *
+ * General rules
+ *  - Every function returns an int status (LSM_OK = 0, errors < 0).  On error the
+ *    out-parameters are left untouched.  Nothing is printed, nothing aborts.
+ *  - The library never allocates or frees device memory and never creates streams.
+ *    The caller owns the workspace, every d_* buffer and the stream (in this repo:
+ *    PyTorch tensors and torch.cuda streams).  `stream` is a cudaStream_t passed as
+ *    void* (NULL = the legacy default stream).  lsm_t itself lives on the host heap.
+ *  - Pointers named d_* are DEVICE pointers, h_* are HOST pointers; unprefixed
+ *    out-parameters (E, M, counts) are host pointers.
+ *  - Calls that take a stream only enqueue work on it (asynchronous).  Calls that
+ *    return values to the host synchronise the stream last given to this handle.
+ *  - There is no CPU fallback: without a CUDA device every compute call returns
+ *    LSM_ERR_CUDA.
+ *
+ * Models (argument `model`, `two_S`):
+ *  LSM_ISING, two_S = 1 : s_i = +/-1,  H = -J sum_<ij> s_i s_j - h sum_i s_i
+ *                         (sign convention D1); trial move s -> -s.
+ *  LSM_ISING, two_S = 2 : s_i in {-1,0,+1}, same H; trial move = one of the two other
+ *                         values, chosen uniformly (D5; BASELINE.json config 4).
+ *  LSM_NE_HEATBATH      : North-East model, occupation n_i in {0,1},
+ *                         J = 0, H = sum n_i, c = 1/(1+exp(1/T)) (D6).  A site may change
+ *                         only if its north (x,y+1) and east (x+1,y) neighbours are both
+ *                         up (D8); then n_i is redrawn from Bernoulli(c) (D7).
+ *  LSM_NE_METROPOLIS    : same constraint, Metropolis flip: 1->0 always,
+ *                         0->1 with probability exp(-1/T).
+ *  Acceptance (P = min[1, exp(-dH/T)]) is an integer compare of a 32-bit
+ *  random word w with a 33-bit threshold thr = floor(P * 2^32) in [0, 2^32]: accept iff
+ *  w < thr (D3).
+ *
+ * Lattice: periodic, hypercubic, dims = 2 or 3, linear size L (even, >= 4; D10),
+ *  N = L^dims sites, canonical site id i = x + L*(y + L*z), parity (x+y+z)&1.
+ * One sweep (= one Monte Carlo step) = half-sweep over parity 0, then over
+ *  parity 1 (the two kernel launches of PAPER.md:96-97; D9) = N attempted updates.
+ * Random numbers: Philox4x32-10, key = seed, counter = (site group, sweep, half) (D2).
+ *  The handle keeps a 64-bit sweep counter t; sweep t uses counter field t.
+ *
+ * Values at the boundary (int8): spin-1/2 -> {-1,+1}; spin-1 -> {-1,0,+1}; NE -> {0,1};
+ *  canonical order.  The device-internal encoding (split even/odd colour arrays, flag
+ *  bits) is private.
+ *
+ * Integer observables: M = sum_i s_i (NE: number of up sites); bond sum
+ *  B = sum_<ij> s_i s_j, each bond once (NE: 0).  E = -J*B - h*M (NE: E = M) (D1, D15).
+ */
+#ifndef LSM_H
+#define LSM_H
+
+#include <stddef.h>
+#include <stdint.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+typedef struct lsm lsm_t; /* opaque, host heap */
+
+enum { LSM_ISING = 0, LSM_NE_HEATBATH = 1, LSM_NE_METROPOLIS = 2 };
+enum {
+    LSM_OK = 0,
+    LSM_ERR_ARG = -1,         /* dims not 2|3, L odd or < 4, T <= 0 or non-finite, NULL, n < 0 */
+    LSM_ERR_UNSUPPORTED = -2, /* two_S not 1|2; NE with dims != 2, J != 0 or two_S != 1        */
+    LSM_ERR_CUDA = -3,        /* a CUDA runtime call failed (text: lsm_last_cuda_error)         */
+    LSM_ERR_WORKSPACE = -4,   /* workspace too small or not 256-byte aligned                   */
+    LSM_ERR_STATE = -5        /* call needs tracking to be on (lsm_persistence)                */
+};
+/* Kernel families (lsm_set_kernel).  AUTO picks the fastest one that supports the lattice. */
+enum { LSM_KERNEL_AUTO = 0, LSM_KERNEL_GENERIC = 1, LSM_KERNEL_TILED = 2, LSM_KERNEL_RESIDENT = 3 };
+
+/* Device bytes lsm_create needs for this lattice (two colour arrays + small state). */
+int lsm_workspace_bytes(int dims, int L, int two_S, int model, size_t *bytes);
+
+/* Build the threshold table on the host (D3), draw the initial state from `seed` on the
+ * device (D4: +/-1 uniform; {-1,0,+1} uniform; Bernoulli(c)), compute (B, M), take the
+ * reference snapshot (as lsm_reset_reference).  d_workspace: device, >= lsm_workspace_bytes,
+ * 256-byte aligned, owned by the caller and must outlive the handle.  Asynchronous on stream. */
+int lsm_create(int dims, int L, int two_S, int model, double J, double h, double T, uint64_t seed,
+               void *d_workspace, size_t workspace_bytes, void *stream, lsm_t **out);
+int lsm_destroy(lsm_t *);
+
+/* n checkerboard sweeps.  Asynchronous.  Observables are evaluated for the
+ * last sweep only (they feed lsm_measure). */
+int lsm_sweep(lsm_t *, int64_t n, void *stream);
+/* n sweeps, writing (B, M) after every sweep to d_obs[k][0..1], k = 0..n-1 (device, int64,
+ * 16*n bytes, overwritten).  The sums are fused into the sweep kernels (exact integers). */
+int lsm_sweep_record(lsm_t *, int64_t n, int64_t *d_obs, void *stream);
+/* Same with a HOST result buffer h_obs[n][2]; the device->host copy is enqueued on stream and
+ * the call returns after it completed (synchronises).  d_scratch: device, 16*n bytes. */
+int lsm_sweep_record_host(lsm_t *, int64_t n, int64_t *h_obs, int64_t *d_scratch, void *stream);
+
+/* Running observables of the current configuration (synchronises). */
+int lsm_measure(lsm_t *, double *E, int64_t *M);
+int lsm_measure_int(lsm_t *, int64_t *bond_sum, int64_t *M, uint64_t *sweeps_done);
+/* Recompute (B, M) from scratch with the full reduction kernel (synchronises); also refreshes
+ * the running values.  Must equal lsm_measure_int at any time. */
+int lsm_measure_full(lsm_t *, int64_t *bond_sum, int64_t *M);
+
+/* never_changed = #{i: the value of site i never differed from its predecessor since the
+ * reference time} (persistence, D12); overlap = sum_i sigma_i(ref) sigma_i(now), sigma = s
+ * (Ising) or 2n-1 (NE) (numerator of PAPER.md:120 Eq. 4, D11).  Synchronises.
+ * LSM_ERR_STATE if tracking is off. */
+int lsm_persistence(lsm_t *, int64_t *never_changed, int64_t *overlap);
+/* Reference snapshot := current configuration, "ever changed" flags cleared, tracking on. */
+int lsm_reset_reference(lsm_t *, void *stream);
+/* on = 0: stop tracking (flags and snapshot dropped; sweeps get slightly cheaper);
+ * on = 1: same as lsm_reset_reference.  Tracking is ON after lsm_create. */
+int lsm_set_tracking(lsm_t *, int on, void *stream);
+
+/* Configuration in canonical order, N int8 values. */
+int lsm_get_spins(lsm_t *, int8_t *d_out, void *stream);
+int lsm_get_spins_host(lsm_t *, int8_t *h_out, int8_t *d_scratch /* N bytes */, void *stream);
+/* Replace configuration and sweep counter, recompute (B, M); snapshot and flags untouched.
+ * Values outside the model's set give LSM_ERR_ARG only for NULL; they are not range-checked. */
+int lsm_set_spins(lsm_t *, const int8_t *d_in, uint64_t sweep_counter, void *stream);
+int lsm_set_spins_host(lsm_t *, const int8_t *h_in, int8_t *d_scratch /* N bytes */,
+                       uint64_t sweep_counter, void *stream);
+
+int lsm_set_temperature(lsm_t *, double T); /* rebuilds the thresholds (host, D3) */
+/* Host copy of the 33-bit thresholds, in the canonical order:
+ *  Ising two_S=1: idx = b*(2d+1) + (nn+2d)/2, b=(s+1)/2                         [2(2d+1)]
+ *  Ising two_S=2: idx = ((s+1)*2 + kk)*(4d+1) + (nn+2d), proposal (s+1+1+kk)%3  [6(4d+1)]
+ *  NE: {floor(c*2^32), floor(exp(-1/T)*2^32), 2^32}                              [3]
+ * out may be NULL to query count.  out must hold 128 entries. */
+int lsm_get_thresholds(lsm_t *, uint64_t *out, int *count);
+
+int lsm_set_kernel(lsm_t *, int kernel_family);           /* LSM_KERNEL_*; UNSUPPORTED if it cannot run this lattice */
+int lsm_get_kernel(lsm_t *, int *kernel_family_in_use);
+int lsm_get_launch_count(lsm_t *, uint64_t *kernels_launched); /* kernels this handle has enqueued */
+
+/* Host-side derived doubles from the integer series (D11-D13), exact integer accumulation. */
+int lsm_binder_u4(const int64_t *obs /* [n][2] host */, int64_t n, double *U4);   /* 1 - <M^4>/(3<M^2>^2) */
+int lsm_heat_capacity(const int64_t *obs, int64_t n, int64_t N, double J, double h, double T, double *C_per_site);
+int lsm_phi(int64_t overlap, int64_t N, double c, double *phi);                  /* PAPER.md:120 Eq. 4, D11 */
+int lsm_persistence_fraction(int64_t never_changed, int64_t N, double *P);
+int lsm_energy(int model, double J, double h, int64_t bond_sum, int64_t M, double *E);
+
+/* Test hooks.  lsm_philox_device: run the kernels' Philox4x32-10 on the device for n (counter, key)
+ * pairs: d_ctr_key[n][6] -> d_out[n][4] (uint32, device).  lsm_philox_throughput: register-only
+ * Philox microbenchmark (integer roofline): every thread of `blocks` x 256 runs `calls` dependent
+ * calls and writes one word to d_sink[blocks*256]. */
+int lsm_philox_device(const uint32_t *d_ctr_key, uint32_t *d_out, int64_t n, void *stream);
+int lsm_philox_throughput(int blocks, int calls, uint32_t *d_sink, void *stream);
+
+const char *lsm_strerror(int code);
+const char *lsm_last_cuda_error(void);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* LSM_H */

@@ -1,0 +1,459 @@
+// lsm_api.cu -- host side of the C ABI declared in include/lsm.h.  Argument checks, the threshold
+// table (reading D3), kernel-family dispatch and stream-ordered bookkeeping; every step of the hot
+// path itself runs in the kernels of lsm_generic.cu / lsm_tiled.cu.
+#include "../../include/lsm.h"
+#include "lsm_internal.cuh"
+#include "lsm_tiled.cuh"
+
+#include <cmath>
+#include <cstdlib>
+#include <cstring>
+#include <new>
+#include <string>
+
+using namespace lsmk;
+
+struct lsm {
+    int dims, L, two_S, model_abi, model;
+    double J, h, T, c;
+    uint64_t seed;
+    int64_t N;
+    Lat lat;
+    long long *d_run;   // running (B, M) of the current configuration
+    long long *d_tmp;   // scratch pair for reductions
+    uint64_t t;         // sweeps done
+    int tracking;
+    int kernel_pref, kernel_in_use;
+    cudaStream_t last_stream;
+    uint64_t launches;
+    uint64_t thr[128];
+    int nthr;
+    Thr64 thr_param;
+    TiledTables tiled;
+};
+
+static thread_local std::string g_cuda_err;
+static int cuda_fail(cudaError_t e)
+{
+    g_cuda_err = std::string(cudaGetErrorName(e)) + ": " + cudaGetErrorString(e);
+    return LSM_ERR_CUDA;
+}
+#define CU(x) do { cudaError_t e__ = (x); if (e__ != cudaSuccess) return cuda_fail(e__); } while (0)
+
+static size_t align256(size_t v) { return (v + 255) & ~(size_t)255; }
+static const size_t STATE_BYTES = 256;
+
+static int check_shape(int dims, int L, int two_S, int model)
+{
+    if (dims != 2 && dims != 3) return LSM_ERR_ARG;
+    if (L < 4 || (L & 1)) return LSM_ERR_ARG;
+    if (dims == 2 && L > 131072) return LSM_ERR_ARG;
+    if (dims == 3 && L > 2048) return LSM_ERR_ARG;
+    if (model == LSM_ISING) { if (two_S != 1 && two_S != 2) return LSM_ERR_UNSUPPORTED; }
+    else if (model == LSM_NE_HEATBATH || model == LSM_NE_METROPOLIS) {
+        if (dims != 2 || two_S != 1) return LSM_ERR_UNSUPPORTED;
+    } else return LSM_ERR_ARG;
+    return LSM_OK;
+}
+
+extern "C" int lsm_workspace_bytes(int dims, int L, int two_S, int model, size_t *bytes)
+{
+    if (!bytes) return LSM_ERR_ARG;
+    int rc = check_shape(dims, L, two_S, model);
+    if (rc != LSM_OK) return rc;
+    size_t N = (size_t)L * L * (dims == 3 ? (size_t)L : 1);
+    *bytes = STATE_BYTES + 2 * align256(N / 2) + 256;
+    return LSM_OK;
+}
+
+// ---------------------------------------------------------------------------- thresholds (a0)
+// Reading D3: x = J*nn + h; dE = -(s'-s)*x; p = exp(-dE/T); thr = 2^32 if dE <= 0 or p >= 1,
+// else floor(p * 2^32).  Plain IEEE double, division by T, no contraction (-ffp-contract=off).
+static uint64_t thr_from_p(double p)
+{
+    if (p >= 1.0) return (uint64_t)1 << 32;
+    return (uint64_t)std::floor(std::ldexp(p, 32));
+}
+static uint64_t thr_flip(double J, double h, double T, int s_old, int s_new, int nn)
+{
+    double x = J * (double)nn + h;
+    double dE = -(double)(s_new - s_old) * x;
+    if (dE <= 0.0) return (uint64_t)1 << 32;
+    return thr_from_p(std::exp(-dE / T));
+}
+
+static void build_tables(lsm *o)
+{
+    const int d = o->dims;
+    int n = 0;
+    if (o->model == M_ISING_HALF) {
+        for (int b = 0; b < 2; ++b)
+            for (int j = 0; j <= 2 * d; ++j) o->thr[n++] = thr_flip(o->J, o->h, o->T, 2 * b - 1, 1 - 2 * b, 2 * j - 2 * d);
+    } else if (o->model == M_ISING_ONE) {
+        for (int a = 0; a < 3; ++a)
+            for (int kk = 0; kk < 2; ++kk)
+                for (int j = 0; j <= 4 * d; ++j)
+                    o->thr[n++] = thr_flip(o->J, o->h, o->T, a - 1, (a + 1 + kk) % 3 - 1, j - 2 * d);
+    } else {
+        o->c = 1.0 / (1.0 + std::exp(1.0 / o->T));          // reading D6
+        o->thr[n++] = thr_from_p(o->c);
+        o->thr[n++] = thr_from_p(std::exp(-1.0 / o->T));
+        o->thr[n++] = (uint64_t)1 << 32;
+    }
+    o->nthr = n;
+    std::memset(&o->thr_param, 0, sizeof(o->thr_param));
+    for (int i = 0; i < n; ++i) o->thr_param.thr[i] = o->thr[i];
+    o->thr_param.count = n;
+    build_tiled_tables(o->model, d, o->J, o->h, o->thr, n, &o->tiled);
+}
+
+static void choose_kernel(lsm *o)
+{
+    int want = o->kernel_pref;
+    bool tiled_ok = tiled_supported(o->lat, o->model, o->tiled);
+    if (want == LSM_KERNEL_AUTO) want = tiled_ok ? LSM_KERNEL_TILED : LSM_KERNEL_GENERIC;
+    if (want == LSM_KERNEL_TILED && !tiled_ok) want = LSM_KERNEL_GENERIC;
+    if (want == LSM_KERNEL_RESIDENT) want = tiled_ok ? LSM_KERNEL_TILED : LSM_KERNEL_GENERIC;
+    o->kernel_in_use = want;
+}
+
+// ---------------------------------------------------------------------------- life cycle
+static int refresh_running(lsm *o, cudaStream_t s)
+{
+    CU(launch_measure_full(o->lat, o->model, o->d_run, s));
+    o->launches += 1;
+    return LSM_OK;
+}
+
+extern "C" int lsm_create(int dims, int L, int two_S, int model, double J, double h, double T, uint64_t seed,
+                          void *d_workspace, size_t workspace_bytes, void *stream, lsm_t **out)
+{
+    if (!out || !d_workspace) return LSM_ERR_ARG;
+    int rc = check_shape(dims, L, two_S, model);
+    if (rc != LSM_OK) return rc;
+    if (!(T > 0.0) || !std::isfinite(T) || !std::isfinite(J) || !std::isfinite(h)) return LSM_ERR_ARG;
+    if (model != LSM_ISING && J != 0.0) return LSM_ERR_UNSUPPORTED;
+    size_t need = 0;
+    lsm_workspace_bytes(dims, L, two_S, model, &need);
+    if (workspace_bytes < need || ((uintptr_t)d_workspace & 255)) return LSM_ERR_WORKSPACE;
+
+    lsm *o = new (std::nothrow) lsm();
+    if (!o) return LSM_ERR_ARG;
+    o->dims = dims; o->L = L; o->two_S = two_S; o->model_abi = model;
+    o->model = model == LSM_ISING ? (two_S == 1 ? M_ISING_HALF : M_ISING_ONE)
+             : (model == LSM_NE_HEATBATH ? M_NE_HEATBATH : M_NE_METROPOLIS);
+    o->J = J; o->h = h; o->T = T; o->c = 0.0; o->seed = seed;
+    o->N = (int64_t)L * L * (dims == 3 ? L : 1);
+    uint8_t *base = (uint8_t *)d_workspace;
+    o->d_run = (long long *)base;
+    o->d_tmp = (long long *)(base + 64);
+    o->lat.col[0] = base + STATE_BYTES;
+    o->lat.col[1] = base + STATE_BYTES + align256((size_t)o->N / 2);
+    o->lat.L = L; o->lat.Lh = L / 2; o->lat.dims = dims; o->lat.Lz = dims == 3 ? L : 1;
+    o->lat.half = o->N / 2;
+    o->t = 0; o->tracking = 1; o->kernel_pref = LSM_KERNEL_AUTO; o->launches = 0;
+    o->last_stream = (cudaStream_t)stream;
+    build_tables(o);
+    choose_kernel(o);
+
+    cudaStream_t s = (cudaStream_t)stream;
+    cudaError_t e = cudaMemsetAsync(base, 0, STATE_BYTES, s);
+    if (e == cudaSuccess) e = launch_init(o->lat, o->model, seed, o->thr[0], s);
+    if (e == cudaSuccess) e = launch_reset_reference(o->lat, o->model, 1, s);
+    if (e == cudaSuccess) e = launch_measure_full(o->lat, o->model, o->d_run, s);
+    if (e != cudaSuccess) { delete o; return cuda_fail(e); }
+    o->launches += 3;
+    *out = o;
+    return LSM_OK;
+}
+
+extern "C" int lsm_destroy(lsm_t *o)
+{
+    if (!o) return LSM_ERR_ARG;
+    delete o;
+    return LSM_OK;
+}
+
+// ---------------------------------------------------------------------------- sweeps (a2-a7)
+static int enqueue_half(lsm *o, int half, long long *obs, int want_B, cudaStream_t s)
+{
+    SweepArgs a;
+    a.lat = o->lat; a.model = o->model; a.half = half;
+    a.key = make_sweep_key(o->seed, o->t, (uint32_t)half);
+    a.track = o->tracking; a.obs = obs; a.want_B = want_B;
+    if (o->kernel_in_use == LSM_KERNEL_TILED) CU(launch_sweep_tiled(a, o->tiled, s));
+    else CU(launch_sweep_generic(a, o->thr_param, s));
+    o->launches += 1;
+    return LSM_OK;
+}
+
+static int sweep_impl(lsm *o, int64_t n, long long *d_obs, cudaStream_t s)
+{
+    o->last_stream = s;
+    if (n == 0) return LSM_OK;
+    if (d_obs) CU(cudaMemsetAsync(d_obs, 0, (size_t)n * 16, s));
+    else CU(cudaMemsetAsync(o->d_run, 0, 16, s));
+    for (int64_t k = 0; k < n; ++k) {
+        long long *obs = d_obs ? d_obs + 2 * k : (k == n - 1 ? o->d_run : nullptr);
+        int rc = enqueue_half(o, 0, obs, 0, s);
+        if (rc != LSM_OK) return rc;
+        rc = enqueue_half(o, 1, obs, 1, s);
+        if (rc != LSM_OK) return rc;
+        o->t += 1;
+    }
+    if (d_obs) CU(cudaMemcpyAsync(o->d_run, d_obs + 2 * (n - 1), 16, cudaMemcpyDeviceToDevice, s));
+    return LSM_OK;
+}
+
+extern "C" int lsm_sweep(lsm_t *o, int64_t n, void *stream)
+{
+    if (!o || n < 0) return LSM_ERR_ARG;
+    return sweep_impl(o, n, nullptr, (cudaStream_t)stream);
+}
+
+extern "C" int lsm_sweep_record(lsm_t *o, int64_t n, int64_t *d_obs, void *stream)
+{
+    if (!o || n < 0 || (!d_obs && n > 0)) return LSM_ERR_ARG;
+    return sweep_impl(o, n, (long long *)d_obs, (cudaStream_t)stream);
+}
+
+extern "C" int lsm_sweep_record_host(lsm_t *o, int64_t n, int64_t *h_obs, int64_t *d_scratch, void *stream)
+{
+    if (!o || n < 0 || ((!h_obs || !d_scratch) && n > 0)) return LSM_ERR_ARG;
+    cudaStream_t s = (cudaStream_t)stream;
+    int rc = sweep_impl(o, n, (long long *)d_scratch, s);
+    if (rc != LSM_OK) return rc;
+    if (n > 0) CU(cudaMemcpyAsync(h_obs, d_scratch, (size_t)n * 16, cudaMemcpyDeviceToHost, s));
+    CU(cudaStreamSynchronize(s));
+    return LSM_OK;
+}
+
+// ---------------------------------------------------------------------------- observables
+static int read_pair(lsm *o, const long long *d, long long out[2])
+{
+    CU(cudaMemcpyAsync(out, d, 16, cudaMemcpyDeviceToHost, o->last_stream));
+    CU(cudaStreamSynchronize(o->last_stream));
+    return LSM_OK;
+}
+
+extern "C" int lsm_energy(int model, double J, double h, int64_t B, int64_t M, double *E)
+{
+    if (!E) return LSM_ERR_ARG;
+    *E = model == LSM_ISING ? -J * (double)B - h * (double)M : (double)M;   // D1, D15
+    return LSM_OK;
+}
+
+extern "C" int lsm_measure_int(lsm_t *o, int64_t *B, int64_t *M, uint64_t *sweeps_done)
+{
+    if (!o) return LSM_ERR_ARG;
+    long long v[2];
+    int rc = read_pair(o, o->d_run, v);
+    if (rc != LSM_OK) return rc;
+    if (B) *B = v[0];
+    if (M) *M = v[1];
+    if (sweeps_done) *sweeps_done = o->t;
+    return LSM_OK;
+}
+
+extern "C" int lsm_measure(lsm_t *o, double *E, int64_t *M)
+{
+    if (!o) return LSM_ERR_ARG;
+    int64_t b, m;
+    int rc = lsm_measure_int(o, &b, &m, nullptr);
+    if (rc != LSM_OK) return rc;
+    if (E) lsm_energy(o->model_abi, o->J, o->h, b, m, E);
+    if (M) *M = m;
+    return LSM_OK;
+}
+
+extern "C" int lsm_measure_full(lsm_t *o, int64_t *B, int64_t *M)
+{
+    if (!o) return LSM_ERR_ARG;
+    int rc = refresh_running(o, o->last_stream);
+    if (rc != LSM_OK) return rc;
+    return lsm_measure_int(o, B, M, nullptr);
+}
+
+extern "C" int lsm_persistence(lsm_t *o, int64_t *never_changed, int64_t *overlap)
+{
+    if (!o) return LSM_ERR_ARG;
+    if (!o->tracking) return LSM_ERR_STATE;
+    CU(launch_persistence(o->lat, o->model, o->d_tmp, o->last_stream));
+    o->launches += 1;
+    long long v[2];
+    int rc = read_pair(o, o->d_tmp, v);
+    if (rc != LSM_OK) return rc;
+    if (never_changed) *never_changed = v[0];
+    if (overlap) *overlap = v[1];
+    return LSM_OK;
+}
+
+extern "C" int lsm_set_tracking(lsm_t *o, int on, void *stream)
+{
+    if (!o) return LSM_ERR_ARG;
+    cudaStream_t s = (cudaStream_t)stream;
+    o->last_stream = s;
+    CU(launch_reset_reference(o->lat, o->model, on ? 1 : 0, s));
+    o->launches += 1;
+    o->tracking = on ? 1 : 0;
+    return LSM_OK;
+}
+
+extern "C" int lsm_reset_reference(lsm_t *o, void *stream) { return lsm_set_tracking(o, 1, stream); }
+
+// ---------------------------------------------------------------------------- configuration I/O
+extern "C" int lsm_get_spins(lsm_t *o, int8_t *d_out, void *stream)
+{
+    if (!o || !d_out) return LSM_ERR_ARG;
+    o->last_stream = (cudaStream_t)stream;
+    CU(launch_get_spins(o->lat, o->model, d_out, o->last_stream));
+    o->launches += 1;
+    return LSM_OK;
+}
+
+extern "C" int lsm_get_spins_host(lsm_t *o, int8_t *h_out, int8_t *d_scratch, void *stream)
+{
+    if (!o || !h_out || !d_scratch) return LSM_ERR_ARG;
+    int rc = lsm_get_spins(o, d_scratch, stream);
+    if (rc != LSM_OK) return rc;
+    CU(cudaMemcpyAsync(h_out, d_scratch, (size_t)o->N, cudaMemcpyDeviceToHost, o->last_stream));
+    CU(cudaStreamSynchronize(o->last_stream));
+    return LSM_OK;
+}
+
+extern "C" int lsm_set_spins(lsm_t *o, const int8_t *d_in, uint64_t sweep_counter, void *stream)
+{
+    if (!o || !d_in) return LSM_ERR_ARG;
+    o->last_stream = (cudaStream_t)stream;
+    CU(launch_set_spins(o->lat, o->model, d_in, o->last_stream));
+    o->launches += 1;
+    o->t = sweep_counter;
+    return refresh_running(o, o->last_stream);
+}
+
+extern "C" int lsm_set_spins_host(lsm_t *o, const int8_t *h_in, int8_t *d_scratch, uint64_t sweep_counter, void *stream)
+{
+    if (!o || !h_in || !d_scratch) return LSM_ERR_ARG;
+    CU(cudaMemcpyAsync(d_scratch, h_in, (size_t)o->N, cudaMemcpyHostToDevice, (cudaStream_t)stream));
+    return lsm_set_spins(o, d_scratch, sweep_counter, stream);
+}
+
+extern "C" int lsm_set_temperature(lsm_t *o, double T)
+{
+    if (!o || !(T > 0.0) || !std::isfinite(T)) return LSM_ERR_ARG;
+    o->T = T;
+    build_tables(o);
+    choose_kernel(o);
+    return LSM_OK;
+}
+
+extern "C" int lsm_get_thresholds(lsm_t *o, uint64_t *out, int *count)
+{
+    if (!o || !count) return LSM_ERR_ARG;
+    if (out) for (int i = 0; i < o->nthr; ++i) out[i] = o->thr[i];
+    *count = o->nthr;
+    return LSM_OK;
+}
+
+extern "C" int lsm_set_kernel(lsm_t *o, int family)
+{
+    if (!o || family < LSM_KERNEL_AUTO || family > LSM_KERNEL_RESIDENT) return LSM_ERR_ARG;
+    if (family == LSM_KERNEL_TILED && !tiled_supported(o->lat, o->model, o->tiled)) return LSM_ERR_UNSUPPORTED;
+    if (family == LSM_KERNEL_RESIDENT) return LSM_ERR_UNSUPPORTED;
+    o->kernel_pref = family;
+    choose_kernel(o);
+    return LSM_OK;
+}
+
+extern "C" int lsm_get_kernel(lsm_t *o, int *family)
+{
+    if (!o || !family) return LSM_ERR_ARG;
+    *family = o->kernel_in_use;
+    return LSM_OK;
+}
+
+extern "C" int lsm_get_launch_count(lsm_t *o, uint64_t *n)
+{
+    if (!o || !n) return LSM_ERR_ARG;
+    *n = o->launches;
+    return LSM_OK;
+}
+
+// ---------------------------------------------------------------------------- derived doubles
+extern "C" int lsm_binder_u4(const int64_t *obs, int64_t n, double *U4)
+{
+    if (!obs || !U4 || n <= 0) return LSM_ERR_ARG;
+    unsigned __int128 s2 = 0, s4 = 0;
+    for (int64_t k = 0; k < n; ++k) {
+        __int128 m = obs[2 * k + 1];
+        unsigned __int128 m2 = (unsigned __int128)(m * m);
+        s2 += m2;
+        s4 += m2 * m2;
+    }
+    if (s2 == 0) return LSM_ERR_ARG;
+    long double a = (long double)s4 * (long double)n, b = 3.0L * (long double)s2 * (long double)s2;
+    *U4 = (double)(1.0L - a / b);
+    return LSM_OK;
+}
+
+extern "C" int lsm_heat_capacity(const int64_t *obs, int64_t n, int64_t N, double J, double h, double T, double *C)
+{
+    if (!obs || !C || n <= 0 || N <= 0 || !(T > 0.0)) return LSM_ERR_ARG;
+    long double mean = 0.0L;
+    for (int64_t k = 0; k < n; ++k) mean += -(long double)J * obs[2 * k] - (long double)h * obs[2 * k + 1];
+    mean /= (long double)n;
+    long double var = 0.0L;
+    for (int64_t k = 0; k < n; ++k) {
+        long double e = -(long double)J * obs[2 * k] - (long double)h * obs[2 * k + 1] - mean;
+        var += e * e;
+    }
+    var /= (long double)n;
+    *C = (double)(var / ((long double)N * (long double)T * (long double)T));
+    return LSM_OK;
+}
+
+extern "C" int lsm_phi(int64_t overlap, int64_t N, double c, double *phi)
+{
+    if (!phi || N <= 0) return LSM_ERR_ARG;
+    double q = (2.0 * c - 1.0) * (2.0 * c - 1.0);
+    if (q >= 1.0) return LSM_ERR_ARG;
+    *phi = ((double)overlap / (double)N - q) / (1.0 - q);
+    return LSM_OK;
+}
+
+extern "C" int lsm_persistence_fraction(int64_t never_changed, int64_t N, double *P)
+{
+    if (!P || N <= 0) return LSM_ERR_ARG;
+    *P = (double)never_changed / (double)N;
+    return LSM_OK;
+}
+
+// ---------------------------------------------------------------------------- test hooks
+extern "C" int lsm_philox_device(const uint32_t *d_ck, uint32_t *d_out, int64_t n, void *stream)
+{
+    if (n < 0 || ((!d_ck || !d_out) && n > 0)) return LSM_ERR_ARG;
+    CU(launch_philox_device(d_ck, d_out, n, (cudaStream_t)stream));
+    return LSM_OK;
+}
+
+extern "C" int lsm_philox_throughput(int blocks, int calls, uint32_t *d_sink, void *stream)
+{
+    if (blocks <= 0 || calls < 0 || !d_sink) return LSM_ERR_ARG;
+    CU(launch_philox_throughput(blocks, calls, d_sink, (cudaStream_t)stream));
+    return LSM_OK;
+}
+
+extern "C" const char *lsm_strerror(int code)
+{
+    switch (code) {
+    case LSM_OK: return "ok";
+    case LSM_ERR_ARG: return "invalid argument";
+    case LSM_ERR_UNSUPPORTED: return "unsupported model / lattice / kernel combination";
+    case LSM_ERR_CUDA: return "CUDA runtime error (see lsm_last_cuda_error)";
+    case LSM_ERR_WORKSPACE: return "workspace too small or misaligned";
+    case LSM_ERR_STATE: return "tracking is off";
+    default: return "unknown error code";
+    }
+}
+
+extern "C" const char *lsm_last_cuda_error(void) { return g_cuda_err.c_str(); }

@@ -1,0 +1,397 @@
+// lsm_generic.cu -- the scalar kernel family: one thread per site of the active colour, any even
+// L >= 4, every model.  It is the first parity-checked path and the fallback for lattices the tiled
+// kernels do not cover; it also holds the once-per-call kernels (initial state, full reduction,
+// persistence/overlap reduction, layout conversion) and the Philox test hooks.
+//
+// Method: PAPER.md:88 (Metropolis), 90-98 (two launches per sweep, one per sublattice), 118 (NE
+// constraint); readings D1-D12 of DESIGN.md.  No code is shared with oracle/.
+#include "lsm_internal.cuh"
+
+namespace lsmk {
+
+int sm_count()
+{
+    static int n = 0;
+    if (n == 0) {
+        int dev = 0;
+        if (cudaGetDevice(&dev) != cudaSuccess) return 148;
+        if (cudaDeviceGetAttribute(&n, cudaDevAttrMultiProcessorCount, dev) != cudaSuccess || n <= 0) n = 148;
+    }
+    return n;
+}
+
+static inline int grid_for(long long work_items, int threads, int ctas_per_sm)
+{
+    long long g = (work_items + threads - 1) / threads;
+    long long cap = (long long)sm_count() * ctas_per_sm;
+    if (g > cap) g = cap;
+    if (g < 1) g = 1;
+    return (int)g;
+}
+
+// ------------------------------------------------------------------------------------------
+// Geometry of the split layout.  Colour c holds the sites with (x+y+z)&1 == c; inside its array a
+// site sits at k = i>>1 = m + Lh*(y + L*z) with x = 2m + q, q = (y+z+c)&1.  Its six (four)
+// neighbours all have the other colour: same m in rows y+-1 and planes z+-1, and in its own row the
+// bytes m and m+1 (q = 1) or m-1 and m (q = 0).
+// ------------------------------------------------------------------------------------------
+struct Site {
+    int m, y, z, q;
+    long long row;   // (z*L + y) * Lh
+};
+__device__ __forceinline__ Site site_of(const Lat &lat, long long k, int colour)
+{
+    Site s;
+    long long r = k / lat.Lh;
+    s.m = (int)(k - r * lat.Lh);
+    s.z = (int)(r / lat.L);
+    s.y = (int)(r - (long long)s.z * lat.L);
+    s.q = (s.y + s.z + colour) & 1;
+    s.row = r * lat.Lh;
+    return s;
+}
+
+template <int MODEL>
+__device__ __forceinline__ int neighbour_value_sum(const Lat &lat, const uint8_t *__restrict__ oth, const Site &s,
+                                                   uint32_t &north, uint32_t &east)
+{
+    constexpr uint32_t VAL = Enc<MODEL>::VAL;
+    const int L = lat.L, Lh = lat.Lh;
+    int yu = s.y + 1 == L ? 0 : s.y + 1, yd = s.y == 0 ? L - 1 : s.y - 1;
+    long long plane = (long long)s.z * L;
+    uint32_t up = oth[(plane + yu) * Lh + s.m] & VAL;
+    uint32_t dn = oth[(plane + yd) * Lh + s.m] & VAL;
+    uint32_t ce = oth[s.row + s.m] & VAL;
+    int ms = s.q ? (s.m + 1 == Lh ? 0 : s.m + 1) : (s.m == 0 ? Lh - 1 : s.m - 1);
+    uint32_t sd = oth[s.row + ms] & VAL;
+    int sum = (int)(up + dn + ce + sd);
+    if (lat.dims == 3) {
+        int zu = s.z + 1 == L ? 0 : s.z + 1, zd = s.z == 0 ? L - 1 : s.z - 1;
+        sum += (int)(oth[((long long)zu * L + s.y) * Lh + s.m] & VAL);
+        sum += (int)(oth[((long long)zd * L + s.y) * Lh + s.m] & VAL);
+    }
+    north = up;                 // (x, y+1)
+    east = s.q ? sd : ce;       // (x+1, y): byte m+1 of the row when q = 1, byte m when q = 0
+    return sum;
+}
+
+// ------------------------------------------------------------------------------------------
+// a2-a6, scalar form.
+// ------------------------------------------------------------------------------------------
+template <int MODEL>
+__global__ void __launch_bounds__(256) k_sweep_generic(SweepArgs a, Thr64 thr)
+{
+    constexpr uint32_t VAL = Enc<MODEL>::VAL, CHG = Enc<MODEL>::CHG;
+    __shared__ unsigned long long s_thr[96];
+    for (int i = threadIdx.x; i < 96; i += blockDim.x) s_thr[i] = thr.thr[i];
+    __syncthreads();
+
+    const Lat &lat = a.lat;
+    uint8_t *__restrict__ own = a.half ? lat.col[1] : lat.col[0];
+    const uint8_t *__restrict__ oth = a.half ? lat.col[0] : lat.col[1];
+    const int d = lat.dims;
+    long long accB = 0, accM = 0;
+
+    for (long long k = (long long)blockIdx.x * blockDim.x + threadIdx.x; k < lat.half;
+         k += (long long)gridDim.x * blockDim.x) {
+        Site s = site_of(lat, k, a.half);
+        uint32_t old = own[k], v = old & VAL, vn = v;
+        uint32_t north, east;
+        int sum = neighbour_value_sum<MODEL>(lat, oth, s, north, east);
+        int s_new, nn;
+        if (MODEL == M_ISING_HALF) {
+            uint4 r = philox4x32_10((uint32_t)(k >> 2), (uint32_t)(k >> 34), a.key.c2, a.key.c3, a.key.k0, a.key.k1);
+            uint32_t w = (k & 2) ? ((k & 1) ? r.w : r.z) : ((k & 1) ? r.y : r.x);
+            unsigned long long t = s_thr[v * (2 * d + 1) + sum];
+            if ((unsigned long long)w < t) vn = v ^ 1u;
+            s_new = 2 * (int)vn - 1;
+            nn = 2 * sum - 2 * d;
+        } else if (MODEL == M_ISING_ONE) {
+            uint4 r = philox4x32_10((uint32_t)(k >> 1), (uint32_t)(k >> 33), a.key.c2, a.key.c3, a.key.k0, a.key.k1);
+            uint32_t w0 = (k & 1) ? r.z : r.x, w1 = (k & 1) ? r.w : r.y;
+            uint32_t kk = w0 >> 31;
+            uint32_t ap = v + 1 + kk;
+            ap = ap >= 3 ? ap - 3 : ap;
+            unsigned long long t = s_thr[(v * 2 + kk) * (4 * d + 1) + sum];
+            if ((unsigned long long)w1 < t) vn = ap;
+            s_new = (int)vn - 1;
+            nn = sum - 2 * d;
+        } else {
+            if (north & east) {
+                uint4 r = philox4x32_10((uint32_t)(k >> 2), (uint32_t)(k >> 34), a.key.c2, a.key.c3, a.key.k0, a.key.k1);
+                uint32_t w = (k & 2) ? ((k & 1) ? r.w : r.z) : ((k & 1) ? r.y : r.x);
+                if (MODEL == M_NE_HEATBATH) vn = ((unsigned long long)w < s_thr[0]) ? 1u : 0u;
+                else if ((unsigned long long)w < s_thr[1 + v]) vn = v ^ 1u;
+            }
+            s_new = (int)vn;
+            nn = 0;
+        }
+        if (vn != v) {
+            uint32_t nb = (old & ~VAL) | vn;
+            if (a.track) nb |= CHG;
+            own[k] = (uint8_t)nb;
+        }
+        accM += s_new;
+        accB += s_new * nn;
+    }
+    if (a.obs) block_accumulate2(accB, accM, a.obs, a.want_B != 0, true);
+}
+
+cudaError_t launch_sweep_generic(const SweepArgs &a, const Thr64 &thr, cudaStream_t s)
+{
+    int grid = grid_for(a.lat.half, 256, 8);
+    switch (a.model) {
+    case M_ISING_HALF:    k_sweep_generic<M_ISING_HALF><<<grid, 256, 0, s>>>(a, thr); break;
+    case M_ISING_ONE:     k_sweep_generic<M_ISING_ONE><<<grid, 256, 0, s>>>(a, thr); break;
+    case M_NE_HEATBATH:   k_sweep_generic<M_NE_HEATBATH><<<grid, 256, 0, s>>>(a, thr); break;
+    default:              k_sweep_generic<M_NE_METROPOLIS><<<grid, 256, 0, s>>>(a, thr); break;
+    }
+    return cudaGetLastError();
+}
+
+// ------------------------------------------------------------------------------------------
+// a1: initial state (reading D4): stream 2, t = 0, group = i>>2 over the CANONICAL id, word i&3.
+// ------------------------------------------------------------------------------------------
+__global__ void __launch_bounds__(256) k_init(Lat lat, int model, SweepKey key, unsigned long long thr_c)
+{
+    long long groups = (2 * lat.half + 3) >> 2;
+    for (long long g = (long long)blockIdx.x * blockDim.x + threadIdx.x; g < groups;
+         g += (long long)gridDim.x * blockDim.x) {
+        uint4 r = philox4x32_10((uint32_t)g, (uint32_t)(g >> 32), key.c2, key.c3, key.k0, key.k1);
+        uint32_t w[4] = {r.x, r.y, r.z, r.w};
+#pragma unroll
+        for (int j = 0; j < 4; ++j) {
+            long long i = 4 * g + j;
+            if (i >= 2 * lat.half) break;
+            long long ry = i / lat.L;
+            int x = (int)(i - ry * lat.L);
+            int z = (int)(ry / lat.L);
+            int y = (int)(ry - (long long)z * lat.L);
+            uint32_t v;
+            if (model == M_ISING_HALF) v = w[j] >> 31;
+            else if (model == M_ISING_ONE) v = __umulhi(w[j], 3u);
+            else v = ((unsigned long long)w[j] < thr_c) ? 1u : 0u;
+            uint8_t *dst = ((x + y + z) & 1) ? lat.col[1] : lat.col[0];
+            dst[i >> 1] = (uint8_t)v;
+        }
+    }
+}
+
+cudaError_t launch_init(const Lat &lat, int model, unsigned long long seed, unsigned long long thr_c, cudaStream_t s)
+{
+    SweepKey key = make_sweep_key(seed, 0ull, 2u);
+    long long groups = (2 * lat.half + 3) >> 2;
+    k_init<<<grid_for(groups, 256, 8), 256, 0, s>>>(lat, model, key, thr_c);
+    return cudaGetLastError();
+}
+
+// ------------------------------------------------------------------------------------------
+// a8: full reduction.  Every bond joins a colour-0 and a colour-1 site, so
+// B = sum over colour-0 sites of s_i * nn_i; M sums both colours.
+// ------------------------------------------------------------------------------------------
+template <int MODEL>
+__global__ void __launch_bounds__(256) k_measure_full(Lat lat, long long *out)
+{
+    constexpr uint32_t VAL = Enc<MODEL>::VAL;
+    const uint8_t *__restrict__ c0 = lat.col[0];
+    const uint8_t *__restrict__ c1 = lat.col[1];
+    long long accB = 0, accM = 0;
+    for (long long k = (long long)blockIdx.x * blockDim.x + threadIdx.x; k < lat.half;
+         k += (long long)gridDim.x * blockDim.x) {
+        Site s = site_of(lat, k, 0);
+        uint32_t north, east;
+        int sum = neighbour_value_sum<MODEL>(lat, c1, s, north, east);
+        int v0 = (int)(c0[k] & VAL), v1 = (int)(c1[k] & VAL);
+        if (MODEL == M_ISING_HALF) {
+            accM += 2 * (v0 + v1) - 2;
+            accB += (2 * v0 - 1) * (2 * sum - 2 * lat.dims);
+        } else if (MODEL == M_ISING_ONE) {
+            accM += v0 + v1 - 2;
+            accB += (v0 - 1) * (sum - 2 * lat.dims);
+        } else {
+            accM += v0 + v1;
+        }
+    }
+    block_accumulate2(accB, accM, out, true, true);
+}
+
+cudaError_t launch_measure_full(const Lat &lat, int model, long long *d_BM, cudaStream_t s)
+{
+    cudaError_t e = cudaMemsetAsync(d_BM, 0, 2 * sizeof(long long), s);
+    if (e != cudaSuccess) return e;
+    int grid = grid_for(lat.half, 256, 8);
+    if (model == M_ISING_HALF) k_measure_full<M_ISING_HALF><<<grid, 256, 0, s>>>(lat, d_BM);
+    else if (model == M_ISING_ONE) k_measure_full<M_ISING_ONE><<<grid, 256, 0, s>>>(lat, d_BM);
+    else k_measure_full<M_NE_HEATBATH><<<grid, 256, 0, s>>>(lat, d_BM);
+    return cudaGetLastError();
+}
+
+// ------------------------------------------------------------------------------------------
+// a9: persistence / overlap reduction over the flag and reference bits (readings D11, D12).
+// 16 sites per 128-bit load.
+// ------------------------------------------------------------------------------------------
+template <int MODEL>
+__device__ __forceinline__ void persist_byte(uint32_t b, long long &nc, long long &ov)
+{
+    constexpr uint32_t VAL = Enc<MODEL>::VAL, CHG = Enc<MODEL>::CHG, REF = Enc<MODEL>::REF;
+    constexpr int SH = Enc<MODEL>::REF_SHIFT;
+    nc += (b & CHG) ? 0 : 1;
+    int now = (int)(b & VAL), ref = (int)((b & REF) >> SH);
+    if (MODEL == M_ISING_ONE) ov += (now - 1) * (ref - 1);
+    else ov += (2 * now - 1) * (2 * ref - 1);
+}
+
+template <int MODEL>
+__global__ void __launch_bounds__(256) k_persistence(Lat lat, long long *out)
+{
+    long long nc = 0, ov = 0;
+#pragma unroll
+    for (int c = 0; c < 2; ++c) {
+        const uint8_t *__restrict__ p = c ? lat.col[1] : lat.col[0];
+        long long nvec = lat.half >> 4;
+        const uint4 *__restrict__ pv = reinterpret_cast<const uint4 *>(p);
+        for (long long i = (long long)blockIdx.x * blockDim.x + threadIdx.x; i < nvec;
+             i += (long long)gridDim.x * blockDim.x) {
+            uint4 v = pv[i];
+            uint32_t w[4] = {v.x, v.y, v.z, v.w};
+#pragma unroll
+            for (int j = 0; j < 4; ++j)
+#pragma unroll
+                for (int b = 0; b < 4; ++b) persist_byte<MODEL>((w[j] >> (8 * b)) & 0xFFu, nc, ov);
+        }
+        for (long long i = (nvec << 4) + (long long)blockIdx.x * blockDim.x + threadIdx.x; i < lat.half;
+             i += (long long)gridDim.x * blockDim.x)
+            persist_byte<MODEL>(p[i], nc, ov);
+    }
+    block_accumulate2(nc, ov, out, true, true);
+}
+
+cudaError_t launch_persistence(const Lat &lat, int model, long long *d_out2, cudaStream_t s)
+{
+    cudaError_t e = cudaMemsetAsync(d_out2, 0, 2 * sizeof(long long), s);
+    if (e != cudaSuccess) return e;
+    int grid = grid_for((lat.half >> 4) + 1, 256, 8);
+    if (model == M_ISING_ONE) k_persistence<M_ISING_ONE><<<grid, 256, 0, s>>>(lat, d_out2);
+    else if (model == M_ISING_HALF) k_persistence<M_ISING_HALF><<<grid, 256, 0, s>>>(lat, d_out2);
+    else k_persistence<M_NE_HEATBATH><<<grid, 256, 0, s>>>(lat, d_out2);
+    return cudaGetLastError();
+}
+
+// Reference snapshot := current value, flags cleared (tracking_on) / all upper bits dropped (off).
+template <int MODEL>
+__global__ void __launch_bounds__(256) k_reset_reference(Lat lat, int tracking_on)
+{
+    constexpr uint32_t VAL = Enc<MODEL>::VAL;
+    constexpr int SH = Enc<MODEL>::REF_SHIFT;
+#pragma unroll
+    for (int c = 0; c < 2; ++c) {
+        uint8_t *p = c ? lat.col[1] : lat.col[0];
+        for (long long i = (long long)blockIdx.x * blockDim.x + threadIdx.x; i < lat.half;
+             i += (long long)gridDim.x * blockDim.x) {
+            uint32_t v = p[i] & VAL;
+            p[i] = (uint8_t)(tracking_on ? (v | (v << SH)) : v);
+        }
+    }
+}
+
+cudaError_t launch_reset_reference(const Lat &lat, int model, int tracking_on, cudaStream_t s)
+{
+    int grid = grid_for(lat.half, 256, 8);
+    if (model == M_ISING_ONE) k_reset_reference<M_ISING_ONE><<<grid, 256, 0, s>>>(lat, tracking_on);
+    else k_reset_reference<M_ISING_HALF><<<grid, 256, 0, s>>>(lat, tracking_on);
+    return cudaGetLastError();
+}
+
+// ------------------------------------------------------------------------------------------
+// Canonical int8 values <-> split internal layout.
+// ------------------------------------------------------------------------------------------
+__device__ __forceinline__ void canon_to_split(const Lat &lat, long long i, int &colour)
+{
+    long long ry = i / lat.L;
+    int x = (int)(i - ry * lat.L);
+    int z = (int)(ry / lat.L);
+    int y = (int)(ry - (long long)z * lat.L);
+    colour = (x + y + z) & 1;
+}
+
+__global__ void __launch_bounds__(256) k_get_spins(Lat lat, int model, int8_t *__restrict__ out)
+{
+    for (long long i = (long long)blockIdx.x * blockDim.x + threadIdx.x; i < 2 * lat.half;
+         i += (long long)gridDim.x * blockDim.x) {
+        int c;
+        canon_to_split(lat, i, c);
+        uint32_t b = (c ? lat.col[1] : lat.col[0])[i >> 1];
+        int v;
+        if (model == M_ISING_HALF) v = 2 * (int)(b & 1u) - 1;
+        else if (model == M_ISING_ONE) v = (int)(b & 3u) - 1;
+        else v = (int)(b & 1u);
+        out[i] = (int8_t)v;
+    }
+}
+
+__global__ void __launch_bounds__(256) k_set_spins(Lat lat, int model, const int8_t *__restrict__ in)
+{
+    for (long long i = (long long)blockIdx.x * blockDim.x + threadIdx.x; i < 2 * lat.half;
+         i += (long long)gridDim.x * blockDim.x) {
+        int c;
+        canon_to_split(lat, i, c);
+        int s = in[i];
+        uint32_t v, mask;
+        if (model == M_ISING_HALF) { v = s > 0 ? 1u : 0u; mask = 1u; }
+        else if (model == M_ISING_ONE) { v = (uint32_t)((s < -1 ? -1 : (s > 1 ? 1 : s)) + 1); mask = 3u; }
+        else { v = s != 0 ? 1u : 0u; mask = 1u; }
+        uint8_t *p = &(c ? lat.col[1] : lat.col[0])[i >> 1];
+        *p = (uint8_t)((*p & ~mask) | v);
+    }
+}
+
+cudaError_t launch_get_spins(const Lat &lat, int model, int8_t *d_out, cudaStream_t s)
+{
+    k_get_spins<<<grid_for(2 * lat.half, 256, 8), 256, 0, s>>>(lat, model, d_out);
+    return cudaGetLastError();
+}
+cudaError_t launch_set_spins(const Lat &lat, int model, const int8_t *d_in, cudaStream_t s)
+{
+    k_set_spins<<<grid_for(2 * lat.half, 256, 8), 256, 0, s>>>(lat, model, d_in);
+    return cudaGetLastError();
+}
+
+// ------------------------------------------------------------------------------------------
+// Test hooks: the device Philox on arbitrary (counter, key) pairs, and a register-only Philox
+// throughput loop (the integer roofline of step a4).
+// ------------------------------------------------------------------------------------------
+__global__ void k_philox_device(const uint32_t *__restrict__ ck, uint32_t *__restrict__ out, long long n)
+{
+    for (long long i = (long long)blockIdx.x * blockDim.x + threadIdx.x; i < n;
+         i += (long long)gridDim.x * blockDim.x) {
+        const uint32_t *p = ck + 6 * i;
+        uint4 r = philox4x32_10(p[0], p[1], p[2], p[3], p[4], p[5]);
+        out[4 * i + 0] = r.x; out[4 * i + 1] = r.y; out[4 * i + 2] = r.z; out[4 * i + 3] = r.w;
+    }
+}
+cudaError_t launch_philox_device(const uint32_t *d_ck, uint32_t *d_out, long long n, cudaStream_t s)
+{
+    if (n <= 0) return cudaSuccess;
+    k_philox_device<<<grid_for(n, 128, 8), 128, 0, s>>>(d_ck, d_out, n);
+    return cudaGetLastError();
+}
+
+__global__ void __launch_bounds__(256) k_philox_throughput(int calls, uint32_t *__restrict__ sink)
+{
+    uint32_t tid = blockIdx.x * blockDim.x + threadIdx.x;
+    uint32_t acc = 0;
+    // independent calls (counter = loop index), as in the sweep kernels: ILP across calls
+#pragma unroll 4
+    for (int i = 0; i < calls; ++i) {
+        uint4 r = philox4x32_10(tid, 0u, (uint32_t)i, 1u, 0x1234567u, 0x89abcdefu);
+        acc ^= r.x ^ r.y ^ r.z ^ r.w;
+    }
+    sink[tid] = acc;
+}
+cudaError_t launch_philox_throughput(int blocks, int calls, uint32_t *d_sink, cudaStream_t s)
+{
+    k_philox_throughput<<<blocks, 256, 0, s>>>(calls, d_sink);
+    return cudaGetLastError();
+}
+
+}  // namespace lsmk

@@ -1,0 +1,329 @@
+"""Thin Python binding of liblsm (include/lsm.h): argument marshalling only.
+
+Every step of the hot path runs in the CUDA kernels behind the C ABI; PyTorch is used for device
+memory (`torch.empty(..., device="cuda")`) and streams (`torch.cuda.current_stream()`), nothing else.
+There is no CPU fallback: if liblsm.so is missing or there is no CUDA device, calls raise.
+"""
+from __future__ import annotations
+
+import ctypes
+import os
+
+import numpy as np
+
+_PKG = os.path.dirname(os.path.abspath(__file__))
+_LIB_PATH = os.path.join(_PKG, "liblsm.so")
+
+ISING, NE_HEATBATH, NE_METROPOLIS = 0, 1, 2
+KERNEL_AUTO, KERNEL_GENERIC, KERNEL_TILED, KERNEL_RESIDENT = 0, 1, 2, 3
+OK, ERR_ARG, ERR_UNSUPPORTED, ERR_CUDA, ERR_WORKSPACE, ERR_STATE = 0, -1, -2, -3, -4, -5
+
+# name -> (restype, argtypes); every symbol include/lsm.h declares
+_vp, _i32, _i64, _u64, _dbl, _sz = (ctypes.c_void_p, ctypes.c_int, ctypes.c_int64, ctypes.c_uint64,
+                                    ctypes.c_double, ctypes.c_size_t)
+_P = ctypes.POINTER
+SIGNATURES = {
+    "lsm_workspace_bytes": (_i32, [_i32, _i32, _i32, _i32, _P(_sz)]),
+    "lsm_create": (_i32, [_i32, _i32, _i32, _i32, _dbl, _dbl, _dbl, _u64, _vp, _sz, _vp, _P(_vp)]),
+    "lsm_destroy": (_i32, [_vp]),
+    "lsm_sweep": (_i32, [_vp, _i64, _vp]),
+    "lsm_sweep_record": (_i32, [_vp, _i64, _vp, _vp]),
+    "lsm_sweep_record_host": (_i32, [_vp, _i64, _vp, _vp, _vp]),
+    "lsm_measure": (_i32, [_vp, _P(_dbl), _P(_i64)]),
+    "lsm_measure_int": (_i32, [_vp, _P(_i64), _P(_i64), _P(_u64)]),
+    "lsm_measure_full": (_i32, [_vp, _P(_i64), _P(_i64)]),
+    "lsm_persistence": (_i32, [_vp, _P(_i64), _P(_i64)]),
+    "lsm_reset_reference": (_i32, [_vp, _vp]),
+    "lsm_set_tracking": (_i32, [_vp, _i32, _vp]),
+    "lsm_get_spins": (_i32, [_vp, _vp, _vp]),
+    "lsm_get_spins_host": (_i32, [_vp, _vp, _vp, _vp]),
+    "lsm_set_spins": (_i32, [_vp, _vp, _u64, _vp]),
+    "lsm_set_spins_host": (_i32, [_vp, _vp, _vp, _u64, _vp]),
+    "lsm_set_temperature": (_i32, [_vp, _dbl]),
+    "lsm_get_thresholds": (_i32, [_vp, _P(_u64), _P(_i32)]),
+    "lsm_set_kernel": (_i32, [_vp, _i32]),
+    "lsm_get_kernel": (_i32, [_vp, _P(_i32)]),
+    "lsm_get_launch_count": (_i32, [_vp, _P(_u64)]),
+    "lsm_binder_u4": (_i32, [_vp, _i64, _P(_dbl)]),
+    "lsm_heat_capacity": (_i32, [_vp, _i64, _i64, _dbl, _dbl, _dbl, _P(_dbl)]),
+    "lsm_phi": (_i32, [_i64, _i64, _dbl, _P(_dbl)]),
+    "lsm_persistence_fraction": (_i32, [_i64, _i64, _P(_dbl)]),
+    "lsm_energy": (_i32, [_i32, _dbl, _dbl, _i64, _i64, _P(_dbl)]),
+    "lsm_philox_device": (_i32, [_vp, _vp, _i64, _vp]),
+    "lsm_philox_throughput": (_i32, [_i32, _i32, _vp, _vp]),
+    "lsm_strerror": (ctypes.c_char_p, [_i32]),
+    "lsm_last_cuda_error": (ctypes.c_char_p, []),
+}
+
+_lib = None
+
+
+def lib_path() -> str:
+    return _LIB_PATH
+
+
+def load():
+    """dlopen liblsm.so and bind every declared symbol.  Raises if the library is missing:
+    the product path never falls back to anything else."""
+    global _lib
+    if _lib is None:
+        if not os.path.exists(_LIB_PATH):
+            raise RuntimeError(
+                f"{_LIB_PATH} not found: build it with `python -m paper_1209_0296_b200.build` "
+                "(there is no CPU fallback)")
+        L = ctypes.CDLL(_LIB_PATH)
+        for name, (res, args) in SIGNATURES.items():
+            fn = getattr(L, name)
+            fn.restype = res
+            fn.argtypes = args
+        _lib = L
+    return _lib
+
+
+class LsmError(RuntimeError):
+    def __init__(self, code, where):
+        L = load()
+        msg = L.lsm_strerror(code).decode()
+        if code == ERR_CUDA:
+            msg += " -- " + L.lsm_last_cuda_error().decode()
+        super().__init__(f"{where}: {msg} ({code})")
+        self.code = code
+
+
+def _check(code, where):
+    if code != OK:
+        raise LsmError(code, where)
+
+
+def _stream_ptr(stream):
+    import torch
+
+    s = torch.cuda.current_stream() if stream is None else stream
+    return ctypes.c_void_p(s.cuda_stream)
+
+
+def workspace_bytes(dims, L, two_S=1, model=ISING) -> int:
+    n = _sz()
+    _check(load().lsm_workspace_bytes(dims, L, two_S, model, ctypes.byref(n)), "lsm_workspace_bytes")
+    return int(n.value)
+
+
+class Lattice:
+    """One lattice = one lsm_t handle plus the torch-owned device workspace behind it."""
+
+    def __init__(self, dims, L, two_S=1, model=ISING, J=1.0, h=0.0, T=1.0, seed=0, device="cuda:0", stream=None):
+        import torch
+
+        if not torch.cuda.is_available():
+            raise RuntimeError("liblsm needs a CUDA device (there is no CPU fallback)")
+        self._lib = load()
+        self.dims, self.L, self.two_S, self.model = int(dims), int(L), int(two_S), int(model)
+        self.J, self.h, self.T, self.seed = float(J), float(h), float(T), int(seed)
+        self.device = torch.device(device)
+        self.N = self.L ** self.dims
+        nbytes = workspace_bytes(dims, L, two_S, model)
+        with torch.cuda.device(self.device):
+            self._ws = torch.empty(nbytes + 256, dtype=torch.uint8, device=self.device)
+            off = (-self._ws.data_ptr()) % 256
+            self._ws_ptr = self._ws.data_ptr() + off
+            h_ = _vp()
+            _check(self._lib.lsm_create(self.dims, self.L, self.two_S, self.model, self.J, self.h, self.T,
+                                        self.seed, _vp(self._ws_ptr), nbytes, _stream_ptr(stream),
+                                        ctypes.byref(h_)), "lsm_create")
+        self._h = h_
+        self._scratch = None
+
+    # ------------------------------------------------------------------ life cycle
+    def close(self):
+        if getattr(self, "_h", None):
+            self._lib.lsm_destroy(self._h)
+            self._h = None
+            self._ws = None
+            self._scratch = None
+
+    def __del__(self):
+        try:
+            self.close()
+        except Exception:
+            pass
+
+    def _dev_scratch(self, nbytes):
+        import torch
+
+        if self._scratch is None or self._scratch.numel() < nbytes:
+            self._scratch = torch.empty(nbytes, dtype=torch.uint8, device=self.device)
+        return self._scratch
+
+    # ------------------------------------------------------------------ sweeps
+    def sweep(self, n=1, stream=None):
+        _check(self._lib.lsm_sweep(self._h, int(n), _stream_ptr(stream)), "lsm_sweep")
+
+    def sweep_record(self, n, out=None, stream=None):
+        """n sweeps; returns a device int64 tensor [n, 2] = (B, M) after each sweep (asynchronous)."""
+        import torch
+
+        if out is None:
+            out = torch.empty((int(n), 2), dtype=torch.int64, device=self.device)
+        assert out.is_cuda and out.dtype == torch.int64 and out.is_contiguous() and out.numel() >= 2 * int(n)
+        _check(self._lib.lsm_sweep_record(self._h, int(n), _vp(out.data_ptr()), _stream_ptr(stream)),
+               "lsm_sweep_record")
+        return out
+
+    def sweep_record_host(self, n, h_obs=None, stream=None):
+        """n sweeps with the (B, M) series delivered into a HOST array (pinned torch tensor or numpy)."""
+        import torch
+
+        if h_obs is None:
+            h_obs = torch.empty((int(n), 2), dtype=torch.int64).pin_memory()
+        ptr = h_obs.data_ptr() if hasattr(h_obs, "data_ptr") else h_obs.ctypes.data
+        sc = self._dev_scratch(16 * max(int(n), 1))
+        _check(self._lib.lsm_sweep_record_host(self._h, int(n), _vp(ptr), _vp(sc.data_ptr()), _stream_ptr(stream)),
+               "lsm_sweep_record_host")
+        return h_obs
+
+    # ------------------------------------------------------------------ observables
+    def measure(self):
+        E, M = _dbl(), _i64()
+        _check(self._lib.lsm_measure(self._h, ctypes.byref(E), ctypes.byref(M)), "lsm_measure")
+        return float(E.value), int(M.value)
+
+    def measure_int(self):
+        B, M, t = _i64(), _i64(), _u64()
+        _check(self._lib.lsm_measure_int(self._h, ctypes.byref(B), ctypes.byref(M), ctypes.byref(t)),
+               "lsm_measure_int")
+        return int(B.value), int(M.value), int(t.value)
+
+    def measure_full(self):
+        B, M = _i64(), _i64()
+        _check(self._lib.lsm_measure_full(self._h, ctypes.byref(B), ctypes.byref(M)), "lsm_measure_full")
+        return int(B.value), int(M.value)
+
+    def persistence(self):
+        a, b = _i64(), _i64()
+        _check(self._lib.lsm_persistence(self._h, ctypes.byref(a), ctypes.byref(b)), "lsm_persistence")
+        return int(a.value), int(b.value)
+
+    def reset_reference(self, stream=None):
+        _check(self._lib.lsm_reset_reference(self._h, _stream_ptr(stream)), "lsm_reset_reference")
+
+    def set_tracking(self, on, stream=None):
+        _check(self._lib.lsm_set_tracking(self._h, 1 if on else 0, _stream_ptr(stream)), "lsm_set_tracking")
+
+    # ------------------------------------------------------------------ configuration I/O
+    def get_spins(self, out=None, stream=None):
+        import torch
+
+        if out is None:
+            out = torch.empty(self.N, dtype=torch.int8, device=self.device)
+        assert out.is_cuda and out.dtype == torch.int8 and out.numel() == self.N and out.is_contiguous()
+        _check(self._lib.lsm_get_spins(self._h, _vp(out.data_ptr()), _stream_ptr(stream)), "lsm_get_spins")
+        return out
+
+    def get_spins_host(self, h_out=None, stream=None):
+        if h_out is None:
+            h_out = np.empty(self.N, dtype=np.int8)
+        ptr = h_out.data_ptr() if hasattr(h_out, "data_ptr") else h_out.ctypes.data
+        sc = self._dev_scratch(self.N)
+        _check(self._lib.lsm_get_spins_host(self._h, _vp(ptr), _vp(sc.data_ptr()), _stream_ptr(stream)),
+               "lsm_get_spins_host")
+        return h_out
+
+    def set_spins(self, d_in, sweep_counter, stream=None):
+        import torch
+
+        assert d_in.is_cuda and d_in.dtype == torch.int8 and d_in.numel() == self.N and d_in.is_contiguous()
+        _check(self._lib.lsm_set_spins(self._h, _vp(d_in.data_ptr()), int(sweep_counter), _stream_ptr(stream)),
+               "lsm_set_spins")
+
+    def set_spins_host(self, h_in, sweep_counter, stream=None):
+        if hasattr(h_in, "data_ptr"):
+            ptr, n = h_in.data_ptr(), h_in.numel()
+        else:
+            h_in = np.ascontiguousarray(h_in, dtype=np.int8)
+            ptr, n = h_in.ctypes.data, h_in.size
+        assert n == self.N
+        sc = self._dev_scratch(self.N)
+        _check(self._lib.lsm_set_spins_host(self._h, _vp(ptr), _vp(sc.data_ptr()), int(sweep_counter),
+                                            _stream_ptr(stream)), "lsm_set_spins_host")
+
+    def set_temperature(self, T):
+        _check(self._lib.lsm_set_temperature(self._h, float(T)), "lsm_set_temperature")
+        self.T = float(T)
+
+    def thresholds(self):
+        buf = (_u64 * 128)()
+        n = _i32()
+        _check(self._lib.lsm_get_thresholds(self._h, buf, ctypes.byref(n)), "lsm_get_thresholds")
+        return [int(buf[i]) for i in range(n.value)]
+
+    # ------------------------------------------------------------------ kernel family / counters
+    def set_kernel(self, family):
+        _check(self._lib.lsm_set_kernel(self._h, int(family)), "lsm_set_kernel")
+
+    @property
+    def kernel(self):
+        k = _i32()
+        _check(self._lib.lsm_get_kernel(self._h, ctypes.byref(k)), "lsm_get_kernel")
+        return int(k.value)
+
+    @property
+    def launch_count(self):
+        n = _u64()
+        _check(self._lib.lsm_get_launch_count(self._h, ctypes.byref(n)), "lsm_get_launch_count")
+        return int(n.value)
+
+
+# ---------------------------------------------------------------------- derived doubles (host math in the library)
+def binder_u4(obs) -> float:
+    a = np.ascontiguousarray(obs, dtype=np.int64).reshape(-1, 2)
+    out = _dbl()
+    _check(load().lsm_binder_u4(_vp(a.ctypes.data), a.shape[0], ctypes.byref(out)), "lsm_binder_u4")
+    return float(out.value)
+
+
+def heat_capacity(obs, N, J, h, T) -> float:
+    a = np.ascontiguousarray(obs, dtype=np.int64).reshape(-1, 2)
+    out = _dbl()
+    _check(load().lsm_heat_capacity(_vp(a.ctypes.data), a.shape[0], int(N), float(J), float(h), float(T),
+                                    ctypes.byref(out)), "lsm_heat_capacity")
+    return float(out.value)
+
+
+def phi(overlap, N, c) -> float:
+    out = _dbl()
+    _check(load().lsm_phi(int(overlap), int(N), float(c), ctypes.byref(out)), "lsm_phi")
+    return float(out.value)
+
+
+def persistence_fraction(never_changed, N) -> float:
+    out = _dbl()
+    _check(load().lsm_persistence_fraction(int(never_changed), int(N), ctypes.byref(out)), "lsm_persistence_fraction")
+    return float(out.value)
+
+
+def energy(model, J, h, B, M) -> float:
+    out = _dbl()
+    _check(load().lsm_energy(int(model), float(J), float(h), int(B), int(M), ctypes.byref(out)), "lsm_energy")
+    return float(out.value)
+
+
+# ---------------------------------------------------------------------- test hooks
+def philox_device(ctr_key):
+    """ctr_key: int array [n, 6] (c0..c3, k0, k1) -> uint32 array [n, 4] computed by the device Philox."""
+    import torch
+
+    a = torch.as_tensor(np.ascontiguousarray(ctr_key, dtype=np.uint32).view(np.int32)).cuda()
+    out = torch.empty((a.shape[0], 4), dtype=torch.int32, device=a.device)
+    _check(load().lsm_philox_device(_vp(a.data_ptr()), _vp(out.data_ptr()), a.shape[0], _stream_ptr(None)),
+           "lsm_philox_device")
+    return out.cpu().numpy().view(np.uint32)
+
+
+def philox_throughput(blocks, calls, stream=None):
+    """Enqueue the register-only Philox loop; returns the sink tensor (keeps it alive)."""
+    import torch
+
+    sink = torch.empty(blocks * 256, dtype=torch.int32, device="cuda")
+    _check(load().lsm_philox_throughput(int(blocks), int(calls), _vp(sink.data_ptr()), _stream_ptr(stream)),
+           "lsm_philox_throughput")
+    return sink

@@ -1,0 +1,69 @@
+"""Seeded synthetic workloads shaped like the paper's (shared by tests/ and bench.py).
+
+This module holds configuration data only -- lattice shapes, couplings, temperatures, seeds and run
+lengths of BASELINE.json's five configs -- and none of the method's arithmetic.
+The lattices themselves are drawn on the device (and, independently, by the oracle) from the seed.
+"""
+from __future__ import annotations
+
+import math
+from dataclasses import dataclass, replace
+
+ISING, NE_HEATBATH, NE_METROPOLIS = 0, 1, 2
+
+
+def seed_of(cfg: int, variant: int = 0) -> int:
+    """seed = 12090296 * 2^32 + cfg * 256 + variant (variant = temperature / concentration index)."""
+    return (12090296 << 32) + cfg * 256 + variant
+
+
+def ne_temperature(c: float) -> float:
+    """T with c = 1/(1+exp(1/T)) (reading D6): what the harness passes for a target concentration."""
+    return 1.0 / math.log((1.0 - c) / c)
+
+
+@dataclass(frozen=True)
+class Workload:
+    name: str
+    cfg: int
+    dims: int
+    L: int
+    two_S: int = 1
+    model: int = ISING
+    J: float = 1.0
+    h: float = 0.0
+    T: float = 1.0
+    seed: int = 0
+    sweeps: int = 1
+    note: str = ""
+
+    @property
+    def N(self) -> int:
+        return self.L ** self.dims
+
+    def create_args(self):
+        return dict(dims=self.dims, L=self.L, two_S=self.two_S, model=self.model, J=self.J, h=self.h,
+                    T=self.T, seed=self.seed)
+
+    def scaled(self, L: int, sweeps: int | None = None) -> "Workload":
+        """Same physics on a smaller lattice (the reduced shapes of the parity tests)."""
+        return replace(self, L=L, sweeps=self.sweeps if sweeps is None else sweeps,
+                       name=f"{self.name}@L{L}")
+
+
+def configs() -> dict[str, Workload]:
+    out = {}
+    out["cfg1"] = Workload("cfg1", 1, 2, 64, T=2.269, seed=seed_of(1), sweeps=1000,
+                           note="2D Ising spin-1/2 64^2 near Tc, (E, M) after every sweep")
+    for v, T in enumerate((2.0, 2.269, 2.6)):
+        out[f"cfg2_T{T}"] = Workload(f"cfg2_T{T}", 2, 2, 8192, T=T, seed=seed_of(2, v), sweeps=10_000,
+                                     note="2D Ising spin-1/2 8192^2, per-sweep E, M, U4 over the last 5000 sweeps")
+    out["cfg3"] = Workload("cfg3", 3, 3, 512, T=4.5115, seed=seed_of(3), sweeps=2000,
+                           note="3D Ising spin-1/2 512^3 near the 3D Tc")
+    out["cfg4"] = Workload("cfg4", 4, 3, 256, two_S=2, h=0.01, T=3.0, seed=seed_of(4), sweeps=2000,
+                           note="3D spin-1 Ising 256^3")
+    for v, c in enumerate((0.10, 0.20, 0.30)):
+        out[f"cfg5_c{c:.2f}"] = Workload(f"cfg5_c{c:.2f}", 5, 2, 8192, model=NE_HEATBATH, J=0.0,
+                                         T=ne_temperature(c), seed=seed_of(5, v), sweeps=100_000,
+                                         note="2D North-East heat-bath 8192^2, persistence every 100 sweeps")
+    return out

@@ -1,0 +1,292 @@
+"""GPU parity: the CUDA path (through the C ABI) against the CPU oracle, element by element.
+
+Integer results (configuration, bond sum B, magnetisation M, never-changed count, overlap) must be
+bit-exact after every sweep; derived doubles within 1e-9 relative (BASELINE.json north_star)."""
+import ctypes
+import math
+
+import numpy as np
+import pytest
+
+from oracle import lsm_oracle as O
+from paper_1209_0296_b200 import build as B
+from paper_1209_0296_b200 import lsm
+from paper_1209_0296_b200 import workloads as W
+
+pytestmark = pytest.mark.gpu
+
+
+@pytest.fixture(scope="module", autouse=True)
+def _built():
+    B.build()
+    lsm.load()
+
+
+def make_pair(family=lsm.KERNEL_AUTO, **kw):
+    lat = lsm.Lattice(**kw)
+    if family != lsm.KERNEL_AUTO:
+        lat.set_kernel(family)
+    return lat, O.Oracle(**kw)
+
+
+def assert_same_state(lat, orc, check_persistence=True):
+    g = lat.get_spins().cpu().numpy()
+    o = orc.get_spins()
+    bad = np.flatnonzero(g != o)
+    assert bad.size == 0, f"{bad.size} sites differ, first at {bad[:5]}"
+    Bg, Mg, tg = lat.measure_int()
+    assert (Bg, Mg) == orc.measure_int()
+    assert tg == orc.sweeps_done
+    assert lat.measure_full() == (Bg, Mg)      # P14: fused running sums == full reduction
+    if check_persistence:
+        assert lat.persistence() == orc.persistence()
+
+
+SHAPES = [
+    # (kwargs, sweeps) -- sizes span several tiles and ragged tails; L not a multiple of 32 included
+    (dict(dims=2, L=4, T=2.269), 40),
+    (dict(dims=2, L=6, T=2.0), 40),
+    (dict(dims=2, L=34, T=2.269), 30),
+    (dict(dims=2, L=64, T=2.269), 60),
+    (dict(dims=2, L=96, T=2.6, h=0.05), 30),
+    (dict(dims=2, L=160, T=1.5, J=0.7, h=-0.3), 25),
+    (dict(dims=2, L=256, T=2.269), 25),
+    (dict(dims=2, L=64, T=0.05), 20),               # thresholds 0 ("never") and 2^32 ("always")
+    (dict(dims=2, L=64, T=1e6), 10),                # p ~ 1 - 1e-5: thresholds just below 2^32
+    (dict(dims=2, L=32, T=2.0, J=0.0, h=0.4), 20),  # free spins
+    (dict(dims=2, L=32, T=2.0, J=-1.0), 20),        # antiferromagnet
+    (dict(dims=3, L=4, T=4.5115), 30),
+    (dict(dims=3, L=6, T=4.0, h=0.1), 20),
+    (dict(dims=3, L=32, T=4.5115), 20),
+    (dict(dims=3, L=64, T=4.5115), 8),
+    (dict(dims=3, L=34, T=3.0), 8),
+    (dict(dims=2, L=4, two_S=2, T=3.0, h=0.01), 40),
+    (dict(dims=2, L=64, two_S=2, T=1.5, h=0.01), 30),
+    (dict(dims=3, L=6, two_S=2, T=3.0, h=0.01), 20),
+    (dict(dims=3, L=32, two_S=2, T=3.0, h=0.01), 12),
+    (dict(dims=3, L=64, two_S=2, T=3.0, h=0.01), 6),
+    (dict(dims=2, L=4, model=lsm.NE_HEATBATH, J=0.0, T=W.ne_temperature(0.3)), 40),
+    (dict(dims=2, L=34, model=lsm.NE_HEATBATH, J=0.0, T=W.ne_temperature(0.2)), 40),
+    (dict(dims=2, L=64, model=lsm.NE_HEATBATH, J=0.0, T=W.ne_temperature(0.1)), 60),
+    (dict(dims=2, L=256, model=lsm.NE_HEATBATH, J=0.0, T=W.ne_temperature(0.3)), 40),
+    (dict(dims=2, L=64, model=lsm.NE_METROPOLIS, J=0.0, T=W.ne_temperature(0.3)), 60),
+    (dict(dims=2, L=160, model=lsm.NE_METROPOLIS, J=0.0, T=W.ne_temperature(0.2)), 30),
+]
+FAMILIES = [lsm.KERNEL_GENERIC, lsm.KERNEL_TILED]
+
+
+def test_device_philox_known_answers_and_random():
+    rows = []
+    want = []
+    for line in open(__file__.replace("test_gpu_parity.py", "golden/philox4x32_10_kat.txt")):
+        if line.startswith("#") or not line.strip():
+            continue
+        v = [int(t, 16) for t in line.split()]
+        rows.append(v[:6])
+        want.append(v[6:])
+    rng = np.random.default_rng(3)
+    extra = rng.integers(0, 2 ** 32, size=(500, 6), dtype=np.uint64)
+    rows += extra.tolist()
+    want += [list(O.philox4x32_10(r[:4], r[4:])) for r in extra.tolist()]
+    got = lsm.philox_device(np.array(rows, dtype=np.uint64).astype(np.uint32))
+    assert np.array_equal(got, np.array(want, dtype=np.uint64).astype(np.uint32))
+
+
+@pytest.mark.parametrize("kw", [
+    dict(dims=2, L=8, T=2.269), dict(dims=2, L=8, T=2.0, J=0.5, h=0.25), dict(dims=3, L=8, T=4.5115),
+    dict(dims=3, L=8, T=0.3, h=-0.2), dict(dims=2, L=8, two_S=2, T=3.0, h=0.01),
+    dict(dims=3, L=8, two_S=2, T=3.0, h=0.01), dict(dims=3, L=8, two_S=2, T=0.4, J=2.0, h=0.0),
+    dict(dims=2, L=8, model=lsm.NE_HEATBATH, J=0.0, T=W.ne_temperature(0.1)),
+    dict(dims=2, L=8, model=lsm.NE_METROPOLIS, J=0.0, T=W.ne_temperature(0.3)),
+])
+def test_threshold_tables_identical(kw):
+    lat, orc = make_pair(seed=1, **kw)
+    assert lat.thresholds() == orc.thresholds()
+    for T in (0.02, 1.0, 2.269, 37.5):
+        lat.set_temperature(T)
+        orc.set_temperature(T)
+        assert lat.thresholds() == orc.thresholds()
+
+
+@pytest.mark.parametrize("family", FAMILIES)
+@pytest.mark.parametrize("kw,nsweeps", SHAPES)
+def test_sweep_parity(kw, nsweeps, family):
+    """Initial state, every per-sweep (B, M), final configuration, persistence and overlap."""
+    try:
+        lat, orc = make_pair(family, seed=W.seed_of(9, nsweeps), **kw)
+    except lsm.LsmError as e:
+        if e.code == lsm.ERR_UNSUPPORTED and family == lsm.KERNEL_TILED:
+            pytest.skip("tiled family does not cover this lattice (generic covers it)")
+        raise
+    assert lat.kernel == family
+    assert_same_state(lat, orc)                      # a1: initial state from the seed
+    half = nsweeps // 2
+    got = lat.sweep_record(half).cpu().numpy()
+    want = orc.sweep_record(half)
+    assert np.array_equal(got, want), np.flatnonzero((got != want).any(axis=1))[:5]
+    assert_same_state(lat, orc)
+    lat.sweep(nsweeps - half)                        # no per-sweep record: observables of the last sweep only
+    orc.sweep(nsweeps - half)
+    assert_same_state(lat, orc)
+    E, M = lat.measure()
+    assert E == orc.energy() and M == orc.measure_int()[1]
+
+
+@pytest.mark.parametrize("family", FAMILIES)
+def test_cfg1_full_length(family):
+    """BASELINE.json config 1 at full length: 64x64, T=2.269, 1000 sweeps, (E, M) after every sweep."""
+    w = W.configs()["cfg1"]
+    lat, orc = make_pair(family, **w.create_args())
+    got = lat.sweep_record(w.sweeps).cpu().numpy()
+    want = orc.sweep_record(w.sweeps)
+    assert np.array_equal(got, want)
+    assert_same_state(lat, orc)
+    # derived doubles within 1e-9 relative
+    u_g, u_o = lsm.binder_u4(got[500:]), O.binder_u4(want[500:, 1])
+    assert abs(u_g - u_o) <= 1e-9 * abs(u_o)
+    c_g, c_o = lsm.heat_capacity(got[500:], w.N, w.J, w.h, w.T), O.heat_capacity_per_site(want[500:], w.N, w.J, w.h, w.T)
+    assert abs(c_g - c_o) <= 1e-9 * abs(c_o)
+
+
+@pytest.mark.parametrize("name,L,nsweeps", [
+    ("cfg2_T2.0", 256, 300), ("cfg2_T2.269", 256, 1000), ("cfg2_T2.6", 512, 100),
+    ("cfg3", 64, 150), ("cfg4", 64, 60), ("cfg5_c0.10", 256, 1000), ("cfg5_c0.30", 256, 400),
+])
+def test_reduced_shapes_of_configs_2_to_5(name, L, nsweeps):
+    """Same physics and seeds as BASELINE.json configs 2-5 on lattices the oracle finishes in seconds."""
+    w = W.configs()[name].scaled(L, nsweeps)
+    lat, orc = make_pair(**w.create_args())
+    is_ne = w.model != lsm.ISING
+    chunk = 100 if is_ne else nsweeps
+    done = 0
+    while done < nsweeps:
+        n = min(chunk, nsweeps - done)
+        got = lat.sweep_record(n).cpu().numpy()
+        want = orc.sweep_record(n)
+        assert np.array_equal(got, want)
+        done += n
+        if is_ne:   # cfg5: persistence (and Phi) every 100 sweeps
+            nc_g, ov_g = lat.persistence()
+            nc_o, ov_o = orc.persistence()
+            assert (nc_g, ov_g) == (nc_o, ov_o)
+            c = orc.concentration
+            assert lsm.persistence_fraction(nc_g, w.N) == O.persistence_fraction(nc_o, w.N)
+            a, b = lsm.phi(ov_g, w.N, c), O.phi(ov_o, w.N, c)
+            assert abs(a - b) <= 1e-9 * max(abs(b), 1e-300)
+    assert_same_state(lat, orc)
+
+
+def test_checkpoint_resume_and_host_buffers():
+    kw = dict(dims=2, L=64, T=2.269, seed=5)
+    lat, orc = make_pair(**kw)
+    lat.sweep(7)
+    orc.sweep(7)
+    snap = lat.get_spins_host()
+    assert np.array_equal(snap, orc.get_spins())
+    lat2 = lsm.Lattice(**kw)
+    lat2.set_spins_host(snap, 7)
+    assert lat2.measure_int() == lat.measure_int()
+    h1 = lat.sweep_record_host(9)
+    h2 = lat2.sweep_record_host(9)
+    want = orc.sweep_record(9)
+    assert np.array_equal(np.asarray(h1), want) and np.array_equal(np.asarray(h2), want)
+    assert_same_state(lat, orc, check_persistence=True)
+    # set_spins leaves the reference snapshot and flags alone: lat2 was re-referenced at create (t=0 draw)
+    import torch
+
+    up = torch.ones(64 * 64, dtype=torch.int8, device="cuda")
+    lat.set_spins(up, 100)
+    orc.set_spins(np.ones(64 * 64, dtype=np.int8), 100)
+    assert lat.measure_int() == (2 * 4096, 4096, 100)
+    lat.reset_reference()
+    orc.reset_reference()
+    lat.sweep(5)
+    orc.sweep(5)
+    assert_same_state(lat, orc)
+
+
+def test_tracking_off_and_on():
+    kw = dict(dims=2, L=64, T=2.269, seed=6)
+    lat, orc = make_pair(**kw)
+    lat.set_tracking(False)
+    with pytest.raises(lsm.LsmError) as ei:
+        lat.persistence()
+    assert ei.value.code == lsm.ERR_STATE
+    lat.sweep(6)
+    orc.sweep(6)
+    assert_same_state(lat, orc, check_persistence=False)
+    lat.reset_reference()
+    orc.reset_reference()
+    lat.sweep(6)
+    orc.sweep(6)
+    assert_same_state(lat, orc)
+
+
+def test_zero_sweeps_and_temperature_change():
+    kw = dict(dims=3, L=8, T=4.5115, seed=8)
+    lat, orc = make_pair(**kw)
+    lat.sweep(0)
+    assert lat.sweep_record(0).shape == (0, 2)
+    assert_same_state(lat, orc)
+    for T in (1.0, 6.0, 0.1):
+        lat.set_temperature(T)
+        orc.set_temperature(T)
+        got = lat.sweep_record(5).cpu().numpy()
+        assert np.array_equal(got, orc.sweep_record(5))
+    assert_same_state(lat, orc)
+    assert lat.launch_count > 0
+
+
+def test_sweep_counter_above_32_bits():
+    """The 64-bit sweep counter reaches the Philox counter's c3 field (reading D2)."""
+    kw = dict(dims=2, L=32, T=2.269, seed=11)
+    lat, orc = make_pair(**kw)
+    t0 = (5 << 32) + 0xFFFFFFFE
+    s = orc.get_spins()
+    lat.set_spins_host(s, t0)
+    orc.set_spins(s, t0)
+    got = lat.sweep_record(4).cpu().numpy()
+    assert np.array_equal(got, orc.sweep_record(4))
+    assert_same_state(lat, orc, check_persistence=False)
+
+
+FULL = [
+    # (config, sweeps checked from t=0, late time for the one-step spot check)
+    ("cfg2_T2.269", 2, 37),
+    ("cfg3", 1, 21),
+    ("cfg4", 2, 15),
+    ("cfg5_c0.20", 2, 203),
+]
+
+
+@pytest.mark.parametrize("name,k_first,t_late", FULL)
+def test_full_size_prefix_and_late_spot_check(name, k_first, t_late):
+    """BASELINE.json's full sizes in the launch configuration bench.py times (AUTO kernel family,
+    tracking as bench.py sets it): the first sweeps element by element, then a one-step spot check at
+    a late time -- download the GPU state at sweep t, hand it to the oracle with the same counter,
+    one oracle sweep, compare with the GPU at t+1.  Valid because the random words are a pure
+    function of (seed, sweep, half, site)."""
+    w = W.configs()[name]
+    lat, orc = make_pair(**w.create_args())
+    if w.model == lsm.ISING:
+        lat.set_tracking(False)      # as bench.py runs cfg1-4
+    g0 = lat.get_spins_host()
+    assert np.array_equal(g0, orc.get_spins())
+    got = lat.sweep_record(k_first).cpu().numpy()
+    want = orc.sweep_record(k_first)
+    assert np.array_equal(got, want)
+    assert np.array_equal(lat.get_spins_host(), orc.get_spins())
+    lat.sweep(t_late - k_first)
+    state = lat.get_spins_host()
+    orc.set_spins(state, t_late)
+    series = lat.sweep_record(1).cpu().numpy()
+    orc.sweep(1)
+    after = lat.get_spins_host()
+    ref = orc.get_spins()
+    assert np.array_equal(after, ref)
+    assert tuple(series[0]) == orc.measure_int()
+    # properties that hold at any size
+    N = w.N
+    Bv, Mv, t = lat.measure_int()
+    assert t == t_late + 1 and abs(Mv) <= N and abs(Bv) <= w.dims * N
+    assert lat.measure_full() == (Bv, Mv)
