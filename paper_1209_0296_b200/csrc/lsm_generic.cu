@@ -79,7 +79,7 @@ __device__ __forceinline__ int neighbour_value_sum(const Lat &lat, const uint8_t
 // a2-a6, scalar form.
 // ------------------------------------------------------------------------------------------
 template <int MODEL>
-__global__ void __launch_bounds__(256) k_sweep_generic(SweepArgs a, Thr64 thr)
+__global__ void __launch_bounds__(256) k_sweep_generic(const __grid_constant__ SweepArgs a, const __grid_constant__ Thr64 thr)
 {
     constexpr uint32_t VAL = Enc<MODEL>::VAL, CHG = Enc<MODEL>::CHG;
     __shared__ unsigned long long s_thr[96];

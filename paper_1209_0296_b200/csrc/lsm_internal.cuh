@@ -114,6 +114,27 @@ __device__ __forceinline__ void block_accumulate2(long long a, long long b, long
     __syncthreads();
 }
 
+// Same, with the caller's shared scratch (blockDim.x <= 256).
+__device__ __forceinline__ void block_accumulate2_in(long long (*red)[8], long long a, long long b, long long *out,
+                                                     bool do_a, bool do_b)
+{
+    a = warp_sum(a);
+    b = warp_sum(b);
+    int lane = threadIdx.x & 31, w = threadIdx.x >> 5, nw = (blockDim.x + 31) >> 5;
+    if (lane == 0) { red[0][w] = a; red[1][w] = b; }
+    __syncthreads();
+    if (w == 0) {
+        a = lane < nw ? red[0][lane & 7] : 0;
+        b = lane < nw ? red[1][lane & 7] : 0;
+        a = warp_sum(a);
+        b = warp_sum(b);
+        if (lane == 0) {
+            if (do_a && a != 0) atomicAdd((unsigned long long *)&out[0], (unsigned long long)a);
+            if (do_b && b != 0) atomicAdd((unsigned long long *)&out[1], (unsigned long long)b);
+        }
+    }
+}
+
 // ------------------------------------------------------------------------------------------
 // Launchers implemented in the .cu files (host side, enqueue only; return cudaError_t).
 // ------------------------------------------------------------------------------------------
