@@ -11,12 +11,17 @@
 // Per 32-bit lane of the word (4 sites) the thread makes exactly one Philox4x32-10 call (reading D2:
 // group = byte offset >> 2), sums the neighbour bytes with plain 32-bit adds (no carries: a byte
 // never exceeds 2d), looks the four thresholds up in shared memory and folds the four compare
-// results into the lane with predicated ORs.  Nothing branches on lattice data.
+// results into the lane with predicated adds.  Nothing branches on lattice data.
 //
-// The binding unit is the integer multiplier: each Philox call costs 20 IMAD.WIDE.U32 (18 after
-// hoisting the two warp-uniform products of rounds 1-2, see PhiloxSweepConsts).
+// What binds (measured): on B200 an IMAD.WIDE occupies the FMA-heavy pipe for 4 cycles
+// AND one issue slot of the 16-lane ALU pipe, so a warp needs 2*(ALU instructions + wide multiplies)
+// cycles per step.  The rule code is therefore written to spend as few ALU-pipe instructions as it
+// can: table indexed by (spin, up-neighbour count) so no "aligned count" is formed, "w <= thr-1"
+// compares so certain acceptance needs no mask, compare results merged with predicated IMAD adds
+// (FMA pipe), row parity known at compile time so the side neighbour costs one funnel shift.
 #include "lsm_tiled.cuh"
 
+#include <cstdlib>
 #include <cstring>
 
 namespace lsmk {
@@ -26,7 +31,8 @@ namespace lsmk {
 // (c0 = group, c1 = 0, c2 = sweep, c3 = stream tag): c1, c2, c3 and the key are the same for every
 // site, so in round 1 the product M1*c2 and in round 2 the product M0*c0' do not depend on the
 // site.  The host evaluates them once per launch; the function below is bit-identical to the plain
-// ten rounds (test: lsm_philox_device on the same counters, and every parity test).
+// ten rounds (every parity test exercises it against the oracle's plain Philox).
+// 18 IMAD.WIDE.U32 + 19 LOP3 per call.
 // ------------------------------------------------------------------------------------------
 struct PhiloxSweepConsts {
     uint32_t x1;        // c3 ^ k1                      (round 1: n2 = hi(M0*c0) ^ x1)
@@ -101,13 +107,11 @@ struct TiledGeom {
     int ncol;              // R * wpr word columns
     int S;                 // march segments; threads = ncol * S
     int half;              // colour
+    int parity_rows;       // 1: a warp's cross rows all have the same parity (see column_of)
     long long *obs;        // (B, M) accumulator or nullptr
 };
 
-struct HalfTab {           // spin-1/2
-    uint32_t t32[16];
-    uint32_t k0w, k1w;     // 0x7F + always_below[b], replicated in the four bytes
-};
+struct HalfTab { uint32_t t[16]; };            // spin-1/2: t[n + 8*b] = thr - 1  (accept iff w <= t)
 struct NeTab { uint32_t t32; int always; };
 struct OneTab { uint2 e[96]; };
 template <int MODEL> struct TabOf { using type = NeTab; };
@@ -116,14 +120,9 @@ template <> struct TabOf<M_ISING_ONE> { using type = OneTab; };
 
 __device__ __forceinline__ uint32_t bytesum(uint32_t v) { return __dp4a(v, 0x01010101u, 0u); }
 
-// ------------------------------------------------------------------------------------------
-// Per-lane (4 sites) update rules
-// ------------------------------------------------------------------------------------------
-// Ising spin-1/2 (PAPER.md:88; readings D1, D3).  own: 4 site bytes; nsum: byte-wise sum of the
-// 2d neighbour lanes; r: the four random words of this lane's Philox call.
 // s_t: shared-state-space address of the threshold table (warp-uniform, lives in a uniform
-// register).  The per-site table offset is one byte extract of the pre-scaled index word 4*idx and
-// the load is LDS [R + UR]: two instructions per site besides the compare and the predicated OR.
+// register).  The per-site table offset is one byte extract of the pre-scaled index word and the
+// load is LDS [R + UR].
 __device__ __forceinline__ uint32_t lds_u32(uint32_t s_t, uint32_t byte_off)
 {
     uint32_t v;
@@ -131,32 +130,34 @@ __device__ __forceinline__ uint32_t lds_u32(uint32_t s_t, uint32_t byte_off)
     return v;
 }
 
-template <int DIMS, bool TRACK, bool FIELD, int OBS>
+// ------------------------------------------------------------------------------------------
+// Per-lane (4 sites) update rules
+// ------------------------------------------------------------------------------------------
+// Ising spin-1/2 (PAPER.md:88; readings D1, D3).  own: 4 site bytes; nsum: byte-wise sum of the
+// 2d neighbour lanes (= number of up neighbours per site); r: the four random words of the lane.
+// The table holds thr-1 for every (b, n), so "w < thr" is "w <= t" and thr = 2^32 needs no special
+// case (tables with a thr = 0 entry are left to the scalar family, see tiled_supported).
+template <bool TRACK, int OBS>
 __device__ __forceinline__ uint32_t rule_half(uint32_t own, uint32_t nsum, uint4 r, uint32_t s_t,
-                                              uint32_t k0w, uint32_t k1w, uint32_t &accA, uint32_t &accU)
+                                              uint32_t &accU, uint32_t &accN, uint32_t &accBN)
 {
-    constexpr uint32_t K2D = (uint32_t)(2 * DIMS) * 0x01010101u;
-    uint32_t b = TRACK ? (own & 0x01010101u) : own;
-    uint32_t n = TRACK ? (nsum & 0x07070707u) : nsum;      // up-neighbour count per byte
-    uint32_t c = K2D - n;                                  // down-neighbour count
-    uint32_t bm = b * 0xFFu;
-    uint32_t a = (n & bm) | (c & ~bm);                     // neighbours aligned with the spin
-    uint32_t adr = a << 2;                                 // byte offset of t32[a] (+ 32 b with a field)
-    if (FIELD) adr = b * 32u + adr;
-    uint32_t kw = FIELD ? ((k1w & bm) | (k0w & ~bm)) : k0w;
-    uint32_t f = (kw - a) & 0x80808080u;                   // bit 7 <=> a < always_below: dE <= 0
-    if (r.x < lds_u32(s_t, adr & 0xFFu)) f |= 0x00000080u;
-    if (r.y < lds_u32(s_t, __byte_perm(adr, 0u, 0x4441))) f |= 0x00008000u;
-    if (r.z < lds_u32(s_t, __byte_perm(adr, 0u, 0x4442))) f |= 0x00800000u;
-    if (r.w < lds_u32(s_t, adr >> 24)) f |= 0x80000000u;
-    uint32_t fl = f >> 7;                                  // 0/1 per byte: flip
-    uint32_t b2 = b ^ fl;
+    const uint32_t b = TRACK ? (own & 0x01010101u) : own;
+    const uint32_t n = TRACK ? (nsum & 0x07070707u) : nsum;
+    const uint32_t adr = b * 32u + n * 4u;                 // byte offset of t[n + 8b], per site byte
+    uint32_t t = b;                                        // b + accepted flips (bytes end up 0, 1 or 2)
+    if (r.x <= lds_u32(s_t, adr & 0xFFu)) t += 0x00000001u;
+    if (r.y <= lds_u32(s_t, __byte_perm(adr, 0u, 0x4441))) t += 0x00000100u;
+    if (r.z <= lds_u32(s_t, __byte_perm(adr, 0u, 0x4442))) t += 0x00010000u;
+    if (r.w <= lds_u32(s_t, adr >> 24)) t += 0x01000000u;
+    const uint32_t b2 = t & 0x01010101u;                   // b xor flip
     if (OBS >= 1) accU += b2;
     if (OBS >= 2) {
-        uint32_t b2m = b2 * 0xFFu;
-        accA += (n & b2m) | (c & ~b2m);                    // aligned count after the update
+        accN += n;
+        accBN += n & (b2 * 0xFFu);
     }
-    return TRACK ? ((own ^ fl) | (fl << 3)) : b2;
+    if (!TRACK) return b2;
+    const uint32_t fl = b ^ b2;
+    return (own ^ fl) | (fl << 3);                         // value bit, and "ever changed" (0x08) set on a flip
 }
 
 // North-East model (readings D7, D8): facilitated iff north and east are up.
@@ -209,162 +210,221 @@ __device__ __forceinline__ uint32_t rule_one(uint32_t own, uint32_t nsum, uint4 
 }
 
 // ------------------------------------------------------------------------------------------
-// The marching kernel.  MODEL selects the rule; DIMS the neighbourhood.
+// One thread's march.  Q is the row parity bit q = (march + cross + colour) & 1 of the current step
+// when it is known at compile time (0 / 1: the side neighbour is the byte to the left / right), or
+// 2 when it has to be read from the register (warps whose lanes mix row parities).
 // ------------------------------------------------------------------------------------------
-template <int MODEL, int DIMS, bool TRACK, bool FIELD, int OBS>
-__global__ void __launch_bounds__(256) k_sweep_tiled(const __grid_constant__ TiledGeom g, const __grid_constant__ PhiloxSweepConsts pc,
-                                                     const __grid_constant__ typename TabOf<MODEL>::type tab)
+template <int MODEL, int DIMS, bool TRACK, int OBS>
+struct March {
+    const uint4 *pC;        // other colour, word of the current step
+    uint4 *pO;              // own colour, word of the current step
+    const uint32_t *pE;     // other colour, start of the current compact row (32-bit lanes)
+    uint4 P, C;             // other colour at march-1 and march
+    uint32_t grp;           // Philox group of lane 0 of the current word
+    int m, q;
+    int e_hi, e_lo, dyp, dyn, rowstride, L;
+    long long wrapw;
+    int totU, totN, totBN;  // per-thread sums; < 2^31 for every legal lattice
+    uint32_t s_t;
+    const uint2 *s_e;
+    uint32_t ne_t32;
+    int ne_always;
+
+    template <int Q>
+    __device__ __forceinline__ void step(const PhiloxSweepConsts &pc)
+    {
+        const int qq = Q == 2 ? q : Q;
+        const uint4 *pN = pC + rowstride;
+        if (m + 1 == L) pN -= wrapw;
+        const uint4 N = *pN;
+        const uint4 O = *pO;
+        const uint32_t e = pE[qq ? e_hi : e_lo];
+        uint4 Yp, Yn;
+        if (DIMS == 3) {
+            Yp = pC[dyp];
+            Yn = pC[dyn];
+        }
+        // the neighbour one byte to the right (q = 1) or left (q = 0) of every site of the word
+        uint32_t sd[4];
+        if (qq) {
+            sd[0] = __funnelshift_r(C.x, C.y, 8);
+            sd[1] = __funnelshift_r(C.y, C.z, 8);
+            sd[2] = __funnelshift_r(C.z, C.w, 8);
+            sd[3] = __funnelshift_r(C.w, e, 8);
+        } else {
+            sd[0] = __funnelshift_r(e, C.x, 24);
+            sd[1] = __funnelshift_r(C.x, C.y, 24);
+            sd[2] = __funnelshift_r(C.y, C.z, 24);
+            sd[3] = __funnelshift_r(C.z, C.w, 24);
+        }
+        const uint32_t o[4] = {O.x, O.y, O.z, O.w};
+        const uint32_t p[4] = {P.x, P.y, P.z, P.w};
+        const uint32_t n[4] = {N.x, N.y, N.z, N.w};
+        const uint32_t c[4] = {C.x, C.y, C.z, C.w};
+        uint32_t yp[4] = {0, 0, 0, 0}, yn[4] = {0, 0, 0, 0};
+        if (DIMS == 3) {
+            yp[0] = Yp.x; yp[1] = Yp.y; yp[2] = Yp.z; yp[3] = Yp.w;
+            yn[0] = Yn.x; yn[1] = Yn.y; yn[2] = Yn.z; yn[3] = Yn.w;
+        }
+        uint32_t out[4];
+
+        if (MODEL == M_ISING_HALF) {
+            uint32_t accU = 0, accN = 0, accBN = 0;
+#pragma unroll
+            for (int d = 0; d < 4; ++d) {
+                uint32_t ns = p[d] + n[d] + c[d] + sd[d];
+                if (DIMS == 3) ns += yp[d] + yn[d];
+                uint4 r = philox_sweep(grp + d, pc);
+                out[d] = rule_half<TRACK, OBS>(o[d], ns, r, s_t, accU, accN, accBN);
+            }
+            if (OBS >= 1) totU += bytesum(accU);
+            if (OBS >= 2) { totN += bytesum(accN); totBN += bytesum(accBN); }
+        } else if (MODEL == M_ISING_ONE) {
+            int accB = 0, accM = 0;
+#pragma unroll
+            for (int d = 0; d < 4; ++d) {
+                uint32_t ns;
+                if (TRACK) {
+                    // flags sit at 0x10/0x60: two flagged bytes still add without a carry
+                    ns = ((p[d] + n[d]) & 0x0F0F0F0Fu) + ((c[d] + sd[d]) & 0x0F0F0F0Fu);
+                    if (DIMS == 3) ns += (yp[d] + yn[d]) & 0x0F0F0F0Fu;
+                } else {
+                    ns = p[d] + n[d] + c[d] + sd[d];
+                    if (DIMS == 3) ns += yp[d] + yn[d];
+                }
+                uint4 ra = philox_sweep(2u * (grp + d), pc);
+                uint4 rb = philox_sweep(2u * (grp + d) + 1u, pc);
+                out[d] = rule_one<DIMS, TRACK, OBS>(o[d], ns, ra, rb, s_e, accB, accM);
+            }
+            totU += accM;
+            totBN += accB;
+        } else {
+            uint32_t accU = 0;
+#pragma unroll
+            for (int d = 0; d < 4; ++d) {
+                uint32_t east = qq ? sd[d] : c[d];
+                out[d] = rule_ne<TRACK, MODEL == M_NE_METROPOLIS, OBS>(o[d], n[d], east, grp + d, pc, ne_t32, ne_always, accU);
+            }
+            if (OBS >= 1) totU += bytesum(accU);
+        }
+        *pO = make_uint4(out[0], out[1], out[2], out[3]);
+        P = C;
+        C = N;
+        pC += rowstride;
+        pO += rowstride;
+        pE += rowstride * 4;
+        grp += (uint32_t)rowstride * 4u;
+        m += 1;
+        if (Q == 2) q ^= 1;
+    }
+
+    template <int Q0>
+    __device__ __forceinline__ void run(int m1, const PhiloxSweepConsts &pc)
+    {
+        constexpr int Q1 = Q0 == 2 ? 2 : 1 - Q0;
+        while (m + 1 < m1) {
+            step<Q0>(pc);
+            step<Q1>(pc);
+        }
+        if (m < m1) step<Q0>(pc);
+    }
+};
+
+// Thread -> (cross row y, word j).  With parity_rows the 32 lanes of a warp take 32/wpr rows of the
+// SAME parity (rows y0, y0+2, ...; the neighbouring warp takes the rows in between), so that q is
+// warp-uniform and can be a compile-time constant of the unrolled loop; every row is still read
+// as whole contiguous 16*wpr-byte pieces.
+__device__ __forceinline__ void column_of(const TiledGeom &g, int col, int &y, int &j)
+{
+    if (g.R == 1) { y = 0; j = col; return; }
+    if (g.parity_rows && g.wpr < 32) {
+        const int rpw = 32 / g.wpr;
+        const int wg = col >> 5, lane = col & 31;
+        y = (wg >> 1) * (2 * rpw) + 2 * (lane / g.wpr) + (wg & 1);
+        j = lane % g.wpr;
+    } else {
+        y = col / g.wpr;
+        j = col - y * g.wpr;
+    }
+}
+
+#ifndef LSM_TILED_MINBLOCKS
+#define LSM_TILED_MINBLOCKS 4
+#endif
+template <int MODEL, int DIMS, bool TRACK, int OBS>
+__global__ void __launch_bounds__(256, LSM_TILED_MINBLOCKS)
+k_sweep_tiled(const __grid_constant__ TiledGeom g, const __grid_constant__ PhiloxSweepConsts pc,
+              const __grid_constant__ typename TabOf<MODEL>::type tab)
 {
     __shared__ __align__(16) struct {
         uint32_t t[16];
         long long red[2][8];
         uint2 e[MODEL == M_ISING_ONE ? 96 : 1];
     } sm;
-    uint2 *s_e = sm.e;
-    uint32_t k0w = 0, k1w = 0, ne_t32 = 0;
     uint32_t s_t = (uint32_t)__cvta_generic_to_shared(sm.t);
     asm volatile("" : "+r"(s_t));   // keep the (warp-uniform) table address out of the divergent region below
-    int ne_always = 0;
+    March<MODEL, DIMS, TRACK, OBS> M;
+    M.ne_t32 = 0;
+    M.ne_always = 0;
     if constexpr (MODEL == M_ISING_HALF) {
-        if (threadIdx.x < 16) sm.t[threadIdx.x] = tab.t32[threadIdx.x];
-        k0w = tab.k0w;
-        k1w = tab.k1w;
+        if (threadIdx.x < 16) sm.t[threadIdx.x] = tab.t[threadIdx.x];
     } else if constexpr (MODEL == M_ISING_ONE) {
-        if (threadIdx.x < 96) s_e[threadIdx.x] = tab.e[threadIdx.x];
+        if (threadIdx.x < 96) sm.e[threadIdx.x] = tab.e[threadIdx.x];
     } else {
-        ne_t32 = tab.t32;
-        ne_always = tab.always;
+        M.ne_t32 = tab.t32;
+        M.ne_always = tab.always;
     }
     __syncthreads();
+    M.s_t = s_t;
+    M.s_e = sm.e;
+    M.totU = M.totN = M.totBN = 0;
 
-    const uint4 *__restrict__ oth = reinterpret_cast<const uint4 *>(g.oth);
-    const uint32_t *__restrict__ oth32 = reinterpret_cast<const uint32_t *>(g.oth);
-    uint4 *__restrict__ own = reinterpret_cast<uint4 *>(g.own);
-
-    long long gt = (long long)blockIdx.x * blockDim.x + threadIdx.x;
-    const bool active = gt < (long long)g.ncol * g.S;
-    int totA = 0, totU = 0;         // per-thread sums (a' or s'*nn ; value sum): < 2^31 for any legal L
+    const long long gt = (long long)blockIdx.x * blockDim.x + threadIdx.x;
     int nsites = 0;
-
-    if (active) {
+    if (gt < (long long)g.ncol * g.S) {
         const int seg = (int)(gt / g.ncol);
         const int col = (int)(gt - (long long)seg * g.ncol);
-        const int y = DIMS == 3 ? col / g.wpr : 0;
-        const int j = col - y * g.wpr;
+        int y, j;
+        column_of(g, col, y, j);
         const int m0 = (int)(((long long)g.L * seg) / g.S);
         const int m1 = (int)(((long long)g.L * (seg + 1)) / g.S);
         const int yu = (y + 1 == g.R) ? 0 : y + 1, yd = (y == 0) ? g.R - 1 : y - 1;
-        const int e_hi = ((j + 1 == g.wpr) ? 0 : j + 1) * 4;        // first lane of the next word
-        const int e_lo = ((j == 0) ? g.wpr - 1 : j - 1) * 4 + 3;    // last lane of the previous word
-        const int rowstride = g.R * g.wpr;                          // words per march step
-        const long long wrapw = (long long)g.L * rowstride;         // words per colour array
-        const int dyp = (yd - y) * g.wpr, dyn = (yu - y) * g.wpr;   // cross-row neighbours (3D), in words
-
-        const long long w0 = (long long)m0 * rowstride + y * g.wpr + j;
-        const uint4 *pC = oth + w0;                                  // other colour, this march step
-        uint4 *pO = own + w0;
-        const uint32_t *pE = oth32 + ((long long)m0 * rowstride + y * g.wpr) * 4;   // start of the compact row
-        uint32_t grp = (uint32_t)w0 * 4u;                            // Philox group of lane 0 (byte offset >> 2)
-        int q = (m0 + y + g.half) & 1;
-        uint4 P = *(m0 == 0 ? pC + (wrapw - rowstride) : pC - rowstride);
-        uint4 C = *pC;
+        M.e_hi = ((j + 1 == g.wpr) ? 0 : j + 1) * 4;               // first lane of the next word
+        M.e_lo = ((j == 0) ? g.wpr - 1 : j - 1) * 4 + 3;           // last lane of the previous word
+        M.rowstride = g.R * g.wpr;                                 // words per march step
+        M.wrapw = (long long)g.L * M.rowstride;                    // words per colour array
+        M.dyp = (yd - y) * g.wpr;                                  // cross-row neighbours (3D), in words
+        M.dyn = (yu - y) * g.wpr;
+        M.L = g.L;
+        const long long w0 = (long long)m0 * M.rowstride + y * g.wpr + j;
+        M.pC = reinterpret_cast<const uint4 *>(g.oth) + w0;
+        M.pO = reinterpret_cast<uint4 *>(g.own) + w0;
+        M.pE = reinterpret_cast<const uint32_t *>(g.oth) + ((long long)m0 * M.rowstride + y * g.wpr) * 4;
+        M.grp = (uint32_t)w0 * 4u;
+        M.m = m0;
+        M.q = (m0 + y + g.half) & 1;
+        M.P = *(m0 == 0 ? M.pC + (M.wrapw - M.rowstride) : M.pC - M.rowstride);
+        M.C = *M.pC;
         nsites = 16 * (m1 - m0);
-
-        for (int m = m0; m < m1; ++m) {
-            const uint4 *pN = pC + rowstride;
-            if (m + 1 == g.L) pN -= wrapw;
-            const uint4 N = *pN;
-            const uint4 O = *pO;
-            const uint32_t e = pE[q ? e_hi : e_lo];
-            uint4 Yp, Yn;
-            if (DIMS == 3) {
-                Yp = pC[dyp];
-                Yn = pC[dyn];
-            }
-            // the neighbour one byte to the right (q = 1) or left (q = 0) of every site of the word
-            uint32_t sd[4];
-            if (q) {
-                sd[0] = __funnelshift_r(C.x, C.y, 8);
-                sd[1] = __funnelshift_r(C.y, C.z, 8);
-                sd[2] = __funnelshift_r(C.z, C.w, 8);
-                sd[3] = __funnelshift_r(C.w, e, 8);
-            } else {
-                sd[0] = __funnelshift_r(e, C.x, 24);
-                sd[1] = __funnelshift_r(C.x, C.y, 24);
-                sd[2] = __funnelshift_r(C.y, C.z, 24);
-                sd[3] = __funnelshift_r(C.z, C.w, 24);
-            }
-            const uint32_t o[4] = {O.x, O.y, O.z, O.w};
-            const uint32_t p[4] = {P.x, P.y, P.z, P.w};
-            const uint32_t n[4] = {N.x, N.y, N.z, N.w};
-            const uint32_t c[4] = {C.x, C.y, C.z, C.w};
-            uint32_t yp[4], yn[4];
-            if (DIMS == 3) {
-                yp[0] = Yp.x; yp[1] = Yp.y; yp[2] = Yp.z; yp[3] = Yp.w;
-                yn[0] = Yn.x; yn[1] = Yn.y; yn[2] = Yn.z; yn[3] = Yn.w;
-            }
-            uint32_t out[4];
-
-            if (MODEL == M_ISING_HALF) {
-                uint32_t accA = 0, accU = 0;
-#pragma unroll
-                for (int d = 0; d < 4; ++d) {
-                    uint32_t ns = p[d] + n[d] + c[d] + sd[d];
-                    if (DIMS == 3) ns += yp[d] + yn[d];
-                    uint4 r = philox_sweep(grp + d, pc);
-                    out[d] = rule_half<DIMS, TRACK, FIELD, OBS>(o[d], ns, r, s_t, k0w, k1w, accA, accU);
-                }
-                if (OBS >= 1) totU += bytesum(accU);
-                if (OBS >= 2) totA += bytesum(accA);
-            } else if (MODEL == M_ISING_ONE) {
-                int accB = 0, accM = 0;
-#pragma unroll
-                for (int d = 0; d < 4; ++d) {
-                    uint32_t ns;
-                    if (TRACK) {
-                        // flags sit at 0x10/0x60: two flagged bytes still add without a carry
-                        ns = ((p[d] + n[d]) & 0x0F0F0F0Fu) + ((c[d] + sd[d]) & 0x0F0F0F0Fu);
-                        if (DIMS == 3) ns += (yp[d] + yn[d]) & 0x0F0F0F0Fu;
-                    } else {
-                        ns = p[d] + n[d] + c[d] + sd[d];
-                        if (DIMS == 3) ns += yp[d] + yn[d];
-                    }
-                    uint4 ra = philox_sweep(2u * (grp + d), pc);
-                    uint4 rb = philox_sweep(2u * (grp + d) + 1u, pc);
-                    out[d] = rule_one<DIMS, TRACK, OBS>(o[d], ns, ra, rb, s_e, accB, accM);
-                }
-                totU += accM;
-                totA += accB;
-            } else {
-                uint32_t accU = 0;
-#pragma unroll
-                for (int d = 0; d < 4; ++d) {
-                    uint32_t east = q ? sd[d] : c[d];
-                    out[d] = rule_ne<TRACK, MODEL == M_NE_METROPOLIS, OBS>(o[d], n[d], east, grp + d, pc, ne_t32, ne_always, accU);
-                }
-                if (OBS >= 1) totU += bytesum(accU);
-            }
-            *pO = make_uint4(out[0], out[1], out[2], out[3]);
-            P = C;
-            C = N;
-            pC += rowstride;
-            pO += rowstride;
-            pE += rowstride * 4;
-            grp += (uint32_t)rowstride * 4u;
-            q ^= 1;
+        if (g.parity_rows) {            // warp-uniform branch: q is a constant inside each loop
+            if (M.q) M.template run<1>(m1, pc);
+            else M.template run<0>(m1, pc);
+        } else {
+            M.template run<2>(m1, pc);
         }
     }
 
     if (OBS >= 1) {
         long long cB = 0, cM = 0;
         if (MODEL == M_ISING_HALF) {
-            cM = 2LL * totU - nsites;                         // sum of (2b'-1)
-            cB = 2LL * totA - (long long)(2 * DIMS) * nsites; // sum of s'*nn = sum of (2a' - 2d)
+            // sum of s' = 2b'-1 ; sum of s'*nn = sum (2b'-1)(2n-2d)
+            cM = 2LL * M.totU - nsites;
+            cB = 4LL * M.totBN - 2LL * M.totN - 4LL * DIMS * M.totU + 2LL * DIMS * nsites;
         } else if (MODEL == M_ISING_ONE) {
-            cM = totU;
-            cB = totA;
+            cM = M.totU;
+            cB = M.totBN;
         } else {
-            cM = totU;
+            cM = M.totU;
         }
         block_accumulate2_in(sm.red, cB, cM, g.obs, OBS >= 2, true);
     }
@@ -380,22 +440,15 @@ void build_tiled_tables(int model, int dims, double J, double h, const uint64_t 
     const uint64_t ALWAYS = (uint64_t)1 << 32;
     auto clip = [&](uint64_t v) { return v >= ALWAYS ? 0xFFFFFFFFu : (uint32_t)v; };
     const int d = dims;
+    (void)J; (void)h; (void)nthr;
     if (model == M_ISING_HALF) {
-        t.field = (h != 0.0) ? 1 : 0;
-        t.usable = (J > 0.0) ? 1 : 0;   // dE increasing in the aligned count needs J > 0
-        for (int b = 0; b < 2; ++b) {
-            int below = 0;
-            bool mono = true;
-            for (int a = 0; a <= 2 * d; ++a) {
-                int n = b ? a : 2 * d - a;                 // up-neighbour count
+        t.usable = 1;
+        for (int b = 0; b < 2; ++b)
+            for (int n = 0; n <= 2 * d; ++n) {
                 uint64_t v = thr[b * (2 * d + 1) + n];
-                t.t32[a + 8 * b] = clip(v);
-                if (v == ALWAYS) { if (a != below) mono = false; below = a + 1; }
+                if (v == 0) t.usable = 0;                  // "never" cannot be written as w <= thr-1
+                t.t32[n + 8 * b] = (uint32_t)(v - 1);
             }
-            t.always_below[b] = (uint32_t)below;
-            if (!mono) t.usable = 0;
-        }
-        if (!t.field) for (int a = 0; a < 8; ++a) if (t.t32[a] != t.t32[a + 8]) t.usable = 0;
     } else if (model == M_ISING_ONE) {
         t.usable = 1;
         for (int a = 0; a < 3; ++a)
@@ -412,7 +465,6 @@ void build_tiled_tables(int model, int dims, double J, double h, const uint64_t 
         t.ne_up_always = thr[1] == ALWAYS ? 1 : 0;
         if (thr[0] == ALWAYS) t.usable = 0;
     }
-    (void)nthr;
     *out = t;
 }
 
@@ -425,33 +477,32 @@ bool tiled_supported(const Lat &lat, int model, const TiledTables &t)
     return true;
 }
 
-static int g_tiled_ctas_per_sm = 4;
+// Launch shape: threads = word columns x march segments, one wave of CTAS_PER_SM resident CTAs per
+// SM (finer segments do not help: measured, profiles/).  Overridable for tuning experiments.
+static int env_int(const char *name, int dflt)
+{
+    const char *v = getenv(name);
+    return (v && *v) ? atoi(v) : dflt;
+}
+static int g_tiled_ctas_per_sm = env_int("LSM_TILED_CTAS_PER_SM", 4);
+static int g_tiled_waves_x4 = env_int("LSM_TILED_WAVES_X4", 4);   // waves in quarters
 
-template <int MODEL, int DIMS, bool TRACK, bool FIELD>
+template <int MODEL, int DIMS, bool TRACK>
 static cudaError_t launch_obs(int obs_mode, dim3 grid, cudaStream_t s, const TiledGeom &g, const PhiloxSweepConsts &pc,
                               const typename TabOf<MODEL>::type &tab)
 {
-    if (obs_mode == 0) k_sweep_tiled<MODEL, DIMS, TRACK, FIELD, 0><<<grid, 256, 0, s>>>(g, pc, tab);
-    else if (obs_mode == 1) k_sweep_tiled<MODEL, DIMS, TRACK, FIELD, 1><<<grid, 256, 0, s>>>(g, pc, tab);
-    else k_sweep_tiled<MODEL, DIMS, TRACK, FIELD, 2><<<grid, 256, 0, s>>>(g, pc, tab);
+    if (obs_mode == 0) k_sweep_tiled<MODEL, DIMS, TRACK, 0><<<grid, 256, 0, s>>>(g, pc, tab);
+    else if (obs_mode == 1) k_sweep_tiled<MODEL, DIMS, TRACK, 1><<<grid, 256, 0, s>>>(g, pc, tab);
+    else k_sweep_tiled<MODEL, DIMS, TRACK, 2><<<grid, 256, 0, s>>>(g, pc, tab);
     return cudaGetLastError();
 }
 
 template <int MODEL, int DIMS>
-static cudaError_t launch_track_field(bool track, bool field, int obs_mode, dim3 grid, cudaStream_t s, const TiledGeom &g,
-                                      const PhiloxSweepConsts &pc, const typename TabOf<MODEL>::type &tab)
+static cudaError_t launch_track(bool track, int obs_mode, dim3 grid, cudaStream_t s, const TiledGeom &g,
+                                const PhiloxSweepConsts &pc, const typename TabOf<MODEL>::type &tab)
 {
-    if constexpr (MODEL == M_ISING_HALF) {
-        if (track) {
-            if (field) return launch_obs<MODEL, DIMS, true, true>(obs_mode, grid, s, g, pc, tab);
-            return launch_obs<MODEL, DIMS, true, false>(obs_mode, grid, s, g, pc, tab);
-        }
-        if (field) return launch_obs<MODEL, DIMS, false, true>(obs_mode, grid, s, g, pc, tab);
-        return launch_obs<MODEL, DIMS, false, false>(obs_mode, grid, s, g, pc, tab);
-    } else {
-        if (track) return launch_obs<MODEL, DIMS, true, false>(obs_mode, grid, s, g, pc, tab);
-        return launch_obs<MODEL, DIMS, false, false>(obs_mode, grid, s, g, pc, tab);
-    }
+    if (track) return launch_obs<MODEL, DIMS, true>(obs_mode, grid, s, g, pc, tab);
+    return launch_obs<MODEL, DIMS, false>(obs_mode, grid, s, g, pc, tab);
 }
 
 cudaError_t launch_sweep_tiled(const SweepArgs &a, const TiledTables &t, cudaStream_t s)
@@ -465,7 +516,12 @@ cudaError_t launch_sweep_tiled(const SweepArgs &a, const TiledTables &t, cudaStr
     g.ncol = g.R * g.wpr;
     g.half = a.half;
     g.obs = a.obs;
-    long long target = (long long)sm_count() * g_tiled_ctas_per_sm * 256;
+    // q = (march + y + colour) & 1 is warp-uniform if a warp sees one row parity only
+    if (g.R == 1) g.parity_rows = 1;                                   // 2D: y = 0 for every thread
+    else if (g.wpr % 32 == 0) g.parity_rows = 1;
+    else if (g.wpr < 32 && 32 % g.wpr == 0 && g.R % (2 * (32 / g.wpr)) == 0) g.parity_rows = 1;
+    else g.parity_rows = 0;
+    long long target = (long long)sm_count() * g_tiled_ctas_per_sm * 256 * g_tiled_waves_x4 / 4;
     long long S = target / g.ncol;
     if (S < 1) S = 1;
     if (S > g.L) S = g.L;
@@ -475,30 +531,28 @@ cudaError_t launch_sweep_tiled(const SweepArgs &a, const TiledTables &t, cudaStr
 
     PhiloxSweepConsts pc = make_philox_consts(a.key);
     int obs_mode = a.obs ? (a.want_B ? 2 : 1) : 0;
-    const bool track = a.track != 0, field = t.field != 0;
+    const bool track = a.track != 0;
     const bool d3 = a.lat.dims == 3;
     switch (a.model) {
     case M_ISING_HALF: {
         HalfTab ht;
-        for (int i = 0; i < 16; ++i) ht.t32[i] = t.t32[i];
-        ht.k0w = (0x7Fu + t.always_below[0]) * 0x01010101u;
-        ht.k1w = (0x7Fu + t.always_below[1]) * 0x01010101u;
-        return d3 ? launch_track_field<M_ISING_HALF, 3>(track, field, obs_mode, grid, s, g, pc, ht)
-                  : launch_track_field<M_ISING_HALF, 2>(track, field, obs_mode, grid, s, g, pc, ht);
+        for (int i = 0; i < 16; ++i) ht.t[i] = t.t32[i];
+        return d3 ? launch_track<M_ISING_HALF, 3>(track, obs_mode, grid, s, g, pc, ht)
+                  : launch_track<M_ISING_HALF, 2>(track, obs_mode, grid, s, g, pc, ht);
     }
     case M_ISING_ONE: {
         OneTab ot;
         for (int i = 0; i < 96; ++i) ot.e[i] = t.s1[i];
-        return d3 ? launch_track_field<M_ISING_ONE, 3>(track, false, obs_mode, grid, s, g, pc, ot)
-                  : launch_track_field<M_ISING_ONE, 2>(track, false, obs_mode, grid, s, g, pc, ot);
+        return d3 ? launch_track<M_ISING_ONE, 3>(track, obs_mode, grid, s, g, pc, ot)
+                  : launch_track<M_ISING_ONE, 2>(track, obs_mode, grid, s, g, pc, ot);
     }
     case M_NE_HEATBATH: {
         NeTab nt = {t.ne_t32[0], 0};
-        return launch_track_field<M_NE_HEATBATH, 2>(track, false, obs_mode > 1 ? 1 : obs_mode, grid, s, g, pc, nt);
+        return launch_track<M_NE_HEATBATH, 2>(track, obs_mode > 1 ? 1 : obs_mode, grid, s, g, pc, nt);
     }
     default: {
         NeTab nt = {t.ne_t32[1], t.ne_up_always};
-        return launch_track_field<M_NE_METROPOLIS, 2>(track, false, obs_mode > 1 ? 1 : obs_mode, grid, s, g, pc, nt);
+        return launch_track<M_NE_METROPOLIS, 2>(track, obs_mode > 1 ? 1 : obs_mode, grid, s, g, pc, nt);
     }
     }
 }

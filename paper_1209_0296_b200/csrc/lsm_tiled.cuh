@@ -9,17 +9,14 @@ namespace lsmk {
 // Threshold tables in the form the vectorised kernels index.  Built on the host from the canonical
 // 33-bit table (lsm_get_thresholds order), so both families accept exactly the same (w, state) pairs.
 struct TiledTables {
-    int usable;            // 0: this (model, J, h) combination is left to the scalar family
-    int field;             // spin-1/2: h != 0, the table row depends on the spin value
-    // spin-1/2: idx = a + 8*b, a = number of neighbours aligned with the spin, b = (s+1)/2.
-    //   t32 = thr clipped to 32 bits; acceptance with certainty (thr = 2^32) is the byte-parallel
-    //   test a < always_below[b] (dE = 4J(a-d) +- 2h is increasing in a for J > 0).
+    int usable;            // 0: this table is left to the scalar family
+    // spin-1/2: t32[n + 8*b] = thr - 1 (accept iff w <= t32), b = (s+1)/2, n = up-neighbour count.
+    //   A table with a thr = 0 ("never") entry has no such form -> usable = 0.
     uint32_t t32[16];
-    uint32_t always_below[2];
     // NE: [0] heat-bath / init threshold, [1] Metropolis 0->1 threshold (32-bit clipped) + flag
     uint32_t ne_t32[2];
     int ne_up_always;
-    // spin-1: entry[(a*2+kk)*16 + sum] = { t32, proposed a' | always << 4 }
+    // spin-1: entry[(a*2+kk)*16 + sum] = { thr clipped to 32 bits, proposed a' | (thr == 2^32) << 4 }
     uint2 s1[96];
 };
 
