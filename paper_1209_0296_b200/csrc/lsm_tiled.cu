@@ -108,6 +108,7 @@ struct TiledGeom {
     int S;                 // march segments; threads = ncol * S
     int half;              // colour
     int parity_rows;       // 1: a warp's cross rows all have the same parity (see column_of)
+    int one;               // the constant 1, kept opaque to the compiler (see rule_half)
     long long *obs;        // (B, M) accumulator or nullptr
 };
 
@@ -137,18 +138,29 @@ __device__ __forceinline__ uint32_t lds_u32(uint32_t s_t, uint32_t byte_off)
 // 2d neighbour lanes (= number of up neighbours per site); r: the four random words of the lane.
 // The table holds thr-1 for every (b, n), so "w < thr" is "w <= t" and thr = 2^32 needs no special
 // case (tables with a thr = 0 entry are left to the scalar family, see tiled_supported).
+// t + INC if w <= thr.  `one` is a register that holds 1 but is opaque to the compiler, so the
+// predicated merge stays a multiply-add (IMAD): it issues on the FMA pipe, which has slack, instead of
+// the binding ALU pipe.
+template <uint32_t INC>
+__device__ __forceinline__ uint32_t add_if_le(uint32_t t, uint32_t w, uint32_t thr, uint32_t one)
+{
+    asm("{\n\t.reg .pred p;\n\tsetp.le.u32 p, %1, %2;\n\t@p mad.lo.u32 %0, %3, %4, %0;\n\t}"
+        : "+r"(t) : "r"(w), "r"(thr), "r"(one), "n"(INC));
+    return t;
+}
+
 template <bool TRACK, int OBS>
-__device__ __forceinline__ uint32_t rule_half(uint32_t own, uint32_t nsum, uint4 r, uint32_t s_t,
+__device__ __forceinline__ uint32_t rule_half(uint32_t own, uint32_t nsum, uint4 r, uint32_t s_t, uint32_t one,
                                               uint32_t &accU, uint32_t &accN, uint32_t &accBN)
 {
     const uint32_t b = TRACK ? (own & 0x01010101u) : own;
     const uint32_t n = TRACK ? (nsum & 0x07070707u) : nsum;
     const uint32_t adr = b * 32u + n * 4u;                 // byte offset of t[n + 8b], per site byte
     uint32_t t = b;                                        // b + accepted flips (bytes end up 0, 1 or 2)
-    if (r.x <= lds_u32(s_t, adr & 0xFFu)) t += 0x00000001u;
-    if (r.y <= lds_u32(s_t, __byte_perm(adr, 0u, 0x4441))) t += 0x00000100u;
-    if (r.z <= lds_u32(s_t, __byte_perm(adr, 0u, 0x4442))) t += 0x00010000u;
-    if (r.w <= lds_u32(s_t, adr >> 24)) t += 0x01000000u;
+    t = add_if_le<0x00000001u>(t, r.x, lds_u32(s_t, adr & 0xFFu), one);
+    t = add_if_le<0x00000100u>(t, r.y, lds_u32(s_t, __byte_perm(adr, 0u, 0x4441)), one);
+    t = add_if_le<0x00010000u>(t, r.z, lds_u32(s_t, __byte_perm(adr, 0u, 0x4442)), one);
+    t = add_if_le<0x01000000u>(t, r.w, lds_u32(s_t, adr >> 24), one);
     const uint32_t b2 = t & 0x01010101u;                   // b xor flip
     if (OBS >= 1) accU += b2;
     if (OBS >= 2) {
@@ -225,20 +237,44 @@ struct March {
     int e_hi, e_lo, dyp, dyn, rowstride, L;
     long long wrapw;
     int totU, totN, totBN;  // per-thread sums; < 2^31 for every legal lattice
-    uint32_t s_t;
+    uint32_t s_t, one;
     const uint2 *s_e;
     uint32_t ne_t32;
     int ne_always;
+
+#ifndef LSM_TILED_PREFETCH
+#define LSM_TILED_PREFETCH 0
+#endif
+    uint4 Nn, On;           // software pipeline, distance 1: loads of the next step, issued before this step computes
+    uint32_t en;
+    int m_end;
+
+    // loads of the step `ahead` march positions after the current one (row parity qa)
+    __device__ __forceinline__ void fetch(int ahead, int qa)
+    {
+        const uint4 *pN = pC + (ahead + 1) * rowstride;
+        if (m + ahead + 1 >= L) pN -= wrapw;
+        Nn = *pN;
+        On = pO[ahead * rowstride];
+        en = pE[ahead * rowstride * 4 + (qa ? e_hi : e_lo)];
+    }
 
     template <int Q>
     __device__ __forceinline__ void step(const PhiloxSweepConsts &pc)
     {
         const int qq = Q == 2 ? q : Q;
+#if LSM_TILED_PREFETCH
+        const uint4 N = Nn;
+        const uint4 O = On;
+        const uint32_t e = en;
+        if (m + 1 < m_end) fetch(1, qq ^ 1);
+#else
         const uint4 *pN = pC + rowstride;
         if (m + 1 == L) pN -= wrapw;
         const uint4 N = *pN;
         const uint4 O = *pO;
         const uint32_t e = pE[qq ? e_hi : e_lo];
+#endif
         uint4 Yp, Yn;
         if (DIMS == 3) {
             Yp = pC[dyp];
@@ -275,7 +311,7 @@ struct March {
                 uint32_t ns = p[d] + n[d] + c[d] + sd[d];
                 if (DIMS == 3) ns += yp[d] + yn[d];
                 uint4 r = philox_sweep(grp + d, pc);
-                out[d] = rule_half<TRACK, OBS>(o[d], ns, r, s_t, accU, accN, accBN);
+                out[d] = rule_half<TRACK, OBS>(o[d], ns, r, s_t, one, accU, accN, accBN);
             }
             if (OBS >= 1) totU += bytesum(accU);
             if (OBS >= 2) { totN += bytesum(accN); totBN += bytesum(accBN); }
@@ -322,6 +358,10 @@ struct March {
     __device__ __forceinline__ void run(int m1, const PhiloxSweepConsts &pc)
     {
         constexpr int Q1 = Q0 == 2 ? 2 : 1 - Q0;
+        m_end = m1;
+#if LSM_TILED_PREFETCH
+        fetch(0, Q0 == 2 ? q : Q0);
+#endif
         while (m + 1 < m1) {
             step<Q0>(pc);
             step<Q1>(pc);
@@ -376,6 +416,7 @@ k_sweep_tiled(const __grid_constant__ TiledGeom g, const __grid_constant__ Philo
     }
     __syncthreads();
     M.s_t = s_t;
+    M.one = (uint32_t)g.one;
     M.s_e = sm.e;
     M.totU = M.totN = M.totBN = 0;
 
@@ -516,6 +557,7 @@ cudaError_t launch_sweep_tiled(const SweepArgs &a, const TiledTables &t, cudaStr
     g.ncol = g.R * g.wpr;
     g.half = a.half;
     g.obs = a.obs;
+    g.one = 1;
     // q = (march + y + colour) & 1 is warp-uniform if a warp sees one row parity only
     if (g.R == 1) g.parity_rows = 1;                                   // 2D: y = 0 for every thread
     else if (g.wpr % 32 == 0) g.parity_rows = 1;
