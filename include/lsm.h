@@ -147,6 +147,11 @@ int lsm_energy(int model, double J, double h, int64_t bond_sum, int64_t M, doubl
  * calls and writes one word to d_sink[blocks*256]. */
 int lsm_philox_device(const uint32_t *d_ctr_key, uint32_t *d_out, int64_t n, void *stream);
 int lsm_philox_throughput(int blocks, int calls, uint32_t *d_sink, void *stream);
+/* lsm_pipe_probe: register-only integer instruction streams that show how the ALU and FMA pipes share
+ * issue.  mode 0: 16 LOP3, 1: 8 IMAD, 2: 8 IMAD.WIDE, 3: 8 IMAD + 16 LOP3, 4: 4 Philox calls,
+ * 5/6/7: 4 Philox calls + 80/160/240 independent LOP3 -- per loop iteration and thread; `blocks` x 256
+ * threads run `iters` iterations and write one word each to d_sink[blocks*256]. */
+int lsm_pipe_probe(int mode, int blocks, int iters, uint32_t *d_sink, void *stream);
 
 const char *lsm_strerror(int code);
 const char *lsm_last_cuda_error(void);

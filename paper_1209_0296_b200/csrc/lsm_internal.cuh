@@ -158,6 +158,7 @@ cudaError_t launch_get_spins(const Lat &lat, int model, int8_t *d_out, cudaStrea
 cudaError_t launch_set_spins(const Lat &lat, int model, const int8_t *d_in, cudaStream_t s);
 cudaError_t launch_philox_device(const uint32_t *d_ck, uint32_t *d_out, long long n, cudaStream_t s);
 cudaError_t launch_philox_throughput(int blocks, int calls, uint32_t *d_sink, cudaStream_t s);
+cudaError_t launch_pipe_probe(int mode, int blocks, int iters, uint32_t *d_sink, cudaStream_t s);
 
 int sm_count();
 

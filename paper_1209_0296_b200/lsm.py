@@ -51,6 +51,7 @@ SIGNATURES = {
     "lsm_energy": (_i32, [_i32, _dbl, _dbl, _i64, _i64, _P(_dbl)]),
     "lsm_philox_device": (_i32, [_vp, _vp, _i64, _vp]),
     "lsm_philox_throughput": (_i32, [_i32, _i32, _vp, _vp]),
+    "lsm_pipe_probe": (_i32, [_i32, _i32, _i32, _vp, _vp]),
     "lsm_strerror": (ctypes.c_char_p, [_i32]),
     "lsm_last_cuda_error": (ctypes.c_char_p, []),
 }
@@ -326,4 +327,14 @@ def philox_throughput(blocks, calls, stream=None):
     sink = torch.empty(blocks * 256, dtype=torch.int32, device="cuda")
     _check(load().lsm_philox_throughput(int(blocks), int(calls), _vp(sink.data_ptr()), _stream_ptr(stream)),
            "lsm_philox_throughput")
+    return sink
+
+
+def pipe_probe(mode, blocks, iters, stream=None):
+    """Enqueue one integer-pipe probe stream (see include/lsm.h); returns the sink tensor."""
+    import torch
+
+    sink = torch.empty(blocks * 256, dtype=torch.int32, device="cuda")
+    _check(load().lsm_pipe_probe(int(mode), int(blocks), int(iters), _vp(sink.data_ptr()), _stream_ptr(stream)),
+           "lsm_pipe_probe")
     return sink
