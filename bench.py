@@ -41,6 +41,8 @@ def parse():
     ap.add_argument("--workload", default="cfg2_T2.269")
     ap.add_argument("--sweeps-per-step", type=int, default=SWEEPS_PER_STEP)
     ap.add_argument("--no-extras", action="store_true", help="skip the secondary workloads / cpu baseline")
+    ap.add_argument("--kernel", default="auto", choices=["auto", "generic", "tiled", "resident"],
+                    help="kernel family (lsm_set_kernel); auto = the library's choice")
     return ap.parse_args()
 
 
@@ -186,6 +188,8 @@ def run_ours(args, w):
     lat = lsm.Lattice(**wl.create_args(), device=f"cuda:{local}")
     if wl.model == lsm.ISING:
         lat.set_tracking(False)  # persistence is not part of configs 1-4
+    if args.kernel != "auto":
+        lat.set_kernel({"generic": lsm.KERNEL_GENERIC, "tiled": lsm.KERNEL_TILED, "resident": lsm.KERNEL_RESIDENT}[args.kernel])
     N = lat.N
     obs = torch.empty((S, 2), dtype=torch.int64, device=lat.device)
     flush = torch.empty(256 << 20, dtype=torch.uint8, device=lat.device)  # > 126 MB L2

@@ -13,13 +13,13 @@ import sys
 PKG = os.path.dirname(os.path.abspath(__file__))
 CSRC = os.path.join(PKG, "csrc")
 LIB = os.path.join(PKG, "liblsm.so")
-SOURCES = ["lsm_api.cu", "lsm_generic.cu", "lsm_tiled.cu"]
+SOURCES = ["lsm_api.cu", "lsm_generic.cu", "lsm_tiled.cu", "lsm_resident.cu"]
 NVCC_FLAGS = [
     "-gencode", "arch=compute_100a,code=sm_100a",
     "-lineinfo", "-O3", "-std=c++17",
     # the threshold arithmetic of reading D3 must be plain IEEE double on the host
     "-Xcompiler", "-fPIC,-ffp-contract=off",
-    "-shared",
+    "-shared", "--threads", "0",
 ]
 
 

@@ -30,6 +30,8 @@ struct lsm {
     int nthr;
     Thr64 thr_param;
     TiledTables tiled;
+    unsigned *d_flags;  // resident family: one progress word per CTA
+    ResidentPlan plan;
 };
 
 static thread_local std::string g_cuda_err;
@@ -41,7 +43,7 @@ static int cuda_fail(cudaError_t e)
 #define CU(x) do { cudaError_t e__ = (x); if (e__ != cudaSuccess) return cuda_fail(e__); } while (0)
 
 static size_t align256(size_t v) { return (v + 255) & ~(size_t)255; }
-static const size_t STATE_BYTES = 256;
+static const size_t STATE_BYTES = 256 + 4 * (size_t)RESIDENT_MAX_CTAS;   // running sums, scratch, resident-kernel flags
 
 static int check_shape(int dims, int L, int two_S, int model)
 {
@@ -113,7 +115,8 @@ static void choose_kernel(lsm *o)
     bool tiled_ok = tiled_supported(o->lat, o->model, o->tiled);
     if (want == LSM_KERNEL_AUTO) want = tiled_ok ? LSM_KERNEL_TILED : LSM_KERNEL_GENERIC;
     if (want == LSM_KERNEL_TILED && !tiled_ok) want = LSM_KERNEL_GENERIC;
-    if (want == LSM_KERNEL_RESIDENT) want = tiled_ok ? LSM_KERNEL_TILED : LSM_KERNEL_GENERIC;
+    if (want == LSM_KERNEL_RESIDENT && !resident_plan(o->lat, o->model, o->tracking, o->tiled, &o->plan))
+        want = tiled_ok ? LSM_KERNEL_TILED : LSM_KERNEL_GENERIC;
     o->kernel_in_use = want;
 }
 
@@ -147,6 +150,7 @@ extern "C" int lsm_create(int dims, int L, int two_S, int model, double J, doubl
     uint8_t *base = (uint8_t *)d_workspace;
     o->d_run = (long long *)base;
     o->d_tmp = (long long *)(base + 64);
+    o->d_flags = (unsigned *)(base + 256);
     o->lat.col[0] = base + STATE_BYTES;
     o->lat.col[1] = base + STATE_BYTES + align256((size_t)o->N / 2);
     o->lat.L = L; o->lat.Lh = L / 2; o->lat.dims = dims; o->lat.Lz = dims == 3 ? L : 1;
@@ -187,10 +191,46 @@ static int enqueue_half(lsm *o, int half, long long *obs, int want_B, cudaStream
     return LSM_OK;
 }
 
+// Resident family: whole sweeps per launch.  Without a per-sweep record only the last sweep is
+// measured (into the running pair), so it gets a launch of its own.
+static int resident_launch(lsm *o, int64_t n, long long *obs, cudaStream_t s)
+{
+    const int64_t CHUNK = 1 << 20;
+    while (n > 0) {
+        int k = (int)(n < CHUNK ? n : CHUNK);
+        CU(cudaMemsetAsync(o->d_flags, 0, 8 * (size_t)o->plan.grid, s));
+        CU(launch_sweep_resident(o->lat, o->model, o->tracking, o->seed, o->t, k, obs, o->d_flags, 0u, o->plan,
+                                 o->tiled, s));
+        o->launches += 1;
+        o->t += (uint64_t)k;
+        if (obs) obs += 2 * (int64_t)k;
+        n -= k;
+    }
+    return LSM_OK;
+}
+
+static int sweep_resident(lsm *o, int64_t n, long long *d_obs, cudaStream_t s)
+{
+    if (d_obs) {
+        CU(cudaMemsetAsync(d_obs, 0, (size_t)n * 16, s));
+        int rc = resident_launch(o, n, d_obs, s);
+        if (rc != LSM_OK) return rc;
+        CU(cudaMemcpyAsync(o->d_run, d_obs + 2 * (n - 1), 16, cudaMemcpyDeviceToDevice, s));
+        return LSM_OK;
+    }
+    if (n > 1) {
+        int rc = resident_launch(o, n - 1, nullptr, s);
+        if (rc != LSM_OK) return rc;
+    }
+    CU(cudaMemsetAsync(o->d_run, 0, 16, s));
+    return resident_launch(o, 1, o->d_run, s);
+}
+
 static int sweep_impl(lsm *o, int64_t n, long long *d_obs, cudaStream_t s)
 {
     o->last_stream = s;
     if (n == 0) return LSM_OK;
+    if (o->kernel_in_use == LSM_KERNEL_RESIDENT) return sweep_resident(o, n, d_obs, s);
     if (d_obs) CU(cudaMemsetAsync(d_obs, 0, (size_t)n * 16, s));
     else CU(cudaMemsetAsync(o->d_run, 0, 16, s));
     for (int64_t k = 0; k < n; ++k) {
@@ -296,6 +336,7 @@ extern "C" int lsm_set_tracking(lsm_t *o, int on, void *stream)
     CU(launch_reset_reference(o->lat, o->model, on ? 1 : 0, s));
     o->launches += 1;
     o->tracking = on ? 1 : 0;
+    choose_kernel(o);          // the resident family's grid depends on the instantiation's occupancy
     return LSM_OK;
 }
 
@@ -359,7 +400,8 @@ extern "C" int lsm_set_kernel(lsm_t *o, int family)
 {
     if (!o || family < LSM_KERNEL_AUTO || family > LSM_KERNEL_RESIDENT) return LSM_ERR_ARG;
     if (family == LSM_KERNEL_TILED && !tiled_supported(o->lat, o->model, o->tiled)) return LSM_ERR_UNSUPPORTED;
-    if (family == LSM_KERNEL_RESIDENT) return LSM_ERR_UNSUPPORTED;
+    if (family == LSM_KERNEL_RESIDENT && !resident_plan(o->lat, o->model, o->tracking, o->tiled, &o->plan))
+        return LSM_ERR_UNSUPPORTED;
     o->kernel_pref = family;
     choose_kernel(o);
     return LSM_OK;

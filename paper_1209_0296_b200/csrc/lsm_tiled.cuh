@@ -24,4 +24,13 @@ void build_tiled_tables(int model, int dims, double J, double h, const uint64_t 
 bool tiled_supported(const Lat &lat, int model, const TiledTables &t);
 cudaError_t launch_sweep_tiled(const SweepArgs &a, const TiledTables &t, cudaStream_t s);
 
+// Resident family (lsm_resident.cu): one cooperative launch runs `nsweeps` whole sweeps; CTAs
+// synchronise with the owners of the adjacent slabs only.  plan.grid CTAs must be co-resident.
+struct ResidentPlan { int S, nb, bs, grid; };   // march segments, CTAs per segment, threads per CTA
+constexpr int RESIDENT_MAX_CTAS = 2048;              // flag words reserved in the workspace
+bool resident_plan(const Lat &lat, int model, int track, const TiledTables &t, ResidentPlan *out);
+cudaError_t launch_sweep_resident(const Lat &lat, int model, int track, unsigned long long seed, unsigned long long t0,
+                                  int nsweeps, long long *d_obs, unsigned *d_flags, unsigned epoch0,
+                                  const ResidentPlan &plan, const TiledTables &t, cudaStream_t s);
+
 }  // namespace lsmk

@@ -71,8 +71,16 @@ SHAPES = [
     (dict(dims=2, L=256, model=lsm.NE_HEATBATH, J=0.0, T=W.ne_temperature(0.3)), 40),
     (dict(dims=2, L=64, model=lsm.NE_METROPOLIS, J=0.0, T=W.ne_temperature(0.3)), 60),
     (dict(dims=2, L=160, model=lsm.NE_METROPOLIS, J=0.0, T=W.ne_temperature(0.2)), 30),
+    # large enough for the resident family (whole CTAs of word columns, several march segments)
+    (dict(dims=2, L=1024, T=2.269), 12),
+    (dict(dims=2, L=2048, T=2.0, h=0.02), 7),
+    (dict(dims=3, L=128, T=4.5115), 5),
+    (dict(dims=2, L=1024, two_S=2, T=1.5, h=0.01), 8),
+    (dict(dims=3, L=96, two_S=2, T=3.0, h=0.01), 6),
+    (dict(dims=2, L=1024, model=lsm.NE_HEATBATH, J=0.0, T=W.ne_temperature(0.3)), 16),
+    (dict(dims=2, L=3072, model=lsm.NE_METROPOLIS, J=0.0, T=W.ne_temperature(0.2)), 6),
 ]
-FAMILIES = [lsm.KERNEL_GENERIC, lsm.KERNEL_TILED]
+FAMILIES = [lsm.KERNEL_GENERIC, lsm.KERNEL_TILED, lsm.KERNEL_RESIDENT]
 
 
 def test_device_philox_known_answers_and_random():
@@ -115,8 +123,8 @@ def test_sweep_parity(kw, nsweeps, family):
     try:
         lat, orc = make_pair(family, seed=W.seed_of(9, nsweeps), **kw)
     except lsm.LsmError as e:
-        if e.code == lsm.ERR_UNSUPPORTED and family == lsm.KERNEL_TILED:
-            pytest.skip("tiled family does not cover this lattice (generic covers it)")
+        if e.code == lsm.ERR_UNSUPPORTED and family != lsm.KERNEL_GENERIC:
+            pytest.skip("this family does not cover this lattice (generic covers it)")
         raise
     assert lat.kernel == family
     assert_same_state(lat, orc)                      # a1: initial state from the seed
@@ -136,7 +144,12 @@ def test_sweep_parity(kw, nsweeps, family):
 def test_cfg1_full_length(family):
     """BASELINE.json config 1 at full length: 64x64, T=2.269, 1000 sweeps, (E, M) after every sweep."""
     w = W.configs()["cfg1"]
-    lat, orc = make_pair(family, **w.create_args())
+    try:
+        lat, orc = make_pair(family, **w.create_args())
+    except lsm.LsmError as e:
+        if e.code == lsm.ERR_UNSUPPORTED and family == lsm.KERNEL_RESIDENT:
+            pytest.skip("64 x 64 has fewer word columns than one CTA of the resident family")
+        raise
     got = lat.sweep_record(w.sweeps).cpu().numpy()
     want = orc.sweep_record(w.sweeps)
     assert np.array_equal(got, want)
@@ -259,17 +272,20 @@ FULL = [
 ]
 
 
+@pytest.mark.parametrize("family", [lsm.KERNEL_AUTO, lsm.KERNEL_RESIDENT])
 @pytest.mark.parametrize("name,k_first,t_late", FULL)
-def test_full_size_prefix_and_late_spot_check(name, k_first, t_late):
+def test_full_size_prefix_and_late_spot_check(name, k_first, t_late, family):
     """BASELINE.json's full sizes in the launch configuration bench.py times (AUTO kernel family,
     tracking as bench.py sets it): the first sweeps element by element, then a one-step spot check at
     a late time -- download the GPU state at sweep t, hand it to the oracle with the same counter,
     one oracle sweep, compare with the GPU at t+1.  Valid because the random words are a pure
     function of (seed, sweep, half, site)."""
     w = W.configs()[name]
-    lat, orc = make_pair(**w.create_args())
+    lat, orc = make_pair(family, **w.create_args())
     if w.model == lsm.ISING:
         lat.set_tracking(False)      # as bench.py runs cfg1-4
+    if family != lsm.KERNEL_AUTO:
+        assert lat.kernel == family
     g0 = lat.get_spins_host()
     assert np.array_equal(g0, orc.get_spins())
     got = lat.sweep_record(k_first).cpu().numpy()
