@@ -139,7 +139,7 @@ k_sweep_resident(const __grid_constant__ ResidentArgs a, const __grid_constant__
         M.s_t = s_t;
         M.one = (uint32_t)a.g.one;
         M.s_e = sm.e;
-        M.totU = M.totN = M.totBN = 0;
+        M.totU = M.totBN = 0;
         const int n = march_init(M, a.g, a.col[half], a.col[half ^ 1], half, seg, col, up);
         // The direction is a compile-time constant only where the rule needs it (North-East: north = y + 1).
         if (NE && !up) {
@@ -160,9 +160,8 @@ k_sweep_resident(const __grid_constant__ ResidentArgs a, const __grid_constant__
 
         if (OBS >= 1) {
             long long cB, cM;
-            march_observables<MODEL, DIMS>(M, 16 * n, cB, cM);
-            // the bond sum is complete after the second colour (every bond joins the two colours)
-            block_accumulate2_in(sm.red, cB, cM, a.obs + 2 * (gh >> 1), half == 1, true);
+            march_observables<MODEL, DIMS>(M, 16 * n, half == 1, cB, cM);
+            block_accumulate2_in(sm.red, cB, cM, a.obs + 2 * (gh >> 1), true, true);
         }
         // publish: every thread's stores -> CTA barrier -> fence -> flag
         __syncthreads();

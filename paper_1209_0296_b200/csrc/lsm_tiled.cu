@@ -47,6 +47,11 @@ k_sweep_tiled(const __grid_constant__ TiledGeom g, const __grid_constant__ Philo
         long long red[2][8];
         uint2 e[MODEL == M_ISING_ONE ? 96 : 1];
     } sm;
+    // Programmatic dependent launch: the next half-sweep's CTAs may be scheduled as soon as SM resources
+    // free up; they run their prologue (table, geometry) and then wait below until this grid has
+    // completed and flushed -- the kernel boundary stays the barrier of PAPER.md:96,108, only the
+    // launch latency and ramp are taken off the critical path.
+    asm volatile("griddepcontrol.launch_dependents;" ::: "memory");
     uint32_t s_t = (uint32_t)__cvta_generic_to_shared(sm.t);
     asm volatile("" : "+r"(s_t));   // keep the (warp-uniform) table address out of the divergent region below
     March<MODEL, DIMS, TRACK, OBS> M;
@@ -61,10 +66,11 @@ k_sweep_tiled(const __grid_constant__ TiledGeom g, const __grid_constant__ Philo
         M.ne_always = tab.always;
     }
     __syncthreads();
+    asm volatile("griddepcontrol.wait;" ::: "memory");   // the previous launch's spins are visible from here on
     M.s_t = s_t;
     M.one = (uint32_t)g.one;
     M.s_e = sm.e;
-    M.totU = M.totN = M.totBN = 0;
+    M.totU = M.totBN = 0;
 
     const long long gt = (long long)blockIdx.x * blockDim.x + threadIdx.x;
     int nsites = 0;
@@ -83,8 +89,8 @@ k_sweep_tiled(const __grid_constant__ TiledGeom g, const __grid_constant__ Philo
 
     if (OBS >= 1) {
         long long cB, cM;
-        march_observables<MODEL, DIMS>(M, nsites, cB, cM);
-        block_accumulate2_in(sm.red, cB, cM, g.obs, OBS >= 2, true);
+        march_observables<MODEL, DIMS>(M, nsites, OBS >= 2, cB, cM);   // OBS = 1: first colour, 2: second colour
+        block_accumulate2_in(sm.red, cB, cM, g.obs, true, true);
     }
 }
 
@@ -144,15 +150,25 @@ static int env_int(const char *name, int dflt)
 }
 static int g_tiled_ctas_per_sm = env_int("LSM_TILED_CTAS_PER_SM", 4);
 static int g_tiled_waves_x4 = env_int("LSM_TILED_WAVES_X4", 4);   // waves in quarters
+static int g_tiled_pdl = env_int("LSM_TILED_PDL", 1);               // programmatic dependent launch
 
 template <int MODEL, int DIMS, bool TRACK>
 static cudaError_t launch_obs(int obs_mode, dim3 grid, cudaStream_t s, const TiledGeom &g, const PhiloxSweepConsts &pc,
                               const typename TabOf<MODEL>::type &tab)
 {
-    if (obs_mode == 0) k_sweep_tiled<MODEL, DIMS, TRACK, 0><<<grid, 256, 0, s>>>(g, pc, tab);
-    else if (obs_mode == 1) k_sweep_tiled<MODEL, DIMS, TRACK, 1><<<grid, 256, 0, s>>>(g, pc, tab);
-    else k_sweep_tiled<MODEL, DIMS, TRACK, 2><<<grid, 256, 0, s>>>(g, pc, tab);
-    return cudaGetLastError();
+    cudaLaunchConfig_t cfg;
+    memset(&cfg, 0, sizeof(cfg));
+    cfg.gridDim = grid;
+    cfg.blockDim = dim3(256);
+    cfg.stream = s;
+    cudaLaunchAttribute at[1];
+    at[0].id = cudaLaunchAttributeProgrammaticStreamSerialization;
+    at[0].val.programmaticStreamSerializationAllowed = g_tiled_pdl ? 1 : 0;
+    cfg.attrs = at;
+    cfg.numAttrs = 1;
+    if (obs_mode == 0) return cudaLaunchKernelEx(&cfg, k_sweep_tiled<MODEL, DIMS, TRACK, 0>, g, pc, tab);
+    if (obs_mode == 1) return cudaLaunchKernelEx(&cfg, k_sweep_tiled<MODEL, DIMS, TRACK, 1>, g, pc, tab);
+    return cudaLaunchKernelEx(&cfg, k_sweep_tiled<MODEL, DIMS, TRACK, 2>, g, pc, tab);
 }
 
 template <int MODEL, int DIMS>

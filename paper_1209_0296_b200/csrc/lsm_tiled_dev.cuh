@@ -141,9 +141,11 @@ __device__ __forceinline__ uint32_t add_if_le(uint32_t t, uint32_t w, uint32_t t
     return t;
 }
 
+// Observables (a6) cost no ALU-pipe instruction: the up-count and the sum of b'*n are IDP.4A dot products
+// (FMA-heavy pipe) straight into the thread's 32-bit totals.
 template <bool TRACK, int OBS>
 __device__ __forceinline__ uint32_t rule_half(uint32_t own, uint32_t nsum, uint4 r, uint32_t s_t, uint32_t one,
-                                              uint32_t &accU, uint32_t &accN, uint32_t &accBN)
+                                              int &totU, int &totBN)
 {
     const uint32_t b = TRACK ? (own & 0x01010101u) : own;
     const uint32_t n = TRACK ? (nsum & 0x07070707u) : nsum;
@@ -154,11 +156,8 @@ __device__ __forceinline__ uint32_t rule_half(uint32_t own, uint32_t nsum, uint4
     t = add_if_le<0x00010000u>(t, r.z, lds_u32(s_t, __byte_perm(adr, 0u, 0x4442)), one);
     t = add_if_le<0x01000000u>(t, r.w, lds_u32(s_t, adr >> 24), one);
     const uint32_t b2 = t & 0x01010101u;                   // b xor flip
-    if (OBS >= 1) accU += b2;
-    if (OBS >= 2) {
-        accN += n;
-        accBN += n & (b2 * 0xFFu);
-    }
+    if (OBS >= 1) totU = (int)__dp4a(b2, 0x01010101u, (uint32_t)totU);
+    if (OBS >= 2) totBN = (int)__dp4a(n, b2, (uint32_t)totBN);
     if (!TRACK) return b2;
     const uint32_t fl = b ^ b2;
     return (own ^ fl) | (fl << 3);                         // value bit, and "ever changed" (0x08) set on a flip
@@ -228,7 +227,7 @@ struct March {
     int m, q;
     int e_hi, e_lo, dyp, dyn, rowstride, m_wrap, mstep;
     long long wrapw;
-    int totU, totN, totBN;  // per-thread sums; < 2^31 for every legal lattice
+    int totU, totBN;        // per-thread sums; < 2^31 for every legal lattice
     uint32_t s_t, one;
     const uint2 *s_e;
     uint32_t ne_t32;
@@ -277,16 +276,13 @@ struct March {
         uint32_t out[4];
 
         if (MODEL == M_ISING_HALF) {
-            uint32_t accU = 0, accN = 0, accBN = 0;
 #pragma unroll
             for (int d = 0; d < 4; ++d) {
                 uint32_t ns = p[d] + n[d] + c[d] + sd[d];
                 if (DIMS == 3) ns += yp[d] + yn[d];
                 uint4 r = philox_sweep(grp + d, pc);
-                out[d] = rule_half<TRACK, OBS>(o[d], ns, r, s_t, one, accU, accN, accBN);
+                out[d] = rule_half<TRACK, OBS>(o[d], ns, r, s_t, one, totU, totBN);
             }
-            if (OBS >= 1) totU += bytesum(accU);
-            if (OBS >= 2) { totN += bytesum(accN); totBN += bytesum(accBN); }
         } else if (MODEL == M_ISING_ONE) {
             int accB = 0, accM = 0;
 #pragma unroll
@@ -417,20 +413,25 @@ __device__ __forceinline__ int march_init(March<MODEL, DIMS, TRACK, OBS> &M, con
     return m1 - m0;
 }
 
-// Per-thread sums -> the thread's contribution to (B, M) of SURVEY.md 8(a) a6.
+// Per-thread sums -> the thread's contribution to (B, M) of SURVEY.md 8(a) a6.  `second` = this half-sweep
+// updated the second colour of its sweep.
+// Spin-1/2: s = 2b-1, nn = 2n-2d (n = up neighbours), and every bond joins the two colours, so
+//   B = sum_{i in colour 1} s'_i nn_i = 4 sum b'n - 2 sum n - 4d U1 + dN   with   sum_{colour 1} n = 2d U0
+// (each up site of colour 0 is a neighbour of 2d colour-1 sites).  Hence the first colour contributes
+// -4d U0 and the second 4 sum b'n - 4d U1 + 2d nsites; no separate sum of n is needed.
 template <int MODEL, int DIMS, bool TRACK, int OBS>
-__device__ __forceinline__ void march_observables(const March<MODEL, DIMS, TRACK, OBS> &M, int nsites, long long &cB,
-                                                  long long &cM)
+__device__ __forceinline__ void march_observables(const March<MODEL, DIMS, TRACK, OBS> &M, int nsites, bool second,
+                                                  long long &cB, long long &cM)
 {
     cB = 0;
     cM = 0;
     if (MODEL == M_ISING_HALF) {
-        // sum of s' = 2b'-1 ; sum of s'*nn = sum (2b'-1)(2n-2d)
         cM = 2LL * M.totU - nsites;
-        cB = 4LL * M.totBN - 2LL * M.totN - 4LL * DIMS * M.totU + 2LL * DIMS * nsites;
+        cB = -4LL * DIMS * M.totU;
+        if (second) cB += 4LL * M.totBN + 2LL * DIMS * nsites;
     } else if (MODEL == M_ISING_ONE) {
         cM = M.totU;
-        cB = M.totBN;
+        if (second) cB = M.totBN;
     } else {
         cM = M.totU;
     }
