@@ -30,6 +30,9 @@ BYTES_PER_UPDATE = 3  # read own colour, read other colour, write own colour (in
 # 1/4 Philox4x32-10 call = 5 wide multiplies + 5 three-input XORs, + 1 compare + 1 merge
 INT_SLOTS_PER_UPDATE = 12
 INT_SLOTS_PER_UPDATE_SPIN1 = 22
+# dram__bytes_read.sum + dram__bytes_write.sum per half-sweep launch of the cfg2 workload, from the one
+# `ncu --set full` capture summarised in profiles/r1_tiled_ncu_full.md (caches flushed by ncu before the launch)
+NCU_DRAM_BYTES_PER_LAUNCH = {"cfg2_T2.269": 67.18e6 + 0.83e6}
 
 
 def parse():
@@ -270,9 +273,12 @@ def run_ours(args, w):
     alu_peak = sm_count * 64 * sm_max_mhz * 1e6 / 1e9           # G integer instruction slots / s
     alu_achieved = slots * updates_per_launch / avg_launch_s / 1e9
     roofline = {"bound": "alu", "achieved": alu_achieved, "peak": alu_peak, "unit": "Gslot/s",
-                "frac": alu_achieved / alu_peak, "traffic": None,
+                "frac": alu_achieved / alu_peak,
+                "traffic": NCU_DRAM_BYTES_PER_LAUNCH.get(wl.name) if lat.kernel == 2 else None,
+                "traffic_unit": "bytes per launch (ncu dram read+write, cold L2; algorithmic = 3 B x updates_per_launch)",
                 "peak_source": f"{sm_count} SMs x 64 integer lanes/clk x clocks.max.sm {sm_max_mhz} MHz (DESIGN.md 6; pipe_probe)",
-                "kernel": "k_sweep_tiled (half-sweep)" if lat.kernel == 2 else "k_sweep_generic (half-sweep)",
+                "kernel": {2: "k_sweep_tiled (half-sweep)", 3: "k_sweep_resident (per half-sweep share of one launch)"}.get(
+                    lat.kernel, "k_sweep_generic (half-sweep)"),
                 "algorithmic_int_slots_per_update": slots, "updates_per_launch": updates_per_launch,
                 "avg_launch_us": avg_launch_s * 1e6}
     hbm_achieved = BYTES_PER_UPDATE * updates_per_launch / avg_launch_s / 1e9
@@ -304,7 +310,7 @@ def run_ours(args, w):
         line["other_workloads"] = other_workloads(lsm, torch, w.name)
         from paper_1209_0296_b200 import workloads as W
 
-        sweeps = 2
+        sweeps = 4
         v, dt, n = time_oracle(w, w.L, sweeps)
         line["cpu_baseline"] = {"value": v / 1e9, "unit": "Gflips/s", "cores": 1, "kind": "oracle",
                                 "sample": f"{sweeps} sweeps of the full {w.L}^{w.dims} lattice ({n} updates, {dt:.1f} s), single thread of {os.cpu_count()}"}
