@@ -487,7 +487,7 @@ extern "C" int lsm_philox_throughput(int blocks, int calls, uint32_t *d_sink, vo
 
 extern "C" int lsm_pipe_probe(int mode, int blocks, int iters, uint32_t *d_sink, void *stream)
 {
-    if (mode < 0 || mode > 7 || blocks <= 0 || iters < 0 || !d_sink) return LSM_ERR_ARG;
+    if (mode < 0 || mode > 10 || blocks <= 0 || iters < 0 || !d_sink) return LSM_ERR_ARG;
     CU(launch_pipe_probe(mode, blocks, iters, d_sink, (cudaStream_t)stream));
     return LSM_OK;
 }

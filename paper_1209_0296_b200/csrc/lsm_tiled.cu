@@ -38,7 +38,7 @@ PhiloxSweepConsts make_philox_consts(const SweepKey &k)
 }
 
 template <int MODEL, int DIMS, bool TRACK, int OBS>
-__global__ void __launch_bounds__(256, LSM_TILED_MINBLOCKS)
+__global__ void __launch_bounds__(256, MODEL == M_ISING_ONE ? LSM_TILED_MINBLOCKS_ONE : LSM_TILED_MINBLOCKS)
 k_sweep_tiled(const __grid_constant__ TiledGeom g, const __grid_constant__ PhiloxSweepConsts pc,
               const __grid_constant__ typename TabOf<MODEL>::type tab)
 {
@@ -47,6 +47,11 @@ k_sweep_tiled(const __grid_constant__ TiledGeom g, const __grid_constant__ Philo
         long long red[2][8];
         uint2 e[MODEL == M_ISING_ONE ? 96 : 1];
     } sm;
+    // two-stage per-thread ring of the asynchronous copies (March::step_pf): N, O [, Yp, Yn] words and the edge lane
+    // (spin-1 keeps the direct loads: its rule needs the registers the copies' addresses would take)
+    constexpr bool PF = LSM_TILED_PF_ONE || MODEL != M_ISING_ONE;
+    __shared__ __align__(16) uint4 ring[PF ? (DIMS == 3 ? 8 : 4) * 256 : 1];
+    __shared__ uint32_t ringE[PF ? 2 * 256 : 1];
     // Programmatic dependent launch: the next half-sweep's CTAs may be scheduled as soon as SM resources
     // free up; they run their prologue (table, geometry) and then wait below until this grid has
     // completed and flushed -- the kernel boundary stays the barrier of PAPER.md:96,108, only the
@@ -71,6 +76,8 @@ k_sweep_tiled(const __grid_constant__ TiledGeom g, const __grid_constant__ Philo
     M.one = (uint32_t)g.one;
     M.s_e = sm.e;
     M.totU = M.totBN = 0;
+    M.s_ring = (uint32_t)__cvta_generic_to_shared(ring) + threadIdx.x * 16u;
+    M.s_ringE = (uint32_t)__cvta_generic_to_shared(ringE) + threadIdx.x * 4u;
 
     const long long gt = (long long)blockIdx.x * blockDim.x + threadIdx.x;
     int nsites = 0;
@@ -80,10 +87,10 @@ k_sweep_tiled(const __grid_constant__ TiledGeom g, const __grid_constant__ Philo
         const int n = march_init(M, g, g.own, g.oth, g.half, seg, col, true);
         nsites = 16 * n;
         if (g.parity_rows) {            // warp-uniform branch: q is a constant inside each loop
-            if (M.q) M.template run<1, true>(n, pc);
-            else M.template run<0, true>(n, pc);
+            if (M.q) PF ? M.template run_pf<1, true>(n, pc) : M.template run<1, true>(n, pc);
+            else PF ? M.template run_pf<0, true>(n, pc) : M.template run<0, true>(n, pc);
         } else {
-            M.template run<2, true>(n, pc);
+            PF ? M.template run_pf<2, true>(n, pc) : M.template run<2, true>(n, pc);
         }
     }
 
@@ -149,6 +156,7 @@ static int env_int(const char *name, int dflt)
     return (v && *v) ? atoi(v) : dflt;
 }
 static int g_tiled_ctas_per_sm = env_int("LSM_TILED_CTAS_PER_SM", 4);
+static int g_tiled_ctas_per_sm_one = env_int("LSM_TILED_CTAS_PER_SM_ONE", LSM_TILED_MINBLOCKS_ONE);
 static int g_tiled_waves_x4 = env_int("LSM_TILED_WAVES_X4", 4);   // waves in quarters
 static int g_tiled_pdl = env_int("LSM_TILED_PDL", 1);               // programmatic dependent launch
 
@@ -196,7 +204,8 @@ cudaError_t launch_sweep_tiled(const SweepArgs &a, const TiledTables &t, cudaStr
     else if (g.wpr % 32 == 0) g.parity_rows = 1;
     else if (g.wpr < 32 && 32 % g.wpr == 0 && g.R % (2 * (32 / g.wpr)) == 0) g.parity_rows = 1;
     else g.parity_rows = 0;
-    long long target = (long long)sm_count() * g_tiled_ctas_per_sm * 256 * g_tiled_waves_x4 / 4;
+    const int per_sm = a.model == M_ISING_ONE ? g_tiled_ctas_per_sm_one : g_tiled_ctas_per_sm;
+    long long target = (long long)sm_count() * per_sm * 256 * g_tiled_waves_x4 / 4;
     long long S = target / g.ncol;
     if (S < 1) S = 1;
     if (S > g.L) S = g.L;

@@ -8,6 +8,14 @@
 #define LSM_TILED_MINBLOCKS 4
 #endif
 
+// spin-1 needs two Philox calls and 64-bit table entries per lane: 3 CTAs per SM (85 registers) avoid its spills
+#ifndef LSM_TILED_MINBLOCKS_ONE
+#define LSM_TILED_MINBLOCKS_ONE 3
+#endif
+#ifndef LSM_TILED_PF_ONE
+#define LSM_TILED_PF_ONE 0
+#endif
+
 namespace lsmk {
 
 // ------------------------------------------------------------------------------------------
@@ -237,20 +245,13 @@ struct March {
     // half-sweeps of the resident family) or downwards (rowstride < 0): P is the row the march came
     // from, N the row it goes to; `m_wrap` is the position whose successor wraps around the lattice and
     // `wrapw` the (signed) pointer correction.  UP matters to the North-East rule only (north = y + 1).
+    // The update of one word (16 sites) at the current march position, given the other colour's word at the
+    // next row (N), the own word (O), the edge lane of the adjacent word (e) and, in 3D, the cross rows.
     template <int Q, bool UP, class PC>
-    __device__ __forceinline__ void step(const PC &pc)
+    __device__ __forceinline__ uint4 update_word(const PC &pc, const uint4 N, const uint4 O, const uint32_t e,
+                                                 const uint4 Yp, const uint4 Yn)
     {
         const int qq = Q == 2 ? q : Q;
-        const uint4 *pN = pC + rowstride;
-        if (m == m_wrap) pN -= wrapw;
-        const uint4 N = *pN;
-        const uint4 O = *pO;
-        const uint32_t e = pE[qq ? e_hi : e_lo];
-        uint4 Yp, Yn;
-        if (DIMS == 3) {
-            Yp = pC[dyp];
-            Yn = pC[dyn];
-        }
         // the neighbour one byte to the right (q = 1) or left (q = 0) of every site of the word
         uint32_t sd[4];
         if (qq) {
@@ -312,7 +313,28 @@ struct March {
             }
             if (OBS >= 1) totU += bytesum(accU);
         }
-        *pO = make_uint4(out[0], out[1], out[2], out[3]);
+        return make_uint4(out[0], out[1], out[2], out[3]);
+    }
+
+    // One step at march position m.  The march runs upwards (rowstride > 0, the tiled family and the even
+    // half-sweeps of the resident family) or downwards (rowstride < 0): P is the row the march came
+    // from, N the row it goes to; `m_wrap` is the position whose successor wraps around the lattice and
+    // `wrapw` the (signed) pointer correction.  UP matters to the North-East rule only (north = y + 1).
+    template <int Q, bool UP, class PC>
+    __device__ __forceinline__ void step(const PC &pc)
+    {
+        const int qq = Q == 2 ? q : Q;
+        const uint4 *pN = pC + rowstride;
+        if (m == m_wrap) pN -= wrapw;
+        const uint4 N = *pN;
+        const uint4 O = *pO;
+        const uint32_t e = pE[qq ? e_hi : e_lo];
+        uint4 Yp = make_uint4(0, 0, 0, 0), Yn = Yp;
+        if (DIMS == 3) {
+            Yp = pC[dyp];
+            Yn = pC[dyn];
+        }
+        *pO = update_word<Q, UP>(pc, N, O, e, Yp, Yn);
         P = C;
         C = N;
         pC += rowstride;
@@ -321,6 +343,120 @@ struct March {
         grp += (uint32_t)rowstride * 4u;
         m += mstep;
         if (Q == 2) q ^= 1;
+    }
+
+    // ---- asynchronous-copy variant of the step (tiled family) --------------------------------------
+    // The words a step needs from global memory (N, O, e and the 3D cross rows) are copied one step ahead
+    // into a two-stage, per-thread shared-memory ring with cp.async: the copy costs no registers and its
+    // L2/HBM latency is hidden behind a whole step of arithmetic.  A thread reads back only what it copied
+    // itself, so cp.async.wait_group is the only synchronisation.  Addresses are 32-bit word offsets
+    // into the colour arrays (one IMAD.WIDE per address) instead of 64-bit pointer arithmetic.
+    const uint8_t *b_oth;   // array bases
+    uint8_t *b_own;
+    uint32_t offN;          // word offset of the other colour's row the NEXT step will use as N... see step_pf
+    uint32_t offS;          // word offset of the own word of the current step
+    uint32_t nw32;          // words per colour array
+    int rs32, wrapfix;      // signed words per march step; correction applied when offN leaves [0, nw32)
+    int ed_hi, ed_lo;       // byte offset from the other colour's word of this thread to the edge lane (q = 1 / 0)
+    int dypb, dynb;         // byte offsets to the cross-row words (3D)
+    uint32_t s_ring;        // shared address of this thread's slot in stage 0 of the N ring
+    uint32_t s_ringE;       // ... of the e ring
+
+    static constexpr uint32_t RING_STAGE = 256u * 16u;              // bytes per stage of a 16-byte ring
+    static constexpr uint32_t RING_O = 2u * RING_STAGE;             // own-colour ring behind the N ring
+    static constexpr uint32_t RING_YP = 4u * RING_STAGE, RING_YN = 6u * RING_STAGE;
+    static constexpr uint32_t RINGE_STAGE = 256u * 4u;
+
+    __device__ __forceinline__ static void cp16(uint32_t dst, const void *src)
+    {
+        asm volatile("cp.async.ca.shared.global [%0], [%1], 16;" ::"r"(dst), "l"(src) : "memory");
+    }
+    __device__ __forceinline__ static void cp4(uint32_t dst, const void *src)
+    {
+        asm volatile("cp.async.ca.shared.global [%0], [%1], 4;" ::"r"(dst), "l"(src) : "memory");
+    }
+    __device__ __forceinline__ static uint4 lds128(uint32_t a)
+    {
+        uint4 v;
+        asm volatile("ld.shared.v4.u32 {%0,%1,%2,%3}, [%4];" : "=r"(v.x), "=r"(v.y), "=r"(v.z), "=r"(v.w) : "r"(a) : "memory");
+        return v;
+    }
+    __device__ __forceinline__ static uint32_t lds32v(uint32_t a)
+    {
+        uint32_t v;
+        asm volatile("ld.shared.u32 %0, [%1];" : "=r"(v) : "r"(a) : "memory");
+        return v;
+    }
+
+    // Copies for the step whose current row is at word offset `cur` (own word, edge lane, cross rows) and whose
+    // next row is at `nxt`, into ring stage ST; QN = row parity of that step.
+    template <int QN, int ST>
+    __device__ __forceinline__ void prefetch(uint32_t cur, uint32_t nxt)
+    {
+        const uint8_t *aC = b_oth + (size_t)cur * 16u;
+        cp16(s_ring + ST * RING_STAGE, b_oth + (size_t)nxt * 16u);
+        cp16(s_ring + RING_O + ST * RING_STAGE, b_own + (size_t)cur * 16u);
+        const int qn = QN == 2 ? (q ^ 1) : QN;
+        cp4(s_ringE + ST * RINGE_STAGE, aC + (qn ? ed_hi : ed_lo));
+        if (DIMS == 3) {
+            cp16(s_ring + RING_YP + ST * RING_STAGE, aC + dypb);
+            cp16(s_ring + RING_YN + ST * RING_STAGE, aC + dynb);
+        }
+        asm volatile("cp.async.commit_group;" ::: "memory");
+    }
+
+    __device__ __forceinline__ uint32_t advance(uint32_t off) const
+    {
+        off += (uint32_t)rs32;
+        if (off >= nw32) off += (uint32_t)wrapfix;    // unsigned compare: catches both directions
+        return off;
+    }
+
+    // Step with ring stage ST holding this step's words; issues the copies of the next step into ST ^ 1.
+    template <int Q, int ST, bool UP, class PC>
+    __device__ __forceinline__ void step_pf(const PC &pc)
+    {
+        constexpr int QN = Q == 2 ? 2 : 1 - Q;
+        const uint32_t cur = offN;                    // next step's current row = this step's N row
+        offN = advance(cur);
+        prefetch<QN, ST ^ 1>(cur, offN);
+        asm volatile("cp.async.wait_group 1;" ::: "memory");
+        const uint4 N = lds128(s_ring + ST * RING_STAGE);
+        const uint4 O = lds128(s_ring + RING_O + ST * RING_STAGE);
+        const uint32_t e = lds32v(s_ringE + ST * RINGE_STAGE);
+        uint4 Yp = make_uint4(0, 0, 0, 0), Yn = Yp;
+        if (DIMS == 3) {
+            Yp = lds128(s_ring + RING_YP + ST * RING_STAGE);
+            Yn = lds128(s_ring + RING_YN + ST * RING_STAGE);
+        }
+        const uint4 out = update_word<Q, UP>(pc, N, O, e, Yp, Yn);
+        *reinterpret_cast<uint4 *>(b_own + (size_t)offS * 16u) = out;
+        P = C;
+        C = N;
+        offS += (uint32_t)rs32;
+        grp += (uint32_t)rs32 * 4u;
+        if (Q == 2) q ^= 1;
+    }
+
+    template <int Q0, bool UP, class PC>
+    __device__ __forceinline__ void run_pf(int n, const PC &pc)
+    {
+        constexpr int Q1 = Q0 == 2 ? 2 : 1 - Q0;
+        // copies of the first step into stage 0
+        {
+            const uint32_t cur = offS;
+            offN = advance(cur);
+            if (Q0 == 2) q ^= 1;                      // prefetch<> takes the parity of the step AFTER q's
+            prefetch<Q0, 0>(cur, offN);
+            if (Q0 == 2) q ^= 1;
+        }
+        int k = 0;
+        for (; k + 1 < n; k += 2) {
+            step_pf<Q0, 0, UP>(pc);
+            step_pf<Q1, 1, UP>(pc);
+        }
+        if (k < n) step_pf<Q0, 0, UP>(pc);
+        asm volatile("cp.async.wait_group 0;" ::: "memory");
     }
 
     // n steps from the current position, 2x unrolled so that the row parity is a compile-time constant.
@@ -403,6 +539,17 @@ __device__ __forceinline__ int march_init(March<MODEL, DIMS, TRACK, OBS> &M, con
     M.pO = reinterpret_cast<uint4 *>(own) + w0;
     M.pE = reinterpret_cast<const uint32_t *>(oth) + ((long long)ms * rs + y * g.wpr) * 4;
     M.grp = (uint32_t)w0 * 4u;
+    M.b_oth = oth;
+    M.b_own = own;
+    M.offS = (uint32_t)w0;
+    M.offN = (uint32_t)w0;
+    M.nw32 = (uint32_t)nw;
+    M.rs32 = M.rowstride;
+    M.wrapfix = up ? -(int)nw : (int)nw;
+    M.ed_hi = (M.e_hi - j * 4) * 4;
+    M.ed_lo = (M.e_lo - j * 4) * 4;
+    M.dypb = M.dyp * 16;
+    M.dynb = M.dyn * 16;
     M.m = ms;
     M.q = (ms + y + half) & 1;
     // the row the march comes from

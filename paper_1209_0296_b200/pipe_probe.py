@@ -18,6 +18,9 @@ MODES = [
     (5, "4 Philox calls + 80 LOP3", 80, 0, 160),
     (6, "4 Philox calls + 160 LOP3", 80, 0, 240),
     (7, "4 Philox calls + 240 LOP3", 80, 0, 320),
+    (8, "4 Philox calls + 80 IMAD", 80, 80, 80),
+    (9, "4 Philox calls + 80 IMAD + 80 LOP3", 80, 80, 160),
+    (10, "4 Philox calls + 80 IMAD + 160 LOP3", 80, 80, 240),
 ]
 
 
