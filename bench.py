@@ -187,7 +187,9 @@ def run_ours(args, w):
     K, Wm = args.steps, max(args.warmup, 3)
     from dataclasses import replace
 
-    wl = replace(w, seed=w.seed + 1000 * rank)  # replicas: independent seeds, no communication
+    from paper_1209_0296_b200 import replicas
+
+    wl = replace(w, seed=replicas.rank_seed(w.seed, rank))  # replicas: independent seeds, no communication
     lat = lsm.Lattice(**wl.create_args(), device=f"cuda:{local}")
     if wl.model == lsm.ISING:
         lat.set_tracking(False)  # persistence is not part of configs 1-4
@@ -221,12 +223,8 @@ def run_ours(args, w):
     launches = lat.launch_count - launches0
     step_ms = [a.elapsed_time(b) for a, b in ev]
     total_ms = sum(step_ms)
-    t = torch.tensor([total_ms], dtype=torch.float64, device=lat.device)
-    if world > 1:
-        dist.all_reduce(t, op=dist.ReduceOp.MAX)
-    total_ms_max = float(t.item())
-    updates_all = float(N) * S * K * world
-    value = updates_all / (total_ms_max * 1e-3) / 1e9
+    total_ms_max, updates_all, ups = replicas.aggregate(total_ms, N * S * K, lat.device)
+    value = ups / 1e9
 
     # sanity of the state after the timed region: fused running sums == full reduction (a6 vs a8)
     Bv, Mv, tdone = lat.measure_int()
@@ -250,10 +248,7 @@ def run_ours(args, w):
     e1.record()
     torch.cuda.synchronize()
     e2e_ms = e0.elapsed_time(e1)
-    t = torch.tensor([e2e_ms], dtype=torch.float64, device=lat.device)
-    if world > 1:
-        dist.all_reduce(t, op=dist.ReduceOp.MAX)
-    e2e_value = float(N) * S * Ke * world / (float(t.item()) * 1e-3) / 1e9
+    e2e_value = replicas.aggregate(e2e_ms, N * S * Ke, lat.device)[2] / 1e9
 
     if rank != 0:
         if world > 1:
