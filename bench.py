@@ -44,6 +44,8 @@ def parse():
     ap.add_argument("--workload", default="cfg2_T2.269")
     ap.add_argument("--sweeps-per-step", type=int, default=SWEEPS_PER_STEP)
     ap.add_argument("--no-extras", action="store_true", help="skip the secondary workloads / cpu baseline")
+    ap.add_argument("--size-scan", action="store_true",
+                    help="instead of the benchmark: us/sweep of the tiled and the small (cluster) family over lattice sizes")
     ap.add_argument("--kernel", default="auto", choices=["auto", "generic", "tiled", "resident"],
                     help="kernel family (lsm_set_kernel); auto = the library's choice")
     return ap.parse_args()
@@ -371,8 +373,49 @@ def other_workloads(lsm, torch, skip):
     return out
 
 
+def size_scan():
+    """us per sweep (per-sweep (B, M) recorded) of the tiled and the small family from 32^2 to 1024^2 and 16^3 to 64^3:
+    where one launch per half-sweep stops paying (the paper's own lattice sizes)."""
+    import torch
+
+    from paper_1209_0296_b200 import build, lsm
+
+    build.build()
+    rows = []
+    for dims, L in [(2, 32), (2, 64), (2, 128), (2, 256), (2, 512), (2, 1024), (3, 16), (3, 32), (3, 64)]:
+        row = {"dims": dims, "L": L}
+        for fam, name in ((lsm.KERNEL_TILED, "tiled"), (lsm.KERNEL_SMALL, "small")):
+            lat = lsm.Lattice(dims=dims, L=L, T=2.269 if dims == 2 else 4.5115, seed=3)
+            lat.set_tracking(False)
+            try:
+                lat.set_kernel(fam)
+            except lsm.LsmError:
+                row[name] = None
+                continue
+            n = 500
+            obs = torch.empty((n, 2), dtype=torch.int64, device="cuda")
+            lat.sweep_record(n, out=obs)
+            torch.cuda.synchronize()
+            e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+            e0.record()
+            lat.sweep_record(n, out=obs)
+            e1.record()
+            torch.cuda.synchronize()
+            ms = e0.elapsed_time(e1)
+            row[name] = {"us_per_sweep": ms * 1e3 / n, "gflips": lat.N * n / ms / 1e6}
+            lat.close()
+        lat = lsm.Lattice(dims=dims, L=L, T=2.269 if dims == 2 else 4.5115, seed=3)
+        row["auto_family"] = {1: "generic", 2: "tiled", 3: "resident", 4: "small"}.get(lat.kernel)
+        lat.close()
+        rows.append(row)
+        print(json.dumps(row), flush=True)
+    return 0
+
+
 def main():
     args = parse()
+    if args.size_scan:
+        return size_scan()
     from paper_1209_0296_b200 import workloads as W
 
     w = W.configs()[args.workload]

@@ -72,7 +72,7 @@ enum {
     LSM_ERR_STATE = -5        /* call needs tracking to be on (lsm_persistence)                */
 };
 /* Kernel families (lsm_set_kernel).  AUTO picks the fastest one that supports the lattice. */
-enum { LSM_KERNEL_AUTO = 0, LSM_KERNEL_GENERIC = 1, LSM_KERNEL_TILED = 2, LSM_KERNEL_RESIDENT = 3 };
+enum { LSM_KERNEL_AUTO = 0, LSM_KERNEL_GENERIC = 1, LSM_KERNEL_TILED = 2, LSM_KERNEL_RESIDENT = 3, LSM_KERNEL_SMALL = 4 };
 
 /* Device bytes lsm_create needs for this lattice (two colour arrays + small state). */
 int lsm_workspace_bytes(int dims, int L, int two_S, int model, size_t *bytes);

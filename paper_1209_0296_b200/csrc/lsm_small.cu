@@ -1,0 +1,414 @@
+// lsm_small.cu -- the single-CTA kernel family for small lattices: ONE launch runs many sweeps.
+//
+// The paper reports that small lattices cannot hide the cost of a kernel launch per half-sweep
+// (2x at 32^2 against 150x at 512^2), and it ends the kernel only because its GPUs had
+// no other barrier between the two colours.  A lattice of a few thousand sites is
+// work for one SM: here one thread block owns the whole lattice, its threads take one word column
+// and a short march segment each (the thread -> site map and the arithmetic are the tiled family's
+// March, unchanged, so results are bit-identical), and the barrier between half-sweeps is
+// __syncthreads().  The colour arrays stay in global memory; after the first touch every access is
+// an L1 hit on the block's SM (bar.sync orders the block's global writes before its later reads).
+// Per-sweep (B, M): per-thread sums -> warp shuffle -> shared-memory atomics -> one 16-byte store.
+#include "lsm_tiled_dev.cuh"
+
+#include <cooperative_groups.h>
+#include <cstdlib>
+#include <cstring>
+
+namespace lsmk {
+
+struct SmallArgs {
+    uint8_t *col[2];
+    TiledGeom g;                 // own/oth/half/obs are set per half-sweep on the device
+    unsigned long long seed, t0; // first sweep of this launch
+    int nsweeps;
+    long long *obs;              // [nsweeps][2] (B, M), or nullptr
+};
+
+template <int MODEL, int DIMS, bool TRACK, int OBS>
+__global__ void __launch_bounds__(1024, 1)
+k_sweep_small(const __grid_constant__ SmallArgs a, const __grid_constant__ PhiloxSweepConsts pk,
+              const __grid_constant__ typename TabOf<MODEL>::type tab)
+{
+    __shared__ __align__(16) struct {
+        uint32_t t[16];
+        int acc[2][2];           // (B, M) of the sweep in flight, double-buffered by sweep parity
+        uint2 e[MODEL == M_ISING_ONE ? 96 : 1];
+    } sm;
+    uint32_t s_t = (uint32_t)__cvta_generic_to_shared(sm.t);
+    asm volatile("" : "+r"(s_t));
+    if constexpr (MODEL == M_ISING_HALF) {
+        if (threadIdx.x < 16) sm.t[threadIdx.x] = tab.t[threadIdx.x];
+    } else if constexpr (MODEL == M_ISING_ONE) {
+        if (threadIdx.x < 96) sm.e[threadIdx.x] = tab.e[threadIdx.x];
+    }
+    if (threadIdx.x < 4) sm.acc[threadIdx.x >> 1][threadIdx.x & 1] = 0;
+    __syncthreads();
+
+    constexpr bool NE = MODEL == M_NE_HEATBATH || MODEL == M_NE_METROPOLIS;
+    const int nthr = a.g.ncol * a.g.S;
+    const bool active = (int)threadIdx.x < nthr;
+    const int seg = active ? (int)threadIdx.x / a.g.ncol : 0;
+    const int col = active ? (int)threadIdx.x - seg * a.g.ncol : 0;
+
+    const int nhalves = 2 * a.nsweeps;
+#pragma unroll 1
+    for (int gh = 0; gh < nhalves; ++gh) {
+        const int half = gh & 1, sw = gh >> 1;
+        const unsigned long long t = a.t0 + (unsigned long long)sw;
+        PhiloxDyn pc = {0u, 0u, 0u, 0u, pk};
+        philox_half_consts(make_sweep_key(a.seed, t, (uint32_t)half), pk.rk0, pk.rk1, pc.x1, pc.y2, pc.z2, pc.w3);
+
+        March<MODEL, DIMS, TRACK, OBS> M;
+        M.ne_t32 = 0;
+        M.ne_always = 0;
+        if constexpr (NE) {
+            M.ne_t32 = tab.t32;
+            M.ne_always = tab.always;
+        }
+        M.s_t = s_t;
+        M.one = (uint32_t)a.g.one;
+        M.s_e = sm.e;
+        M.totU = M.totBN = 0;
+        int nsites = 0;
+        if (active) {
+            const int n = march_init(M, a.g, a.col[half], a.col[half ^ 1], half, seg, col, true);
+            nsites = 16 * n;
+            M.template run<2, true>(n, pc);          // a warp spans rows of both parities: q is per thread
+        }
+        if (OBS >= 1) {
+            long long cB, cM;
+            march_observables<MODEL, DIMS>(M, nsites, half == 1, cB, cM);
+            const int wB = warp_sum((int)cB), wM = warp_sum((int)cM);   // |B| <= 3N, |M| <= N: far below 2^31 here
+            if ((threadIdx.x & 31) == 0) {
+                if (wB != 0) atomicAdd(&sm.acc[sw & 1][0], wB);
+                if (wM != 0) atomicAdd(&sm.acc[sw & 1][1], wM);
+            }
+        }
+        __syncthreads();                              // the barrier between the two colours
+        if (OBS >= 1 && half == 1 && threadIdx.x == 0) {
+            // the next adds to this buffer belong to sweep sw + 2: two barriers away
+            a.obs[2 * sw] = sm.acc[sw & 1][0];
+            a.obs[2 * sw + 1] = sm.acc[sw & 1][1];
+            sm.acc[sw & 1][0] = 0;
+            sm.acc[sw & 1][1] = 0;
+        }
+    }
+}
+
+// Lane-granular cluster variant for power-of-two L.  A thread owns 32-bit lanes (4 sites, one Philox call)
+// instead of whole words, and the lattice is cut into slabs of march rows, one slab per thread block of a
+// thread-block cluster (1, 2, 4 or 8 SMs).  Each block keeps its slab of both colours in shared memory for
+// the whole launch; the rows m-1 / m+1 across a slab boundary are read from the neighbour block's shared
+// memory (distributed shared memory), and the barrier between the colours is the cluster barrier --
+// hardware-supported, far cheaper than ending the kernel.  This is the regime of the
+// paper's own lattices (32^2 ... 512^2), which a launch per half-sweep cannot serve well.
+// Same rules, same (group, word) -> site map as every other family: bit-identical.
+template <int MODEL, int DIMS, bool TRACK, int OBS>
+__global__ void __launch_bounds__(1024, 1)
+k_sweep_small_lane(const __grid_constant__ SmallArgs a, const __grid_constant__ PhiloxSweepConsts pk,
+                   const __grid_constant__ typename TabOf<MODEL>::type tab, const int lg_lpr, const int lg_L,
+                   const int lg_rpc)
+{
+    namespace cg = cooperative_groups;
+    cg::cluster_group cluster = cg::this_cluster();
+    const uint32_t rank = cluster.block_rank(), nrank = cluster.num_blocks();
+
+    __shared__ __align__(16) struct {
+        uint32_t t[16];
+        int acc[2][2];           // this block's share of (B, M) of the sweep in flight, double-buffered
+        uint2 e[MODEL == M_ISING_ONE ? 96 : 1];
+    } sm;
+    uint32_t s_t = (uint32_t)__cvta_generic_to_shared(sm.t);
+    asm volatile("" : "+r"(s_t));
+    if constexpr (MODEL == M_ISING_HALF) {
+        if (threadIdx.x < 16) sm.t[threadIdx.x] = tab.t[threadIdx.x];
+    } else if constexpr (MODEL == M_ISING_ONE) {
+        if (threadIdx.x < 96) sm.e[threadIdx.x] = tab.e[threadIdx.x];
+    }
+    if (threadIdx.x < 4) sm.acc[threadIdx.x >> 1][threadIdx.x & 1] = 0;
+
+    constexpr bool NE = MODEL == M_NE_HEATBATH || MODEL == M_NE_METROPOLIS;
+    const uint32_t lpr = 1u << lg_lpr, L = 1u << lg_L;
+    const int lg_R = DIMS == 3 ? lg_L : 0;
+    const uint32_t R = 1u << lg_R;
+    const int lg_slab = lg_rpc + lg_R + lg_lpr;               // log2(lanes per colour in one slab)
+    const uint32_t nl = 1u << lg_slab;
+    const uint32_t base = rank << lg_slab;                     // first lane of this slab in the colour array
+    const uint32_t one = (uint32_t)a.g.one;
+    uint32_t ne_t32 = 0;
+    int ne_always = 0;
+    if constexpr (NE) {
+        ne_t32 = tab.t32;
+        ne_always = tab.always;
+    }
+
+    extern __shared__ __align__(16) uint32_t s_lat[];
+    uint32_t *const s_col[2] = {s_lat, s_lat + nl};
+    for (uint32_t i = threadIdx.x; i < nl; i += blockDim.x) {
+        s_col[0][i] = reinterpret_cast<const uint32_t *>(a.col[0])[base + i];
+        s_col[1][i] = reinterpret_cast<const uint32_t *>(a.col[1])[base + i];
+    }
+    // the slabs above and below (the same shared-memory offsets in the neighbour blocks)
+    const uint32_t r_dn = (rank + nrank - 1) % nrank, r_up = (rank + 1) % nrank;
+    const uint32_t *const dn_col[2] = {cluster.map_shared_rank(s_col[0], r_dn), cluster.map_shared_rank(s_col[1], r_dn)};
+    const uint32_t *const up_col[2] = {cluster.map_shared_rank(s_col[0], r_up), cluster.map_shared_rank(s_col[1], r_up)};
+    const uint32_t rpc = 1u << lg_rpc;
+    if (nrank > 1) cluster.sync();
+    else __syncthreads();
+
+    int thrB = 0, thrM = 0;
+    const int nhalves = 2 * a.nsweeps;
+#pragma unroll 1
+    for (int gh = 0; gh < nhalves; ++gh) {
+        const int half = gh & 1, sw = gh >> 1;
+        const unsigned long long t = a.t0 + (unsigned long long)sw;
+        PhiloxDyn pc = {0u, 0u, 0u, 0u, pk};
+        philox_half_consts(make_sweep_key(a.seed, t, (uint32_t)half), pk.rk0, pk.rk1, pc.x1, pc.y2, pc.z2, pc.w3);
+        uint32_t *own = s_col[half];
+        const uint32_t *oth = s_col[half ^ 1];
+        int totU = 0, totBN = 0, nsites = 0;
+        if (half == 0) thrB = thrM = 0;
+#pragma unroll 1
+        for (uint32_t li = threadIdx.x; li < nl; li += blockDim.x) {
+            const uint32_t gl = base + li;                                    // lane index in the colour array
+            const uint32_t x = li & (lpr - 1), row = li >> lg_lpr;           // local row = ml * R + y
+            const uint32_t y = row & (R - 1), ml = row >> lg_R;
+            const uint32_t m = (rank << lg_rpc) + ml;
+            const uint32_t qq = (m + y + (uint32_t)half) & 1u;
+            const uint32_t c = oth[li];
+            const uint32_t o = own[li];
+            const uint32_t p = ml > 0 ? oth[li - (R << lg_lpr)] : dn_col[half ^ 1][li + ((rpc - 1) << (lg_R + lg_lpr))];
+            const uint32_t n = ml + 1 < rpc ? oth[li + (R << lg_lpr)] : up_col[half ^ 1][li - ((rpc - 1) << (lg_R + lg_lpr))];
+            const uint32_t cs = oth[(row << lg_lpr) + ((qq ? x + 1 : x - 1) & (lpr - 1))];
+            const uint32_t sd = qq ? __funnelshift_r(c, cs, 8) : __funnelshift_r(cs, c, 24);
+            uint32_t yp = 0, yn = 0;
+            if (DIMS == 3) {
+                yp = oth[((ml << lg_R) + ((y - 1) & (R - 1))) * lpr + x];
+                yn = oth[((ml << lg_R) + ((y + 1) & (R - 1))) * lpr + x];
+            }
+            uint32_t out;
+            if (MODEL == M_ISING_HALF) {
+                uint32_t ns = p + n + c + sd;
+                if (DIMS == 3) ns += yp + yn;
+                out = rule_half<TRACK, OBS>(o, ns, philox_sweep(gl, pc), s_t, one, totU, totBN);
+            } else if (MODEL == M_ISING_ONE) {
+                uint32_t ns;
+                if (TRACK) {
+                    ns = ((p + n) & 0x0F0F0F0Fu) + ((c + sd) & 0x0F0F0F0Fu);
+                    if (DIMS == 3) ns += (yp + yn) & 0x0F0F0F0Fu;
+                } else {
+                    ns = p + n + c + sd;
+                    if (DIMS == 3) ns += yp + yn;
+                }
+                int accB = 0, accM = 0;
+                out = rule_one<DIMS, TRACK, OBS>(o, ns, philox_sweep(2u * gl, pc), philox_sweep(2u * gl + 1u, pc), sm.e,
+                                                 accB, accM);
+                totU += accM;
+                totBN += accB;
+            } else {
+                uint32_t accU = 0;
+                out = rule_ne<TRACK, MODEL == M_NE_METROPOLIS, OBS>(o, n, qq ? sd : c, gl, pc, ne_t32, ne_always, accU);
+                if (OBS >= 1) totU += (int)bytesum(accU);
+            }
+            own[li] = out;
+            nsites += 4;
+        }
+        if (OBS >= 1) {
+            March<MODEL, DIMS, TRACK, OBS> M;          // only the per-thread sums are used
+            M.totU = totU;
+            M.totBN = totBN;
+            long long cB, cM;
+            march_observables<MODEL, DIMS>(M, nsites, half == 1, cB, cM);
+            thrB += (int)cB;                           // |B| <= 3N, |M| <= N with N <= 2^20: far below 2^31
+            thrM += (int)cM;
+            if (half == 1) {                           // once per sweep: warp reduce -> block-local shared atomics
+                const int wB = __reduce_add_sync(0xffffffffu, thrB), wM = __reduce_add_sync(0xffffffffu, thrM);
+                if ((threadIdx.x & 31) == 0) {
+                    if (wB != 0) atomicAdd(&sm.acc[sw & 1][0], wB);
+                    if (wM != 0) atomicAdd(&sm.acc[sw & 1][1], wM);
+                }
+            }
+        }
+        // the barrier between the two colours
+        if (nrank > 1) cluster.sync();
+        else __syncthreads();
+        if (OBS >= 1 && half == 1 && threadIdx.x == 0) {
+            // one fire-and-forget 64-bit add per block into the sweep's (zeroed) slot; the next adds to this
+            // shared buffer belong to sweep sw + 2: two barriers away
+            const int vB = sm.acc[sw & 1][0], vM = sm.acc[sw & 1][1];
+            if (vB != 0) atomicAdd((unsigned long long *)&a.obs[2 * sw], (unsigned long long)(long long)vB);
+            if (vM != 0) atomicAdd((unsigned long long *)&a.obs[2 * sw + 1], (unsigned long long)(long long)vM);
+            sm.acc[sw & 1][0] = 0;
+            sm.acc[sw & 1][1] = 0;
+        }
+    }
+    for (uint32_t i = threadIdx.x; i < nl; i += blockDim.x) {
+        reinterpret_cast<uint32_t *>(a.col[0])[base + i] = s_col[0][i];
+        reinterpret_cast<uint32_t *>(a.col[1])[base + i] = s_col[1][i];
+    }
+    if (nrank > 1) cluster.sync();      // no block may exit while a neighbour can still read its shared memory
+}
+
+// ------------------------------------------------------------------------------------------
+// Host side
+// ------------------------------------------------------------------------------------------
+PhiloxSweepConsts make_philox_consts(const SweepKey &k);   // lsm_tiled.cu
+
+static int ilog2(int v)
+{
+    int l = 0;
+    while ((1 << l) < v) ++l;
+    return l;
+}
+
+template <int MODEL, int DIMS>
+static cudaError_t small_launch_to(bool track, bool obs, int threads, cudaStream_t s, const SmallArgs &a,
+                                   const PhiloxSweepConsts &pk, const typename TabOf<MODEL>::type &tab, int lg_lpr,
+                                   int lg_L, int nclu)
+{
+    if (lg_L > 0) {
+        const size_t smem = ((size_t)1 << (DIMS * lg_L)) / (size_t)nclu;   // N / cluster bytes: the slab of both colours
+        const int lg_rpc = lg_L - ilog2(nclu);
+        auto go = [&](auto kern) -> cudaError_t {
+            if (smem > 48 * 1024) {
+                cudaError_t e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+                if (e != cudaSuccess) return e;
+            }
+            if (nclu > 8) {
+                cudaError_t e = cudaFuncSetAttribute(kern, cudaFuncAttributeNonPortableClusterSizeAllowed, 1);
+                if (e != cudaSuccess) return e;
+            }
+            cudaLaunchConfig_t cfg;
+            memset(&cfg, 0, sizeof(cfg));
+            cfg.gridDim = dim3((unsigned)nclu);
+            cfg.blockDim = dim3((unsigned)threads);
+            cfg.dynamicSmemBytes = smem;
+            cfg.stream = s;
+            cudaLaunchAttribute at[1];
+            at[0].id = cudaLaunchAttributeClusterDimension;
+            at[0].val.clusterDim.x = (unsigned)nclu;
+            at[0].val.clusterDim.y = 1;
+            at[0].val.clusterDim.z = 1;
+            cfg.attrs = at;
+            cfg.numAttrs = 1;
+            return cudaLaunchKernelEx(&cfg, kern, a, pk, tab, lg_lpr, lg_L, lg_rpc);
+        };
+        if (track) return obs ? go(k_sweep_small_lane<MODEL, DIMS, true, 2>) : go(k_sweep_small_lane<MODEL, DIMS, true, 0>);
+        return obs ? go(k_sweep_small_lane<MODEL, DIMS, false, 2>) : go(k_sweep_small_lane<MODEL, DIMS, false, 0>);
+    }
+    if (track) {
+        if (obs) k_sweep_small<MODEL, DIMS, true, 2><<<1, threads, 0, s>>>(a, pk, tab);
+        else k_sweep_small<MODEL, DIMS, true, 0><<<1, threads, 0, s>>>(a, pk, tab);
+    } else {
+        if (obs) k_sweep_small<MODEL, DIMS, false, 2><<<1, threads, 0, s>>>(a, pk, tab);
+        else k_sweep_small<MODEL, DIMS, false, 0><<<1, threads, 0, s>>>(a, pk, tab);
+    }
+    return cudaGetLastError();
+}
+
+static int small_max_cluster()
+{
+    const char *v = getenv("LSM_SMALL_MAX_CLUSTER");
+    const int c = (v && *v) ? atoi(v) : 16;
+    return c < 1 ? 1 : c > 16 ? 16 : c;
+}
+
+static int small_max_sites()
+{
+    const char *v = getenv("LSM_SMALL_MAX_SITES");
+    return (v && *v) ? atoi(v) : 262144;   // above 512^2 / 64^3 the tiled family wins (profiles/r1_small_family.md)
+}
+
+// Plan: every word column gets as many march segments as 1024 threads allow.
+bool small_plan(const Lat &lat, int model, const TiledTables &t, SmallPlan *out, bool ignore_size_limit)
+{
+    if (!tiled_supported(lat, model, t)) return false;
+    const long long N = 2 * lat.half;
+    if (N > 1048576) return false;                    // int accumulators; beyond this the tiled family is faster anyway
+    if (!ignore_size_limit && N > small_max_sites()) return false;
+    const int R = lat.dims == 3 ? lat.L : 1, wpr = lat.Lh / 16;
+    const long long ncol = (long long)R * wpr;
+    if (ncol > 1024 && (lat.L & (lat.L - 1)) != 0) return false;
+    long long S = ncol > 1024 ? 1 : 1024 / ncol;
+    if (S > lat.L) S = lat.L;
+    out->S = (int)S;
+    out->threads = (int)(((ncol * S + 31) / 32) * 32);
+    out->lane = 0;
+    out->cluster = 1;
+    const char *v = getenv("LSM_SMALL_LANE");
+    const bool want_lane = !(v && *v == '0');
+    if (want_lane && (lat.L & (lat.L - 1)) == 0) {    // power of two: lane-granular threads, index math by shifts
+        const long long nlanes = lat.half / 4;
+        // thread blocks of the cluster: >= 128 lanes (4 warps) each, at most 16 (B200 schedules 16-block clusters;
+        // measured: profiles/r1_small_family.md) -- a half-sweep of a small lattice is bound by latency, not issue
+        int c = 1;
+        while (c < small_max_cluster() && nlanes / (2 * c) >= 128 && 2 * c <= lat.L) c *= 2;
+        const char *vc = getenv("LSM_SMALL_CLUSTER");
+        if (vc && *vc) {
+            const int want = atoi(vc);
+            if (want >= 1 && want <= 16 && (want & (want - 1)) == 0 && want <= lat.L && nlanes / want >= 32) c = want;
+        }
+        if (N / c <= 196608) {                          // the slab must fit shared memory
+            out->lane = 1;
+            out->cluster = c;
+            const long long per = nlanes / c;
+            out->threads = (int)(per < 1024 ? ((per + 31) / 32) * 32 : 1024);
+        }
+    }
+    if (!out->lane && ncol > 1024) return false;
+    if (!out->lane && !ignore_size_limit && N > 32768) return false;   // one SM: ~7.7 Gflips, the tiled family wins above
+    return true;
+}
+
+cudaError_t launch_sweep_small(const Lat &lat, int model, int track, unsigned long long seed, unsigned long long t0,
+                               int nsweeps, long long *d_obs, const SmallPlan &plan, const TiledTables &t,
+                               cudaStream_t s)
+{
+    SmallArgs a;
+    memset(&a, 0, sizeof(a));
+    a.col[0] = lat.col[0];
+    a.col[1] = lat.col[1];
+    a.g.L = lat.L;
+    a.g.R = lat.dims == 3 ? lat.L : 1;
+    a.g.wpr = lat.Lh / 16;
+    a.g.ncol = a.g.R * a.g.wpr;
+    a.g.S = plan.S;
+    a.g.one = 1;
+    a.g.parity_rows = 0;                              // column_of: plain (row, word) order
+    a.seed = seed;
+    a.t0 = t0;
+    a.nsweeps = nsweeps;
+    a.obs = d_obs;
+    PhiloxSweepConsts pk = make_philox_consts(make_sweep_key(seed, t0, 0u));   // only the round keys are used
+    const bool obs = d_obs != nullptr, tr = track != 0;
+    int lg_L = 0, lg_lpr = 0;
+    if (plan.lane) {
+        while ((1 << lg_L) < lat.L) ++lg_L;
+        lg_lpr = lg_L - 3;                              // L/2 bytes per compact row = L/8 lanes
+    }
+    switch (model) {
+    case M_ISING_HALF: {
+        HalfTab ht;
+        for (int i = 0; i < 16; ++i) ht.t[i] = t.t32[i];
+        return lat.dims == 3 ? small_launch_to<M_ISING_HALF, 3>(tr, obs, plan.threads, s, a, pk, ht, lg_lpr, lg_L, plan.cluster)
+                             : small_launch_to<M_ISING_HALF, 2>(tr, obs, plan.threads, s, a, pk, ht, lg_lpr, lg_L, plan.cluster);
+    }
+    case M_ISING_ONE: {
+        OneTab ot;
+        for (int i = 0; i < 96; ++i) ot.e[i] = t.s1[i];
+        return lat.dims == 3 ? small_launch_to<M_ISING_ONE, 3>(tr, obs, plan.threads, s, a, pk, ot, lg_lpr, lg_L, plan.cluster)
+                             : small_launch_to<M_ISING_ONE, 2>(tr, obs, plan.threads, s, a, pk, ot, lg_lpr, lg_L, plan.cluster);
+    }
+    case M_NE_HEATBATH: {
+        NeTab nt = {t.ne_t32[0], 0};
+        return small_launch_to<M_NE_HEATBATH, 2>(tr, obs, plan.threads, s, a, pk, nt, lg_lpr, lg_L, plan.cluster);
+    }
+    default: {
+        NeTab nt = {t.ne_t32[1], t.ne_up_always};
+        return small_launch_to<M_NE_METROPOLIS, 2>(tr, obs, plan.threads, s, a, pk, nt, lg_lpr, lg_L, plan.cluster);
+    }
+    }
+}
+
+}  // namespace lsmk

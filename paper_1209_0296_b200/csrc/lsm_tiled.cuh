@@ -33,4 +33,12 @@ cudaError_t launch_sweep_resident(const Lat &lat, int model, int track, unsigned
                                   int nsweeps, long long *d_obs, unsigned *d_flags, unsigned epoch0,
                                   const ResidentPlan &plan, const TiledTables &t, cudaStream_t s);
 
+// Small family (lsm_small.cu): one thread block owns the whole lattice and runs `nsweeps` sweeps in one
+// launch, __syncthreads() between the colours.  Chosen automatically up to LSM_SMALL_MAX_SITES sites.
+struct SmallPlan { int S, threads, lane, cluster; };   // lane = 1: 32-bit lanes per thread, `cluster` thread blocks
+bool small_plan(const Lat &lat, int model, const TiledTables &t, SmallPlan *out, bool ignore_size_limit);
+cudaError_t launch_sweep_small(const Lat &lat, int model, int track, unsigned long long seed, unsigned long long t0,
+                               int nsweeps, long long *d_obs, const SmallPlan &plan, const TiledTables &t,
+                               cudaStream_t s);
+
 }  // namespace lsmk
