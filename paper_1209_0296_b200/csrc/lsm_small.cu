@@ -323,14 +323,16 @@ static int small_max_sites()
 // Plan: every word column gets as many march segments as 1024 threads allow.
 bool small_plan(const Lat &lat, int model, const TiledTables &t, SmallPlan *out, bool ignore_size_limit)
 {
-    if (!tiled_supported(lat, model, t)) return false;
+    if (!t.usable) return false;
+    const bool pow2 = lat.L >= 8 && (lat.L & (lat.L - 1)) == 0;       // lane-granular kernel: whole 32-bit lanes per row
+    const bool words = tiled_supported(lat, model, t);                // word-granular kernel: whole 16-byte words per row
+    if (!pow2 && !words) return false;
     const long long N = 2 * lat.half;
     if (N > 1048576) return false;                    // int accumulators; beyond this the tiled family is faster anyway
     if (!ignore_size_limit && N > small_max_sites()) return false;
     const int R = lat.dims == 3 ? lat.L : 1, wpr = lat.Lh / 16;
     const long long ncol = (long long)R * wpr;
-    if (ncol > 1024 && (lat.L & (lat.L - 1)) != 0) return false;
-    long long S = ncol > 1024 ? 1 : 1024 / ncol;
+    long long S = (ncol > 1024 || ncol < 1) ? 1 : 1024 / ncol;
     if (S > lat.L) S = lat.L;
     out->S = (int)S;
     out->threads = (int)(((ncol * S + 31) / 32) * 32);
@@ -338,7 +340,7 @@ bool small_plan(const Lat &lat, int model, const TiledTables &t, SmallPlan *out,
     out->cluster = 1;
     const char *v = getenv("LSM_SMALL_LANE");
     const bool want_lane = !(v && *v == '0');
-    if (want_lane && (lat.L & (lat.L - 1)) == 0) {    // power of two: lane-granular threads, index math by shifts
+    if (want_lane && pow2) {    // power of two: lane-granular threads, index math by shifts
         const long long nlanes = lat.half / 4;
         // thread blocks of the cluster: >= 128 lanes (4 warps) each, at most 16 (B200 schedules 16-block clusters;
         // measured: profiles/r1_small_family.md) -- a half-sweep of a small lattice is bound by latency, not issue
@@ -356,7 +358,7 @@ bool small_plan(const Lat &lat, int model, const TiledTables &t, SmallPlan *out,
             out->threads = (int)(per < 1024 ? ((per + 31) / 32) * 32 : 1024);
         }
     }
-    if (!out->lane && ncol > 1024) return false;
+    if (!out->lane && (!words || ncol > 1024)) return false;
     if (!out->lane && !ignore_size_limit && N > 32768) return false;   // one SM: ~7.7 Gflips, the tiled family wins above
     return true;
 }

@@ -46,6 +46,8 @@ SHAPES = [
     # (kwargs, sweeps) -- sizes span several tiles and ragged tails; L not a multiple of 32 included
     (dict(dims=2, L=4, T=2.269), 40),
     (dict(dims=2, L=6, T=2.0), 40),
+    (dict(dims=2, L=8, T=2.269), 40),                # one 32-bit lane per compact row (small family)
+    (dict(dims=2, L=16, T=2.0, h=0.1), 40),
     (dict(dims=2, L=34, T=2.269), 30),
     (dict(dims=2, L=64, T=2.269), 60),
     (dict(dims=2, L=96, T=2.6, h=0.05), 30),
@@ -57,15 +59,19 @@ SHAPES = [
     (dict(dims=2, L=32, T=2.0, J=-1.0), 20),        # antiferromagnet
     (dict(dims=3, L=4, T=4.5115), 30),
     (dict(dims=3, L=6, T=4.0, h=0.1), 20),
+    (dict(dims=3, L=8, T=4.5115), 30),
+    (dict(dims=3, L=16, T=4.0, h=-0.05), 20),
     (dict(dims=3, L=32, T=4.5115), 20),
     (dict(dims=3, L=64, T=4.5115), 8),
     (dict(dims=3, L=34, T=3.0), 8),
     (dict(dims=2, L=4, two_S=2, T=3.0, h=0.01), 40),
     (dict(dims=2, L=64, two_S=2, T=1.5, h=0.01), 30),
     (dict(dims=3, L=6, two_S=2, T=3.0, h=0.01), 20),
+    (dict(dims=3, L=16, two_S=2, T=3.0, h=0.01), 20),
     (dict(dims=3, L=32, two_S=2, T=3.0, h=0.01), 12),
     (dict(dims=3, L=64, two_S=2, T=3.0, h=0.01), 6),
     (dict(dims=2, L=4, model=lsm.NE_HEATBATH, J=0.0, T=W.ne_temperature(0.3)), 40),
+    (dict(dims=2, L=16, model=lsm.NE_HEATBATH, J=0.0, T=W.ne_temperature(0.3)), 40),
     (dict(dims=2, L=34, model=lsm.NE_HEATBATH, J=0.0, T=W.ne_temperature(0.2)), 40),
     (dict(dims=2, L=64, model=lsm.NE_HEATBATH, J=0.0, T=W.ne_temperature(0.1)), 60),
     (dict(dims=2, L=256, model=lsm.NE_HEATBATH, J=0.0, T=W.ne_temperature(0.3)), 40),
