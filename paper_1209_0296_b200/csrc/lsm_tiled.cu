@@ -38,7 +38,7 @@ PhiloxSweepConsts make_philox_consts(const SweepKey &k)
 }
 
 template <int MODEL, int DIMS, bool TRACK, int OBS>
-__global__ void __launch_bounds__(256, MODEL == M_ISING_ONE ? LSM_TILED_MINBLOCKS_ONE : LSM_TILED_MINBLOCKS)
+__global__ void __launch_bounds__(256, tiled_minblocks(MODEL))
 k_sweep_tiled(const __grid_constant__ TiledGeom g, const __grid_constant__ PhiloxSweepConsts pc,
               const __grid_constant__ typename TabOf<MODEL>::type tab)
 {
@@ -155,8 +155,7 @@ static int env_int(const char *name, int dflt)
     const char *v = getenv(name);
     return (v && *v) ? atoi(v) : dflt;
 }
-static int g_tiled_ctas_per_sm = env_int("LSM_TILED_CTAS_PER_SM", 4);
-static int g_tiled_ctas_per_sm_one = env_int("LSM_TILED_CTAS_PER_SM_ONE", LSM_TILED_MINBLOCKS_ONE);
+static int g_tiled_ctas_per_sm = env_int("LSM_TILED_CTAS_PER_SM", 0);   // 0: tiled_minblocks(model)
 static int g_tiled_waves_x4 = env_int("LSM_TILED_WAVES_X4", 4);   // waves in quarters
 static int g_tiled_pdl = env_int("LSM_TILED_PDL", 1);               // programmatic dependent launch
 
@@ -204,7 +203,7 @@ cudaError_t launch_sweep_tiled(const SweepArgs &a, const TiledTables &t, cudaStr
     else if (g.wpr % 32 == 0) g.parity_rows = 1;
     else if (g.wpr < 32 && 32 % g.wpr == 0 && g.R % (2 * (32 / g.wpr)) == 0) g.parity_rows = 1;
     else g.parity_rows = 0;
-    const int per_sm = a.model == M_ISING_ONE ? g_tiled_ctas_per_sm_one : g_tiled_ctas_per_sm;
+    const int per_sm = g_tiled_ctas_per_sm > 0 ? g_tiled_ctas_per_sm : tiled_minblocks(a.model);
     long long target = (long long)sm_count() * per_sm * 256 * g_tiled_waves_x4 / 4;
     long long S = target / g.ncol;
     if (S < 1) S = 1;

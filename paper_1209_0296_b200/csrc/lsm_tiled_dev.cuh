@@ -12,11 +12,22 @@
 #ifndef LSM_TILED_MINBLOCKS_ONE
 #define LSM_TILED_MINBLOCKS_ONE 3
 #endif
+// spin-1/2 Ising: the march is bound by pipe issue, not by latency (4 independent Philox chains per thread), and runs
+// fastest with 2 CTAs per SM and up to 128 registers (measured 1/2/3/4/5/6 CTAs: 1132/1163/1141/1120/1027/970
+// Gflips/s on cfg2); the North-East rule, which skips Philox for most lanes, prefers 4.
+#ifndef LSM_TILED_MINBLOCKS_HALF
+#define LSM_TILED_MINBLOCKS_HALF 2
+#endif
 #ifndef LSM_TILED_PF_ONE
 #define LSM_TILED_PF_ONE 0
 #endif
 
 namespace lsmk {
+
+constexpr int tiled_minblocks(int model)
+{
+    return model == M_ISING_ONE ? LSM_TILED_MINBLOCKS_ONE : model == M_ISING_HALF ? LSM_TILED_MINBLOCKS_HALF : LSM_TILED_MINBLOCKS;
+}
 
 // ------------------------------------------------------------------------------------------
 // Philox4x32-10 with the warp-uniform part hoisted.  In a half-sweep the counter is
