@@ -328,6 +328,107 @@ void orc_sweep_ordered(orc_t *o, int64_t n, int descending)
 
 void orc_sweep(orc_t *o, int64_t n) { orc_sweep_ordered(o, n, 0); }
 
+/* ------------------------------------------- North-East, random-tile schedule -- */
+/* The paper's "corrected algorithm" for the North-East model (PAPER.md:128-140,
+ * steps 3-10), which it prefers to the checkerboard sweep because random picks
+ * keep the relaxation dynamics of the serial code:
+ *   3. the lattice is divided into Q sub-lattices ("tiles") of P = b*b spins;
+ *   5. every block picks a different tile (Q blocks, Q tiles: each tile is
+ *      handled exactly once per launch) and copies it "including its
+ *      boundaries" -- only the upper and right ones are needed (Fig. 4);
+ *   6. lambda threads concurrently pick lambda spins of the tile at random
+ *      and update them;  7. synchronise;  8. repeat q times, q*lambda = P/2;
+ *   9. copy the tile back;  10. relaunch and redo 5-8: one lattice sweep.
+ * Readings (D17-D21), chosen so that the result is unique:
+ *   D17 one sweep = 2 launches; the sweep counter t counts sweeps.
+ *   D18 a tile's boundary cells are read from the lattice as it was when the
+ *       launch started and never refreshed; only interior cells are written.
+ *       Hence the result does not depend on which block takes which tile.
+ *   D19 the lambda picks of a sub-step all read the tile as it was when the
+ *       sub-step started; writes are applied in thread order, so on a
+ *       same-site collision the highest thread index wins.
+ *   D20 thread j picks r = floor(w_pos * P / 2^32), (px, py) = (r mod b, r div b);
+ *       the update rule is that of reading D7 with acceptance word w_acc.
+ *   D21 Philox counter c0 = tile id (tx + (L/b)*ty), c1 = k*ceil(lambda/2) + (j>>1)
+ *       for sub-step k and thread j, c2 = lo32(t), c3 = (4 + launch) | hi32(t)<<2;
+ *       w_pos = word 2(j&1), w_acc = word 2(j&1)+1.
+ * tiles_descending != 0 walks the tiles in reverse order (pin: same result). */
+int orc_sweep_random_tile(orc_t *o, int64_t n, int b, int lambda, int tiles_descending)
+{
+    if (o->model != ORC_NE_HEATBATH && o->model != ORC_NE_METROPOLIS) return -1;
+    int L = o->L;
+    if (b < 1 || L % b != 0 || lambda < 1) return -1;
+    int P = b * b;
+    if (P % (2 * lambda) != 0) return -1;
+    int q = P / (2 * lambda), nt = L / b, calls = (lambda + 1) / 2;
+    int8_t *start = (int8_t *)malloc((size_t)o->N);
+    int *site = (int *)malloc(sizeof(int) * (size_t)lambda);
+    int *val = (int *)malloc(sizeof(int) * (size_t)lambda);
+    if (!start || !site || !val) { free(start); free(site); free(val); return -2; }
+    uint32_t key[2] = {(uint32_t)o->seed, (uint32_t)(o->seed >> 32)};
+    for (int64_t it = 0; it < n; ++it) {
+        for (uint32_t launch = 0; launch < 2; ++launch) {
+            memcpy(start, o->s, (size_t)o->N);                 /* D18: the lattice at launch start */
+            for (int tt = 0; tt < nt * nt; ++tt) {
+                int T = tiles_descending ? nt * nt - 1 - tt : tt;
+                int tx = T % nt, ty = T / nt, x0 = tx * b, y0 = ty * b;
+                for (int k = 0; k < q; ++k) {
+                    for (int j = 0; j < lambda; ++j) {         /* decisions: all read the sub-step's start */
+                        uint32_t ctr[4], w[4];
+                        ctr[0] = (uint32_t)T;
+                        ctr[1] = (uint32_t)(k * calls + (j >> 1));
+                        ctr[2] = (uint32_t)o->t;
+                        ctr[3] = (4u + launch) | ((uint32_t)(o->t >> 32) << 2);
+                        orc_philox4x32_10(ctr, key, w);
+                        uint32_t w_pos = w[2 * (j & 1)], w_acc = w[2 * (j & 1) + 1];
+                        int r = (int)(((uint64_t)w_pos * (uint64_t)P) >> 32);
+                        int px = r % b, py = r / b;
+                        int x = x0 + px, y = y0 + py;
+                        /* north and east: interior cells from the evolving lattice, boundary cells from `start` */
+                        int xn = x, yn = y + 1, xe = x + 1, ye = y;
+                        int north = (py + 1 < b) ? o->s[site_id(o, xn, yn, 0)] : start[site_id(o, xn, wrap(yn, L), 0)];
+                        int east = (px + 1 < b) ? o->s[site_id(o, xe, ye, 0)] : start[site_id(o, wrap(xe, L), ye, 0)];
+                        int64_t i = site_id(o, x, y, 0);
+                        int s_old = o->s[i], s_new = s_old;
+                        if (north == 1 && east == 1) {
+                            if (o->model == ORC_NE_HEATBATH) {
+                                s_new = ((uint64_t)w_acc < o->thr[0]) ? 1 : 0;
+                            } else {
+                                uint64_t thr = (s_old == 0) ? o->thr[1] : o->thr[2];
+                                if ((uint64_t)w_acc < thr) s_new = 1 - s_old;
+                            }
+                        }
+                        site[j] = (int)i;
+                        val[j] = s_new;
+                    }
+                    for (int j = 0; j < lambda; ++j) {         /* D19: writes in thread order */
+                        int dup = 0;
+                        for (int j2 = j + 1; j2 < lambda; ++j2) dup |= (site[j2] == site[j]);
+                        if (dup) continue;                     /* a higher thread wrote the same site */
+                        if (val[j] != o->s[site[j]]) o->changed[site[j]] = 1;
+                        o->s[site[j]] = (int8_t)val[j];
+                    }
+                }
+            }
+        }
+        o->t += 1;
+    }
+    free(start); free(site); free(val);
+    return 0;
+}
+
+/* obs[2*k] = B (= 0), obs[2*k+1] = M after sweep k of this call. */
+void orc_measure(const orc_t *o, int64_t *B, int64_t *M);
+int orc_sweep_random_tile_record(orc_t *o, int64_t n, int b, int lambda, int64_t *obs)
+{
+    for (int64_t k = 0; k < n; ++k) {
+        int rc = orc_sweep_random_tile(o, 1, b, lambda, 0);
+        if (rc != 0) return rc;
+        orc_measure(o, &obs[2 * k], &obs[2 * k + 1]);
+    }
+    return 0;
+}
+
 /* ------------------------------------------------------------- observables -- */
 /* M = sum s_i; B = sum over bonds of s_i s_j, each bond once (east, north, up).
  * NE (reading D15): M = number of up sites, B = 0.                          */

@@ -70,6 +70,10 @@ def lib():
         L.orc_concentration.restype = dbl
         L.orc_concentration.argtypes = [vp]
         L.orc_philox4x32_10.argtypes = [vp, vp, vp]
+        L.orc_sweep_random_tile.restype = i32
+        L.orc_sweep_random_tile.argtypes = [vp, i64, i32, i32, i32]
+        L.orc_sweep_random_tile_record.restype = i32
+        L.orc_sweep_random_tile_record.argtypes = [vp, i64, i32, i32, vp]
         _lib = L
     return _lib
 
@@ -110,6 +114,17 @@ class Oracle:
     def sweep_record(self, n):
         obs = np.zeros((int(n), 2), dtype=np.int64)
         lib().orc_sweep_record(self._h, int(n), obs.ctypes.data)
+        return obs
+
+    def sweep_random_tile(self, n=1, b=32, lam=16, tiles_descending=False):
+        """The paper's corrected North-East algorithm (readings D17-D21)."""
+        if lib().orc_sweep_random_tile(self._h, int(n), int(b), int(lam), 1 if tiles_descending else 0) != 0:
+            raise ValueError("random-tile schedule: NE model, b | L and 2*lambda | b*b required")
+
+    def sweep_random_tile_record(self, n, b=32, lam=16):
+        obs = np.zeros((int(n), 2), dtype=np.int64)
+        if lib().orc_sweep_random_tile_record(self._h, int(n), int(b), int(lam), obs.ctypes.data) != 0:
+            raise ValueError("random-tile schedule: NE model, b | L and 2*lambda | b*b required")
         return obs
 
     def measure_int(self):
