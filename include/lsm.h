@@ -95,6 +95,18 @@ int lsm_sweep_record(lsm_t *, int64_t n, int64_t *d_obs, void *stream);
  * the call returns after it completed (synchronises).  d_scratch: device, 16*n bytes. */
 int lsm_sweep_record_host(lsm_t *, int64_t n, int64_t *h_obs, int64_t *d_scratch, void *stream);
 
+/* North-East model only: n sweeps of the paper's "corrected algorithm" (steps 3-10) instead of
+ * the checkerboard sweep, which the paper rejects for relaxation dynamics.  The lattice is
+ * divided into tiles of tile_edge x tile_edge spins (P = tile_edge^2); a sweep is two launches; in each, every
+ * tile is handled once: lambda threads pick lambda of its spins at random and update them (rule of the handle's
+ * model), synchronise, q times with q * lambda = P/2.  Readings D17-D21: tile boundaries (upper and
+ * right, Fig. 4) are those of the launch start; the picks of a sub-step read the tile as the sub-step found it;
+ * on a same-site collision the highest thread wins; Philox counter (tile, sub-step * ceil(lambda/2) + thread/2,
+ * sweep, 4 + launch).  d_obs: NULL, or device [n][2] receiving (0, M) after every sweep.  Asynchronous.
+ * UNSUPPORTED unless tile_edge is a power of two in [8, 128] dividing L, lambda a power of two in [1, 32] and
+ * 2 * lambda divides P.  Shares the sweep counter with lsm_sweep. */
+int lsm_sweep_random_tile(lsm_t *, int64_t n, int tile_edge, int lambda, int64_t *d_obs, void *stream);
+
 /* Running observables of the current configuration (synchronises). */
 int lsm_measure(lsm_t *, double *E, int64_t *M);
 int lsm_measure_int(lsm_t *, int64_t *bond_sum, int64_t *M, uint64_t *sweeps_done);

@@ -33,6 +33,7 @@ struct lsm {
     unsigned *d_flags;  // resident family: one progress word per CTA
     ResidentPlan plan;
     SmallPlan small;
+    uint8_t *alt[2];    // NE models: second lattice buffer of the random-tile schedule (reading D18)
 };
 
 static thread_local std::string g_cuda_err;
@@ -66,6 +67,7 @@ extern "C" int lsm_workspace_bytes(int dims, int L, int two_S, int model, size_t
     if (rc != LSM_OK) return rc;
     size_t N = (size_t)L * L * (dims == 3 ? (size_t)L : 1);
     *bytes = STATE_BYTES + 2 * align256(N / 2) + 256;
+    if (model != LSM_ISING) *bytes += 2 * align256(N / 2);   // second buffer of the random-tile schedule
     return LSM_OK;
 }
 
@@ -158,6 +160,11 @@ extern "C" int lsm_create(int dims, int L, int two_S, int model, double J, doubl
     o->d_flags = (unsigned *)(base + 256);
     o->lat.col[0] = base + STATE_BYTES;
     o->lat.col[1] = base + STATE_BYTES + align256((size_t)o->N / 2);
+    o->alt[0] = o->alt[1] = nullptr;
+    if (model != LSM_ISING) {
+        o->alt[0] = o->lat.col[1] + align256((size_t)o->N / 2);
+        o->alt[1] = o->alt[0] + align256((size_t)o->N / 2);
+    }
     o->lat.L = L; o->lat.Lh = L / 2; o->lat.dims = dims; o->lat.Lz = dims == 3 ? L : 1;
     o->lat.half = o->N / 2;
     o->t = 0; o->tracking = 1; o->kernel_pref = LSM_KERNEL_AUTO; o->launches = 0;
@@ -264,6 +271,36 @@ extern "C" int lsm_sweep_record(lsm_t *o, int64_t n, int64_t *d_obs, void *strea
 {
     if (!o || n < 0 || (!d_obs && n > 0)) return LSM_ERR_ARG;
     return sweep_impl(o, n, (long long *)d_obs, (cudaStream_t)stream);
+}
+
+// The paper's corrected North-East algorithm: two launches per sweep, each reading one
+// lattice buffer and writing the other (reading D18).
+extern "C" int lsm_sweep_random_tile(lsm_t *o, int64_t n, int tile_edge, int lambda, int64_t *d_obs, void *stream)
+{
+    if (!o || n < 0) return LSM_ERR_ARG;
+    if (o->model != M_NE_HEATBATH && o->model != M_NE_METROPOLIS) return LSM_ERR_UNSUPPORTED;
+    if (!ne_tile_supported(o->lat, tile_edge, lambda)) return LSM_ERR_UNSUPPORTED;
+    cudaStream_t s = (cudaStream_t)stream;
+    o->last_stream = s;
+    if (n == 0) return LSM_OK;
+    const uint64_t ALWAYS = (uint64_t)1 << 32;
+    const uint32_t thr_c = o->thr[0] >= ALWAYS ? 0xFFFFFFFFu : (uint32_t)o->thr[0];
+    const uint32_t thr_up = o->thr[1] >= ALWAYS ? 0xFFFFFFFFu : (uint32_t)o->thr[1];
+    if (d_obs) CU(cudaMemsetAsync(d_obs, 0, (size_t)n * 16, s));
+    else CU(cudaMemsetAsync(o->d_run, 0, 16, s));
+    for (int64_t k = 0; k < n; ++k) {
+        long long *obs = d_obs ? (long long *)d_obs + 2 * k : (k == n - 1 ? o->d_run : nullptr);
+        for (int launch = 0; launch < 2; ++launch) {
+            CU(launch_ne_random_tile(o->lat, o->alt, o->model == M_NE_METROPOLIS, tile_edge, lambda, o->seed, o->t,
+                                     launch, thr_c, thr_up, o->thr[1] >= ALWAYS ? 1 : 0, o->tracking,
+                                     launch == 1 ? obs : nullptr, s));
+            o->launches += 1;
+            for (int c = 0; c < 2; ++c) { uint8_t *tmp = o->lat.col[c]; o->lat.col[c] = o->alt[c]; o->alt[c] = tmp; }
+        }
+        o->t += 1;
+    }
+    if (d_obs) CU(cudaMemcpyAsync(o->d_run, (long long *)d_obs + 2 * (n - 1), 16, cudaMemcpyDeviceToDevice, s));
+    return LSM_OK;
 }
 
 extern "C" int lsm_sweep_record_host(lsm_t *o, int64_t n, int64_t *h_obs, int64_t *d_scratch, void *stream)

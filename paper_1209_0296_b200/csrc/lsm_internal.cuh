@@ -160,6 +160,12 @@ cudaError_t launch_philox_device(const uint32_t *d_ck, uint32_t *d_out, long lon
 cudaError_t launch_philox_throughput(int blocks, int calls, uint32_t *d_sink, cudaStream_t s);
 cudaError_t launch_pipe_probe(int mode, int blocks, int iters, uint32_t *d_sink, cudaStream_t s);
 
+// North-East random-tile schedule (lsm_ne_tile.cu): reads lat.col, writes dst.
+bool ne_tile_supported(const Lat &lat, int b, int lam);
+cudaError_t launch_ne_random_tile(const Lat &lat, uint8_t *const dst[2], bool metropolis, int b, int lam,
+                                  unsigned long long seed, unsigned long long t, int launch, uint32_t thr_c,
+                                  uint32_t thr_up, int up_always, int track, long long *obs, cudaStream_t s);
+
 int sm_count();
 
 }  // namespace lsmk

@@ -1,0 +1,186 @@
+// lsm_ne_tile.cu -- the paper's "corrected algorithm" for the North-East model (steps 3-10):
+// the lattice is divided into Q tiles of P = b*b spins; in each of the two launches of a sweep every tile is
+// handled once: it is copied with its upper and right boundaries (Fig. 4) into shared memory, lambda threads pick
+// lambda spins of the tile at random and update them, synchronise, q times with q*lambda = P/2, and the tile is
+// copied back.  Readings D17-D21 make the result unique so that it can be bit-exact against the CPU
+// oracle: boundaries are those of the launch start (the kernel reads one lattice buffer and writes the other),
+// the lambda picks of a sub-step read the tile as the sub-step found it, and on a same-site collision the
+// highest thread wins.
+//
+// B200 mapping: a group of lambda lanes of a warp owns a tile (lambda = 16: two tiles per warp), so steps 6-7 --
+// pick, synchronise -- are warp-level (match.any finds collisions, bar.warp.sync is the barrier) and a CTA keeps
+// 256/lambda tiles in flight.  The tile sits in shared memory in the lattice's own split-colour layout (two
+// arrays of (b+1) rows x b/2 bytes plus the east boundary column), so the copies are plain 32-bit words.
+// Random words: one Philox4x32-10 call serves two picks (position and acceptance word each); the even lane of a
+// pair computes it and hands two words to the odd lane by shuffle.
+#include "lsm_internal.cuh"
+
+#include <cstring>
+
+namespace lsmk {
+
+struct NeTileArgs {
+    const uint8_t *src[2];   // lattice at launch start (colour arrays)
+    uint8_t *dst[2];         // lattice after the launch
+    int L, Lh;               // Lh = L/2 bytes per compact row
+    int lg_b, lg_lam;        // tile edge and lambda are powers of two
+    int ntx;                 // tiles per lattice row
+    int ntiles;
+    uint32_t k0, k1, c2, c3; // Philox key and the (sweep, launch) fields of the counter
+    uint32_t thr_c, thr_up;  // floor(c 2^32), floor(exp(-1/T) 2^32) clipped to 32 bits
+    int up_always;           // Metropolis: exp(-1/T) rounds to 2^32
+    int track;
+    long long *obs;          // (B, M) slot receiving the up-count after the launch, or nullptr
+};
+
+template <bool METRO>
+__global__ void __launch_bounds__(256)
+k_ne_random_tile(const __grid_constant__ NeTileArgs a)
+{
+    extern __shared__ __align__(16) uint8_t s_tiles[];
+    const int b = 1 << a.lg_b, lam = 1 << a.lg_lam, P = b * b;
+    const int lane = threadIdx.x & 31, j = lane & (lam - 1);          // j: thread index within the tile's group
+    const int grp_in_warp = lane >> a.lg_lam, grp_per_warp = 32 >> a.lg_lam;
+    const int warp_global = (blockIdx.x * blockDim.x + threadIdx.x) >> 5;
+    const int nwarps = (gridDim.x * blockDim.x) >> 5;
+    const int rowb = b >> 1;                                          // bytes per tile row and colour
+    const int col_bytes = (b + 1) * rowb;                             // rows 0..b (row b = north boundary)
+    const int tile_bytes = (2 * col_bytes + b + 15) & ~15;            // + east boundary column
+    uint8_t *const tile = s_tiles + (size_t)((threadIdx.x >> 5) * grp_per_warp + grp_in_warp) * tile_bytes;
+    uint8_t *const east = tile + 2 * col_bytes;
+    const int q = P >> (a.lg_lam + 1), calls = (lam + 1) >> 1;
+    int ups = 0;
+
+    for (int base = warp_global * grp_per_warp; base < a.ntiles; base += nwarps * grp_per_warp) {
+        const int T = base + grp_in_warp;
+        const bool live = T < a.ntiles;                                // tail groups idle but keep the warp converged
+        const int ty = live ? T / a.ntx : 0, tx = live ? T - ty * a.ntx : 0;
+        const int x0 = tx << a.lg_b, y0 = ty << a.lg_b;
+        // ---- step 5: tile + upper and right boundaries -> shared memory
+        if (live) {
+            const int lanes_row = rowb >> 2;                           // 32-bit words per tile row and colour
+            for (int i = j; i < 2 * (b + 1) * lanes_row; i += lam) {
+                const int c = i / ((b + 1) * lanes_row), rem = i - c * (b + 1) * lanes_row;
+                const int rr = rem / lanes_row, u = rem - rr * lanes_row;
+                int yy = y0 + rr;
+                if (yy >= a.L) yy -= a.L;
+                const uint32_t v = *reinterpret_cast<const uint32_t *>((c ? a.src[1] : a.src[0]) + (size_t)yy * a.Lh + (x0 >> 1) + 4 * u);
+                *reinterpret_cast<uint32_t *>((tile + c * col_bytes) + rr * rowb + 4 * u) = v;
+            }
+            int xe = x0 + b;
+            if (xe >= a.L) xe -= a.L;
+            for (int py = j; py < b; py += lam) {
+                const int yy = y0 + py;
+                east[py] = (((xe + yy) & 1) ? a.src[1] : a.src[0])[(size_t)yy * a.Lh + (xe >> 1)];
+            }
+        }
+        __syncwarp();
+        // ---- steps 6-8: q sub-steps of lambda simultaneous random picks
+        for (int k = 0; k < q; ++k) {
+            uint4 w = make_uint4(0, 0, 0, 0);
+            if ((j & 1) == 0) w = philox4x32_10((uint32_t)T, (uint32_t)(k * calls + (j >> 1)), a.c2, a.c3, a.k0, a.k1);
+            const uint32_t pz = __shfl_sync(0xffffffffu, w.z, lane & ~1), pw = __shfl_sync(0xffffffffu, w.w, lane & ~1);
+            const uint32_t w_pos = (j & 1) ? pz : w.x, w_acc = (j & 1) ? pw : w.y;
+            const int r = (int)__umulhi(w_pos, (uint32_t)P);
+            const int px = r & (b - 1), py = r >> a.lg_b;
+            const int c = (px + py) & 1;                               // x0, y0 are even
+            uint8_t *const me = (tile + c * col_bytes) + py * rowb + (px >> 1);
+            const uint32_t own = *me;
+            const uint32_t north = (tile + (c ^ 1) * col_bytes)[(py + 1) * rowb + (px >> 1)];
+            const uint32_t est = (px + 1 < b) ? (tile + (c ^ 1) * col_bytes)[py * rowb + ((px + 1) >> 1)] : east[py];
+            uint32_t n_new = own & 1u;
+            if ((north & est & 1u) != 0u) {                            // facilitated
+                if (METRO) {
+                    if ((own & 1u) != 0u || a.up_always || w_acc < a.thr_up) n_new ^= 1u;
+                } else {
+                    n_new = w_acc < a.thr_c ? 1u : 0u;
+                }
+            }
+            // same site picked twice in this sub-step: the highest thread of the group wins (reading D19)
+            const uint32_t same = __match_any_sync(0xffffffffu, (uint32_t)r | ((uint32_t)grp_in_warp << 16) |
+                                                                    (live ? 0u : 0x80000000u));
+            const bool winner = (same >> lane) == 1u;                  // no higher lane holds the same key
+            __syncwarp();                                              // all picks have read the sub-step's start
+            if (live && winner && n_new != (own & 1u)) *me = (uint8_t)((own ^ 1u) | (a.track ? 0x08u : 0u));
+            __syncwarp();                                              // step 7
+        }
+        // ---- step 9: copy the tile back (interior only); count the up sites for the fused observable
+        if (live) {
+            const int lanes_row = rowb >> 2;
+            for (int i = j; i < 2 * b * lanes_row; i += lam) {
+                const int c = i / (b * lanes_row), rem = i - c * b * lanes_row;
+                const int rr = rem / lanes_row, u = rem - rr * lanes_row;
+                const uint32_t v = *reinterpret_cast<const uint32_t *>((tile + c * col_bytes) + rr * rowb + 4 * u);
+                *reinterpret_cast<uint32_t *>((c ? a.dst[1] : a.dst[0]) + (size_t)(y0 + rr) * a.Lh + (x0 >> 1) + 4 * u) = v;
+                ups += (int)__dp4a(v & 0x01010101u, 0x01010101u, 0u);
+            }
+        }
+        __syncwarp();
+    }
+    if (a.obs) {
+        const int s = __reduce_add_sync(0xffffffffu, ups);
+        if (lane == 0 && s != 0) atomicAdd((unsigned long long *)&a.obs[1], (unsigned long long)s);
+    }
+}
+
+// Shared memory of one tile (must match the kernel).
+static size_t ne_tile_bytes(int b) { return (size_t)((2 * (b + 1) * (b / 2) + b + 15) & ~15); }
+
+bool ne_tile_supported(const Lat &lat, int b, int lam)
+{
+    if (lat.dims != 2) return false;
+    if (b < 8 || b > 128 || (b & (b - 1)) != 0 || lat.L % b != 0) return false;
+    if (lam < 1 || lam > 32 || (lam & (lam - 1)) != 0) return false;
+    if ((b * b) % (2 * lam) != 0) return false;
+    return true;
+}
+
+// Threads per CTA: as many tile groups as fit ~96 KB of shared memory (at least one warp).
+static int ne_tile_threads(int b, int lam)
+{
+    int threads = 256;
+    while (threads > 32 && (threads / lam) * ne_tile_bytes(b) > 96 * 1024) threads >>= 1;
+    return threads;
+}
+
+cudaError_t launch_ne_random_tile(const Lat &lat, uint8_t *const dst[2], bool metropolis, int b, int lam,
+                                  unsigned long long seed, unsigned long long t, int launch, uint32_t thr_c,
+                                  uint32_t thr_up, int up_always, int track, long long *obs, cudaStream_t s)
+{
+    NeTileArgs a;
+    memset(&a, 0, sizeof(a));
+    a.src[0] = lat.col[0];
+    a.src[1] = lat.col[1];
+    a.dst[0] = dst[0];
+    a.dst[1] = dst[1];
+    a.L = lat.L;
+    a.Lh = lat.Lh;
+    while ((1 << a.lg_b) < b) ++a.lg_b;
+    while ((1 << a.lg_lam) < lam) ++a.lg_lam;
+    a.ntx = lat.L / b;
+    a.ntiles = a.ntx * a.ntx;
+    a.k0 = (uint32_t)seed;
+    a.k1 = (uint32_t)(seed >> 32);
+    a.c2 = (uint32_t)t;
+    a.c3 = (4u + (uint32_t)launch) | ((uint32_t)(t >> 32) << 2);     // reading D21: stream tags 4, 5
+    a.thr_c = thr_c;
+    a.thr_up = thr_up;
+    a.up_always = up_always;
+    a.track = track;
+    a.obs = obs;
+    const int threads = ne_tile_threads(b, lam);
+    const int tiles_per_cta = threads / lam;
+    const size_t smem = tiles_per_cta * ne_tile_bytes(b);
+    int grid = (a.ntiles + tiles_per_cta - 1) / tiles_per_cta;
+    const int cap = sm_count() * 8;
+    if (grid > cap) grid = cap;
+    auto kern = metropolis ? k_ne_random_tile<true> : k_ne_random_tile<false>;
+    if (smem > 48 * 1024) {
+        cudaError_t e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+        if (e != cudaSuccess) return e;
+    }
+    kern<<<grid, threads, smem, s>>>(a);
+    return cudaGetLastError();
+}
+
+}  // namespace lsmk

@@ -312,3 +312,51 @@ def test_full_size_prefix_and_late_spot_check(name, k_first, t_late, family):
     Bv, Mv, t = lat.measure_int()
     assert t == t_late + 1 and abs(Mv) <= N and abs(Bv) <= w.dims * N
     assert lat.measure_full() == (Bv, Mv)
+
+
+# ------------------------------------------------------------------ NEXT-1: the paper's corrected North-East algorithm
+@pytest.mark.parametrize("model", [lsm.NE_HEATBATH, lsm.NE_METROPOLIS])
+@pytest.mark.parametrize("L,b,lam,c,nsweeps", [
+    (64, 32, 16, 0.42, 30),      # the paper's best configuration (32 x 32 tiles, lambda = 16)
+    (64, 8, 4, 0.45, 20),        # small tiles: same-site collisions in most sub-steps
+    (64, 8, 32, 0.45, 20),       # lambda = P/2: a single sub-step per launch
+    (128, 16, 1, 0.30, 12),      # lambda = 1: serial inside a tile
+    (64, 64, 1, 0.42, 6),        # Q = lambda = 1: the serial limit
+    (256, 64, 8, 0.20, 10),
+    (384, 128, 32, 0.30, 5),     # tiles of 16 KiB, L not a power of two
+    (1024, 32, 16, 0.42, 4),     # several waves of CTAs, tail groups
+])
+def test_random_tile_schedule_parity(model, L, b, lam, c, nsweeps):
+    """Configuration, per-sweep M, persistence and overlap after every stage; mixes with checkerboard sweeps."""
+    kw = dict(dims=2, L=L, model=model, J=0.0, T=W.ne_temperature(c), seed=W.seed_of(5, 7) + L + lam)
+    lat, orc = make_pair(**kw)
+    half = nsweeps // 2
+    got = lat.sweep_random_tile(half, b, lam, record=True).cpu().numpy()
+    want = orc.sweep_random_tile_record(half, b, lam)
+    assert np.array_equal(got, want), np.flatnonzero((got != want).any(axis=1))[:5]
+    assert_same_state(lat, orc)
+    lat.sweep_random_tile(nsweeps - half, b, lam)            # no record: running M of the last sweep only
+    orc.sweep_random_tile(nsweeps - half, b, lam)
+    assert_same_state(lat, orc)
+    lat.sweep(3)                                             # the checkerboard sweep shares state and sweep counter
+    orc.sweep(3)
+    lat.sweep_random_tile(2, b, lam)
+    orc.sweep_random_tile(2, b, lam)
+    assert_same_state(lat, orc)
+    lat.set_tracking(False)
+    lat.sweep_random_tile(2, b, lam)
+    orc.sweep_random_tile(2, b, lam)
+    assert np.array_equal(lat.get_spins().cpu().numpy(), orc.get_spins())
+    assert lat.measure_int()[:2] == orc.measure_int()
+
+
+def test_random_tile_schedule_rejections():
+    lat = lsm.Lattice(dims=2, L=64, model=lsm.NE_HEATBATH, J=0.0, T=1.0, seed=3)
+    for b, lam in ((24, 16), (32, 3), (4, 2), (32, 64), (256, 16)):
+        with pytest.raises(lsm.LsmError) as e:
+            lat.sweep_random_tile(1, b, lam)
+        assert e.value.code == lsm.ERR_UNSUPPORTED
+    ising = lsm.Lattice(dims=2, L=64, T=2.0, seed=3)
+    with pytest.raises(lsm.LsmError) as e:
+        ising.sweep_random_tile(1, 32, 16)
+    assert e.value.code == lsm.ERR_UNSUPPORTED
