@@ -33,6 +33,17 @@ struct NeTileArgs {
     long long *obs;          // (B, M) slot receiving the up-count after the launch, or nullptr
 };
 
+__device__ __forceinline__ uint32_t lds_u8(uint32_t a)
+{
+    uint32_t v;
+    asm volatile("ld.shared.u8 %0, [%1];" : "=r"(v) : "r"(a) : "memory");
+    return v;
+}
+__device__ __forceinline__ void sts_u8(uint32_t a, uint32_t v)
+{
+    asm volatile("st.shared.u8 [%0], %1;" ::"r"(a), "r"(v) : "memory");
+}
+
 template <bool METRO>
 __global__ void __launch_bounds__(256)
 k_ne_random_tile(const __grid_constant__ NeTileArgs a)
@@ -45,23 +56,29 @@ k_ne_random_tile(const __grid_constant__ NeTileArgs a)
     const int nwarps = (gridDim.x * blockDim.x) >> 5;
     const int rowb = b >> 1;                                          // bytes per tile row and colour
     const int col_bytes = (b + 1) * rowb;                             // rows 0..b (row b = north boundary)
-    const int tile_bytes = (2 * col_bytes + b + 15) & ~15;            // + east boundary column
+    const int tile_bytes = (2 * col_bytes + b + (lam > 1 ? P : 0) + 15) & ~15;   // + east column + claim bytes
     uint8_t *const tile = s_tiles + (size_t)((threadIdx.x >> 5) * grp_per_warp + grp_in_warp) * tile_bytes;
     uint8_t *const east = tile + 2 * col_bytes;
+    // 32-bit shared-space addresses for the pick loop (no generic-address conversion per access)
+    const uint32_t s_tile = (uint32_t)__cvta_generic_to_shared(tile), s_east = s_tile + 2u * (uint32_t)col_bytes,
+                   s_claim = s_east + (uint32_t)b;
+    const uint32_t chg = a.track ? 0x08u : 0u, thr_c = a.thr_c, thr_up = a.thr_up;
+    const bool up_always = a.up_always != 0;
     const int q = P >> (a.lg_lam + 1), calls = (lam + 1) >> 1;
     int ups = 0;
 
     for (int base = warp_global * grp_per_warp; base < a.ntiles; base += nwarps * grp_per_warp) {
         const int T = base + grp_in_warp;
         const bool live = T < a.ntiles;                                // tail groups idle but keep the warp converged
-        const int ty = live ? T / a.ntx : 0, tx = live ? T - ty * a.ntx : 0;
+        const int ty = live ? T / a.ntx : 0, tx = live ? T - ty * a.ntx : 0;   // one division per tile
         const int x0 = tx << a.lg_b, y0 = ty << a.lg_b;
+        const uint32_t key_hi = ((uint32_t)grp_in_warp << 16) | (live ? 0u : 0x80000000u);
         // ---- step 5: tile + upper and right boundaries -> shared memory
         if (live) {
-            const int lanes_row = rowb >> 2;                           // 32-bit words per tile row and colour
-            for (int i = j; i < 2 * (b + 1) * lanes_row; i += lam) {
-                const int c = i / ((b + 1) * lanes_row), rem = i - c * (b + 1) * lanes_row;
-                const int rr = rem / lanes_row, u = rem - rr * lanes_row;
+            // word i of the tile -> (row, colour, word in row): all powers of two, no divisions
+            const int lg_lr = a.lg_b - 3;                              // log2(32-bit words per tile row and colour)
+            for (int i = j; i < ((b + 1) << (lg_lr + 1)); i += lam) {
+                const int rr = i >> (lg_lr + 1), c = (i >> lg_lr) & 1, u = i & ((1 << lg_lr) - 1);
                 int yy = y0 + rr;
                 if (yy >= a.L) yy -= a.L;
                 const uint32_t v = *reinterpret_cast<const uint32_t *>((c ? a.src[1] : a.src[0]) + (size_t)yy * a.Lh + (x0 >> 1) + 4 * u);
@@ -76,40 +93,66 @@ k_ne_random_tile(const __grid_constant__ NeTileArgs a)
         }
         __syncwarp();
         // ---- steps 6-8: q sub-steps of lambda simultaneous random picks
+        uint4 w = make_uint4(0, 0, 0, 0);
         for (int k = 0; k < q; ++k) {
-            uint4 w = make_uint4(0, 0, 0, 0);
-            if ((j & 1) == 0) w = philox4x32_10((uint32_t)T, (uint32_t)(k * calls + (j >> 1)), a.c2, a.c3, a.k0, a.k1);
-            const uint32_t pz = __shfl_sync(0xffffffffu, w.z, lane & ~1), pw = __shfl_sync(0xffffffffu, w.w, lane & ~1);
-            const uint32_t w_pos = (j & 1) ? pz : w.x, w_acc = (j & 1) ? pw : w.y;
+            // One Philox call serves the two picks of a lane pair (reading D21).  Over two consecutive sub-steps the
+            // even lane computes the pair's call of sub-step k and the odd lane that of sub-step k + 1, and each
+            // hands two words to its partner: every lane computes one call per two sub-steps, none idles.
+            uint32_t w_pos, w_acc;
+            if (lam == 1) {
+                w = philox4x32_10((uint32_t)T, (uint32_t)k, a.c2, a.c3, a.k0, a.k1);
+                w_pos = w.x;
+                w_acc = w.y;
+            } else {
+                if ((k & 1) == 0) {
+                    const int kk = k + (j & 1);                        // the odd lane works one sub-step ahead
+                    if (kk < q) w = philox4x32_10((uint32_t)T, (uint32_t)(kk * calls + (j >> 1)), a.c2, a.c3, a.k0, a.k1);
+                    const uint32_t pz = __shfl_xor_sync(0xffffffffu, w.z, 1), pw = __shfl_xor_sync(0xffffffffu, w.w, 1);
+                    w_pos = (j & 1) ? pz : w.x;                        // sub-step k: the even lane's call
+                    w_acc = (j & 1) ? pw : w.y;
+                } else {
+                    const uint32_t px_ = __shfl_xor_sync(0xffffffffu, w.x, 1), py_ = __shfl_xor_sync(0xffffffffu, w.y, 1);
+                    w_pos = (j & 1) ? w.z : px_;                       // sub-step k: the odd lane's call
+                    w_acc = (j & 1) ? w.w : py_;
+                }
+            }
             const int r = (int)__umulhi(w_pos, (uint32_t)P);
+            // Same site picked twice in this sub-step: the highest thread of the group wins (reading D19).  MATCH.ANY
+            // would find the collisions directly but costs as much as the rest of the sub-step (measured: 100 against
+            // 186 Gflips/s), and collisions are rare (lambda^2 / 2P per sub-step).  So every lane writes its index into
+            // a claim byte of the picked site; after the barrier a lane that reads back another index has collided,
+            // and only then is MATCH used.  Stale claim bytes cannot hide a collision: every lane overwrites its
+            // site's byte before it reads it.
+            if (lam > 1) sts_u8(s_claim + (uint32_t)r, (uint32_t)j);
             const int px = r & (b - 1), py = r >> a.lg_b;
             const int c = (px + py) & 1;                               // x0, y0 are even
-            uint8_t *const me = (tile + c * col_bytes) + py * rowb + (px >> 1);
-            const uint32_t own = *me;
-            const uint32_t north = (tile + (c ^ 1) * col_bytes)[(py + 1) * rowb + (px >> 1)];
-            const uint32_t est = (px + 1 < b) ? (tile + (c ^ 1) * col_bytes)[py * rowb + ((px + 1) >> 1)] : east[py];
+            const uint32_t me = s_tile + (uint32_t)(c * col_bytes + py * rowb + (px >> 1));
+            const uint32_t oth = s_tile + (uint32_t)((c ^ 1) * col_bytes + py * rowb);
+            const uint32_t own = lds_u8(me);
+            const uint32_t north = lds_u8(oth + (uint32_t)(rowb + (px >> 1)));
+            const uint32_t est = lds_u8((px + 1 < b) ? oth + (uint32_t)((px + 1) >> 1) : s_east + (uint32_t)py);
             uint32_t n_new = own & 1u;
             if ((north & est & 1u) != 0u) {                            // facilitated
                 if (METRO) {
-                    if ((own & 1u) != 0u || a.up_always || w_acc < a.thr_up) n_new ^= 1u;
+                    if ((own & 1u) != 0u || up_always || w_acc < thr_up) n_new ^= 1u;
                 } else {
-                    n_new = w_acc < a.thr_c ? 1u : 0u;
+                    n_new = w_acc < thr_c ? 1u : 0u;
                 }
             }
-            // same site picked twice in this sub-step: the highest thread of the group wins (reading D19)
-            const uint32_t same = __match_any_sync(0xffffffffu, (uint32_t)r | ((uint32_t)grp_in_warp << 16) |
-                                                                    (live ? 0u : 0x80000000u));
-            const bool winner = (same >> lane) == 1u;                  // no higher lane holds the same key
             __syncwarp();                                              // all picks have read the sub-step's start
-            if (live && winner && n_new != (own & 1u)) *me = (uint8_t)((own ^ 1u) | (a.track ? 0x08u : 0u));
+            bool winner = true;
+            if (lam > 1 && __any_sync(0xffffffffu, lds_u8(s_claim + (uint32_t)r) != (uint32_t)j)) {
+                const uint32_t same = __match_any_sync(0xffffffffu, (uint32_t)r | key_hi);
+                winner = (same >> lane) == 1u;                         // no higher lane holds the same key
+            }
+            if (live && winner && n_new != (own & 1u)) sts_u8(me, (own ^ 1u) | chg);
             __syncwarp();                                              // step 7
         }
         // ---- step 9: copy the tile back (interior only); count the up sites for the fused observable
         if (live) {
-            const int lanes_row = rowb >> 2;
-            for (int i = j; i < 2 * b * lanes_row; i += lam) {
-                const int c = i / (b * lanes_row), rem = i - c * b * lanes_row;
-                const int rr = rem / lanes_row, u = rem - rr * lanes_row;
+            const int lg_lr = a.lg_b - 3;
+            for (int i = j; i < (b << (lg_lr + 1)); i += lam) {
+                const int rr = i >> (lg_lr + 1), c = (i >> lg_lr) & 1, u = i & ((1 << lg_lr) - 1);
                 const uint32_t v = *reinterpret_cast<const uint32_t *>((tile + c * col_bytes) + rr * rowb + 4 * u);
                 *reinterpret_cast<uint32_t *>((c ? a.dst[1] : a.dst[0]) + (size_t)(y0 + rr) * a.Lh + (x0 >> 1) + 4 * u) = v;
                 ups += (int)__dp4a(v & 0x01010101u, 0x01010101u, 0u);
@@ -124,7 +167,10 @@ k_ne_random_tile(const __grid_constant__ NeTileArgs a)
 }
 
 // Shared memory of one tile (must match the kernel).
-static size_t ne_tile_bytes(int b) { return (size_t)((2 * (b + 1) * (b / 2) + b + 15) & ~15); }
+static size_t ne_tile_bytes(int b, int lam)
+{
+    return (size_t)((2 * (b + 1) * (b / 2) + b + (lam > 1 ? b * b : 0) + 15) & ~15);
+}
 
 bool ne_tile_supported(const Lat &lat, int b, int lam)
 {
@@ -132,14 +178,14 @@ bool ne_tile_supported(const Lat &lat, int b, int lam)
     if (b < 8 || b > 128 || (b & (b - 1)) != 0 || lat.L % b != 0) return false;
     if (lam < 1 || lam > 32 || (lam & (lam - 1)) != 0) return false;
     if ((b * b) % (2 * lam) != 0) return false;
-    return true;
+    return (32 / lam) * ne_tile_bytes(b, lam) <= 200 * 1024;   // one warp's tiles must fit shared memory
 }
 
 // Threads per CTA: as many tile groups as fit ~96 KB of shared memory (at least one warp).
 static int ne_tile_threads(int b, int lam)
 {
     int threads = 256;
-    while (threads > 32 && (threads / lam) * ne_tile_bytes(b) > 96 * 1024) threads >>= 1;
+    while (threads > 32 && (threads / lam) * ne_tile_bytes(b, lam) > 96 * 1024) threads >>= 1;
     return threads;
 }
 
@@ -170,7 +216,7 @@ cudaError_t launch_ne_random_tile(const Lat &lat, uint8_t *const dst[2], bool me
     a.obs = obs;
     const int threads = ne_tile_threads(b, lam);
     const int tiles_per_cta = threads / lam;
-    const size_t smem = tiles_per_cta * ne_tile_bytes(b);
+    const size_t smem = tiles_per_cta * ne_tile_bytes(b, lam);
     int grid = (a.ntiles + tiles_per_cta - 1) / tiles_per_cta;
     const int cap = sm_count() * 8;
     if (grid > cap) grid = cap;
