@@ -86,16 +86,15 @@ k_sweep_resident(const __grid_constant__ ResidentArgs a, const __grid_constant__
                  const __grid_constant__ typename TabOf<MODEL>::type tab)
 {
     __shared__ __align__(16) struct {
-        uint32_t t[16];
+        uint32_t t[MODEL == M_ISING_ONE ? 64 : 16];
         long long red[2][8];
-        uint2 e[MODEL == M_ISING_ONE ? 96 : 1];
     } sm;
     uint32_t s_t = (uint32_t)__cvta_generic_to_shared(sm.t);
     asm volatile("" : "+r"(s_t));
     if constexpr (MODEL == M_ISING_HALF) {
         if (threadIdx.x < 16) sm.t[threadIdx.x] = tab.t[threadIdx.x];
     } else if constexpr (MODEL == M_ISING_ONE) {
-        for (int i = threadIdx.x; i < 96; i += blockDim.x) sm.e[i] = tab.e[i];
+        for (int i = threadIdx.x; i < 64; i += blockDim.x) sm.t[i] = tab.t[i];
     }
     __syncthreads();
 
@@ -138,8 +137,7 @@ k_sweep_resident(const __grid_constant__ ResidentArgs a, const __grid_constant__
         }
         M.s_t = s_t;
         M.one = (uint32_t)a.g.one;
-        M.s_e = sm.e;
-        M.totU = M.totBN = 0;
+        M.totU = M.totBN = M.totS = 0;
         const int n = march_init(M, a.g, a.col[half], a.col[half ^ 1], half, seg, col, up);
         // The direction is a compile-time constant only where the rule needs it (North-East: north = y + 1).
         if (NE && !up) {
@@ -223,7 +221,7 @@ static cudaError_t dispatch(int model, int dims, bool track, int obs, int grid, 
     }
     case M_ISING_ONE: {
         OneTab ot;
-        for (int i = 0; i < 96; ++i) ot.e[i] = t.s1[i];
+        for (int i = 0; i < 64; ++i) ot.t[i] = t.s1[i];
         return dims == 3 ? launch_to<M_ISING_ONE, 3>(track, obs, grid, s, a, pk, ot, max_grid, bs)
                          : launch_to<M_ISING_ONE, 2>(track, obs, grid, s, a, pk, ot, max_grid, bs);
     }

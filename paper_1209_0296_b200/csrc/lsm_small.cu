@@ -31,16 +31,15 @@ k_sweep_small(const __grid_constant__ SmallArgs a, const __grid_constant__ Philo
               const __grid_constant__ typename TabOf<MODEL>::type tab)
 {
     __shared__ __align__(16) struct {
-        uint32_t t[16];
+        uint32_t t[MODEL == M_ISING_ONE ? 64 : 16];
         int acc[2][2];           // (B, M) of the sweep in flight, double-buffered by sweep parity
-        uint2 e[MODEL == M_ISING_ONE ? 96 : 1];
     } sm;
     uint32_t s_t = (uint32_t)__cvta_generic_to_shared(sm.t);
     asm volatile("" : "+r"(s_t));
     if constexpr (MODEL == M_ISING_HALF) {
         if (threadIdx.x < 16) sm.t[threadIdx.x] = tab.t[threadIdx.x];
     } else if constexpr (MODEL == M_ISING_ONE) {
-        if (threadIdx.x < 96) sm.e[threadIdx.x] = tab.e[threadIdx.x];
+        if (threadIdx.x < 64) sm.t[threadIdx.x] = tab.t[threadIdx.x];
     }
     if (threadIdx.x < 4) sm.acc[threadIdx.x >> 1][threadIdx.x & 1] = 0;
     __syncthreads();
@@ -68,8 +67,7 @@ k_sweep_small(const __grid_constant__ SmallArgs a, const __grid_constant__ Philo
         }
         M.s_t = s_t;
         M.one = (uint32_t)a.g.one;
-        M.s_e = sm.e;
-        M.totU = M.totBN = 0;
+        M.totU = M.totBN = M.totS = 0;
         int nsites = 0;
         if (active) {
             const int n = march_init(M, a.g, a.col[half], a.col[half ^ 1], half, seg, col, true);
@@ -115,16 +113,15 @@ k_sweep_small_lane(const __grid_constant__ SmallArgs a, const __grid_constant__ 
     const uint32_t rank = cluster.block_rank(), nrank = cluster.num_blocks();
 
     __shared__ __align__(16) struct {
-        uint32_t t[16];
+        uint32_t t[MODEL == M_ISING_ONE ? 64 : 16];
         int acc[2][2];           // this block's share of (B, M) of the sweep in flight, double-buffered
-        uint2 e[MODEL == M_ISING_ONE ? 96 : 1];
     } sm;
     uint32_t s_t = (uint32_t)__cvta_generic_to_shared(sm.t);
     asm volatile("" : "+r"(s_t));
     if constexpr (MODEL == M_ISING_HALF) {
         if (threadIdx.x < 16) sm.t[threadIdx.x] = tab.t[threadIdx.x];
     } else if constexpr (MODEL == M_ISING_ONE) {
-        if (threadIdx.x < 96) sm.e[threadIdx.x] = tab.e[threadIdx.x];
+        if (threadIdx.x < 64) sm.t[threadIdx.x] = tab.t[threadIdx.x];
     }
     if (threadIdx.x < 4) sm.acc[threadIdx.x >> 1][threadIdx.x & 1] = 0;
 
@@ -167,7 +164,7 @@ k_sweep_small_lane(const __grid_constant__ SmallArgs a, const __grid_constant__ 
         philox_half_consts(make_sweep_key(a.seed, t, (uint32_t)half), pk.rk0, pk.rk1, pc.x1, pc.y2, pc.z2, pc.w3);
         uint32_t *own = s_col[half];
         const uint32_t *oth = s_col[half ^ 1];
-        int totU = 0, totBN = 0, nsites = 0;
+        int totU = 0, totBN = 0, totS = 0, nsites = 0;
         if (half == 0) thrB = thrM = 0;
 #pragma unroll 1
         for (uint32_t li = threadIdx.x; li < nl; li += blockDim.x) {
@@ -201,11 +198,8 @@ k_sweep_small_lane(const __grid_constant__ SmallArgs a, const __grid_constant__ 
                     ns = p + n + c + sd;
                     if (DIMS == 3) ns += yp + yn;
                 }
-                int accB = 0, accM = 0;
-                out = rule_one<DIMS, TRACK, OBS>(o, ns, philox_sweep(2u * gl, pc), philox_sweep(2u * gl + 1u, pc), sm.e,
-                                                 accB, accM);
-                totU += accM;
-                totBN += accB;
+                out = rule_one<DIMS, TRACK, OBS>(o, ns, philox_sweep(2u * gl, pc), philox_sweep(2u * gl + 1u, pc), s_t, one,
+                                                 totU, totBN, totS);
             } else {
                 uint32_t accU = 0;
                 out = rule_ne<TRACK, MODEL == M_NE_METROPOLIS, OBS>(o, n, qq ? sd : c, gl, pc, ne_t32, ne_always, accU);
@@ -218,6 +212,7 @@ k_sweep_small_lane(const __grid_constant__ SmallArgs a, const __grid_constant__ 
             March<MODEL, DIMS, TRACK, OBS> M;          // only the per-thread sums are used
             M.totU = totU;
             M.totBN = totBN;
+            M.totS = totS;
             long long cB, cM;
             march_observables<MODEL, DIMS>(M, nsites, half == 1, cB, cM);
             thrB += (int)cB;                           // |B| <= 3N, |M| <= N with N <= 2^20: far below 2^31
@@ -398,7 +393,7 @@ cudaError_t launch_sweep_small(const Lat &lat, int model, int track, unsigned lo
     }
     case M_ISING_ONE: {
         OneTab ot;
-        for (int i = 0; i < 96; ++i) ot.e[i] = t.s1[i];
+        for (int i = 0; i < 64; ++i) ot.t[i] = t.s1[i];
         return lat.dims == 3 ? small_launch_to<M_ISING_ONE, 3>(tr, obs, plan.threads, s, a, pk, ot, lg_lpr, lg_L, plan.cluster)
                              : small_launch_to<M_ISING_ONE, 2>(tr, obs, plan.threads, s, a, pk, ot, lg_lpr, lg_L, plan.cluster);
     }

@@ -43,9 +43,8 @@ k_sweep_tiled(const __grid_constant__ TiledGeom g, const __grid_constant__ Philo
               const __grid_constant__ typename TabOf<MODEL>::type tab)
 {
     __shared__ __align__(16) struct {
-        uint32_t t[16];
+        uint32_t t[MODEL == M_ISING_ONE ? 64 : 16];
         long long red[2][8];
-        uint2 e[MODEL == M_ISING_ONE ? 96 : 1];
     } sm;
     // two-stage per-thread ring of the asynchronous copies (March::step_pf): N, O [, Yp, Yn] words and the edge lane
     // (spin-1 keeps the direct loads: its rule needs the registers the copies' addresses would take)
@@ -65,7 +64,7 @@ k_sweep_tiled(const __grid_constant__ TiledGeom g, const __grid_constant__ Philo
     if constexpr (MODEL == M_ISING_HALF) {
         if (threadIdx.x < 16) sm.t[threadIdx.x] = tab.t[threadIdx.x];
     } else if constexpr (MODEL == M_ISING_ONE) {
-        if (threadIdx.x < 96) sm.e[threadIdx.x] = tab.e[threadIdx.x];
+        if (threadIdx.x < 64) sm.t[threadIdx.x] = tab.t[threadIdx.x];
     } else {
         M.ne_t32 = tab.t32;
         M.ne_always = tab.always;
@@ -74,8 +73,7 @@ k_sweep_tiled(const __grid_constant__ TiledGeom g, const __grid_constant__ Philo
     asm volatile("griddepcontrol.wait;" ::: "memory");   // the previous launch's spins are visible from here on
     M.s_t = s_t;
     M.one = (uint32_t)g.one;
-    M.s_e = sm.e;
-    M.totU = M.totBN = 0;
+    M.totU = M.totBN = M.totS = 0;
     M.s_ring = (uint32_t)__cvta_generic_to_shared(ring) + threadIdx.x * 16u;
     M.s_ringE = (uint32_t)__cvta_generic_to_shared(ringE) + threadIdx.x * 4u;
 
@@ -122,13 +120,21 @@ void build_tiled_tables(int model, int dims, double J, double h, const uint64_t 
             }
     } else if (model == M_ISING_ONE) {
         t.usable = 1;
+        // canonical table: idx = ((a*2 + kk) * (4d+1) + sum), a' = (a + 1 + kk) % 3.  Classes of s' - s and one
+        // representative (a, kk) each; the others must carry the same thresholds.
+        const int W = 4 * d + 1;
+        const int rep[4][2] = {{0, 0}, {0, 1}, {1, 1}, {2, 0}};          // +1, +2, -1, -2
+        const int cls[3][2] = {{0, 1}, {0, 2}, {3, 2}};                  // dcode of (a, kk)
         for (int a = 0; a < 3; ++a)
             for (int kk = 0; kk < 2; ++kk)
-                for (int s = 0; s <= 4 * d; ++s) {
-                    uint64_t v = thr[(a * 2 + kk) * (4 * d + 1) + s];
-                    uint32_t ap = (uint32_t)((a + 1 + kk) % 3);
-                    t.s1[(a * 2 + kk) * 16 + s] = make_uint2(clip(v), ap | (v == ALWAYS ? 0x10u : 0u));
-                }
+                for (int s = 0; s < W; ++s)
+                    if (thr[(a * 2 + kk) * W + s] != thr[(rep[cls[a][kk]][0] * 2 + rep[cls[a][kk]][1]) * W + s]) t.usable = 0;
+        for (int c = 0; c < 4; ++c)
+            for (int s = 0; s < W; ++s) {
+                uint64_t v = thr[(rep[c][0] * 2 + rep[c][1]) * W + s];
+                if (v == 0) t.usable = 0;                  // "never" cannot be written as w <= thr-1
+                t.s1[c * 16 + s] = (uint32_t)(v - 1);
+            }
     } else {
         t.usable = 1;
         t.ne_t32[0] = clip(thr[0]);
@@ -225,7 +231,7 @@ cudaError_t launch_sweep_tiled(const SweepArgs &a, const TiledTables &t, cudaStr
     }
     case M_ISING_ONE: {
         OneTab ot;
-        for (int i = 0; i < 96; ++i) ot.e[i] = t.s1[i];
+        for (int i = 0; i < 64; ++i) ot.t[i] = t.s1[i];
         return d3 ? launch_track<M_ISING_ONE, 3>(track, obs_mode, grid, s, g, pc, ot)
                   : launch_track<M_ISING_ONE, 2>(track, obs_mode, grid, s, g, pc, ot);
     }

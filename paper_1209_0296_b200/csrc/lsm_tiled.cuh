@@ -16,8 +16,9 @@ struct TiledTables {
     // NE: [0] heat-bath / init threshold, [1] Metropolis 0->1 threshold (32-bit clipped) + flag
     uint32_t ne_t32[2];
     int ne_up_always;
-    // spin-1: entry[(a*2+kk)*16 + sum] = { thr clipped to 32 bits, proposed a' | (thr == 2^32) << 4 }
-    uint2 s1[96];
+    // spin-1: s1[16*dcode + sum] = thr - 1 (accept iff w1 <= s1), dcode = class of s' - s: 0: +1, 1: +2, 2: -1, 3: -2;
+    //   sum = sum of the neighbours' a = s + 1.  The threshold depends on (s' - s, sum) only (reading D3).
+    uint32_t s1[64];
 };
 
 void build_tiled_tables(int model, int dims, double J, double h, const uint64_t *thr, int nthr, TiledTables *out);

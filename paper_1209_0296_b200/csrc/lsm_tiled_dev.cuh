@@ -8,9 +8,9 @@
 #define LSM_TILED_MINBLOCKS 4
 #endif
 
-// spin-1 needs two Philox calls and 64-bit table entries per lane: 3 CTAs per SM (85 registers) avoid its spills
+// spin-1 needs two Philox calls per lane; measured 2/3/4 CTAs per SM: 518/478/414 Gflips/s on cfg4
 #ifndef LSM_TILED_MINBLOCKS_ONE
-#define LSM_TILED_MINBLOCKS_ONE 3
+#define LSM_TILED_MINBLOCKS_ONE 2
 #endif
 // spin-1/2 Ising: the march is bound by pipe issue, not by latency (4 independent Philox chains per thread), and runs
 // fastest with 2 CTAs per SM and up to 128 registers (measured 1/2/3/4/5/6 CTAs: 1132/1163/1141/1120/1027/970
@@ -125,7 +125,7 @@ struct TiledGeom {
 
 struct HalfTab { uint32_t t[16]; };            // spin-1/2: t[n + 8*b] = thr - 1  (accept iff w <= t)
 struct NeTab { uint32_t t32; int always; };
-struct OneTab { uint2 e[96]; };
+struct OneTab { uint32_t t[64]; };            // spin-1: t[16*dcode + sum] = thr - 1, dcode = class of s' - s
 template <int MODEL> struct TabOf { using type = NeTab; };
 template <> struct TabOf<M_ISING_HALF> { using type = HalfTab; };
 template <> struct TabOf<M_ISING_ONE> { using type = OneTab; };
@@ -206,27 +206,72 @@ __device__ __forceinline__ uint32_t rule_ne(uint32_t own, uint32_t north, uint32
     return (own & ~0x01010101u) | n2 | (f << 3);
 }
 
-// Ising spin-1 (reading D5): two words per site, so a lane needs two Philox calls.
-template <int DIMS, bool TRACK, int OBS>
-__device__ __forceinline__ uint32_t rule_one(uint32_t own, uint32_t nsum, uint4 ra, uint4 rb, const uint2 *s_e,
-                                             int &accB, int &accM)
+// Ising spin-1 (reading D5): two words per site, so a lane needs two Philox calls (ra: sites 0, 1; rb: sites 2, 3;
+// proposal word w0 = x / z, acceptance word w1 = y / w).  Byte-parallel over the 4 sites of the lane:
+//   kk = msb(w0)                      -> byte mask (PRMT with sign replication)
+//   proposal a' = (a + 1 + kk) mod 3  -> x = a ^ a' is a boolean function of (a1, a0, kk): two LOP3 + one bit-select
+//   threshold                         -> depends on (s' - s, sum) only (D3, no single-ion term): the four classes
+//                                        d = 0: +1, 1: +2, 2: -1, 3: -2 are again boolean functions of (a1, a0, kk);
+//                                        table byte offset 64 d + 4 sum <= 240 fits the per-site byte of one word
+//   accept iff w1 <= thr - 1          -> per site: extract, LDS, ISETP, predicated IMAD (as in rule_half)
+// Observables: raw sums SA = sum a', SAS = sum a' * sum, SS = sum of sums (IDP.4A); march_observables converts.
+__device__ __forceinline__ uint32_t prmt(uint32_t a, uint32_t b, uint32_t sel)
 {
-    const uint32_t w0[4] = {ra.x, ra.z, rb.x, rb.z};
-    const uint32_t w1[4] = {ra.y, ra.w, rb.y, rb.w};
-    uint32_t nw = own;
-#pragma unroll
-    for (int k = 0; k < 4; ++k) {
-        uint32_t a = (own >> (8 * k)) & 3u;
-        uint32_t sum = (nsum >> (8 * k)) & 0xFu;
-        uint32_t kk = w0[k] >> 31;
-        uint2 e = s_e[((a * 2u + kk) << 4) | sum];
-        bool acc = (w1[k] < e.x) || (e.y & 0x10u);
-        uint32_t a2 = acc ? (e.y & 3u) : a;
-        uint32_t x = a ^ a2;                               // change of the two value bits
-        nw ^= x << (8 * k);
-        if (TRACK && x != 0u) nw |= 0x10u << (8 * k);      // "ever changed"
-        if (OBS >= 1) accM += (int)a2 - 1;
-        if (OBS >= 2) accB += ((int)a2 - 1) * ((int)sum - 2 * DIMS);
+    uint32_t r;
+    asm("prmt.b32 %0, %1, %2, %3;" : "=r"(r) : "r"(a), "r"(b), "r"(sel));
+    return r;
+}
+// boolean functions of (A, B, C) evaluated bitwise by one LOP3
+template <int LUT> __device__ __forceinline__ uint32_t lop3(uint32_t a, uint32_t b, uint32_t c)
+{
+    uint32_t r;
+    asm("lop3.b32 %0, %1, %2, %3, %4;" : "=r"(r) : "r"(a), "r"(b), "r"(c), "n"(LUT));
+    return r;
+}
+// LUT of f(A, B, C): bit (4A + 2B + C) of the constant
+__host__ __device__ constexpr int lut3(bool f000, bool f001, bool f010, bool f011, bool f100, bool f101, bool f110, bool f111)
+{
+    return (f000 ? 1 : 0) | (f001 ? 2 : 0) | (f010 ? 4 : 0) | (f011 ? 8 : 0) | (f100 ? 16 : 0) | (f101 ? 32 : 0) |
+           (f110 ? 64 : 0) | (f111 ? 128 : 0);
+}
+
+template <int DIMS, bool TRACK, int OBS>
+__device__ __forceinline__ uint32_t rule_one(uint32_t own, uint32_t nsum, uint4 ra, uint4 rb, uint32_t s_t, uint32_t one,
+                                             int &totSA, int &totSAS, int &totSS)
+{
+    // kk byte mask: 0xFF where the proposal word's top bit is set
+    // (inline PTX: __byte_perm() drops bit 3 of the selector nibbles, the "replicate the sign" flag)
+    const uint32_t klo = prmt(ra.x, ra.z, 0x00FBu), khi = prmt(rb.x, rb.z, 0x00FBu);
+    const uint32_t kk = prmt(klo, khi, 0x5410u);
+    const uint32_t dn = own >> 1, up = own << 1;           // a1 at bit 0 / a0 at bit 1 of every byte
+    // at bit 0: A = a0 (own), B = a1 (own >> 1), C = kk.   rows: (a0, a1, kk)
+    //   x0 = bit 0 of a ^ a':  a=0: !kk ; a=1 (a0=1,a1=0): 1 ; a=2 (a0=0,a1=1): kk
+    //   d0 = bit 0 of dcode :  a=0: kk  ; a=1: 0 ; a=2: !kk
+    constexpr int X0 = lut3(true, false, false, true, true, true, false, false);
+    constexpr int D0 = lut3(false, true, true, false, false, false, false, false);
+    // at bit 1: A = a1 (own), B = a0 (own << 1), C = kk.   rows: (a1, a0, kk)
+    //   x1 = bit 1 of a ^ a':  a=0: kk ; a=1 (a1=0,a0=1): !kk ; a=2 (a1=1,a0=0): 1
+    //   d1 = bit 1 of dcode :  a=0: 0  ; a=1: kk ; a=2: 1
+    constexpr int X1 = lut3(false, true, true, false, true, true, false, false);
+    constexpr int D1 = lut3(false, false, false, true, true, true, false, false);
+    const uint32_t x = lop3<0xCA>(0x01010101u, lop3<X0>(own, dn, kk), lop3<X1>(own, up, kk));   // bit 0 | bit 1 (select)
+    const uint32_t d = lop3<0xCA>(0x01010101u, lop3<D0>(own, dn, kk), lop3<D1>(own, up, kk)) & 0x03030303u;
+    const uint32_t adr = d * 64u + nsum * 4u;              // byte offset of t[16 d + sum], per site byte
+    uint32_t acc = 0u;                                     // 0xFF in the byte of every accepted site
+    acc = add_if_le<0x000000FFu>(acc, ra.y, lds_u32(s_t, adr & 0xFFu), one);
+    acc = add_if_le<0x0000FF00u>(acc, ra.w, lds_u32(s_t, __byte_perm(adr, 0u, 0x4441)), one);
+    acc = add_if_le<0x00FF0000u>(acc, rb.y, lds_u32(s_t, __byte_perm(adr, 0u, 0x4442)), one);
+    acc = add_if_le<0xFF000000u>(acc, rb.w, lds_u32(s_t, adr >> 24), one);
+    const uint32_t fl = x & acc & 0x03030303u;             // change of the two value bits
+    uint32_t nw = own ^ fl;
+    if (TRACK) nw |= ((fl | (fl >> 1)) & 0x01010101u) << 4;    // "ever changed"
+    if (OBS >= 1) {
+        const uint32_t a2 = TRACK ? (nw & 0x03030303u) : nw;
+        totSA = (int)__dp4a(a2, 0x01010101u, (uint32_t)totSA);
+        if (OBS >= 2) {
+            totSAS = (int)__dp4a(a2, nsum, (uint32_t)totSAS);
+            totSS = (int)__dp4a(nsum, 0x01010101u, (uint32_t)totSS);
+        }
     }
     return nw;
 }
@@ -246,9 +291,8 @@ struct March {
     int m, q;
     int e_hi, e_lo, dyp, dyn, rowstride, m_wrap, mstep;
     long long wrapw;
-    int totU, totBN;        // per-thread sums; < 2^31 for every legal lattice
+    int totU, totBN, totS;  // per-thread sums; < 2^31 for every legal lattice (spin-1: sum a', sum a' * sum, sum of sums)
     uint32_t s_t, one;
-    const uint2 *s_e;
     uint32_t ne_t32;
     int ne_always;
 
@@ -296,7 +340,6 @@ struct March {
                 out[d] = rule_half<TRACK, OBS>(o[d], ns, r, s_t, one, totU, totBN);
             }
         } else if (MODEL == M_ISING_ONE) {
-            int accB = 0, accM = 0;
 #pragma unroll
             for (int d = 0; d < 4; ++d) {
                 uint32_t ns;
@@ -310,10 +353,8 @@ struct March {
                 }
                 uint4 ra = philox_sweep(2u * (grp + d), pc);
                 uint4 rb = philox_sweep(2u * (grp + d) + 1u, pc);
-                out[d] = rule_one<DIMS, TRACK, OBS>(o[d], ns, ra, rb, s_e, accB, accM);
+                out[d] = rule_one<DIMS, TRACK, OBS>(o[d], ns, ra, rb, s_t, one, totU, totBN, totS);
             }
-            totU += accM;
-            totBN += accB;
         } else {
             uint32_t accU = 0;
 #pragma unroll
@@ -588,8 +629,9 @@ __device__ __forceinline__ void march_observables(const March<MODEL, DIMS, TRACK
         cB = -4LL * DIMS * M.totU;
         if (second) cB += 4LL * M.totBN + 2LL * DIMS * nsites;
     } else if (MODEL == M_ISING_ONE) {
-        cM = M.totU;
-        if (second) cB = M.totBN;
+        // s' = a' - 1, nn = sum - 2d:  M = SA - n;  B = sum s' nn = SAS - 2d SA - SS + 2d n   (second colour only)
+        cM = (long long)M.totU - nsites;
+        if (second) cB = (long long)M.totBN - 2LL * DIMS * M.totU - M.totS + 2LL * DIMS * nsites;
     } else {
         cM = M.totU;
     }
