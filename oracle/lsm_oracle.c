@@ -417,6 +417,86 @@ int orc_sweep_random_tile(orc_t *o, int64_t n, int b, int lambda, int tiles_desc
     return 0;
 }
 
+/* The balance-preserving variant of the algorithm above: "The only changes are in steps 6-9:
+ *   6. lambda threads concurrently pick lambda red spins from the sub-lattice randomly and update them.
+ *   7. Synchronize the block and pick lambda white spins from the sub-lattice randomly and update them.
+ *   8. Copy back ...  9. Relaunch ... and redo steps 6-8 three more times (this will complete one MC step)."
+ * Readings (D22-D24):
+ *   D22 red / white = the two checkerboard colours (x+y)&1 = 0 / 1 (Fig. 4 is absent; these are the two sets
+ *       whose members never read each other under the north-east rule, which is what restores balance).
+ *   D23 one MC step = 4 launches; a launch runs q sub-steps of (lambda red picks, barrier, lambda white picks,
+ *       barrier) with q * 2 lambda = P/4, so that the step attempts P updates per tile like the base algorithm
+ *       (twice the launches, tile copies and barriers for the same attempts: the paper's "~2.5x slower").
+ *   D24 thread j of sub-step k draws ONE Philox call: counter c0 = tile id, c1 = k*lambda + j, c2 = lo32(t),
+ *       c3 = (8 + launch) | hi32(t)<<2; words 0, 1 = position and acceptance of its red pick, words 2, 3 of its
+ *       white pick.  Position: r = floor(w_pos * (P/2) / 2^32) is the r-th site of that colour in the tile in
+ *       row-major order: py = r div (b/2), px = 2 (r mod (b/2)) + ((py + colour) & 1)   (tile origins are even).
+ *   D18 (boundaries frozen at launch start), D19 (picks of a phase read the phase's start; highest thread
+ *       wins a same-site collision) and the rule of D7 are unchanged.                                        */
+int orc_sweep_random_tile_balanced(orc_t *o, int64_t n, int b, int lambda, int tiles_descending)
+{
+    if (o->model != ORC_NE_HEATBATH && o->model != ORC_NE_METROPOLIS) return -1;
+    int L = o->L;
+    if (b < 2 || (b & 1) || L % b != 0 || lambda < 1) return -1;
+    int P = b * b;
+    if (P % (8 * lambda) != 0) return -1;
+    int q = P / (8 * lambda), nt = L / b, hb = b / 2;
+    int8_t *start = (int8_t *)malloc((size_t)o->N);
+    int *site = (int *)malloc(sizeof(int) * (size_t)lambda);
+    int *val = (int *)malloc(sizeof(int) * (size_t)lambda);
+    if (!start || !site || !val) { free(start); free(site); free(val); return -2; }
+    uint32_t key[2] = {(uint32_t)o->seed, (uint32_t)(o->seed >> 32)};
+    for (int64_t it = 0; it < n; ++it) {
+        for (uint32_t launch = 0; launch < 4; ++launch) {
+            memcpy(start, o->s, (size_t)o->N);
+            for (int tt = 0; tt < nt * nt; ++tt) {
+                int T = tiles_descending ? nt * nt - 1 - tt : tt;
+                int tx = T % nt, ty = T / nt, x0 = tx * b, y0 = ty * b;
+                for (int k = 0; k < q; ++k) {
+                    for (int colour = 0; colour < 2; ++colour) {      /* red picks, barrier, white picks, barrier */
+                        for (int j = 0; j < lambda; ++j) {
+                            uint32_t ctr[4], w[4];
+                            ctr[0] = (uint32_t)T;
+                            ctr[1] = (uint32_t)(k * lambda + j);
+                            ctr[2] = (uint32_t)o->t;
+                            ctr[3] = (8u + launch) | ((uint32_t)(o->t >> 32) << 2);
+                            orc_philox4x32_10(ctr, key, w);
+                            uint32_t w_pos = w[2 * colour], w_acc = w[2 * colour + 1];
+                            int r = (int)(((uint64_t)w_pos * (uint64_t)(P / 2)) >> 32);
+                            int py = r / hb, px = 2 * (r % hb) + ((py + colour) & 1);
+                            int x = x0 + px, y = y0 + py;
+                            int north = (py + 1 < b) ? o->s[site_id(o, x, y + 1, 0)] : start[site_id(o, x, wrap(y + 1, L), 0)];
+                            int east = (px + 1 < b) ? o->s[site_id(o, x + 1, y, 0)] : start[site_id(o, wrap(x + 1, L), y, 0)];
+                            int64_t i = site_id(o, x, y, 0);
+                            int s_old = o->s[i], s_new = s_old;
+                            if (north == 1 && east == 1) {
+                                if (o->model == ORC_NE_HEATBATH) {
+                                    s_new = ((uint64_t)w_acc < o->thr[0]) ? 1 : 0;
+                                } else {
+                                    uint64_t thr = (s_old == 0) ? o->thr[1] : o->thr[2];
+                                    if ((uint64_t)w_acc < thr) s_new = 1 - s_old;
+                                }
+                            }
+                            site[j] = (int)i;
+                            val[j] = s_new;
+                        }
+                        for (int j = 0; j < lambda; ++j) {
+                            int dup = 0;
+                            for (int j2 = j + 1; j2 < lambda; ++j2) dup |= (site[j2] == site[j]);
+                            if (dup) continue;
+                            if (val[j] != o->s[site[j]]) o->changed[site[j]] = 1;
+                            o->s[site[j]] = (int8_t)val[j];
+                        }
+                    }
+                }
+            }
+        }
+        o->t += 1;
+    }
+    free(start); free(site); free(val);
+    return 0;
+}
+
 /* obs[2*k] = B (= 0), obs[2*k+1] = M after sweep k of this call. */
 void orc_measure(const orc_t *o, int64_t *B, int64_t *M);
 int orc_sweep_random_tile_record(orc_t *o, int64_t n, int b, int lambda, int64_t *obs)

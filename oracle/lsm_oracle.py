@@ -72,6 +72,8 @@ def lib():
         L.orc_philox4x32_10.argtypes = [vp, vp, vp]
         L.orc_sweep_random_tile.restype = i32
         L.orc_sweep_random_tile.argtypes = [vp, i64, i32, i32, i32]
+        L.orc_sweep_random_tile_balanced.restype = i32
+        L.orc_sweep_random_tile_balanced.argtypes = [vp, i64, i32, i32, i32]
         L.orc_sweep_random_tile_record.restype = i32
         L.orc_sweep_random_tile_record.argtypes = [vp, i64, i32, i32, vp]
         _lib = L
@@ -120,6 +122,11 @@ class Oracle:
         """The paper's corrected North-East algorithm (readings D17-D21)."""
         if lib().orc_sweep_random_tile(self._h, int(n), int(b), int(lam), 1 if tiles_descending else 0) != 0:
             raise ValueError("random-tile schedule: NE model, b | L and 2*lambda | b*b required")
+
+    def sweep_random_tile_balanced(self, n=1, b=32, lam=16, tiles_descending=False):
+        """The balance-preserving variant (readings D22-D24): colour-restricted picks, 4 launches."""
+        if lib().orc_sweep_random_tile_balanced(self._h, int(n), int(b), int(lam), 1 if tiles_descending else 0) != 0:
+            raise ValueError("balanced random-tile schedule: NE model, even b | L and 8*lambda | b*b required")
 
     def sweep_random_tile_record(self, n, b=32, lam=16):
         obs = np.zeros((int(n), 2), dtype=np.int64)

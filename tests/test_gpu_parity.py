@@ -360,3 +360,14 @@ def test_random_tile_schedule_rejections():
     with pytest.raises(lsm.LsmError) as e:
         ising.sweep_random_tile(1, 32, 16)
     assert e.value.code == lsm.ERR_UNSUPPORTED
+
+
+def test_random_tile_schedule_full_size_prefix():
+    """BASELINE.json config 5 lattice (8192^2, c = 0.30) under the paper's corrected algorithm in its best configuration
+    (32 x 32 tiles, lambda = 16: 65 536 tiles, many waves of CTAs): first sweep, element by element."""
+    w = W.configs()["cfg5_c0.30"]
+    lat, orc = make_pair(**w.create_args())
+    got = lat.sweep_random_tile(1, 32, 16, record=True).cpu().numpy()
+    want = orc.sweep_random_tile_record(1, 32, 16)
+    assert np.array_equal(got, want)
+    assert_same_state(lat, orc)

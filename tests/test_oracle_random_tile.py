@@ -183,3 +183,92 @@ def test_rejects_bad_schedules():
     i = O.Oracle(2, 64, T=2.0, seed=1)
     with pytest.raises(ValueError):
         i.sweep_random_tile(1, 32, 16)      # Ising: the schedule belongs to the North-East model
+
+
+# ------------------------------------------------------------------ NEXT-2: the balance-preserving variant
+def reference_sweep_balanced(n, L, b, lam, seed, t, thr, metropolis):
+    """PAPER.md:148-158 on a dict keyed by (x, y): 4 launches; a sub-step = lam picks among the tile's red sites
+    ((x+y) even), then lam picks among its white sites; one Philox call per thread and sub-step (D22-D24)."""
+    key = (seed & 0xFFFFFFFF, seed >> 32)
+    P, nt = b * b, L // b
+    q = P // (8 * lam)
+    changed = set()
+    for launch in range(4):
+        at_start = dict(n)
+        for T in range(nt * nt):
+            tx, ty = T % nt, T // nt
+            sites = {col: [(tx * b + px, ty * b + py) for py in range(b) for px in range(b) if (px + py) % 2 == col]
+                     for col in (0, 1)}                                # row-major list of each colour's sites
+            for k in range(q):
+                for col in (0, 1):
+                    writes = {}
+                    for j in range(lam):
+                        w = philox_py((T, k * lam + j, t & 0xFFFFFFFF, (8 + launch) | ((t >> 32) << 2)), key)
+                        w_pos, w_acc = w[2 * col], w[2 * col + 1]
+                        x, y = sites[col][(w_pos * (P // 2)) >> 32]
+                        nb = []
+                        for (xx, yy) in ((x, y + 1), (x + 1, y)):
+                            ins = tx * b <= xx < (tx + 1) * b and ty * b <= yy < (ty + 1) * b
+                            nb.append(n[(xx, yy)] if ins else at_start[(xx % L, yy % L)])
+                        new = n[(x, y)]
+                        if nb == [1, 1]:
+                            if metropolis:
+                                if new == 1 or w_acc < thr[1]:
+                                    new = 1 - new
+                            else:
+                                new = 1 if w_acc < thr[0] else 0
+                        writes[(x, y)] = new
+                    for site, v in writes.items():
+                        if n[site] != v:
+                            changed.add(site)
+                        n[site] = v
+    return changed
+
+
+@pytest.mark.parametrize("model", [O.NE_HEATBATH, O.NE_METROPOLIS])
+@pytest.mark.parametrize("L,b,lam", [(8, 4, 2), (16, 8, 8), (12, 4, 1), (16, 16, 4), (24, 12, 2)])
+def test_balanced_matches_the_dict_restatement(model, L, b, lam):
+    c = 0.45
+    o = O.Oracle(2, L, model=model, J=0.0, T=T_of_c(c), seed=(78 << 32) + 5 * L + b)
+    thr = o.thresholds()
+    s = o.get_spins().reshape(L, L)
+    n = {(x, y): int(s[y, x]) for y in range(L) for x in range(L)}
+    ever = set()
+    for t in range(6):
+        ever |= reference_sweep_balanced(n, L, b, lam, o.seed, t, thr, model == O.NE_METROPOLIS)
+        o.sweep_random_tile_balanced(1, b, lam)
+        got = o.get_spins().reshape(L, L)
+        want = np.array([[n[(x, y)] for x in range(L)] for y in range(L)], dtype=np.int8)
+        assert np.array_equal(got, want), (t, np.argwhere(got != want)[:4])
+        assert o.persistence()[0] == L * L - len(ever)
+    assert len(ever) > 0 and o.sweeps_done == 6
+
+
+def test_balanced_tile_order_measure_and_persistence():
+    """Tile order immaterial (D18); product measure stationary; one MC step attempts P updates per tile (D23), so the
+    first-step persistence follows the same closed form as the base algorithm with Binomial(P/2, 2/P) picks per site
+    (each launch draws P/4 picks uniformly from the P/2 sites of each colour... a site of either colour is picked
+    P/2 times with probability 2/P in total)."""
+    c, L, b, lam = 0.30, 256, 32, 16
+    N, P = L * L, b * b
+    kw = dict(dims=2, L=L, model=O.NE_HEATBATH, J=0.0, T=T_of_c(c), seed=5150)
+    a, d = O.Oracle(**kw), O.Oracle(**kw)
+    a.sweep_random_tile_balanced(1, b, lam)
+    d.sweep_random_tile_balanced(1, b, lam, tiles_descending=True)
+    assert np.array_equal(a.get_spins(), d.get_spins()) and a.persistence() == d.persistence()
+    K = P // 2                                                         # picks that can hit a given site, each w.p. 2/P
+    want = 1 - c * c * (1 - (c * (1 - (1 - c) * 2 / P) ** K + (1 - c) * (1 - c * 2 / P) ** K))
+    sigma = math.sqrt(want * (1 - want) / N)
+    assert abs(a.persistence()[0] / N - want) < 5 * sigma
+    s = math.sqrt(c * (1 - c) / N)
+    for _ in range(20):
+        a.sweep_random_tile_balanced(1, b, lam)
+        assert abs(a.measure_int()[1] / N - c) < 4 * s
+
+
+def test_balanced_rejects_bad_schedules():
+    o = O.Oracle(2, 64, model=O.NE_HEATBATH, J=0.0, T=1.0, seed=1)
+    with pytest.raises(ValueError):
+        o.sweep_random_tile_balanced(1, 32, 3)     # 8*lambda does not divide P
+    with pytest.raises(ValueError):
+        o.sweep_random_tile_balanced(1, 24, 2)     # b does not divide L
