@@ -379,6 +379,15 @@ def other_workloads(lsm, torch, skip):
                 s_rt = e0.elapsed_time(e1) * 1e-3
                 out[name + "_random_tile_b32_lambda16"] = {"gflips": w.N * n_rt / s_rt / 1e9,
                                                            "us_per_sweep": s_rt / n_rt * 1e6, "launches_per_sweep": 2}
+                lat.sweep_random_tile(n_rt, 32, 16, out=obs, balanced=True)
+                torch.cuda.synchronize()
+                e0.record()
+                lat.sweep_random_tile(n_rt, 32, 16, out=obs, balanced=True)   # balance-preserving variant
+                e1.record()
+                torch.cuda.synchronize()
+                s_rt = e0.elapsed_time(e1) * 1e-3
+                out[name + "_random_tile_balanced_b32_lambda16"] = {"gflips": w.N * n_rt / s_rt / 1e9,
+                                                                    "us_per_sweep": s_rt / n_rt * 1e6, "launches_per_sweep": 4}
             lat.close()
             del lat, obs
         except Exception as e:  # a secondary workload must not take the headline down

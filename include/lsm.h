@@ -106,6 +106,13 @@ int lsm_sweep_record_host(lsm_t *, int64_t n, int64_t *h_obs, int64_t *d_scratch
  * UNSUPPORTED unless tile_edge is a power of two in [8, 128] dividing L, lambda a power of two in [1, 32] and
  * 2 * lambda divides P.  Shares the sweep counter with lsm_sweep. */
 int lsm_sweep_random_tile(lsm_t *, int64_t n, int tile_edge, int lambda, int64_t *d_obs, void *stream);
+/* Its balance-preserving variant ("~2.5x slower"): a sub-step is lambda picks among the tile's red
+ * sites, a barrier, lambda picks among its white sites, a barrier; four launches complete one MC step.  Readings
+ * D22-D24: red / white = checkerboard colours (x+y)&1 = 0 / 1; q * 2 lambda = P/4 per launch, so a step attempts P
+ * updates per tile; one Philox call per thread and sub-step, counter (tile, sub-step * lambda + thread, sweep,
+ * 8 + launch), words 0, 1 = red pick, 2, 3 = white pick; position r = floor(w P/2 / 2^32) = r-th site of the colour
+ * in row-major order.  UNSUPPORTED unless additionally 8 * lambda divides P. */
+int lsm_sweep_random_tile_balanced(lsm_t *, int64_t n, int tile_edge, int lambda, int64_t *d_obs, void *stream);
 
 /* Running observables of the current configuration (synchronises). */
 int lsm_measure(lsm_t *, double *E, int64_t *M);

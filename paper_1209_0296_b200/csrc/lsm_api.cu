@@ -275,11 +275,11 @@ extern "C" int lsm_sweep_record(lsm_t *o, int64_t n, int64_t *d_obs, void *strea
 
 // The paper's corrected North-East algorithm: two launches per sweep, each reading one
 // lattice buffer and writing the other (reading D18).
-extern "C" int lsm_sweep_random_tile(lsm_t *o, int64_t n, int tile_edge, int lambda, int64_t *d_obs, void *stream)
+static int random_tile_impl(lsm_t *o, int64_t n, int tile_edge, int lambda, int64_t *d_obs, void *stream, bool balanced)
 {
     if (!o || n < 0) return LSM_ERR_ARG;
     if (o->model != M_NE_HEATBATH && o->model != M_NE_METROPOLIS) return LSM_ERR_UNSUPPORTED;
-    if (!ne_tile_supported(o->lat, tile_edge, lambda)) return LSM_ERR_UNSUPPORTED;
+    if (!ne_tile_supported(o->lat, tile_edge, lambda, balanced)) return LSM_ERR_UNSUPPORTED;
     cudaStream_t s = (cudaStream_t)stream;
     o->last_stream = s;
     if (n == 0) return LSM_OK;
@@ -290,10 +290,11 @@ extern "C" int lsm_sweep_random_tile(lsm_t *o, int64_t n, int tile_edge, int lam
     else CU(cudaMemsetAsync(o->d_run, 0, 16, s));
     for (int64_t k = 0; k < n; ++k) {
         long long *obs = d_obs ? (long long *)d_obs + 2 * k : (k == n - 1 ? o->d_run : nullptr);
-        for (int launch = 0; launch < 2; ++launch) {
-            CU(launch_ne_random_tile(o->lat, o->alt, o->model == M_NE_METROPOLIS, tile_edge, lambda, o->seed, o->t,
+        const int nlaunch = balanced ? 4 : 2;                       // reading D23 / D17
+        for (int launch = 0; launch < nlaunch; ++launch) {
+            CU(launch_ne_random_tile(o->lat, o->alt, o->model == M_NE_METROPOLIS, balanced, tile_edge, lambda, o->seed, o->t,
                                      launch, thr_c, thr_up, o->thr[1] >= ALWAYS ? 1 : 0, o->tracking,
-                                     launch == 1 ? obs : nullptr, s));
+                                     launch == nlaunch - 1 ? obs : nullptr, s));
             o->launches += 1;
             for (int c = 0; c < 2; ++c) { uint8_t *tmp = o->lat.col[c]; o->lat.col[c] = o->alt[c]; o->alt[c] = tmp; }
         }
@@ -301,6 +302,17 @@ extern "C" int lsm_sweep_random_tile(lsm_t *o, int64_t n, int tile_edge, int lam
     }
     if (d_obs) CU(cudaMemcpyAsync(o->d_run, (long long *)d_obs + 2 * (n - 1), 16, cudaMemcpyDeviceToDevice, s));
     return LSM_OK;
+}
+
+extern "C" int lsm_sweep_random_tile(lsm_t *o, int64_t n, int tile_edge, int lambda, int64_t *d_obs, void *stream)
+{
+    return random_tile_impl(o, n, tile_edge, lambda, d_obs, stream, false);
+}
+
+// The balance-preserving variant: colour-restricted picks, four launches per MC step.
+extern "C" int lsm_sweep_random_tile_balanced(lsm_t *o, int64_t n, int tile_edge, int lambda, int64_t *d_obs, void *stream)
+{
+    return random_tile_impl(o, n, tile_edge, lambda, d_obs, stream, true);
 }
 
 extern "C" int lsm_sweep_record_host(lsm_t *o, int64_t n, int64_t *h_obs, int64_t *d_scratch, void *stream)

@@ -161,8 +161,8 @@ cudaError_t launch_philox_throughput(int blocks, int calls, uint32_t *d_sink, cu
 cudaError_t launch_pipe_probe(int mode, int blocks, int iters, uint32_t *d_sink, cudaStream_t s);
 
 // North-East random-tile schedule (lsm_ne_tile.cu): reads lat.col, writes dst.
-bool ne_tile_supported(const Lat &lat, int b, int lam);
-cudaError_t launch_ne_random_tile(const Lat &lat, uint8_t *const dst[2], bool metropolis, int b, int lam,
+bool ne_tile_supported(const Lat &lat, int b, int lam, bool balanced);
+cudaError_t launch_ne_random_tile(const Lat &lat, uint8_t *const dst[2], bool metropolis, bool balanced, int b, int lam,
                                   unsigned long long seed, unsigned long long t, int launch, uint32_t thr_c,
                                   uint32_t thr_up, int up_always, int track, long long *obs, cudaStream_t s);
 

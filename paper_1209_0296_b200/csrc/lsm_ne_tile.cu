@@ -44,7 +44,7 @@ __device__ __forceinline__ void sts_u8(uint32_t a, uint32_t v)
     asm volatile("st.shared.u8 [%0], %1;" ::"r"(a), "r"(v) : "memory");
 }
 
-template <bool METRO>
+template <bool METRO, bool BAL>
 __global__ void __launch_bounds__(256)
 k_ne_random_tile(const __grid_constant__ NeTileArgs a)
 {
@@ -64,7 +64,7 @@ k_ne_random_tile(const __grid_constant__ NeTileArgs a)
                    s_claim = s_east + (uint32_t)b;
     const uint32_t chg = a.track ? 0x08u : 0u, thr_c = a.thr_c, thr_up = a.thr_up;
     const bool up_always = a.up_always != 0;
-    const int q = P >> (a.lg_lam + 1), calls = (lam + 1) >> 1;
+    const int q = BAL ? P >> (a.lg_lam + 3) : P >> (a.lg_lam + 1), calls = (lam + 1) >> 1;   // D23 / D17
     int ups = 0;
 
     for (int base = warp_global * grp_per_warp; base < a.ntiles; base += nwarps * grp_per_warp) {
@@ -92,40 +92,14 @@ k_ne_random_tile(const __grid_constant__ NeTileArgs a)
             }
         }
         __syncwarp();
-        // ---- steps 6-8: q sub-steps of lambda simultaneous random picks
-        uint4 w = make_uint4(0, 0, 0, 0);
-        for (int k = 0; k < q; ++k) {
-            // One Philox call serves the two picks of a lane pair (reading D21).  Over two consecutive sub-steps the
-            // even lane computes the pair's call of sub-step k and the odd lane that of sub-step k + 1, and each
-            // hands two words to its partner: every lane computes one call per two sub-steps, none idles.
-            uint32_t w_pos, w_acc;
-            if (lam == 1) {
-                w = philox4x32_10((uint32_t)T, (uint32_t)k, a.c2, a.c3, a.k0, a.k1);
-                w_pos = w.x;
-                w_acc = w.y;
-            } else {
-                if ((k & 1) == 0) {
-                    const int kk = k + (j & 1);                        // the odd lane works one sub-step ahead
-                    if (kk < q) w = philox4x32_10((uint32_t)T, (uint32_t)(kk * calls + (j >> 1)), a.c2, a.c3, a.k0, a.k1);
-                    const uint32_t pz = __shfl_xor_sync(0xffffffffu, w.z, 1), pw = __shfl_xor_sync(0xffffffffu, w.w, 1);
-                    w_pos = (j & 1) ? pz : w.x;                        // sub-step k: the even lane's call
-                    w_acc = (j & 1) ? pw : w.y;
-                } else {
-                    const uint32_t px_ = __shfl_xor_sync(0xffffffffu, w.x, 1), py_ = __shfl_xor_sync(0xffffffffu, w.y, 1);
-                    w_pos = (j & 1) ? w.z : px_;                       // sub-step k: the odd lane's call
-                    w_acc = (j & 1) ? w.w : py_;
-                }
-            }
-            const int r = (int)__umulhi(w_pos, (uint32_t)P);
-            // Same site picked twice in this sub-step: the highest thread of the group wins (reading D19).  MATCH.ANY
-            // would find the collisions directly but costs as much as the rest of the sub-step (measured: 100 against
-            // 186 Gflips/s), and collisions are rare (lambda^2 / 2P per sub-step).  So every lane writes its index into
-            // a claim byte of the picked site; after the barrier a lane that reads back another index has collided,
-            // and only then is MATCH used.  Stale claim bytes cannot hide a collision: every lane overwrites its
-            // site's byte before it reads it.
+        // One pick: site (px, py) of colour c = (px + py) & 1 with claim index r, acceptance word w_acc.
+        // Same site picked twice in one phase: the highest thread of the group wins (reading D19).  MATCH.ANY would
+        // find the collisions directly but costs as much as the rest of the sub-step (measured: 100 against 186
+        // Gflips/s), and collisions are rare (lambda^2 / 2P per sub-step).  So every lane writes its index into a claim
+        // byte of the picked site; after the barrier a lane that reads back another index has collided, and only then
+        // is MATCH used.  Stale claim bytes cannot hide a collision: every lane overwrites its byte before it reads it.
+        auto pick = [&](const int r, const int px, const int py, const int c, const uint32_t w_acc) {
             if (lam > 1) sts_u8(s_claim + (uint32_t)r, (uint32_t)j);
-            const int px = r & (b - 1), py = r >> a.lg_b;
-            const int c = (px + py) & 1;                               // x0, y0 are even
             const uint32_t me = s_tile + (uint32_t)(c * col_bytes + py * rowb + (px >> 1));
             const uint32_t oth = s_tile + (uint32_t)((c ^ 1) * col_bytes + py * rowb);
             const uint32_t own = lds_u8(me);
@@ -139,7 +113,7 @@ k_ne_random_tile(const __grid_constant__ NeTileArgs a)
                     n_new = w_acc < thr_c ? 1u : 0u;
                 }
             }
-            __syncwarp();                                              // all picks have read the sub-step's start
+            __syncwarp();                                              // all picks have read the phase's start
             bool winner = true;
             if (lam > 1 && __any_sync(0xffffffffu, lds_u8(s_claim + (uint32_t)r) != (uint32_t)j)) {
                 const uint32_t same = __match_any_sync(0xffffffffu, (uint32_t)r | key_hi);
@@ -147,6 +121,48 @@ k_ne_random_tile(const __grid_constant__ NeTileArgs a)
             }
             if (live && winner && n_new != (own & 1u)) sts_u8(me, (own ^ 1u) | chg);
             __syncwarp();                                              // step 7
+        };
+        if (BAL) {
+            // ---- balance-preserving variant (readings D22-D24): lambda red picks, barrier, lambda
+            // white picks, barrier; one Philox call per lane and sub-step (words 0, 1: red pick; 2, 3: white pick)
+            for (int k = 0; k < q; ++k) {
+                const uint4 w = philox4x32_10((uint32_t)T, (uint32_t)(k * lam + j), a.c2, a.c3, a.k0, a.k1);
+#pragma unroll
+                for (int c = 0; c < 2; ++c) {
+                    const int r = (int)__umulhi(c ? w.z : w.x, (uint32_t)(P >> 1));   // r-th site of colour c, row-major
+                    const int py = r >> (a.lg_b - 1), m = r & (rowb - 1);
+                    pick(r, 2 * m + ((py + c) & 1), py, c, c ? w.w : w.y);
+                }
+            }
+        } else {
+            // ---- steps 6-8: q sub-steps of lambda simultaneous random picks
+            uint4 w = make_uint4(0, 0, 0, 0);
+            for (int k = 0; k < q; ++k) {
+                // One Philox call serves the two picks of a lane pair (reading D21).  Over two consecutive sub-steps the
+                // even lane computes the pair's call of sub-step k and the odd lane that of sub-step k + 1, and each
+                // hands two words to its partner: every lane computes one call per two sub-steps, none idles.
+                uint32_t w_pos, w_acc;
+                if (lam == 1) {
+                    w = philox4x32_10((uint32_t)T, (uint32_t)k, a.c2, a.c3, a.k0, a.k1);
+                    w_pos = w.x;
+                    w_acc = w.y;
+                } else {
+                    if ((k & 1) == 0) {
+                        const int kk = k + (j & 1);                        // the odd lane works one sub-step ahead
+                        if (kk < q) w = philox4x32_10((uint32_t)T, (uint32_t)(kk * calls + (j >> 1)), a.c2, a.c3, a.k0, a.k1);
+                        const uint32_t pz = __shfl_xor_sync(0xffffffffu, w.z, 1), pw = __shfl_xor_sync(0xffffffffu, w.w, 1);
+                        w_pos = (j & 1) ? pz : w.x;                        // sub-step k: the even lane's call
+                        w_acc = (j & 1) ? pw : w.y;
+                    } else {
+                        const uint32_t px_ = __shfl_xor_sync(0xffffffffu, w.x, 1), py_ = __shfl_xor_sync(0xffffffffu, w.y, 1);
+                        w_pos = (j & 1) ? w.z : px_;                       // sub-step k: the odd lane's call
+                        w_acc = (j & 1) ? w.w : py_;
+                    }
+                }
+                const int r = (int)__umulhi(w_pos, (uint32_t)P);
+                const int px = r & (b - 1), py = r >> a.lg_b;
+                pick(r, px, py, (px + py) & 1, w_acc);                 // x0, y0 are even
+            }
         }
         // ---- step 9: copy the tile back (interior only); count the up sites for the fused observable
         if (live) {
@@ -172,12 +188,12 @@ static size_t ne_tile_bytes(int b, int lam)
     return (size_t)((2 * (b + 1) * (b / 2) + b + (lam > 1 ? b * b : 0) + 15) & ~15);
 }
 
-bool ne_tile_supported(const Lat &lat, int b, int lam)
+bool ne_tile_supported(const Lat &lat, int b, int lam, bool balanced)
 {
     if (lat.dims != 2) return false;
     if (b < 8 || b > 128 || (b & (b - 1)) != 0 || lat.L % b != 0) return false;
     if (lam < 1 || lam > 32 || (lam & (lam - 1)) != 0) return false;
-    if ((b * b) % (2 * lam) != 0) return false;
+    if ((b * b) % ((balanced ? 8 : 2) * lam) != 0) return false;   // q * lambda = P/2 (D17) or q * 2 lambda = P/4 (D23)
     return (32 / lam) * ne_tile_bytes(b, lam) <= 200 * 1024;   // one warp's tiles must fit shared memory
 }
 
@@ -189,7 +205,7 @@ static int ne_tile_threads(int b, int lam)
     return threads;
 }
 
-cudaError_t launch_ne_random_tile(const Lat &lat, uint8_t *const dst[2], bool metropolis, int b, int lam,
+cudaError_t launch_ne_random_tile(const Lat &lat, uint8_t *const dst[2], bool metropolis, bool balanced, int b, int lam,
                                   unsigned long long seed, unsigned long long t, int launch, uint32_t thr_c,
                                   uint32_t thr_up, int up_always, int track, long long *obs, cudaStream_t s)
 {
@@ -208,7 +224,7 @@ cudaError_t launch_ne_random_tile(const Lat &lat, uint8_t *const dst[2], bool me
     a.k0 = (uint32_t)seed;
     a.k1 = (uint32_t)(seed >> 32);
     a.c2 = (uint32_t)t;
-    a.c3 = (4u + (uint32_t)launch) | ((uint32_t)(t >> 32) << 2);     // reading D21: stream tags 4, 5
+    a.c3 = ((balanced ? 8u : 4u) + (uint32_t)launch) | ((uint32_t)(t >> 32) << 2);   // D21: tags 4, 5; D24: 8..11
     a.thr_c = thr_c;
     a.thr_up = thr_up;
     a.up_always = up_always;
@@ -220,7 +236,8 @@ cudaError_t launch_ne_random_tile(const Lat &lat, uint8_t *const dst[2], bool me
     int grid = (a.ntiles + tiles_per_cta - 1) / tiles_per_cta;
     const int cap = sm_count() * 8;
     if (grid > cap) grid = cap;
-    auto kern = metropolis ? k_ne_random_tile<true> : k_ne_random_tile<false>;
+    auto kern = balanced ? (metropolis ? k_ne_random_tile<true, true> : k_ne_random_tile<false, true>)
+                         : (metropolis ? k_ne_random_tile<true, false> : k_ne_random_tile<false, false>);
     if (smem > 48 * 1024) {
         cudaError_t e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
         if (e != cudaSuccess) return e;

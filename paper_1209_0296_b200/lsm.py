@@ -30,6 +30,7 @@ SIGNATURES = {
     "lsm_sweep_record": (_i32, [_vp, _i64, _vp, _vp]),
     "lsm_sweep_record_host": (_i32, [_vp, _i64, _vp, _vp, _vp]),
     "lsm_sweep_random_tile": (_i32, [_vp, _i64, _i32, _i32, _vp, _vp]),
+    "lsm_sweep_random_tile_balanced": (_i32, [_vp, _i64, _i32, _i32, _vp, _vp]),
     "lsm_measure": (_i32, [_vp, _P(_dbl), _P(_i64)]),
     "lsm_measure_int": (_i32, [_vp, _P(_i64), _P(_i64), _P(_u64)]),
     "lsm_measure_full": (_i32, [_vp, _P(_i64), _P(_i64)]),
@@ -171,16 +172,18 @@ class Lattice:
                "lsm_sweep_record")
         return out
 
-    def sweep_random_tile(self, n=1, b=32, lam=16, record=False, out=None, stream=None):
+    def sweep_random_tile(self, n=1, b=32, lam=16, record=False, out=None, stream=None, balanced=False):
         """North-East model: n sweeps of the paper's corrected algorithm: random picks of `lam`
-        threads in tiles of b x b spins.  record=True returns the device [n, 2] series (0, M)."""
+        threads in tiles of b x b spins; balanced=True: its balance-preserving variant.
+        record=True returns the device [n, 2] series (0, M)."""
         import torch
 
         if record and out is None:
             out = torch.empty((int(n), 2), dtype=torch.int64, device=self.device)
         ptr = _vp(out.data_ptr()) if out is not None else None
-        _check(self._lib.lsm_sweep_random_tile(self._h, int(n), int(b), int(lam), ptr, _stream_ptr(stream)),
-               "lsm_sweep_random_tile")
+        fn = self._lib.lsm_sweep_random_tile_balanced if balanced else self._lib.lsm_sweep_random_tile
+        _check(fn(self._h, int(n), int(b), int(lam), ptr, _stream_ptr(stream)),
+               "lsm_sweep_random_tile_balanced" if balanced else "lsm_sweep_random_tile")
         return out
 
     def sweep_record_host(self, n, h_obs=None, stream=None):

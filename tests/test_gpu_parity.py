@@ -371,3 +371,32 @@ def test_random_tile_schedule_full_size_prefix():
     want = orc.sweep_random_tile_record(1, 32, 16)
     assert np.array_equal(got, want)
     assert_same_state(lat, orc)
+
+
+# ------------------------------------------------------------------ NEXT-2: the balance-preserving variant
+@pytest.mark.parametrize("model", [lsm.NE_HEATBATH, lsm.NE_METROPOLIS])
+@pytest.mark.parametrize("L,b,lam,c,nsweeps", [
+    (64, 32, 16, 0.42, 20),
+    (64, 8, 8, 0.45, 20),        # P/2 = 32 sites per colour and 8 picks: collisions in most phases
+    (128, 16, 1, 0.30, 8),
+    (64, 64, 1, 0.42, 4),
+    (384, 128, 32, 0.30, 4),
+    (1024, 32, 16, 0.42, 3),
+])
+def test_random_tile_balanced_parity(model, L, b, lam, c, nsweeps):
+    kw = dict(dims=2, L=L, model=model, J=0.0, T=W.ne_temperature(c), seed=W.seed_of(5, 9) + L + lam)
+    lat, orc = make_pair(**kw)
+    got = lat.sweep_random_tile(nsweeps, b, lam, record=True, balanced=True).cpu().numpy()
+    orc.sweep_random_tile_balanced(nsweeps - 1, b, lam)
+    assert np.array_equal(got[-2, 1], orc.measure_int()[1])
+    orc.sweep_random_tile_balanced(1, b, lam)
+    assert_same_state(lat, orc)
+    lat.sweep_random_tile(1, b, lam)                         # the three schedules share state and sweep counter
+    orc.sweep_random_tile(1, b, lam)
+    lat.sweep(1)
+    orc.sweep(1)
+    lat.sweep_random_tile(2, b, lam, balanced=True)
+    orc.sweep_random_tile_balanced(2, b, lam)
+    assert_same_state(lat, orc)
+    with pytest.raises(lsm.LsmError):
+        lat.sweep_random_tile(1, 8, 16, balanced=True)       # 8 * lambda does not divide P = 64

@@ -246,9 +246,8 @@ def test_balanced_matches_the_dict_restatement(model, L, b, lam):
 
 def test_balanced_tile_order_measure_and_persistence():
     """Tile order immaterial (D18); product measure stationary; one MC step attempts P updates per tile (D23), so the
-    first-step persistence follows the same closed form as the base algorithm with Binomial(P/2, 2/P) picks per site
-    (each launch draws P/4 picks uniformly from the P/2 sites of each colour... a site of either colour is picked
-    P/2 times with probability 2/P in total)."""
+    first-step persistence follows the closed form of the base algorithm with Binomial(P/2, 2/P) picks per site (the
+    step draws P/2 picks for each colour, each uniform over that colour's P/2 sites)."""
     c, L, b, lam = 0.30, 256, 32, 16
     N, P = L * L, b * b
     kw = dict(dims=2, L=L, model=O.NE_HEATBATH, J=0.0, T=T_of_c(c), seed=5150)
