@@ -400,3 +400,44 @@ def test_random_tile_balanced_parity(model, L, b, lam, c, nsweeps):
     assert_same_state(lat, orc)
     with pytest.raises(lsm.LsmError):
         lat.sweep_random_tile(1, 8, 16, balanced=True)       # 8 * lambda does not divide P = 64
+
+
+# ------------------------------------------------------------------ NEXT-3: the temperature ramp of the paper's Fig. 6
+def test_temperature_ramp_matches_the_oracle():
+    """start at T = 2.4, lower T in steps, measure M, E and the heat capacity at each T -- one lattice
+    carried through; integer series identical to the oracle's, derived doubles within 1e-9."""
+    from paper_1209_0296_b200 import ramp
+
+    temps = ramp.temperatures(2.4, 2.1, 0.1)
+    assert temps == [2.4, 2.3, 2.2, 2.1]
+    kw = dict(dims=2, L=128, T=temps[0], seed=W.seed_of(6, 1))
+    lat, orc = make_pair(**kw)
+    assert lat.kernel == lsm.KERNEL_SMALL                       # one launch per block of sweeps on the paper's own size
+    rows = ramp.temperature_ramp(lat, temps, n_equil=30, n_meas=60, keep_series=True)
+    for r in rows:
+        orc.set_temperature(r["T"])
+        orc.sweep(30)
+        want = orc.sweep_record(60)
+        assert np.array_equal(r["series"], want)
+        c_o = O.heat_capacity_per_site(want, lat.N, 1.0, 0.0, r["T"])
+        assert abs(r["c"] - c_o) <= 1e-9 * abs(c_o)
+        u_o = O.binder_u4(want[:, 1])
+        assert abs(r["u4"] - u_o) <= 1e-9 * abs(u_o)
+        e_o = sum(O.energy_from_int(int(b), int(m), 1.0, 0.0) for b, m in want) / (len(want) * lat.N)
+        assert abs(r["e"] - e_o) <= 1e-9 * abs(e_o)
+    assert_same_state(lat, orc, check_persistence=False)
+
+
+def test_temperature_ramp_finds_the_transition():
+    """Equilibrium check of the whole chain on the paper's protocol (shortened): the heat capacity of a 64^2 lattice
+    peaks within 0.06 of Tc = 2/ln(1+sqrt 2), and |m| follows Onsager's 0.911 at T = 2.0 within 1 %."""
+    from paper_1209_0296_b200 import ramp
+
+    temps = ramp.temperatures(2.5, 2.0, 0.02)
+    lat = lsm.Lattice(dims=2, L=64, T=temps[0], seed=W.seed_of(6, 2))
+    lat.set_tracking(False)
+    rows = ramp.temperature_ramp(lat, temps, n_equil=3000, n_meas=20000)
+    peak = max(rows, key=lambda r: r["c"])
+    assert abs(peak["T"] - ramp.TC_2D) < 0.06, peak
+    assert abs(rows[-1]["abs_m"] - 0.91131938) < 0.01, rows[-1]
+    assert abs(rows[-1]["e"] - (-1.74556458)) < 0.01, rows[-1]
