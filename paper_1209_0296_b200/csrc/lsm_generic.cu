@@ -215,10 +215,92 @@ __global__ void __launch_bounds__(256) k_measure_full(Lat lat, long long *out)
     block_accumulate2(accB, accM, out, true, true);
 }
 
+// Word-granular full reduction for lattices with whole 16-byte words per compact row (L % 32 == 0): a thread
+// takes words of colour 1 and the same-index words of colour 0; the neighbour sums of 16 sites are byte-parallel
+// adds of the colour-0 words at march +-1, cross row +-1 (3D) and the one-byte-shifted word of the own row, as in
+// the sweep kernels.  Every bond joins the two colours, so B = sum over colour-1 sites of s_i * nn_i.
+template <int MODEL, int DIMS>
+__global__ void __launch_bounds__(256) k_measure_words(Lat lat, long long *out)
+{
+    constexpr uint32_t VAL = Enc<MODEL>::VAL * 0x01010101u;
+    const uint4 *__restrict__ c0 = reinterpret_cast<const uint4 *>(lat.col[0]);
+    const uint4 *__restrict__ c1 = reinterpret_cast<const uint4 *>(lat.col[1]);
+    const uint32_t *__restrict__ c0l = reinterpret_cast<const uint32_t *>(lat.col[0]);
+    const int wpr = lat.Lh >> 4, R = DIMS == 3 ? lat.L : 1, rs = R * wpr;
+    const long long nw = (long long)lat.L * rs;
+    int sA0 = 0, sA1 = 0, sAS = 0, sS = 0;           // sums of values (colour 0 / 1), of value * neighbour sum, of sums
+    long long nwords = 0;
+    for (long long w = (long long)blockIdx.x * blockDim.x + threadIdx.x; w < nw; w += (long long)gridDim.x * blockDim.x) {
+        const long long row = w / wpr;
+        const int j = (int)(w - row * wpr);
+        const int m = (int)(row / R), y = (int)(row - (long long)m * R);
+        const int q = (m + y + 1) & 1;                // colour-1 sites of this row: x = 2k + q
+        const uint4 O = c1[w], C = c0[w];
+        const uint4 P = c0[m == 0 ? w + nw - rs : w - rs], N = c0[m + 1 == lat.L ? w - nw + rs : w + rs];
+        const int je = q ? (j + 1 == wpr ? 0 : j + 1) : (j == 0 ? wpr - 1 : j - 1);
+        const uint32_t e = c0l[(row * wpr + je) * 4 + (q ? 0 : 3)];
+        uint4 Yp = make_uint4(0, 0, 0, 0), Yn = Yp;
+        if (DIMS == 3) {
+            Yp = c0[w + (y == 0 ? (long long)(R - 1) * wpr : -(long long)wpr)];
+            Yn = c0[w + (y + 1 == R ? -(long long)(R - 1) * wpr : (long long)wpr)];
+        }
+        const uint32_t o[4] = {O.x, O.y, O.z, O.w}, c[4] = {C.x, C.y, C.z, C.w}, p[4] = {P.x, P.y, P.z, P.w},
+                       n[4] = {N.x, N.y, N.z, N.w}, yp[4] = {Yp.x, Yp.y, Yp.z, Yp.w}, yn[4] = {Yn.x, Yn.y, Yn.z, Yn.w};
+        uint32_t sd[4];
+        if (q) {
+            sd[0] = __funnelshift_r(c[0], c[1], 8); sd[1] = __funnelshift_r(c[1], c[2], 8);
+            sd[2] = __funnelshift_r(c[2], c[3], 8); sd[3] = __funnelshift_r(c[3], e, 8);
+        } else {
+            sd[0] = __funnelshift_r(e, c[0], 24); sd[1] = __funnelshift_r(c[0], c[1], 24);
+            sd[2] = __funnelshift_r(c[1], c[2], 24); sd[3] = __funnelshift_r(c[2], c[3], 24);
+        }
+#pragma unroll
+        for (int d = 0; d < 4; ++d) {
+            uint32_t ns = (p[d] & VAL) + (n[d] & VAL) + (c[d] & VAL) + (sd[d] & VAL);
+            if (DIMS == 3) ns += (yp[d] & VAL) + (yn[d] & VAL);
+            const uint32_t v1 = o[d] & VAL, v0 = c[d] & VAL;
+            sA0 = (int)__dp4a(v0, 0x01010101u, (uint32_t)sA0);
+            sA1 = (int)__dp4a(v1, 0x01010101u, (uint32_t)sA1);
+            if (MODEL == M_ISING_HALF || MODEL == M_ISING_ONE) {
+                sAS = (int)__dp4a(v1, ns, (uint32_t)sAS);
+                if (MODEL == M_ISING_ONE) sS = (int)__dp4a(ns, 0x01010101u, (uint32_t)sS);
+            }
+        }
+        ++nwords;
+    }
+    const long long n1 = 16 * nwords;                 // colour-1 sites (= colour-0 sites) this thread visited
+    long long accB = 0, accM = 0;
+    if (MODEL == M_ISING_HALF) {
+        // s = 2b - 1, nn = 2n - 2d, sum over colour-1 sites of n = 2d * (ups of colour 0)
+        accM = 2LL * (sA0 + sA1) - 2 * n1;
+        accB = 4LL * sAS - 4LL * DIMS * sA1 - 4LL * DIMS * sA0 + 2LL * DIMS * n1;
+    } else if (MODEL == M_ISING_ONE) {
+        accM = (long long)sA0 + sA1 - 2 * n1;
+        accB = (long long)sAS - 2LL * DIMS * sA1 - sS + 2LL * DIMS * n1;
+    } else {
+        accM = (long long)sA0 + sA1;
+    }
+    block_accumulate2(accB, accM, out, true, true);
+}
+
 cudaError_t launch_measure_full(const Lat &lat, int model, long long *d_BM, cudaStream_t s)
 {
     cudaError_t e = cudaMemsetAsync(d_BM, 0, 2 * sizeof(long long), s);
     if (e != cudaSuccess) return e;
+    if (lat.Lh % 16 == 0) {
+        const int grid = grid_for(lat.half >> 4, 256, 8);
+        const bool d3 = lat.dims == 3;
+        if (model == M_ISING_HALF) {
+            if (d3) k_measure_words<M_ISING_HALF, 3><<<grid, 256, 0, s>>>(lat, d_BM);
+            else k_measure_words<M_ISING_HALF, 2><<<grid, 256, 0, s>>>(lat, d_BM);
+        } else if (model == M_ISING_ONE) {
+            if (d3) k_measure_words<M_ISING_ONE, 3><<<grid, 256, 0, s>>>(lat, d_BM);
+            else k_measure_words<M_ISING_ONE, 2><<<grid, 256, 0, s>>>(lat, d_BM);
+        } else {
+            k_measure_words<M_NE_HEATBATH, 2><<<grid, 256, 0, s>>>(lat, d_BM);
+        }
+        return cudaGetLastError();
+    }
     int grid = grid_for(lat.half, 256, 8);
     if (model == M_ISING_HALF) k_measure_full<M_ISING_HALF><<<grid, 256, 0, s>>>(lat, d_BM);
     else if (model == M_ISING_ONE) k_measure_full<M_ISING_ONE><<<grid, 256, 0, s>>>(lat, d_BM);
