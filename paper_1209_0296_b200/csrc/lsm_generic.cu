@@ -427,14 +427,98 @@ __global__ void __launch_bounds__(256) k_set_spins(Lat lat, int model, const int
     }
 }
 
+// Word-granular conversions for lattices with whole 16-byte words per compact row: a thread converts 32 consecutive
+// sites of one canonical row = one word of each colour (even x -> colour (y+z)&1, odd x -> the other), de-/interleaving
+// bytes with PRMT.  Same value conventions as the scalar kernels above.
+__device__ __forceinline__ uint32_t prmt_b(uint32_t a, uint32_t b, uint32_t sel)
+{
+    uint32_t r;
+    asm("prmt.b32 %0, %1, %2, %3;" : "=r"(r) : "r"(a), "r"(b), "r"(sel));
+    return r;
+}
+__device__ __forceinline__ uint32_t encode4(uint32_t s, int model)
+{
+    const uint32_t nz = (((s & 0x7F7F7F7Fu) + 0x7F7F7F7Fu) | s) & 0x80808080u;     // bit 7: byte != 0
+    const uint32_t pos = (nz & ~s) >> 7;                                            // int8 > 0
+    if (model == M_ISING_HALF) return pos;
+    if (model == M_ISING_ONE) return (pos << 1) | ((nz ^ 0x80808080u) >> 7);       // < 0: 0, == 0: 1, > 0: 2
+    return nz >> 7;
+}
+__device__ __forceinline__ uint32_t decode4(uint32_t b, int model)
+{
+    if (model == M_ISING_HALF) {
+        const uint32_t t = b & 0x01010101u;
+        return t | ((t ^ 0x01010101u) * 0xFFu);                                     // 1 -> +1, 0 -> -1
+    }
+    if (model == M_ISING_ONE) {
+        const uint32_t z = (b | (b >> 1)) & 0x01010101u;                            // a != 0
+        return ((b & 0x02020202u) >> 1) | ((z ^ 0x01010101u) * 0xFFu);              // 2 -> +1, 1 -> 0, 0 -> -1
+    }
+    return b & 0x01010101u;
+}
+
+__global__ void __launch_bounds__(256) k_set_spins_words(Lat lat, int model, const int8_t *__restrict__ in)
+{
+    const int wpr = lat.Lh >> 4;
+    const long long nw = lat.half >> 4;
+    const uint32_t keep = model == M_ISING_ONE ? 0xFCFCFCFCu : 0xFEFEFEFEu;
+    for (long long w = (long long)blockIdx.x * blockDim.x + threadIdx.x; w < nw; w += (long long)gridDim.x * blockDim.x) {
+        const long long row = w / wpr;                                              // canonical row z*L + y
+        const int ce = (int)((row % lat.L + row / lat.L) & 1);                      // colour of the even-x sites
+        const uint4 *src = reinterpret_cast<const uint4 *>(in + 2 * 16 * w);
+        const uint4 A = src[0], B = src[1];
+        const uint32_t x[8] = {A.x, A.y, A.z, A.w, B.x, B.y, B.z, B.w};
+        uint32_t ev[4], od[4];
+#pragma unroll
+        for (int t = 0; t < 4; ++t) {
+            ev[t] = encode4(prmt_b(x[2 * t], x[2 * t + 1], 0x6420u), model);
+            od[t] = encode4(prmt_b(x[2 * t], x[2 * t + 1], 0x7531u), model);
+        }
+        uint4 *pe = reinterpret_cast<uint4 *>(ce ? lat.col[1] : lat.col[0]) + w;
+        uint4 *po = reinterpret_cast<uint4 *>(ce ? lat.col[0] : lat.col[1]) + w;
+        uint4 oe = *pe, oo = *po;                                                   // flags and snapshot stay
+        *pe = make_uint4((oe.x & keep) | ev[0], (oe.y & keep) | ev[1], (oe.z & keep) | ev[2], (oe.w & keep) | ev[3]);
+        *po = make_uint4((oo.x & keep) | od[0], (oo.y & keep) | od[1], (oo.z & keep) | od[2], (oo.w & keep) | od[3]);
+    }
+}
+
+__global__ void __launch_bounds__(256) k_get_spins_words(Lat lat, int model, int8_t *__restrict__ out)
+{
+    const int wpr = lat.Lh >> 4;
+    const long long nw = lat.half >> 4;
+    for (long long w = (long long)blockIdx.x * blockDim.x + threadIdx.x; w < nw; w += (long long)gridDim.x * blockDim.x) {
+        const long long row = w / wpr;
+        const int ce = (int)((row % lat.L + row / lat.L) & 1);
+        const uint4 E = reinterpret_cast<const uint4 *>(ce ? lat.col[1] : lat.col[0])[w];
+        const uint4 O = reinterpret_cast<const uint4 *>(ce ? lat.col[0] : lat.col[1])[w];
+        const uint32_t ev[4] = {decode4(E.x, model), decode4(E.y, model), decode4(E.z, model), decode4(E.w, model)};
+        const uint32_t od[4] = {decode4(O.x, model), decode4(O.y, model), decode4(O.z, model), decode4(O.w, model)};
+        uint32_t x[8];
+#pragma unroll
+        for (int t = 0; t < 4; ++t) {
+            x[2 * t] = prmt_b(ev[t], od[t], 0x5140u);                               // e0 o0 e1 o1
+            x[2 * t + 1] = prmt_b(ev[t], od[t], 0x7362u);                           // e2 o2 e3 o3
+        }
+        uint4 *dst = reinterpret_cast<uint4 *>(out + 2 * 16 * w);
+        dst[0] = make_uint4(x[0], x[1], x[2], x[3]);
+        dst[1] = make_uint4(x[4], x[5], x[6], x[7]);
+    }
+}
+
 cudaError_t launch_get_spins(const Lat &lat, int model, int8_t *d_out, cudaStream_t s)
 {
-    k_get_spins<<<grid_for(2 * lat.half, 256, 8), 256, 0, s>>>(lat, model, d_out);
+    if (lat.Lh % 16 == 0 && ((uintptr_t)d_out & 15) == 0)
+        k_get_spins_words<<<grid_for(lat.half >> 4, 256, 8), 256, 0, s>>>(lat, model, d_out);
+    else
+        k_get_spins<<<grid_for(2 * lat.half, 256, 8), 256, 0, s>>>(lat, model, d_out);
     return cudaGetLastError();
 }
 cudaError_t launch_set_spins(const Lat &lat, int model, const int8_t *d_in, cudaStream_t s)
 {
-    k_set_spins<<<grid_for(2 * lat.half, 256, 8), 256, 0, s>>>(lat, model, d_in);
+    if (lat.Lh % 16 == 0 && ((uintptr_t)d_in & 15) == 0)
+        k_set_spins_words<<<grid_for(lat.half >> 4, 256, 8), 256, 0, s>>>(lat, model, d_in);
+    else
+        k_set_spins<<<grid_for(2 * lat.half, 256, 8), 256, 0, s>>>(lat, model, d_in);
     return cudaGetLastError();
 }
 
