@@ -44,8 +44,11 @@ __device__ __forceinline__ void sts_u8(uint32_t a, uint32_t v)
     asm volatile("st.shared.u8 [%0], %1;" ::"r"(a), "r"(v) : "memory");
 }
 
+#ifndef LSM_NE_TILE_MINBLOCKS
+#define LSM_NE_TILE_MINBLOCKS 4
+#endif
 template <bool METRO, bool BAL>
-__global__ void __launch_bounds__(256)
+__global__ void __launch_bounds__(256, LSM_NE_TILE_MINBLOCKS)
 k_ne_random_tile(const __grid_constant__ NeTileArgs a)
 {
     extern __shared__ __align__(16) uint8_t s_tiles[];
@@ -75,14 +78,18 @@ k_ne_random_tile(const __grid_constant__ NeTileArgs a)
         const uint32_t key_hi = ((uint32_t)grp_in_warp << 16) | (live ? 0u : 0x80000000u);
         // ---- step 5: tile + upper and right boundaries -> shared memory
         if (live) {
-            // word i of the tile -> (row, colour, word in row): all powers of two, no divisions
-            const int lg_lr = a.lg_b - 3;                              // log2(32-bit words per tile row and colour)
-            for (int i = j; i < ((b + 1) << (lg_lr + 1)); i += lam) {
-                const int rr = i >> (lg_lr + 1), c = (i >> lg_lr) & 1, u = i & ((1 << lg_lr) - 1);
+            // Asynchronous copies (LDGSTS) in chunks of 16 bytes (4 for tiles narrower than 32 sites): all of a lane's
+            // chunks are in flight together, one round trip to L2/HBM per tile instead of one per chunk.
+            // chunk i -> (row, colour, chunk in row): all powers of two, no divisions
+            const int lg_cw = rowb >= 16 ? 4 : 2, lg_cr = a.lg_b - 1 - lg_cw;          // log2(chunk bytes), log2(chunks per row and colour)
+            for (int i = j; i < ((b + 1) << (lg_cr + 1)); i += lam) {
+                const int rr = i >> (lg_cr + 1), c = (i >> lg_cr) & 1, u = i & ((1 << lg_cr) - 1);
                 int yy = y0 + rr;
                 if (yy >= a.L) yy -= a.L;
-                const uint32_t v = *reinterpret_cast<const uint32_t *>((c ? a.src[1] : a.src[0]) + (size_t)yy * a.Lh + (x0 >> 1) + 4 * u);
-                *reinterpret_cast<uint32_t *>((tile + c * col_bytes) + rr * rowb + 4 * u) = v;
+                const uint8_t *g = (c ? a.src[1] : a.src[0]) + (size_t)yy * a.Lh + (x0 >> 1) + (u << lg_cw);
+                const uint32_t d = s_tile + (uint32_t)(c * col_bytes + rr * rowb + (u << lg_cw));
+                if (lg_cw == 4) asm volatile("cp.async.ca.shared.global [%0], [%1], 16;" ::"r"(d), "l"(g) : "memory");
+                else asm volatile("cp.async.ca.shared.global [%0], [%1], 4;" ::"r"(d), "l"(g) : "memory");
             }
             int xe = x0 + b;
             if (xe >= a.L) xe -= a.L;
@@ -91,6 +98,7 @@ k_ne_random_tile(const __grid_constant__ NeTileArgs a)
                 east[py] = (((xe + yy) & 1) ? a.src[1] : a.src[0])[(size_t)yy * a.Lh + (xe >> 1)];
             }
         }
+        asm volatile("cp.async.commit_group;\n\tcp.async.wait_group 0;" ::: "memory");
         __syncwarp();
         // One pick: site (px, py) of colour c = (px + py) & 1 with claim index r, acceptance word w_acc.
         // Same site picked twice in one phase: the highest thread of the group wins (reading D19).  MATCH.ANY would
@@ -166,12 +174,23 @@ k_ne_random_tile(const __grid_constant__ NeTileArgs a)
         }
         // ---- step 9: copy the tile back (interior only); count the up sites for the fused observable
         if (live) {
-            const int lg_lr = a.lg_b - 3;
-            for (int i = j; i < (b << (lg_lr + 1)); i += lam) {
-                const int rr = i >> (lg_lr + 1), c = (i >> lg_lr) & 1, u = i & ((1 << lg_lr) - 1);
-                const uint32_t v = *reinterpret_cast<const uint32_t *>((tile + c * col_bytes) + rr * rowb + 4 * u);
-                *reinterpret_cast<uint32_t *>((c ? a.dst[1] : a.dst[0]) + (size_t)(y0 + rr) * a.Lh + (x0 >> 1) + 4 * u) = v;
-                ups += (int)__dp4a(v & 0x01010101u, 0x01010101u, 0u);
+            if (rowb >= 16) {
+                const int lg_cr = a.lg_b - 5;                          // 16-byte chunks per row and colour
+                for (int i = j; i < (b << (lg_cr + 1)); i += lam) {
+                    const int rr = i >> (lg_cr + 1), c = (i >> lg_cr) & 1, u = i & ((1 << lg_cr) - 1);
+                    const uint4 v = *reinterpret_cast<const uint4 *>((tile + c * col_bytes) + rr * rowb + 16 * u);
+                    *reinterpret_cast<uint4 *>((c ? a.dst[1] : a.dst[0]) + (size_t)(y0 + rr) * a.Lh + (x0 >> 1) + 16 * u) = v;
+                    ups += (int)__dp4a((v.x & 0x01010101u) + (v.y & 0x01010101u) + (v.z & 0x01010101u) + (v.w & 0x01010101u),
+                                       0x01010101u, 0u);
+                }
+            } else {
+                const int lg_lr = a.lg_b - 3;
+                for (int i = j; i < (b << (lg_lr + 1)); i += lam) {
+                    const int rr = i >> (lg_lr + 1), c = (i >> lg_lr) & 1, u = i & ((1 << lg_lr) - 1);
+                    const uint32_t v = *reinterpret_cast<const uint32_t *>((tile + c * col_bytes) + rr * rowb + 4 * u);
+                    *reinterpret_cast<uint32_t *>((c ? a.dst[1] : a.dst[0]) + (size_t)(y0 + rr) * a.Lh + (x0 >> 1) + 4 * u) = v;
+                    ups += (int)__dp4a(v & 0x01010101u, 0x01010101u, 0u);
+                }
             }
         }
         __syncwarp();
