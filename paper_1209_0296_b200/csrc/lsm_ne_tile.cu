@@ -27,6 +27,7 @@ struct NeTileArgs {
     int ntx;                 // tiles per lattice row
     int ntiles;
     uint32_t k0, k1, c2, c3; // Philox key and the (sweep, launch) fields of the counter
+    uint32_t rk0[10], rk1[10];   // round keys k0 + r W0, k1 + r W1 (kernel-parameter bank: operands of the round's LOP3)
     uint32_t thr_c, thr_up;  // floor(c 2^32), floor(exp(-1/T) 2^32) clipped to 32 bits
     int up_always;           // Metropolis: exp(-1/T) rounds to 2^32
     int track;
@@ -42,6 +43,22 @@ __device__ __forceinline__ uint32_t lds_u8(uint32_t a)
 __device__ __forceinline__ void sts_u8(uint32_t a, uint32_t v)
 {
     asm volatile("st.shared.u8 [%0], %1;" ::"r"(a), "r"(v) : "memory");
+}
+
+// Philox4x32-10 on counter (c0, c1, a.c2, a.c3) with the round keys read from the kernel parameters.
+__device__ __forceinline__ uint4 philox_rk(uint32_t c0, uint32_t c1, const NeTileArgs &a)
+{
+    uint32_t c2 = a.c2, c3 = a.c3;
+#pragma unroll
+    for (int r = 0; r < 10; ++r) {
+        const unsigned long long p0 = (unsigned long long)PHILOX_M0 * c0, p1 = (unsigned long long)PHILOX_M1 * c2;
+        const uint32_t n0 = (uint32_t)(p1 >> 32) ^ c1 ^ a.rk0[r], n2 = (uint32_t)(p0 >> 32) ^ c3 ^ a.rk1[r];
+        c1 = (uint32_t)p1;
+        c3 = (uint32_t)p0;
+        c0 = n0;
+        c2 = n2;
+    }
+    return make_uint4(c0, c1, c2, c3);
 }
 
 #ifndef LSM_NE_TILE_MINBLOCKS
@@ -134,7 +151,7 @@ k_ne_random_tile(const __grid_constant__ NeTileArgs a)
             // ---- balance-preserving variant (readings D22-D24): lambda red picks, barrier, lambda
             // white picks, barrier; one Philox call per lane and sub-step (words 0, 1: red pick; 2, 3: white pick)
             for (int k = 0; k < q; ++k) {
-                const uint4 w = philox4x32_10((uint32_t)T, (uint32_t)(k * lam + j), a.c2, a.c3, a.k0, a.k1);
+                const uint4 w = philox_rk((uint32_t)T, (uint32_t)(k * lam + j), a);
 #pragma unroll
                 for (int c = 0; c < 2; ++c) {
                     const int r = (int)__umulhi(c ? w.z : w.x, (uint32_t)(P >> 1));   // r-th site of colour c, row-major
@@ -144,32 +161,33 @@ k_ne_random_tile(const __grid_constant__ NeTileArgs a)
             }
         } else {
             // ---- steps 6-8: q sub-steps of lambda simultaneous random picks
-            uint4 w = make_uint4(0, 0, 0, 0);
-            for (int k = 0; k < q; ++k) {
-                // One Philox call serves the two picks of a lane pair (reading D21).  Over two consecutive sub-steps the
-                // even lane computes the pair's call of sub-step k and the odd lane that of sub-step k + 1, and each
-                // hands two words to its partner: every lane computes one call per two sub-steps, none idles.
-                uint32_t w_pos, w_acc;
-                if (lam == 1) {
-                    w = philox4x32_10((uint32_t)T, (uint32_t)k, a.c2, a.c3, a.k0, a.k1);
-                    w_pos = w.x;
-                    w_acc = w.y;
-                } else {
-                    if ((k & 1) == 0) {
-                        const int kk = k + (j & 1);                        // the odd lane works one sub-step ahead
-                        if (kk < q) w = philox4x32_10((uint32_t)T, (uint32_t)(kk * calls + (j >> 1)), a.c2, a.c3, a.k0, a.k1);
-                        const uint32_t pz = __shfl_xor_sync(0xffffffffu, w.z, 1), pw = __shfl_xor_sync(0xffffffffu, w.w, 1);
-                        w_pos = (j & 1) ? pz : w.x;                        // sub-step k: the even lane's call
-                        w_acc = (j & 1) ? pw : w.y;
-                    } else {
-                        const uint32_t px_ = __shfl_xor_sync(0xffffffffu, w.x, 1), py_ = __shfl_xor_sync(0xffffffffu, w.y, 1);
-                        w_pos = (j & 1) ? w.z : px_;                       // sub-step k: the odd lane's call
-                        w_acc = (j & 1) ? w.w : py_;
-                    }
-                }
+            auto go = [&](const uint32_t w_pos, const uint32_t w_acc) {
                 const int r = (int)__umulhi(w_pos, (uint32_t)P);
                 const int px = r & (b - 1), py = r >> a.lg_b;
                 pick(r, px, py, (px + py) & 1, w_acc);                 // x0, y0 are even
+            };
+            if (lam == 1) {
+                for (int k = 0; k < q; ++k) {
+                    const uint4 w = philox_rk((uint32_t)T, (uint32_t)k, a);
+                    go(w.x, w.y);
+                }
+            } else {
+                // One Philox call serves the two picks of a lane pair (reading D21).  Over two consecutive sub-steps the
+                // even lane computes the pair's call of sub-step k and the odd lane that of sub-step k + 1, and each
+                // hands two words to its partner: every lane computes one call per two sub-steps, none idles.
+                for (int k = 0; k < q; k += 2) {
+                    const int kk = k + (j & 1);                        // the odd lane works one sub-step ahead
+                    uint4 w = make_uint4(0, 0, 0, 0);
+                    if (kk < q) w = philox_rk((uint32_t)T, (uint32_t)(kk * calls + (j >> 1)), a);
+                    {                                                  // sub-step k: the even lane's call
+                        const uint32_t pz = __shfl_xor_sync(0xffffffffu, w.z, 1), pw = __shfl_xor_sync(0xffffffffu, w.w, 1);
+                        go((j & 1) ? pz : w.x, (j & 1) ? pw : w.y);
+                    }
+                    if (k + 1 < q) {                                   // sub-step k + 1: the odd lane's call
+                        const uint32_t px_ = __shfl_xor_sync(0xffffffffu, w.x, 1), py_ = __shfl_xor_sync(0xffffffffu, w.y, 1);
+                        go((j & 1) ? w.z : px_, (j & 1) ? w.w : py_);
+                    }
+                }
             }
         }
         // ---- step 9: copy the tile back (interior only); count the up sites for the fused observable
@@ -242,6 +260,10 @@ cudaError_t launch_ne_random_tile(const Lat &lat, uint8_t *const dst[2], bool me
     a.ntiles = a.ntx * a.ntx;
     a.k0 = (uint32_t)seed;
     a.k1 = (uint32_t)(seed >> 32);
+    for (int r = 0; r < 10; ++r) {
+        a.rk0[r] = a.k0 + (uint32_t)r * PHILOX_W0;
+        a.rk1[r] = a.k1 + (uint32_t)r * PHILOX_W1;
+    }
     a.c2 = (uint32_t)t;
     a.c3 = ((balanced ? 8u : 4u) + (uint32_t)launch) | ((uint32_t)(t >> 32) << 2);   // D21: tags 4, 5; D24: 8..11
     a.thr_c = thr_c;
