@@ -8,11 +8,13 @@
 // highest thread wins.
 //
 // B200 mapping: a group of lambda lanes of a warp owns a tile (lambda = 16: two tiles per warp), so steps 6-7 --
-// pick, synchronise -- are warp-level (match.any finds collisions, bar.warp.sync is the barrier) and a CTA keeps
-// 256/lambda tiles in flight.  The tile sits in shared memory in the lattice's own split-colour layout (two
-// arrays of (b+1) rows x b/2 bytes plus the east boundary column), so the copies are plain 32-bit words.
-// Random words: one Philox4x32-10 call serves two picks (position and acceptance word each); the even lane of a
-// pair computes it and hands two words to the odd lane by shuffle.
+// pick, synchronise -- are warp-level (bar.warp.sync is the barrier; collisions are found through claim bytes in
+// shared memory, MATCH.ANY only when one was seen) and a CTA keeps 256/lambda tiles in flight.  The tile sits in
+// shared memory in the lattice's own split-colour layout (two arrays of (b+1) rows x b/2 bytes plus the east
+// boundary column), loaded with cp.async and written back in 16-byte words.
+// Random words: one Philox4x32-10 call serves two picks (position and acceptance word each); over two consecutive
+// sub-steps each lane of a pair computes one of the pair's two calls and hands two words to its partner by shuffle.
+// The balance-preserving variant (readings D22-D24) is the BAL instantiation of the same kernel.
 #include "lsm_internal.cuh"
 
 #include <cstring>
