@@ -131,9 +131,11 @@ k_sweep_resident(const __grid_constant__ ResidentArgs a, const __grid_constant__
         March<MODEL, DIMS, TRACK, OBS> M;
         M.ne_t32 = 0;
         M.ne_always = 0;
+        M.ne_all4 = false;
         if constexpr (NE) {
             M.ne_t32 = tab.t32;
             M.ne_always = tab.always;
+            M.ne_all4 = tab.all4 != 0;
         }
         M.s_t = s_t;
         M.one = (uint32_t)a.g.one;
@@ -226,11 +228,11 @@ static cudaError_t dispatch(int model, int dims, bool track, int obs, int grid, 
                          : launch_to<M_ISING_ONE, 2>(track, obs, grid, s, a, pk, ot, max_grid, bs);
     }
     case M_NE_HEATBATH: {
-        NeTab nt = {t.ne_t32[0], 0};
+        NeTab nt = {t.ne_t32[0], 0, t.ne_all4};
         return launch_to<M_NE_HEATBATH, 2>(track, obs, grid, s, a, pk, nt, max_grid, bs);
     }
     default: {
-        NeTab nt = {t.ne_t32[1], t.ne_up_always};
+        NeTab nt = {t.ne_t32[1], t.ne_up_always, t.ne_all4};
         return launch_to<M_NE_METROPOLIS, 2>(track, obs, grid, s, a, pk, nt, max_grid, bs);
     }
     }

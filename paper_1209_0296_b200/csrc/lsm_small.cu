@@ -61,9 +61,11 @@ k_sweep_small(const __grid_constant__ SmallArgs a, const __grid_constant__ Philo
         March<MODEL, DIMS, TRACK, OBS> M;
         M.ne_t32 = 0;
         M.ne_always = 0;
+        M.ne_all4 = false;
         if constexpr (NE) {
             M.ne_t32 = tab.t32;
             M.ne_always = tab.always;
+            M.ne_all4 = tab.all4 != 0;
         }
         M.s_t = s_t;
         M.one = (uint32_t)a.g.one;
@@ -398,11 +400,11 @@ cudaError_t launch_sweep_small(const Lat &lat, int model, int track, unsigned lo
                              : small_launch_to<M_ISING_ONE, 2>(tr, obs, plan.threads, s, a, pk, ot, lg_lpr, lg_L, plan.cluster);
     }
     case M_NE_HEATBATH: {
-        NeTab nt = {t.ne_t32[0], 0};
+        NeTab nt = {t.ne_t32[0], 0, t.ne_all4};
         return small_launch_to<M_NE_HEATBATH, 2>(tr, obs, plan.threads, s, a, pk, nt, lg_lpr, lg_L, plan.cluster);
     }
     default: {
-        NeTab nt = {t.ne_t32[1], t.ne_up_always};
+        NeTab nt = {t.ne_t32[1], t.ne_up_always, t.ne_all4};
         return small_launch_to<M_NE_METROPOLIS, 2>(tr, obs, plan.threads, s, a, pk, nt, lg_lpr, lg_L, plan.cluster);
     }
     }

@@ -61,6 +61,7 @@ k_sweep_tiled(const __grid_constant__ TiledGeom g, const __grid_constant__ Philo
     March<MODEL, DIMS, TRACK, OBS> M;
     M.ne_t32 = 0;
     M.ne_always = 0;
+    M.ne_all4 = false;
     if constexpr (MODEL == M_ISING_HALF) {
         if (threadIdx.x < 16) sm.t[threadIdx.x] = tab.t[threadIdx.x];
     } else if constexpr (MODEL == M_ISING_ONE) {
@@ -68,6 +69,7 @@ k_sweep_tiled(const __grid_constant__ TiledGeom g, const __grid_constant__ Philo
     } else {
         M.ne_t32 = tab.t32;
         M.ne_always = tab.always;
+        M.ne_all4 = tab.all4 != 0;
     }
     __syncthreads();
     asm volatile("griddepcontrol.wait;" ::: "memory");   // the previous launch's spins are visible from here on
@@ -140,6 +142,7 @@ void build_tiled_tables(int model, int dims, double J, double h, const uint64_t 
         t.ne_t32[0] = clip(thr[0]);
         t.ne_t32[1] = clip(thr[1]);
         t.ne_up_always = thr[1] == ALWAYS ? 1 : 0;
+        t.ne_all4 = (double)thr[0] >= 0.15 * 4294967296.0 ? 1 : 0;
         if (thr[0] == ALWAYS) t.usable = 0;
     }
     *out = t;
@@ -236,11 +239,11 @@ cudaError_t launch_sweep_tiled(const SweepArgs &a, const TiledTables &t, cudaStr
                   : launch_track<M_ISING_ONE, 2>(track, obs_mode, grid, s, g, pc, ot);
     }
     case M_NE_HEATBATH: {
-        NeTab nt = {t.ne_t32[0], 0};
+        NeTab nt = {t.ne_t32[0], 0, t.ne_all4};
         return launch_track<M_NE_HEATBATH, 2>(track, obs_mode > 1 ? 1 : obs_mode, grid, s, g, pc, nt);
     }
     default: {
-        NeTab nt = {t.ne_t32[1], t.ne_up_always};
+        NeTab nt = {t.ne_t32[1], t.ne_up_always, t.ne_all4};
         return launch_track<M_NE_METROPOLIS, 2>(track, obs_mode > 1 ? 1 : obs_mode, grid, s, g, pc, nt);
     }
     }

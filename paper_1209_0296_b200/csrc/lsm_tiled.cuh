@@ -16,6 +16,7 @@ struct TiledTables {
     // NE: [0] heat-bath / init threshold, [1] Metropolis 0->1 threshold (32-bit clipped) + flag
     uint32_t ne_t32[2];
     int ne_up_always;
+    int ne_all4;           // up-concentration >= 0.15: the vectorised rule runs the four Philox calls of a word together
     // spin-1: s1[16*dcode + sum] = thr - 1 (accept iff w1 <= s1), dcode = class of s' - s: 0: +1, 1: +2, 2: -1, 3: -2;
     //   sum = sum of the neighbours' a = s + 1.  The threshold depends on (s' - s, sum) only (reading D3).
     uint32_t s1[64];

@@ -124,7 +124,7 @@ struct TiledGeom {
 };
 
 struct HalfTab { uint32_t t[16]; };            // spin-1/2: t[n + 8*b] = thr - 1  (accept iff w <= t)
-struct NeTab { uint32_t t32; int always; };
+struct NeTab { uint32_t t32; int always; int all4; };   // all4: one Philox region per word (c >= 0.15)
 struct OneTab { uint32_t t[64]; };            // spin-1: t[16*dcode + sum] = thr - 1, dcode = class of s' - s
 template <int MODEL> struct TabOf { using type = NeTab; };
 template <> struct TabOf<M_ISING_HALF> { using type = HalfTab; };
@@ -295,6 +295,7 @@ struct March {
     uint32_t s_t, one;
     uint32_t ne_t32;
     int ne_always;
+    bool ne_all4;
 
     // One step at march position m.  The march runs upwards (rowstride > 0, the tiled family and the even
     // half-sweeps of the resident family) or downwards (rowstride < 0): P is the row the march came
@@ -357,11 +358,43 @@ struct March {
             }
         } else {
             uint32_t accU = 0;
+            // Two forms, chosen per launch by the up-concentration c (warp-uniform flag): above c ~ 0.15 nearly every warp
+            // has a facilitated site in each of the four lanes, so one divergent region per WORD runs the four Philox
+            // calls together (instruction-level parallelism, round keys loaded once: 961 -> 1085 Gflips/s at c = 0.2);
+            // below, one region per LANE skips more calls (c = 0.1: 1144 against 1081).
+            if (ne_all4) {
+            uint32_t fac[4];
+#pragma unroll
+            for (int d = 0; d < 4; ++d) fac[d] = (UP ? n[d] : p[d]) & (qq ? sd[d] : c[d]) & 0x01010101u;
+            uint32_t lt[4] = {0u, 0u, 0u, 0u};
+            if ((fac[0] | fac[1] | fac[2] | fac[3]) != 0u) {
+#pragma unroll
+                for (int d = 0; d < 4; ++d) {
+                    const uint4 r = philox_sweep(grp + d, pc);
+                    uint32_t l = ne_always ? 0x01010101u : 0u;
+                    if (r.x < ne_t32) l |= 0x00000001u;
+                    if (r.y < ne_t32) l |= 0x00000100u;
+                    if (r.z < ne_t32) l |= 0x00010000u;
+                    if (r.w < ne_t32) l |= 0x01000000u;
+                    lt[d] = l;
+                }
+            }
+#pragma unroll
+            for (int d = 0; d < 4; ++d) {
+                const uint32_t nv = TRACK ? (o[d] & 0x01010101u) : o[d];
+                uint32_t n2;
+                if (MODEL == M_NE_METROPOLIS) n2 = nv ^ (fac[d] & (nv | lt[d]));
+                else n2 = (nv & ~fac[d]) | (lt[d] & fac[d]);
+                if (OBS >= 1) accU += n2;
+                out[d] = TRACK ? ((o[d] & ~0x01010101u) | n2 | ((nv ^ n2) << 3)) : n2;
+            }
+            } else {
 #pragma unroll
             for (int d = 0; d < 4; ++d) {
                 uint32_t east = qq ? sd[d] : c[d];
                 out[d] = rule_ne<TRACK, MODEL == M_NE_METROPOLIS, OBS>(o[d], UP ? n[d] : p[d], east, grp + d, pc, ne_t32,
                                                                         ne_always, accU);
+            }
             }
             if (OBS >= 1) totU += bytesum(accU);
         }
