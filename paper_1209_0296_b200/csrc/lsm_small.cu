@@ -39,7 +39,7 @@ k_sweep_small(const __grid_constant__ SmallArgs a, const __grid_constant__ Philo
     if constexpr (MODEL == M_ISING_HALF) {
         if (threadIdx.x < 16) sm.t[threadIdx.x] = tab.t[threadIdx.x];
     } else if constexpr (MODEL == M_ISING_ONE) {
-        if (threadIdx.x < 64) sm.t[threadIdx.x] = tab.t[threadIdx.x];
+        for (int i = threadIdx.x; i < 64; i += blockDim.x) sm.t[i] = tab.t[i];   // blocks may have 32 threads
     }
     if (threadIdx.x < 4) sm.acc[threadIdx.x >> 1][threadIdx.x & 1] = 0;
     __syncthreads();
@@ -123,7 +123,7 @@ k_sweep_small_lane(const __grid_constant__ SmallArgs a, const __grid_constant__ 
     if constexpr (MODEL == M_ISING_HALF) {
         if (threadIdx.x < 16) sm.t[threadIdx.x] = tab.t[threadIdx.x];
     } else if constexpr (MODEL == M_ISING_ONE) {
-        if (threadIdx.x < 64) sm.t[threadIdx.x] = tab.t[threadIdx.x];
+        for (int i = threadIdx.x; i < 64; i += blockDim.x) sm.t[i] = tab.t[i];   // blocks may have 32 threads
     }
     if (threadIdx.x < 4) sm.acc[threadIdx.x >> 1][threadIdx.x & 1] = 0;
 

@@ -65,6 +65,8 @@ SHAPES = [
     (dict(dims=3, L=64, T=4.5115), 8),
     (dict(dims=3, L=34, T=3.0), 8),
     (dict(dims=2, L=4, two_S=2, T=3.0, h=0.01), 40),
+    (dict(dims=2, L=8, two_S=2, T=2.0, h=0.3), 30),       # small family with a single warp: 64-entry table, 32 threads
+    (dict(dims=2, L=16, two_S=2, T=3.9, h=-0.4), 30),
     (dict(dims=2, L=64, two_S=2, T=1.5, h=0.01), 30),
     (dict(dims=3, L=6, two_S=2, T=3.0, h=0.01), 20),
     (dict(dims=3, L=16, two_S=2, T=3.0, h=0.01), 20),
@@ -441,3 +443,50 @@ def test_temperature_ramp_finds_the_transition():
     assert abs(peak["T"] - ramp.TC_2D) < 0.06, peak
     assert abs(rows[-1]["abs_m"] - 0.91131938) < 0.01, rows[-1]
     assert abs(rows[-1]["e"] - (-1.74556458)) < 0.01, rows[-1]
+
+
+# ------------------------------------------------------------------ seeded random parameters across all families
+def _fuzz_cases():
+    rng = np.random.default_rng(20121209)
+    cases = []
+    for i in range(24):
+        kind = i % 4
+        if kind == 0:
+            kw = dict(dims=2, L=int(rng.choice([32, 64, 96, 128, 224])), T=float(rng.uniform(0.3, 6.0)),
+                      J=float(rng.choice([-1.0, 0.5, 1.0, 2.0])), h=float(rng.choice([0.0, 0.0, -0.7, 0.13, 3.0])))
+        elif kind == 1:
+            kw = dict(dims=3, L=int(rng.choice([8, 16, 32, 64])), T=float(rng.uniform(0.5, 9.0)),
+                      J=float(rng.choice([-1.0, 1.0, 0.3])), h=float(rng.choice([0.0, 0.25, -2.0])))
+        elif kind == 2:
+            kw = dict(dims=int(rng.choice([2, 3])), L=int(rng.choice([16, 32, 64])), two_S=2, T=float(rng.uniform(0.4, 5.0)),
+                      J=float(rng.choice([-1.0, 1.0, 0.6])), h=float(rng.choice([0.01, -0.4, 1.5])))
+        else:
+            kw = dict(dims=2, L=int(rng.choice([16, 64, 96, 256])), model=int(rng.choice([lsm.NE_HEATBATH, lsm.NE_METROPOLIS])),
+                      J=0.0, T=W.ne_temperature(float(rng.uniform(0.03, 0.49))))
+        kw["seed"] = int(rng.integers(1, 2 ** 62))
+        cases.append(kw)
+    return cases
+
+
+@pytest.mark.parametrize("kw", _fuzz_cases())
+def test_seeded_random_parameters_all_families(kw):
+    """Couplings of either sign, fields that make some moves certain or impossible, temperatures from frozen to hot,
+    concentrations on both sides of the per-word / per-lane switch of the North-East rule: every family that accepts
+    the lattice must reproduce the oracle (families whose tables cannot express a "never" threshold refuse)."""
+    ran = 0
+    for family in FAMILIES:
+        lat = lsm.Lattice(**kw)
+        try:
+            lat.set_kernel(family)
+        except lsm.LsmError as e:
+            assert e.code == lsm.ERR_UNSUPPORTED
+            continue
+        if lat.kernel != family:                      # the library fell back (e.g. a "never" entry): covered by that family
+            continue
+        orc = O.Oracle(**kw)
+        got = lat.sweep_record(6).cpu().numpy()
+        assert np.array_equal(got, orc.sweep_record(6)), (family, kw)
+        assert_same_state(lat, orc)
+        ran += 1
+        lat.close()
+    assert ran >= 1
