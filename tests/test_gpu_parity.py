@@ -490,3 +490,54 @@ def test_seeded_random_parameters_all_families(kw):
         ran += 1
         lat.close()
     assert ran >= 1
+
+
+def _tile_fuzz_cases():
+    rng = np.random.default_rng(1209029601)
+    cases = []
+    while len(cases) < 16:
+        b = int(rng.choice([8, 16, 32, 64]))
+        lam = int(rng.choice([1, 2, 4, 8, 16, 32]))
+        bal = bool(rng.integers(0, 2))
+        if (b * b) % ((8 if bal else 2) * lam) != 0:
+            continue
+        if lam == 1 and b > 32:
+            continue                                  # one thread walking P/2 sub-steps of a big tile: slow, covered above
+        L = b * int(rng.choice([1, 2, 3, 5, 8]))
+        cases.append((L, b, lam, bal, float(rng.uniform(0.05, 0.49)), int(rng.choice([lsm.NE_HEATBATH, lsm.NE_METROPOLIS])),
+                      int(rng.integers(1, 2 ** 62))))
+    return cases
+
+
+@pytest.mark.parametrize("L,b,lam,bal,c,model,seed", _tile_fuzz_cases())
+def test_seeded_random_tile_schedules(L, b, lam, bal, c, model, seed):
+    kw = dict(dims=2, L=L, model=model, J=0.0, T=W.ne_temperature(c), seed=seed)
+    lat, orc = make_pair(**kw)
+    got = lat.sweep_random_tile(4, b, lam, record=True, balanced=bal).cpu().numpy()
+    if bal:
+        orc.sweep_random_tile_balanced(4, b, lam)
+        assert got[-1, 1] == orc.measure_int()[1]
+    else:
+        assert np.array_equal(got, orc.sweep_random_tile_record(4, b, lam))
+    assert_same_state(lat, orc)
+
+
+def test_checkpoint_roundtrip_random_states():
+    """get_spins / set_spins (word-granular and scalar conversion kernels) on arbitrary configurations: what goes in comes
+    out, flags and snapshot survive, and the run continues bit-exactly from the restored state and sweep counter."""
+    rng = np.random.default_rng(7)
+    for kw, values in ((dict(dims=2, L=96, T=2.3), (-1, 1)), (dict(dims=2, L=34, T=2.3), (-1, 1)),
+                       (dict(dims=3, L=32, two_S=2, T=3.0, h=0.01), (-1, 0, 1)), (dict(dims=3, L=6, two_S=2, T=3.0), (-1, 0, 1)),
+                       (dict(dims=2, L=64, model=lsm.NE_HEATBATH, J=0.0, T=1.0), (0, 1))):
+        lat, orc = make_pair(seed=11, **kw)
+        lat.sweep(3)
+        orc.sweep(3)
+        state = rng.choice(np.array(values, dtype=np.int8), size=lat.N)
+        import torch
+        lat.set_spins(torch.from_numpy(state).cuda(), 1000)
+        orc.set_spins(state, 1000)
+        assert np.array_equal(lat.get_spins().cpu().numpy(), state)
+        assert_same_state(lat, orc)                   # persistence / overlap against the untouched snapshot and flags
+        got = lat.sweep_record(4).cpu().numpy()
+        assert np.array_equal(got, orc.sweep_record(4))
+        assert_same_state(lat, orc)
