@@ -541,3 +541,51 @@ def test_checkpoint_roundtrip_random_states():
         got = lat.sweep_record(4).cpu().numpy()
         assert np.array_equal(got, orc.sweep_record(4))
         assert_same_state(lat, orc)
+
+
+@pytest.mark.parametrize("case", range(8))
+def test_seeded_random_operation_sequences(case):
+    """A handle driven through a random sequence of calls -- sweeps with and without record, kernel-family switches,
+    temperature changes, tracking off/on, reference resets, random-tile sweeps -- stays identical to the oracle driven
+    through the same sequence."""
+    rng = np.random.default_rng(4000 + case)
+    ne = case % 2 == 1
+    if ne:
+        kw = dict(dims=2, L=int(rng.choice([64, 128])), model=int(rng.choice([lsm.NE_HEATBATH, lsm.NE_METROPOLIS])), J=0.0,
+                  T=W.ne_temperature(float(rng.uniform(0.1, 0.45))))
+    else:
+        kw = dict(dims=int(rng.choice([2, 3])), L=32, two_S=int(rng.choice([1, 2])), T=float(rng.uniform(1.5, 5.0)),
+                  h=float(rng.choice([0.0, 0.05])))
+    kw["seed"] = int(rng.integers(1, 2 ** 62))
+    lat, orc = make_pair(**kw)
+    tracking = True
+    for step in range(14):
+        op = int(rng.integers(0, 7))
+        n = int(rng.integers(1, 5))
+        if op == 0:
+            lat.sweep(n)
+            orc.sweep(n)
+        elif op == 1:
+            assert np.array_equal(lat.sweep_record(n).cpu().numpy(), orc.sweep_record(n)), (case, step)
+        elif op == 2:
+            try:
+                lat.set_kernel(int(rng.choice(FAMILIES + [lsm.KERNEL_AUTO])))
+            except lsm.LsmError as e:
+                assert e.code == lsm.ERR_UNSUPPORTED
+        elif op == 3:
+            T = W.ne_temperature(float(rng.uniform(0.1, 0.45))) if ne else float(rng.uniform(1.0, 6.0))
+            lat.set_temperature(T)
+            orc.set_temperature(T)
+        elif op == 4:
+            tracking = not tracking
+            lat.set_tracking(tracking)
+            if tracking:
+                orc.reset_reference()                 # switching tracking on is a reference reset (include/lsm.h)
+        elif op == 5 and tracking:
+            lat.reset_reference()
+            orc.reset_reference()
+        elif op == 6 and ne:
+            bal = bool(rng.integers(0, 2))
+            lat.sweep_random_tile(n, 32, 16, balanced=bal)
+            (orc.sweep_random_tile_balanced if bal else orc.sweep_random_tile)(n, 32, 16)
+        assert_same_state(lat, orc, check_persistence=tracking)
