@@ -71,7 +71,14 @@ enum {
     LSM_ERR_WORKSPACE = -4,   /* workspace too small or not 256-byte aligned                   */
     LSM_ERR_STATE = -5        /* call needs tracking to be on (lsm_persistence)                */
 };
-/* Kernel families (lsm_set_kernel).  AUTO picks the fastest one that supports the lattice. */
+/* Kernel families (lsm_set_kernel).  AUTO picks the fastest one that supports the lattice:
+ *  SMALL    one launch for all sweeps of a call: lattice slabs in the shared memory of a thread-block cluster,
+ *           cluster barrier between the colours (L a power of two >= 8; other L with L % 32 == 0 up to 32 768
+ *           sites); chosen up to 262 144 sites (512^2, 64^3);
+ *  TILED    one launch per half-sweep, 16 sites per 128-bit word (L % 32 == 0, no "never" threshold);
+ *  RESIDENT one cooperative launch for all sweeps with neighbour-flag synchronisation (opt-in, large lattices);
+ *  GENERIC  one thread per site, any even L >= 4, any table.
+ * All families produce bit-identical results (same random-word map D2, same thresholds D3). */
 enum { LSM_KERNEL_AUTO = 0, LSM_KERNEL_GENERIC = 1, LSM_KERNEL_TILED = 2, LSM_KERNEL_RESIDENT = 3, LSM_KERNEL_SMALL = 4 };
 
 /* Device bytes lsm_create needs for this lattice (two colour arrays + small state). */
