@@ -258,10 +258,19 @@ def test_zero_sweeps_and_temperature_change():
     assert lat.launch_count > 0
 
 
-def test_sweep_counter_above_32_bits():
-    """The 64-bit sweep counter reaches the Philox counter's c3 field (reading D2)."""
-    kw = dict(dims=2, L=32, T=2.269, seed=11)
-    lat, orc = make_pair(**kw)
+@pytest.mark.parametrize("family", FAMILIES)
+@pytest.mark.parametrize("kw", [dict(dims=2, L=32, T=2.269), dict(dims=2, L=1024, T=2.269),
+                                dict(dims=3, L=32, two_S=2, T=3.0, h=0.01),
+                                dict(dims=2, L=64, model=lsm.NE_HEATBATH, J=0.0, T=W.ne_temperature(0.3))])
+def test_sweep_counter_above_32_bits(kw, family):
+    """The 64-bit sweep counter reaches the Philox counter's c3 field (reading D2), also when the counter's low word
+    wraps in the middle of a call (kernels that run several sweeps per launch compute it on the device)."""
+    lat, orc = make_pair(seed=11, **kw)
+    try:
+        lat.set_kernel(family)
+    except lsm.LsmError as e:
+        assert e.code == lsm.ERR_UNSUPPORTED
+        pytest.skip("this family does not cover this lattice")
     t0 = (5 << 32) + 0xFFFFFFFE
     s = orc.get_spins()
     lat.set_spins_host(s, t0)
@@ -269,6 +278,13 @@ def test_sweep_counter_above_32_bits():
     got = lat.sweep_record(4).cpu().numpy()
     assert np.array_equal(got, orc.sweep_record(4))
     assert_same_state(lat, orc, check_persistence=False)
+    if kw.get("model", lsm.ISING) != lsm.ISING:
+        lat.set_spins_host(s, t0)
+        orc.set_spins(s, t0)
+        for bal in (False, True):
+            lat.sweep_random_tile(3, 32, 16, balanced=bal)
+            (orc.sweep_random_tile_balanced if bal else orc.sweep_random_tile)(3, 32, 16)
+        assert_same_state(lat, orc, check_persistence=False)
 
 
 FULL = [
