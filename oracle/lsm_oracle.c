@@ -22,6 +22,13 @@
  *                          3^16 states (P8)
  *   NE ................... product measure (P11), first-sweep persistence
  *                          closed form (P12), frozen-set bound (P13)
+ *   NE random tiles ...... (orc_sweep_random_tile, and its
+ *                          balance-preserving variant)
+ *                          dict-keyed Python restatement with its own Philox on
+ *                          collision-heavy tiles, tile-order independence,
+ *                          product measure, closed-form first-sweep persistence,
+ *                          frozen-set bound, serial limit Q = lambda = 1
+ *                          (tests/test_oracle_random_tile.py)
  *   "parity unpinned": none of the functions; the unpinned items are
  *   particular non-equilibrium VALUES, not code paths.
  *
