@@ -27,7 +27,8 @@
  *  LSM_ISING, two_S = 2 : s_i in {-1,0,+1}, same H; trial move = one of the two other
  *                         values, chosen uniformly (D5; BASELINE.json config 4).
  *  LSM_NE_HEATBATH      : North-East model, occupation n_i in {0,1},
- *                         J = 0, H = sum n_i, c = 1/(1+exp(1/T)) (D6).  A site may change
+ *                         J = 0, H = sum n_i, c = 1/(1+exp(1/T)) (D6: the paper's +/-1 spins give
+ *                         c = 1/(1+exp(2/T_paper)), i.e. T_paper = 2 T here).  A site may change
  *                         only if its north (x,y+1) and east (x+1,y) neighbours are both
  *                         up (D8); then n_i is redrawn from Bernoulli(c) (D7).
  *  LSM_NE_METROPOLIS    : same constraint, Metropolis flip: 1->0 always,
@@ -41,7 +42,9 @@
  * One sweep (= one Monte Carlo step) = half-sweep over parity 0, then over
  *  parity 1 (the two kernel launches of PAPER.md:96-97; D9) = N attempted updates.
  * Random numbers: Philox4x32-10, key = seed, counter = (site group, sweep, half) (D2).
- *  The handle keeps a 64-bit sweep counter t; sweep t uses counter field t.
+ *  The handle keeps a 64-bit sweep counter t < 2^60; sweep t uses counter fields c2 = lo32(t),
+ *  c3 = tag | hi32(t) << 4, the low four bits of c3 being the stream tag alone (0/1 = half-sweep,
+ *  2 = initial state, 4/5 and 8..11 = random-tile launches), so streams never alias (D2).
  *
  * Values at the boundary (int8): spin-1/2 -> {-1,+1}; spin-1 -> {-1,0,+1}; NE -> {0,1};
  *  canonical order.  The device-internal encoding (split even/odd colour arrays, flag
@@ -110,8 +113,10 @@ int lsm_sweep_record_host(lsm_t *, int64_t n, int64_t *h_obs, int64_t *d_scratch
  * right, Fig. 4) are those of the launch start; the picks of a sub-step read the tile as the sub-step found it;
  * on a same-site collision the highest thread wins; Philox counter (tile, sub-step * ceil(lambda/2) + thread/2,
  * sweep, 4 + launch).  d_obs: NULL, or device [n][2] receiving (0, M) after every sweep.  Asynchronous.
- * UNSUPPORTED unless tile_edge is a power of two in [8, 128] dividing L, lambda a power of two in [1, 32] and
- * 2 * lambda divides P.  Shares the sweep counter with lsm_sweep. */
+ * UNSUPPORTED unless tile_edge is a power of two in [8, 128] dividing L, lambda a power of two in [1, 32],
+ * 2 * lambda divides P, and the 32/lambda tiles a warp holds fit the block's shared memory:
+ * (32/lambda) * ((b+1)*b + b + (lambda > 1 ? b*b : 0)) <= 200 KB with b = tile_edge, which refuses
+ * tile_edge = 128 with lambda <= 4 and tile_edge = 64 with lambda = 1.  Shares the sweep counter with lsm_sweep. */
 int lsm_sweep_random_tile(lsm_t *, int64_t n, int tile_edge, int lambda, int64_t *d_obs, void *stream);
 /* Its balance-preserving variant ("~2.5x slower"): a sub-step is lambda picks among the tile's red
  * sites, a barrier, lambda picks among its white sites, a barrier; four launches complete one MC step.  Readings
@@ -142,7 +147,8 @@ int lsm_set_tracking(lsm_t *, int on, void *stream);
 /* Configuration in canonical order, N int8 values. */
 int lsm_get_spins(lsm_t *, int8_t *d_out, void *stream);
 int lsm_get_spins_host(lsm_t *, int8_t *h_out, int8_t *d_scratch /* N bytes */, void *stream);
-/* Replace configuration and sweep counter, recompute (B, M); snapshot and flags untouched.
+/* Replace configuration and sweep counter (LSM_ERR_ARG unless sweep_counter < 2^60), recompute (B, M);
+ * snapshot and flags untouched.
  * Values outside the model's set give LSM_ERR_ARG only for NULL; they are not range-checked. */
 int lsm_set_spins(lsm_t *, const int8_t *d_in, uint64_t sweep_counter, void *stream);
 int lsm_set_spins_host(lsm_t *, const int8_t *h_in, int8_t *d_scratch /* N bytes */,

@@ -94,7 +94,9 @@ void orc_philox4x32_10(const uint32_t ctr[4], const uint32_t key[2], uint32_t ou
 /* Random words of one site (reading D2 detail).
  * stream: 0 = half-sweep of parity 0, 1 = parity 1, 2 = initial state.
  * group g and sweep t fill the 128-bit counter as
- *   c0 = lo32(g), c1 = hi32(g), c2 = lo32(t), c3 = stream | (hi32(t) << 2). */
+ *   c0 = lo32(g), c1 = hi32(g), c2 = lo32(t), c3 = stream | (hi32(t) << 4):
+ * the low four bits of c3 belong to the stream tag alone (tags 0..15; t < 2^60),
+ * so no two (tag, t) pairs share a counter (reading D2). */
 static void words_of_group(uint64_t seed, uint64_t g, uint64_t t, uint32_t stream,
                            uint32_t out[4])
 {
@@ -102,7 +104,7 @@ static void words_of_group(uint64_t seed, uint64_t g, uint64_t t, uint32_t strea
     ctr[0] = (uint32_t)g;
     ctr[1] = (uint32_t)(g >> 32);
     ctr[2] = (uint32_t)t;
-    ctr[3] = stream | ((uint32_t)(t >> 32) << 2);
+    ctr[3] = stream | ((uint32_t)(t >> 32) << 4);
     key[0] = (uint32_t)seed;
     key[1] = (uint32_t)(seed >> 32);
     orc_philox4x32_10(ctr, key, out);
@@ -357,7 +359,7 @@ void orc_sweep(orc_t *o, int64_t n) { orc_sweep_ordered(o, n, 0); }
  *   D20 thread j picks r = floor(w_pos * P / 2^32), (px, py) = (r mod b, r div b);
  *       the update rule is that of reading D7 with acceptance word w_acc.
  *   D21 Philox counter c0 = tile id (tx + (L/b)*ty), c1 = k*ceil(lambda/2) + (j>>1)
- *       for sub-step k and thread j, c2 = lo32(t), c3 = (4 + launch) | hi32(t)<<2;
+ *       for sub-step k and thread j, c2 = lo32(t), c3 = (4 + launch) | hi32(t)<<4;
  *       w_pos = word 2(j&1), w_acc = word 2(j&1)+1.
  * tiles_descending != 0 walks the tiles in reverse order (pin: same result). */
 int orc_sweep_random_tile(orc_t *o, int64_t n, int b, int lambda, int tiles_descending)
@@ -385,7 +387,7 @@ int orc_sweep_random_tile(orc_t *o, int64_t n, int b, int lambda, int tiles_desc
                         ctr[0] = (uint32_t)T;
                         ctr[1] = (uint32_t)(k * calls + (j >> 1));
                         ctr[2] = (uint32_t)o->t;
-                        ctr[3] = (4u + launch) | ((uint32_t)(o->t >> 32) << 2);
+                        ctr[3] = (4u + launch) | ((uint32_t)(o->t >> 32) << 4);
                         orc_philox4x32_10(ctr, key, w);
                         uint32_t w_pos = w[2 * (j & 1)], w_acc = w[2 * (j & 1) + 1];
                         int r = (int)(((uint64_t)w_pos * (uint64_t)P) >> 32);
@@ -435,7 +437,7 @@ int orc_sweep_random_tile(orc_t *o, int64_t n, int b, int lambda, int tiles_desc
  *       barrier) with q * 2 lambda = P/4, so that the step attempts P updates per tile like the base algorithm
  *       (twice the launches, tile copies and barriers for the same attempts: the paper's "~2.5x slower").
  *   D24 thread j of sub-step k draws ONE Philox call: counter c0 = tile id, c1 = k*lambda + j, c2 = lo32(t),
- *       c3 = (8 + launch) | hi32(t)<<2; words 0, 1 = position and acceptance of its red pick, words 2, 3 of its
+ *       c3 = (8 + launch) | hi32(t)<<4; words 0, 1 = position and acceptance of its red pick, words 2, 3 of its
  *       white pick.  Position: r = floor(w_pos * (P/2) / 2^32) is the r-th site of that colour in the tile in
  *       row-major order: py = r div (b/2), px = 2 (r mod (b/2)) + ((py + colour) & 1)   (tile origins are even).
  *   D18 (boundaries frozen at launch start), D19 (picks of a phase read the phase's start; highest thread
@@ -466,7 +468,7 @@ int orc_sweep_random_tile_balanced(orc_t *o, int64_t n, int b, int lambda, int t
                             ctr[0] = (uint32_t)T;
                             ctr[1] = (uint32_t)(k * lambda + j);
                             ctr[2] = (uint32_t)o->t;
-                            ctr[3] = (8u + launch) | ((uint32_t)(o->t >> 32) << 2);
+                            ctr[3] = (8u + launch) | ((uint32_t)(o->t >> 32) << 4);
                             orc_philox4x32_10(ctr, key, w);
                             uint32_t w_pos = w[2 * colour], w_acc = w[2 * colour + 1];
                             int r = (int)(((uint64_t)w_pos * (uint64_t)(P / 2)) >> 32);
@@ -510,6 +512,17 @@ int orc_sweep_random_tile_record(orc_t *o, int64_t n, int b, int lambda, int64_t
 {
     for (int64_t k = 0; k < n; ++k) {
         int rc = orc_sweep_random_tile(o, 1, b, lambda, 0);
+        if (rc != 0) return rc;
+        orc_measure(o, &obs[2 * k], &obs[2 * k + 1]);
+    }
+    return 0;
+}
+
+/* Same for the balance-preserving variant: obs[2*k] = 0, obs[2*k+1] = M after MC step k of this call. */
+int orc_sweep_random_tile_balanced_record(orc_t *o, int64_t n, int b, int lambda, int64_t *obs)
+{
+    for (int64_t k = 0; k < n; ++k) {
+        int rc = orc_sweep_random_tile_balanced(o, 1, b, lambda, 0);
         if (rc != 0) return rc;
         orc_measure(o, &obs[2 * k], &obs[2 * k + 1]);
     }

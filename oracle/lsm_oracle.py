@@ -22,6 +22,11 @@ import numpy as np
 _HERE = os.path.dirname(os.path.abspath(__file__))
 _SRC = os.path.join(_HERE, "lsm_oracle.c")
 _LIB = os.path.join(_HERE, "liblsm_oracle.so")
+# tests/test_oracle_mutants.py points this at a deliberately broken copy of lsm_oracle.c to prove that the pins
+# notice; nothing else sets it.
+if os.environ.get("LSM_ORACLE_SRC"):
+    _SRC = os.path.abspath(os.environ["LSM_ORACLE_SRC"])
+    _LIB = _SRC + ".so"
 
 ISING, NE_HEATBATH, NE_METROPOLIS = 0, 1, 2
 
@@ -76,6 +81,8 @@ def lib():
         L.orc_sweep_random_tile_balanced.argtypes = [vp, i64, i32, i32, i32]
         L.orc_sweep_random_tile_record.restype = i32
         L.orc_sweep_random_tile_record.argtypes = [vp, i64, i32, i32, vp]
+        L.orc_sweep_random_tile_balanced_record.restype = i32
+        L.orc_sweep_random_tile_balanced_record.argtypes = [vp, i64, i32, i32, vp]
         _lib = L
     return _lib
 
@@ -132,6 +139,12 @@ class Oracle:
         obs = np.zeros((int(n), 2), dtype=np.int64)
         if lib().orc_sweep_random_tile_record(self._h, int(n), int(b), int(lam), obs.ctypes.data) != 0:
             raise ValueError("random-tile schedule: NE model, b | L and 2*lambda | b*b required")
+        return obs
+
+    def sweep_random_tile_balanced_record(self, n, b=32, lam=16):
+        obs = np.zeros((int(n), 2), dtype=np.int64)
+        if lib().orc_sweep_random_tile_balanced_record(self._h, int(n), int(b), int(lam), obs.ctypes.data) != 0:
+            raise ValueError("balanced random-tile schedule: NE model, even b | L and 8*lambda | b*b required")
         return obs
 
     def measure_int(self):

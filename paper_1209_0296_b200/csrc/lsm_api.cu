@@ -422,7 +422,7 @@ extern "C" int lsm_get_spins_host(lsm_t *o, int8_t *h_out, int8_t *d_scratch, vo
 
 extern "C" int lsm_set_spins(lsm_t *o, const int8_t *d_in, uint64_t sweep_counter, void *stream)
 {
-    if (!o || !d_in) return LSM_ERR_ARG;
+    if (!o || !d_in || (sweep_counter >> 60) != 0) return LSM_ERR_ARG;   // D2: the tag owns the low 4 bits of c3
     o->last_stream = (cudaStream_t)stream;
     CU(launch_set_spins(o->lat, o->model, d_in, o->last_stream));
     o->launches += 1;

@@ -61,7 +61,7 @@ __device__ __forceinline__ uint4 philox4x32_10(uint32_t c0, uint32_t c1, uint32_
     return make_uint4(c0, c1, c2, c3);
 }
 
-// Counter fields of reading D2: c0/c1 = group, c2 = lo32(t), c3 = stream | hi32(t) << 2.
+// Counter fields of reading D2: c0/c1 = group, c2 = lo32(t), c3 = stream | hi32(t) << 4 (tag in the low 4 bits, t < 2^60).
 struct SweepKey {
     uint32_t k0, k1;   // seed
     uint32_t c2, c3;   // sweep and stream tag of this half-sweep
@@ -72,7 +72,7 @@ __host__ __device__ inline SweepKey make_sweep_key(unsigned long long seed, unsi
     k.k0 = (uint32_t)seed;
     k.k1 = (uint32_t)(seed >> 32);
     k.c2 = (uint32_t)t;
-    k.c3 = stream | ((uint32_t)(t >> 32) << 2);
+    k.c3 = stream | ((uint32_t)(t >> 32) << 4);
     return k;
 }
 

@@ -267,7 +267,7 @@ cudaError_t launch_ne_random_tile(const Lat &lat, uint8_t *const dst[2], bool me
         a.rk1[r] = a.k1 + (uint32_t)r * PHILOX_W1;
     }
     a.c2 = (uint32_t)t;
-    a.c3 = ((balanced ? 8u : 4u) + (uint32_t)launch) | ((uint32_t)(t >> 32) << 2);   // D21: tags 4, 5; D24: 8..11
+    a.c3 = ((balanced ? 8u : 4u) + (uint32_t)launch) | ((uint32_t)(t >> 32) << 4);   // D21: tags 4, 5; D24: 8..11
     a.thr_c = thr_c;
     a.thr_up = thr_up;
     a.up_always = up_always;

@@ -39,7 +39,7 @@ def reference_sweep(n, L, b, lam, seed, t, thr, metropolis):
             for k in range(q):
                 writes = {}
                 for j in range(lam):
-                    w = philox_py((T, k * calls + (j >> 1), t & 0xFFFFFFFF, (4 + launch) | ((t >> 32) << 2)), key)
+                    w = philox_py((T, k * calls + (j >> 1), t & 0xFFFFFFFF, (4 + launch) | (((t >> 32) << 4) & 0xFFFFFFFF)), key)
                     w_pos, w_acc = w[2 * (j & 1)], w[2 * (j & 1) + 1]
                     r = (w_pos * P) >> 32
                     x, y = tx * b + r % b, ty * b + r // b
@@ -203,7 +203,7 @@ def reference_sweep_balanced(n, L, b, lam, seed, t, thr, metropolis):
                 for col in (0, 1):
                     writes = {}
                     for j in range(lam):
-                        w = philox_py((T, k * lam + j, t & 0xFFFFFFFF, (8 + launch) | ((t >> 32) << 2)), key)
+                        w = philox_py((T, k * lam + j, t & 0xFFFFFFFF, (8 + launch) | (((t >> 32) << 4) & 0xFFFFFFFF)), key)
                         w_pos, w_acc = w[2 * col], w[2 * col + 1]
                         x, y = sites[col][(w_pos * (P // 2)) >> 32]
                         nb = []
