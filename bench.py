@@ -30,9 +30,20 @@ BYTES_PER_UPDATE = 3  # read own colour, read other colour, write own colour (in
 # 1/4 Philox4x32-10 call = 5 wide multiplies + 5 three-input XORs, + 1 compare + 1 merge
 INT_SLOTS_PER_UPDATE = 12
 INT_SLOTS_PER_UPDATE_SPIN1 = 22
-# dram__bytes_read.sum + dram__bytes_write.sum per half-sweep launch of the cfg2 workload, from the one
-# `ncu --set full` capture summarised in profiles/r1_tiled_ncu_full.md (caches flushed by ncu before the launch)
-NCU_DRAM_BYTES_PER_LAUNCH = {"cfg2_T2.269": 67.18e6 + 0.83e6}
+# dram__bytes_read.sum + dram__bytes_write.sum per half-sweep launch, from the `ncu --set full` captures summarised
+# under profiles/ (caches flushed by ncu before the launch): workload -> (bytes, summary file)
+NCU_DRAM_BYTES_PER_LAUNCH = {
+    "cfg2_T2.269": (67.18e6 + 0.83e6, "profiles/r1_tiled_ncu_full.md"),
+    "cfg3": (138.46e6 + 28.19e6, "profiles/r2_tiled_variants_ncu.md"),
+    "cfg4": (16.86e6 + 0.0e6, "profiles/r2_tiled_variants_ncu.md"),
+    "cfg5_c0.10": (67.19e6 + 1.22e6, "profiles/r2_tiled_variants_ncu.md"),
+    "cfg5_c0.30": (67.18e6 + 0.75e6, "profiles/r2_tiled_variants_ncu.md"),
+    "hbm3d_1024": (1083.86e6 + 497.63e6, "profiles/r2_tiled_variants_ncu.md"),
+}
+KERNEL_FAMILY = {1: "generic", 2: "tiled", 3: "resident", 4: "small"}
+KERNEL_NAME = {1: "k_sweep_generic (half-sweep)", 2: "k_sweep_tiled (half-sweep)",
+               3: "k_sweep_resident (per half-sweep share of one launch)",
+               4: "k_sweep_small_lane (per half-sweep share of one launch)"}
 
 
 def parse():
@@ -46,7 +57,9 @@ def parse():
     ap.add_argument("--no-extras", action="store_true", help="skip the secondary workloads / cpu baseline")
     ap.add_argument("--size-scan", action="store_true",
                     help="instead of the benchmark: us/sweep of the tiled and the small (cluster) family over lattice sizes")
-    ap.add_argument("--kernel", default="auto", choices=["auto", "generic", "tiled", "resident"],
+    ap.add_argument("--pipe-probe", action="store_true",
+                    help="instead of the benchmark: the integer-pipe microbenchmarks behind the 'alu' roofline (DESIGN.md 6)")
+    ap.add_argument("--kernel", default="auto", choices=["auto", "generic", "tiled", "resident", "small"],
                     help="kernel family (lsm_set_kernel); auto = the library's choice")
     return ap.parse_args()
 
@@ -196,7 +209,8 @@ def run_ours(args, w):
     if wl.model == lsm.ISING:
         lat.set_tracking(False)  # persistence is not part of configs 1-4
     if args.kernel != "auto":
-        lat.set_kernel({"generic": lsm.KERNEL_GENERIC, "tiled": lsm.KERNEL_TILED, "resident": lsm.KERNEL_RESIDENT}[args.kernel])
+        lat.set_kernel({"generic": lsm.KERNEL_GENERIC, "tiled": lsm.KERNEL_TILED, "resident": lsm.KERNEL_RESIDENT,
+                        "small": lsm.KERNEL_SMALL}[args.kernel])
     N = lat.N
     obs = torch.empty((S, 2), dtype=torch.int64, device=lat.device)
     flush = torch.empty(256 << 20, dtype=torch.uint8, device=lat.device)  # > 126 MB L2
@@ -257,32 +271,11 @@ def run_ours(args, w):
             dist.destroy_process_group()
         return 0
 
-    # ---- roofline of the dominant kernel (the half-sweep kernel), DESIGN.md 6.
-    # The path is bound by integer-pipe instruction slots (measured: paper_1209_0296_b200.pipe_probe),
-    # not by HBM bytes; the HBM view is reported next to it.
-    hbm_peak, peak_src, _ = measured_peaks()
+    # ---- roofline of the dominant kernel (the half-sweep kernel), DESIGN.md 6
     n_sweep_launches = 2 * S * K
     avg_launch_s = (sum(step_ms) * 1e-3) / n_sweep_launches
-    updates_per_launch = N // 2
     sm_count = torch.cuda.get_device_properties(local).multi_processor_count
-    sm_max_mhz = clocks.get("sm_max_mhz") or 1965
-    slots = INT_SLOTS_PER_UPDATE_SPIN1 if wl.two_S == 2 else INT_SLOTS_PER_UPDATE
-    alu_peak = sm_count * 64 * sm_max_mhz * 1e6 / 1e9           # G integer instruction slots / s
-    alu_achieved = slots * updates_per_launch / avg_launch_s / 1e9
-    roofline = {"bound": "alu", "achieved": alu_achieved, "peak": alu_peak, "unit": "Gslot/s",
-                "frac": alu_achieved / alu_peak,
-                "traffic": NCU_DRAM_BYTES_PER_LAUNCH.get(wl.name) if lat.kernel == 2 else None,
-                "traffic_unit": "bytes per launch (ncu dram read+write, cold L2; algorithmic = 3 B x updates_per_launch)",
-                "peak_source": f"{sm_count} SMs x 64 integer lanes/clk x clocks.max.sm {sm_max_mhz} MHz (DESIGN.md 6; pipe_probe)",
-                "kernel": {2: "k_sweep_tiled (half-sweep)", 3: "k_sweep_resident (per half-sweep share of one launch)"}.get(
-                    lat.kernel, "k_sweep_generic (half-sweep)"),
-                "algorithmic_int_slots_per_update": slots, "updates_per_launch": updates_per_launch,
-                "avg_launch_us": avg_launch_s * 1e6}
-    hbm_achieved = BYTES_PER_UPDATE * updates_per_launch / avg_launch_s / 1e9
-    roofline_hbm = {"bound": "hbm", "achieved": hbm_achieved, "peak": hbm_peak, "unit": "GB/s",
-                    "frac": hbm_achieved / hbm_peak, "peak_source": peak_src,
-                    "algorithmic_bytes_per_update": BYTES_PER_UPDATE,
-                    "note": "context only: the 64 MiB lattice is L2-resident, DRAM traffic is far below the algorithmic bytes"}
+    roofline, roofline_hbm = rooflines(wl, lat.kernel, avg_launch_s, sm_count, clocks.get("sm_max_mhz") or 1965)
 
     line = {
         "metric": "site_updates_per_sec", "value": value, "unit": "Gflips/s", "n_gpus": world, "steps": K,
@@ -291,8 +284,8 @@ def run_ours(args, w):
         "config": {"workload": wl.name, "lattice": f"{wl.L}^{wl.dims}", "model": "Ising spin-1/2" if wl.two_S == 1 and wl.model == 0 else wl.note,
                    "T": wl.T, "J": wl.J, "h": wl.h, "sweeps_per_step": S, "record": "(B, M) after every sweep",
                    "parallelism": "replicas only" if world > 1 else "single GPU",
-                   "kernel_family": {1: "generic", 2: "tiled", 3: "resident"}.get(lat.kernel, "?"),
-                   "l2": "256 MiB flush write between timed steps; the 64 MiB lattice is re-read from L2 within a step"},
+                   "kernel_family": KERNEL_FAMILY.get(lat.kernel, "?"),
+                   "l2": "256 MiB flush write between timed steps; within a step a lattice smaller than the 126 MB L2 is re-read from L2"},
         "roofline": roofline,
         "roofline_hbm": roofline_hbm,
         "e2e": {"value": e2e_value, "unit": "Gflips/s", "h2d_bytes_per_step": N, "d2h_bytes_per_step": 16 * S,
@@ -304,7 +297,7 @@ def run_ours(args, w):
 
     if not args.no_extras and world == 1:
         line["philox_only"] = philox_microbench(lsm, torch)
-        line["other_workloads"] = other_workloads(lsm, torch, w.name)
+        line["other_workloads"] = other_workloads(lsm, torch, w.name, sm_count, clocks.get("sm_max_mhz") or 1965)
         from paper_1209_0296_b200 import workloads as W
 
         sweeps = 4
@@ -317,6 +310,40 @@ def run_ours(args, w):
     if world > 1:
         dist.destroy_process_group()
     return 0
+
+
+def rooflines(w, family, avg_launch_s, sm_count, sm_max_mhz):
+    """Both rooflines of one half-sweep launch and which of them binds this workload.
+
+    alu: integer instruction slots (12 per update for one Philox word per site, 22 for two) against
+         SMs x 64 lanes x max SM clock -- one 16-lane math instruction per 2 cycles and sub-partition, the rate
+         `bench.py --pipe-probe` measures on this GPU;
+    hbm: 3 algorithmic bytes per update against the measured copy bandwidth (MEASURED_PEAKS.json)."""
+    hbm_peak, peak_src, _ = measured_peaks()
+    updates_per_launch = w.N // 2
+    slots = INT_SLOTS_PER_UPDATE_SPIN1 if w.two_S == 2 else INT_SLOTS_PER_UPDATE
+    alu_peak = sm_count * 64 * sm_max_mhz * 1e6 / 1e9           # G integer instruction slots / s
+    alu_achieved = slots * updates_per_launch / avg_launch_s / 1e9
+    hbm_achieved = BYTES_PER_UPDATE * updates_per_launch / avg_launch_s / 1e9
+    binding = "alu" if alu_peak / slots < hbm_peak / BYTES_PER_UPDATE else "hbm"
+    traffic = NCU_DRAM_BYTES_PER_LAUNCH.get(w.name) if family == 2 else None
+    roofline = {"bound": "alu", "achieved": alu_achieved, "peak": alu_peak, "unit": "Gslot/s",
+                "frac": alu_achieved / alu_peak,
+                "traffic": traffic[0] if traffic else None,
+                "traffic_source": traffic[1] if traffic else None,
+                "traffic_unit": "bytes per launch (ncu dram read+write, cold L2; algorithmic = 3 B x updates_per_launch)",
+                "peak_source": f"{sm_count} SMs x 64 integer lanes/clk x clocks.max.sm {sm_max_mhz} MHz (DESIGN.md 6; bench.py --pipe-probe)",
+                "kernel": KERNEL_NAME.get(family, "?"), "binding_bound": binding,
+                "bound_gflips": {"alu": alu_peak / slots, "hbm": hbm_peak / BYTES_PER_UPDATE},
+                "algorithmic_int_slots_per_update": slots, "updates_per_launch": updates_per_launch,
+                "avg_launch_us": avg_launch_s * 1e6}
+    lattice_mib = w.N / 2 ** 20
+    roofline_hbm = {"bound": "hbm", "achieved": hbm_achieved, "peak": hbm_peak, "unit": "GB/s",
+                    "frac": hbm_achieved / hbm_peak, "peak_source": peak_src,
+                    "algorithmic_bytes_per_update": BYTES_PER_UPDATE,
+                    "note": (f"the {lattice_mib:.0f} MiB lattice is L2-resident between launches: DRAM traffic is below the algorithmic bytes"
+                             if lattice_mib < 100 else f"the {lattice_mib:.0f} MiB lattice exceeds the 126 MB L2: every launch streams it from HBM")}
+    return roofline, roofline_hbm
 
 
 def philox_microbench(lsm, torch):
@@ -336,16 +363,17 @@ def philox_microbench(lsm, torch):
             "updates_bound_gflips_1word": 4 * calls_s / 1e9, "updates_bound_gflips_2words": 2 * calls_s / 1e9}
 
 
-def other_workloads(lsm, torch, skip):
+def other_workloads(lsm, torch, skip, sm_count, sm_max_mhz):
     """Short timings of the other BASELINE.json configs (context for the headline number)."""
     from paper_1209_0296_b200 import workloads as W
 
     out = {}
     for name, sweeps in (("cfg1", 1000), ("cfg2_T2.0", 100), ("cfg2_T2.6", 100), ("cfg3", 40), ("cfg4", 100),
-                         ("cfg5_c0.10", 100), ("cfg5_c0.20", 100), ("cfg5_c0.30", 100)):
+                         ("cfg5_c0.10", 100), ("cfg5_c0.20", 100), ("cfg5_c0.30", 100), ("hbm3d_1024", 6),
+                         ("cold2d_T0.30", 100)):
         if name == skip:
             continue
-        w = W.configs()[name]
+        w = W.by_name(name)
         try:
             lat = lsm.Lattice(**w.create_args())
             if w.model == lsm.ISING:
@@ -365,7 +393,12 @@ def other_workloads(lsm, torch, skip):
             s = e0.elapsed_time(e1) * 1e-3
             gf = w.N * sweeps * reps / s / 1e9
             out[name] = {"gflips": gf, "alg_GBps": gf * BYTES_PER_UPDATE, "us_per_sweep": s / (sweeps * reps) * 1e6,
-                         "kernel_family": lat.kernel}
+                         "kernel_family": KERNEL_FAMILY.get(lat.kernel, "?")}
+            if lat.kernel == 2:           # one launch per half-sweep: the per-launch rooflines apply
+                r, rh = rooflines(w, lat.kernel, s / (2 * sweeps * reps), sm_count, sm_max_mhz)
+                out[name]["roofline"] = {k: r[k] for k in ("bound", "achieved", "peak", "unit", "frac", "traffic",
+                                                           "traffic_source", "binding_bound", "avg_launch_us")}
+                out[name]["roofline_hbm"] = {k: rh[k] for k in ("achieved", "peak", "unit", "frac", "note")}
             if name == "cfg5_c0.30":
                 # the paper's corrected North-East algorithm on the same lattice (32 x 32 tiles,
                 # lambda = 16 is the paper's best configuration)
@@ -427,7 +460,7 @@ def size_scan():
             row[name] = {"us_per_sweep": ms * 1e3 / n, "gflips": lat.N * n / ms / 1e6}
             lat.close()
         lat = lsm.Lattice(dims=dims, L=L, T=2.269 if dims == 2 else 4.5115, seed=3)
-        row["auto_family"] = {1: "generic", 2: "tiled", 3: "resident", 4: "small"}.get(lat.kernel)
+        row["auto_family"] = KERNEL_FAMILY.get(lat.kernel)
         lat.close()
         rows.append(row)
         print(json.dumps(row), flush=True)
@@ -460,15 +493,77 @@ def size_scan():
     return 0
 
 
+PROBE_MODES = [
+    # mode, stream per loop iteration and thread, wide multiplies, other IMADs, ALU-pipe instructions
+    (0, "16 LOP3", 0, 0, 16),
+    (1, "8 IMAD", 0, 8, 0),
+    (2, "8 IMAD.WIDE (+8 adds)", 8, 0, 8),
+    (3, "8 IMAD + 16 LOP3", 0, 8, 16),
+    (4, "4 Philox calls (80 WIDE + 80 LOP3)", 80, 0, 80),
+    (5, "4 Philox calls + 80 LOP3", 80, 0, 160),
+    (6, "4 Philox calls + 160 LOP3", 80, 0, 240),
+    (7, "4 Philox calls + 240 LOP3", 80, 0, 320),
+    (8, "4 Philox calls + 80 IMAD", 80, 80, 80),
+    (9, "4 Philox calls + 80 IMAD + 80 LOP3", 80, 80, 160),
+    (10, "4 Philox calls + 80 IMAD + 160 LOP3", 80, 80, 240),
+]
+
+
+def pipe_probe(blocks_per_sm=8, iters=1024):
+    """Register-only integer instruction streams (csrc/probe/pipe_probe.cu, its own libpipe_probe.so): cycles per loop
+    iteration and warp against the issue law of DESIGN.md 6 -- every 16-lane math instruction (ALU or FMA-heavy pipe)
+    takes one 2-cycle issue slot of its sub-partition, a wide multiply additionally keeps the multiplier busy for 4:
+    cycles = max(4 W + 2 I, 2 (W + I + A) + 2 x 3 loop instructions)."""
+    import ctypes
+
+    import torch
+
+    from paper_1209_0296_b200 import build
+
+    lib = ctypes.CDLL(build.build_probe())
+    lib.pipe_probe_run.restype = ctypes.c_int
+    lib.pipe_probe_run.argtypes = [ctypes.c_int, ctypes.c_int, ctypes.c_int, ctypes.c_void_p, ctypes.c_void_p]
+    props = torch.cuda.get_device_properties(0)
+    sms = props.multi_processor_count
+    try:
+        import pynvml
+
+        pynvml.nvmlInit()
+        mhz = pynvml.nvmlDeviceGetMaxClockInfo(pynvml.nvmlDeviceGetHandleByIndex(0), pynvml.NVML_CLOCK_SM)
+    except Exception:
+        mhz = 1965
+    warps_per_smsp = blocks_per_sm * 8 / 4.0
+    blocks = sms * blocks_per_sm
+    sink = torch.empty(blocks * 256, dtype=torch.int32, device="cuda")
+    stream = ctypes.c_void_p(torch.cuda.current_stream().cuda_stream)
+    print(f"# {props.name}  clocks.max.sm {mhz} MHz  {warps_per_smsp:.0f} warps per sub-partition, {iters} iterations")
+    print("| stream | measured cycles/iter/warp | law max(4W+2I, 2(W+I+A+3)) | math instr per cycle and sub-partition |")
+    print("|---|---|---|---|")
+    for mode, name, Wd, I, A in PROBE_MODES:
+        assert lib.pipe_probe_run(mode, blocks, 32, sink.data_ptr(), stream) == 0
+        torch.cuda.synchronize()
+        e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        e0.record()
+        assert lib.pipe_probe_run(mode, blocks, iters, sink.data_ptr(), stream) == 0
+        e1.record()
+        torch.cuda.synchronize()
+        cyc = e0.elapsed_time(e1) * 1e-3 * mhz * 1e6 / iters / warps_per_smsp
+        law = max(4 * Wd + 2 * I, 2 * (Wd + I + A + 3))
+        print(f"| {name} | {cyc:.1f} | {law} | {(Wd + I + A + 3) / cyc:.3f} |")
+    return 0
+
+
 def main():
     args = parse()
+    if args.pipe_probe:
+        return pipe_probe()
     if args.size_scan:
         # more hardware queues than the default 8, so that more than 8 handles can sweep side by side
         os.environ.setdefault("CUDA_DEVICE_MAX_CONNECTIONS", "32")
         return size_scan()
     from paper_1209_0296_b200 import workloads as W
 
-    w = W.configs()[args.workload]
+    w = W.by_name(args.workload)
     if args.impl == "reference":
         return run_reference(args, w)
     return run_ours(args, w)

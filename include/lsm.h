@@ -169,6 +169,9 @@ int lsm_get_launch_count(lsm_t *, uint64_t *kernels_launched); /* kernels this h
 /* Host-side derived doubles from the integer series (D11-D13), exact integer accumulation. */
 int lsm_binder_u4(const int64_t *obs /* [n][2] host */, int64_t n, double *U4);   /* 1 - <M^4>/(3<M^2>^2) */
 int lsm_heat_capacity(const int64_t *obs, int64_t n, int64_t N, double J, double h, double T, double *C_per_site);
+/* Per-site means of a recorded series: e = <E>/N with E = -J*B - h*M (D1), abs_m = <|M|>/N (the
+ * energy and magnetisation curves of Fig. 6).  Either out-pointer may be NULL. */
+int lsm_series_means(const int64_t *obs, int64_t n, int64_t N, double J, double h, double *e_per_site, double *abs_m_per_site);
 int lsm_phi(int64_t overlap, int64_t N, double c, double *phi);                  /* PAPER.md:120 Eq. 4, D11 */
 int lsm_persistence_fraction(int64_t never_changed, int64_t N, double *P);
 int lsm_energy(int model, double J, double h, int64_t bond_sum, int64_t M, double *E);
@@ -179,11 +182,6 @@ int lsm_energy(int model, double J, double h, int64_t bond_sum, int64_t M, doubl
  * calls and writes one word to d_sink[blocks*256]. */
 int lsm_philox_device(const uint32_t *d_ctr_key, uint32_t *d_out, int64_t n, void *stream);
 int lsm_philox_throughput(int blocks, int calls, uint32_t *d_sink, void *stream);
-/* lsm_pipe_probe: register-only integer instruction streams that show how the ALU and FMA pipes share
- * issue.  mode 0: 16 LOP3, 1: 8 IMAD, 2: 8 IMAD.WIDE, 3: 8 IMAD + 16 LOP3, 4: 4 Philox calls,
- * 5/6/7: 4 Philox calls + 80/160/240 independent LOP3 -- per loop iteration and thread; `blocks` x 256
- * threads run `iters` iterations and write one word each to d_sink[blocks*256]. */
-int lsm_pipe_probe(int mode, int blocks, int iters, uint32_t *d_sink, void *stream);
 
 const char *lsm_strerror(int code);
 const char *lsm_last_cuda_error(void);

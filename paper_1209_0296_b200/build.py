@@ -23,8 +23,25 @@ NVCC_FLAGS = [
 ]
 
 
+PROBE_LIB = os.path.join(PKG, "libpipe_probe.so")
+PROBE_SRC = os.path.join(CSRC, "probe", "pipe_probe.cu")
+
+
+def build_probe(force: bool = False) -> str:
+    """libpipe_probe.so: the integer-pipe microbenchmarks behind `bench.py --pipe-probe` (not part of liblsm.so)."""
+    if not force and os.path.exists(PROBE_LIB) and os.path.getmtime(PROBE_LIB) >= os.path.getmtime(PROBE_SRC):
+        return PROBE_LIB
+    tmp = PROBE_LIB + f".tmp{os.getpid()}"
+    r = subprocess.run([os.environ.get("NVCC", "nvcc"), *NVCC_FLAGS, "-o", tmp, PROBE_SRC], capture_output=True, text=True)
+    if r.returncode != 0:
+        sys.stderr.write(r.stdout + r.stderr)
+        raise RuntimeError("nvcc failed building libpipe_probe.so")
+    os.replace(tmp, PROBE_LIB)
+    return PROBE_LIB
+
+
 def _inputs():
-    out = [os.path.join(CSRC, f) for f in os.listdir(CSRC) if f.endswith((".cu", ".cuh", ".h"))]
+    out = [os.path.join(CSRC, f) for f in os.listdir(CSRC) if f.endswith((".cu", ".cuh", ".h"))]   # not csrc/probe/
     out.append(os.path.join(os.path.dirname(PKG), "include", "lsm.h"))
     return out
 

@@ -513,6 +513,21 @@ extern "C" int lsm_heat_capacity(const int64_t *obs, int64_t n, int64_t N, doubl
     return LSM_OK;
 }
 
+extern "C" int lsm_series_means(const int64_t *obs, int64_t n, int64_t N, double J, double h, double *e, double *abs_m)
+{
+    if (!obs || n <= 0 || N <= 0) return LSM_ERR_ARG;
+    __int128 sB = 0, sM = 0, sA = 0;
+    for (int64_t k = 0; k < n; ++k) {
+        sB += obs[2 * k];
+        sM += obs[2 * k + 1];
+        sA += obs[2 * k + 1] < 0 ? -(__int128)obs[2 * k + 1] : (__int128)obs[2 * k + 1];
+    }
+    const long double den = (long double)n * (long double)N;
+    if (e) *e = (double)((-(long double)J * (long double)sB - (long double)h * (long double)sM) / den);
+    if (abs_m) *abs_m = (double)((long double)sA / den);
+    return LSM_OK;
+}
+
 extern "C" int lsm_phi(int64_t overlap, int64_t N, double c, double *phi)
 {
     if (!phi || N <= 0) return LSM_ERR_ARG;
@@ -541,13 +556,6 @@ extern "C" int lsm_philox_throughput(int blocks, int calls, uint32_t *d_sink, vo
 {
     if (blocks <= 0 || calls < 0 || !d_sink) return LSM_ERR_ARG;
     CU(launch_philox_throughput(blocks, calls, d_sink, (cudaStream_t)stream));
-    return LSM_OK;
-}
-
-extern "C" int lsm_pipe_probe(int mode, int blocks, int iters, uint32_t *d_sink, void *stream)
-{
-    if (mode < 0 || mode > 10 || blocks <= 0 || iters < 0 || !d_sink) return LSM_ERR_ARG;
-    CU(launch_pipe_probe(mode, blocks, iters, d_sink, (cudaStream_t)stream));
     return LSM_OK;
 }
 

@@ -560,71 +560,4 @@ cudaError_t launch_philox_throughput(int blocks, int calls, uint32_t *d_sink, cu
     return cudaGetLastError();
 }
 
-// Integer-pipe probe: register-only instruction streams whose timing shows how the ALU
-// pipe (LOP3/IADD3/ISETP/PRMT) and the FMA-heavy pipe (IMAD, IMAD.WIDE) share issue on this GPU.
-//   mode 0: 16 LOP3            1: 8 IMAD (32-bit)          2: 8 IMAD.WIDE.U32 (+8 adds)
-//        3: 8 IMAD + 16 LOP3   4: 4 Philox calls           5/6/7: 4 Philox calls + 80/160/240 LOP3
-//        8/9/10: 4 Philox calls + 80 IMAD + 0/80/160 LOP3
-// per loop iteration and thread.
-#define LSM_PROBE_LOP(a, b, c) a = (a ^ b) & (c | 0x55555555u);
-template <int MODE>
-__global__ void __launch_bounds__(256) k_pipe_probe(int iters, uint32_t *__restrict__ sink, uint32_t k0, uint32_t k1)
-{
-    uint32_t tid = blockIdx.x * blockDim.x + threadIdx.x;
-    uint32_t a[8], b[8];
-#pragma unroll
-    for (int i = 0; i < 8; ++i) { a[i] = (tid * (i + 1)) ^ k0; b[i] = tid + i * 77u + k1; }
-    uint32_t acc = 0;
-    constexpr int NLOP = MODE == 0 ? 8 : MODE == 3 ? 8 : MODE == 5 ? 40 : MODE == 6 ? 80 : MODE == 7 ? 120 : MODE == 9 ? 40 : MODE == 10 ? 80 : 0;
-    constexpr int NIMAD = MODE >= 8 ? 80 : 0;   // modes 8-10: 4 Philox calls + 80 IMAD (+ 80 / 160 LOP3)
-#pragma unroll 1
-    for (int it = 0; it < iters; ++it) {
-        if (MODE == 1 || MODE == 3) {
-#pragma unroll
-            for (int i = 0; i < 8; ++i) a[i] = a[i] * 0x9E3779B9u + b[i];
-        }
-        if (MODE == 2) {
-#pragma unroll
-            for (int i = 0; i < 8; ++i) {
-                unsigned long long p = (unsigned long long)a[i] * PHILOX_M0;
-                a[i] = (uint32_t)(p >> 32) + (uint32_t)p;
-            }
-        }
-        if (MODE >= 4) {
-#pragma unroll
-            for (int c = 0; c < 4; ++c) {
-                uint4 r = philox4x32_10(tid * 4u + c, 0u, (uint32_t)it, 1u, k0, k1);
-                acc ^= r.x ^ r.y ^ r.z ^ r.w;
-            }
-        }
-#pragma unroll
-        for (int i = 0; i < NIMAD; ++i) a[i & 7] = a[i & 7] * 0x9E3779B9u + a[(i + 3) & 7];
-#pragma unroll
-        for (int i = 0; i < NLOP; ++i) LSM_PROBE_LOP(b[i & 7], b[(i + 1) & 7], b[(i + 3) & 7])
-    }
-#pragma unroll
-    for (int i = 0; i < 8; ++i) acc ^= a[i] ^ b[i];
-    sink[tid] = acc;
-}
-
-cudaError_t launch_pipe_probe(int mode, int blocks, int iters, uint32_t *d_sink, cudaStream_t s)
-{
-    const uint32_t k0 = 0x1234567u, k1 = 0x89abcdefu;
-    switch (mode) {
-    case 0: k_pipe_probe<0><<<blocks, 256, 0, s>>>(iters, d_sink, k0, k1); break;
-    case 1: k_pipe_probe<1><<<blocks, 256, 0, s>>>(iters, d_sink, k0, k1); break;
-    case 2: k_pipe_probe<2><<<blocks, 256, 0, s>>>(iters, d_sink, k0, k1); break;
-    case 3: k_pipe_probe<3><<<blocks, 256, 0, s>>>(iters, d_sink, k0, k1); break;
-    case 4: k_pipe_probe<4><<<blocks, 256, 0, s>>>(iters, d_sink, k0, k1); break;
-    case 5: k_pipe_probe<5><<<blocks, 256, 0, s>>>(iters, d_sink, k0, k1); break;
-    case 6: k_pipe_probe<6><<<blocks, 256, 0, s>>>(iters, d_sink, k0, k1); break;
-    case 7: k_pipe_probe<7><<<blocks, 256, 0, s>>>(iters, d_sink, k0, k1); break;
-    case 8: k_pipe_probe<8><<<blocks, 256, 0, s>>>(iters, d_sink, k0, k1); break;
-    case 9: k_pipe_probe<9><<<blocks, 256, 0, s>>>(iters, d_sink, k0, k1); break;
-    case 10: k_pipe_probe<10><<<blocks, 256, 0, s>>>(iters, d_sink, k0, k1); break;
-    default: return cudaErrorInvalidValue;
-    }
-    return cudaGetLastError();
-}
-
 }  // namespace lsmk

@@ -158,7 +158,6 @@ cudaError_t launch_get_spins(const Lat &lat, int model, int8_t *d_out, cudaStrea
 cudaError_t launch_set_spins(const Lat &lat, int model, const int8_t *d_in, cudaStream_t s);
 cudaError_t launch_philox_device(const uint32_t *d_ck, uint32_t *d_out, long long n, cudaStream_t s);
 cudaError_t launch_philox_throughput(int blocks, int calls, uint32_t *d_sink, cudaStream_t s);
-cudaError_t launch_pipe_probe(int mode, int blocks, int iters, uint32_t *d_sink, cudaStream_t s);
 
 // North-East random-tile schedule (lsm_ne_tile.cu): reads lat.col, writes dst.
 bool ne_tile_supported(const Lat &lat, int b, int lam, bool balanced);

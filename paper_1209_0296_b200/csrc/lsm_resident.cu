@@ -41,7 +41,6 @@ struct ResidentArgs {
     long long *obs;              // [nsweeps][2] (B, M) slots, zeroed by the host; or nullptr
     unsigned *flags;             // first[grid] then done[grid]: progress words of every CTA
     unsigned epoch0;             // value of every flag when the launch starts
-    int dbg;                     // tuning experiments only (LSM_RESIDENT_DBG): 1 = no waiting, 2 = no nanosleep
 };
 
 __device__ __forceinline__ unsigned ld_relaxed_gpu(const unsigned *p)
@@ -60,7 +59,6 @@ struct ResidentHooks {
     unsigned *first_me;
     const unsigned *done_end;    // done[] word of the neighbour on the side where the march ends
     unsigned need;               // epoch0 + g
-    int dbg;
     __device__ __forceinline__ void after_first()
     {
         __syncthreads();
@@ -71,7 +69,7 @@ struct ResidentHooks {
     }
     __device__ __forceinline__ void before_last()
     {
-        if (threadIdx.x == 0 && dbg != 1) {
+        if (threadIdx.x == 0) {
             while ((int)(ld_relaxed_gpu(done_end) - need) < 0) __nanosleep(32);
             __threadfence();
         }
@@ -113,7 +111,7 @@ k_sweep_resident(const __grid_constant__ ResidentArgs a, const __grid_constant__
         const bool up = half == 0;                  // nhalves is even: directions alternate across sweeps too
         const unsigned long long t = a.t0 + (unsigned long long)(gh >> 1);
         const unsigned need = a.epoch0 + (unsigned)gh;
-        if (gh > 0 && a.dbg != 1) {
+        if (gh > 0) {
             if (threadIdx.x < 3) {
                 const unsigned *w = first + (up ? below : above);                             // start side
                 if (threadIdx.x == 1) w = done + seg * a.nb + (cb == 0 ? a.nb - 1 : cb - 1);  // cross axis
@@ -123,7 +121,7 @@ k_sweep_resident(const __grid_constant__ ResidentArgs a, const __grid_constant__
             }
             __syncthreads();
         }
-        ResidentHooks hk = {first + blockIdx.x, done + (up ? above : below), need, a.dbg};
+        ResidentHooks hk = {first + blockIdx.x, done + (up ? above : below), need};
 
         PhiloxDyn pc = {0u, 0u, 0u, 0u, pk};
         philox_half_consts(make_sweep_key(a.seed, t, (uint32_t)half), pk.rk0, pk.rk1, pc.x1, pc.y2, pc.z2, pc.w3);
@@ -176,12 +174,6 @@ k_sweep_resident(const __grid_constant__ ResidentArgs a, const __grid_constant__
 // Host side
 // ------------------------------------------------------------------------------------------
 PhiloxSweepConsts make_philox_consts(const SweepKey &k);   // lsm_tiled.cu
-
-static int env_int(const char *name, int dflt)
-{
-    const char *v = getenv(name);
-    return (v && *v) ? atoi(v) : dflt;
-}
 
 template <int MODEL, int DIMS, bool TRACK, int OBS>
 static cudaError_t launch_one(int grid, cudaStream_t s, const ResidentArgs &a, const PhiloxSweepConsts &pk,
@@ -265,8 +257,6 @@ bool resident_plan(const Lat &lat, int model, int track, const TiledTables &t, R
         if (dispatch(model, lat.dims, track != 0, obs, 0, 0, dummy, pk, t, &c, 256) != cudaSuccess) return false;
         if (obs == 0 || c < cap) cap = c;
     }
-    const int limit = env_int("LSM_RESIDENT_MAX_CTAS", cap);
-    if (limit < cap) cap = limit;
     if (cap > RESIDENT_MAX_CTAS / 2) cap = RESIDENT_MAX_CTAS / 2;    // two flag words per CTA
     long long S = cap / nb;
     if (S > lat.L) S = lat.L;
@@ -304,7 +294,6 @@ cudaError_t launch_sweep_resident(const Lat &lat, int model, int track, unsigned
     a.obs = d_obs;
     a.flags = d_flags;
     a.epoch0 = epoch0;
-    a.dbg = env_int("LSM_RESIDENT_DBG", 0);
     SweepKey k = make_sweep_key(seed, t0, 0u);
     PhiloxSweepConsts pk = make_philox_consts(k);     // only the round keys are used by the resident kernel
     return dispatch(model, lat.dims, track != 0, d_obs != nullptr, plan.grid, s, a, pk, t, nullptr, plan.bs);

@@ -304,18 +304,15 @@ static cudaError_t small_launch_to(bool track, bool obs, int threads, cudaStream
     return cudaGetLastError();
 }
 
-static int small_max_cluster()
-{
-    const char *v = getenv("LSM_SMALL_MAX_CLUSTER");
-    const int c = (v && *v) ? atoi(v) : 16;
-    return c < 1 ? 1 : c > 16 ? 16 : c;
-}
-
-static int small_max_sites()
-{
-    const char *v = getenv("LSM_SMALL_MAX_SITES");
-    return (v && *v) ? atoi(v) : 262144;   // above 512^2 / 64^3 the tiled family wins (profiles/r1_small_family.md)
-}
+// Compile-time knobs for tuning experiments; the library reads no environment variables.
+#ifndef LSM_SMALL_MAX_CLUSTER
+#define LSM_SMALL_MAX_CLUSTER 16         // B200 schedules 16-block clusters
+#endif
+#ifndef LSM_SMALL_MAX_SITES
+#define LSM_SMALL_MAX_SITES 262144       // above 512^2 / 64^3 the tiled family wins (profiles/r1_small_family.md)
+#endif
+static int small_max_cluster() { return LSM_SMALL_MAX_CLUSTER; }
+static int small_max_sites() { return LSM_SMALL_MAX_SITES; }
 
 // Plan: every word column gets as many march segments as 1024 threads allow.
 bool small_plan(const Lat &lat, int model, const TiledTables &t, SmallPlan *out, bool ignore_size_limit)
@@ -335,19 +332,12 @@ bool small_plan(const Lat &lat, int model, const TiledTables &t, SmallPlan *out,
     out->threads = (int)(((ncol * S + 31) / 32) * 32);
     out->lane = 0;
     out->cluster = 1;
-    const char *v = getenv("LSM_SMALL_LANE");
-    const bool want_lane = !(v && *v == '0');
-    if (want_lane && pow2) {    // power of two: lane-granular threads, index math by shifts
+    if (pow2) {    // power of two: lane-granular threads, index math by shifts
         const long long nlanes = lat.half / 4;
         // thread blocks of the cluster: >= 128 lanes (4 warps) each, at most 16 (B200 schedules 16-block clusters;
         // measured: profiles/r1_small_family.md) -- a half-sweep of a small lattice is bound by latency, not issue
         int c = 1;
         while (c < small_max_cluster() && nlanes / (2 * c) >= 128 && 2 * c <= lat.L) c *= 2;
-        const char *vc = getenv("LSM_SMALL_CLUSTER");
-        if (vc && *vc) {
-            const int want = atoi(vc);
-            if (want >= 1 && want <= 16 && (want & (want - 1)) == 0 && want <= lat.L && nlanes / want >= 32) c = want;
-        }
         if (N / c <= 196608) {                          // the slab must fit shared memory
             out->lane = 1;
             out->cluster = c;

@@ -158,15 +158,20 @@ bool tiled_supported(const Lat &lat, int model, const TiledTables &t)
 }
 
 // Launch shape: threads = word columns x march segments, one wave of CTAS_PER_SM resident CTAs per
-// SM (finer segments do not help: measured, profiles/).  Overridable for tuning experiments.
-static int env_int(const char *name, int dflt)
-{
-    const char *v = getenv(name);
-    return (v && *v) ? atoi(v) : dflt;
-}
-static int g_tiled_ctas_per_sm = env_int("LSM_TILED_CTAS_PER_SM", 0);   // 0: tiled_minblocks(model)
-static int g_tiled_waves_x4 = env_int("LSM_TILED_WAVES_X4", 4);   // waves in quarters
-static int g_tiled_pdl = env_int("LSM_TILED_PDL", 1);               // programmatic dependent launch
+// SM (finer segments do not help: measured, profiles/).  Compile-time knobs for tuning experiments
+// (-DLSM_TILED_...); the library reads no environment variables.
+#ifndef LSM_TILED_CTAS_PER_SM
+#define LSM_TILED_CTAS_PER_SM 0          // 0: tiled_minblocks(model)
+#endif
+#ifndef LSM_TILED_WAVES_X4
+#define LSM_TILED_WAVES_X4 4             // waves in quarters
+#endif
+#ifndef LSM_TILED_PDL
+#define LSM_TILED_PDL 1                  // programmatic dependent launch
+#endif
+static const int g_tiled_ctas_per_sm = LSM_TILED_CTAS_PER_SM;
+static const int g_tiled_waves_x4 = LSM_TILED_WAVES_X4;
+static const int g_tiled_pdl = LSM_TILED_PDL;
 
 template <int MODEL, int DIMS, bool TRACK>
 static cudaError_t launch_obs(int obs_mode, dim3 grid, cudaStream_t s, const TiledGeom &g, const PhiloxSweepConsts &pc,

@@ -48,12 +48,12 @@ SIGNATURES = {
     "lsm_get_launch_count": (_i32, [_vp, _P(_u64)]),
     "lsm_binder_u4": (_i32, [_vp, _i64, _P(_dbl)]),
     "lsm_heat_capacity": (_i32, [_vp, _i64, _i64, _dbl, _dbl, _dbl, _P(_dbl)]),
+    "lsm_series_means": (_i32, [_vp, _i64, _i64, _dbl, _dbl, _P(_dbl), _P(_dbl)]),
     "lsm_phi": (_i32, [_i64, _i64, _dbl, _P(_dbl)]),
     "lsm_persistence_fraction": (_i32, [_i64, _i64, _P(_dbl)]),
     "lsm_energy": (_i32, [_i32, _dbl, _dbl, _i64, _i64, _P(_dbl)]),
     "lsm_philox_device": (_i32, [_vp, _vp, _i64, _vp]),
     "lsm_philox_throughput": (_i32, [_i32, _i32, _vp, _vp]),
-    "lsm_pipe_probe": (_i32, [_i32, _i32, _i32, _vp, _vp]),
     "lsm_strerror": (ctypes.c_char_p, [_i32]),
     "lsm_last_cuda_error": (ctypes.c_char_p, []),
 }
@@ -98,11 +98,25 @@ def _check(code, where):
         raise LsmError(code, where)
 
 
-def _stream_ptr(stream):
+def _stream_ptr(stream, device=None):
     import torch
 
-    s = torch.cuda.current_stream() if stream is None else stream
+    s = torch.cuda.current_stream(device) if stream is None else stream
     return ctypes.c_void_p(s.cuda_stream)
+
+
+def _on_device(fn):
+    """Run a Lattice method with the lattice's GPU current: the library launches on the calling thread's current
+    device, and the default stream is that device's current stream."""
+    import functools
+
+    @functools.wraps(fn)
+    def wrapped(self, *a, **kw):
+        import torch
+
+        with torch.cuda.device(self.device):
+            return fn(self, *a, **kw)
+    return wrapped
 
 
 def workspace_bytes(dims, L, two_S=1, model=ISING) -> int:
@@ -125,20 +139,31 @@ class Lattice:
         self.device = torch.device(device)
         self.N = self.L ** self.dims
         nbytes = workspace_bytes(dims, L, two_S, model)
+        self._h = None
+        self._last_stream = None
         with torch.cuda.device(self.device):
             self._ws = torch.empty(nbytes + 256, dtype=torch.uint8, device=self.device)
             off = (-self._ws.data_ptr()) % 256
             self._ws_ptr = self._ws.data_ptr() + off
             h_ = _vp()
             _check(self._lib.lsm_create(self.dims, self.L, self.two_S, self.model, self.J, self.h, self.T,
-                                        self.seed, _vp(self._ws_ptr), nbytes, _stream_ptr(stream),
+                                        self.seed, _vp(self._ws_ptr), nbytes, self._sp(stream),
                                         ctypes.byref(h_)), "lsm_create")
         self._h = h_
         self._scratch = None
 
+    def _sp(self, stream):
+        import torch
+
+        self._last_stream = torch.cuda.current_stream(self.device) if stream is None else stream
+        return ctypes.c_void_p(self._last_stream.cuda_stream)
+
     # ------------------------------------------------------------------ life cycle
+    @_on_device
     def close(self):
         if getattr(self, "_h", None):
+            if self._last_stream is not None:
+                self._last_stream.synchronize()      # work may still be in flight on a stream other than the allocator's
             self._lib.lsm_destroy(self._h)
             self._h = None
             self._ws = None
@@ -158,9 +183,11 @@ class Lattice:
         return self._scratch
 
     # ------------------------------------------------------------------ sweeps
+    @_on_device
     def sweep(self, n=1, stream=None):
-        _check(self._lib.lsm_sweep(self._h, int(n), _stream_ptr(stream)), "lsm_sweep")
+        _check(self._lib.lsm_sweep(self._h, int(n), self._sp(stream)), "lsm_sweep")
 
+    @_on_device
     def sweep_record(self, n, out=None, stream=None):
         """n sweeps; returns a device int64 tensor [n, 2] = (B, M) after each sweep (asynchronous)."""
         import torch
@@ -168,10 +195,11 @@ class Lattice:
         if out is None:
             out = torch.empty((int(n), 2), dtype=torch.int64, device=self.device)
         assert out.is_cuda and out.dtype == torch.int64 and out.is_contiguous() and out.numel() >= 2 * int(n)
-        _check(self._lib.lsm_sweep_record(self._h, int(n), _vp(out.data_ptr()), _stream_ptr(stream)),
+        _check(self._lib.lsm_sweep_record(self._h, int(n), _vp(out.data_ptr()), self._sp(stream)),
                "lsm_sweep_record")
         return out
 
+    @_on_device
     def sweep_random_tile(self, n=1, b=32, lam=16, record=False, out=None, stream=None, balanced=False):
         """North-East model: n sweeps of the paper's corrected algorithm: random picks of `lam`
         threads in tiles of b x b spins; balanced=True: its balance-preserving variant.
@@ -182,10 +210,11 @@ class Lattice:
             out = torch.empty((int(n), 2), dtype=torch.int64, device=self.device)
         ptr = _vp(out.data_ptr()) if out is not None else None
         fn = self._lib.lsm_sweep_random_tile_balanced if balanced else self._lib.lsm_sweep_random_tile
-        _check(fn(self._h, int(n), int(b), int(lam), ptr, _stream_ptr(stream)),
+        _check(fn(self._h, int(n), int(b), int(lam), ptr, self._sp(stream)),
                "lsm_sweep_random_tile_balanced" if balanced else "lsm_sweep_random_tile")
         return out
 
+    @_on_device
     def sweep_record_host(self, n, h_obs=None, stream=None):
         """n sweeps with the (B, M) series delivered into a HOST array (pinned torch tensor or numpy)."""
         import torch
@@ -194,64 +223,74 @@ class Lattice:
             h_obs = torch.empty((int(n), 2), dtype=torch.int64).pin_memory()
         ptr = h_obs.data_ptr() if hasattr(h_obs, "data_ptr") else h_obs.ctypes.data
         sc = self._dev_scratch(16 * max(int(n), 1))
-        _check(self._lib.lsm_sweep_record_host(self._h, int(n), _vp(ptr), _vp(sc.data_ptr()), _stream_ptr(stream)),
+        _check(self._lib.lsm_sweep_record_host(self._h, int(n), _vp(ptr), _vp(sc.data_ptr()), self._sp(stream)),
                "lsm_sweep_record_host")
         return h_obs
 
     # ------------------------------------------------------------------ observables
+    @_on_device
     def measure(self):
         E, M = _dbl(), _i64()
         _check(self._lib.lsm_measure(self._h, ctypes.byref(E), ctypes.byref(M)), "lsm_measure")
         return float(E.value), int(M.value)
 
+    @_on_device
     def measure_int(self):
         B, M, t = _i64(), _i64(), _u64()
         _check(self._lib.lsm_measure_int(self._h, ctypes.byref(B), ctypes.byref(M), ctypes.byref(t)),
                "lsm_measure_int")
         return int(B.value), int(M.value), int(t.value)
 
+    @_on_device
     def measure_full(self):
         B, M = _i64(), _i64()
         _check(self._lib.lsm_measure_full(self._h, ctypes.byref(B), ctypes.byref(M)), "lsm_measure_full")
         return int(B.value), int(M.value)
 
+    @_on_device
     def persistence(self):
         a, b = _i64(), _i64()
         _check(self._lib.lsm_persistence(self._h, ctypes.byref(a), ctypes.byref(b)), "lsm_persistence")
         return int(a.value), int(b.value)
 
+    @_on_device
     def reset_reference(self, stream=None):
-        _check(self._lib.lsm_reset_reference(self._h, _stream_ptr(stream)), "lsm_reset_reference")
+        _check(self._lib.lsm_reset_reference(self._h, self._sp(stream)), "lsm_reset_reference")
 
+    @_on_device
     def set_tracking(self, on, stream=None):
-        _check(self._lib.lsm_set_tracking(self._h, 1 if on else 0, _stream_ptr(stream)), "lsm_set_tracking")
+        _check(self._lib.lsm_set_tracking(self._h, 1 if on else 0, self._sp(stream)), "lsm_set_tracking")
 
     # ------------------------------------------------------------------ configuration I/O
+    @_on_device
     def get_spins(self, out=None, stream=None):
         import torch
 
         if out is None:
             out = torch.empty(self.N, dtype=torch.int8, device=self.device)
         assert out.is_cuda and out.dtype == torch.int8 and out.numel() == self.N and out.is_contiguous()
-        _check(self._lib.lsm_get_spins(self._h, _vp(out.data_ptr()), _stream_ptr(stream)), "lsm_get_spins")
+        _check(self._lib.lsm_get_spins(self._h, _vp(out.data_ptr()), self._sp(stream)), "lsm_get_spins")
         return out
 
+    @_on_device
     def get_spins_host(self, h_out=None, stream=None):
         if h_out is None:
             h_out = np.empty(self.N, dtype=np.int8)
         ptr = h_out.data_ptr() if hasattr(h_out, "data_ptr") else h_out.ctypes.data
         sc = self._dev_scratch(self.N)
-        _check(self._lib.lsm_get_spins_host(self._h, _vp(ptr), _vp(sc.data_ptr()), _stream_ptr(stream)),
+        _check(self._lib.lsm_get_spins_host(self._h, _vp(ptr), _vp(sc.data_ptr()), self._sp(stream)),
                "lsm_get_spins_host")
         return h_out
 
+    @_on_device
     def set_spins(self, d_in, sweep_counter, stream=None):
         import torch
 
         assert d_in.is_cuda and d_in.dtype == torch.int8 and d_in.numel() == self.N and d_in.is_contiguous()
-        _check(self._lib.lsm_set_spins(self._h, _vp(d_in.data_ptr()), int(sweep_counter), _stream_ptr(stream)),
+        _check(self._lib.lsm_set_spins(self._h, _vp(d_in.data_ptr()), int(sweep_counter), self._sp(stream)),
                "lsm_set_spins")
 
+    @_on_device
     def set_spins_host(self, h_in, sweep_counter, stream=None):
         if hasattr(h_in, "data_ptr"):
             ptr, n = h_in.data_ptr(), h_in.numel()
@@ -261,12 +300,14 @@ class Lattice:
         assert n == self.N
         sc = self._dev_scratch(self.N)
         _check(self._lib.lsm_set_spins_host(self._h, _vp(ptr), _vp(sc.data_ptr()), int(sweep_counter),
-                                            _stream_ptr(stream)), "lsm_set_spins_host")
+                                            self._sp(stream)), "lsm_set_spins_host")
 
+    @_on_device
     def set_temperature(self, T):
         _check(self._lib.lsm_set_temperature(self._h, float(T)), "lsm_set_temperature")
         self.T = float(T)
 
+    @_on_device
     def thresholds(self):
         buf = (_u64 * 128)()
         n = _i32()
@@ -274,16 +315,19 @@ class Lattice:
         return [int(buf[i]) for i in range(n.value)]
 
     # ------------------------------------------------------------------ kernel family / counters
+    @_on_device
     def set_kernel(self, family):
         _check(self._lib.lsm_set_kernel(self._h, int(family)), "lsm_set_kernel")
 
     @property
+    @_on_device
     def kernel(self):
         k = _i32()
         _check(self._lib.lsm_get_kernel(self._h, ctypes.byref(k)), "lsm_get_kernel")
         return int(k.value)
 
     @property
+    @_on_device
     def launch_count(self):
         n = _u64()
         _check(self._lib.lsm_get_launch_count(self._h, ctypes.byref(n)), "lsm_get_launch_count")
@@ -304,6 +348,15 @@ def heat_capacity(obs, N, J, h, T) -> float:
     _check(load().lsm_heat_capacity(_vp(a.ctypes.data), a.shape[0], int(N), float(J), float(h), float(T),
                                     ctypes.byref(out)), "lsm_heat_capacity")
     return float(out.value)
+
+
+def series_means(obs, N, J, h) -> tuple[float, float]:
+    """(<E>/N, <|M|>/N) of a recorded (B, M) series."""
+    a = np.ascontiguousarray(obs, dtype=np.int64).reshape(-1, 2)
+    e, m = _dbl(), _dbl()
+    _check(load().lsm_series_means(_vp(a.ctypes.data), a.shape[0], int(N), float(J), float(h), ctypes.byref(e),
+                                   ctypes.byref(m)), "lsm_series_means")
+    return float(e.value), float(m.value)
 
 
 def phi(overlap, N, c) -> float:
@@ -343,14 +396,4 @@ def philox_throughput(blocks, calls, stream=None):
     sink = torch.empty(blocks * 256, dtype=torch.int32, device="cuda")
     _check(load().lsm_philox_throughput(int(blocks), int(calls), _vp(sink.data_ptr()), _stream_ptr(stream)),
            "lsm_philox_throughput")
-    return sink
-
-
-def pipe_probe(mode, blocks, iters, stream=None):
-    """Enqueue one integer-pipe probe stream (see include/lsm.h); returns the sink tensor."""
-    import torch
-
-    sink = torch.empty(blocks * 256, dtype=torch.int32, device="cuda")
-    _check(load().lsm_pipe_probe(int(mode), int(blocks), int(iters), _vp(sink.data_ptr()), _stream_ptr(stream)),
-           "lsm_pipe_probe")
     return sink

@@ -31,14 +31,13 @@ def temperatures(T_start: float, T_stop: float, T_step: float) -> list[float]:
 
 
 def summarise(obs: np.ndarray, N: int, J: float, h: float, T: float) -> dict:
-    """Per-site averages over a measured (B, M) series (integers in, doubles out)."""
-    B, M = obs[:, 0].astype(object), obs[:, 1].astype(object)
-    n = len(obs)
-    e = float(-J * float(sum(B)) - h * float(sum(M))) / (n * N)
+    """Per-site averages over a measured (B, M) series: every number comes from the library (lsm_series_means,
+    lsm_heat_capacity, lsm_binder_u4: exact integer accumulation, one rounding at the end)."""
+    e, abs_m = lsm.series_means(obs, N, J, h)
     return {
         "T": T,
         "e": e,
-        "abs_m": float(sum(abs(int(v)) for v in M)) / (n * N),
+        "abs_m": abs_m,
         "c": lsm.heat_capacity(obs, N, J, h, T),
         "u4": lsm.binder_u4(obs),
     }

@@ -67,3 +67,22 @@ def configs() -> dict[str, Workload]:
                                          T=ne_temperature(c), seed=seed_of(5, v), sweeps=100_000,
                                          note="2D North-East heat-bath 8192^2, persistence every 100 sweeps")
     return out
+
+
+def extras() -> dict[str, Workload]:
+    """Workloads beyond BASELINE.json's five, used by bench.py for the rooflines: a lattice far larger than the
+    126 MB L2 (the HBM-streaming case SURVEY.md 8(d) asks for -- config 3's 128 MiB is borderline), and a cold
+    2D lattice whose table has "never" entries (exp(-8/T) < 2^-32 below T ~ 0.36)."""
+    out = {}
+    out["hbm3d_1024"] = Workload("hbm3d_1024", 6, 3, 1024, T=4.5115, seed=seed_of(6), sweeps=100,
+                                 note="3D Ising spin-1/2 1024^3 (1 GiB of spins): the HBM-streaming case")
+    out["hbm2d_32768"] = Workload("hbm2d_32768", 6, 2, 32768, T=2.269, seed=seed_of(6, 1), sweeps=100,
+                                  note="2D Ising spin-1/2 32768^2 (1 GiB of spins)")
+    out["cold2d_T0.30"] = Workload("cold2d_T0.30", 7, 2, 8192, T=0.30, seed=seed_of(7), sweeps=100,
+                                   note="2D Ising spin-1/2 8192^2 at T = 0.30: thresholds with never-accepted entries")
+    return out
+
+
+def by_name(name: str) -> Workload:
+    both = {**configs(), **extras()}
+    return both[name]
