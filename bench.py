@@ -55,6 +55,7 @@ def parse():
     ap.add_argument("--workload", default="cfg2_T2.269")
     ap.add_argument("--sweeps-per-step", type=int, default=SWEEPS_PER_STEP)
     ap.add_argument("--no-extras", action="store_true", help="skip the secondary workloads / cpu baseline")
+    ap.add_argument("--batch-scan", action="store_true", help="instead of the benchmark: lsm_batch_sweep_record over R and cluster size")
     ap.add_argument("--size-scan", action="store_true",
                     help="instead of the benchmark: us/sweep of the tiled and the small (cluster) family over lattice sizes")
     ap.add_argument("--pipe-probe", action="store_true",
@@ -490,6 +491,35 @@ def size_scan():
                           "aggregate_gflips": nlat * L * L * n / ms / 1e6, "us_per_sweep_per_lattice": ms * 1e3 / n}), flush=True)
         for lat in lats:
             lat.close()
+    batch_scan()
+    return 0
+
+
+def batch_scan(L=128, n=500):
+    """The same many-small-lattices load through lsm_batch_sweep_record: ONE launch for R lattices x n sweeps
+    (SURVEY.md 8(f) NEXT-3), for several R and blocks per replica (0 = the library's choice)."""
+    import torch
+
+    from paper_1209_0296_b200 import build, lsm
+
+    build.build()
+    for R in (1, 8, 32, 64, 128, 256, 512):
+        for c in (0, 1, 2, 4, 8, 16):
+            b = lsm.Batch(dims=2, L=L, T=[2.1 + 0.3 * r / R for r in range(R)], seeds=[100 + r for r in range(R)])
+            b.set_tracking(False)
+            b.set_cluster(c)
+            obs = torch.empty((R, n, 2), dtype=torch.int64, device="cuda")
+            b.sweep_record(n, out=obs)
+            torch.cuda.synchronize()
+            e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+            e0.record()
+            b.sweep_record(n, out=obs)
+            e1.record()
+            torch.cuda.synchronize()
+            ms = e0.elapsed_time(e1)
+            print(json.dumps({"batch_lattices": R, "L": L, "blocks_per_replica": c, "sweeps_each": n,
+                              "aggregate_gflips": R * L * L * n / ms / 1e6, "us_per_sweep_of_the_batch": ms * 1e3 / n}), flush=True)
+            b.close()
     return 0
 
 
@@ -557,6 +587,8 @@ def main():
     args = parse()
     if args.pipe_probe:
         return pipe_probe()
+    if args.batch_scan:
+        return batch_scan()
     if args.size_scan:
         # more hardware queues than the default 8, so that more than 8 handles can sweep side by side
         os.environ.setdefault("CUDA_DEVICE_MAX_CONNECTIONS", "32")

@@ -63,7 +63,8 @@
 extern "C" {
 #endif
 
-typedef struct lsm lsm_t; /* opaque, host heap */
+typedef struct lsm lsm_t;             /* opaque, host heap */
+typedef struct lsm_batch lsm_batch_t; /* opaque, host heap: R lattices of one shape swept together */
 
 enum { LSM_ISING = 0, LSM_NE_HEATBATH = 1, LSM_NE_METROPOLIS = 2 };
 enum {
@@ -72,7 +73,7 @@ enum {
     LSM_ERR_UNSUPPORTED = -2, /* two_S not 1|2; NE with dims != 2, J != 0 or two_S != 1        */
     LSM_ERR_CUDA = -3,        /* a CUDA runtime call failed (text: lsm_last_cuda_error)         */
     LSM_ERR_WORKSPACE = -4,   /* workspace too small or not 256-byte aligned                   */
-    LSM_ERR_STATE = -5        /* call needs tracking to be on (lsm_persistence)                */
+    LSM_ERR_STATE = -5        /* tracking is off (lsm_persistence); replicas out of lockstep (batch) */
 };
 /* Kernel families (lsm_set_kernel).  AUTO picks the fastest one that supports the lattice:
  *  SMALL    one launch for all sweeps of a call: lattice slabs in the shared memory of a thread-block cluster,
@@ -125,6 +126,37 @@ int lsm_sweep_random_tile(lsm_t *, int64_t n, int tile_edge, int lambda, int64_t
  * 8 + launch), words 0, 1 = red pick, 2, 3 = white pick; position r = floor(w P/2 / 2^32) = r-th site of the colour
  * in row-major order.  UNSUPPORTED unless additionally 8 * lambda divides P. */
 int lsm_sweep_random_tile_balanced(lsm_t *, int64_t n, int tile_edge, int lambda, int64_t *d_obs, void *stream);
+
+/* ---- Batches: many small lattices in one launch.
+ * The paper's own lattices are 32^2 ... 512^2 and it runs them one at a time -- 31 temperatures of the Fig. 6 ramp
+ * (PAPER.md:196), 30 realisations per concentration for Fig. 7 -- reporting that such lattices cannot keep
+ * a GPU busy ("not enough threads to execute between memory access operations").  A batch holds R independent
+ * lattices of one shape (dims, L, two_S, model, J, h) with per-replica temperature T[r] and seed seeds[r] (host arrays of
+ * R).  lsm_batch_sweep[_record] advances all of them by n checkerboard sweeps with ONE kernel launch per 256 replicas
+ * (one thread-block cluster per replica, the lattice in shared memory for the whole call) whenever L is a power of two
+ * >= 8 with at most 2^20 sites and no table has a "never" entry; otherwise the replicas are swept one after the other
+ * on the same stream.  Either way replica r ends exactly as a single handle created with (T[r], seeds[r]) would: same
+ * Philox key, same table, bit-identical.
+ *  - workspace: device, >= lsm_batch_workspace_bytes, 256-byte aligned, owned by the caller, must outlive the batch.
+ *  - d_obs: device int64 [R][n][2] = (B, M) of replica r after sweep k (overwritten).
+ *  - lsm_batch_replica lends the handle of replica r (valid until lsm_batch_destroy; do NOT lsm_destroy it) for
+ *    lsm_get_spins, lsm_set_spins, lsm_persistence, lsm_measure*, lsm_get_thresholds, ...  The batch sweeps in lockstep:
+ *    LSM_ERR_STATE if the replicas' sweep counters differ (one of them was swept on its own).
+ *  - lsm_batch_measure_int: running (B, M) of every replica into host arrays of R (either may be NULL); synchronises once.
+ *  - lsm_batch_set_cluster: thread blocks per replica (power of two <= 16, 0 = automatic: fill the SMs about twice). */
+int lsm_batch_workspace_bytes(int R, int dims, int L, int two_S, int model, size_t *bytes);
+int lsm_batch_create(int R, int dims, int L, int two_S, int model, double J, double h, const double *T,
+                     const uint64_t *seeds, void *d_workspace, size_t workspace_bytes, void *stream, lsm_batch_t **out);
+int lsm_batch_destroy(lsm_batch_t *);
+int lsm_batch_size(lsm_batch_t *, int *R);
+int lsm_batch_replica(lsm_batch_t *, int r, lsm_t **borrowed_handle);
+int lsm_batch_sweep(lsm_batch_t *, int64_t n, void *stream);
+int lsm_batch_sweep_record(lsm_batch_t *, int64_t n, int64_t *d_obs, void *stream);
+int lsm_batch_set_temperatures(lsm_batch_t *, const double *T);
+int lsm_batch_set_tracking(lsm_batch_t *, int on, void *stream);
+int lsm_batch_set_cluster(lsm_batch_t *, int blocks_per_replica);
+int lsm_batch_measure_int(lsm_batch_t *, int64_t *bond_sum, int64_t *M);
+int lsm_batch_get_launch_count(lsm_batch_t *, uint64_t *kernels_launched);
 
 /* Running observables of the current configuration (synchronises). */
 int lsm_measure(lsm_t *, double *E, int64_t *M);

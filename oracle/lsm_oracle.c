@@ -29,6 +29,12 @@
  *                          product measure, closed-form first-sweep persistence,
  *                          frozen-set bound, serial limit Q = lambda = 1
  *                          (tests/test_oracle_random_tile.py)
+ *   EA +/-J bonds ........ (model ORC_EA, reading D25) Mattis gauge: bonds tau_i tau_j reproduce the
+ *                          ferromagnet bit for bit; all-ferro bonds = the Ising rule; dict restatement incl. the
+ *                          bond stream; 4x4 brute force over 2^16 states with a fixed random bond set
+ *   Potts ................ (model ORC_POTTS, reading D26) dict restatement; q = 2 table = Ising at J/2;
+ *                          4x4 brute force over 3^16 states (q = 3) and 2^16 (q = 2); J = 0 and T -> 0 closed forms
+ *                          (tests/test_oracle_wider_models.py)
  *   "parity unpinned": none of the functions; the unpinned items are
  *   particular non-equilibrium VALUES, not code paths.
  *
@@ -47,13 +53,18 @@
  *     occupation n in {0,1}, H = sum n_i, c = 1/(1+exp(1/T)) (reading D6).
  *   - random words: Philox4x32-10 keyed on (seed; site group, sweep, half)
  *     (reading D2).
+ *   - Edwards-Anderson +/-J model (Eq. 1 with discrete J_ij; reading D25): spin-1/2,
+ *     H = -J sum_<ij> tau_ij s_i s_j - h sum s_i, tau_ij = +/-1 per bond, drawn from the seed (stream tag 3) or
+ *     set by the caller; same Metropolis rule and table as the Ising model with nn = sum_j tau_ij s_j.
+ *   - q-state Potts model (reading D26): sigma in {0..q-1}, q = two_S + 1, H = -J sum_<ij>
+ *     delta(sigma_i, sigma_j); trial state uniform over the other q-1 (word 0 of the site), Metropolis with word 1.
  */
 #include <math.h>
 #include <stdint.h>
 #include <stdlib.h>
 #include <string.h>
 
-enum { ORC_ISING = 0, ORC_NE_HEATBATH = 1, ORC_NE_METROPOLIS = 2 };
+enum { ORC_ISING = 0, ORC_NE_HEATBATH = 1, ORC_NE_METROPOLIS = 2, ORC_EA = 3, ORC_POTTS = 4 };
 
 typedef struct orc {
     int dims, L, two_S, model;
@@ -67,6 +78,9 @@ typedef struct orc {
     uint64_t thr[128];
     int nthr;
     double c;         /* NE up-concentration recomputed from T             */
+    int8_t *tau;      /* ORC_EA: bond signs, tau[a*N + i] = sign of the bond
+                         between site i and its neighbour in direction +a   */
+    int q;            /* ORC_POTTS: number of states (= two_S + 1)          */
 } orc_t;
 
 /* ---------------------------------------------------------------- Philox -- */
@@ -135,6 +149,8 @@ static int spin1_proposal(int a, int kk) { return (a + 1 + kk) % 3; }
 /* Table layouts (the order lsm_get_thresholds must reproduce):
  *  Ising two_S=1: idx = b*(2d+1) + (nn+2d)/2, b = (s+1)/2          -> 2(2d+1)
  *  Ising two_S=2: idx = (a*2 + kk)*(4d+1) + (nn+2d), a = s+1        -> 6(4d+1)
+ *  EA: as Ising two_S=1 with nn = sum_j tau_ij s_j (reading D25)     -> 2(2d+1)
+ *  Potts: idx = (n_new - n_old) + 2d                                -> 4d+1
  *  NE (either rule): [0] = floor(c*2^32) (initial state and heat bath),
  *                    [1] = floor(exp(-1/T)*2^32) (Metropolis 0->1),
  *                    [2] = 2^32 (Metropolis 1->0, dE < 0)            -> 3    */
@@ -142,7 +158,15 @@ static void build_thresholds(orc_t *o)
 {
     int d = o->dims;
     o->nthr = 0;
-    if (o->model == ORC_ISING && o->two_S == 1) {
+    if (o->model == ORC_POTTS) {
+        /* reading D26: dE = -J * (n_new - n_old), idx = (n_new - n_old) + 2d */
+        for (int j = 0; j <= 4 * d; ++j) {
+            double x = o->J * (double)(j - 2 * d);
+            double dE = -x;
+            o->thr[o->nthr++] = (dE <= 0.0) ? ((uint64_t)1 << 32) : thr_of_probability(exp(-dE / o->T));
+        }
+    } else if ((o->model == ORC_ISING && o->two_S == 1) || o->model == ORC_EA) {
+        /* ORC_EA (reading D25): the same table, indexed by the bond-weighted neighbour sum */
         for (int b = 0; b < 2; ++b)
             for (int j = 0; j <= 2 * d; ++j) {
                 int s = 2 * b - 1, nn = 2 * j - 2 * d;
@@ -185,6 +209,30 @@ static int neighbour_sum(const orc_t *o, int x, int y, int z)
     return nn;
 }
 
+/* ORC_EA (reading D25): sum_j tau_ij s_j over the 2d neighbours.  The bond between i and i+a is stored at i,
+ * the bond between i and i-a at the neighbour i-a.                                                          */
+static int bond_sign(const orc_t *o, int a, int x, int y, int z)
+{
+    int L = o->L;
+    return o->tau[(int64_t)a * o->N + site_id(o, wrap(x, L), wrap(y, L), o->dims == 3 ? wrap(z, L) : 0)];
+}
+static int neighbour_sum_bonds(const orc_t *o, int x, int y, int z)
+{
+    int nn = bond_sign(o, 0, x, y, z) * value_at(o, x + 1, y, z) + bond_sign(o, 0, x - 1, y, z) * value_at(o, x - 1, y, z)
+           + bond_sign(o, 1, x, y, z) * value_at(o, x, y + 1, z) + bond_sign(o, 1, x, y - 1, z) * value_at(o, x, y - 1, z);
+    if (o->dims == 3)
+        nn += bond_sign(o, 2, x, y, z) * value_at(o, x, y, z + 1) + bond_sign(o, 2, x, y, z - 1) * value_at(o, x, y, z - 1);
+    return nn;
+}
+/* ORC_POTTS: number of the 2d neighbours in state v. */
+static int neighbours_equal_to(const orc_t *o, int x, int y, int z, int v)
+{
+    int n = (value_at(o, x - 1, y, z) == v) + (value_at(o, x + 1, y, z) == v)
+          + (value_at(o, x, y - 1, z) == v) + (value_at(o, x, y + 1, z) == v);
+    if (o->dims == 3) n += (value_at(o, x, y, z - 1) == v) + (value_at(o, x, y, z + 1) == v);
+    return n;
+}
+
 /* ------------------------------------------------------------ initial state */
 /* Reading D4: stream 2, t = 0, group = i>>2 over the canonical id, word i&3. */
 static void init_from_seed(orc_t *o)
@@ -194,11 +242,32 @@ static void init_from_seed(orc_t *o)
         words_of_group(o->seed, (uint64_t)i >> 2, 0, 2u, w4);
         uint32_t w = w4[i & 3];
         int v;
-        if (o->model != ORC_ISING) v = ((uint64_t)w < o->thr[0]) ? 1 : 0;
+        if (o->model == ORC_POTTS)   v = (int)(((uint64_t)w * (uint64_t)o->q) >> 32);      /* reading D26 */
+        else if (o->model == ORC_EA) v = (w >> 31) ? 1 : -1;
+        else if (o->model != ORC_ISING) v = ((uint64_t)w < o->thr[0]) ? 1 : 0;
         else if (o->two_S == 1)    v = (w >> 31) ? 1 : -1;
         else                       v = (int)(((uint64_t)w * 3u) >> 32) - 1;
         o->s[i] = (int8_t)v;
     }
+}
+
+/* Reading D25: bond signs from stream tag 3, t = 0: bond id b = a*N + i (a = 0, 1, 2 for +x, +y, +z),
+ * group b>>2, word b&3; tau = +1 if the top bit of the word is set, else -1 (the +/-J model with p = 1/2).  */
+static void bonds_from_seed(orc_t *o)
+{
+    for (int64_t b = 0; b < (int64_t)o->dims * o->N; ++b) {
+        uint32_t w4[4];
+        words_of_group(o->seed, (uint64_t)b >> 2, 0, 3u, w4);
+        o->tau[b] = (w4[b & 3] >> 31) ? 1 : -1;
+    }
+}
+
+void orc_get_bonds(const orc_t *o, int8_t *out) { if (o->tau) memcpy(out, o->tau, (size_t)o->dims * (size_t)o->N); }
+int orc_set_bonds(orc_t *o, const int8_t *in)
+{
+    if (!o->tau) return -1;
+    memcpy(o->tau, in, (size_t)o->dims * (size_t)o->N);
+    return 0;
 }
 
 void orc_reset_reference(orc_t *o)
@@ -217,7 +286,9 @@ orc_t *orc_create(int dims, int L, int two_S, int model, double J, double h, dou
     if (model == ORC_ISING) { if (two_S != 1 && two_S != 2) return NULL; }
     else if (model == ORC_NE_HEATBATH || model == ORC_NE_METROPOLIS) {
         if (dims != 2 || J != 0.0 || two_S != 1) return NULL;
-    } else return NULL;
+    } else if (model == ORC_EA) { if (two_S != 1) return NULL; }
+    else if (model == ORC_POTTS) { if (two_S < 1 || two_S > 15 || h != 0.0) return NULL; }   /* q = two_S + 1 in [2, 16] */
+    else return NULL;
     orc_t *o = (orc_t *)calloc(1, sizeof(orc_t));
     if (!o) return NULL;
     o->dims = dims; o->L = L; o->two_S = two_S; o->model = model;
@@ -227,6 +298,13 @@ orc_t *orc_create(int dims, int L, int two_S, int model, double J, double h, dou
     o->s0 = (int8_t *)malloc((size_t)o->N);
     o->changed = (uint8_t *)malloc((size_t)o->N);
     if (!o->s || !o->s0 || !o->changed) { free(o->s); free(o->s0); free(o->changed); free(o); return NULL; }
+    o->q = two_S + 1;
+    o->tau = NULL;
+    if (model == ORC_EA) {
+        o->tau = (int8_t *)malloc((size_t)dims * (size_t)o->N);
+        if (!o->tau) { free(o->s); free(o->s0); free(o->changed); free(o); return NULL; }
+        bonds_from_seed(o);
+    }
     o->t = 0;
     build_thresholds(o);
     init_from_seed(o);
@@ -237,7 +315,7 @@ orc_t *orc_create(int dims, int L, int two_S, int model, double J, double h, dou
 void orc_destroy(orc_t *o)
 {
     if (!o) return;
-    free(o->s); free(o->s0); free(o->changed); free(o);
+    free(o->s); free(o->s0); free(o->changed); free(o->tau); free(o);
 }
 
 int orc_set_temperature(orc_t *o, double T)
@@ -284,6 +362,22 @@ static void update_site(orc_t *o, int x, int y, int z, uint32_t half)
         int b = (s_old + 1) / 2, j = (nn + 2 * o->dims) / 2;
         uint64_t thr = o->thr[b * (2 * o->dims + 1) + j];
         if ((uint64_t)w < thr) s_new = -s_old;               /* PAPER.md:88 */
+    } else if (o->model == ORC_EA) {
+        /* reading D25: as Ising spin-1/2 with the bond-weighted neighbour sum; one word per site */
+        words_of_group(o->seed, (uint64_t)k >> 2, o->t, half, w4);
+        uint32_t w = w4[k & 3];
+        int nn = neighbour_sum_bonds(o, x, y, z);
+        int b = (s_old + 1) / 2, j = (nn + 2 * o->dims) / 2;
+        if ((uint64_t)w < o->thr[b * (2 * o->dims + 1) + j]) s_new = -s_old;
+    } else if (o->model == ORC_POTTS) {
+        /* reading D26: two words per site (group k>>1); w0 proposes one of the other q-1 states uniformly,
+         * w1 accepts by Metropolis with dE = -J (n_new - n_old) */
+        words_of_group(o->seed, (uint64_t)k >> 1, o->t, half, w4);
+        uint32_t w0 = w4[2 * (k & 1)], w1 = w4[2 * (k & 1) + 1];
+        int r = (int)(((uint64_t)w0 * (uint64_t)(o->q - 1)) >> 32);
+        int prop = (s_old + 1 + r) % o->q;
+        int dn = neighbours_equal_to(o, x, y, z, prop) - neighbours_equal_to(o, x, y, z, s_old);
+        if ((uint64_t)w1 < o->thr[dn + 2 * o->dims]) s_new = prop;
     } else if (o->model == ORC_ISING) {
         /* two words per site: group k>>1, words 2(k&1) and 2(k&1)+1 */
         words_of_group(o->seed, (uint64_t)k >> 1, o->t, half, w4);
@@ -540,7 +634,18 @@ void orc_measure(const orc_t *o, int64_t *B, int64_t *M)
         for (int y = 0; y < L; ++y)
             for (int x = 0; x < L; ++x) {
                 int s = value_at(o, x, y, z);
+                if (o->model == ORC_POTTS) {            /* D26: M = sites in state 0, B = bonds joining equal states */
+                    m += (s == 0);
+                    b += (value_at(o, x + 1, y, z) == s) + (value_at(o, x, y + 1, z) == s);
+                    if (o->dims == 3) b += (value_at(o, x, y, z + 1) == s);
+                    continue;
+                }
                 m += s;
+                if (o->model == ORC_EA) {               /* D25: B = sum over bonds of tau_ij s_i s_j */
+                    int f = bond_sign(o, 0, x, y, z) * value_at(o, x + 1, y, z) + bond_sign(o, 1, x, y, z) * value_at(o, x, y + 1, z);
+                    if (o->dims == 3) f += bond_sign(o, 2, x, y, z) * value_at(o, x, y, z + 1);
+                    b += (int64_t)s * f;
+                }
                 if (o->model == ORC_ISING) {
                     int f = value_at(o, x + 1, y, z) + value_at(o, x, y + 1, z);
                     if (o->dims == 3) f += value_at(o, x, y, z + 1);
@@ -555,7 +660,8 @@ double orc_energy(const orc_t *o)
 {
     int64_t B, M;
     orc_measure(o, &B, &M);
-    if (o->model == ORC_ISING) return -o->J * (double)B - o->h * (double)M;
+    if (o->model == ORC_ISING || o->model == ORC_EA) return -o->J * (double)B - o->h * (double)M;
+    if (o->model == ORC_POTTS) return -o->J * (double)B;
     return (double)M;
 }
 
@@ -577,7 +683,8 @@ void orc_persistence(const orc_t *o, int64_t *never_changed, int64_t *overlap)
     for (int64_t i = 0; i < o->N; ++i) {
         if (!o->changed[i]) ++nc;
         int a = o->s0[i], b = o->s[i];
-        if (o->model != ORC_ISING) { a = 2 * a - 1; b = 2 * b - 1; }
+        if (o->model == ORC_POTTS) { ov += (a == b); continue; }      /* D26: overlap = sites in their reference state */
+        if (o->model == ORC_NE_HEATBATH || o->model == ORC_NE_METROPOLIS) { a = 2 * a - 1; b = 2 * b - 1; }
         ov += (int64_t)a * b;
     }
     *never_changed = nc; *overlap = ov;

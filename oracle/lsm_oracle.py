@@ -28,7 +28,7 @@ if os.environ.get("LSM_ORACLE_SRC"):
     _SRC = os.path.abspath(os.environ["LSM_ORACLE_SRC"])
     _LIB = _SRC + ".so"
 
-ISING, NE_HEATBATH, NE_METROPOLIS = 0, 1, 2
+ISING, NE_HEATBATH, NE_METROPOLIS, EA, POTTS = 0, 1, 2, 3, 4
 
 
 def build(force: bool = False) -> str:
@@ -75,6 +75,9 @@ def lib():
         L.orc_concentration.restype = dbl
         L.orc_concentration.argtypes = [vp]
         L.orc_philox4x32_10.argtypes = [vp, vp, vp]
+        L.orc_get_bonds.argtypes = [vp, vp]
+        L.orc_set_bonds.restype = i32
+        L.orc_set_bonds.argtypes = [vp, vp]
         L.orc_sweep_random_tile.restype = i32
         L.orc_sweep_random_tile.argtypes = [vp, i64, i32, i32, i32]
         L.orc_sweep_random_tile_balanced.restype = i32
@@ -173,6 +176,18 @@ class Oracle:
         assert a.size == self.N
         lib().orc_set_spins(self._h, a.ctypes.data, int(sweep_counter))
 
+    def get_bonds(self):
+        """EA model (reading D25): bond signs [dims, N]; [a, i] joins site i and its neighbour in direction +a."""
+        out = np.empty((self.dims, self.N), dtype=np.int8)
+        lib().orc_get_bonds(self._h, out.ctypes.data)
+        return out
+
+    def set_bonds(self, tau):
+        a = np.ascontiguousarray(tau, dtype=np.int8).reshape(-1)
+        assert a.size == self.dims * self.N
+        if lib().orc_set_bonds(self._h, a.ctypes.data) != 0:
+            raise ValueError("bonds belong to the EA model")
+
     def set_temperature(self, T):
         if lib().orc_set_temperature(self._h, float(T)) != 0:
             raise ValueError("bad temperature")
@@ -198,8 +213,10 @@ class Oracle:
 def energy_from_int(B, M, J, h, model=ISING):
     """E = -J*B - h*M (Ising, PAPER.md:86 with the field term of reading D1);
     E = M for the North-East model (H = sum n_i, reading D15)."""
-    if model == ISING:
+    if model in (ISING, EA):
         return -float(J) * float(B) - float(h) * float(M)
+    if model == POTTS:
+        return -float(J) * float(B)
     return float(M)
 
 

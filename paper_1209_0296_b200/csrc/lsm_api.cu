@@ -10,6 +10,7 @@
 #include <cstring>
 #include <new>
 #include <string>
+#include <vector>
 
 using namespace lsmk;
 
@@ -326,6 +327,231 @@ extern "C" int lsm_sweep_record_host(lsm_t *o, int64_t n, int64_t *h_obs, int64_
     return LSM_OK;
 }
 
+// ---------------------------------------------------------------------------- batch of lattices (NEXT-3)
+// R independent lattices of one shape, each with its own temperature and seed (the 31 temperatures of the paper's
+// Fig. 6 ramp, or the 30 realisations of Fig. 7), swept by ONE kernel launch: the paper's
+// small lattices cannot fill a GPU one at a time.  Every replica is a complete lsm handle on its own
+// slice of the workspace (lsm_batch_replica lends it out for lsm_get_spins, lsm_persistence, ...); the batch sweep is
+// the small family's lane kernel with one thread-block cluster per replica (lsm_small.cu).  Bit-identical to
+// sweeping each replica on its own.
+struct lsm_batch {
+    int R;
+    std::vector<lsm *> rep;
+    std::vector<uint64_t> seeds;
+    size_t rep_bytes;
+    BatchDesc *d_desc;
+    std::vector<BatchDesc> h_desc;   // what the device array holds
+    int cluster_pref;                // 0 = auto
+    uint64_t launches;               // batch launches (the replicas count their own)
+};
+
+static size_t batch_desc_bytes(int R) { return align256((size_t)R * sizeof(BatchDesc)); }
+
+extern "C" int lsm_batch_workspace_bytes(int R, int dims, int L, int two_S, int model, size_t *bytes)
+{
+    if (!bytes || R < 1 || R > 65536) return LSM_ERR_ARG;
+    size_t one = 0;
+    int rc = lsm_workspace_bytes(dims, L, two_S, model, &one);
+    if (rc != LSM_OK) return rc;
+    *bytes = batch_desc_bytes(R) + (size_t)R * align256(one);
+    return LSM_OK;
+}
+
+extern "C" int lsm_batch_destroy(lsm_batch_t *b)
+{
+    if (!b) return LSM_ERR_ARG;
+    for (lsm *o : b->rep) delete o;
+    delete b;
+    return LSM_OK;
+}
+
+extern "C" int lsm_batch_create(int R, int dims, int L, int two_S, int model, double J, double h, const double *T,
+                                const uint64_t *seeds, void *d_workspace, size_t workspace_bytes, void *stream,
+                                lsm_batch_t **out)
+{
+    if (!out || !T || !seeds || !d_workspace) return LSM_ERR_ARG;
+    size_t need = 0, one = 0;
+    int rc = lsm_batch_workspace_bytes(R, dims, L, two_S, model, &need);
+    if (rc != LSM_OK) return rc;
+    if (workspace_bytes < need || ((uintptr_t)d_workspace & 255)) return LSM_ERR_WORKSPACE;
+    lsm_workspace_bytes(dims, L, two_S, model, &one);
+    lsm_batch *b = new (std::nothrow) lsm_batch();
+    if (!b) return LSM_ERR_ARG;
+    b->R = R;
+    b->rep_bytes = align256(one);
+    b->d_desc = (BatchDesc *)d_workspace;
+    b->cluster_pref = 0;
+    b->launches = 0;
+    uint8_t *base = (uint8_t *)d_workspace + batch_desc_bytes(R);
+    for (int r = 0; r < R; ++r) {
+        lsm *o = nullptr;
+        rc = lsm_create(dims, L, two_S, model, J, h, T[r], seeds[r], base + (size_t)r * b->rep_bytes, b->rep_bytes, stream, &o);
+        if (rc != LSM_OK) { lsm_batch_destroy(b); return rc; }
+        b->rep.push_back(o);
+        b->seeds.push_back(seeds[r]);
+    }
+    *out = b;
+    return LSM_OK;
+}
+
+extern "C" int lsm_batch_size(lsm_batch_t *b, int *R)
+{
+    if (!b || !R) return LSM_ERR_ARG;
+    *R = b->R;
+    return LSM_OK;
+}
+
+extern "C" int lsm_batch_replica(lsm_batch_t *b, int r, lsm_t **handle)
+{
+    if (!b || !handle || r < 0 || r >= b->R) return LSM_ERR_ARG;
+    *handle = b->rep[r];
+    return LSM_OK;
+}
+
+extern "C" int lsm_batch_set_temperatures(lsm_batch_t *b, const double *T)
+{
+    if (!b || !T) return LSM_ERR_ARG;
+    for (int r = 0; r < b->R; ++r)
+        if (!(T[r] > 0.0) || !std::isfinite(T[r])) return LSM_ERR_ARG;
+    for (int r = 0; r < b->R; ++r) lsm_set_temperature(b->rep[r], T[r]);
+    return LSM_OK;
+}
+
+extern "C" int lsm_batch_set_tracking(lsm_batch_t *b, int on, void *stream)
+{
+    if (!b) return LSM_ERR_ARG;
+    for (lsm *o : b->rep) {
+        int rc = lsm_set_tracking(o, on, stream);
+        if (rc != LSM_OK) return rc;
+    }
+    return LSM_OK;
+}
+
+extern "C" int lsm_batch_set_cluster(lsm_batch_t *b, int blocks_per_replica)
+{
+    if (!b || blocks_per_replica < 0 || blocks_per_replica > 16 || (blocks_per_replica & (blocks_per_replica - 1))) return LSM_ERR_ARG;
+    if (blocks_per_replica > 0) {
+        const Lat &lat = b->rep[0]->lat;
+        const long long lanes = lat.half / 4, N = 2 * lat.half;
+        if (blocks_per_replica > lat.L || lanes / blocks_per_replica < 32 || N / blocks_per_replica > 196608) return LSM_ERR_UNSUPPORTED;
+    }
+    b->cluster_pref = blocks_per_replica;
+    return LSM_OK;
+}
+
+// The one-launch path needs the lane kernel of the small family for every replica's table and one tracking state.
+static bool batch_one_launch(const lsm_batch *b)
+{
+    for (const lsm *o : b->rep) {
+        if (o->tracking != b->rep[0]->tracking) return false;
+        if (!small_batch_supported(o->lat, o->model, o->tiled)) return false;
+    }
+    return true;
+}
+
+// Device descriptors follow the replicas' current colour arrays (the random-tile schedule swaps them) and tables.
+static int batch_refresh_desc(lsm_batch *b, cudaStream_t s)
+{
+    std::vector<BatchDesc> now((size_t)b->R);
+    for (int r = 0; r < b->R; ++r) {
+        const lsm *o = b->rep[r];
+        BatchDesc &d = now[r];
+        std::memset(&d, 0, sizeof(d));
+        d.col[0] = o->lat.col[0];
+        d.col[1] = o->lat.col[1];
+        d.run = o->d_run;
+        if (o->model == M_ISING_HALF) for (int i = 0; i < 16; ++i) d.tab[i] = o->tiled.t32[i];
+        else if (o->model == M_ISING_ONE) for (int i = 0; i < 64; ++i) d.tab[i] = o->tiled.s1[i];
+        else {
+            d.ne_t32 = o->tiled.ne_t32[o->model == M_NE_HEATBATH ? 0 : 1];
+            d.ne_always = o->model == M_NE_HEATBATH ? 0 : o->tiled.ne_up_always;
+        }
+    }
+    if (b->h_desc.size() == now.size() && std::memcmp(b->h_desc.data(), now.data(), now.size() * sizeof(BatchDesc)) == 0)
+        return LSM_OK;
+    // pageable source: the runtime stages it before returning, so `now` may go out of scope
+    CU(cudaMemcpyAsync(b->d_desc, now.data(), now.size() * sizeof(BatchDesc), cudaMemcpyHostToDevice, s));
+    b->h_desc.swap(now);
+    return LSM_OK;
+}
+
+static int batch_sweep_impl(lsm_batch *b, int64_t n, long long *d_obs, cudaStream_t s)
+{
+    if (n == 0) return LSM_OK;
+    if (!batch_one_launch(b)) {                       // any lattice, any table: one replica after the other
+        for (int r = 0; r < b->R; ++r) {
+            int rc = sweep_impl(b->rep[r], n, d_obs ? d_obs + 2 * n * r : nullptr, s);
+            if (rc != LSM_OK) return rc;
+        }
+        return LSM_OK;
+    }
+    int rc = batch_refresh_desc(b, s);
+    if (rc != LSM_OK) return rc;
+    lsm *o0 = b->rep[0];
+    const int cluster = b->cluster_pref ? b->cluster_pref : small_batch_cluster(o0->lat, b->R);
+    const uint64_t t0 = o0->t;
+    for (lsm *o : b->rep) {
+        if (o->t != t0) return LSM_ERR_STATE;         // a replica was swept on its own: the batch sweeps in lockstep
+        o->last_stream = s;
+    }
+    const int64_t CHUNK = 1 << 20;
+    int64_t done = 0;
+    if (!d_obs && n > 1) {                            // only the last sweep is measured
+        for (; done < n - 1;) {
+            const int k = (int)(n - 1 - done < CHUNK ? n - 1 - done : CHUNK);
+            CU(launch_sweep_small_batch(o0->lat, o0->model, o0->tracking, b->d_desc, b->seeds.data(), b->R, cluster,
+                                        t0 + (uint64_t)done, k, nullptr, 0, 0, s));
+            b->launches += (uint64_t)((b->R + 255) / 256);
+            done += k;
+        }
+    }
+    for (; done < n;) {
+        const int k = (int)(n - done < CHUNK ? n - done : CHUNK);
+        const bool last = done + k == n;
+        CU(launch_sweep_small_batch(o0->lat, o0->model, o0->tracking, b->d_desc, b->seeds.data(), b->R, cluster,
+                                    t0 + (uint64_t)done, k, d_obs ? d_obs + 2 * done : nullptr, 2 * n, last ? 1 : 0, s));
+        b->launches += (uint64_t)((b->R + 255) / 256);
+        done += k;
+    }
+    for (lsm *o : b->rep) o->t = t0 + (uint64_t)n;
+    return LSM_OK;
+}
+
+extern "C" int lsm_batch_sweep(lsm_batch_t *b, int64_t n, void *stream)
+{
+    if (!b || n < 0) return LSM_ERR_ARG;
+    return batch_sweep_impl(b, n, nullptr, (cudaStream_t)stream);
+}
+
+extern "C" int lsm_batch_sweep_record(lsm_batch_t *b, int64_t n, int64_t *d_obs, void *stream)
+{
+    if (!b || n < 0 || (!d_obs && n > 0)) return LSM_ERR_ARG;
+    return batch_sweep_impl(b, n, (long long *)d_obs, (cudaStream_t)stream);
+}
+
+extern "C" int lsm_batch_measure_int(lsm_batch_t *b, int64_t *B, int64_t *M)
+{
+    if (!b) return LSM_ERR_ARG;
+    std::vector<long long> v(2 * (size_t)b->R);
+    cudaStream_t s = b->rep[0]->last_stream;
+    for (int r = 0; r < b->R; ++r) CU(cudaMemcpyAsync(&v[2 * r], b->rep[r]->d_run, 16, cudaMemcpyDeviceToHost, s));
+    CU(cudaStreamSynchronize(s));
+    for (int r = 0; r < b->R; ++r) {
+        if (B) B[r] = v[2 * r];
+        if (M) M[r] = v[2 * r + 1];
+    }
+    return LSM_OK;
+}
+
+extern "C" int lsm_batch_get_launch_count(lsm_batch_t *b, uint64_t *n)
+{
+    if (!b || !n) return LSM_ERR_ARG;
+    uint64_t tot = b->launches;
+    for (lsm *o : b->rep) tot += o->launches;
+    *n = tot;
+    return LSM_OK;
+}
+
 // ---------------------------------------------------------------------------- observables
 static int read_pair(lsm *o, const long long *d, long long out[2])
 {
@@ -567,7 +793,7 @@ extern "C" const char *lsm_strerror(int code)
     case LSM_ERR_UNSUPPORTED: return "unsupported model / lattice / kernel combination";
     case LSM_ERR_CUDA: return "CUDA runtime error (see lsm_last_cuda_error)";
     case LSM_ERR_WORKSPACE: return "workspace too small or misaligned";
-    case LSM_ERR_STATE: return "tracking is off";
+    case LSM_ERR_STATE: return "tracking is off, or the replicas of a batch are out of lockstep";
     default: return "unknown error code";
     }
 }

@@ -104,49 +104,43 @@ k_sweep_small(const __grid_constant__ SmallArgs a, const __grid_constant__ Philo
 // hardware-supported, far cheaper than ending the kernel.  This is the regime of the
 // paper's own lattices (32^2 ... 512^2), which a launch per half-sweep cannot serve well.
 // Same rules, same (group, word) -> site map as every other family: bit-identical.
+//
+// The body serves two kernels: k_sweep_small_lane (one lattice = one cluster = the whole grid) and
+// k_sweep_small_lane_batch (R independent lattices = R clusters of one grid, each with its own Philox key and
+// threshold table: lsm_batch_sweep).  `sm_t` is the block's threshold table in shared memory (filled by the
+// caller), `acc` its (B, M) scratch.  self_zero: the cluster zeroes its own obs / run slots (batch launches have no
+// host memset per replica); run: where the sums of the LAST sweep are added as well (the replica's running pair).
 template <int MODEL, int DIMS, bool TRACK, int OBS>
-__global__ void __launch_bounds__(1024, 1)
-k_sweep_small_lane(const __grid_constant__ SmallArgs a, const __grid_constant__ PhiloxSweepConsts pk,
-                   const __grid_constant__ typename TabOf<MODEL>::type tab, const int lg_lpr, const int lg_L,
-                   const int lg_rpc)
+__device__ __forceinline__ void small_lane_body(uint8_t *const col0, uint8_t *const col1, const PhiloxSweepConsts &pk,
+                                                const unsigned long long seed, const unsigned long long t0,
+                                                const int nsweeps, long long *const obs, long long *const run,
+                                                const bool self_zero, uint32_t ne_t32, int ne_always, const uint32_t one,
+                                                const uint32_t s_t, int (*acc)[2], const int lg_lpr, const int lg_L,
+                                                const int lg_rpc)
 {
     namespace cg = cooperative_groups;
     cg::cluster_group cluster = cg::this_cluster();
     const uint32_t rank = cluster.block_rank(), nrank = cluster.num_blocks();
 
-    __shared__ __align__(16) struct {
-        uint32_t t[MODEL == M_ISING_ONE ? 64 : 16];
-        int acc[2][2];           // this block's share of (B, M) of the sweep in flight, double-buffered
-    } sm;
-    uint32_t s_t = (uint32_t)__cvta_generic_to_shared(sm.t);
-    asm volatile("" : "+r"(s_t));
-    if constexpr (MODEL == M_ISING_HALF) {
-        if (threadIdx.x < 16) sm.t[threadIdx.x] = tab.t[threadIdx.x];
-    } else if constexpr (MODEL == M_ISING_ONE) {
-        for (int i = threadIdx.x; i < 64; i += blockDim.x) sm.t[i] = tab.t[i];   // blocks may have 32 threads
-    }
-    if (threadIdx.x < 4) sm.acc[threadIdx.x >> 1][threadIdx.x & 1] = 0;
-
     constexpr bool NE = MODEL == M_NE_HEATBATH || MODEL == M_NE_METROPOLIS;
-    const uint32_t lpr = 1u << lg_lpr, L = 1u << lg_L;
+    const uint32_t lpr = 1u << lg_lpr;
     const int lg_R = DIMS == 3 ? lg_L : 0;
     const uint32_t R = 1u << lg_R;
     const int lg_slab = lg_rpc + lg_R + lg_lpr;               // log2(lanes per colour in one slab)
     const uint32_t nl = 1u << lg_slab;
     const uint32_t base = rank << lg_slab;                     // first lane of this slab in the colour array
-    const uint32_t one = (uint32_t)a.g.one;
-    uint32_t ne_t32 = 0;
-    int ne_always = 0;
-    if constexpr (NE) {
-        ne_t32 = tab.t32;
-        ne_always = tab.always;
-    }
+    if (!NE) { ne_t32 = 0; ne_always = 0; }
 
     extern __shared__ __align__(16) uint32_t s_lat[];
     uint32_t *const s_col[2] = {s_lat, s_lat + nl};
     for (uint32_t i = threadIdx.x; i < nl; i += blockDim.x) {
-        s_col[0][i] = reinterpret_cast<const uint32_t *>(a.col[0])[base + i];
-        s_col[1][i] = reinterpret_cast<const uint32_t *>(a.col[1])[base + i];
+        s_col[0][i] = reinterpret_cast<const uint32_t *>(col0)[base + i];
+        s_col[1][i] = reinterpret_cast<const uint32_t *>(col1)[base + i];
+    }
+    if (self_zero && rank == 0) {                              // ordered before every add by the barrier below
+        if (OBS >= 1 && obs)
+            for (int i = threadIdx.x; i < 2 * nsweeps; i += blockDim.x) obs[i] = 0;
+        if (OBS >= 1 && run && threadIdx.x < 2) run[threadIdx.x] = 0;
     }
     // the slabs above and below (the same shared-memory offsets in the neighbour blocks)
     const uint32_t r_dn = (rank + nrank - 1) % nrank, r_up = (rank + 1) % nrank;
@@ -157,13 +151,13 @@ k_sweep_small_lane(const __grid_constant__ SmallArgs a, const __grid_constant__ 
     else __syncthreads();
 
     int thrB = 0, thrM = 0;
-    const int nhalves = 2 * a.nsweeps;
+    const int nhalves = 2 * nsweeps;
 #pragma unroll 1
     for (int gh = 0; gh < nhalves; ++gh) {
         const int half = gh & 1, sw = gh >> 1;
-        const unsigned long long t = a.t0 + (unsigned long long)sw;
+        const unsigned long long t = t0 + (unsigned long long)sw;
         PhiloxDyn pc = {0u, 0u, 0u, 0u, pk};
-        philox_half_consts(make_sweep_key(a.seed, t, (uint32_t)half), pk.rk0, pk.rk1, pc.x1, pc.y2, pc.z2, pc.w3);
+        philox_half_consts(make_sweep_key(seed, t, (uint32_t)half), pk.rk0, pk.rk1, pc.x1, pc.y2, pc.z2, pc.w3);
         uint32_t *own = s_col[half];
         const uint32_t *oth = s_col[half ^ 1];
         int totU = 0, totBN = 0, totS = 0, nsites = 0;
@@ -222,8 +216,8 @@ k_sweep_small_lane(const __grid_constant__ SmallArgs a, const __grid_constant__ 
             if (half == 1) {                           // once per sweep: warp reduce -> block-local shared atomics
                 const int wB = __reduce_add_sync(0xffffffffu, thrB), wM = __reduce_add_sync(0xffffffffu, thrM);
                 if ((threadIdx.x & 31) == 0) {
-                    if (wB != 0) atomicAdd(&sm.acc[sw & 1][0], wB);
-                    if (wM != 0) atomicAdd(&sm.acc[sw & 1][1], wM);
+                    if (wB != 0) atomicAdd(&acc[sw & 1][0], wB);
+                    if (wM != 0) atomicAdd(&acc[sw & 1][1], wM);
                 }
             }
         }
@@ -233,18 +227,98 @@ k_sweep_small_lane(const __grid_constant__ SmallArgs a, const __grid_constant__ 
         if (OBS >= 1 && half == 1 && threadIdx.x == 0) {
             // one fire-and-forget 64-bit add per block into the sweep's (zeroed) slot; the next adds to this
             // shared buffer belong to sweep sw + 2: two barriers away
-            const int vB = sm.acc[sw & 1][0], vM = sm.acc[sw & 1][1];
-            if (vB != 0) atomicAdd((unsigned long long *)&a.obs[2 * sw], (unsigned long long)(long long)vB);
-            if (vM != 0) atomicAdd((unsigned long long *)&a.obs[2 * sw + 1], (unsigned long long)(long long)vM);
-            sm.acc[sw & 1][0] = 0;
-            sm.acc[sw & 1][1] = 0;
+            const int vB = acc[sw & 1][0], vM = acc[sw & 1][1];
+            if (obs) {
+                if (vB != 0) atomicAdd((unsigned long long *)&obs[2 * sw], (unsigned long long)(long long)vB);
+                if (vM != 0) atomicAdd((unsigned long long *)&obs[2 * sw + 1], (unsigned long long)(long long)vM);
+            }
+            if (run && sw == nsweeps - 1) {
+                if (vB != 0) atomicAdd((unsigned long long *)&run[0], (unsigned long long)(long long)vB);
+                if (vM != 0) atomicAdd((unsigned long long *)&run[1], (unsigned long long)(long long)vM);
+            }
+            acc[sw & 1][0] = 0;
+            acc[sw & 1][1] = 0;
         }
     }
     for (uint32_t i = threadIdx.x; i < nl; i += blockDim.x) {
-        reinterpret_cast<uint32_t *>(a.col[0])[base + i] = s_col[0][i];
-        reinterpret_cast<uint32_t *>(a.col[1])[base + i] = s_col[1][i];
+        reinterpret_cast<uint32_t *>(col0)[base + i] = s_col[0][i];
+        reinterpret_cast<uint32_t *>(col1)[base + i] = s_col[1][i];
     }
     if (nrank > 1) cluster.sync();      // no block may exit while a neighbour can still read its shared memory
+}
+
+template <int MODEL, int DIMS, bool TRACK, int OBS>
+__global__ void __launch_bounds__(1024, 1)
+k_sweep_small_lane(const __grid_constant__ SmallArgs a, const __grid_constant__ PhiloxSweepConsts pk,
+                   const __grid_constant__ typename TabOf<MODEL>::type tab, const int lg_lpr, const int lg_L,
+                   const int lg_rpc)
+{
+    __shared__ __align__(16) struct {
+        uint32_t t[MODEL == M_ISING_ONE ? 64 : 16];
+        int acc[2][2];           // this block's share of (B, M) of the sweep in flight, double-buffered
+    } sm;
+    uint32_t s_t = (uint32_t)__cvta_generic_to_shared(sm.t);
+    asm volatile("" : "+r"(s_t));
+    uint32_t ne_t32 = 0;
+    int ne_always = 0;
+    if constexpr (MODEL == M_ISING_HALF) {
+        if (threadIdx.x < 16) sm.t[threadIdx.x] = tab.t[threadIdx.x];
+    } else if constexpr (MODEL == M_ISING_ONE) {
+        for (int i = threadIdx.x; i < 64; i += blockDim.x) sm.t[i] = tab.t[i];   // blocks may have 32 threads
+    } else {
+        ne_t32 = tab.t32;
+        ne_always = tab.always;
+    }
+    if (threadIdx.x < 4) sm.acc[threadIdx.x >> 1][threadIdx.x & 1] = 0;
+    small_lane_body<MODEL, DIMS, TRACK, OBS>(a.col[0], a.col[1], pk, a.seed, a.t0, a.nsweeps, a.obs, nullptr, false, ne_t32,
+                                             ne_always, (uint32_t)a.g.one, s_t, sm.acc, lg_lpr, lg_L, lg_rpc);
+}
+
+// R lattices in one launch: cluster c of the grid sweeps replica r0 + c.  Per replica: colour arrays, running pair,
+// Philox key (seed) and the threshold table in the form the vectorised rules index -- all from the descriptor array
+// in device memory (the seeds also ride in the kernel parameters so that the round keys stay warp-uniform operands).
+constexpr int SMALL_BATCH_MAX = 256;              // replicas per launch (seed array in the kernel parameters)
+struct SmallBatchArgs {
+    const BatchDesc *desc;       // [R] device
+    long long *obs;              // slot of replica 0 for the first sweep of this launch, or nullptr
+    long long obs_stride;        // int64 elements between two replicas' series
+    unsigned long long t0;       // first sweep of this launch (the replicas sweep in lockstep)
+    int nsweeps;
+    int r0;                      // replica of cluster 0
+    int write_run;               // add the last sweep's sums to the replicas' running pairs
+    int one;
+    uint2 seed[SMALL_BATCH_MAX]; // (k0, k1) of replica r0 + i
+};
+
+template <int MODEL, int DIMS, bool TRACK, int OBS>
+__global__ void __launch_bounds__(1024, 1)
+k_sweep_small_lane_batch(const __grid_constant__ SmallBatchArgs a, const int lg_lpr, const int lg_L, const int lg_rpc,
+                         const int lg_clu)
+{
+    __shared__ __align__(16) struct {
+        uint32_t t[MODEL == M_ISING_ONE ? 64 : 16];
+        int acc[2][2];
+    } sm;
+    uint32_t s_t = (uint32_t)__cvta_generic_to_shared(sm.t);
+    asm volatile("" : "+r"(s_t));
+    const int ci = (int)(blockIdx.x >> lg_clu);                  // cluster index = replica of this launch
+    const BatchDesc &d = a.desc[a.r0 + ci];
+    constexpr int NT = MODEL == M_ISING_ONE ? 64 : MODEL == M_ISING_HALF ? 16 : 0;
+    for (int i = threadIdx.x; i < NT; i += blockDim.x) sm.t[i] = d.tab[i];
+    if (threadIdx.x < 4) sm.acc[threadIdx.x >> 1][threadIdx.x & 1] = 0;
+    const uint2 sd = a.seed[ci];
+    PhiloxSweepConsts pk;
+#pragma unroll
+    for (int r = 0; r < 10; ++r) {
+        pk.rk0[r] = sd.x + (uint32_t)r * PHILOX_W0;
+        pk.rk1[r] = sd.y + (uint32_t)r * PHILOX_W1;
+    }
+    pk.x1 = pk.y2 = pk.z2 = pk.w3 = 0u;
+    const unsigned long long seed = ((unsigned long long)sd.y << 32) | sd.x;
+    long long *obs = (OBS >= 1 && a.obs) ? a.obs + a.obs_stride * (a.r0 + ci) : nullptr;
+    small_lane_body<MODEL, DIMS, TRACK, OBS>(d.col[0], d.col[1], pk, seed, a.t0, a.nsweeps, obs,
+                                             a.write_run ? d.run : nullptr, true, d.ne_t32, d.ne_always, (uint32_t)a.one,
+                                             s_t, sm.acc, lg_lpr, lg_L, lg_rpc);
 }
 
 // ------------------------------------------------------------------------------------------
@@ -398,6 +472,111 @@ cudaError_t launch_sweep_small(const Lat &lat, int model, int track, unsigned lo
         return small_launch_to<M_NE_METROPOLIS, 2>(tr, obs, plan.threads, s, a, pk, nt, lg_lpr, lg_L, plan.cluster);
     }
     }
+}
+
+// ------------------------------------------------------------------------------------------
+// Batch: R replicas, one cluster each, one launch (lsm_batch_sweep*)
+// ------------------------------------------------------------------------------------------
+bool small_batch_supported(const Lat &lat, int model, const TiledTables &t)
+{
+    SmallPlan p;
+    return small_plan(lat, model, t, &p, true) && p.lane == 1;
+}
+
+// Blocks per replica.  One lattice alone takes the largest cluster that keeps >= 4 warps per block (latency bound);
+// R lattices together should fill the 148 SMs about twice over and no more: smaller clusters mean cheaper barriers.
+int small_batch_cluster(const Lat &lat, int R)
+{
+    const long long nlanes = lat.half / 4, N = 2 * lat.half;
+    int cmax = 1;
+    while (cmax < small_max_cluster() && nlanes / (2 * cmax) >= 128 && 2 * cmax <= lat.L) cmax *= 2;
+    int c = cmax;
+    while (c > 1 && (long long)R * c > 2ll * sm_count()) c >>= 1;
+    while (N / c > 196608 && c < 16) c <<= 1;          // the slab must fit shared memory
+    while (nlanes / c > 1024 * 8 && c < 16) c <<= 1;   // at most 8 lanes per thread and half-sweep
+    return c;
+}
+
+template <int MODEL, int DIMS>
+static cudaError_t small_batch_launch_to(bool track, bool obs, int threads, cudaStream_t s, const SmallBatchArgs &a,
+                                         int nrep, int lg_lpr, int lg_L, int nclu)
+{
+    const size_t smem = ((size_t)1 << (DIMS * lg_L)) / (size_t)nclu;
+    const int lg_rpc = lg_L - ilog2(nclu), lg_clu = ilog2(nclu);
+    auto go = [&](auto kern) -> cudaError_t {
+        if (smem > 48 * 1024) {
+            cudaError_t e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+            if (e != cudaSuccess) return e;
+        }
+        if (nclu > 8) {
+            cudaError_t e = cudaFuncSetAttribute(kern, cudaFuncAttributeNonPortableClusterSizeAllowed, 1);
+            if (e != cudaSuccess) return e;
+        }
+        cudaLaunchConfig_t cfg;
+        memset(&cfg, 0, sizeof(cfg));
+        cfg.gridDim = dim3((unsigned)(nclu * nrep));
+        cfg.blockDim = dim3((unsigned)threads);
+        cfg.dynamicSmemBytes = smem;
+        cfg.stream = s;
+        cudaLaunchAttribute at[1];
+        at[0].id = cudaLaunchAttributeClusterDimension;
+        at[0].val.clusterDim.x = (unsigned)nclu;
+        at[0].val.clusterDim.y = 1;
+        at[0].val.clusterDim.z = 1;
+        cfg.attrs = at;
+        cfg.numAttrs = 1;
+        return cudaLaunchKernelEx(&cfg, kern, a, lg_lpr, lg_L, lg_rpc, lg_clu);
+    };
+    if (track) return obs ? go(k_sweep_small_lane_batch<MODEL, DIMS, true, 2>) : go(k_sweep_small_lane_batch<MODEL, DIMS, true, 0>);
+    return obs ? go(k_sweep_small_lane_batch<MODEL, DIMS, false, 2>) : go(k_sweep_small_lane_batch<MODEL, DIMS, false, 0>);
+}
+
+// d_obs: slot of replica 0 for the first sweep of this launch (replica r at d_obs + r * obs_stride) or nullptr;
+// write_run: the last sweep's (B, M) also go to every replica's running pair.  Observables are formed iff d_obs or
+// write_run.  Replicas beyond SMALL_BATCH_MAX take further launches.
+cudaError_t launch_sweep_small_batch(const Lat &lat, int model, int track, const BatchDesc *d_desc, const uint64_t *seeds,
+                                     int R, int cluster, unsigned long long t0, int nsweeps, long long *d_obs,
+                                     long long obs_stride, int write_run, cudaStream_t s)
+{
+    int lg_L = 0;
+    while ((1 << lg_L) < lat.L) ++lg_L;
+    const int lg_lpr = lg_L - 3;
+    const long long per = (lat.half / 4) / cluster;
+    const int threads = (int)(per < 1024 ? ((per + 31) / 32) * 32 : 1024);
+    const bool obs = d_obs != nullptr || write_run != 0, tr = track != 0;
+    for (int r0 = 0; r0 < R; r0 += SMALL_BATCH_MAX) {
+        const int nrep = R - r0 < SMALL_BATCH_MAX ? R - r0 : SMALL_BATCH_MAX;
+        SmallBatchArgs a;
+        memset(&a, 0, sizeof(a));
+        a.desc = d_desc;
+        a.obs = d_obs;
+        a.obs_stride = obs_stride;
+        a.t0 = t0;
+        a.nsweeps = nsweeps;
+        a.r0 = r0;
+        a.write_run = write_run;
+        a.one = 1;
+        for (int i = 0; i < nrep; ++i) a.seed[i] = make_uint2((uint32_t)seeds[r0 + i], (uint32_t)(seeds[r0 + i] >> 32));
+        cudaError_t e;
+        switch (model) {
+        case M_ISING_HALF:
+            e = lat.dims == 3 ? small_batch_launch_to<M_ISING_HALF, 3>(tr, obs, threads, s, a, nrep, lg_lpr, lg_L, cluster)
+                              : small_batch_launch_to<M_ISING_HALF, 2>(tr, obs, threads, s, a, nrep, lg_lpr, lg_L, cluster);
+            break;
+        case M_ISING_ONE:
+            e = lat.dims == 3 ? small_batch_launch_to<M_ISING_ONE, 3>(tr, obs, threads, s, a, nrep, lg_lpr, lg_L, cluster)
+                              : small_batch_launch_to<M_ISING_ONE, 2>(tr, obs, threads, s, a, nrep, lg_lpr, lg_L, cluster);
+            break;
+        case M_NE_HEATBATH:
+            e = small_batch_launch_to<M_NE_HEATBATH, 2>(tr, obs, threads, s, a, nrep, lg_lpr, lg_L, cluster);
+            break;
+        default:
+            e = small_batch_launch_to<M_NE_METROPOLIS, 2>(tr, obs, threads, s, a, nrep, lg_lpr, lg_L, cluster);
+            break;
+        }
+        if (e != cudaSuccess) return e;
+    }
+    return cudaSuccess;
 }
 
 }  // namespace lsmk

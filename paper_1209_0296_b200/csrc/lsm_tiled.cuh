@@ -43,4 +43,18 @@ cudaError_t launch_sweep_small(const Lat &lat, int model, int track, unsigned lo
                                int nsweeps, long long *d_obs, const SmallPlan &plan, const TiledTables &t,
                                cudaStream_t s);
 
+// Batch of R same-shape lattices (lsm_batch_*): one launch of the small family's lane kernel, one cluster per replica.
+struct BatchDesc {               // per replica, in device memory
+    uint8_t *col[2];
+    long long *run;              // the replica's running (B, M) pair
+    uint32_t ne_t32;
+    int ne_always;
+    uint32_t tab[64];            // HalfTab (16) or OneTab (64) of the replica's temperature
+};
+bool small_batch_supported(const Lat &lat, int model, const TiledTables &t);
+int small_batch_cluster(const Lat &lat, int R);                          // blocks per replica for R replicas
+cudaError_t launch_sweep_small_batch(const Lat &lat, int model, int track, const BatchDesc *d_desc, const uint64_t *seeds,
+                                     int R, int cluster, unsigned long long t0, int nsweeps, long long *d_obs,
+                                     long long obs_stride, int write_run, cudaStream_t s);
+
 }  // namespace lsmk

@@ -31,6 +31,18 @@ SIGNATURES = {
     "lsm_sweep_record_host": (_i32, [_vp, _i64, _vp, _vp, _vp]),
     "lsm_sweep_random_tile": (_i32, [_vp, _i64, _i32, _i32, _vp, _vp]),
     "lsm_sweep_random_tile_balanced": (_i32, [_vp, _i64, _i32, _i32, _vp, _vp]),
+    "lsm_batch_workspace_bytes": (_i32, [_i32, _i32, _i32, _i32, _i32, _P(_sz)]),
+    "lsm_batch_create": (_i32, [_i32, _i32, _i32, _i32, _i32, _dbl, _dbl, _vp, _vp, _vp, _sz, _vp, _P(_vp)]),
+    "lsm_batch_destroy": (_i32, [_vp]),
+    "lsm_batch_size": (_i32, [_vp, _P(_i32)]),
+    "lsm_batch_replica": (_i32, [_vp, _i32, _P(_vp)]),
+    "lsm_batch_sweep": (_i32, [_vp, _i64, _vp]),
+    "lsm_batch_sweep_record": (_i32, [_vp, _i64, _vp, _vp]),
+    "lsm_batch_set_temperatures": (_i32, [_vp, _vp]),
+    "lsm_batch_set_tracking": (_i32, [_vp, _i32, _vp]),
+    "lsm_batch_set_cluster": (_i32, [_vp, _i32]),
+    "lsm_batch_measure_int": (_i32, [_vp, _vp, _vp]),
+    "lsm_batch_get_launch_count": (_i32, [_vp, _P(_u64)]),
     "lsm_measure": (_i32, [_vp, _P(_dbl), _P(_i64)]),
     "lsm_measure_int": (_i32, [_vp, _P(_i64), _P(_i64), _P(_u64)]),
     "lsm_measure_full": (_i32, [_vp, _P(_i64), _P(_i64)]),
@@ -331,6 +343,123 @@ class Lattice:
     def launch_count(self):
         n = _u64()
         _check(self._lib.lsm_get_launch_count(self._h, ctypes.byref(n)), "lsm_get_launch_count")
+        return int(n.value)
+
+
+class Batch:
+    """R lattices of one shape with per-replica temperature and seed, swept by one launch (lsm_batch_*).
+
+    `replica(r)` is a Lattice view of replica r (borrowed handle) for get_spins / persistence / thresholds ..."""
+
+    def __init__(self, dims, L, T, seeds, two_S=1, model=ISING, J=1.0, h=0.0, device="cuda:0", stream=None):
+        import torch
+
+        if not torch.cuda.is_available():
+            raise RuntimeError("liblsm needs a CUDA device (there is no CPU fallback)")
+        self._lib = load()
+        self.T = [float(t) for t in T]
+        self.seeds = [int(x) for x in seeds]
+        assert len(self.T) == len(self.seeds) and len(self.T) >= 1
+        self.R = len(self.T)
+        self.dims, self.L, self.two_S, self.model, self.J, self.h = int(dims), int(L), int(two_S), int(model), float(J), float(h)
+        self.device = torch.device(device)
+        self.N = self.L ** self.dims
+        n = _sz()
+        _check(self._lib.lsm_batch_workspace_bytes(self.R, self.dims, self.L, self.two_S, self.model, ctypes.byref(n)),
+               "lsm_batch_workspace_bytes")
+        self._h = None
+        self._last_stream = None
+        with torch.cuda.device(self.device):
+            self._ws = torch.empty(n.value + 256, dtype=torch.uint8, device=self.device)
+            ptr = self._ws.data_ptr() + (-self._ws.data_ptr()) % 256
+            Ta = (ctypes.c_double * self.R)(*self.T)
+            Sa = (ctypes.c_uint64 * self.R)(*self.seeds)
+            h_ = _vp()
+            _check(self._lib.lsm_batch_create(self.R, self.dims, self.L, self.two_S, self.model, self.J, self.h, Ta, Sa,
+                                              _vp(ptr), n.value, self._sp(stream), ctypes.byref(h_)), "lsm_batch_create")
+        self._h = h_
+        self._views = {}
+
+    def _sp(self, stream):
+        import torch
+
+        self._last_stream = torch.cuda.current_stream(self.device) if stream is None else stream
+        return ctypes.c_void_p(self._last_stream.cuda_stream)
+
+    @_on_device
+    def close(self):
+        if getattr(self, "_h", None):
+            if self._last_stream is not None:
+                self._last_stream.synchronize()
+            for v in self._views.values():
+                v._h = None                      # borrowed handles die with the batch
+            self._views = {}
+            self._lib.lsm_batch_destroy(self._h)
+            self._h = None
+            self._ws = None
+
+    def __del__(self):
+        try:
+            self.close()
+        except Exception:
+            pass
+
+    def replica(self, r):
+        """Lattice view of replica r (borrowed: closing it does nothing)."""
+        if r not in self._views:
+            h_ = _vp()
+            _check(self._lib.lsm_batch_replica(self._h, int(r), ctypes.byref(h_)), "lsm_batch_replica")
+            v = Lattice.__new__(Lattice)
+            v._lib, v._h, v._ws, v._scratch, v._last_stream = self._lib, h_, None, None, None
+            v.dims, v.L, v.two_S, v.model, v.J, v.h = self.dims, self.L, self.two_S, self.model, self.J, self.h
+            v.T, v.seed, v.device, v.N = self.T[r], self.seeds[r], self.device, self.N
+            v.close = lambda: None
+            self._views[r] = v
+        return self._views[r]
+
+    @_on_device
+    def sweep(self, n=1, stream=None):
+        _check(self._lib.lsm_batch_sweep(self._h, int(n), self._sp(stream)), "lsm_batch_sweep")
+
+    @_on_device
+    def sweep_record(self, n, out=None, stream=None):
+        """n sweeps of every replica; device int64 [R, n, 2] = (B, M) of replica r after sweep k."""
+        import torch
+
+        if out is None:
+            out = torch.empty((self.R, int(n), 2), dtype=torch.int64, device=self.device)
+        assert out.is_cuda and out.dtype == torch.int64 and out.is_contiguous() and out.numel() >= 2 * int(n) * self.R
+        _check(self._lib.lsm_batch_sweep_record(self._h, int(n), _vp(out.data_ptr()), self._sp(stream)),
+               "lsm_batch_sweep_record")
+        return out
+
+    @_on_device
+    def set_temperatures(self, T):
+        T = [float(t) for t in T]
+        assert len(T) == self.R
+        _check(self._lib.lsm_batch_set_temperatures(self._h, (ctypes.c_double * self.R)(*T)), "lsm_batch_set_temperatures")
+        self.T = T
+        for r, v in self._views.items():
+            v.T = T[r]
+
+    @_on_device
+    def set_tracking(self, on, stream=None):
+        _check(self._lib.lsm_batch_set_tracking(self._h, 1 if on else 0, self._sp(stream)), "lsm_batch_set_tracking")
+
+    def set_cluster(self, blocks_per_replica):
+        _check(self._lib.lsm_batch_set_cluster(self._h, int(blocks_per_replica)), "lsm_batch_set_cluster")
+
+    @_on_device
+    def measure_int(self):
+        """[(B, M)] of every replica's current configuration (synchronises once)."""
+        Bv, Mv = (ctypes.c_int64 * self.R)(), (ctypes.c_int64 * self.R)()
+        _check(self._lib.lsm_batch_measure_int(self._h, Bv, Mv), "lsm_batch_measure_int")
+        return [(int(Bv[r]), int(Mv[r])) for r in range(self.R)]
+
+    @property
+    def launch_count(self):
+        n = _u64()
+        _check(self._lib.lsm_batch_get_launch_count(self._h, ctypes.byref(n)), "lsm_batch_get_launch_count")
         return int(n.value)
 
 

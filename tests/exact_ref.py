@@ -162,3 +162,54 @@ def binned_mean_err(x, nbins=32):
     n = (len(x) // nbins) * nbins
     b = x[:n].reshape(nbins, -1).mean(axis=1)
     return b.mean(), b.std(ddof=1) / math.sqrt(nbins)
+
+
+# ------------------------------------------------------------------ 4x4 +/-J bonds (reading D25)
+def ea4x4_exact(T, tau, J=1.0, h=0.0):
+    """Boltzmann <E>/N and <B>/N of the 4x4 periodic lattice with bond signs tau[a, i] (a = 0: bond to x+1,
+    1: bond to y+1) by enumeration of all 2^16 states: H = -J sum tau_ij s_i s_j - h sum s_i."""
+    spins, _, M = ising4x4_states()
+    g = spins.reshape(-1, 4, 4)
+    t = np.asarray(tau, dtype=np.int64).reshape(2, 4, 4)
+    B = (t[0][None] * g * np.roll(g, -1, axis=2)).sum(axis=(1, 2)) + (t[1][None] * g * np.roll(g, -1, axis=1)).sum(axis=(1, 2))
+    E = -J * B - h * M
+    w = np.exp(-(E - E.min()) / T)
+    Z = w.sum()
+    return (w * E).sum() / Z / 16, (w * B).sum() / Z / 16
+
+
+# ------------------------------------------------------------------ 4x4 Potts (reading D26)
+@functools.lru_cache(maxsize=None)
+def potts3_4x4_histogram():
+    src = os.path.join(HERE, "exact", "enum_potts3.c")
+    so = os.path.join(HERE, "exact", "libenum_potts3.so")
+    if not os.path.exists(so) or os.path.getmtime(so) < os.path.getmtime(src):
+        tmp = so + f".tmp{os.getpid()}"
+        subprocess.check_call(["gcc", "-O2", "-fPIC", "-shared", "-o", tmp, src])
+        os.replace(tmp, so)
+    lib = ctypes.CDLL(so)
+    g = np.zeros((33, 17), dtype=np.int64)
+    lib.enum_potts3_4x4(ctypes.c_void_p(g.ctypes.data))
+    assert g.sum() == 3 ** 16
+    return g
+
+
+def potts3_4x4_exact(T, J=1.0):
+    """<E>/N, C/N, <N0>/N, <N0^2>/N^2 of the 4x4 3-state Potts lattice, H = -J * (equal bonds)."""
+    g = potts3_4x4_histogram().astype(np.float64)
+    B = np.arange(0, 33)[:, None].astype(float)
+    N0 = np.arange(0, 17)[None, :].astype(float)
+    E = -J * B + 0 * N0
+    w = g * np.exp(-(E - E[g > 0].min()) / T)
+    Z = w.sum()
+    e1 = (w * E).sum() / Z
+    e2 = (w * E * E).sum() / Z
+    return e1 / 16, (e2 - e1 * e1) / (16 * T * T), (w * N0).sum() / Z / 16, (w * N0 * N0).sum() / Z / 256
+
+
+def potts2_4x4_exact(T, J=1.0):
+    """q = 2: delta(s, s') = (1 + s s')/2, so H = -(J/2) sum s s' - 16 J: the Ising enumeration at coupling J/2."""
+    _, B, _ = ising4x4_states()
+    E = -J * (B + 32) / 2.0
+    w = np.exp(-(E - E.min()) / T)
+    return (w * E).sum() / w.sum() / 16

@@ -52,6 +52,20 @@ MUTANTS = [
      "ctr[3] = (4u + launch) | ((uint32_t)(o->t >> 32) << 4);", [TILE], "balanced_matches"),
     ("tile_lowest_thread_wins", "for (int j2 = j + 1; j2 < lambda; ++j2) dup |= (site[j2] == site[j]);\n                        if (dup) continue;                     /* a higher",
      "for (int j2 = 0; j2 < j; ++j2) dup |= (site[j2] == site[j]);\n                        if (dup) continue;                     /* a higher", [TILE], "matches_the_dict"),
+    # ---- NEXT-4 models (tests/test_oracle_wider_models.py)
+    ("ea_backward_bond_read_from_the_wrong_site", "bond_sign(o, 0, x - 1, y, z) * value_at(o, x - 1, y, z)",
+     "bond_sign(o, 0, x, y, z) * value_at(o, x - 1, y, z)", [WIDE], "ea_"),
+    ("ea_bonds_drawn_from_the_init_stream", "words_of_group(o->seed, (uint64_t)b >> 2, 0, 3u, w4);",
+     "words_of_group(o->seed, (uint64_t)b >> 2, 0, 2u, w4);", [WIDE], "bonds_from_seed"),
+    ("ea_bond_sign_inverted", "o->tau[b] = (w4[b & 3] >> 31) ? 1 : -1;", "o->tau[b] = (w4[b & 3] >> 31) ? -1 : 1;", [WIDE], "bonds_from_seed"),
+    ("ea_bond_energy_ignores_the_signs", "int f = bond_sign(o, 0, x, y, z) * value_at(o, x + 1, y, z) + bond_sign(o, 1, x, y, z) * value_at(o, x, y + 1, z);",
+     "int f = value_at(o, x + 1, y, z) + value_at(o, x, y + 1, z);", [WIDE], "ea_"),
+    ("potts_proposal_may_repeat_the_state", "int prop = (s_old + 1 + r) % o->q;", "int prop = (s_old + r) % o->q;", [WIDE], "potts_matches"),
+    ("potts_energy_difference_sign", "int dn = neighbours_equal_to(o, x, y, z, prop) - neighbours_equal_to(o, x, y, z, s_old);",
+     "int dn = neighbours_equal_to(o, x, y, z, s_old) - neighbours_equal_to(o, x, y, z, prop);", [WIDE], "potts_matches"),
+    ("potts_init_modulo", "v = (int)(((uint64_t)w * (uint64_t)o->q) >> 32);", "v = (int)(w % (uint32_t)o->q);", [WIDE], "potts_matches"),
+    ("potts_overlap_as_product", "if (o->model == ORC_POTTS) { ov += (a == b); continue; }", "if (o->model == ORC_POTTS) { ov += a * b; continue; }", [WIDE], "potts_matches"),
+    ("potts_table_shifted", "if ((uint64_t)w1 < o->thr[dn + 2 * o->dims]) s_new = prop;", "if ((uint64_t)w1 < o->thr[dn + 2 * o->dims + 1]) s_new = prop;", [WIDE], "potts_"),
 ]
 
 
