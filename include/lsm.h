@@ -33,6 +33,13 @@
  *                         up (D8); then n_i is redrawn from Bernoulli(c) (D7).
  *  LSM_NE_METROPOLIS    : same constraint, Metropolis flip: 1->0 always,
  *                         0->1 with probability exp(-1/T).
+ *  LSM_EA, two_S = 1     : Edwards-Anderson +/-J spin glass (Eq. 1 with discrete J_ij; D25):
+ *                         H = -J sum_<ij> tau_ij s_i s_j - h sum s_i, tau_ij = +/-1 per bond, drawn from the seed
+ *                         (p = 1/2) or set with lsm_set_bonds; Ising rule on the bond-weighted neighbour sum.
+ *  LSM_POTTS             : q-state Potts model (D26), q = two_S + 1 in [2, 8], sigma in {0..q-1},
+ *                         H = -J sum_<ij> delta(sigma_i, sigma_j), h must be 0; trial state uniform over the other
+ *                         q-1 states, Metropolis acceptance.  bond_sum = bonds joining equal states, M = sites in
+ *                         state 0, E = -J * bond_sum; overlap of lsm_persistence = sites in their reference state.
  *  Acceptance (P = min[1, exp(-dH/T)]) is an integer compare of a 32-bit
  *  random word w with a 33-bit threshold thr = floor(P * 2^32) in [0, 2^32]: accept iff
  *  w < thr (D3).
@@ -66,7 +73,7 @@ extern "C" {
 typedef struct lsm lsm_t;             /* opaque, host heap */
 typedef struct lsm_batch lsm_batch_t; /* opaque, host heap: R lattices of one shape swept together */
 
-enum { LSM_ISING = 0, LSM_NE_HEATBATH = 1, LSM_NE_METROPOLIS = 2 };
+enum { LSM_ISING = 0, LSM_NE_HEATBATH = 1, LSM_NE_METROPOLIS = 2, LSM_EA = 3, LSM_POTTS = 4 };
 enum {
     LSM_OK = 0,
     LSM_ERR_ARG = -1,         /* dims not 2|3, L odd or < 4, T <= 0 or non-finite, NULL, n < 0 */
@@ -186,11 +193,19 @@ int lsm_set_spins(lsm_t *, const int8_t *d_in, uint64_t sweep_counter, void *str
 int lsm_set_spins_host(lsm_t *, const int8_t *h_in, int8_t *d_scratch /* N bytes */,
                        uint64_t sweep_counter, void *stream);
 
+/* LSM_EA only (else UNSUPPORTED): bond signs in canonical form, d_tau int8 [dims][N] on the device, tau[a][i] = sign
+ * (+1 ferro, -1 antiferro) of the bond between site i and its neighbour in direction +a (a = 0, 1, 2 = x, y, z).
+ * lsm_set_bonds replaces them (values < 0 are antiferromagnetic) and recomputes (B, M). */
+int lsm_set_bonds(lsm_t *, const int8_t *d_tau, void *stream);
+int lsm_get_bonds(lsm_t *, int8_t *d_tau, void *stream);
+
 int lsm_set_temperature(lsm_t *, double T); /* rebuilds the thresholds (host, D3) */
 /* Host copy of the 33-bit thresholds, in the canonical order:
  *  Ising two_S=1: idx = b*(2d+1) + (nn+2d)/2, b=(s+1)/2                         [2(2d+1)]
  *  Ising two_S=2: idx = ((s+1)*2 + kk)*(4d+1) + (nn+2d), proposal (s+1+1+kk)%3  [6(4d+1)]
  *  NE: {floor(c*2^32), floor(exp(-1/T)*2^32), 2^32}                              [3]
+ *  EA: as Ising two_S=1 with nn = sum_j tau_ij s_j                                [2(2d+1)]
+ *  Potts: idx = (n_new - n_old) + 2d                                              [4d+1]
  * out may be NULL to query count.  out must hold 128 entries. */
 int lsm_get_thresholds(lsm_t *, uint64_t *out, int *count);
 

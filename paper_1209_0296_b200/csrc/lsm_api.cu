@@ -57,7 +57,9 @@ static int check_shape(int dims, int L, int two_S, int model)
     if (model == LSM_ISING) { if (two_S != 1 && two_S != 2) return LSM_ERR_UNSUPPORTED; }
     else if (model == LSM_NE_HEATBATH || model == LSM_NE_METROPOLIS) {
         if (dims != 2 || two_S != 1) return LSM_ERR_UNSUPPORTED;
-    } else return LSM_ERR_ARG;
+    } else if (model == LSM_EA) { if (two_S != 1) return LSM_ERR_UNSUPPORTED; }          // reading D25: spin-1/2
+    else if (model == LSM_POTTS) { if (two_S < 1 || two_S > 7) return LSM_ERR_UNSUPPORTED; }   // D26: q = two_S + 1 <= 8
+    else return LSM_ERR_ARG;
     return LSM_OK;
 }
 
@@ -68,7 +70,8 @@ extern "C" int lsm_workspace_bytes(int dims, int L, int two_S, int model, size_t
     if (rc != LSM_OK) return rc;
     size_t N = (size_t)L * L * (dims == 3 ? (size_t)L : 1);
     *bytes = STATE_BYTES + 2 * align256(N / 2) + 256;
-    if (model != LSM_ISING) *bytes += 2 * align256(N / 2);   // second buffer of the random-tile schedule
+    if (model == LSM_NE_HEATBATH || model == LSM_NE_METROPOLIS) *bytes += 2 * align256(N / 2);   // second buffer of the random-tile schedule
+    if (model == LSM_EA) *bytes += 2 * align256(N / 2);      // bond bytes of the two colours
     return LSM_OK;
 }
 
@@ -92,7 +95,15 @@ static void build_tables(lsm *o)
 {
     const int d = o->dims;
     int n = 0;
-    if (o->model == M_ISING_HALF) {
+    if (o->model == M_POTTS) {
+        // reading D26: dE = -J * dn, dn = n_new - n_old, idx = dn + 2d
+        for (int j = 0; j <= 4 * d; ++j) {
+            double x = o->J * (double)(j - 2 * d);
+            double dE = -x;
+            o->thr[n++] = dE <= 0.0 ? ((uint64_t)1 << 32) : thr_from_p(std::exp(-dE / o->T));
+        }
+    } else if (o->model == M_ISING_HALF || o->model == M_EA) {
+        // M_EA (reading D25): the same table, indexed by the bond-weighted up-count
         for (int b = 0; b < 2; ++b)
             for (int j = 0; j <= 2 * d; ++j) o->thr[n++] = thr_flip(o->J, o->h, o->T, 2 * b - 1, 1 - 2 * b, 2 * j - 2 * d);
     } else if (o->model == M_ISING_ONE) {
@@ -143,7 +154,8 @@ extern "C" int lsm_create(int dims, int L, int two_S, int model, double J, doubl
     int rc = check_shape(dims, L, two_S, model);
     if (rc != LSM_OK) return rc;
     if (!(T > 0.0) || !std::isfinite(T) || !std::isfinite(J) || !std::isfinite(h)) return LSM_ERR_ARG;
-    if (model != LSM_ISING && J != 0.0) return LSM_ERR_UNSUPPORTED;
+    if ((model == LSM_NE_HEATBATH || model == LSM_NE_METROPOLIS) && J != 0.0) return LSM_ERR_UNSUPPORTED;
+    if (model == LSM_POTTS && h != 0.0) return LSM_ERR_UNSUPPORTED;        // reading D26: no field term
     size_t need = 0;
     lsm_workspace_bytes(dims, L, two_S, model, &need);
     if (workspace_bytes < need || ((uintptr_t)d_workspace & 255)) return LSM_ERR_WORKSPACE;
@@ -152,6 +164,7 @@ extern "C" int lsm_create(int dims, int L, int two_S, int model, double J, doubl
     if (!o) return LSM_ERR_ARG;
     o->dims = dims; o->L = L; o->two_S = two_S; o->model_abi = model;
     o->model = model == LSM_ISING ? (two_S == 1 ? M_ISING_HALF : M_ISING_ONE)
+             : model == LSM_EA ? M_EA : model == LSM_POTTS ? M_POTTS
              : (model == LSM_NE_HEATBATH ? M_NE_HEATBATH : M_NE_METROPOLIS);
     o->J = J; o->h = h; o->T = T; o->c = 0.0; o->seed = seed;
     o->N = (int64_t)L * L * (dims == 3 ? L : 1);
@@ -162,9 +175,15 @@ extern "C" int lsm_create(int dims, int L, int two_S, int model, double J, doubl
     o->lat.col[0] = base + STATE_BYTES;
     o->lat.col[1] = base + STATE_BYTES + align256((size_t)o->N / 2);
     o->alt[0] = o->alt[1] = nullptr;
-    if (model != LSM_ISING) {
+    o->lat.bnd[0] = o->lat.bnd[1] = nullptr;
+    o->lat.q = model == LSM_POTTS ? two_S + 1 : 0;
+    if (model == LSM_NE_HEATBATH || model == LSM_NE_METROPOLIS) {
         o->alt[0] = o->lat.col[1] + align256((size_t)o->N / 2);
         o->alt[1] = o->alt[0] + align256((size_t)o->N / 2);
+    }
+    if (model == LSM_EA) {
+        o->lat.bnd[0] = o->lat.col[1] + align256((size_t)o->N / 2);
+        o->lat.bnd[1] = o->lat.bnd[0] + align256((size_t)o->N / 2);
     }
     o->lat.L = L; o->lat.Lh = L / 2; o->lat.dims = dims; o->lat.Lz = dims == 3 ? L : 1;
     o->lat.half = o->N / 2;
@@ -176,6 +195,7 @@ extern "C" int lsm_create(int dims, int L, int two_S, int model, double J, doubl
     cudaStream_t s = (cudaStream_t)stream;
     cudaError_t e = cudaMemsetAsync(base, 0, STATE_BYTES, s);
     if (e == cudaSuccess) e = launch_init(o->lat, o->model, seed, o->thr[0], s);
+    if (e == cudaSuccess && o->model == M_EA) { e = launch_ea_bonds_init(o->lat, seed, s); o->launches += 1; }
     if (e == cudaSuccess) e = launch_reset_reference(o->lat, o->model, 1, s);
     if (e == cudaSuccess) e = launch_measure_full(o->lat, o->model, o->d_run, s);
     if (e != cudaSuccess) { delete o; return cuda_fail(e); }
@@ -279,6 +299,7 @@ extern "C" int lsm_sweep_record(lsm_t *o, int64_t n, int64_t *d_obs, void *strea
 static int random_tile_impl(lsm_t *o, int64_t n, int tile_edge, int lambda, int64_t *d_obs, void *stream, bool balanced)
 {
     if (!o || n < 0) return LSM_ERR_ARG;
+    if (o->model != M_NE_HEATBATH && o->model != M_NE_METROPOLIS) return LSM_ERR_UNSUPPORTED;
     if (o->model != M_NE_HEATBATH && o->model != M_NE_METROPOLIS) return LSM_ERR_UNSUPPORTED;
     if (!ne_tile_supported(o->lat, tile_edge, lambda, balanced)) return LSM_ERR_UNSUPPORTED;
     cudaStream_t s = (cudaStream_t)stream;
@@ -563,7 +584,9 @@ static int read_pair(lsm *o, const long long *d, long long out[2])
 extern "C" int lsm_energy(int model, double J, double h, int64_t B, int64_t M, double *E)
 {
     if (!E) return LSM_ERR_ARG;
-    *E = model == LSM_ISING ? -J * (double)B - h * (double)M : (double)M;   // D1, D15
+    if (model == LSM_ISING || model == LSM_EA) *E = -J * (double)B - h * (double)M;   // D1, D25
+    else if (model == LSM_POTTS) *E = -J * (double)B;                                   // D26
+    else *E = (double)M;                                                                // D15
     return LSM_OK;
 }
 
@@ -661,6 +684,28 @@ extern "C" int lsm_set_spins_host(lsm_t *o, const int8_t *h_in, int8_t *d_scratc
     if (!o || !h_in || !d_scratch) return LSM_ERR_ARG;
     CU(cudaMemcpyAsync(d_scratch, h_in, (size_t)o->N, cudaMemcpyHostToDevice, (cudaStream_t)stream));
     return lsm_set_spins(o, d_scratch, sweep_counter, stream);
+}
+
+// Edwards-Anderson bonds (reading D25): canonical int8 tau[dims][N], tau[a][i] = sign of the bond between site i and
+// its neighbour in direction +a.  Replacing the bonds changes B: the running pair is recomputed.
+extern "C" int lsm_set_bonds(lsm_t *o, const int8_t *d_tau, void *stream)
+{
+    if (!o || !d_tau) return LSM_ERR_ARG;
+    if (o->model != M_EA) return LSM_ERR_UNSUPPORTED;
+    o->last_stream = (cudaStream_t)stream;
+    CU(launch_ea_set_bonds(o->lat, d_tau, o->last_stream));
+    o->launches += 1;
+    return refresh_running(o, o->last_stream);
+}
+
+extern "C" int lsm_get_bonds(lsm_t *o, int8_t *d_tau, void *stream)
+{
+    if (!o || !d_tau) return LSM_ERR_ARG;
+    if (o->model != M_EA) return LSM_ERR_UNSUPPORTED;
+    o->last_stream = (cudaStream_t)stream;
+    CU(launch_ea_get_bonds(o->lat, d_tau, o->last_stream));
+    o->launches += 1;
+    return LSM_OK;
 }
 
 extern "C" int lsm_set_temperature(lsm_t *o, double T)

@@ -137,9 +137,97 @@ __global__ void __launch_bounds__(256) k_sweep_generic(const __grid_constant__ S
     if (a.obs) block_accumulate2(accB, accM, a.obs, a.want_B != 0, true);
 }
 
+// The 2d neighbours' bytes in the order k = 0: x-1, 1: x+1, 2: y-1, 3: y+1, 4: z-1, 5: z+1 (the order of the bond
+// bits of M_EA).  x = 2m + q: the other colour's bytes of the own row are x-1 -> m (q = 1) or m-1 (q = 0) and
+// x+1 -> m+1 (q = 1) or m (q = 0).
+__device__ __forceinline__ void neighbour_bytes(const Lat &lat, const uint8_t *__restrict__ oth, const Site &s, uint32_t nb[6])
+{
+    const int L = lat.L, Lh = lat.Lh;
+    const int yu = s.y + 1 == L ? 0 : s.y + 1, yd = s.y == 0 ? L - 1 : s.y - 1;
+    const long long plane = (long long)s.z * L;
+    const int ml = s.m == 0 ? Lh - 1 : s.m - 1, mr = s.m + 1 == Lh ? 0 : s.m + 1;
+    nb[0] = oth[s.row + (s.q ? s.m : ml)];
+    nb[1] = oth[s.row + (s.q ? mr : s.m)];
+    nb[2] = oth[(plane + yd) * Lh + s.m];
+    nb[3] = oth[(plane + yu) * Lh + s.m];
+    nb[4] = nb[5] = 0;
+    if (lat.dims == 3) {
+        const int zu = s.z + 1 == L ? 0 : s.z + 1, zd = s.z == 0 ? L - 1 : s.z - 1;
+        nb[4] = oth[((long long)zd * L + s.y) * Lh + s.m];
+        nb[5] = oth[((long long)zu * L + s.y) * Lh + s.m];
+    }
+}
+
+// NEXT-4 models, scalar form (readings D25, D26).
+//  M_EA   : Ising spin-1/2 rule on the bond-weighted neighbour sum: an antiferromagnetic bond turns the neighbour's
+//           "up" into "down", so the up-count is sum_k (b_k xor bond bit k); same table, same word map.
+//  M_POTTS: two words per site (group k>>1): w0 proposes one of the other q-1 states, w1 accepts by Metropolis on
+//           dn = (neighbours equal to the new state) - (neighbours equal to the old one); table idx dn + 2d.
+// Observables: M_EA  M = sum s', B += s' * nn_eff (second colour only: every bond joins the two colours);
+//              M_POTTS  M = sites in state 0, B += neighbours equal to the new state (second colour only).
+template <int MODEL>
+__global__ void __launch_bounds__(256) k_sweep_wider(const __grid_constant__ SweepArgs a, const __grid_constant__ Thr64 thr)
+{
+    constexpr uint32_t VAL = Enc<MODEL>::VAL, CHG = Enc<MODEL>::CHG;
+    __shared__ unsigned long long s_thr[96];
+    for (int i = threadIdx.x; i < 96; i += blockDim.x) s_thr[i] = thr.thr[i];
+    __syncthreads();
+
+    const Lat &lat = a.lat;
+    uint8_t *__restrict__ own = a.half ? lat.col[1] : lat.col[0];
+    const uint8_t *__restrict__ oth = a.half ? lat.col[0] : lat.col[1];
+    const uint8_t *__restrict__ bnd = MODEL == M_EA ? (a.half ? lat.bnd[1] : lat.bnd[0]) : nullptr;
+    const int d = lat.dims, nk = 2 * d;
+    const uint32_t q = (uint32_t)lat.q;
+    long long accB = 0, accM = 0;
+
+    for (long long k = (long long)blockIdx.x * blockDim.x + threadIdx.x; k < lat.half;
+         k += (long long)gridDim.x * blockDim.x) {
+        const Site s = site_of(lat, k, a.half);
+        const uint32_t old = own[k], v = old & VAL;
+        uint32_t vn = v, nb[6];
+        neighbour_bytes(lat, oth, s, nb);
+        if (MODEL == M_EA) {
+            const uint32_t bb = bnd[k];
+            int sum = 0;
+            for (int j = 0; j < nk; ++j) sum += (int)((nb[j] ^ (bb >> j)) & 1u);
+            uint4 r = philox4x32_10((uint32_t)(k >> 2), (uint32_t)(k >> 34), a.key.c2, a.key.c3, a.key.k0, a.key.k1);
+            uint32_t w = (k & 2) ? ((k & 1) ? r.w : r.z) : ((k & 1) ? r.y : r.x);
+            if ((unsigned long long)w < s_thr[v * (2 * d + 1) + sum]) vn = v ^ 1u;
+            const int s_new = 2 * (int)vn - 1;
+            accM += s_new;
+            accB += s_new * (2 * sum - 2 * d);
+        } else {
+            uint4 r = philox4x32_10((uint32_t)(k >> 1), (uint32_t)(k >> 33), a.key.c2, a.key.c3, a.key.k0, a.key.k1);
+            const uint32_t w0 = (k & 1) ? r.z : r.x, w1 = (k & 1) ? r.w : r.y;
+            uint32_t prop = v + 1u + __umulhi(w0, q - 1u);
+            prop = prop >= q ? prop - q : prop;
+            int n_old = 0, n_new = 0;
+            for (int j = 0; j < nk; ++j) {
+                n_old += (nb[j] & VAL) == v;
+                n_new += (nb[j] & VAL) == prop;
+            }
+            if ((unsigned long long)w1 < s_thr[n_new - n_old + 2 * d]) { vn = prop; n_old = n_new; }
+            accM += vn == 0u;
+            accB += n_old;                      // neighbours equal to the state the site ends up in
+        }
+        if (vn != v) {
+            uint32_t nbyte = (old & ~VAL) | vn;
+            if (a.track) nbyte |= CHG;
+            own[k] = (uint8_t)nbyte;
+        }
+    }
+    if (a.obs) block_accumulate2(accB, accM, a.obs, a.want_B != 0, true);
+}
+
 cudaError_t launch_sweep_generic(const SweepArgs &a, const Thr64 &thr, cudaStream_t s)
 {
     int grid = grid_for(a.lat.half, 256, 8);
+    switch (a.model) {
+    case M_EA:            k_sweep_wider<M_EA><<<grid, 256, 0, s>>>(a, thr); return cudaGetLastError();
+    case M_POTTS:         k_sweep_wider<M_POTTS><<<grid, 256, 0, s>>>(a, thr); return cudaGetLastError();
+    default: break;
+    }
     switch (a.model) {
     case M_ISING_HALF:    k_sweep_generic<M_ISING_HALF><<<grid, 256, 0, s>>>(a, thr); break;
     case M_ISING_ONE:     k_sweep_generic<M_ISING_ONE><<<grid, 256, 0, s>>>(a, thr); break;
@@ -168,8 +256,9 @@ __global__ void __launch_bounds__(256) k_init(Lat lat, int model, SweepKey key, 
             int z = (int)(ry / lat.L);
             int y = (int)(ry - (long long)z * lat.L);
             uint32_t v;
-            if (model == M_ISING_HALF) v = w[j] >> 31;
+            if (model == M_ISING_HALF || model == M_EA) v = w[j] >> 31;
             else if (model == M_ISING_ONE) v = __umulhi(w[j], 3u);
+            else if (model == M_POTTS) v = __umulhi(w[j], (uint32_t)lat.q);       // reading D26
             else v = ((unsigned long long)w[j] < thr_c) ? 1u : 0u;
             uint8_t *dst = ((x + y + z) & 1) ? lat.col[1] : lat.col[0];
             dst[i >> 1] = (uint8_t)v;
@@ -283,10 +372,43 @@ __global__ void __launch_bounds__(256) k_measure_words(Lat lat, long long *out)
     block_accumulate2(accB, accM, out, true, true);
 }
 
+// Full reduction of the NEXT-4 models: B over the colour-0 sites' bonds (every bond joins the two colours).
+template <int MODEL>
+__global__ void __launch_bounds__(256) k_measure_wider(Lat lat, long long *out)
+{
+    constexpr uint32_t VAL = Enc<MODEL>::VAL;
+    long long accB = 0, accM = 0;
+    const int nk = 2 * lat.dims;
+    for (long long k = (long long)blockIdx.x * blockDim.x + threadIdx.x; k < lat.half;
+         k += (long long)gridDim.x * blockDim.x) {
+        const Site s = site_of(lat, k, 0);
+        uint32_t nb[6];
+        neighbour_bytes(lat, lat.col[1], s, nb);
+        const uint32_t v0 = lat.col[0][k] & VAL, v1 = lat.col[1][k] & VAL;
+        if (MODEL == M_EA) {
+            const uint32_t bb = lat.bnd[0][k];
+            int sum = 0;
+            for (int j = 0; j < nk; ++j) sum += (int)((nb[j] ^ (bb >> j)) & 1u);
+            accM += 2 * (int)(v0 + v1) - 2;
+            accB += (2 * (int)v0 - 1) * (2 * sum - nk);
+        } else {
+            for (int j = 0; j < nk; ++j) accB += (nb[j] & VAL) == v0;
+            accM += (v0 == 0u) + (v1 == 0u);
+        }
+    }
+    block_accumulate2(accB, accM, out, true, true);
+}
+
 cudaError_t launch_measure_full(const Lat &lat, int model, long long *d_BM, cudaStream_t s)
 {
     cudaError_t e = cudaMemsetAsync(d_BM, 0, 2 * sizeof(long long), s);
     if (e != cudaSuccess) return e;
+    if (model == M_EA || model == M_POTTS) {
+        const int grid = grid_for(lat.half, 256, 8);
+        if (model == M_EA) k_measure_wider<M_EA><<<grid, 256, 0, s>>>(lat, d_BM);
+        else k_measure_wider<M_POTTS><<<grid, 256, 0, s>>>(lat, d_BM);
+        return cudaGetLastError();
+    }
     if (lat.Lh % 16 == 0) {
         const int grid = grid_for(lat.half >> 4, 256, 8);
         const bool d3 = lat.dims == 3;
@@ -320,6 +442,7 @@ __device__ __forceinline__ void persist_byte(uint32_t b, long long &nc, long lon
     nc += (b & CHG) ? 0 : 1;
     int now = (int)(b & VAL), ref = (int)((b & REF) >> SH);
     if (MODEL == M_ISING_ONE) ov += (now - 1) * (ref - 1);
+    else if (MODEL == M_POTTS) ov += now == ref;              // reading D26: sites in their reference state
     else ov += (2 * now - 1) * (2 * ref - 1);
 }
 
@@ -354,7 +477,8 @@ cudaError_t launch_persistence(const Lat &lat, int model, long long *d_out2, cud
     if (e != cudaSuccess) return e;
     int grid = grid_for((lat.half >> 4) + 1, 256, 8);
     if (model == M_ISING_ONE) k_persistence<M_ISING_ONE><<<grid, 256, 0, s>>>(lat, d_out2);
-    else if (model == M_ISING_HALF) k_persistence<M_ISING_HALF><<<grid, 256, 0, s>>>(lat, d_out2);
+    else if (model == M_POTTS) k_persistence<M_POTTS><<<grid, 256, 0, s>>>(lat, d_out2);
+    else if (model == M_ISING_HALF || model == M_EA) k_persistence<M_ISING_HALF><<<grid, 256, 0, s>>>(lat, d_out2);
     else k_persistence<M_NE_HEATBATH><<<grid, 256, 0, s>>>(lat, d_out2);
     return cudaGetLastError();
 }
@@ -380,6 +504,7 @@ cudaError_t launch_reset_reference(const Lat &lat, int model, int tracking_on, c
 {
     int grid = grid_for(lat.half, 256, 8);
     if (model == M_ISING_ONE) k_reset_reference<M_ISING_ONE><<<grid, 256, 0, s>>>(lat, tracking_on);
+    else if (model == M_POTTS) k_reset_reference<M_POTTS><<<grid, 256, 0, s>>>(lat, tracking_on);
     else k_reset_reference<M_ISING_HALF><<<grid, 256, 0, s>>>(lat, tracking_on);
     return cudaGetLastError();
 }
@@ -404,8 +529,9 @@ __global__ void __launch_bounds__(256) k_get_spins(Lat lat, int model, int8_t *_
         canon_to_split(lat, i, c);
         uint32_t b = (c ? lat.col[1] : lat.col[0])[i >> 1];
         int v;
-        if (model == M_ISING_HALF) v = 2 * (int)(b & 1u) - 1;
+        if (model == M_ISING_HALF || model == M_EA) v = 2 * (int)(b & 1u) - 1;
         else if (model == M_ISING_ONE) v = (int)(b & 3u) - 1;
+        else if (model == M_POTTS) v = (int)(b & 7u);
         else v = (int)(b & 1u);
         out[i] = (int8_t)v;
     }
@@ -419,7 +545,8 @@ __global__ void __launch_bounds__(256) k_set_spins(Lat lat, int model, const int
         canon_to_split(lat, i, c);
         int s = in[i];
         uint32_t v, mask;
-        if (model == M_ISING_HALF) { v = s > 0 ? 1u : 0u; mask = 1u; }
+        if (model == M_ISING_HALF || model == M_EA) { v = s > 0 ? 1u : 0u; mask = 1u; }
+        else if (model == M_POTTS) { v = (uint32_t)(s < 0 ? 0 : (s >= lat.q ? lat.q - 1 : s)); mask = 7u; }
         else if (model == M_ISING_ONE) { v = (uint32_t)((s < -1 ? -1 : (s > 1 ? 1 : s)) + 1); mask = 3u; }
         else { v = s != 0 ? 1u : 0u; mask = 1u; }
         uint8_t *p = &(c ? lat.col[1] : lat.col[0])[i >> 1];
@@ -507,7 +634,8 @@ __global__ void __launch_bounds__(256) k_get_spins_words(Lat lat, int model, int
 
 cudaError_t launch_get_spins(const Lat &lat, int model, int8_t *d_out, cudaStream_t s)
 {
-    if (lat.Lh % 16 == 0 && ((uintptr_t)d_out & 15) == 0)
+    if (model == M_EA) model = M_ISING_HALF;          // same byte encoding of the value
+    if (model != M_POTTS && lat.Lh % 16 == 0 && ((uintptr_t)d_out & 15) == 0)
         k_get_spins_words<<<grid_for(lat.half >> 4, 256, 8), 256, 0, s>>>(lat, model, d_out);
     else
         k_get_spins<<<grid_for(2 * lat.half, 256, 8), 256, 0, s>>>(lat, model, d_out);
@@ -515,10 +643,93 @@ cudaError_t launch_get_spins(const Lat &lat, int model, int8_t *d_out, cudaStrea
 }
 cudaError_t launch_set_spins(const Lat &lat, int model, const int8_t *d_in, cudaStream_t s)
 {
-    if (lat.Lh % 16 == 0 && ((uintptr_t)d_in & 15) == 0)
+    if (model == M_EA) model = M_ISING_HALF;
+    if (model != M_POTTS && lat.Lh % 16 == 0 && ((uintptr_t)d_in & 15) == 0)
         k_set_spins_words<<<grid_for(lat.half >> 4, 256, 8), 256, 0, s>>>(lat, model, d_in);
     else
         k_set_spins<<<grid_for(2 * lat.half, 256, 8), 256, 0, s>>>(lat, model, d_in);
+    return cudaGetLastError();
+}
+
+// ------------------------------------------------------------------------------------------
+// Edwards-Anderson bonds (reading D25).  Canonical form: int8 tau[a][i] = sign of the bond between site i and its
+// neighbour in direction +a.  Device form: one byte per site, bit k = the bond to neighbour k is antiferromagnetic
+// (k = 2a: towards -a, stored canonically at the neighbour; k = 2a + 1: towards +a, stored at the site itself).
+// ------------------------------------------------------------------------------------------
+__device__ __forceinline__ void site_coords(const Lat &lat, long long i, int &x, int &y, int &z)
+{
+    long long ry = i / lat.L;
+    x = (int)(i - ry * lat.L);
+    z = (int)(ry / lat.L);
+    y = (int)(ry - (long long)z * lat.L);
+}
+// canonical id of the neighbour of (x, y, z) one step back along axis a
+__device__ __forceinline__ long long back_neighbour(const Lat &lat, int x, int y, int z, int a)
+{
+    const int L = lat.L;
+    if (a == 0) x = x == 0 ? L - 1 : x - 1;
+    else if (a == 1) y = y == 0 ? L - 1 : y - 1;
+    else z = z == 0 ? L - 1 : z - 1;
+    return x + (long long)L * (y + (long long)L * z);
+}
+
+// tau from the seed: stream tag 3, t = 0, bond id b = a*N + i, group b>>2, word b&3, tau = +1 iff the top bit is set.
+__global__ void __launch_bounds__(256) k_ea_bonds_init(Lat lat, SweepKey key)
+{
+    const long long N = 2 * lat.half;
+    for (long long i = (long long)blockIdx.x * blockDim.x + threadIdx.x; i < N; i += (long long)gridDim.x * blockDim.x) {
+        int x, y, z;
+        site_coords(lat, i, x, y, z);
+        uint32_t bits = 0;
+        for (int a = 0; a < lat.dims; ++a) {
+            const long long bf = (long long)a * N + i, bb = (long long)a * N + back_neighbour(lat, x, y, z, a);
+            const uint4 rf = philox4x32_10((uint32_t)(bf >> 2), (uint32_t)(bf >> 34), key.c2, key.c3, key.k0, key.k1);
+            const uint4 rb = philox4x32_10((uint32_t)(bb >> 2), (uint32_t)(bb >> 34), key.c2, key.c3, key.k0, key.k1);
+            const uint32_t wf = (bf & 2) ? ((bf & 1) ? rf.w : rf.z) : ((bf & 1) ? rf.y : rf.x);
+            const uint32_t wb = (bb & 2) ? ((bb & 1) ? rb.w : rb.z) : ((bb & 1) ? rb.y : rb.x);
+            if (!(wf >> 31)) bits |= 1u << (2 * a + 1);          // antiferromagnetic bond towards +a
+            if (!(wb >> 31)) bits |= 1u << (2 * a);              // ... towards -a
+        }
+        (((x + y + z) & 1) ? lat.bnd[1] : lat.bnd[0])[i >> 1] = (uint8_t)bits;
+    }
+}
+__global__ void __launch_bounds__(256) k_ea_set_bonds(Lat lat, const int8_t *__restrict__ tau)
+{
+    const long long N = 2 * lat.half;
+    for (long long i = (long long)blockIdx.x * blockDim.x + threadIdx.x; i < N; i += (long long)gridDim.x * blockDim.x) {
+        int x, y, z;
+        site_coords(lat, i, x, y, z);
+        uint32_t bits = 0;
+        for (int a = 0; a < lat.dims; ++a) {
+            if (tau[(long long)a * N + i] < 0) bits |= 1u << (2 * a + 1);
+            if (tau[(long long)a * N + back_neighbour(lat, x, y, z, a)] < 0) bits |= 1u << (2 * a);
+        }
+        (((x + y + z) & 1) ? lat.bnd[1] : lat.bnd[0])[i >> 1] = (uint8_t)bits;
+    }
+}
+__global__ void __launch_bounds__(256) k_ea_get_bonds(Lat lat, int8_t *__restrict__ tau)
+{
+    const long long N = 2 * lat.half;
+    for (long long i = (long long)blockIdx.x * blockDim.x + threadIdx.x; i < N; i += (long long)gridDim.x * blockDim.x) {
+        int x, y, z;
+        site_coords(lat, i, x, y, z);
+        const uint32_t bits = (((x + y + z) & 1) ? lat.bnd[1] : lat.bnd[0])[i >> 1];
+        for (int a = 0; a < lat.dims; ++a) tau[(long long)a * N + i] = (bits >> (2 * a + 1)) & 1u ? -1 : 1;
+    }
+}
+cudaError_t launch_ea_bonds_init(const Lat &lat, unsigned long long seed, cudaStream_t s)
+{
+    k_ea_bonds_init<<<grid_for(2 * lat.half, 256, 8), 256, 0, s>>>(lat, make_sweep_key(seed, 0ull, 3u));
+    return cudaGetLastError();
+}
+cudaError_t launch_ea_set_bonds(const Lat &lat, const int8_t *d_tau, cudaStream_t s)
+{
+    k_ea_set_bonds<<<grid_for(2 * lat.half, 256, 8), 256, 0, s>>>(lat, d_tau);
+    return cudaGetLastError();
+}
+cudaError_t launch_ea_get_bonds(const Lat &lat, int8_t *d_tau, cudaStream_t s)
+{
+    k_ea_get_bonds<<<grid_for(2 * lat.half, 256, 8), 256, 0, s>>>(lat, d_tau);
     return cudaGetLastError();
 }
 

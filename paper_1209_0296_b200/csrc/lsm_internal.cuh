@@ -14,7 +14,11 @@ namespace lsmk {
 // Flag bits of spin-1/2 sit at 8/16 so that even six flagged neighbours sum without a carry into
 // the next byte (6*25 = 150 < 256) and one AND with 0x07 recovers the neighbour count.
 // ------------------------------------------------------------------------------------------
-enum Model : int { M_ISING_HALF = 0, M_ISING_ONE = 1, M_NE_HEATBATH = 2, M_NE_METROPOLIS = 3 };
+//   EA (+/-J bonds) : as spin-1/2; the bond signs live in two more colour arrays (Lat::bnd), one byte per site:
+//                     bit k set = the bond to neighbour k is antiferromagnetic, k = 0: x-1, 1: x+1, 2: y-1, 3: y+1,
+//                     4: z-1, 5: z+1 (each bond is stored at both of its ends)
+//   Potts (q <= 8)  : bits[2:0] = state, bit3 = "ever changed", bits[6:4] = reference state
+enum Model : int { M_ISING_HALF = 0, M_ISING_ONE = 1, M_NE_HEATBATH = 2, M_NE_METROPOLIS = 3, M_EA = 4, M_POTTS = 5 };
 
 template <int MODEL> struct Enc {
     static constexpr uint32_t VAL = 0x01, CHG = 0x08, REF = 0x10;
@@ -24,6 +28,10 @@ template <> struct Enc<M_ISING_ONE> {
     static constexpr uint32_t VAL = 0x03, CHG = 0x10, REF = 0x60;
     static constexpr int REF_SHIFT = 5;
 };
+template <> struct Enc<M_POTTS> {
+    static constexpr uint32_t VAL = 0x07, CHG = 0x08, REF = 0x70;
+    static constexpr int REF_SHIFT = 4;
+};
 
 // Lattice view handed to every kernel by value.
 struct Lat {
@@ -31,6 +39,8 @@ struct Lat {
     int L, Lh, dims;     // Lh = L/2 bytes per compact row
     int Lz;              // L for 3D, 1 for 2D
     long long half;      // N/2
+    uint8_t *bnd[2];     // M_EA: bond bytes of the two colours (same geometry as col); else nullptr
+    int q;               // M_POTTS: number of states; else 0
 };
 
 // 33-bit thresholds in the canonical order of lsm_get_thresholds (include/lsm.h).
@@ -156,6 +166,10 @@ cudaError_t launch_persistence(const Lat &lat, int model, long long *d_out2, cud
 cudaError_t launch_reset_reference(const Lat &lat, int model, int tracking_on, cudaStream_t s);
 cudaError_t launch_get_spins(const Lat &lat, int model, int8_t *d_out, cudaStream_t s);
 cudaError_t launch_set_spins(const Lat &lat, int model, const int8_t *d_in, cudaStream_t s);
+// Edwards-Anderson bonds (reading D25; lsm_wider.cu): canonical int8 tau[dims][N] <-> the per-site bond bytes.
+cudaError_t launch_ea_bonds_init(const Lat &lat, unsigned long long seed, cudaStream_t s);
+cudaError_t launch_ea_set_bonds(const Lat &lat, const int8_t *d_tau, cudaStream_t s);
+cudaError_t launch_ea_get_bonds(const Lat &lat, int8_t *d_tau, cudaStream_t s);
 cudaError_t launch_philox_device(const uint32_t *d_ck, uint32_t *d_out, long long n, cudaStream_t s);
 cudaError_t launch_philox_throughput(int blocks, int calls, uint32_t *d_sink, cudaStream_t s);
 

@@ -392,6 +392,7 @@ static int small_max_sites() { return LSM_SMALL_MAX_SITES; }
 bool small_plan(const Lat &lat, int model, const TiledTables &t, SmallPlan *out, bool ignore_size_limit)
 {
     if (!t.usable) return false;
+    if (model == M_EA || model == M_POTTS) return false;   // NEXT-4 models: no small-family kernels
     const bool pow2 = lat.L >= 8 && (lat.L & (lat.L - 1)) == 0;       // lane-granular kernel: whole 32-bit lanes per row
     const bool words = tiled_supported(lat, model, t);                // word-granular kernel: whole 16-byte words per row
     if (!pow2 && !words) return false;

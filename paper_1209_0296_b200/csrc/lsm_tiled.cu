@@ -49,7 +49,7 @@ k_sweep_tiled(const __grid_constant__ TiledGeom g, const __grid_constant__ Philo
     // two-stage per-thread ring of the asynchronous copies (March::step_pf): N, O [, Yp, Yn] words and the edge lane
     // (spin-1 keeps the direct loads: its rule needs the registers the copies' addresses would take)
     constexpr bool PF = LSM_TILED_PF_ONE || MODEL != M_ISING_ONE;
-    __shared__ __align__(16) uint4 ring[PF ? (DIMS == 3 ? 8 : 4) * 256 : 1];
+    __shared__ __align__(16) uint4 ring[PF ? ((DIMS == 3 ? 8 : 4) + (MODEL == M_EA ? 2 : 0)) * 256 : 1];
     __shared__ uint32_t ringE[PF ? 2 * 256 : 1];
     // Programmatic dependent launch: the next half-sweep's CTAs may be scheduled as soon as SM resources
     // free up; they run their prologue (table, geometry) and then wait below until this grid has
@@ -62,7 +62,7 @@ k_sweep_tiled(const __grid_constant__ TiledGeom g, const __grid_constant__ Philo
     M.ne_t32 = 0;
     M.ne_always = 0;
     M.ne_all4 = false;
-    if constexpr (MODEL == M_ISING_HALF) {
+    if constexpr (MODEL == M_ISING_HALF || MODEL == M_EA) {
         if (threadIdx.x < 16) sm.t[threadIdx.x] = tab.t[threadIdx.x];
     } else if constexpr (MODEL == M_ISING_ONE) {
         if (threadIdx.x < 64) sm.t[threadIdx.x] = tab.t[threadIdx.x];
@@ -112,7 +112,9 @@ void build_tiled_tables(int model, int dims, double J, double h, const uint64_t 
     auto clip = [&](uint64_t v) { return v >= ALWAYS ? 0xFFFFFFFFu : (uint32_t)v; };
     const int d = dims;
     (void)J; (void)h; (void)nthr;
-    if (model == M_ISING_HALF) {
+    if (model == M_POTTS) {
+        t.usable = 0;                                       // scalar family only
+    } else if (model == M_ISING_HALF || model == M_EA) {
         t.usable = 1;
         for (int b = 0; b < 2; ++b)
             for (int n = 0; n <= 2 * d; ++n) {
@@ -151,6 +153,7 @@ void build_tiled_tables(int model, int dims, double J, double h, const uint64_t 
 bool tiled_supported(const Lat &lat, int model, const TiledTables &t)
 {
     if (!t.usable) return false;
+    if (model == M_POTTS) return false;                    // scalar family only
     if (lat.Lh % 16 != 0) return false;                    // whole 16-byte words per compact row
     if (lat.half / 4 > 0xFFFFFFFFll) return false;         // Philox group must fit c0 (c1 = 0 is hoisted)
     if (model == M_ISING_ONE && lat.half / 2 > 0xFFFFFFFFll) return false;
@@ -212,6 +215,7 @@ cudaError_t launch_sweep_tiled(const SweepArgs &a, const TiledTables &t, cudaStr
     g.half = a.half;
     g.obs = a.obs;
     g.one = 1;
+    g.bnd = a.model == M_EA ? (a.half ? a.lat.bnd[1] : a.lat.bnd[0]) : nullptr;
     // q = (march + y + colour) & 1 is warp-uniform if a warp sees one row parity only
     if (g.R == 1) g.parity_rows = 1;                                   // 2D: y = 0 for every thread
     else if (g.wpr % 32 == 0) g.parity_rows = 1;
@@ -236,6 +240,12 @@ cudaError_t launch_sweep_tiled(const SweepArgs &a, const TiledTables &t, cudaStr
         for (int i = 0; i < 16; ++i) ht.t[i] = t.t32[i];
         return d3 ? launch_track<M_ISING_HALF, 3>(track, obs_mode, grid, s, g, pc, ht)
                   : launch_track<M_ISING_HALF, 2>(track, obs_mode, grid, s, g, pc, ht);
+    }
+    case M_EA: {
+        HalfTab ht;
+        for (int i = 0; i < 16; ++i) ht.t[i] = t.t32[i];
+        return d3 ? launch_track<M_EA, 3>(track, obs_mode, grid, s, g, pc, ht)
+                  : launch_track<M_EA, 2>(track, obs_mode, grid, s, g, pc, ht);
     }
     case M_ISING_ONE: {
         OneTab ot;

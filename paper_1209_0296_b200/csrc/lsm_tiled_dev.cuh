@@ -26,7 +26,8 @@ namespace lsmk {
 
 constexpr int tiled_minblocks(int model)
 {
-    return model == M_ISING_ONE ? LSM_TILED_MINBLOCKS_ONE : model == M_ISING_HALF ? LSM_TILED_MINBLOCKS_HALF : LSM_TILED_MINBLOCKS;
+    return model == M_ISING_ONE ? LSM_TILED_MINBLOCKS_ONE
+         : (model == M_ISING_HALF || model == M_EA) ? LSM_TILED_MINBLOCKS_HALF : LSM_TILED_MINBLOCKS;
 }
 
 // ------------------------------------------------------------------------------------------
@@ -121,6 +122,7 @@ struct TiledGeom {
     int parity_rows;       // 1: a warp's cross rows all have the same parity (see column_of)
     int one;               // the constant 1, kept opaque to the compiler (see rule_half)
     long long *obs;        // (B, M) accumulator or nullptr
+    const uint8_t *bnd;    // M_EA: bond bytes of the colour being updated (same geometry as own); else nullptr
 };
 
 struct HalfTab { uint32_t t[16]; };            // spin-1/2: t[n + 8*b] = thr - 1  (accept iff w <= t)
@@ -129,6 +131,7 @@ struct OneTab { uint32_t t[64]; };            // spin-1: t[16*dcode + sum] = thr
 template <int MODEL> struct TabOf { using type = NeTab; };
 template <> struct TabOf<M_ISING_HALF> { using type = HalfTab; };
 template <> struct TabOf<M_ISING_ONE> { using type = OneTab; };
+template <> struct TabOf<M_EA> { using type = HalfTab; };     // reading D25: the Ising table on the bond-weighted up-count
 
 __device__ __forceinline__ uint32_t bytesum(uint32_t v) { return __dp4a(v, 0x01010101u, 0u); }
 
@@ -305,7 +308,7 @@ struct March {
     // next row (N), the own word (O), the edge lane of the adjacent word (e) and, in 3D, the cross rows.
     template <int Q, bool UP, class PC>
     __device__ __forceinline__ uint4 update_word(const PC &pc, const uint4 N, const uint4 O, const uint32_t e,
-                                                 const uint4 Yp, const uint4 Yn)
+                                                 const uint4 Yp, const uint4 Yn, const uint4 BW = make_uint4(0, 0, 0, 0))
     {
         const int qq = Q == 2 ? q : Q;
         // the neighbour one byte to the right (q = 1) or left (q = 0) of every site of the word
@@ -339,6 +342,27 @@ struct March {
                 if (DIMS == 3) ns += yp[d] + yn[d];
                 uint4 r = philox_sweep(grp + d, pc);
                 out[d] = rule_half<TRACK, OBS>(o[d], ns, r, s_t, one, totU, totBN);
+            }
+        } else if (MODEL == M_EA) {
+            // Reading D25: an antiferromagnetic bond turns the neighbour's "up" into "down", so the up-count is
+            // sum_k (b_k xor bond bit k), k = 0: x-1, 1: x+1, 2: y-1, 3: y+1, 4: z-1, 5: z+1 (bond byte of the site
+            // being updated).  In the own row the word C holds x+1 (q = 0) or x-1 (q = 1), the shifted word sd the
+            // other one; the march axis is y in 2D and z in 3D.  (a ^ b) & 0x01 also drops the flag bits.
+            const uint32_t bw[4] = {BW.x, BW.y, BW.z, BW.w};
+#pragma unroll
+            for (int d = 0; d < 4; ++d) {
+                const uint32_t xm = qq ? c[d] : sd[d], xp = qq ? sd[d] : c[d];
+                const uint32_t m1 = 0x01010101u;
+                uint32_t ns = lop3<0x28>(xm, bw[d], m1) + lop3<0x28>(xp, bw[d] >> 1, m1);
+                if (DIMS == 3) {
+                    ns += lop3<0x28>(yp[d], bw[d] >> 2, m1) + lop3<0x28>(yn[d], bw[d] >> 3, m1);
+                    ns += lop3<0x28>(p[d], bw[d] >> 4, m1) + lop3<0x28>(n[d], bw[d] >> 5, m1);
+                } else {
+                    ns += lop3<0x28>(p[d], bw[d] >> 2, m1) + lop3<0x28>(n[d], bw[d] >> 3, m1);
+                }
+                uint4 r = philox_sweep(grp + d, pc);
+                out[d] = rule_half<TRACK, OBS>(o[d], ns, r, s_t, one, totU, totBN);
+                if (OBS >= 2) totS = (int)__dp4a(ns, m1, (uint32_t)totS);
             }
         } else if (MODEL == M_ISING_ONE) {
 #pragma unroll
@@ -419,7 +443,12 @@ struct March {
             Yp = pC[dyp];
             Yn = pC[dyn];
         }
-        *pO = update_word<Q, UP>(pc, N, O, e, Yp, Yn);
+        uint4 BW = make_uint4(0, 0, 0, 0);
+        if (MODEL == M_EA) {
+            BW = *pB;
+            pB += rowstride;
+        }
+        *pO = update_word<Q, UP>(pc, N, O, e, Yp, Yn, BW);
         P = C;
         C = N;
         pC += rowstride;
@@ -438,6 +467,8 @@ struct March {
     // into the colour arrays (one IMAD.WIDE per address) instead of 64-bit pointer arithmetic.
     const uint8_t *b_oth;   // array bases
     uint8_t *b_own;
+    const uint8_t *b_bnd;   // M_EA: bond bytes of the own colour
+    const uint4 *pB;        // ... word of the current step (direct-load path)
     uint32_t offN;          // word offset of the other colour's row the NEXT step will use as N... see step_pf
     uint32_t offS;          // word offset of the own word of the current step
     uint32_t nw32;          // words per colour array
@@ -450,6 +481,7 @@ struct March {
     static constexpr uint32_t RING_STAGE = 256u * 16u;              // bytes per stage of a 16-byte ring
     static constexpr uint32_t RING_O = 2u * RING_STAGE;             // own-colour ring behind the N ring
     static constexpr uint32_t RING_YP = 4u * RING_STAGE, RING_YN = 6u * RING_STAGE;
+    static constexpr uint32_t RING_BW = (DIMS == 3 ? 8u : 4u) * RING_STAGE;      // M_EA: bond words behind the others
     static constexpr uint32_t RINGE_STAGE = 256u * 4u;
 
     __device__ __forceinline__ static void cp16(uint32_t dst, const void *src)
@@ -487,6 +519,7 @@ struct March {
             cp16(s_ring + RING_YP + ST * RING_STAGE, aC + dypb);
             cp16(s_ring + RING_YN + ST * RING_STAGE, aC + dynb);
         }
+        if (MODEL == M_EA) cp16(s_ring + RING_BW + ST * RING_STAGE, b_bnd + (size_t)cur * 16u);
         asm volatile("cp.async.commit_group;" ::: "memory");
     }
 
@@ -514,7 +547,9 @@ struct March {
             Yp = lds128(s_ring + RING_YP + ST * RING_STAGE);
             Yn = lds128(s_ring + RING_YN + ST * RING_STAGE);
         }
-        const uint4 out = update_word<Q, UP>(pc, N, O, e, Yp, Yn);
+        uint4 BW = make_uint4(0, 0, 0, 0);
+        if (MODEL == M_EA) BW = lds128(s_ring + RING_BW + ST * RING_STAGE);
+        const uint4 out = update_word<Q, UP>(pc, N, O, e, Yp, Yn, BW);
         *reinterpret_cast<uint4 *>(b_own + (size_t)offS * 16u) = out;
         P = C;
         C = N;
@@ -626,6 +661,8 @@ __device__ __forceinline__ int march_init(March<MODEL, DIMS, TRACK, OBS> &M, con
     M.grp = (uint32_t)w0 * 4u;
     M.b_oth = oth;
     M.b_own = own;
+    M.b_bnd = g.bnd;
+    M.pB = reinterpret_cast<const uint4 *>(g.bnd) + w0;
     M.offS = (uint32_t)w0;
     M.offN = (uint32_t)w0;
     M.nw32 = (uint32_t)nw;
@@ -661,6 +698,11 @@ __device__ __forceinline__ void march_observables(const March<MODEL, DIMS, TRACK
         cM = 2LL * M.totU - nsites;
         cB = -4LL * DIMS * M.totU;
         if (second) cB += 4LL * M.totBN + 2LL * DIMS * nsites;
+    } else if (MODEL == M_EA) {
+        // s' = 2b' - 1, nn_eff = 2n - 2d with n the bond-weighted up-count: the sum of n over a colour is no longer
+        // 2d * (ups of the other colour), so it is accumulated (totS):  B = 4 sum b'n - 2 sum n - 4d U + 2d nsites
+        cM = 2LL * M.totU - nsites;
+        if (second) cB = 4LL * M.totBN - 2LL * M.totS - 4LL * DIMS * M.totU + 2LL * DIMS * nsites;
     } else if (MODEL == M_ISING_ONE) {
         // s' = a' - 1, nn = sum - 2d:  M = SA - n;  B = sum s' nn = SAS - 2d SA - SS + 2d n   (second colour only)
         cM = (long long)M.totU - nsites;

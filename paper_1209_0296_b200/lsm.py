@@ -14,7 +14,7 @@ import numpy as np
 _PKG = os.path.dirname(os.path.abspath(__file__))
 _LIB_PATH = os.path.join(_PKG, "liblsm.so")
 
-ISING, NE_HEATBATH, NE_METROPOLIS = 0, 1, 2
+ISING, NE_HEATBATH, NE_METROPOLIS, EA, POTTS = 0, 1, 2, 3, 4
 KERNEL_AUTO, KERNEL_GENERIC, KERNEL_TILED, KERNEL_RESIDENT, KERNEL_SMALL = 0, 1, 2, 3, 4
 OK, ERR_ARG, ERR_UNSUPPORTED, ERR_CUDA, ERR_WORKSPACE, ERR_STATE = 0, -1, -2, -3, -4, -5
 
@@ -53,6 +53,8 @@ SIGNATURES = {
     "lsm_get_spins_host": (_i32, [_vp, _vp, _vp, _vp]),
     "lsm_set_spins": (_i32, [_vp, _vp, _u64, _vp]),
     "lsm_set_spins_host": (_i32, [_vp, _vp, _vp, _u64, _vp]),
+    "lsm_set_bonds": (_i32, [_vp, _vp, _vp]),
+    "lsm_get_bonds": (_i32, [_vp, _vp, _vp]),
     "lsm_set_temperature": (_i32, [_vp, _dbl]),
     "lsm_get_thresholds": (_i32, [_vp, _P(_u64), _P(_i32)]),
     "lsm_set_kernel": (_i32, [_vp, _i32]),
@@ -313,6 +315,22 @@ class Lattice:
         sc = self._dev_scratch(self.N)
         _check(self._lib.lsm_set_spins_host(self._h, _vp(ptr), _vp(sc.data_ptr()), int(sweep_counter),
                                             self._sp(stream)), "lsm_set_spins_host")
+
+    @_on_device
+    def set_bonds(self, d_tau, stream=None):
+        """EA model: device int8 [dims, N], +1 / -1 per bond (site i, direction +a)."""
+        import torch
+
+        assert d_tau.is_cuda and d_tau.dtype == torch.int8 and d_tau.numel() == self.dims * self.N and d_tau.is_contiguous()
+        _check(self._lib.lsm_set_bonds(self._h, _vp(d_tau.data_ptr()), self._sp(stream)), "lsm_set_bonds")
+
+    @_on_device
+    def get_bonds(self, stream=None):
+        import torch
+
+        out = torch.empty((self.dims, self.N), dtype=torch.int8, device=self.device)
+        _check(self._lib.lsm_get_bonds(self._h, _vp(out.data_ptr()), self._sp(stream)), "lsm_get_bonds")
+        return out
 
     @_on_device
     def set_temperature(self, T):
