@@ -14,6 +14,7 @@
 #include <cooperative_groups.h>
 #include <cstdlib>
 #include <cstring>
+#include <type_traits>
 
 namespace lsmk {
 
@@ -110,7 +111,32 @@ k_sweep_small(const __grid_constant__ SmallArgs a, const __grid_constant__ Philo
 // threshold table: lsm_batch_sweep).  `sm_t` is the block's threshold table in shared memory (filled by the
 // caller), `acc` its (B, M) scratch.  self_zero: the cluster zeroes its own obs / run slots (batch launches have no
 // host memset per replica); run: where the sums of the LAST sweep are added as well (the replica's running pair).
-template <int MODEL, int DIMS, bool TRACK, int OBS>
+__device__ __forceinline__ uint32_t lds_w(uint32_t a)
+{
+    uint32_t v;
+    asm volatile("ld.shared.u32 %0, [%1];" : "=r"(v) : "r"(a) : "memory");
+    return v;
+}
+__device__ __forceinline__ void sts_w(uint32_t a, uint32_t v) { asm volatile("st.shared.u32 [%0], %1;" ::"r"(a), "r"(v) : "memory"); }
+// word of this or another block of the cluster (distributed shared memory)
+__device__ __forceinline__ uint32_t ldc_w(uint32_t a)
+{
+    uint32_t v;
+    asm volatile("ld.shared::cluster.u32 %0, [%1];" : "=r"(v) : "r"(a) : "memory");
+    return v;
+}
+__device__ __forceinline__ uint32_t mapa_u32(uint32_t a, uint32_t rank)
+{
+    uint32_t r;
+    asm volatile("mapa.shared::cluster.u32 %0, %1, %2;" : "=r"(r) : "r"(a), "r"(rank));
+    return r;
+}
+
+// LPT > 0: the block has exactly LPT lanes per thread and the geometry of a thread's lanes (which words hold its 2d
+// neighbours, in this block's shared memory or in a neighbour block's) is computed ONCE, before the sweep loop: a
+// half-sweep of a small lattice is a dependent chain per thread, and the index arithmetic was a third of it.
+// LPT = 0: any number of lanes per thread, geometry recomputed in every half-sweep.
+template <int MODEL, int DIMS, bool TRACK, int OBS, int LPT = 0>
 __device__ __forceinline__ void small_lane_body(uint8_t *const col0, uint8_t *const col1, const PhiloxSweepConsts &pk,
                                                 const unsigned long long seed, const unsigned long long t0,
                                                 const int nsweeps, long long *const obs, long long *const run,
@@ -150,6 +176,31 @@ __device__ __forceinline__ void small_lane_body(uint8_t *const col0, uint8_t *co
     if (nrank > 1) cluster.sync();
     else __syncthreads();
 
+    // hoisted geometry (LPT > 0): shared-window addresses of the colour-0 words; colour 1 lies colB bytes behind
+    constexpr int NL = LPT > 0 ? LPT : 1;
+    const uint32_t colB = nl * 4u;
+    uint32_t a_own[NL], a_p[NL], a_n[NL], a_cs1[NL], a_cs0[NL], a_yp[NL], a_yn[NL], g_q0[NL], g_gl[NL];
+    if (LPT > 0) {
+        const uint32_t s0 = (uint32_t)__cvta_generic_to_shared(s_lat);
+#pragma unroll
+        for (int l = 0; l < NL; ++l) {
+            const uint32_t li = threadIdx.x + (uint32_t)l * blockDim.x;
+            const uint32_t x = li & (lpr - 1), row = li >> lg_lpr;
+            const uint32_t y = row & (R - 1), ml = row >> lg_R;
+            const uint32_t m = (rank << lg_rpc) + ml;
+            g_q0[l] = (m + y) & 1u;                                          // row parity bit of half 0
+            g_gl[l] = base + li;
+            a_own[l] = s0 + li * 4u;
+            const uint32_t up_off = (rpc - 1) << (lg_R + lg_lpr);            // lanes between the first and the last row of a slab
+            a_p[l] = ml > 0 ? mapa_u32(s0 + (li - (R << lg_lpr)) * 4u, rank) : mapa_u32(s0 + (li + up_off) * 4u, r_dn);
+            a_n[l] = ml + 1 < rpc ? mapa_u32(s0 + (li + (R << lg_lpr)) * 4u, rank) : mapa_u32(s0 + (li - up_off) * 4u, r_up);
+            a_cs1[l] = s0 + ((row << lg_lpr) + ((x + 1) & (lpr - 1))) * 4u;  // q = 1: the word to the right
+            a_cs0[l] = s0 + ((row << lg_lpr) + ((x - 1) & (lpr - 1))) * 4u;  // q = 0: the word to the left
+            a_yp[l] = s0 + (((ml << lg_R) + ((y - 1) & (R - 1))) * lpr + x) * 4u;
+            a_yn[l] = s0 + (((ml << lg_R) + ((y + 1) & (R - 1))) * lpr + x) * 4u;
+        }
+    }
+
     int thrB = 0, thrM = 0;
     const int nhalves = 2 * nsweeps;
 #pragma unroll 1
@@ -162,6 +213,46 @@ __device__ __forceinline__ void small_lane_body(uint8_t *const col0, uint8_t *co
         const uint32_t *oth = s_col[half ^ 1];
         int totU = 0, totBN = 0, totS = 0, nsites = 0;
         if (half == 0) thrB = thrM = 0;
+        if (LPT > 0) {
+            const uint32_t ownB = half ? colB : 0u, othB = half ? 0u : colB;
+#pragma unroll
+            for (int l = 0; l < NL; ++l) {
+                const uint32_t qq = g_q0[l] ^ (uint32_t)half;
+                const uint32_t c = lds_w(a_own[l] + othB), o = lds_w(a_own[l] + ownB);
+                const uint32_t p = ldc_w(a_p[l] + othB), n = ldc_w(a_n[l] + othB);
+                const uint32_t cs = lds_w((qq ? a_cs1[l] : a_cs0[l]) + othB);
+                const uint32_t sd = qq ? __funnelshift_r(c, cs, 8) : __funnelshift_r(cs, c, 24);
+                uint32_t yp = 0, yn = 0;
+                if (DIMS == 3) {
+                    yp = lds_w(a_yp[l] + othB);
+                    yn = lds_w(a_yn[l] + othB);
+                }
+                const uint32_t gl = g_gl[l];
+                uint32_t out;
+                if (MODEL == M_ISING_HALF) {
+                    uint32_t ns = p + n + c + sd;
+                    if (DIMS == 3) ns += yp + yn;
+                    out = rule_half<TRACK, OBS>(o, ns, philox_sweep(gl, pc), s_t, one, totU, totBN);
+                } else if (MODEL == M_ISING_ONE) {
+                    uint32_t ns;
+                    if (TRACK) {
+                        ns = ((p + n) & 0x0F0F0F0Fu) + ((c + sd) & 0x0F0F0F0Fu);
+                        if (DIMS == 3) ns += (yp + yn) & 0x0F0F0F0Fu;
+                    } else {
+                        ns = p + n + c + sd;
+                        if (DIMS == 3) ns += yp + yn;
+                    }
+                    out = rule_one<DIMS, TRACK, OBS>(o, ns, philox_sweep(2u * gl, pc), philox_sweep(2u * gl + 1u, pc), s_t, one,
+                                                     totU, totBN, totS);
+                } else {
+                    uint32_t accU = 0;
+                    out = rule_ne<TRACK, MODEL == M_NE_METROPOLIS, OBS>(o, n, qq ? sd : c, gl, pc, ne_t32, ne_always, accU);
+                    if (OBS >= 1) totU += (int)bytesum(accU);
+                }
+                sts_w(a_own[l] + ownB, out);
+                nsites += 4;
+            }
+        } else
 #pragma unroll 1
         for (uint32_t li = threadIdx.x; li < nl; li += blockDim.x) {
             const uint32_t gl = base + li;                                    // lane index in the colour array
@@ -247,7 +338,7 @@ __device__ __forceinline__ void small_lane_body(uint8_t *const col0, uint8_t *co
     if (nrank > 1) cluster.sync();      // no block may exit while a neighbour can still read its shared memory
 }
 
-template <int MODEL, int DIMS, bool TRACK, int OBS>
+template <int MODEL, int DIMS, bool TRACK, int OBS, int LPT>
 __global__ void __launch_bounds__(1024, 1)
 k_sweep_small_lane(const __grid_constant__ SmallArgs a, const __grid_constant__ PhiloxSweepConsts pk,
                    const __grid_constant__ typename TabOf<MODEL>::type tab, const int lg_lpr, const int lg_L,
@@ -270,7 +361,7 @@ k_sweep_small_lane(const __grid_constant__ SmallArgs a, const __grid_constant__ 
         ne_always = tab.always;
     }
     if (threadIdx.x < 4) sm.acc[threadIdx.x >> 1][threadIdx.x & 1] = 0;
-    small_lane_body<MODEL, DIMS, TRACK, OBS>(a.col[0], a.col[1], pk, a.seed, a.t0, a.nsweeps, a.obs, nullptr, false, ne_t32,
+    small_lane_body<MODEL, DIMS, TRACK, OBS, LPT>(a.col[0], a.col[1], pk, a.seed, a.t0, a.nsweeps, a.obs, nullptr, false, ne_t32,
                                              ne_always, (uint32_t)a.g.one, s_t, sm.acc, lg_lpr, lg_L, lg_rpc);
 }
 
@@ -290,7 +381,7 @@ struct SmallBatchArgs {
     uint2 seed[SMALL_BATCH_MAX]; // (k0, k1) of replica r0 + i
 };
 
-template <int MODEL, int DIMS, bool TRACK, int OBS>
+template <int MODEL, int DIMS, bool TRACK, int OBS, int LPT>
 __global__ void __launch_bounds__(1024, 1)
 k_sweep_small_lane_batch(const __grid_constant__ SmallBatchArgs a, const int lg_lpr, const int lg_L, const int lg_rpc,
                          const int lg_clu)
@@ -316,7 +407,7 @@ k_sweep_small_lane_batch(const __grid_constant__ SmallBatchArgs a, const int lg_
     pk.x1 = pk.y2 = pk.z2 = pk.w3 = 0u;
     const unsigned long long seed = ((unsigned long long)sd.y << 32) | sd.x;
     long long *obs = (OBS >= 1 && a.obs) ? a.obs + a.obs_stride * (a.r0 + ci) : nullptr;
-    small_lane_body<MODEL, DIMS, TRACK, OBS>(d.col[0], d.col[1], pk, seed, a.t0, a.nsweeps, obs,
+    small_lane_body<MODEL, DIMS, TRACK, OBS, LPT>(d.col[0], d.col[1], pk, seed, a.t0, a.nsweeps, obs,
                                              a.write_run ? d.run : nullptr, true, d.ne_t32, d.ne_always, (uint32_t)a.one,
                                              s_t, sm.acc, lg_lpr, lg_L, lg_rpc);
 }
@@ -365,8 +456,14 @@ static cudaError_t small_launch_to(bool track, bool obs, int threads, cudaStream
             cfg.numAttrs = 1;
             return cudaLaunchKernelEx(&cfg, kern, a, pk, tab, lg_lpr, lg_L, lg_rpc);
         };
-        if (track) return obs ? go(k_sweep_small_lane<MODEL, DIMS, true, 2>) : go(k_sweep_small_lane<MODEL, DIMS, true, 0>);
-        return obs ? go(k_sweep_small_lane<MODEL, DIMS, false, 2>) : go(k_sweep_small_lane<MODEL, DIMS, false, 0>);
+        // one lane per thread (every lattice up to 16 x 1024 lanes per colour): the hoisted-geometry body
+        const bool one = (((size_t)1 << (DIMS * lg_L)) / 8) / (size_t)nclu == (size_t)threads;
+        if (one) {
+            if (track) return obs ? go(k_sweep_small_lane<MODEL, DIMS, true, 2, 1>) : go(k_sweep_small_lane<MODEL, DIMS, true, 0, 1>);
+            return obs ? go(k_sweep_small_lane<MODEL, DIMS, false, 2, 1>) : go(k_sweep_small_lane<MODEL, DIMS, false, 0, 1>);
+        }
+        if (track) return obs ? go(k_sweep_small_lane<MODEL, DIMS, true, 2, 0>) : go(k_sweep_small_lane<MODEL, DIMS, true, 0, 0>);
+        return obs ? go(k_sweep_small_lane<MODEL, DIMS, false, 2, 0>) : go(k_sweep_small_lane<MODEL, DIMS, false, 0, 0>);
     }
     if (track) {
         if (obs) k_sweep_small<MODEL, DIMS, true, 2><<<1, threads, 0, s>>>(a, pk, tab);
@@ -393,6 +490,7 @@ bool small_plan(const Lat &lat, int model, const TiledTables &t, SmallPlan *out,
 {
     if (!t.usable) return false;
     if (model == M_EA || model == M_POTTS) return false;   // NEXT-4 models: no small-family kernels
+    if (t.has_never) return false;                         // two-compare kernels exist in the tiled family only
     const bool pow2 = lat.L >= 8 && (lat.L & (lat.L - 1)) == 0;       // lane-granular kernel: whole 32-bit lanes per row
     const bool words = tiled_supported(lat, model, t);                // word-granular kernel: whole 16-byte words per row
     if (!pow2 && !words) return false;
@@ -494,7 +592,7 @@ int small_batch_cluster(const Lat &lat, int R)
     int c = cmax;
     while (c > 1 && (long long)R * c > 2ll * sm_count()) c >>= 1;
     while (N / c > 196608 && c < 16) c <<= 1;          // the slab must fit shared memory
-    while (nlanes / c > 1024 * 8 && c < 16) c <<= 1;   // at most 8 lanes per thread and half-sweep
+    while (nlanes / c > 2048 && c < 16) c <<= 1;       // at most two lanes per thread: the hoisted-geometry body
     return c;
 }
 
@@ -528,8 +626,20 @@ static cudaError_t small_batch_launch_to(bool track, bool obs, int threads, cuda
         cfg.numAttrs = 1;
         return cudaLaunchKernelEx(&cfg, kern, a, lg_lpr, lg_L, lg_rpc, lg_clu);
     };
-    if (track) return obs ? go(k_sweep_small_lane_batch<MODEL, DIMS, true, 2>) : go(k_sweep_small_lane_batch<MODEL, DIMS, true, 0>);
-    return obs ? go(k_sweep_small_lane_batch<MODEL, DIMS, false, 2>) : go(k_sweep_small_lane_batch<MODEL, DIMS, false, 0>);
+    const size_t nl = (((size_t)1 << (DIMS * lg_L)) / 8) / (size_t)nclu;      // lanes per colour and block
+    const int lpt = nl == (size_t)threads ? 1 : nl == 2 * (size_t)threads ? 2 : 0;
+    auto pick = [&](auto T, auto O) -> cudaError_t {
+        constexpr bool TR = decltype(T)::value;
+        constexpr int OB = decltype(O)::value;
+        if (lpt == 1) return go(k_sweep_small_lane_batch<MODEL, DIMS, TR, OB, 1>);
+        if (lpt == 2) return go(k_sweep_small_lane_batch<MODEL, DIMS, TR, OB, 2>);
+        return go(k_sweep_small_lane_batch<MODEL, DIMS, TR, OB, 0>);
+    };
+    using std::integral_constant;
+    if (track) return obs ? pick(integral_constant<bool, true>{}, integral_constant<int, 2>{})
+                          : pick(integral_constant<bool, true>{}, integral_constant<int, 0>{});
+    return obs ? pick(integral_constant<bool, false>{}, integral_constant<int, 2>{})
+               : pick(integral_constant<bool, false>{}, integral_constant<int, 0>{});
 }
 
 // d_obs: slot of replica 0 for the first sweep of this launch (replica r at d_obs + r * obs_stride) or nullptr;

@@ -37,13 +37,13 @@ PhiloxSweepConsts make_philox_consts(const SweepKey &k)
     return c;
 }
 
-template <int MODEL, int DIMS, bool TRACK, int OBS>
+template <int MODEL, int DIMS, bool TRACK, int OBS, bool NEV>
 __global__ void __launch_bounds__(256, tiled_minblocks(MODEL))
 k_sweep_tiled(const __grid_constant__ TiledGeom g, const __grid_constant__ PhiloxSweepConsts pc,
-              const __grid_constant__ typename TabOf<MODEL>::type tab)
+              const __grid_constant__ typename TabOf<MODEL>::type tab, const __grid_constant__ NevTab ytab)
 {
     __shared__ __align__(16) struct {
-        uint32_t t[MODEL == M_ISING_ONE ? 64 : 16];
+        uint32_t t[(MODEL == M_ISING_ONE ? 64 : 16) * (NEV ? 2 : 1)];   // NEV: the y table behind the t table
         long long red[2][8];
     } sm;
     // two-stage per-thread ring of the asynchronous copies (March::step_pf): N, O [, Yp, Yn] words and the edge lane
@@ -58,14 +58,16 @@ k_sweep_tiled(const __grid_constant__ TiledGeom g, const __grid_constant__ Philo
     asm volatile("griddepcontrol.launch_dependents;" ::: "memory");
     uint32_t s_t = (uint32_t)__cvta_generic_to_shared(sm.t);
     asm volatile("" : "+r"(s_t));   // keep the (warp-uniform) table address out of the divergent region below
-    March<MODEL, DIMS, TRACK, OBS> M;
+    March<MODEL, DIMS, TRACK, OBS, NEV> M;
     M.ne_t32 = 0;
     M.ne_always = 0;
     M.ne_all4 = false;
     if constexpr (MODEL == M_ISING_HALF || MODEL == M_EA) {
         if (threadIdx.x < 16) sm.t[threadIdx.x] = tab.t[threadIdx.x];
+        if (NEV && threadIdx.x < 16) sm.t[16 + threadIdx.x] = ytab.y[threadIdx.x];
     } else if constexpr (MODEL == M_ISING_ONE) {
         if (threadIdx.x < 64) sm.t[threadIdx.x] = tab.t[threadIdx.x];
+        if (NEV && threadIdx.x < 64) sm.t[64 + threadIdx.x] = ytab.y[threadIdx.x];
     } else {
         M.ne_t32 = tab.t32;
         M.ne_always = tab.always;
@@ -96,7 +98,7 @@ k_sweep_tiled(const __grid_constant__ TiledGeom g, const __grid_constant__ Philo
 
     if (OBS >= 1) {
         long long cB, cM;
-        march_observables<MODEL, DIMS>(M, nsites, OBS >= 2, cB, cM);   // OBS = 1: first colour, 2: second colour
+        march_observables(M, nsites, OBS >= 2, cB, cM);   // OBS = 1: first colour, 2: second colour
         block_accumulate2_in(sm.red, cB, cM, g.obs, true, true);
     }
 }
@@ -119,8 +121,9 @@ void build_tiled_tables(int model, int dims, double J, double h, const uint64_t 
         for (int b = 0; b < 2; ++b)
             for (int n = 0; n <= 2 * d; ++n) {
                 uint64_t v = thr[b * (2 * d + 1) + n];
-                if (v == 0) t.usable = 0;                  // "never" cannot be written as w <= thr-1
-                t.t32[n + 8 * b] = (uint32_t)(v - 1);
+                if (v == 0) t.has_never = 1;               // "never" cannot be written as w <= thr-1: NEV kernels
+                t.t32[n + 8 * b] = v == 0 ? 0u : (uint32_t)(v - 1);
+                t.y32[n + 8 * b] = v == 0 ? 1u : 0u;
             }
     } else if (model == M_ISING_ONE) {
         t.usable = 1;
@@ -136,8 +139,9 @@ void build_tiled_tables(int model, int dims, double J, double h, const uint64_t 
         for (int c = 0; c < 4; ++c)
             for (int s = 0; s < W; ++s) {
                 uint64_t v = thr[(rep[c][0] * 2 + rep[c][1]) * W + s];
-                if (v == 0) t.usable = 0;                  // "never" cannot be written as w <= thr-1
-                t.s1[c * 16 + s] = (uint32_t)(v - 1);
+                if (v == 0) t.has_never = 1;
+                t.s1[c * 16 + s] = v == 0 ? 0u : (uint32_t)(v - 1);
+                t.y32[c * 16 + s] = v == 0 ? 1u : 0u;
             }
     } else {
         t.usable = 1;
@@ -176,9 +180,9 @@ static const int g_tiled_ctas_per_sm = LSM_TILED_CTAS_PER_SM;
 static const int g_tiled_waves_x4 = LSM_TILED_WAVES_X4;
 static const int g_tiled_pdl = LSM_TILED_PDL;
 
-template <int MODEL, int DIMS, bool TRACK>
+template <int MODEL, int DIMS, bool TRACK, bool NEV>
 static cudaError_t launch_obs(int obs_mode, dim3 grid, cudaStream_t s, const TiledGeom &g, const PhiloxSweepConsts &pc,
-                              const typename TabOf<MODEL>::type &tab)
+                              const typename TabOf<MODEL>::type &tab, const NevTab &yt)
 {
     cudaLaunchConfig_t cfg;
     memset(&cfg, 0, sizeof(cfg));
@@ -190,17 +194,28 @@ static cudaError_t launch_obs(int obs_mode, dim3 grid, cudaStream_t s, const Til
     at[0].val.programmaticStreamSerializationAllowed = g_tiled_pdl ? 1 : 0;
     cfg.attrs = at;
     cfg.numAttrs = 1;
-    if (obs_mode == 0) return cudaLaunchKernelEx(&cfg, k_sweep_tiled<MODEL, DIMS, TRACK, 0>, g, pc, tab);
-    if (obs_mode == 1) return cudaLaunchKernelEx(&cfg, k_sweep_tiled<MODEL, DIMS, TRACK, 1>, g, pc, tab);
-    return cudaLaunchKernelEx(&cfg, k_sweep_tiled<MODEL, DIMS, TRACK, 2>, g, pc, tab);
+    if (obs_mode == 0) return cudaLaunchKernelEx(&cfg, k_sweep_tiled<MODEL, DIMS, TRACK, 0, NEV>, g, pc, tab, yt);
+    if (obs_mode == 1) return cudaLaunchKernelEx(&cfg, k_sweep_tiled<MODEL, DIMS, TRACK, 1, NEV>, g, pc, tab, yt);
+    return cudaLaunchKernelEx(&cfg, k_sweep_tiled<MODEL, DIMS, TRACK, 2, NEV>, g, pc, tab, yt);
 }
 
 template <int MODEL, int DIMS>
 static cudaError_t launch_track(bool track, int obs_mode, dim3 grid, cudaStream_t s, const TiledGeom &g,
-                                const PhiloxSweepConsts &pc, const typename TabOf<MODEL>::type &tab)
+                                const PhiloxSweepConsts &pc, const typename TabOf<MODEL>::type &tab,
+                                const TiledTables *nev = nullptr)
 {
-    if (track) return launch_obs<MODEL, DIMS, true>(obs_mode, grid, s, g, pc, tab);
-    return launch_obs<MODEL, DIMS, false>(obs_mode, grid, s, g, pc, tab);
+    NevTab yt;
+    memset(&yt, 0, sizeof(yt));
+    constexpr bool CAN_NEV = MODEL == M_ISING_HALF || MODEL == M_ISING_ONE || MODEL == M_EA;
+    if constexpr (CAN_NEV) {
+        if (nev && nev->has_never) {                       // a table with a "never" entry: the two-compare kernels
+            for (int i = 0; i < 64; ++i) yt.y[i] = nev->y32[i];
+            if (track) return launch_obs<MODEL, DIMS, true, true>(obs_mode, grid, s, g, pc, tab, yt);
+            return launch_obs<MODEL, DIMS, false, true>(obs_mode, grid, s, g, pc, tab, yt);
+        }
+    }
+    if (track) return launch_obs<MODEL, DIMS, true, false>(obs_mode, grid, s, g, pc, tab, yt);
+    return launch_obs<MODEL, DIMS, false, false>(obs_mode, grid, s, g, pc, tab, yt);
 }
 
 cudaError_t launch_sweep_tiled(const SweepArgs &a, const TiledTables &t, cudaStream_t s)
@@ -238,20 +253,20 @@ cudaError_t launch_sweep_tiled(const SweepArgs &a, const TiledTables &t, cudaStr
     case M_ISING_HALF: {
         HalfTab ht;
         for (int i = 0; i < 16; ++i) ht.t[i] = t.t32[i];
-        return d3 ? launch_track<M_ISING_HALF, 3>(track, obs_mode, grid, s, g, pc, ht)
-                  : launch_track<M_ISING_HALF, 2>(track, obs_mode, grid, s, g, pc, ht);
+        return d3 ? launch_track<M_ISING_HALF, 3>(track, obs_mode, grid, s, g, pc, ht, &t)
+                  : launch_track<M_ISING_HALF, 2>(track, obs_mode, grid, s, g, pc, ht, &t);
     }
     case M_EA: {
         HalfTab ht;
         for (int i = 0; i < 16; ++i) ht.t[i] = t.t32[i];
-        return d3 ? launch_track<M_EA, 3>(track, obs_mode, grid, s, g, pc, ht)
-                  : launch_track<M_EA, 2>(track, obs_mode, grid, s, g, pc, ht);
+        return d3 ? launch_track<M_EA, 3>(track, obs_mode, grid, s, g, pc, ht, &t)
+                  : launch_track<M_EA, 2>(track, obs_mode, grid, s, g, pc, ht, &t);
     }
     case M_ISING_ONE: {
         OneTab ot;
         for (int i = 0; i < 64; ++i) ot.t[i] = t.s1[i];
-        return d3 ? launch_track<M_ISING_ONE, 3>(track, obs_mode, grid, s, g, pc, ot)
-                  : launch_track<M_ISING_ONE, 2>(track, obs_mode, grid, s, g, pc, ot);
+        return d3 ? launch_track<M_ISING_ONE, 3>(track, obs_mode, grid, s, g, pc, ot, &t)
+                  : launch_track<M_ISING_ONE, 2>(track, obs_mode, grid, s, g, pc, ot, &t);
     }
     case M_NE_HEATBATH: {
         NeTab nt = {t.ne_t32[0], 0, t.ne_all4};

@@ -10,9 +10,11 @@ namespace lsmk {
 // 33-bit table (lsm_get_thresholds order), so both families accept exactly the same (w, state) pairs.
 struct TiledTables {
     int usable;            // 0: this table is left to the scalar family
-    // spin-1/2: t32[n + 8*b] = thr - 1 (accept iff w <= t32), b = (s+1)/2, n = up-neighbour count.
-    //   A table with a thr = 0 ("never") entry has no such form -> usable = 0.
+    int has_never;         // some entry has thr = 0: only the tiled family's two-compare (NEV) kernels can run it
+    // spin-1/2 (and EA): t32[n + 8*b] = thr - 1 (accept iff w <= t32), b = (s+1)/2, n = up-neighbour count.
+    //   A thr = 0 ("never") entry has no such form: t32 = 0 and y32 = 1 there (accept iff y32 <= w <= t32), else y32 = 0.
     uint32_t t32[16];
+    uint32_t y32[64];      // lower bounds, indexed like t32 (spin-1/2, EA) or like s1 (spin-1)
     // NE: [0] heat-bath / init threshold, [1] Metropolis 0->1 threshold (32-bit clipped) + flag
     uint32_t ne_t32[2];
     int ne_up_always;

@@ -128,6 +128,11 @@ struct TiledGeom {
 struct HalfTab { uint32_t t[16]; };            // spin-1/2: t[n + 8*b] = thr - 1  (accept iff w <= t)
 struct NeTab { uint32_t t32; int always; int all4; };   // all4: one Philox region per word (c >= 0.15)
 struct OneTab { uint32_t t[64]; };            // spin-1: t[16*dcode + sum] = thr - 1, dcode = class of s' - s
+// Tables with a "never" entry (thr = 0: exp(-dE/T) < 2^-32, any cold lattice) cannot be written as w <= thr - 1.  The
+// NEV instantiations of the tiled family carry a second table y at byte offset nev_offset() behind t and accept iff
+// y <= w <= t:  thr in [1, 2^32]: t = thr - 1, y = 0;  thr = 0: t = 0, y = 1 (empty interval).  One more compare per site.
+struct NevTab { uint32_t y[64]; };
+template <int MODEL> __host__ __device__ constexpr uint32_t nev_offset() { return MODEL == M_ISING_ONE ? 256u : 64u; }
 template <int MODEL> struct TabOf { using type = NeTab; };
 template <> struct TabOf<M_ISING_HALF> { using type = HalfTab; };
 template <> struct TabOf<M_ISING_ONE> { using type = OneTab; };
@@ -162,10 +167,25 @@ __device__ __forceinline__ uint32_t add_if_le(uint32_t t, uint32_t w, uint32_t t
         : "+r"(t) : "r"(w), "r"(thr), "r"(one), "n"(INC));
     return t;
 }
+// t + INC if lo <= w <= hi (the NEV form)
+template <uint32_t INC>
+__device__ __forceinline__ uint32_t add_if_in(uint32_t t, uint32_t w, uint32_t hi, uint32_t lo, uint32_t one)
+{
+    asm("{\n\t.reg .pred p;\n\tsetp.ge.u32 p, %1, %3;\n\tsetp.le.and.u32 p, %1, %2, p;\n\t@p mad.lo.u32 %0, %4, %5, %0;\n\t}"
+        : "+r"(t) : "r"(w), "r"(hi), "r"(lo), "r"(one), "n"(INC));
+    return t;
+}
+// The threshold lookup and merge of one site: table byte offset `off`, shared-space table base s_t.
+template <int MODEL, bool NEV, uint32_t INC>
+__device__ __forceinline__ uint32_t accept_site(uint32_t t, uint32_t w, uint32_t s_t, uint32_t off, uint32_t one)
+{
+    if (NEV) return add_if_in<INC>(t, w, lds_u32(s_t, off), lds_u32(s_t + nev_offset<MODEL>(), off), one);
+    return add_if_le<INC>(t, w, lds_u32(s_t, off), one);
+}
 
 // Observables (a6) cost no ALU-pipe instruction: the up-count and the sum of b'*n are IDP.4A dot products
 // (FMA-heavy pipe) straight into the thread's 32-bit totals.
-template <bool TRACK, int OBS>
+template <bool TRACK, int OBS, bool NEV = false>
 __device__ __forceinline__ uint32_t rule_half(uint32_t own, uint32_t nsum, uint4 r, uint32_t s_t, uint32_t one,
                                               int &totU, int &totBN)
 {
@@ -173,10 +193,10 @@ __device__ __forceinline__ uint32_t rule_half(uint32_t own, uint32_t nsum, uint4
     const uint32_t n = TRACK ? (nsum & 0x07070707u) : nsum;
     const uint32_t adr = b * 32u + n * 4u;                 // byte offset of t[n + 8b], per site byte
     uint32_t t = b;                                        // b + accepted flips (bytes end up 0, 1 or 2)
-    t = add_if_le<0x00000001u>(t, r.x, lds_u32(s_t, adr & 0xFFu), one);
-    t = add_if_le<0x00000100u>(t, r.y, lds_u32(s_t, __byte_perm(adr, 0u, 0x4441)), one);
-    t = add_if_le<0x00010000u>(t, r.z, lds_u32(s_t, __byte_perm(adr, 0u, 0x4442)), one);
-    t = add_if_le<0x01000000u>(t, r.w, lds_u32(s_t, adr >> 24), one);
+    t = accept_site<M_ISING_HALF, NEV, 0x00000001u>(t, r.x, s_t, adr & 0xFFu, one);
+    t = accept_site<M_ISING_HALF, NEV, 0x00000100u>(t, r.y, s_t, __byte_perm(adr, 0u, 0x4441), one);
+    t = accept_site<M_ISING_HALF, NEV, 0x00010000u>(t, r.z, s_t, __byte_perm(adr, 0u, 0x4442), one);
+    t = accept_site<M_ISING_HALF, NEV, 0x01000000u>(t, r.w, s_t, adr >> 24, one);
     const uint32_t b2 = t & 0x01010101u;                   // b xor flip
     if (OBS >= 1) totU = (int)__dp4a(b2, 0x01010101u, (uint32_t)totU);
     if (OBS >= 2) totBN = (int)__dp4a(n, b2, (uint32_t)totBN);
@@ -238,7 +258,7 @@ __host__ __device__ constexpr int lut3(bool f000, bool f001, bool f010, bool f01
            (f110 ? 64 : 0) | (f111 ? 128 : 0);
 }
 
-template <int DIMS, bool TRACK, int OBS>
+template <int DIMS, bool TRACK, int OBS, bool NEV = false>
 __device__ __forceinline__ uint32_t rule_one(uint32_t own, uint32_t nsum, uint4 ra, uint4 rb, uint32_t s_t, uint32_t one,
                                              int &totSA, int &totSAS, int &totSS)
 {
@@ -261,10 +281,10 @@ __device__ __forceinline__ uint32_t rule_one(uint32_t own, uint32_t nsum, uint4 
     const uint32_t d = lop3<0xCA>(0x01010101u, lop3<D0>(own, dn, kk), lop3<D1>(own, up, kk)) & 0x03030303u;
     const uint32_t adr = d * 64u + nsum * 4u;              // byte offset of t[16 d + sum], per site byte
     uint32_t acc = 0u;                                     // 0xFF in the byte of every accepted site
-    acc = add_if_le<0x000000FFu>(acc, ra.y, lds_u32(s_t, adr & 0xFFu), one);
-    acc = add_if_le<0x0000FF00u>(acc, ra.w, lds_u32(s_t, __byte_perm(adr, 0u, 0x4441)), one);
-    acc = add_if_le<0x00FF0000u>(acc, rb.y, lds_u32(s_t, __byte_perm(adr, 0u, 0x4442)), one);
-    acc = add_if_le<0xFF000000u>(acc, rb.w, lds_u32(s_t, adr >> 24), one);
+    acc = accept_site<M_ISING_ONE, NEV, 0x000000FFu>(acc, ra.y, s_t, adr & 0xFFu, one);
+    acc = accept_site<M_ISING_ONE, NEV, 0x0000FF00u>(acc, ra.w, s_t, __byte_perm(adr, 0u, 0x4441), one);
+    acc = accept_site<M_ISING_ONE, NEV, 0x00FF0000u>(acc, rb.y, s_t, __byte_perm(adr, 0u, 0x4442), one);
+    acc = accept_site<M_ISING_ONE, NEV, 0xFF000000u>(acc, rb.w, s_t, adr >> 24, one);
     const uint32_t fl = x & acc & 0x03030303u;             // change of the two value bits
     uint32_t nw = own ^ fl;
     if (TRACK) nw |= ((fl | (fl >> 1)) & 0x01010101u) << 4;    // "ever changed"
@@ -284,7 +304,7 @@ __device__ __forceinline__ uint32_t rule_one(uint32_t own, uint32_t nsum, uint4 
 // when it is known at compile time (0 / 1: the side neighbour is the byte to the left / right), or
 // 2 when it has to be read from the register (warps whose lanes mix row parities).
 // ------------------------------------------------------------------------------------------
-template <int MODEL, int DIMS, bool TRACK, int OBS>
+template <int MODEL, int DIMS, bool TRACK, int OBS, bool NEV = false>
 struct March {
     const uint4 *pC;        // other colour, word of the current step
     uint4 *pO;              // own colour, word of the current step
@@ -341,7 +361,7 @@ struct March {
                 uint32_t ns = p[d] + n[d] + c[d] + sd[d];
                 if (DIMS == 3) ns += yp[d] + yn[d];
                 uint4 r = philox_sweep(grp + d, pc);
-                out[d] = rule_half<TRACK, OBS>(o[d], ns, r, s_t, one, totU, totBN);
+                out[d] = rule_half<TRACK, OBS, NEV>(o[d], ns, r, s_t, one, totU, totBN);
             }
         } else if (MODEL == M_EA) {
             // Reading D25: an antiferromagnetic bond turns the neighbour's "up" into "down", so the up-count is
@@ -361,7 +381,7 @@ struct March {
                     ns += lop3<0x28>(p[d], bw[d] >> 2, m1) + lop3<0x28>(n[d], bw[d] >> 3, m1);
                 }
                 uint4 r = philox_sweep(grp + d, pc);
-                out[d] = rule_half<TRACK, OBS>(o[d], ns, r, s_t, one, totU, totBN);
+                out[d] = rule_half<TRACK, OBS, NEV>(o[d], ns, r, s_t, one, totU, totBN);
                 if (OBS >= 2) totS = (int)__dp4a(ns, m1, (uint32_t)totS);
             }
         } else if (MODEL == M_ISING_ONE) {
@@ -378,7 +398,7 @@ struct March {
                 }
                 uint4 ra = philox_sweep(2u * (grp + d), pc);
                 uint4 rb = philox_sweep(2u * (grp + d) + 1u, pc);
-                out[d] = rule_one<DIMS, TRACK, OBS>(o[d], ns, ra, rb, s_t, one, totU, totBN, totS);
+                out[d] = rule_one<DIMS, TRACK, OBS, NEV>(o[d], ns, ra, rb, s_t, one, totU, totBN, totS);
             }
         } else {
             uint32_t accU = 0;
@@ -634,8 +654,8 @@ __device__ __forceinline__ void column_of(const TiledGeom &g, int col, int &y, i
 // Geometry of one thread's march: segment `seg` of the march axis, word column `col`, colour `half`
 // being updated (own) against the other colour (oth), upwards from the segment's first row or
 // downwards from its last.  Returns the number of steps (rows) of the segment.
-template <int MODEL, int DIMS, bool TRACK, int OBS>
-__device__ __forceinline__ int march_init(March<MODEL, DIMS, TRACK, OBS> &M, const TiledGeom &g, uint8_t *own,
+template <int MODEL, int DIMS, bool TRACK, int OBS, bool NEV>
+__device__ __forceinline__ int march_init(March<MODEL, DIMS, TRACK, OBS, NEV> &M, const TiledGeom &g, uint8_t *own,
                                           const uint8_t *oth, int half, int seg, int col, bool up)
 {
     int y, j;
@@ -688,8 +708,8 @@ __device__ __forceinline__ int march_init(March<MODEL, DIMS, TRACK, OBS> &M, con
 //   B = sum_{i in colour 1} s'_i nn_i = 4 sum b'n - 2 sum n - 4d U1 + dN   with   sum_{colour 1} n = 2d U0
 // (each up site of colour 0 is a neighbour of 2d colour-1 sites).  Hence the first colour contributes
 // -4d U0 and the second 4 sum b'n - 4d U1 + 2d nsites; no separate sum of n is needed.
-template <int MODEL, int DIMS, bool TRACK, int OBS>
-__device__ __forceinline__ void march_observables(const March<MODEL, DIMS, TRACK, OBS> &M, int nsites, bool second,
+template <int MODEL, int DIMS, bool TRACK, int OBS, bool NEV>
+__device__ __forceinline__ void march_observables(const March<MODEL, DIMS, TRACK, OBS, NEV> &M, int nsites, bool second,
                                                   long long &cB, long long &cM)
 {
     cB = 0;
