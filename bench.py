@@ -248,24 +248,45 @@ def run_ours(args, w):
     assert lat.measure_full() == (Bv, Mv), "fused observables disagree with the full reduction"
     assert tdone == S * (K + Wm)
 
-    # ---- end-to-end through the C ABI with HOST buffers (pinned), copies inside the timed region
+    # ---- end-to-end through the C ABI with HOST buffers (pinned), copies inside the timed region.
+    # Every step uploads its input configuration (N bytes, lsm_stage_spins_host on a copy stream), installs it
+    # (lsm_set_spins: layout conversion + full reduction), sweeps S times and downloads the (B, M) series
+    # (lsm_sweep_record_host_async).  Two staging buffers: the upload of step k+1 overlaps the sweeps of step k.
     h_in = torch.empty(N, dtype=torch.int8).pin_memory()
     h_in.copy_(lat.get_spins().cpu())
-    h_obs = torch.empty((S, 2), dtype=torch.int64).pin_memory()
     Ke = max(3, min(K, 10))
-    lat.set_spins_host(h_in, tdone)
-    lat.sweep_record_host(S, h_obs)
+    h_obs = [torch.empty((S, 2), dtype=torch.int64).pin_memory() for _ in range(2)]
+    d_obs = [torch.empty((S, 2), dtype=torch.int64, device=lat.device) for _ in range(2)]
+    d_stage = [torch.empty(N, dtype=torch.int8, device=lat.device) for _ in range(2)]
+    copy_stream, comp = torch.cuda.Stream(device=lat.device), torch.cuda.current_stream(lat.device)
+    staged = [torch.cuda.Event() for _ in range(2)]
+    consumed = [torch.cuda.Event() for _ in range(2)]
+
+    def e2e_pass(n_steps):
+        lat.stage_spins_host(h_in, d_stage[0], copy_stream)
+        staged[0].record(copy_stream)
+        for k in range(n_steps):
+            b = k & 1
+            comp.wait_event(staged[b])
+            lat.set_spins(d_stage[b], tdone)                       # convert + full (B, M) reduction, compute stream
+            consumed[b].record(comp)
+            if k + 1 < n_steps:                                    # next step's upload, behind this step's sweeps
+                if k >= 1:
+                    copy_stream.wait_event(consumed[b ^ 1])
+                lat.stage_spins_host(h_in, d_stage[b ^ 1], copy_stream)
+                staged[b ^ 1].record(copy_stream)
+            lat.sweep_record_host_async(S, h_obs[b], d_obs[b])     # S sweeps + D2H of the series (enqueued)
+
+    e2e_pass(2)
     barrier()
-    t0 = time.perf_counter()
     e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
     e0.record()
-    for _ in range(Ke):
-        lat.set_spins_host(h_in, tdone)        # H2D of the step's input configuration (N bytes)
-        lat.sweep_record_host(S, h_obs)        # S sweeps + D2H of the (B, M) series (synchronises)
+    e2e_pass(Ke)
     e1.record()
     torch.cuda.synchronize()
     e2e_ms = e0.elapsed_time(e1)
     e2e_value = replicas.aggregate(e2e_ms, N * S * Ke, lat.device)[2] / 1e9
+    assert int(h_obs[(Ke - 1) & 1][-1, 1]) == lat.measure_int()[1]     # the downloaded series is the one just computed
 
     if rank != 0:
         if world > 1:
@@ -290,7 +311,9 @@ def run_ours(args, w):
         "roofline": roofline,
         "roofline_hbm": roofline_hbm,
         "e2e": {"value": e2e_value, "unit": "Gflips/s", "h2d_bytes_per_step": N, "d2h_bytes_per_step": 16 * S,
-                "steps": Ke, "api": "lsm_set_spins_host + lsm_sweep_record_host (pinned host buffers)"},
+                "steps": Ke,
+                "api": "lsm_stage_spins_host (copy stream) + lsm_set_spins + lsm_sweep_record_host_async, pinned host buffers, "
+                       "two staging buffers: the upload of step k+1 overlaps the sweeps of step k"},
         "gpu_launches": int(launches),
         "clocks": clocks,
         "step_ms_min_med_max": [min(step_ms), statistics.median(step_ms), max(step_ms)],
@@ -536,14 +559,18 @@ PROBE_MODES = [
     (8, "4 Philox calls + 80 IMAD", 80, 80, 80),
     (9, "4 Philox calls + 80 IMAD + 80 LOP3", 80, 80, 160),
     (10, "4 Philox calls + 80 IMAD + 160 LOP3", 80, 80, 240),
+    # the wide multiply split into IMAD.HI + IMAD (counted here as 2 "other IMADs" each, no wide multiply)
+    (11, "8 mul.hi + 8 mul.lo (+8 adds)", 0, 16, 8),
+    (12, "4 Philox calls, hi/lo split (80 HI + 80 LO + 80 LOP3)", 0, 160, 80),
+    (13, "4 Philox calls, hi/lo split + 80 LOP3", 0, 160, 160),
 ]
 
 
 def pipe_probe(blocks_per_sm=8, iters=1024):
     """Register-only integer instruction streams (csrc/probe/pipe_probe.cu, its own libpipe_probe.so): cycles per loop
     iteration and warp against the issue law of DESIGN.md 6 -- every 16-lane math instruction (ALU or FMA-heavy pipe)
-    takes one 2-cycle issue slot of its sub-partition, a wide multiply additionally keeps the multiplier busy for 4:
-    cycles = max(4 W + 2 I, 2 (W + I + A) + 2 x 3 loop instructions)."""
+    FMA-heavy pipe: 4 cycles per wide multiply, 2 per other IMAD; ALU pipe: 2 cycles per instruction, and every wide
+    multiply also takes one ALU-pipe slot: cycles = max(4 W + 2 I, 2 (A + W + 3 loop instructions))."""
     import ctypes
 
     import torch
@@ -567,8 +594,8 @@ def pipe_probe(blocks_per_sm=8, iters=1024):
     sink = torch.empty(blocks * 256, dtype=torch.int32, device="cuda")
     stream = ctypes.c_void_p(torch.cuda.current_stream().cuda_stream)
     print(f"# {props.name}  clocks.max.sm {mhz} MHz  {warps_per_smsp:.0f} warps per sub-partition, {iters} iterations")
-    print("| stream | measured cycles/iter/warp | law max(4W+2I, 2(W+I+A+3)) | math instr per cycle and sub-partition |")
-    print("|---|---|---|---|")
+    print("| stream | measured cycles/iter/warp | law max(4W+2I, 2(A+W+3)) | measured / law | math instr per cycle and sub-partition |")
+    print("|---|---|---|---|---|")
     for mode, name, Wd, I, A in PROBE_MODES:
         assert lib.pipe_probe_run(mode, blocks, 32, sink.data_ptr(), stream) == 0
         torch.cuda.synchronize()
@@ -578,8 +605,8 @@ def pipe_probe(blocks_per_sm=8, iters=1024):
         e1.record()
         torch.cuda.synchronize()
         cyc = e0.elapsed_time(e1) * 1e-3 * mhz * 1e6 / iters / warps_per_smsp
-        law = max(4 * Wd + 2 * I, 2 * (Wd + I + A + 3))
-        print(f"| {name} | {cyc:.1f} | {law} | {(Wd + I + A + 3) / cyc:.3f} |")
+        law = max(4 * Wd + 2 * I, 2 * (A + Wd + 3))
+        print(f"| {name} | {cyc:.1f} | {law} | {cyc / law:.2f} | {(Wd + I + A + 3) / cyc:.3f} |")
     return 0
 
 

@@ -112,6 +112,9 @@ int lsm_sweep_record(lsm_t *, int64_t n, int64_t *d_obs, void *stream);
 /* Same with a HOST result buffer h_obs[n][2]; the device->host copy is enqueued on stream and
  * the call returns after it completed (synchronises).  d_scratch: device, 16*n bytes. */
 int lsm_sweep_record_host(lsm_t *, int64_t n, int64_t *h_obs, int64_t *d_scratch, void *stream);
+/* Same without the final synchronisation: the copy into h_obs (pinned host memory) is enqueued on stream; the
+ * series is valid once the caller has synchronised it.  For pipelines that keep several steps in flight. */
+int lsm_sweep_record_host_async(lsm_t *, int64_t n, int64_t *h_obs, int64_t *d_scratch, void *stream);
 
 /* North-East model only: n sweeps of the paper's "corrected algorithm" (steps 3-10) instead of
  * the checkerboard sweep, which the paper rejects for relaxation dynamics.  The lattice is
@@ -121,10 +124,9 @@ int lsm_sweep_record_host(lsm_t *, int64_t n, int64_t *h_obs, int64_t *d_scratch
  * right, Fig. 4) are those of the launch start; the picks of a sub-step read the tile as the sub-step found it;
  * on a same-site collision the highest thread wins; Philox counter (tile, sub-step * ceil(lambda/2) + thread/2,
  * sweep, 4 + launch).  d_obs: NULL, or device [n][2] receiving (0, M) after every sweep.  Asynchronous.
- * UNSUPPORTED unless tile_edge is a power of two in [8, 128] dividing L, lambda a power of two in [1, 32],
- * 2 * lambda divides P, and the 32/lambda tiles a warp holds fit the block's shared memory:
- * (32/lambda) * ((b+1)*b + b + (lambda > 1 ? b*b : 0)) <= 200 KB with b = tile_edge, which refuses
- * tile_edge = 128 with lambda <= 4 and tile_edge = 64 with lambda = 1.  Shares the sweep counter with lsm_sweep. */
+ * UNSUPPORTED unless tile_edge is a power of two in [8, 128] dividing L, lambda a power of two in [1, 32] and
+ * 2 * lambda divides P.  tile_edge = L with lambda = 1 is the serial limit Q = lambda = 1 of PAPER.md:142 (one thread
+ * updates the whole lattice: slow by construction).  Shares the sweep counter with lsm_sweep. */
 int lsm_sweep_random_tile(lsm_t *, int64_t n, int tile_edge, int lambda, int64_t *d_obs, void *stream);
 /* Its balance-preserving variant ("~2.5x slower"): a sub-step is lambda picks among the tile's red
  * sites, a barrier, lambda picks among its white sites, a barrier; four launches complete one MC step.  Readings
@@ -150,7 +152,7 @@ int lsm_sweep_random_tile_balanced(lsm_t *, int64_t n, int tile_edge, int lambda
  *    lsm_get_spins, lsm_set_spins, lsm_persistence, lsm_measure*, lsm_get_thresholds, ...  The batch sweeps in lockstep:
  *    LSM_ERR_STATE if the replicas' sweep counters differ (one of them was swept on its own).
  *  - lsm_batch_measure_int: running (B, M) of every replica into host arrays of R (either may be NULL); synchronises once.
- *  - lsm_batch_set_cluster: thread blocks per replica (power of two <= 16, 0 = automatic: fill the SMs about twice). */
+ *  - lsm_batch_set_cluster: thread blocks per replica (power of two <= 16, 0 = automatic: about one block per SM). */
 int lsm_batch_workspace_bytes(int R, int dims, int L, int two_S, int model, size_t *bytes);
 int lsm_batch_create(int R, int dims, int L, int two_S, int model, double J, double h, const double *T,
                      const uint64_t *seeds, void *d_workspace, size_t workspace_bytes, void *stream, lsm_batch_t **out);
@@ -192,6 +194,10 @@ int lsm_get_spins_host(lsm_t *, int8_t *h_out, int8_t *d_scratch /* N bytes */, 
 int lsm_set_spins(lsm_t *, const int8_t *d_in, uint64_t sweep_counter, void *stream);
 int lsm_set_spins_host(lsm_t *, const int8_t *h_in, int8_t *d_scratch /* N bytes */,
                        uint64_t sweep_counter, void *stream);
+/* Upload only: h_in (host, N int8, pinned for a truly asynchronous copy) -> d_stage (device, N bytes) on copy_stream,
+ * without touching the lattice.  Lets the upload of the next configuration overlap the sweeps of the current one:
+ * stage on a copy stream, order the streams with an event, then lsm_set_spins(d_stage, ...) on the compute stream. */
+int lsm_stage_spins_host(lsm_t *, const int8_t *h_in, int8_t *d_stage, void *copy_stream);
 
 /* LSM_EA only (else UNSUPPORTED): bond signs in canonical form, d_tau int8 [dims][N] on the device, tau[a][i] = sign
  * (+1 ferro, -1 antiferro) of the bond between site i and its neighbour in direction +a (a = 0, 1, 2 = x, y, z).

@@ -337,6 +337,18 @@ extern "C" int lsm_sweep_random_tile_balanced(lsm_t *o, int64_t n, int tile_edge
     return random_tile_impl(o, n, tile_edge, lambda, d_obs, stream, true);
 }
 
+// As lsm_sweep_record_host, but the device->host copy of the series is only enqueued: h_obs (pinned) is valid after
+// the caller has synchronised `stream`.
+extern "C" int lsm_sweep_record_host_async(lsm_t *o, int64_t n, int64_t *h_obs, int64_t *d_scratch, void *stream)
+{
+    if (!o || n < 0 || ((!h_obs || !d_scratch) && n > 0)) return LSM_ERR_ARG;
+    cudaStream_t s = (cudaStream_t)stream;
+    int rc = sweep_impl(o, n, (long long *)d_scratch, s);
+    if (rc != LSM_OK) return rc;
+    if (n > 0) CU(cudaMemcpyAsync(h_obs, d_scratch, (size_t)n * 16, cudaMemcpyDeviceToHost, s));
+    return LSM_OK;
+}
+
 extern "C" int lsm_sweep_record_host(lsm_t *o, int64_t n, int64_t *h_obs, int64_t *d_scratch, void *stream)
 {
     if (!o || n < 0 || ((!h_obs || !d_scratch) && n > 0)) return LSM_ERR_ARG;
@@ -705,6 +717,16 @@ extern "C" int lsm_get_bonds(lsm_t *o, int8_t *d_tau, void *stream)
     o->last_stream = (cudaStream_t)stream;
     CU(launch_ea_get_bonds(o->lat, d_tau, o->last_stream));
     o->launches += 1;
+    return LSM_OK;
+}
+
+// Pipelined host I/O: the upload of the NEXT configuration can run on a copy stream while the current one is being
+// swept.  lsm_stage_spins_host only copies h_in -> d_stage (it does not touch the lattice); lsm_set_spins(d_stage, ...)
+// then installs it on the compute stream once the caller has ordered the two streams (event).
+extern "C" int lsm_stage_spins_host(lsm_t *o, const int8_t *h_in, int8_t *d_stage, void *copy_stream)
+{
+    if (!o || !h_in || !d_stage) return LSM_ERR_ARG;
+    CU(cudaMemcpyAsync(d_stage, h_in, (size_t)o->N, cudaMemcpyHostToDevice, (cudaStream_t)copy_stream));
     return LSM_OK;
 }
 

@@ -28,6 +28,7 @@ struct NeTileArgs {
     int lg_b, lg_lam;        // tile edge and lambda are powers of two
     int ntx;                 // tiles per lattice row
     int ntiles;
+    int gpw;                 // tile groups of a warp that hold a tile (<= 32 / lambda; fewer when tiles are large)
     uint32_t k0, k1, c2, c3; // Philox key and the (sweep, launch) fields of the counter
     uint32_t rk0[10], rk1[10];   // round keys k0 + r W0, k1 + r W1 (kernel-parameter bank: operands of the round's LOP3)
     uint32_t thr_c, thr_up;  // floor(c 2^32), floor(exp(-1/T) 2^32) clipped to 32 bits
@@ -73,13 +74,18 @@ k_ne_random_tile(const __grid_constant__ NeTileArgs a)
     extern __shared__ __align__(16) uint8_t s_tiles[];
     const int b = 1 << a.lg_b, lam = 1 << a.lg_lam, P = b * b;
     const int lane = threadIdx.x & 31, j = lane & (lam - 1);          // j: thread index within the tile's group
-    const int grp_in_warp = lane >> a.lg_lam, grp_per_warp = 32 >> a.lg_lam;
+    // A warp has 32 / lambda groups of lambda lanes; the first a.gpw of them own a tile at a time (all of them unless
+    // the tiles are too large for shared memory: 128 x 128 tiles with lambda <= 4, the serial limit Q = lambda = 1 of
+    // PAPER.md:142 on a 128^2 lattice).  The other groups idle: they run the same instructions on the last group's tile
+    // but write nothing.
+    const int grp_in_warp = lane >> a.lg_lam, grp_per_warp = a.gpw;
+    const bool has_tile = grp_in_warp < grp_per_warp;
     const int warp_global = (blockIdx.x * blockDim.x + threadIdx.x) >> 5;
     const int nwarps = (gridDim.x * blockDim.x) >> 5;
     const int rowb = b >> 1;                                          // bytes per tile row and colour
     const int col_bytes = (b + 1) * rowb;                             // rows 0..b (row b = north boundary)
     const int tile_bytes = (2 * col_bytes + b + (lam > 1 ? P : 0) + 15) & ~15;   // + east column + claim bytes
-    uint8_t *const tile = s_tiles + (size_t)((threadIdx.x >> 5) * grp_per_warp + grp_in_warp) * tile_bytes;
+    uint8_t *const tile = s_tiles + (size_t)((threadIdx.x >> 5) * grp_per_warp + (has_tile ? grp_in_warp : grp_per_warp - 1)) * tile_bytes;
     uint8_t *const east = tile + 2 * col_bytes;
     // 32-bit shared-space addresses for the pick loop (no generic-address conversion per access)
     const uint32_t s_tile = (uint32_t)__cvta_generic_to_shared(tile), s_east = s_tile + 2u * (uint32_t)col_bytes,
@@ -91,7 +97,7 @@ k_ne_random_tile(const __grid_constant__ NeTileArgs a)
 
     for (int base = warp_global * grp_per_warp; base < a.ntiles; base += nwarps * grp_per_warp) {
         const int T = base + grp_in_warp;
-        const bool live = T < a.ntiles;                                // tail groups idle but keep the warp converged
+        const bool live = has_tile && T < a.ntiles;                    // tail groups idle but keep the warp converged
         const int ty = live ? T / a.ntx : 0, tx = live ? T - ty * a.ntx : 0;   // one division per tile
         const int x0 = tx << a.lg_b, y0 = ty << a.lg_b;
         const uint32_t key_hi = ((uint32_t)grp_in_warp << 16) | (live ? 0u : 0x80000000u);
@@ -126,7 +132,7 @@ k_ne_random_tile(const __grid_constant__ NeTileArgs a)
         // byte of the picked site; after the barrier a lane that reads back another index has collided, and only then
         // is MATCH used.  Stale claim bytes cannot hide a collision: every lane overwrites its byte before it reads it.
         auto pick = [&](const int r, const int px, const int py, const int c, const uint32_t w_acc) {
-            if (lam > 1) sts_u8(s_claim + (uint32_t)r, (uint32_t)j);
+            if (lam > 1 && has_tile) sts_u8(s_claim + (uint32_t)r, (uint32_t)j);
             const uint32_t me = s_tile + (uint32_t)(c * col_bytes + py * rowb + (px >> 1));
             const uint32_t oth = s_tile + (uint32_t)((c ^ 1) * col_bytes + py * rowb);
             const uint32_t own = lds_u8(me);
@@ -142,7 +148,7 @@ k_ne_random_tile(const __grid_constant__ NeTileArgs a)
             }
             __syncwarp();                                              // all picks have read the phase's start
             bool winner = true;
-            if (lam > 1 && __any_sync(0xffffffffu, lds_u8(s_claim + (uint32_t)r) != (uint32_t)j)) {
+            if (lam > 1 && __any_sync(0xffffffffu, has_tile && lds_u8(s_claim + (uint32_t)r) != (uint32_t)j)) {
                 const uint32_t same = __match_any_sync(0xffffffffu, (uint32_t)r | key_hi);
                 winner = (same >> lane) == 1u;                         // no higher lane holds the same key
             }
@@ -233,14 +239,22 @@ bool ne_tile_supported(const Lat &lat, int b, int lam, bool balanced)
     if (b < 8 || b > 128 || (b & (b - 1)) != 0 || lat.L % b != 0) return false;
     if (lam < 1 || lam > 32 || (lam & (lam - 1)) != 0) return false;
     if ((b * b) % ((balanced ? 8 : 2) * lam) != 0) return false;   // q * lambda = P/2 (D17) or q * 2 lambda = P/4 (D23)
-    return (32 / lam) * ne_tile_bytes(b, lam) <= 200 * 1024;   // one warp's tiles must fit shared memory
+    return true;                                                   // one tile always fits: <= 33 KB
 }
 
-// Threads per CTA: as many tile groups as fit ~96 KB of shared memory (at least one warp).
+// Tile groups per warp that hold a tile, and threads per CTA: as many tiles as fit ~96 KB of shared memory.
+static int ne_tile_gpw(int b, int lam)
+{
+    int gpw = 32 / lam;
+    const int fit = (int)((96 * 1024) / ne_tile_bytes(b, lam));
+    if (gpw > fit) gpw = fit < 1 ? 1 : fit;
+    return gpw;
+}
 static int ne_tile_threads(int b, int lam)
 {
+    const int gpw = ne_tile_gpw(b, lam);
     int threads = 256;
-    while (threads > 32 && (threads / lam) * ne_tile_bytes(b, lam) > 96 * 1024) threads >>= 1;
+    while (threads > 32 && (threads / 32) * gpw * ne_tile_bytes(b, lam) > 96 * 1024) threads >>= 1;
     return threads;
 }
 
@@ -274,7 +288,8 @@ cudaError_t launch_ne_random_tile(const Lat &lat, uint8_t *const dst[2], bool me
     a.track = track;
     a.obs = obs;
     const int threads = ne_tile_threads(b, lam);
-    const int tiles_per_cta = threads / lam;
+    a.gpw = ne_tile_gpw(b, lam);
+    const int tiles_per_cta = (threads / 32) * a.gpw;
     const size_t smem = tiles_per_cta * ne_tile_bytes(b, lam);
     int grid = (a.ntiles + tiles_per_cta - 1) / tiles_per_cta;
     const int cap = sm_count() * 8;

@@ -583,14 +583,14 @@ bool small_batch_supported(const Lat &lat, int model, const TiledTables &t)
 }
 
 // Blocks per replica.  One lattice alone takes the largest cluster that keeps >= 4 warps per block (latency bound);
-// R lattices together should fill the 148 SMs about twice over and no more: smaller clusters mean cheaper barriers.
+// R lattices together should fill the 148 SMs once and no more: smaller clusters mean cheaper barriers.
 int small_batch_cluster(const Lat &lat, int R)
 {
     const long long nlanes = lat.half / 4, N = 2 * lat.half;
     int cmax = 1;
     while (cmax < small_max_cluster() && nlanes / (2 * cmax) >= 128 && 2 * cmax <= lat.L) cmax *= 2;
     int c = cmax;
-    while (c > 1 && (long long)R * c > 2ll * sm_count()) c >>= 1;
+    while (c > 1 && (long long)R * c > (long long)sm_count()) c >>= 1;   // measured: one block per SM beats two (32 x 128^2: c = 4)
     while (N / c > 196608 && c < 16) c <<= 1;          // the slab must fit shared memory
     while (nlanes / c > 2048 && c < 16) c <<= 1;       // at most two lanes per thread: the hoisted-geometry body
     return c;

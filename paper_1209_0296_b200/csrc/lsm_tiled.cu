@@ -24,6 +24,11 @@
 #include <cstdlib>
 #include <cstring>
 
+// up-concentration from which the North-East rule runs the four Philox calls of a word together (see update_word)
+#ifndef LSM_NE_ALL4_C
+#define LSM_NE_ALL4_C 0.25
+#endif
+
 namespace lsmk {
 
 PhiloxSweepConsts make_philox_consts(const SweepKey &k)
@@ -88,6 +93,9 @@ k_sweep_tiled(const __grid_constant__ TiledGeom g, const __grid_constant__ Philo
         const int col = (int)(gt - (long long)seg * g.ncol);
         const int n = march_init(M, g, g.own, g.oth, g.half, seg, col, true);
         nsites = 16 * n;
+        if constexpr (MODEL == M_ISING_ONE && LSM_TILED_ONE_UNROLL1 && !PF) {
+            M.template run1<true>(n, pc);
+        } else
         if (g.parity_rows) {            // warp-uniform branch: q is a constant inside each loop
             if (M.q) PF ? M.template run_pf<1, true>(n, pc) : M.template run<1, true>(n, pc);
             else PF ? M.template run_pf<0, true>(n, pc) : M.template run<0, true>(n, pc);
@@ -148,7 +156,7 @@ void build_tiled_tables(int model, int dims, double J, double h, const uint64_t 
         t.ne_t32[0] = clip(thr[0]);
         t.ne_t32[1] = clip(thr[1]);
         t.ne_up_always = thr[1] == ALWAYS ? 1 : 0;
-        t.ne_all4 = (double)thr[0] >= 0.15 * 4294967296.0 ? 1 : 0;
+        t.ne_all4 = (double)thr[0] >= LSM_NE_ALL4_C * 4294967296.0 ? 1 : 0;
         if (thr[0] == ALWAYS) t.usable = 0;
     }
     *out = t;

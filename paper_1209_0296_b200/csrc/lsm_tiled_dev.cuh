@@ -21,6 +21,10 @@
 #ifndef LSM_TILED_PF_ONE
 #define LSM_TILED_PF_ONE 0
 #endif
+// spin-1: one step per loop iteration instead of the 2x-unrolled, parity-specialised loop
+#ifndef LSM_TILED_ONE_UNROLL1
+#define LSM_TILED_ONE_UNROLL1 1
+#endif
 
 namespace lsmk {
 
@@ -402,25 +406,40 @@ struct March {
             }
         } else {
             uint32_t accU = 0;
-            // Two forms, chosen per launch by the up-concentration c (warp-uniform flag): above c ~ 0.15 nearly every warp
-            // has a facilitated site in each of the four lanes, so one divergent region per WORD runs the four Philox
-            // calls together (instruction-level parallelism, round keys loaded once: 961 -> 1085 Gflips/s at c = 0.2);
-            // below, one region per LANE skips more calls (c = 0.1: 1144 against 1081).
-            if (ne_all4) {
-            uint32_t fac[4];
+            // Random words are needed by facilitated sites only (c^2 of them).  Two forms, chosen per launch by the
+            // up-concentration c (warp-uniform flag):
+            //  dense (c >= LSM_NE_ALL4_C): nearly every warp has a facilitated site in each of the four lanes, so one
+            //    divergent region per WORD runs the four Philox calls together (instruction-level parallelism);
+            //  sparse: every thread walks the list of ITS lanes that hold a facilitated site, one Philox call per
+            //    iteration; the warp iterates max-over-threads times -- 1.3 times on average at c = 0.1 and 2.3 at
+            //    c = 0.2, where a region per lane (any of 32 threads needs it: 73 % / 99 %) would run 2.9 / 4.
+            uint32_t fac[4], lt[4] = {0u, 0u, 0u, 0u};
 #pragma unroll
             for (int d = 0; d < 4; ++d) fac[d] = (UP ? n[d] : p[d]) & (qq ? sd[d] : c[d]) & 0x01010101u;
-            uint32_t lt[4] = {0u, 0u, 0u, 0u};
-            if ((fac[0] | fac[1] | fac[2] | fac[3]) != 0u) {
+            auto draw = [&](const uint32_t group) {
+                const uint4 r = philox_sweep(group, pc);
+                uint32_t l = ne_always ? 0x01010101u : 0u;
+                if (r.x < ne_t32) l |= 0x00000001u;
+                if (r.y < ne_t32) l |= 0x00000100u;
+                if (r.z < ne_t32) l |= 0x00010000u;
+                if (r.w < ne_t32) l |= 0x01000000u;
+                return l;
+            };
+            if (ne_all4) {
+                if ((fac[0] | fac[1] | fac[2] | fac[3]) != 0u) {
 #pragma unroll
-                for (int d = 0; d < 4; ++d) {
-                    const uint4 r = philox_sweep(grp + d, pc);
-                    uint32_t l = ne_always ? 0x01010101u : 0u;
-                    if (r.x < ne_t32) l |= 0x00000001u;
-                    if (r.y < ne_t32) l |= 0x00000100u;
-                    if (r.z < ne_t32) l |= 0x00010000u;
-                    if (r.w < ne_t32) l |= 0x01000000u;
-                    lt[d] = l;
+                    for (int d = 0; d < 4; ++d) lt[d] = draw(grp + d);
+                }
+            } else {
+                uint32_t rem = (fac[0] != 0u ? 1u : 0u) | (fac[1] != 0u ? 2u : 0u) | (fac[2] != 0u ? 4u : 0u) | (fac[3] != 0u ? 8u : 0u);
+                while (rem != 0u) {
+                    const uint32_t d = (uint32_t)__ffs((int)rem) - 1u;
+                    rem &= rem - 1u;
+                    const uint32_t l = draw(grp + d);
+                    lt[0] = d == 0u ? l : lt[0];
+                    lt[1] = d == 1u ? l : lt[1];
+                    lt[2] = d == 2u ? l : lt[2];
+                    lt[3] = d == 3u ? l : lt[3];
                 }
             }
 #pragma unroll
@@ -431,14 +450,6 @@ struct March {
                 else n2 = (nv & ~fac[d]) | (lt[d] & fac[d]);
                 if (OBS >= 1) accU += n2;
                 out[d] = TRACK ? ((o[d] & ~0x01010101u) | n2 | ((nv ^ n2) << 3)) : n2;
-            }
-            } else {
-#pragma unroll
-            for (int d = 0; d < 4; ++d) {
-                uint32_t east = qq ? sd[d] : c[d];
-                out[d] = rule_ne<TRACK, MODEL == M_NE_METROPOLIS, OBS>(o[d], UP ? n[d] : p[d], east, grp + d, pc, ne_t32,
-                                                                        ne_always, accU);
-            }
             }
             if (OBS >= 1) totU += bytesum(accU);
         }
@@ -610,6 +621,15 @@ struct March {
             step<Q1, UP>(pc);
         }
         if (k < n) step<Q0, UP>(pc);
+    }
+
+    // One step per loop iteration, row parity read from the register (Q = 2).  For rules whose 2x-unrolled loop does not
+    // fit the instruction cache (spin-1: 16 KB of code per two steps, `no_instruction` stalls 0.55 per issue).
+    template <bool UP, class PC>
+    __device__ __forceinline__ void run1(int n, const PC &pc)
+    {
+#pragma unroll 1
+        for (int k = 0; k < n; ++k) step<2, UP>(pc);
     }
 
     // The same with the resident family's hooks: h.after_first() once the first row is stored,

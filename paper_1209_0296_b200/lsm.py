@@ -29,6 +29,8 @@ SIGNATURES = {
     "lsm_sweep": (_i32, [_vp, _i64, _vp]),
     "lsm_sweep_record": (_i32, [_vp, _i64, _vp, _vp]),
     "lsm_sweep_record_host": (_i32, [_vp, _i64, _vp, _vp, _vp]),
+    "lsm_sweep_record_host_async": (_i32, [_vp, _i64, _vp, _vp, _vp]),
+    "lsm_stage_spins_host": (_i32, [_vp, _vp, _vp, _vp]),
     "lsm_sweep_random_tile": (_i32, [_vp, _i64, _i32, _i32, _vp, _vp]),
     "lsm_sweep_random_tile_balanced": (_i32, [_vp, _i64, _i32, _i32, _vp, _vp]),
     "lsm_batch_workspace_bytes": (_i32, [_i32, _i32, _i32, _i32, _i32, _P(_sz)]),
@@ -240,6 +242,20 @@ class Lattice:
         _check(self._lib.lsm_sweep_record_host(self._h, int(n), _vp(ptr), _vp(sc.data_ptr()), self._sp(stream)),
                "lsm_sweep_record_host")
         return h_obs
+
+    @_on_device
+    def sweep_record_host_async(self, n, h_obs, d_scratch, stream=None):
+        """n sweeps; the (B, M) series lands in the pinned host tensor h_obs once `stream` has been synchronised."""
+        _check(self._lib.lsm_sweep_record_host_async(self._h, int(n), _vp(h_obs.data_ptr()), _vp(d_scratch.data_ptr()),
+                                                     self._sp(stream)), "lsm_sweep_record_host_async")
+        return h_obs
+
+    @_on_device
+    def stage_spins_host(self, h_in, d_stage, copy_stream):
+        """Upload only (pinned host tensor -> device staging tensor) on copy_stream; install with set_spins(d_stage, t)."""
+        assert h_in.numel() == self.N and d_stage.numel() == self.N and d_stage.is_cuda
+        _check(self._lib.lsm_stage_spins_host(self._h, _vp(h_in.data_ptr()), _vp(d_stage.data_ptr()),
+                                              ctypes.c_void_p(copy_stream.cuda_stream)), "lsm_stage_spins_host")
 
     # ------------------------------------------------------------------ observables
     @_on_device

@@ -386,6 +386,34 @@ def test_random_tile_schedule_parity(model, L, b, lam, c, nsweeps):
     assert lat.measure_int()[:2] == orc.measure_int()
 
 
+@pytest.mark.parametrize("model", [lsm.NE_HEATBATH, lsm.NE_METROPOLIS])
+@pytest.mark.parametrize("L,b,lam", [(128, 128, 1), (128, 128, 4), (64, 64, 1), (256, 128, 2)])
+def test_random_tile_large_tiles_small_lambda(model, L, b, lam):
+    """Tiles too large for every lane group of a warp to hold one (128 x 128 with lambda <= 4), down to the serial
+    limit Q = lambda = 1 of PAPER.md:142 on a 128^2 lattice."""
+    kw = dict(dims=2, L=L, model=model, J=0.0, T=W.ne_temperature(0.42), seed=W.seed_of(5, 11) + L + lam)
+    lat, orc = make_pair(**kw)
+    got = lat.sweep_random_tile(3, b, lam, record=True).cpu().numpy()
+    assert np.array_equal(got, orc.sweep_random_tile_record(3, b, lam))
+    assert_same_state(lat, orc)
+
+
+@pytest.mark.slow
+def test_lambda_convergence_to_the_serial_limit():
+    """PAPER.md:142,155 (Fig. 5): Phi(t) of the corrected algorithm with 32 x 32 tiles follows the serial limit
+    Q = lambda = 1 for lambda up to 16 (about 1.5 % of the tile).  Statistical: 6 realisations of a 128^2 lattice at
+    c = 0.42; tolerance = 4 standard errors of the difference + 0.02."""
+    from paper_1209_0296_b200 import lambda_scan
+
+    times = [10, 30, 100, 300]
+    res = lambda_scan.phi_curves(128, 0.42, [(128, 1), (32, 1), (32, 4), (32, 16), (8, 32)], times, 6)
+    ref = res[(128, 1)]
+    assert all(0.0 < p < 1.0 for p in ref["phi"]) and ref["phi"] == sorted(ref["phi"], reverse=True)   # a decaying curve
+    for key in ((32, 1), (32, 4), (32, 16)):
+        for p, se, q, sq in zip(res[key]["phi"], res[key]["se"], ref["phi"], ref["se"]):
+            assert abs(p - q) < 4 * math.hypot(se, sq) + 0.02, (key, res[key], ref)
+
+
 def test_random_tile_schedule_rejections():
     lat = lsm.Lattice(dims=2, L=64, model=lsm.NE_HEATBATH, J=0.0, T=1.0, seed=3)
     for b, lam in ((24, 16), (32, 3), (4, 2), (32, 64), (256, 16)):
