@@ -27,11 +27,11 @@ MUTANTS = [
     ("stream_tag_ignored", "ctr[3] = stream | ((uint32_t)(t >> 32) << 4);", "ctr[3] = ((uint32_t)(t >> 32) << 4);", [REST], "checkerboard_sweep and 2-4-1-0"),
     ("init_spin1_modulo_instead_of_mulhi", "(int)(((uint64_t)w * 3u) >> 32) - 1", "(int)(w % 3u) - 1", [REST], "init_matches"),
     ("init_word_index_shifted", "uint32_t w = w4[i & 3];", "uint32_t w = w4[(i + 1) & 3];", [REST], "init_matches"),
-    ("init_spin_half_uses_low_bit", "v = (w >> 31) ? 1 : -1;", "v = (w & 1u) ? 1 : -1;", [REST], "init_matches"),
-    ("spin1_words_swapped", "uint32_t w0 = w4[2 * (k & 1)], w1 = w4[2 * (k & 1) + 1];",
-     "uint32_t w1 = w4[2 * (k & 1)], w0 = w4[2 * (k & 1) + 1];", [REST], "checkerboard_sweep and 2-4-2-0"),
-    ("spin1_group_of_four_sites", "words_of_group(o->seed, (uint64_t)k >> 1, o->t, half, w4);",
-     "words_of_group(o->seed, (uint64_t)k >> 2, o->t, half, w4);", [REST], "checkerboard_sweep and 2-4-2-0"),
+    ("init_spin_half_uses_low_bit", "else if (o->two_S == 1)    v = (w >> 31) ? 1 : -1;", "else if (o->two_S == 1)    v = (w & 1u) ? 1 : -1;", [REST], "init_matches"),
+    ("spin1_words_swapped", "uint32_t w0 = w4[2 * (k & 1)], w1 = w4[2 * (k & 1) + 1];\n        int nn = neighbour_sum(o, x, y, z);",
+     "uint32_t w1 = w4[2 * (k & 1)], w0 = w4[2 * (k & 1) + 1];\n        int nn = neighbour_sum(o, x, y, z);", [REST], "checkerboard_sweep and 2-4-2-0"),
+    ("spin1_group_of_four_sites", "/* two words per site: group k>>1, words 2(k&1) and 2(k&1)+1 */\n        words_of_group(o->seed, (uint64_t)k >> 1, o->t, half, w4);",
+     "/* two words per site: group k>>1, words 2(k&1) and 2(k&1)+1 */\n        words_of_group(o->seed, (uint64_t)k >> 2, o->t, half, w4);", [REST], "checkerboard_sweep and 2-4-2-0"),
     ("spin1_proposal_other_direction", "return (a + 1 + kk) % 3;", "return (a + 2 - kk) % 3;", [REST], "checkerboard_sweep and 2-4-2-0"),
     ("ne_west_instead_of_east", "east = value_at(o, x + 1, y, 0);", "east = value_at(o, x - 1, y, 0);", [REST], "checkerboard_sweep and 2-6-1-1"),
     ("ne_south_instead_of_north", "int north = value_at(o, x, y + 1, 0),", "int north = value_at(o, x, y - 1, 0),", [REST], "checkerboard_sweep and 2-6-1-1"),
@@ -60,6 +60,11 @@ MUTANTS = [
     ("ea_bond_sign_inverted", "o->tau[b] = (w4[b & 3] >> 31) ? 1 : -1;", "o->tau[b] = (w4[b & 3] >> 31) ? -1 : 1;", [WIDE], "bonds_from_seed"),
     ("ea_bond_energy_ignores_the_signs", "int f = bond_sign(o, 0, x, y, z) * value_at(o, x + 1, y, z) + bond_sign(o, 1, x, y, z) * value_at(o, x, y + 1, z);",
      "int f = value_at(o, x + 1, y, z) + value_at(o, x, y + 1, z);", [WIDE], "ea_"),
+    ("ea_init_uses_low_bit", "else if (o->model == ORC_EA) v = (w >> 31) ? 1 : -1;", "else if (o->model == ORC_EA) v = (w & 1u) ? 1 : -1;", [WIDE], "ea_"),
+    ("potts_words_swapped", "uint32_t w0 = w4[2 * (k & 1)], w1 = w4[2 * (k & 1) + 1];\n        int r =",
+     "uint32_t w1 = w4[2 * (k & 1)], w0 = w4[2 * (k & 1) + 1];\n        int r =", [WIDE], "potts_matches"),
+    ("potts_group_of_four_sites", "words_of_group(o->seed, (uint64_t)k >> 1, o->t, half, w4);\n        uint32_t w0 = w4[2 * (k & 1)], w1 = w4[2 * (k & 1) + 1];\n        int r =",
+     "words_of_group(o->seed, (uint64_t)k >> 2, o->t, half, w4);\n        uint32_t w0 = w4[2 * (k & 1)], w1 = w4[2 * (k & 1) + 1];\n        int r =", [WIDE], "potts_matches"),
     ("potts_proposal_may_repeat_the_state", "int prop = (s_old + 1 + r) % o->q;", "int prop = (s_old + r) % o->q;", [WIDE], "potts_matches"),
     ("potts_energy_difference_sign", "int dn = neighbours_equal_to(o, x, y, z, prop) - neighbours_equal_to(o, x, y, z, s_old);",
      "int dn = neighbours_equal_to(o, x, y, z, s_old) - neighbours_equal_to(o, x, y, z, prop);", [WIDE], "potts_matches"),
