@@ -40,10 +40,11 @@ NCU_DRAM_BYTES_PER_LAUNCH = {
     "cfg5_c0.30": (67.18e6 + 0.75e6, "profiles/r2_tiled_variants_ncu.md"),
     "hbm3d_1024": (1083.86e6 + 497.63e6, "profiles/r2_tiled_variants_ncu.md"),
 }
-KERNEL_FAMILY = {1: "generic", 2: "tiled", 3: "resident", 4: "small"}
+KERNEL_FAMILY = {1: "generic", 2: "tiled", 3: "resident", 4: "small", 5: "slab"}
 KERNEL_NAME = {1: "k_sweep_generic (half-sweep)", 2: "k_sweep_tiled (half-sweep)",
                3: "k_sweep_resident (per half-sweep share of one launch)",
-               4: "k_sweep_small_lane (per half-sweep share of one launch)"}
+               4: "k_sweep_small_lane (per half-sweep share of one launch)",
+               5: "k_sweep_slab (per half-sweep share of one launch)"}
 
 
 def parse():
@@ -60,7 +61,7 @@ def parse():
                     help="instead of the benchmark: us/sweep of the tiled and the small (cluster) family over lattice sizes")
     ap.add_argument("--pipe-probe", action="store_true",
                     help="instead of the benchmark: the integer-pipe microbenchmarks behind the 'alu' roofline (DESIGN.md 6)")
-    ap.add_argument("--kernel", default="auto", choices=["auto", "generic", "tiled", "resident", "small"],
+    ap.add_argument("--kernel", default="auto", choices=["auto", "generic", "tiled", "resident", "small", "slab"],
                     help="kernel family (lsm_set_kernel); auto = the library's choice")
     return ap.parse_args()
 
@@ -211,7 +212,7 @@ def run_ours(args, w):
         lat.set_tracking(False)  # persistence is not part of configs 1-4
     if args.kernel != "auto":
         lat.set_kernel({"generic": lsm.KERNEL_GENERIC, "tiled": lsm.KERNEL_TILED, "resident": lsm.KERNEL_RESIDENT,
-                        "small": lsm.KERNEL_SMALL}[args.kernel])
+                        "small": lsm.KERNEL_SMALL, "slab": lsm.KERNEL_SLAB}[args.kernel])
     N = lat.N
     obs = torch.empty((S, 2), dtype=torch.int64, device=lat.device)
     flush = torch.empty(256 << 20, dtype=torch.uint8, device=lat.device)  # > 126 MB L2
@@ -461,9 +462,10 @@ def size_scan():
 
     build.build()
     rows = []
-    for dims, L in [(2, 32), (2, 64), (2, 128), (2, 256), (2, 512), (2, 1024), (3, 16), (3, 32), (3, 64)]:
+    for dims, L in [(2, 32), (2, 64), (2, 128), (2, 256), (2, 512), (2, 1024), (2, 2048), (2, 4096), (3, 16), (3, 32), (3, 64),
+                    (3, 128)]:
         row = {"dims": dims, "L": L}
-        for fam, name in ((lsm.KERNEL_TILED, "tiled"), (lsm.KERNEL_SMALL, "small")):
+        for fam, name in ((lsm.KERNEL_TILED, "tiled"), (lsm.KERNEL_SMALL, "small"), (lsm.KERNEL_SLAB, "slab")):
             lat = lsm.Lattice(dims=dims, L=L, T=2.269 if dims == 2 else 4.5115, seed=3)
             lat.set_tracking(False)
             try:
@@ -471,7 +473,7 @@ def size_scan():
             except lsm.LsmError:
                 row[name] = None
                 continue
-            n = 500
+            n = 500 if lat.N <= 1 << 22 else 100
             obs = torch.empty((n, 2), dtype=torch.int64, device="cuda")
             lat.sweep_record(n, out=obs)
             torch.cuda.synchronize()

@@ -88,9 +88,13 @@ enum {
  *           sites); chosen up to 262 144 sites (512^2, 64^3);
  *  TILED    one launch per half-sweep, 16 sites per 128-bit word (L % 32 == 0, no "never" threshold);
  *  RESIDENT one cooperative launch for all sweeps with neighbour-flag synchronisation (opt-in, large lattices);
+ *  SLAB     one cooperative launch for all sweeps of a call with the whole lattice resident in the shared memory of
+ *           one CTA per SM: slabs of march rows, boundary rows exchanged through L2 behind one progress flag per
+ *           CTA, interior updates overlap the exchange (L a power of two, up to 4096^2 / 128^3);
  *  GENERIC  one thread per site, any even L >= 4, any table.
  * All families produce bit-identical results (same random-word map D2, same thresholds D3). */
-enum { LSM_KERNEL_AUTO = 0, LSM_KERNEL_GENERIC = 1, LSM_KERNEL_TILED = 2, LSM_KERNEL_RESIDENT = 3, LSM_KERNEL_SMALL = 4 };
+enum { LSM_KERNEL_AUTO = 0, LSM_KERNEL_GENERIC = 1, LSM_KERNEL_TILED = 2, LSM_KERNEL_RESIDENT = 3, LSM_KERNEL_SMALL = 4,
+       LSM_KERNEL_SLAB = 5 };
 
 /* Device bytes lsm_create needs for this lattice (two colour arrays + small state). */
 int lsm_workspace_bytes(int dims, int L, int two_S, int model, size_t *bytes);

@@ -34,6 +34,7 @@ struct lsm {
     unsigned *d_flags;  // resident family: one progress word per CTA
     ResidentPlan plan;
     SmallPlan small;
+    SlabPlan slab;
     uint8_t *alt[2];    // NE models: second lattice buffer of the random-tile schedule (reading D18)
 };
 
@@ -136,6 +137,8 @@ static void choose_kernel(lsm *o)
     if (want == LSM_KERNEL_TILED && !tiled_ok) want = LSM_KERNEL_GENERIC;
     if (want == LSM_KERNEL_RESIDENT && !resident_plan(o->lat, o->model, o->tracking, o->tiled, &o->plan))
         want = tiled_ok ? LSM_KERNEL_TILED : LSM_KERNEL_GENERIC;
+    if (want == LSM_KERNEL_SLAB && !slab_plan(o->lat, o->model, o->tiled, &o->slab))
+        want = tiled_ok ? LSM_KERNEL_TILED : LSM_KERNEL_GENERIC;
     o->kernel_in_use = want;
 }
 
@@ -233,6 +236,9 @@ static int resident_launch(lsm *o, int64_t n, long long *obs, cudaStream_t s)
         int k = (int)(n < CHUNK ? n : CHUNK);
         if (o->kernel_in_use == LSM_KERNEL_SMALL) {
             CU(launch_sweep_small(o->lat, o->model, o->tracking, o->seed, o->t, k, obs, o->small, o->tiled, s));
+        } else if (o->kernel_in_use == LSM_KERNEL_SLAB) {
+            CU(cudaMemsetAsync(o->d_flags, 0, 4 * (size_t)o->slab.G, s));
+            CU(launch_sweep_slab(o->lat, o->model, o->tracking, o->seed, o->t, k, obs, o->d_flags, o->slab, o->tiled, s));
         } else {
             CU(cudaMemsetAsync(o->d_flags, 0, 8 * (size_t)o->plan.grid, s));
             CU(launch_sweep_resident(o->lat, o->model, o->tracking, o->seed, o->t, k, obs, o->d_flags, 0u, o->plan,
@@ -267,7 +273,8 @@ static int sweep_impl(lsm *o, int64_t n, long long *d_obs, cudaStream_t s)
 {
     o->last_stream = s;
     if (n == 0) return LSM_OK;
-    if (o->kernel_in_use == LSM_KERNEL_RESIDENT || o->kernel_in_use == LSM_KERNEL_SMALL) return sweep_resident(o, n, d_obs, s);
+    if (o->kernel_in_use == LSM_KERNEL_RESIDENT || o->kernel_in_use == LSM_KERNEL_SMALL || o->kernel_in_use == LSM_KERNEL_SLAB)
+        return sweep_resident(o, n, d_obs, s);
     if (d_obs) CU(cudaMemsetAsync(d_obs, 0, (size_t)n * 16, s));
     else CU(cudaMemsetAsync(o->d_run, 0, 16, s));
     for (int64_t k = 0; k < n; ++k) {
@@ -749,11 +756,12 @@ extern "C" int lsm_get_thresholds(lsm_t *o, uint64_t *out, int *count)
 
 extern "C" int lsm_set_kernel(lsm_t *o, int family)
 {
-    if (!o || family < LSM_KERNEL_AUTO || family > LSM_KERNEL_SMALL) return LSM_ERR_ARG;
+    if (!o || family < LSM_KERNEL_AUTO || family > LSM_KERNEL_SLAB) return LSM_ERR_ARG;
     if (family == LSM_KERNEL_TILED && !tiled_supported(o->lat, o->model, o->tiled)) return LSM_ERR_UNSUPPORTED;
     if (family == LSM_KERNEL_RESIDENT && !resident_plan(o->lat, o->model, o->tracking, o->tiled, &o->plan))
         return LSM_ERR_UNSUPPORTED;
     if (family == LSM_KERNEL_SMALL && !small_plan(o->lat, o->model, o->tiled, &o->small, true)) return LSM_ERR_UNSUPPORTED;
+    if (family == LSM_KERNEL_SLAB && !slab_plan(o->lat, o->model, o->tiled, &o->slab)) return LSM_ERR_UNSUPPORTED;
     o->kernel_pref = family;
     choose_kernel(o);
     return LSM_OK;

@@ -45,6 +45,14 @@ cudaError_t launch_sweep_small(const Lat &lat, int model, int track, unsigned lo
                                int nsweeps, long long *d_obs, const SmallPlan &plan, const TiledTables &t,
                                cudaStream_t s);
 
+// Slab family (lsm_slab.cu): one cooperative launch runs `nsweeps` whole sweeps with the lattice resident in the
+// shared memory of G CTAs (one per SM); boundary rows travel through L2 with one progress flag per CTA.
+struct SlabPlan { int G, rows_max, threads, smem; };
+bool slab_plan(const Lat &lat, int model, const TiledTables &t, SlabPlan *out);
+cudaError_t launch_sweep_slab(const Lat &lat, int model, int track, unsigned long long seed, unsigned long long t0,
+                              int nsweeps, long long *d_obs, unsigned *d_flags, const SlabPlan &plan, const TiledTables &t,
+                              cudaStream_t s);
+
 // Batch of R same-shape lattices (lsm_batch_*): one launch of the small family's lane kernel, one cluster per replica.
 struct BatchDesc {               // per replica, in device memory
     uint8_t *col[2];

@@ -88,7 +88,7 @@ SHAPES = [
     (dict(dims=2, L=1024, model=lsm.NE_HEATBATH, J=0.0, T=W.ne_temperature(0.3)), 16),
     (dict(dims=2, L=3072, model=lsm.NE_METROPOLIS, J=0.0, T=W.ne_temperature(0.2)), 6),
 ]
-FAMILIES = [lsm.KERNEL_GENERIC, lsm.KERNEL_TILED, lsm.KERNEL_RESIDENT, lsm.KERNEL_SMALL]
+FAMILIES = [lsm.KERNEL_GENERIC, lsm.KERNEL_TILED, lsm.KERNEL_RESIDENT, lsm.KERNEL_SMALL, lsm.KERNEL_SLAB]
 
 
 def test_device_philox_known_answers_and_random():
