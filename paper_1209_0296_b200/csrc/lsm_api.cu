@@ -35,6 +35,8 @@ struct lsm {
     ResidentPlan plan;
     SmallPlan small;
     SlabPlan slab;
+    uint32_t *d_mbox;   // slab family: mailbox rows at the end of the workspace (nullptr: shape not covered)
+    size_t mbox_bytes;
     uint8_t *alt[2];    // NE models: second lattice buffer of the random-tile schedule (reading D18)
 };
 
@@ -64,6 +66,13 @@ static int check_shape(int dims, int L, int two_S, int model)
     return LSM_OK;
 }
 
+static int internal_model(int model, int two_S)
+{
+    return model == LSM_ISING ? (two_S == 1 ? M_ISING_HALF : M_ISING_ONE)
+         : model == LSM_EA ? M_EA : model == LSM_POTTS ? M_POTTS
+         : (model == LSM_NE_HEATBATH ? M_NE_HEATBATH : M_NE_METROPOLIS);
+}
+
 extern "C" int lsm_workspace_bytes(int dims, int L, int two_S, int model, size_t *bytes)
 {
     if (!bytes) return LSM_ERR_ARG;
@@ -73,6 +82,7 @@ extern "C" int lsm_workspace_bytes(int dims, int L, int two_S, int model, size_t
     *bytes = STATE_BYTES + 2 * align256(N / 2) + 256;
     if (model == LSM_NE_HEATBATH || model == LSM_NE_METROPOLIS) *bytes += 2 * align256(N / 2);   // second buffer of the random-tile schedule
     if (model == LSM_EA) *bytes += 2 * align256(N / 2);      // bond bytes of the two colours
+    *bytes += align256(slab_mailbox_bytes(dims, L, internal_model(model, two_S)));   // slab family: boundary-row mailboxes
     return LSM_OK;
 }
 
@@ -166,9 +176,7 @@ extern "C" int lsm_create(int dims, int L, int two_S, int model, double J, doubl
     lsm *o = new (std::nothrow) lsm();
     if (!o) return LSM_ERR_ARG;
     o->dims = dims; o->L = L; o->two_S = two_S; o->model_abi = model;
-    o->model = model == LSM_ISING ? (two_S == 1 ? M_ISING_HALF : M_ISING_ONE)
-             : model == LSM_EA ? M_EA : model == LSM_POTTS ? M_POTTS
-             : (model == LSM_NE_HEATBATH ? M_NE_HEATBATH : M_NE_METROPOLIS);
+    o->model = internal_model(model, two_S);
     o->J = J; o->h = h; o->T = T; o->c = 0.0; o->seed = seed;
     o->N = (int64_t)L * L * (dims == 3 ? L : 1);
     uint8_t *base = (uint8_t *)d_workspace;
@@ -188,6 +196,8 @@ extern "C" int lsm_create(int dims, int L, int two_S, int model, double J, doubl
         o->lat.bnd[0] = o->lat.col[1] + align256((size_t)o->N / 2);
         o->lat.bnd[1] = o->lat.bnd[0] + align256((size_t)o->N / 2);
     }
+    o->mbox_bytes = slab_mailbox_bytes(dims, L, o->model);
+    o->d_mbox = o->mbox_bytes ? (uint32_t *)(base + need - align256(o->mbox_bytes)) : nullptr;
     o->lat.L = L; o->lat.Lh = L / 2; o->lat.dims = dims; o->lat.Lz = dims == 3 ? L : 1;
     o->lat.half = o->N / 2;
     o->t = 0; o->tracking = 1; o->kernel_pref = LSM_KERNEL_AUTO; o->launches = 0;
@@ -237,8 +247,8 @@ static int resident_launch(lsm *o, int64_t n, long long *obs, cudaStream_t s)
         if (o->kernel_in_use == LSM_KERNEL_SMALL) {
             CU(launch_sweep_small(o->lat, o->model, o->tracking, o->seed, o->t, k, obs, o->small, o->tiled, s));
         } else if (o->kernel_in_use == LSM_KERNEL_SLAB) {
-            CU(cudaMemsetAsync(o->d_flags, 0, 4 * (size_t)o->slab.G, s));
-            CU(launch_sweep_slab(o->lat, o->model, o->tracking, o->seed, o->t, k, obs, o->d_flags, o->slab, o->tiled, s));
+            CU(cudaMemsetAsync(o->d_mbox, 0x80, o->mbox_bytes, s));     // every mailbox lane: sweep parity 1 (lsm_slab.cu)
+            CU(launch_sweep_slab(o->lat, o->model, o->tracking, o->seed, o->t, k, obs, o->d_mbox, o->slab, o->tiled, s));
         } else {
             CU(cudaMemsetAsync(o->d_flags, 0, 8 * (size_t)o->plan.grid, s));
             CU(launch_sweep_resident(o->lat, o->model, o->tracking, o->seed, o->t, k, obs, o->d_flags, 0u, o->plan,

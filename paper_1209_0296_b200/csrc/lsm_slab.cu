@@ -1,5 +1,5 @@
-// lsm_slab.cu -- the slab family for mid-size lattices (1024^2 ... 4096^2, 128^3 ... 256^3): ONE launch runs many
-// sweeps and the whole lattice lives in the shared memory of the 148 SMs.
+// lsm_slab.cu -- the slab family for mid-size lattices (1024^2 ... 4096^2, 128^3): ONE launch runs many sweeps and
+// the whole lattice lives in the shared memory of the 148 SMs.
 //
 // The paper ends the kernel after every half-sweep because that was its only grid-wide barrier and
 // reports what that costs on small lattices.  On B200 a dependent launch costs ~2.5-3 us, a half-sweep of
@@ -8,18 +8,19 @@
 //   * the lattice is cut into G slabs of march rows (y in 2D, z planes in 3D), one per CTA, one CTA per SM, all
 //     co-resident (cooperative launch); a CTA keeps its slab of BOTH colours in shared memory for the whole launch,
 //     plus one halo row of each colour below and above;
-//   * k sweeps = 2k half-sweeps run inside the launch.  In a half-sweep a CTA first updates its two BOUNDARY rows,
-//     stores them to the lattice in global memory (their home address: L2 is the mailbox) and publishes a progress
-//     flag; then it updates its interior rows while the flag and the rows travel.  Before the next half-sweep it
-//     waits for the flags of the two adjacent slabs only and copies their fresh boundary rows into its halo;
-//   * nothing else touches global memory until the slab is written back at the end of the launch.
-// The barrier between the colours thus becomes a point-to-point dependency on two neighbours whose
-// latency overlaps the interior update.  Same rules, same Philox counters (group = lane index in the colour array) as
-// every other family: bit-identical results.
+//   * k sweeps = 2k half-sweeps run inside the launch.  In a half-sweep a CTA updates its two BOUNDARY rows first and
+//     stores them into its mailbox in global memory (L2), then its interior rows; before the next half-sweep it
+//     copies the fresh boundary rows of the two adjacent slabs from their mailboxes into its halo;
+//   * the mailbox words validate themselves: bit 31 of every 32-bit lane (bit 7 of a site byte is unused by every
+//     encoding, lsm_internal.cuh) carries the parity of the sweep that wrote it, the reader spins on each lane until
+//     the parity is the one it expects.  No flag, no fence, no barrier beyond the CTA's own: the barrier between the
+//     colours has become a point-to-point dependency on two neighbours that costs one L2 round trip.
+// Same rules, same Philox counters (group = lane index in the colour array) as every other family: bit-identical.
 //
-// Write-after-read on the global boundary rows: a CTA rewrites its colour-c boundary rows in half-sweep h + 2; the
-// neighbour read version h at the start of its half-sweep h + 1 and flagged h + 2 only after that; the CTA waits for
-// that flag before it starts half-sweep h + 2.  So one copy of each row is enough.
+// Why one mailbox row per (CTA, side, colour) is enough: a CTA rewrites its colour-c rows in half-sweep h + 2.  To
+// start h + 2 it needs the neighbours' rows of half-sweep h + 1, and a neighbour computes those only after it has
+// copied this CTA's rows of half-sweep h.  The host sets every mailbox lane to parity 1 before a launch; sweep k of
+// the launch writes parity k & 1.
 #include "lsm_tiled_dev.cuh"
 
 #include <cstring>
@@ -36,25 +37,25 @@ struct SlabArgs {
     int rows_max;                // most march rows of any slab (shared-memory stride)
     int one;
     long long *obs;              // [nsweeps][2] (B, M) slots zeroed by the host, or nullptr
-    unsigned *flags;             // [G] half-sweeps whose boundary rows are published; zero when the launch starts
+    uint32_t *mbox;              // [G][first, last][colour][lanes of a march row]; every lane 0x80808080 at launch
 };
 
-__device__ __forceinline__ unsigned slab_ld_acquire(const unsigned *p)
-{
-    unsigned v;
-    asm volatile("ld.acquire.gpu.global.u32 %0, [%1];" : "=r"(v) : "l"(p) : "memory");
-    return v;
-}
-__device__ __forceinline__ void slab_st_release(unsigned *p, unsigned v)
-{
-    asm volatile("st.release.gpu.global.u32 [%0], %1;" ::"l"(p), "r"(v) : "memory");
-}
-// L2-coherent load of a word another CTA stored during this launch (never served from this SM's L1)
 __device__ __forceinline__ uint32_t slab_ld_l2(const uint32_t *p)
 {
     uint32_t v;
     asm volatile("ld.relaxed.gpu.global.u32 %0, [%1];" : "=r"(v) : "l"(p) : "memory");
     return v;
+}
+__device__ __forceinline__ void slab_st_l2(uint32_t *p, uint32_t v)
+{
+    asm volatile("st.relaxed.gpu.global.u32 [%0], %1;" ::"l"(p), "r"(v) : "memory");
+}
+// spin until the lane carries the expected sweep parity in bit 31; returns the lane without it
+__device__ __forceinline__ uint32_t slab_take(const uint32_t *p, uint32_t tag31)
+{
+    uint32_t v;
+    do { v = slab_ld_l2(p); } while (((v ^ tag31) & 0x80000000u) != 0u);
+    return v & 0x7FFFFFFFu;
 }
 
 template <int MODEL, int DIMS, bool TRACK, int OBS, bool NEV>
@@ -96,53 +97,74 @@ k_sweep_slab(const __grid_constant__ SlabArgs a, const __grid_constant__ PhiloxS
     const uint32_t mb = (uint32_t)((m0 == 0 ? a.L : m0) - 1), ma = (uint32_t)(m1 == a.L ? 0 : m1);
     const int g_below = g == 0 ? G - 1 : g - 1, g_above = g + 1 == G ? 0 : g + 1;
 
-    // the slab: local march row 0 = halo below, 1 ... rows = own rows, rows + 1 = halo above
+    // the slab in shared memory: local march row 1 ... rows (rows 0 and rows + 1 of the layout are spare)
     for (uint32_t i = tid; i < (rows << lg_row); i += nthr) {
         s_col[0][rowl + i] = a.col[0][((uint32_t)m0 << lg_row) + i];
         s_col[1][rowl + i] = a.col[1][((uint32_t)m0 << lg_row) + i];
     }
-    for (uint32_t i = tid; i < rowl; i += nthr) {               // half-sweep 0 reads colour 1 as it was at launch
-        s_col[1][i] = a.col[1][(mb << lg_row) + i];
-        s_col[1][((rows + 1) << lg_row) + i] = a.col[1][(ma << lg_row) + i];
-    }
     __syncthreads();
+
+    // mailbox rows: [cta][0 = first row, 1 = last row][colour]
+    auto mbox_row = [&](int cta, int which, int colour) { return a.mbox + ((size_t)((cta * 2 + which) * 2 + colour) << lg_row); };
 
     int thrB = 0, thrM = 0;
     const int nhalves = 2 * a.nsweeps;
+    const uint32_t total = rows << lg_row, nA = (rows >= 2u ? 2u : 1u) << lg_row;
+    auto flush_obs = [&](int sw) {                         // thread 0, after a barrier behind the sweep's last add
+        const int vB = sm.acc[sw & 1][0], vM = sm.acc[sw & 1][1];
+        if (vB != 0) atomicAdd((unsigned long long *)&a.obs[2 * sw], (unsigned long long)(long long)vB);
+        if (vM != 0) atomicAdd((unsigned long long *)&a.obs[2 * sw + 1], (unsigned long long)(long long)vM);
+        sm.acc[sw & 1][0] = 0;                             // next used by sweep sw + 2: several barriers away
+        sm.acc[sw & 1][1] = 0;
+    };
 #pragma unroll 1
     for (int gh = 0; gh < nhalves; ++gh) {
         const int half = gh & 1, sw = gh >> 1;
         uint32_t *const own = s_col[half];
         uint32_t *const oth = s_col[half ^ 1];
-        uint32_t *const g_own = a.col[half];
         if (gh > 0) {
-            // the adjacent slabs have published the boundary rows of half-sweep gh - 1 (the colour read now)
-            if (tid < 2) {
-                const unsigned *w = a.flags + (tid ? g_above : g_below);
-                while ((int)(slab_ld_acquire(w) - (unsigned)gh) < 0) { }
-            }
-            __syncthreads();
-            const uint32_t *const g_oth = a.col[half ^ 1];
-            for (uint32_t i = tid; i < rowl; i += nthr) {
-                oth[i] = slab_ld_l2(g_oth + (mb << lg_row) + i);
-                oth[((rows + 1) << lg_row) + i] = slab_ld_l2(g_oth + (ma << lg_row) + i);
-            }
-            __syncthreads();
+            __syncthreads();                               // the previous half-sweep's rows of this slab are complete
+            if (OBS >= 1 && half == 0 && tid == 0) flush_obs(sw - 1);
         }
+        // The rows of the adjacent slabs that touch this one: written by their owners in half-sweep gh - 1 (mailbox,
+        // sweep parity in bit 31), or the lattice as the launch found it (gh = 0).  A boundary lane needs exactly one
+        // lane of them (the same lane index), so the thread that updates it spins on that lane itself.
+        const uint32_t tag31 = (uint32_t)((gh - 1) >> 1) << 31;
+        const uint32_t *const below = gh ? mbox_row(g_below, 1, half ^ 1) : a.col[1] + (mb << lg_row);
+        const uint32_t *const above = gh ? mbox_row(g_above, 0, half ^ 1) : a.col[1] + (ma << lg_row);
         const unsigned long long t = a.t0 + (unsigned long long)sw;
         PhiloxDyn pc = {0u, 0u, 0u, 0u, pk};
         philox_half_consts(make_sweep_key(a.seed, t, (uint32_t)half), pk.rk0, pk.rk1, pc.x1, pc.y2, pc.z2, pc.w3);
         int totU = 0, totBN = 0, totS = 0, nsites = 0;
         if (half == 0) thrB = thrM = 0;
+        const uint32_t wtag = (uint32_t)(sw & 1) << 31;
+        uint32_t *const mb_first = mbox_row(g, 0, half), *const mb_last = mbox_row(g, 1, half);
 
-        // one 32-bit lane (4 sites, one Philox call; spin-1: two): local march row ml, lane r of the march row
-        auto lane = [&](const uint32_t ml, const uint32_t r, const bool edge) {
+        // Lanes of the slab in the order boundary rows (1 and `rows`), then interior rows: the adjacent slabs wait for
+        // the former, so every thread takes them first.  One lane = 4 sites, one Philox call (spin-1: two).
+#pragma unroll 1
+        for (uint32_t i = tid; i < total; i += nthr) {
+            const bool edge = i < nA;
+            const uint32_t ml = edge ? ((i >> lg_row) ? rows : 1u) : 2u + ((i - nA) >> lg_row);
+            const uint32_t r = i & (rowl - 1);
             const uint32_t x = r & (lpr - 1), y = r >> lg_lpr;
             const uint32_t m = (uint32_t)m0 + ml - 1u;
             const uint32_t qq = (m + y + (uint32_t)half) & 1u;
             const uint32_t li = (ml << lg_row) + r;
+            const uint32_t gl = (m << lg_row) + r;              // lane index in the colour array = Philox group (D2)
+            // the random words do not depend on the neighbours: drawn before a boundary lane waits for its halo lane
+            uint4 rw = make_uint4(0u, 0u, 0u, 0u), rw2 = rw;
+            if (MODEL == M_ISING_HALF) rw = philox_sweep(gl, pc);
+            if (MODEL == M_ISING_ONE) {
+                rw = philox_sweep(2u * gl, pc);
+                rw2 = philox_sweep(2u * gl + 1u, pc);
+            }
             const uint32_t c = oth[li], o = own[li];
-            const uint32_t p = oth[li - rowl], n = oth[li + rowl];
+            uint32_t p, n;
+            if (ml == 1u) p = gh ? slab_take(below + r, tag31) : below[r];
+            else p = oth[li - rowl];
+            if (ml == rows) n = gh ? slab_take(above + r, tag31) : above[r];
+            else n = oth[li + rowl];
             const uint32_t cs = oth[(li - x) + ((qq ? x + 1u : x - 1u) & (lpr - 1))];
             const uint32_t sd = qq ? __funnelshift_r(c, cs, 8) : __funnelshift_r(cs, c, 24);
             uint32_t yp = 0, yn = 0;
@@ -150,12 +172,11 @@ k_sweep_slab(const __grid_constant__ SlabArgs a, const __grid_constant__ PhiloxS
                 yp = oth[(ml << lg_row) + (((y - 1u) & (R - 1)) << lg_lpr) + x];
                 yn = oth[(ml << lg_row) + (((y + 1u) & (R - 1)) << lg_lpr) + x];
             }
-            const uint32_t gl = (m << lg_row) + r;              // lane index in the colour array = Philox group (D2)
             uint32_t out;
             if (MODEL == M_ISING_HALF) {
                 uint32_t ns = p + n + c + sd;
                 if (DIMS == 3) ns += yp + yn;
-                out = rule_half<TRACK, OBS, NEV>(o, ns, philox_sweep(gl, pc), s_t, (uint32_t)a.one, totU, totBN);
+                out = rule_half<TRACK, OBS, NEV>(o, ns, rw, s_t, (uint32_t)a.one, totU, totBN);
             } else if (MODEL == M_ISING_ONE) {
                 uint32_t ns;
                 if (TRACK) {
@@ -165,32 +186,18 @@ k_sweep_slab(const __grid_constant__ SlabArgs a, const __grid_constant__ PhiloxS
                     ns = p + n + c + sd;
                     if (DIMS == 3) ns += yp + yn;
                 }
-                out = rule_one<DIMS, TRACK, OBS, NEV>(o, ns, philox_sweep(2u * gl, pc), philox_sweep(2u * gl + 1u, pc), s_t,
-                                                      (uint32_t)a.one, totU, totBN, totS);
+                out = rule_one<DIMS, TRACK, OBS, NEV>(o, ns, rw, rw2, s_t, (uint32_t)a.one, totU, totBN, totS);
             } else {
                 uint32_t accU = 0;
                 out = rule_ne<TRACK, MODEL == M_NE_METROPOLIS, OBS>(o, n, qq ? sd : c, gl, pc, ne_t32, ne_always, accU);
                 if (OBS >= 1) totU += (int)bytesum(accU);
             }
             own[li] = out;
-            if (edge) g_own[gl] = out;
+            if (edge) {
+                if (ml == 1u) slab_st_l2(mb_first + r, out | wtag);
+                if (ml == rows) slab_st_l2(mb_last + r, out | wtag);
+            }
             nsites += 4;
-        };
-
-        // boundary rows first: the adjacent slabs wait for them
-        const uint32_t nA = (rows >= 2u ? 2u : 1u) << lg_row;
-#pragma unroll 1
-        for (uint32_t i = tid; i < nA; i += nthr) lane((i >> lg_row) ? rows : 1u, i & (rowl - 1), true);
-        __syncthreads();
-        if (tid == 0) {
-            __threadfence();
-            slab_st_release(a.flags + g, (unsigned)gh + 1u);
-        }
-        // interior rows while the flag travels
-        if (rows > 2u) {
-            const uint32_t nB = (rows - 2u) << lg_row;
-#pragma unroll 1
-            for (uint32_t i = tid; i < nB; i += nthr) lane(2u + (i >> lg_row), i & (rowl - 1), false);
         }
         if (OBS >= 1) {
             March<MODEL, DIMS, TRACK, OBS, NEV> M;         // only the per-thread sums are used
@@ -209,21 +216,13 @@ k_sweep_slab(const __grid_constant__ SlabArgs a, const __grid_constant__ PhiloxS
                 }
             }
         }
-        __syncthreads();                                   // this CTA's rows of the colour are complete
-        if (OBS >= 1 && half == 1 && tid == 0) {
-            const int vB = sm.acc[sw & 1][0], vM = sm.acc[sw & 1][1];
-            if (vB != 0) atomicAdd((unsigned long long *)&a.obs[2 * sw], (unsigned long long)(long long)vB);
-            if (vM != 0) atomicAdd((unsigned long long *)&a.obs[2 * sw + 1], (unsigned long long)(long long)vM);
-            sm.acc[sw & 1][0] = 0;                         // next used by sweep sw + 2: several barriers away
-            sm.acc[sw & 1][1] = 0;
-        }
     }
-    // write the interior rows back (the boundary rows went out when they were last updated)
-    if (rows > 2u) {
-        for (uint32_t i = tid; i < ((rows - 2u) << lg_row); i += nthr) {
-            a.col[0][(((uint32_t)m0 + 1u) << lg_row) + i] = s_col[0][2u * rowl + i];
-            a.col[1][(((uint32_t)m0 + 1u) << lg_row) + i] = s_col[1][2u * rowl + i];
-        }
+    __syncthreads();
+    if (OBS >= 1 && nhalves > 0 && tid == 0) flush_obs(a.nsweeps - 1);
+    // write the slab back
+    for (uint32_t i = tid; i < total; i += nthr) {
+        a.col[0][((uint32_t)m0 << lg_row) + i] = s_col[0][rowl + i];
+        a.col[1][((uint32_t)m0 << lg_row) + i] = s_col[1][rowl + i];
     }
 }
 
@@ -243,17 +242,26 @@ static int slab_ilog2(long long v)
 #define LSM_SLAB_SMEM_MAX (220 * 1024)     // dynamic shared memory per CTA (227 KB opt-in minus the static part)
 #endif
 
+// Mailbox bytes reserved in the workspace for this shape (0: the slab family never runs it).  Depends on the shape
+// only, so that lsm_workspace_bytes needs no device: SLAB_MAX_CTAS slabs x (first, last) x 2 colours x one march row.
+size_t slab_mailbox_bytes(int dims, int L, int model)
+{
+    if (model != M_ISING_HALF && model != M_ISING_ONE && model != M_NE_HEATBATH && model != M_NE_METROPOLIS) return 0;
+    if ((L & (L - 1)) != 0) return 0;                                 // lane index math by shifts
+    if (dims == 2 ? (L < 512 || L > 4096) : (L < 64 || L > 128)) return 0;   // below: the small family; above: does not fit
+    const size_t rowbytes = (size_t)(L / 2) * (dims == 3 ? (size_t)L : 1);
+    return (size_t)SLAB_MAX_CTAS * 4 * rowbytes;
+}
+
 bool slab_plan(const Lat &lat, int model, const TiledTables &t, SlabPlan *out)
 {
     if (!t.usable) return false;
-    if (model != M_ISING_HALF && model != M_ISING_ONE && model != M_NE_HEATBATH && model != M_NE_METROPOLIS) return false;
-    if (lat.L < 32 || (lat.L & (lat.L - 1)) != 0) return false;      // lane index math by shifts
-    const long long N = 2 * lat.half;
-    if (N > (1ll << 25)) return false;
+    if (slab_mailbox_bytes(lat.dims, lat.L, model) == 0) return false;
     int coop = 0, dev = 0;
     if (cudaGetDevice(&dev) != cudaSuccess) return false;
     if (cudaDeviceGetAttribute(&coop, cudaDevAttrCooperativeLaunch, dev) != cudaSuccess || !coop) return false;
     int G = sm_count();                                               // one CTA per SM, all co-resident
+    if (G > SLAB_MAX_CTAS) G = SLAB_MAX_CTAS;
     if (G > lat.L) G = lat.L;
     if (G < 2) return false;
     const int rows_max = (lat.L + G - 1) / G;
@@ -296,9 +304,9 @@ static cudaError_t slab_launch_to(bool track, bool obs, const SlabPlan &plan, cu
     return obs ? go(k_sweep_slab<MODEL, DIMS, false, 2, false>) : go(k_sweep_slab<MODEL, DIMS, false, 0, false>);
 }
 
-// d_flags: plan.G words, zeroed by the caller on the same stream before this launch.
+// d_mbox: slab_mailbox_bytes() bytes, every byte set to 0x80 by the caller on the same stream before this launch.
 cudaError_t launch_sweep_slab(const Lat &lat, int model, int track, unsigned long long seed, unsigned long long t0,
-                              int nsweeps, long long *d_obs, unsigned *d_flags, const SlabPlan &plan, const TiledTables &t,
+                              int nsweeps, long long *d_obs, uint32_t *d_mbox, const SlabPlan &plan, const TiledTables &t,
                               cudaStream_t s)
 {
     SlabArgs a;
@@ -315,7 +323,7 @@ cudaError_t launch_sweep_slab(const Lat &lat, int model, int track, unsigned lon
     a.rows_max = plan.rows_max;
     a.one = 1;
     a.obs = d_obs;
-    a.flags = d_flags;
+    a.mbox = d_mbox;
     PhiloxSweepConsts pk = make_philox_consts(make_sweep_key(seed, t0, 0u));   // only the round keys are used
     const bool obs = d_obs != nullptr, tr = track != 0;
     switch (model) {

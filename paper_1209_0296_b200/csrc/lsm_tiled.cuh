@@ -46,11 +46,13 @@ cudaError_t launch_sweep_small(const Lat &lat, int model, int track, unsigned lo
                                cudaStream_t s);
 
 // Slab family (lsm_slab.cu): one cooperative launch runs `nsweeps` whole sweeps with the lattice resident in the
-// shared memory of G CTAs (one per SM); boundary rows travel through L2 with one progress flag per CTA.
+// shared memory of G CTAs (one per SM); boundary rows travel through self-validating mailbox words in L2.
 struct SlabPlan { int G, rows_max, threads, smem; };
+constexpr int SLAB_MAX_CTAS = 192;                                   // mailbox rows reserved in the workspace
+size_t slab_mailbox_bytes(int dims, int L, int model);               // internal Model id; 0: shape not covered
 bool slab_plan(const Lat &lat, int model, const TiledTables &t, SlabPlan *out);
 cudaError_t launch_sweep_slab(const Lat &lat, int model, int track, unsigned long long seed, unsigned long long t0,
-                              int nsweeps, long long *d_obs, unsigned *d_flags, const SlabPlan &plan, const TiledTables &t,
+                              int nsweeps, long long *d_obs, uint32_t *d_mbox, const SlabPlan &plan, const TiledTables &t,
                               cudaStream_t s);
 
 // Batch of R same-shape lattices (lsm_batch_*): one launch of the small family's lane kernel, one cluster per replica.
