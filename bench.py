@@ -484,6 +484,20 @@ def size_scan():
             torch.cuda.synchronize()
             ms = e0.elapsed_time(e1)
             row[name] = {"us_per_sweep": ms * 1e3 / n, "gflips": lat.N * n / ms / 1e6}
+            if fam == lsm.KERNEL_SLAB:                   # temporal depth: half-sweeps between two boundary exchanges
+                row[name]["depth"] = lat.temporal_depth
+                for depth in (1, 2, 3, 4):
+                    try:
+                        lat.set_temporal_depth(depth)
+                    except lsm.LsmError:
+                        break
+                    lat.sweep_record(n, out=obs)
+                    torch.cuda.synchronize()
+                    e0.record()
+                    lat.sweep_record(n, out=obs)
+                    e1.record()
+                    torch.cuda.synchronize()
+                    row[name][f"gflips_depth{depth}"] = lat.N * n / e0.elapsed_time(e1) / 1e6
             lat.close()
         lat = lsm.Lattice(dims=dims, L=L, T=2.269 if dims == 2 else 4.5115, seed=3)
         row["auto_family"] = KERNEL_FAMILY.get(lat.kernel)

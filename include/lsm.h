@@ -221,6 +221,13 @@ int lsm_get_thresholds(lsm_t *, uint64_t *out, int *count);
 
 int lsm_set_kernel(lsm_t *, int kernel_family);           /* LSM_KERNEL_*; UNSUPPORTED if it cannot run this lattice */
 int lsm_get_kernel(lsm_t *, int *kernel_family_in_use);
+/* Temporal blocking of the SLAB family (the barrier between the colours is
+ * what small lattices cannot afford): `depth` half-sweeps run between two exchanges of boundary rows, each slab
+ * updating depth-1-j halo rows on either side redundantly in step j (reproducible: the random words are a function
+ * of (seed, sweep, colour, site), D2).  0 = the default for the shape; 1 = no redundant update; at most 4 (L <= 1024),
+ * 2 (L = 2048), 1 (otherwise): UNSUPPORTED beyond.  Results do not depend on it.  get: depth in use (0 unless SLAB). */
+int lsm_set_temporal_depth(lsm_t *, int depth);
+int lsm_get_temporal_depth(lsm_t *, int *depth_in_use);
 int lsm_get_launch_count(lsm_t *, uint64_t *kernels_launched); /* kernels this handle has enqueued */
 
 /* Host-side derived doubles from the integer series (D11-D13), exact integer accumulation. */

@@ -37,6 +37,7 @@ struct lsm {
     SlabPlan slab;
     uint32_t *d_mbox;   // slab family: mailbox rows at the end of the workspace (nullptr: shape not covered)
     size_t mbox_bytes;
+    int slab_depth;     // requested temporal depth of the slab family (0: default)
     uint8_t *alt[2];    // NE models: second lattice buffer of the random-tile schedule (reading D18)
 };
 
@@ -147,7 +148,7 @@ static void choose_kernel(lsm *o)
     if (want == LSM_KERNEL_TILED && !tiled_ok) want = LSM_KERNEL_GENERIC;
     if (want == LSM_KERNEL_RESIDENT && !resident_plan(o->lat, o->model, o->tracking, o->tiled, &o->plan))
         want = tiled_ok ? LSM_KERNEL_TILED : LSM_KERNEL_GENERIC;
-    if (want == LSM_KERNEL_SLAB && !slab_plan(o->lat, o->model, o->tiled, &o->slab))
+    if (want == LSM_KERNEL_SLAB && !slab_plan(o->lat, o->model, o->tiled, o->slab_depth, &o->slab))
         want = tiled_ok ? LSM_KERNEL_TILED : LSM_KERNEL_GENERIC;
     o->kernel_in_use = want;
 }
@@ -200,7 +201,7 @@ extern "C" int lsm_create(int dims, int L, int two_S, int model, double J, doubl
     o->d_mbox = o->mbox_bytes ? (uint32_t *)(base + need - align256(o->mbox_bytes)) : nullptr;
     o->lat.L = L; o->lat.Lh = L / 2; o->lat.dims = dims; o->lat.Lz = dims == 3 ? L : 1;
     o->lat.half = o->N / 2;
-    o->t = 0; o->tracking = 1; o->kernel_pref = LSM_KERNEL_AUTO; o->launches = 0;
+    o->t = 0; o->tracking = 1; o->kernel_pref = LSM_KERNEL_AUTO; o->launches = 0; o->slab_depth = 0;
     o->last_stream = (cudaStream_t)stream;
     build_tables(o);
     choose_kernel(o);
@@ -771,9 +772,25 @@ extern "C" int lsm_set_kernel(lsm_t *o, int family)
     if (family == LSM_KERNEL_RESIDENT && !resident_plan(o->lat, o->model, o->tracking, o->tiled, &o->plan))
         return LSM_ERR_UNSUPPORTED;
     if (family == LSM_KERNEL_SMALL && !small_plan(o->lat, o->model, o->tiled, &o->small, true)) return LSM_ERR_UNSUPPORTED;
-    if (family == LSM_KERNEL_SLAB && !slab_plan(o->lat, o->model, o->tiled, &o->slab)) return LSM_ERR_UNSUPPORTED;
+    if (family == LSM_KERNEL_SLAB && !slab_plan(o->lat, o->model, o->tiled, o->slab_depth, &o->slab)) return LSM_ERR_UNSUPPORTED;
     o->kernel_pref = family;
     choose_kernel(o);
+    return LSM_OK;
+}
+
+extern "C" int lsm_set_temporal_depth(lsm_t *o, int depth)
+{
+    if (!o || depth < 0) return LSM_ERR_ARG;
+    if (depth > slab_depth_max(o->dims, o->L, o->model)) return LSM_ERR_UNSUPPORTED;
+    o->slab_depth = depth;
+    choose_kernel(o);
+    return LSM_OK;
+}
+
+extern "C" int lsm_get_temporal_depth(lsm_t *o, int *depth)
+{
+    if (!o || !depth) return LSM_ERR_ARG;
+    *depth = o->kernel_in_use == LSM_KERNEL_SLAB ? o->slab.D : 0;
     return LSM_OK;
 }
 

@@ -1,28 +1,33 @@
-// lsm_slab.cu -- the slab family for mid-size lattices (1024^2 ... 4096^2, 128^3): ONE launch runs many sweeps and
-// the whole lattice lives in the shared memory of the 148 SMs.
+// lsm_slab.cu -- the slab family for mid-size lattices (512^2 ... 4096^2, 64^3, 128^3): ONE launch runs many sweeps,
+// the whole lattice lives in the shared memory of the SMs, and several half-sweeps run between two exchanges
+// (temporal blocking with redundant halo updates).
 //
 // The paper ends the kernel after every half-sweep because that was its only grid-wide barrier and
 // reports what that costs on small lattices.  On B200 a dependent launch costs ~2.5-3 us, a half-sweep of
 // 1024^2 is 0.45 us of work: the tiled family reaches 13 % (1024^2) to 40 % (2048^2) of its large-lattice rate there.
 // A lattice of up to ~28 MB fits the shared memory of the whole GPU, and a site reads nearest neighbours only, so:
 //   * the lattice is cut into G slabs of march rows (y in 2D, z planes in 3D), one per CTA, one CTA per SM, all
-//     co-resident (cooperative launch); a CTA keeps its slab of BOTH colours in shared memory for the whole launch,
-//     plus one halo row of each colour below and above;
-//   * k sweeps = 2k half-sweeps run inside the launch.  In a half-sweep a CTA updates its two BOUNDARY rows first and
-//     stores them into its mailbox in global memory (L2), then its interior rows; before the next half-sweep it
-//     copies the fresh boundary rows of the two adjacent slabs from their mailboxes into its halo;
-//   * the mailbox words validate themselves: bit 31 of every 32-bit lane (bit 7 of a site byte is unused by every
-//     encoding, lsm_internal.cuh) carries the parity of the sweep that wrote it, the reader spins on each lane until
-//     the parity is the one it expects.  No flag, no fence, no barrier beyond the CTA's own: the barrier between the
-//     colours has become a point-to-point dependency on two neighbours that costs one L2 round trip.
-// Same rules, same Philox counters (group = lane index in the colour array) as every other family: bit-identical.
-//
-// Why one mailbox row per (CTA, side, colour) is enough: a CTA rewrites its colour-c rows in half-sweep h + 2.  To
-// start h + 2 it needs the neighbours' rows of half-sweep h + 1, and a neighbour computes those only after it has
-// copied this CTA's rows of half-sweep h.  The host sets every mailbox lane to parity 1 before a launch; sweep k of
-// the launch writes parity k & 1.
+//     co-resident (cooperative launch).  A CTA keeps its slab of BOTH colours in shared memory for the whole launch,
+//     plus D halo rows of each colour below and above (D = temporal depth);
+//   * time runs in epochs of D half-sweeps.  At the start of an epoch the halo holds the D adjacent rows of both
+//     neighbours as of that time.  Step j of the epoch updates the slab's own rows AND the D-1-j nearest halo rows on
+//     either side: a halo update is exactly the update its owner makes (same neighbours, same Philox counter =
+//     lane index in the colour array, same table), so it is reproduced rather than communicated.  After D steps
+//     the own rows are exact and the halo is used up;
+//   * exchange: while it makes the last two steps of an epoch a CTA stores the first and the last D of its own rows
+//     (of the colour updated in that step) into its mailbox in global memory (L2); the adjacent CTAs copy them into
+//     their halos at the start of the next epoch.  Mailbox lanes validate themselves: bit 31 of every 32-bit lane
+//     (bit 7 of a site byte is unused by every encoding, lsm_internal.cuh) carries one bit of the epoch number and the
+//     reader spins on each lane until it shows the expected one -- no flag, no fence.  One exchange costs about one
+//     microsecond of latency on B200 whatever its size, which is why it pays to make it once per D half-sweeps;
+//   * D = 1 is the plain scheme (one row of the colour just updated per half-sweep, no redundant update).
+// Mailboxes are double-buffered by epoch parity: a CTA rewrites buffer e & 1 in epoch e + 2, which it can only start
+// after it has read the neighbours' rows of epoch e + 1, and those were computed from this CTA's rows of epoch e.
+// The host sets every mailbox lane to 0x80808080 before a launch; epoch e writes bit 31 = (e >> 1) & 1.
+// Only own rows count for the per-sweep (B, M).  Bit-identical to every other family.
 #include "lsm_tiled_dev.cuh"
 
+#include <cooperative_groups.h>
 #include <cstring>
 
 namespace lsmk {
@@ -35,9 +40,11 @@ struct SlabArgs {
     int lg_lpr;                  // log2(lanes per compact row) = log2(L) - 3
     int lg_R;                    // log2(cross rows per march row): 0 in 2D, log2(L) in 3D
     int rows_max;                // most march rows of any slab (shared-memory stride)
+    int D;                       // temporal depth: half-sweeps per exchange; every slab has >= 2 D rows
+    int dmax;                    // mailbox rows reserved per slot
     int one;
     long long *obs;              // [nsweeps][2] (B, M) slots zeroed by the host, or nullptr
-    uint32_t *mbox;              // [G][first, last][colour][lanes of a march row]; every lane 0x80808080 at launch
+    uint32_t *mbox;              // [G][first, last][epoch parity][colour][dmax][lanes of a march row]
 };
 
 __device__ __forceinline__ uint32_t slab_ld_l2(const uint32_t *p)
@@ -50,7 +57,7 @@ __device__ __forceinline__ void slab_st_l2(uint32_t *p, uint32_t v)
 {
     asm volatile("st.relaxed.gpu.global.u32 [%0], %1;" ::"l"(p), "r"(v) : "memory");
 }
-// spin until the lane carries the expected sweep parity in bit 31; returns the lane without it
+// spin until the lane carries the expected epoch bit in bit 31; returns the lane without it
 __device__ __forceinline__ uint32_t slab_take(const uint32_t *p, uint32_t tag31)
 {
     uint32_t v;
@@ -69,7 +76,6 @@ k_sweep_slab(const __grid_constant__ SlabArgs a, const __grid_constant__ PhiloxS
         int acc[2][2];           // this CTA's share of (B, M) of the sweep in flight, double-buffered by sweep parity
     } sm;
     extern __shared__ __align__(16) uint32_t s_lat[];
-    constexpr bool NE = MODEL == M_NE_HEATBATH || MODEL == M_NE_METROPOLIS;
     uint32_t s_t = (uint32_t)__cvta_generic_to_shared(sm.t);
     asm volatile("" : "+r"(s_t));
     uint32_t ne_t32 = 0;
@@ -89,27 +95,33 @@ k_sweep_slab(const __grid_constant__ SlabArgs a, const __grid_constant__ PhiloxS
     const int g = (int)blockIdx.x, G = (int)gridDim.x;
     const int lg_lpr = a.lg_lpr, lg_row = a.lg_lpr + a.lg_R;
     const uint32_t lpr = 1u << lg_lpr, R = 1u << a.lg_R, rowl = 1u << lg_row;   // lanes per compact row / march row
+    const uint32_t Lm = (uint32_t)a.L - 1u;
+    const uint32_t D = (uint32_t)a.D;
     const int m0 = (int)(((long long)a.L * g) / G), m1 = (int)(((long long)a.L * (g + 1)) / G);
     const uint32_t rows = (uint32_t)(m1 - m0);
-    const uint32_t colstride = (uint32_t)(a.rows_max + 2) << lg_row;            // shared lanes per colour
+    const uint32_t colstride = ((uint32_t)a.rows_max + 2u * D) << lg_row;       // shared lanes per colour
     uint32_t *const s_col[2] = {s_lat, s_lat + colstride};
-    // march rows of the adjacent slabs that touch this one, and their owners
-    const uint32_t mb = (uint32_t)((m0 == 0 ? a.L : m0) - 1), ma = (uint32_t)(m1 == a.L ? 0 : m1);
     const int g_below = g == 0 ? G - 1 : g - 1, g_above = g + 1 == G ? 0 : g + 1;
+    // local march row lr <-> global march row (m0 - D + lr) mod L: 0 ... D-1 halo below, D ... D+rows-1 own rows,
+    // D+rows ... rows+2D-1 halo above
+    const uint32_t mbase = (uint32_t)(m0 + a.L) - D;
 
-    // the slab in shared memory: local march row 1 ... rows (rows 0 and rows + 1 of the layout are spare)
-    for (uint32_t i = tid; i < (rows << lg_row); i += nthr) {
-        s_col[0][rowl + i] = a.col[0][((uint32_t)m0 << lg_row) + i];
-        s_col[1][rowl + i] = a.col[1][((uint32_t)m0 << lg_row) + i];
+    // the slab and its halo as the launch finds the lattice
+    for (uint32_t i = tid; i < ((rows + 2u * D) << lg_row); i += nthr) {
+        const uint32_t lr = i >> lg_row, r = i & (rowl - 1);
+        const uint32_t src = (((mbase + lr) & Lm) << lg_row) + r;
+        s_col[0][i] = a.col[0][src];
+        s_col[1][i] = a.col[1][src];
     }
     __syncthreads();
+    // No CTA may write its slab back (end of the kernel) before the adjacent CTAs have read their initial halos; with
+    // fewer half-sweeps than one epoch there is no exchange that would order the two.
+    cooperative_groups::this_grid().sync();
 
-    // mailbox rows: [cta][0 = first row, 1 = last row][colour]
-    auto mbox_row = [&](int cta, int which, int colour) { return a.mbox + ((size_t)((cta * 2 + which) * 2 + colour) << lg_row); };
-
-    int thrB = 0, thrM = 0;
-    const int nhalves = 2 * a.nsweeps;
-    const uint32_t total = rows << lg_row, nA = (rows >= 2u ? 2u : 1u) << lg_row;
+    // mailbox rows
+    auto mbox_row = [&](int cta, int side, uint32_t buf, int colour, uint32_t k) {
+        return a.mbox + ((size_t)((((uint32_t)(cta * 2 + side) * 2u + buf) * 2u + (uint32_t)colour) * (uint32_t)a.dmax + k) << lg_row);
+    };
     auto flush_obs = [&](int sw) {                         // thread 0, after a barrier behind the sweep's last add
         const int vB = sm.acc[sw & 1][0], vM = sm.acc[sw & 1][1];
         if (vB != 0) atomicAdd((unsigned long long *)&a.obs[2 * sw], (unsigned long long)(long long)vB);
@@ -117,112 +129,133 @@ k_sweep_slab(const __grid_constant__ SlabArgs a, const __grid_constant__ PhiloxS
         sm.acc[sw & 1][0] = 0;                             // next used by sweep sw + 2: several barriers away
         sm.acc[sw & 1][1] = 0;
     };
-#pragma unroll 1
-    for (int gh = 0; gh < nhalves; ++gh) {
-        const int half = gh & 1, sw = gh >> 1;
-        uint32_t *const own = s_col[half];
-        uint32_t *const oth = s_col[half ^ 1];
-        if (gh > 0) {
-            __syncthreads();                               // the previous half-sweep's rows of this slab are complete
-            if (OBS >= 1 && half == 0 && tid == 0) flush_obs(sw - 1);
-        }
-        // The rows of the adjacent slabs that touch this one: written by their owners in half-sweep gh - 1 (mailbox,
-        // sweep parity in bit 31), or the lattice as the launch found it (gh = 0).  A boundary lane needs exactly one
-        // lane of them (the same lane index), so the thread that updates it spins on that lane itself.
-        const uint32_t tag31 = (uint32_t)((gh - 1) >> 1) << 31;
-        const uint32_t *const below = gh ? mbox_row(g_below, 1, half ^ 1) : a.col[1] + (mb << lg_row);
-        const uint32_t *const above = gh ? mbox_row(g_above, 0, half ^ 1) : a.col[1] + (ma << lg_row);
-        const unsigned long long t = a.t0 + (unsigned long long)sw;
-        PhiloxDyn pc = {0u, 0u, 0u, 0u, pk};
-        philox_half_consts(make_sweep_key(a.seed, t, (uint32_t)half), pk.rk0, pk.rk1, pc.x1, pc.y2, pc.z2, pc.w3);
-        int totU = 0, totBN = 0, totS = 0, nsites = 0;
-        if (half == 0) thrB = thrM = 0;
-        const uint32_t wtag = (uint32_t)(sw & 1) << 31;
-        uint32_t *const mb_first = mbox_row(g, 0, half), *const mb_last = mbox_row(g, 1, half);
 
-        // Lanes of the slab in the order boundary rows (1 and `rows`), then interior rows: the adjacent slabs wait for
-        // the former, so every thread takes them first.  One lane = 4 sites, one Philox call (spin-1: two).
+    int thrB = 0, thrM = 0;
+    const uint32_t H = 2u * (uint32_t)a.nsweeps;
+    uint32_t e = 0;
 #pragma unroll 1
-        for (uint32_t i = tid; i < total; i += nthr) {
-            const bool edge = i < nA;
-            const uint32_t ml = edge ? ((i >> lg_row) ? rows : 1u) : 2u + ((i - nA) >> lg_row);
-            const uint32_t r = i & (rowl - 1);
-            const uint32_t x = r & (lpr - 1), y = r >> lg_lpr;
-            const uint32_t m = (uint32_t)m0 + ml - 1u;
-            const uint32_t qq = (m + y + (uint32_t)half) & 1u;
-            const uint32_t li = (ml << lg_row) + r;
-            const uint32_t gl = (m << lg_row) + r;              // lane index in the colour array = Philox group (D2)
-            // the random words do not depend on the neighbours: drawn before a boundary lane waits for its halo lane
-            uint4 rw = make_uint4(0u, 0u, 0u, 0u), rw2 = rw;
-            if (MODEL == M_ISING_HALF) rw = philox_sweep(gl, pc);
-            if (MODEL == M_ISING_ONE) {
-                rw = philox_sweep(2u * gl, pc);
-                rw2 = philox_sweep(2u * gl + 1u, pc);
+    for (uint32_t h0 = 0; h0 < H; h0 += D, ++e) {
+        const uint32_t De = H - h0 < D ? H - h0 : D;       // steps of this epoch (the last one may be shorter)
+        const bool last = h0 + D >= H;
+        if (e > 0) {
+            __syncthreads();                               // the previous epoch's rows of this slab are complete
+            // halo: the rows the adjacent slabs stored during epoch e - 1.  D = 1: only the colour of that one step.
+            const uint32_t pe = e - 1u, buf = pe & 1u, tag31 = ((pe >> 1) & 1u) << 31;
+            const uint32_t ncol = D == 1u ? 1u : 2u, c0 = D == 1u ? ((h0 - 1u) & 1u) : 0u;
+            const uint32_t per_side = (ncol * D) << lg_row;
+#pragma unroll 1
+            for (uint32_t i = tid; i < 2u * per_side; i += nthr) {
+                const uint32_t above = i >= per_side ? 1u : 0u;
+                const uint32_t w = i - above * per_side;
+                const uint32_t r = w & (rowl - 1), kc = w >> lg_row;      // kc = ci * D + k
+                const uint32_t ci = kc >= D ? 1u : 0u, k = kc - ci * D;
+                const int colour = (int)(c0 + ci);
+                // below: the neighbour's LAST D rows -> local rows 0 ... D-1; above: its FIRST D rows -> D+rows ...
+                const uint32_t *src = mbox_row(above ? g_above : g_below, above ? 0 : 1, buf, colour, k) + r;
+                const uint32_t lr = above ? D + rows + k : k;
+                s_col[colour][(lr << lg_row) + r] = slab_take(src, tag31);
             }
-            const uint32_t c = oth[li], o = own[li];
-            uint32_t p, n;
-            if (ml == 1u) p = gh ? slab_take(below + r, tag31) : below[r];
-            else p = oth[li - rowl];
-            if (ml == rows) n = gh ? slab_take(above + r, tag31) : above[r];
-            else n = oth[li + rowl];
-            const uint32_t cs = oth[(li - x) + ((qq ? x + 1u : x - 1u) & (lpr - 1))];
-            const uint32_t sd = qq ? __funnelshift_r(c, cs, 8) : __funnelshift_r(cs, c, 24);
-            uint32_t yp = 0, yn = 0;
-            if (DIMS == 3) {
-                yp = oth[(ml << lg_row) + (((y - 1u) & (R - 1)) << lg_lpr) + x];
-                yn = oth[(ml << lg_row) + (((y + 1u) & (R - 1)) << lg_lpr) + x];
-            }
-            uint32_t out;
-            if (MODEL == M_ISING_HALF) {
-                uint32_t ns = p + n + c + sd;
-                if (DIMS == 3) ns += yp + yn;
-                out = rule_half<TRACK, OBS, NEV>(o, ns, rw, s_t, (uint32_t)a.one, totU, totBN);
-            } else if (MODEL == M_ISING_ONE) {
-                uint32_t ns;
-                if (TRACK) {
-                    ns = ((p + n) & 0x0F0F0F0Fu) + ((c + sd) & 0x0F0F0F0Fu);
-                    if (DIMS == 3) ns += (yp + yn) & 0x0F0F0F0Fu;
-                } else {
-                    ns = p + n + c + sd;
-                    if (DIMS == 3) ns += yp + yn;
-                }
-                out = rule_one<DIMS, TRACK, OBS, NEV>(o, ns, rw, rw2, s_t, (uint32_t)a.one, totU, totBN, totS);
-            } else {
-                uint32_t accU = 0;
-                out = rule_ne<TRACK, MODEL == M_NE_METROPOLIS, OBS>(o, n, qq ? sd : c, gl, pc, ne_t32, ne_always, accU);
-                if (OBS >= 1) totU += (int)bytesum(accU);
-            }
-            own[li] = out;
-            if (edge) {
-                if (ml == 1u) slab_st_l2(mb_first + r, out | wtag);
-                if (ml == rows) slab_st_l2(mb_last + r, out | wtag);
-            }
-            nsites += 4;
         }
-        if (OBS >= 1) {
-            March<MODEL, DIMS, TRACK, OBS, NEV> M;         // only the per-thread sums are used
-            M.totU = totU;
-            M.totBN = totBN;
-            M.totS = totS;
-            long long cB, cM;
-            march_observables<MODEL, DIMS>(M, nsites, half == 1, cB, cM);
-            thrB += (int)cB;                               // one slab holds < 2^20 sites: far below 2^31
-            thrM += (int)cM;
-            if (half == 1) {
-                const int wB = __reduce_add_sync(0xffffffffu, thrB), wM = __reduce_add_sync(0xffffffffu, thrM);
-                if ((tid & 31u) == 0u) {
-                    if (wB != 0) atomicAdd(&sm.acc[sw & 1][0], wB);
-                    if (wM != 0) atomicAdd(&sm.acc[sw & 1][1], wM);
+#pragma unroll 1
+        for (uint32_t j = 0; j < De; ++j) {
+            const uint32_t gh = h0 + j;
+            const int half = (int)(gh & 1u), sw = (int)(gh >> 1);
+            if (j > 0 || e > 0) __syncthreads();           // the rows (and halo) this step reads are complete
+            if (OBS >= 1 && half == 0 && gh > 0 && tid == 0) flush_obs(sw - 1);
+            uint32_t *const own = s_col[half];
+            const uint32_t *const oth = s_col[half ^ 1];
+            const uint32_t ext = De - 1u - j;              // halo rows updated on either side (redundant updates)
+            const bool publish = !last && j + 2u >= D;     // this colour's rows are final for the coming exchange
+            const unsigned long long t = a.t0 + (unsigned long long)sw;
+            PhiloxDyn pc = {0u, 0u, 0u, 0u, pk};
+            philox_half_consts(make_sweep_key(a.seed, t, (uint32_t)half), pk.rk0, pk.rk1, pc.x1, pc.y2, pc.z2, pc.w3);
+            int totU = 0, totBN = 0, totS = 0, nsites = 0;
+            if (half == 0) thrB = thrM = 0;
+            const uint32_t wtag = ((e >> 1) & 1u) << 31;
+            // Row order: the 2 D rows the neighbours wait for first (first D and last D own rows), then the others.
+            const uint32_t nA = publish ? 2u * D : 0u, nrows = rows + 2u * ext;
+            const uint32_t total = nrows << lg_row;
+#pragma unroll 1
+            for (uint32_t i = tid; i < total; i += nthr) {
+                const uint32_t s = i >> lg_row, r = i & (rowl - 1);
+                uint32_t lr;
+                if (s < nA) lr = s < D ? D + s : rows + (s - D);
+                else if (!publish) lr = D - ext + s;
+                else {
+                    const uint32_t s2 = s - nA, mid = rows - 2u * D;
+                    lr = s2 < ext ? D - ext + s2 : (s2 < ext + mid ? 2u * D + (s2 - ext) : rows + D + (s2 - ext - mid));
+                }
+                const bool own_row = lr >= D && lr < D + rows;
+                const uint32_t x = r & (lpr - 1), y = r >> lg_lpr;
+                const uint32_t m = (mbase + lr) & Lm;
+                const uint32_t qq = (m + y + (uint32_t)half) & 1u;
+                const uint32_t li = (lr << lg_row) + r;
+                const uint32_t gl = (m << lg_row) + r;          // lane index in the colour array = Philox group (D2)
+                const uint32_t c = oth[li], o = own[li];
+                const uint32_t p = oth[li - rowl], n = oth[li + rowl];
+                const uint32_t cs = oth[(li - x) + ((qq ? x + 1u : x - 1u) & (lpr - 1))];
+                const uint32_t sd = qq ? __funnelshift_r(c, cs, 8) : __funnelshift_r(cs, c, 24);
+                uint32_t yp = 0, yn = 0;
+                if (DIMS == 3) {
+                    yp = oth[(lr << lg_row) + (((y - 1u) & (R - 1)) << lg_lpr) + x];
+                    yn = oth[(lr << lg_row) + (((y + 1u) & (R - 1)) << lg_lpr) + x];
+                }
+                int lU = 0, lBN = 0, lS = 0;                    // this lane's sums: counted for own rows only
+                uint32_t out;
+                if (MODEL == M_ISING_HALF) {
+                    uint32_t ns = p + n + c + sd;
+                    if (DIMS == 3) ns += yp + yn;
+                    out = rule_half<TRACK, OBS, NEV>(o, ns, philox_sweep(gl, pc), s_t, (uint32_t)a.one, lU, lBN);
+                } else if (MODEL == M_ISING_ONE) {
+                    uint32_t ns;
+                    if (TRACK) {
+                        ns = ((p + n) & 0x0F0F0F0Fu) + ((c + sd) & 0x0F0F0F0Fu);
+                        if (DIMS == 3) ns += (yp + yn) & 0x0F0F0F0Fu;
+                    } else {
+                        ns = p + n + c + sd;
+                        if (DIMS == 3) ns += yp + yn;
+                    }
+                    out = rule_one<DIMS, TRACK, OBS, NEV>(o, ns, philox_sweep(2u * gl, pc), philox_sweep(2u * gl + 1u, pc), s_t,
+                                                          (uint32_t)a.one, lU, lBN, lS);
+                } else {
+                    uint32_t accU = 0;
+                    out = rule_ne<TRACK, MODEL == M_NE_METROPOLIS, OBS>(o, n, qq ? sd : c, gl, pc, ne_t32, ne_always, accU);
+                    if (OBS >= 1) lU = (int)bytesum(accU);
+                }
+                own[li] = out;
+                if (s < nA) slab_st_l2(mbox_row(g, s < D ? 0 : 1, e & 1u, half, s < D ? s : s - D) + r, out | wtag);
+                if (OBS >= 1 && own_row) {
+                    totU += lU;
+                    totBN += lBN;
+                    totS += lS;
+                    nsites += 4;
+                }
+            }
+            if (OBS >= 1) {
+                March<MODEL, DIMS, TRACK, OBS, NEV> M;     // only the per-thread sums are used
+                M.totU = totU;
+                M.totBN = totBN;
+                M.totS = totS;
+                long long cB, cM;
+                march_observables<MODEL, DIMS>(M, nsites, half == 1, cB, cM);
+                thrB += (int)cB;                           // one slab holds < 2^20 sites: far below 2^31
+                thrM += (int)cM;
+                if (half == 1) {
+                    const int wB = __reduce_add_sync(0xffffffffu, thrB), wM = __reduce_add_sync(0xffffffffu, thrM);
+                    if ((tid & 31u) == 0u) {
+                        if (wB != 0) atomicAdd(&sm.acc[sw & 1][0], wB);
+                        if (wM != 0) atomicAdd(&sm.acc[sw & 1][1], wM);
+                    }
                 }
             }
         }
     }
     __syncthreads();
-    if (OBS >= 1 && nhalves > 0 && tid == 0) flush_obs(a.nsweeps - 1);
+    if (OBS >= 1 && H > 0u && tid == 0) flush_obs(a.nsweeps - 1);
     // write the slab back
-    for (uint32_t i = tid; i < total; i += nthr) {
-        a.col[0][((uint32_t)m0 << lg_row) + i] = s_col[0][rowl + i];
-        a.col[1][((uint32_t)m0 << lg_row) + i] = s_col[1][rowl + i];
+    for (uint32_t i = tid; i < (rows << lg_row); i += nthr) {
+        a.col[0][((uint32_t)m0 << lg_row) + i] = s_col[0][(D << lg_row) + i];
+        a.col[1][((uint32_t)m0 << lg_row) + i] = s_col[1][(D << lg_row) + i];
     }
 }
 
@@ -242,40 +275,57 @@ static int slab_ilog2(long long v)
 #define LSM_SLAB_SMEM_MAX (220 * 1024)     // dynamic shared memory per CTA (227 KB opt-in minus the static part)
 #endif
 
-// Mailbox bytes reserved in the workspace for this shape (0: the slab family never runs it).  Depends on the shape
-// only, so that lsm_workspace_bytes needs no device: SLAB_MAX_CTAS slabs x (first, last) x 2 colours x one march row.
-size_t slab_mailbox_bytes(int dims, int L, int model)
+// Largest temporal depth the mailboxes of this shape are sized for (0: the slab family never runs it).  Deep halos pay
+// where a half-sweep is shorter than an exchange (~1 us): the smaller 2D lattices.
+int slab_depth_max(int dims, int L, int model)
 {
     if (model != M_ISING_HALF && model != M_ISING_ONE && model != M_NE_HEATBATH && model != M_NE_METROPOLIS) return 0;
     if ((L & (L - 1)) != 0) return 0;                                 // lane index math by shifts
     if (dims == 2 ? (L < 512 || L > 4096) : (L < 64 || L > 128)) return 0;   // below: the small family; above: does not fit
-    const size_t rowbytes = (size_t)(L / 2) * (dims == 3 ? (size_t)L : 1);
-    return (size_t)SLAB_MAX_CTAS * 4 * rowbytes;
+    if (dims == 3) return 1;
+    return L <= 1024 ? 4 : L == 2048 ? 2 : 1;
 }
 
-bool slab_plan(const Lat &lat, int model, const TiledTables &t, SlabPlan *out)
+// Mailbox bytes reserved in the workspace for this shape.  Depends on the shape only, so that lsm_workspace_bytes
+// needs no device: SLAB_MAX_CTAS slabs x (first, last) x 2 epoch parities x 2 colours x depth_max march rows.
+size_t slab_mailbox_bytes(int dims, int L, int model)
+{
+    const size_t rowbytes = (size_t)(L / 2) * (dims == 3 ? (size_t)L : 1);
+    return (size_t)SLAB_MAX_CTAS * 8 * (size_t)slab_depth_max(dims, L, model) * rowbytes;
+}
+
+#ifndef LSM_SLAB_DEPTH_1024
+#define LSM_SLAB_DEPTH_1024 4            // default temporal depth for L <= 1024 (2D)
+#endif
+
+// depth: 0 = the default for this shape, else 1 ... slab_depth_max
+bool slab_plan(const Lat &lat, int model, const TiledTables &t, int depth, SlabPlan *out)
 {
     if (!t.usable) return false;
-    if (slab_mailbox_bytes(lat.dims, lat.L, model) == 0) return false;
+    const int dmax = slab_depth_max(lat.dims, lat.L, model);
+    if (dmax == 0 || depth < 0 || depth > dmax) return false;
+    int D = depth ? depth : (lat.dims == 2 && lat.L <= 1024 ? LSM_SLAB_DEPTH_1024 : dmax);
+    if (D > dmax) D = dmax;
     int coop = 0, dev = 0;
     if (cudaGetDevice(&dev) != cudaSuccess) return false;
     if (cudaDeviceGetAttribute(&coop, cudaDevAttrCooperativeLaunch, dev) != cudaSuccess || !coop) return false;
     int G = sm_count();                                               // one CTA per SM, all co-resident
     if (G > SLAB_MAX_CTAS) G = SLAB_MAX_CTAS;
-    if (G > lat.L) G = lat.L;
+    if (G > lat.L / (2 * D)) G = lat.L / (2 * D);                     // every slab: >= 2 D rows (disjoint first / last D)
     if (G < 2) return false;
     const int rows_max = (lat.L + G - 1) / G;
     const long long rowl = (lat.dims == 3 ? (long long)lat.L : 1) * (lat.L / 8);   // lanes per march row and colour
-    const long long smem = 2ll * (rows_max + 2) * rowl * 4;
+    const long long smem = 2ll * (rows_max + 2 * D) * rowl * 4;
     if (smem > LSM_SLAB_SMEM_MAX) return false;
-    long long per = (long long)rows_max * rowl;                       // lanes per half-sweep of the largest slab
-    if (2 * rowl > per) per = 2 * rowl;
+    long long per = (long long)(rows_max + 2 * (D - 1)) * rowl;       // lanes of the largest step of the largest slab
     int threads = (int)(per < 1024 ? ((per + 31) / 32) * 32 : 1024);
     if (threads < 64) threads = 64;
     out->G = G;
     out->rows_max = rows_max;
     out->threads = threads;
     out->smem = (int)smem;
+    out->D = D;
+    out->dmax = dmax;
     return true;
 }
 
@@ -321,6 +371,8 @@ cudaError_t launch_sweep_slab(const Lat &lat, int model, int track, unsigned lon
     a.lg_lpr = lg_L - 3;
     a.lg_R = lat.dims == 3 ? lg_L : 0;
     a.rows_max = plan.rows_max;
+    a.D = plan.D;
+    a.dmax = plan.dmax;
     a.one = 1;
     a.obs = d_obs;
     a.mbox = d_mbox;

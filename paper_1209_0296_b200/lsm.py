@@ -61,6 +61,8 @@ SIGNATURES = {
     "lsm_get_thresholds": (_i32, [_vp, _P(_u64), _P(_i32)]),
     "lsm_set_kernel": (_i32, [_vp, _i32]),
     "lsm_get_kernel": (_i32, [_vp, _P(_i32)]),
+    "lsm_set_temporal_depth": (_i32, [_vp, _i32]),
+    "lsm_get_temporal_depth": (_i32, [_vp, _P(_i32)]),
     "lsm_get_launch_count": (_i32, [_vp, _P(_u64)]),
     "lsm_binder_u4": (_i32, [_vp, _i64, _P(_dbl)]),
     "lsm_heat_capacity": (_i32, [_vp, _i64, _i64, _dbl, _dbl, _dbl, _P(_dbl)]),
@@ -371,6 +373,18 @@ class Lattice:
         k = _i32()
         _check(self._lib.lsm_get_kernel(self._h, ctypes.byref(k)), "lsm_get_kernel")
         return int(k.value)
+
+    @_on_device
+    def set_temporal_depth(self, depth):
+        """Half-sweeps between two boundary exchanges of the slab family (0: default); results do not depend on it."""
+        _check(self._lib.lsm_set_temporal_depth(self._h, int(depth)), "lsm_set_temporal_depth")
+
+    @property
+    @_on_device
+    def temporal_depth(self):
+        d = _i32()
+        _check(self._lib.lsm_get_temporal_depth(self._h, ctypes.byref(d)), "lsm_get_temporal_depth")
+        return int(d.value)
 
     @property
     @_on_device

@@ -148,6 +148,53 @@ def test_sweep_parity(kw, nsweeps, family):
     assert E == orc.energy() and M == orc.measure_int()[1]
 
 
+SLAB_DEPTH_CASES = [
+    # (kwargs, depths): temporal blocking of the slab family -- every depth the shape allows, incl. a "never" table
+    (dict(dims=2, L=512, T=2.269), (1, 2, 3, 4)),
+    (dict(dims=2, L=1024, T=0.3, h=0.1), (2, 4)),
+    (dict(dims=2, L=1024, two_S=2, T=1.5, h=0.01), (1, 3)),
+    (dict(dims=2, L=512, model=lsm.NE_HEATBATH, J=0.0, T=W.ne_temperature(0.3)), (2, 3, 4)),
+    (dict(dims=2, L=1024, model=lsm.NE_METROPOLIS, J=0.0, T=W.ne_temperature(0.2)), (4,)),
+    (dict(dims=2, L=2048, T=2.269, h=-0.02), (1, 2)),
+    (dict(dims=2, L=4096, T=2.6), (1,)),
+    (dict(dims=3, L=64, T=4.5115), (1,)),
+    (dict(dims=3, L=128, two_S=2, T=3.0, h=0.01), (1,)),
+]
+
+
+@pytest.mark.parametrize("kw,depths", SLAB_DEPTH_CASES)
+def test_slab_temporal_blocking_parity(kw, depths):
+    """SURVEY 8(f) NEXT-4, temporal blocking: `depth` half-sweeps between two boundary exchanges with redundant halo
+    updates must give the oracle's configuration and per-sweep (B, M) for every depth, across calls whose lengths leave
+    partial epochs (odd numbers of sweeps, one-sweep calls, calls with and without the record)."""
+    calls = ((5, True), (3, False), (1, True), (4, True))
+    orc = O.Oracle(seed=W.seed_of(11, 1), **kw)
+    want, states = [], []
+    for n, rec in calls:
+        want.append(orc.sweep_record(n) if rec else orc.sweep(n))
+        states.append((orc.get_spins().copy(), orc.measure_int(), orc.persistence()))
+    for depth in depths:
+        lat = lsm.Lattice(seed=W.seed_of(11, 1), **kw)
+        lat.set_kernel(lsm.KERNEL_SLAB)
+        lat.set_temporal_depth(depth)
+        assert lat.kernel == lsm.KERNEL_SLAB and lat.temporal_depth == depth
+        for (n, rec), w, (spins, bm, pers) in zip(calls, want, states):
+            if rec:
+                got = lat.sweep_record(n).cpu().numpy()
+                assert np.array_equal(got, w), (depth, n)
+            else:
+                lat.sweep(n)
+            assert np.array_equal(lat.get_spins().cpu().numpy(), spins), (depth, n)
+            assert lat.measure_int()[:2] == bm and lat.measure_full() == bm
+            assert lat.persistence() == pers
+        lat.close()
+    lat = lsm.Lattice(seed=1, **kw)
+    lat.set_kernel(lsm.KERNEL_SLAB)
+    with pytest.raises(lsm.LsmError):
+        lat.set_temporal_depth(5)
+    lat.close()
+
+
 @pytest.mark.parametrize("family", FAMILIES)
 def test_cfg1_full_length(family):
     """BASELINE.json config 1 at full length: 64x64, T=2.269, 1000 sweeps, (E, M) after every sweep."""
