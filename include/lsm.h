@@ -85,12 +85,13 @@ enum {
 /* Kernel families (lsm_set_kernel).  AUTO picks the fastest one that supports the lattice:
  *  SMALL    one launch for all sweeps of a call: lattice slabs in the shared memory of a thread-block cluster,
  *           cluster barrier between the colours (L a power of two >= 8; other L with L % 32 == 0 up to 32 768
- *           sites); chosen up to 262 144 sites (512^2, 64^3);
+ *           sites); chosen below 262 144 sites (up to 256^2, 32^3);
  *  TILED    one launch per half-sweep, 16 sites per 128-bit word (L % 32 == 0, no "never" threshold);
  *  RESIDENT one cooperative launch for all sweeps with neighbour-flag synchronisation (opt-in, large lattices);
  *  SLAB     one cooperative launch for all sweeps of a call with the whole lattice resident in the shared memory of
- *           one CTA per SM: slabs of march rows, boundary rows exchanged through L2 behind one progress flag per
- *           CTA, interior updates overlap the exchange (L a power of two, up to 4096^2 / 128^3);
+ *           one CTA per SM: slabs of march rows, boundary rows exchanged through self-validating mailbox words in L2, one per
+ *           CTA, several half-sweeps per exchange (lsm_set_temporal_depth); L a power of two, 512^2 ... 4096^2,
+ *           64^3, 128^3, where AUTO chooses it;
  *  GENERIC  one thread per site, any even L >= 4, any table.
  * All families produce bit-identical results (same random-word map D2, same thresholds D3). */
 enum { LSM_KERNEL_AUTO = 0, LSM_KERNEL_GENERIC = 1, LSM_KERNEL_TILED = 2, LSM_KERNEL_RESIDENT = 3, LSM_KERNEL_SMALL = 4,

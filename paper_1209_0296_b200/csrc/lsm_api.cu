@@ -140,9 +140,12 @@ static void choose_kernel(lsm *o)
 {
     int want = o->kernel_pref;
     bool tiled_ok = tiled_supported(o->lat, o->model, o->tiled);
-    if (want == LSM_KERNEL_AUTO)
-        want = small_plan(o->lat, o->model, o->tiled, &o->small, false) ? LSM_KERNEL_SMALL
-             : tiled_ok ? LSM_KERNEL_TILED : LSM_KERNEL_GENERIC;
+    if (want == LSM_KERNEL_AUTO) {
+        // 512^2 ... 4096^2, 64^3, 128^3: the lattice lives in the SMs' shared memory (profiles/r2_slab_family.md)
+        if (o->N >= 262144 && slab_plan(o->lat, o->model, o->tiled, o->slab_depth, &o->slab)) want = LSM_KERNEL_SLAB;
+        else want = small_plan(o->lat, o->model, o->tiled, &o->small, false) ? LSM_KERNEL_SMALL
+                  : tiled_ok ? LSM_KERNEL_TILED : LSM_KERNEL_GENERIC;
+    }
     if (want == LSM_KERNEL_SMALL && !small_plan(o->lat, o->model, o->tiled, &o->small, true))
         want = tiled_ok ? LSM_KERNEL_TILED : LSM_KERNEL_GENERIC;
     if (want == LSM_KERNEL_TILED && !tiled_ok) want = LSM_KERNEL_GENERIC;

@@ -65,8 +65,22 @@ __device__ __forceinline__ uint32_t slab_take(const uint32_t *p, uint32_t tag31)
     return v & 0x7FFFFFFFu;
 }
 
+// the same for the four lanes of a 16-byte word (each lane carries its own epoch bit, so a torn word is only retried)
+__device__ __forceinline__ uint4 slab_take4(const uint32_t *p, uint32_t tag31)
+{
+    uint4 v;
+    do {
+        asm volatile("ld.relaxed.gpu.global.v4.u32 {%0,%1,%2,%3}, [%4];" : "=r"(v.x), "=r"(v.y), "=r"(v.z), "=r"(v.w) : "l"(p) : "memory");
+    } while (((((v.x ^ tag31) | (v.y ^ tag31)) | ((v.z ^ tag31) | (v.w ^ tag31))) & 0x80000000u) != 0u);
+    return make_uint4(v.x & 0x7FFFFFFFu, v.y & 0x7FFFFFFFu, v.z & 0x7FFFFFFFu, v.w & 0x7FFFFFFFu);
+}
+__device__ __forceinline__ void slab_st4_l2(uint32_t *p, uint4 v)
+{
+    asm volatile("st.relaxed.gpu.global.v4.u32 [%0], {%1,%2,%3,%4};" ::"l"(p), "r"(v.x), "r"(v.y), "r"(v.z), "r"(v.w) : "memory");
+}
+
 template <int MODEL, int DIMS, bool TRACK, int OBS, bool NEV>
-__global__ void __launch_bounds__(1024, 1)
+__global__ void __launch_bounds__(512, 1)
 k_sweep_slab(const __grid_constant__ SlabArgs a, const __grid_constant__ PhiloxSweepConsts pk,
              const __grid_constant__ typename TabOf<MODEL>::type tab, const __grid_constant__ NevTab ytab)
 {
@@ -80,6 +94,7 @@ k_sweep_slab(const __grid_constant__ SlabArgs a, const __grid_constant__ PhiloxS
     asm volatile("" : "+r"(s_t));
     uint32_t ne_t32 = 0;
     int ne_always = 0;
+    bool ne_all4 = false;
     if constexpr (MODEL == M_ISING_HALF || MODEL == M_ISING_ONE) {
         for (int i = threadIdx.x; i < NT; i += blockDim.x) {
             sm.t[i] = tab.t[i];
@@ -88,13 +103,16 @@ k_sweep_slab(const __grid_constant__ SlabArgs a, const __grid_constant__ PhiloxS
     } else {
         ne_t32 = tab.t32;
         ne_always = tab.always;
+        ne_all4 = tab.all4 != 0;
     }
     if (threadIdx.x < 4) sm.acc[threadIdx.x >> 1][threadIdx.x & 1] = 0;
 
     const uint32_t tid = threadIdx.x, nthr = blockDim.x;
     const int g = (int)blockIdx.x, G = (int)gridDim.x;
     const int lg_lpr = a.lg_lpr, lg_row = a.lg_lpr + a.lg_R;
-    const uint32_t lpr = 1u << lg_lpr, R = 1u << a.lg_R, rowl = 1u << lg_row;   // lanes per compact row / march row
+    const uint32_t R = 1u << a.lg_R, rowl = 1u << lg_row;                       // cross rows; lanes per march row
+    const int lg_wpr = lg_lpr - 2, lg_wrow = lg_row - 2;                        // 16-byte words per compact / march row
+    const uint32_t wpr = 1u << lg_wpr, wrow = 1u << lg_wrow;
     const uint32_t Lm = (uint32_t)a.L - 1u;
     const uint32_t D = (uint32_t)a.D;
     const int m0 = (int)(((long long)a.L * g) / G), m1 = (int)(((long long)a.L * (g + 1)) / G);
@@ -142,18 +160,18 @@ k_sweep_slab(const __grid_constant__ SlabArgs a, const __grid_constant__ PhiloxS
             // halo: the rows the adjacent slabs stored during epoch e - 1.  D = 1: only the colour of that one step.
             const uint32_t pe = e - 1u, buf = pe & 1u, tag31 = ((pe >> 1) & 1u) << 31;
             const uint32_t ncol = D == 1u ? 1u : 2u, c0 = D == 1u ? ((h0 - 1u) & 1u) : 0u;
-            const uint32_t per_side = (ncol * D) << lg_row;
+            const uint32_t per_side = (ncol * D) << lg_wrow;        // in 16-byte words: one L2 round trip moves four lanes
 #pragma unroll 1
             for (uint32_t i = tid; i < 2u * per_side; i += nthr) {
                 const uint32_t above = i >= per_side ? 1u : 0u;
                 const uint32_t w = i - above * per_side;
-                const uint32_t r = w & (rowl - 1), kc = w >> lg_row;      // kc = ci * D + k
+                const uint32_t wr = w & (wrow - 1), kc = w >> lg_wrow;    // kc = ci * D + k
                 const uint32_t ci = kc >= D ? 1u : 0u, k = kc - ci * D;
                 const int colour = (int)(c0 + ci);
                 // below: the neighbour's LAST D rows -> local rows 0 ... D-1; above: its FIRST D rows -> D+rows ...
-                const uint32_t *src = mbox_row(above ? g_above : g_below, above ? 0 : 1, buf, colour, k) + r;
+                const uint32_t *src = mbox_row(above ? g_above : g_below, above ? 0 : 1, buf, colour, k) + (wr << 2);
                 const uint32_t lr = above ? D + rows + k : k;
-                s_col[colour][(lr << lg_row) + r] = slab_take(src, tag31);
+                reinterpret_cast<uint4 *>(s_col[colour])[(lr << lg_wrow) + wr] = slab_take4(src, tag31);
             }
         }
 #pragma unroll 1
@@ -171,13 +189,21 @@ k_sweep_slab(const __grid_constant__ SlabArgs a, const __grid_constant__ PhiloxS
             philox_half_consts(make_sweep_key(a.seed, t, (uint32_t)half), pk.rk0, pk.rk1, pc.x1, pc.y2, pc.z2, pc.w3);
             int totU = 0, totBN = 0, totS = 0, nsites = 0;
             if (half == 0) thrB = thrM = 0;
-            const uint32_t wtag = ((e >> 1) & 1u) << 31;
+            const uint32_t wtag = ((e >> 1) & 1u) << 31, e_par = e & 1u;
             // Row order: the 2 D rows the neighbours wait for first (first D and last D own rows), then the others.
+            // A thread takes one 16-byte word (16 sites, four independent Philox calls) at a time: the update of a
+            // word is the tiled family's (March::update_word), fed from shared memory.
             const uint32_t nA = publish ? 2u * D : 0u, nrows = rows + 2u * ext;
-            const uint32_t total = nrows << lg_row;
+            const uint32_t total = nrows << lg_wrow;
+            March<MODEL, DIMS, TRACK, OBS, NEV> W;
+            W.s_t = s_t;
+            W.one = (uint32_t)a.one;
+            W.ne_t32 = ne_t32;
+            W.ne_always = ne_always;
+            W.ne_all4 = ne_all4;
 #pragma unroll 1
             for (uint32_t i = tid; i < total; i += nthr) {
-                const uint32_t s = i >> lg_row, r = i & (rowl - 1);
+                const uint32_t s = i >> lg_wrow, wr = i & (wrow - 1);
                 uint32_t lr;
                 if (s < nA) lr = s < D ? D + s : rows + (s - D);
                 else if (!publish) lr = D - ext + s;
@@ -186,49 +212,37 @@ k_sweep_slab(const __grid_constant__ SlabArgs a, const __grid_constant__ PhiloxS
                     lr = s2 < ext ? D - ext + s2 : (s2 < ext + mid ? 2u * D + (s2 - ext) : rows + D + (s2 - ext - mid));
                 }
                 const bool own_row = lr >= D && lr < D + rows;
-                const uint32_t x = r & (lpr - 1), y = r >> lg_lpr;
+                const uint32_t xw = wr & (wpr - 1), y = wr >> lg_wpr;
                 const uint32_t m = (mbase + lr) & Lm;
                 const uint32_t qq = (m + y + (uint32_t)half) & 1u;
-                const uint32_t li = (lr << lg_row) + r;
-                const uint32_t gl = (m << lg_row) + r;          // lane index in the colour array = Philox group (D2)
-                const uint32_t c = oth[li], o = own[li];
-                const uint32_t p = oth[li - rowl], n = oth[li + rowl];
-                const uint32_t cs = oth[(li - x) + ((qq ? x + 1u : x - 1u) & (lpr - 1))];
-                const uint32_t sd = qq ? __funnelshift_r(c, cs, 8) : __funnelshift_r(cs, c, 24);
-                uint32_t yp = 0, yn = 0;
+                const uint32_t wi = (lr << lg_wrow) + wr;           // word index in the shared colour array
+                const uint4 *const othw = reinterpret_cast<const uint4 *>(oth);
+                W.C = othw[wi];
+                W.P = othw[wi - wrow];
+                const uint4 N = othw[wi + wrow];
+                const uint4 O = reinterpret_cast<const uint4 *>(own)[wi];
+                // the lane beyond the word's end in its compact row: first lane of the next word (q = 1) or last lane of
+                // the previous one (q = 0), periodic in x
+                const uint32_t edge = oth[(((wi - xw) + ((qq ? xw + 1u : xw - 1u) & (wpr - 1))) << 2) + (qq ? 0u : 3u)];
+                uint4 Yp = make_uint4(0u, 0u, 0u, 0u), Yn = Yp;
                 if (DIMS == 3) {
-                    yp = oth[(lr << lg_row) + (((y - 1u) & (R - 1)) << lg_lpr) + x];
-                    yn = oth[(lr << lg_row) + (((y + 1u) & (R - 1)) << lg_lpr) + x];
+                    Yp = othw[(lr << lg_wrow) + (((y - 1u) & (R - 1)) << lg_wpr) + xw];
+                    Yn = othw[(lr << lg_wrow) + (((y + 1u) & (R - 1)) << lg_wpr) + xw];
                 }
-                int lU = 0, lBN = 0, lS = 0;                    // this lane's sums: counted for own rows only
-                uint32_t out;
-                if (MODEL == M_ISING_HALF) {
-                    uint32_t ns = p + n + c + sd;
-                    if (DIMS == 3) ns += yp + yn;
-                    out = rule_half<TRACK, OBS, NEV>(o, ns, philox_sweep(gl, pc), s_t, (uint32_t)a.one, lU, lBN);
-                } else if (MODEL == M_ISING_ONE) {
-                    uint32_t ns;
-                    if (TRACK) {
-                        ns = ((p + n) & 0x0F0F0F0Fu) + ((c + sd) & 0x0F0F0F0Fu);
-                        if (DIMS == 3) ns += (yp + yn) & 0x0F0F0F0Fu;
-                    } else {
-                        ns = p + n + c + sd;
-                        if (DIMS == 3) ns += yp + yn;
-                    }
-                    out = rule_one<DIMS, TRACK, OBS, NEV>(o, ns, philox_sweep(2u * gl, pc), philox_sweep(2u * gl + 1u, pc), s_t,
-                                                          (uint32_t)a.one, lU, lBN, lS);
-                } else {
-                    uint32_t accU = 0;
-                    out = rule_ne<TRACK, MODEL == M_NE_METROPOLIS, OBS>(o, n, qq ? sd : c, gl, pc, ne_t32, ne_always, accU);
-                    if (OBS >= 1) lU = (int)bytesum(accU);
+                W.q = (int)qq;
+                W.grp = ((m << lg_wrow) + wr) << 2;                 // Philox group of the word's first lane (D2)
+                W.totU = W.totBN = W.totS = 0;                      // this word's sums: counted for own rows only
+                const uint4 out = W.template update_word<2, true>(pc, N, O, edge, Yp, Yn);
+                reinterpret_cast<uint4 *>(own)[wi] = out;
+                if (s < nA) {
+                    uint32_t *const dst = mbox_row(g, s < D ? 0 : 1, e_par, half, s < D ? s : s - D) + (wr << 2);
+                    slab_st4_l2(dst, make_uint4(out.x | wtag, out.y | wtag, out.z | wtag, out.w | wtag));
                 }
-                own[li] = out;
-                if (s < nA) slab_st_l2(mbox_row(g, s < D ? 0 : 1, e & 1u, half, s < D ? s : s - D) + r, out | wtag);
                 if (OBS >= 1 && own_row) {
-                    totU += lU;
-                    totBN += lBN;
-                    totS += lS;
-                    nsites += 4;
+                    totU += W.totU;
+                    totBN += W.totBN;
+                    totS += W.totS;
+                    nsites += 16;
                 }
             }
             if (OBS >= 1) {
@@ -294,9 +308,9 @@ size_t slab_mailbox_bytes(int dims, int L, int model)
     return (size_t)SLAB_MAX_CTAS * 8 * (size_t)slab_depth_max(dims, L, model) * rowbytes;
 }
 
-#ifndef LSM_SLAB_DEPTH_1024
-#define LSM_SLAB_DEPTH_1024 4            // default temporal depth for L <= 1024 (2D)
-#endif
+// Default temporal depth (measured on B200, profiles/r2_slab_family.md): an exchange costs ~1 us, a redundant row
+// 1/rows of a step; 512^2 (3-4 rows per slab) runs fastest with 3, 1024^2 and 2048^2 with 2, 4096^2 and 3D with 1.
+static int slab_depth_default(int dims, int L) { return dims == 3 ? 1 : L <= 512 ? 3 : L <= 2048 ? 2 : 1; }
 
 // depth: 0 = the default for this shape, else 1 ... slab_depth_max
 bool slab_plan(const Lat &lat, int model, const TiledTables &t, int depth, SlabPlan *out)
@@ -304,7 +318,7 @@ bool slab_plan(const Lat &lat, int model, const TiledTables &t, int depth, SlabP
     if (!t.usable) return false;
     const int dmax = slab_depth_max(lat.dims, lat.L, model);
     if (dmax == 0 || depth < 0 || depth > dmax) return false;
-    int D = depth ? depth : (lat.dims == 2 && lat.L <= 1024 ? LSM_SLAB_DEPTH_1024 : dmax);
+    int D = depth ? depth : slab_depth_default(lat.dims, lat.L);
     if (D > dmax) D = dmax;
     int coop = 0, dev = 0;
     if (cudaGetDevice(&dev) != cudaSuccess) return false;
@@ -317,8 +331,8 @@ bool slab_plan(const Lat &lat, int model, const TiledTables &t, int depth, SlabP
     const long long rowl = (lat.dims == 3 ? (long long)lat.L : 1) * (lat.L / 8);   // lanes per march row and colour
     const long long smem = 2ll * (rows_max + 2 * D) * rowl * 4;
     if (smem > LSM_SLAB_SMEM_MAX) return false;
-    long long per = (long long)(rows_max + 2 * (D - 1)) * rowl;       // lanes of the largest step of the largest slab
-    int threads = (int)(per < 1024 ? ((per + 31) / 32) * 32 : 1024);
+    long long per = (long long)(rows_max + 2 * (D - 1)) * rowl / 4;   // words of the largest step of the largest slab
+    int threads = (int)(per < 512 ? ((per + 31) / 32) * 32 : 512);
     if (threads < 64) threads = 64;
     out->G = G;
     out->rows_max = rows_max;
