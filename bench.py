@@ -366,7 +366,8 @@ def rooflines(w, family, avg_launch_s, sm_count, sm_max_mhz):
     roofline_hbm = {"bound": "hbm", "achieved": hbm_achieved, "peak": hbm_peak, "unit": "GB/s",
                     "frac": hbm_achieved / hbm_peak, "peak_source": peak_src,
                     "algorithmic_bytes_per_update": BYTES_PER_UPDATE,
-                    "note": (f"the {lattice_mib:.0f} MiB lattice is L2-resident between launches: DRAM traffic is below the algorithmic bytes"
+                    "note": ("the lattice stays in the SMs' shared memory for the whole launch: global traffic is the boundary-row mailboxes (L2) only"
+                             if family == 5 else f"the {lattice_mib:.0f} MiB lattice is L2-resident between launches: DRAM traffic is below the algorithmic bytes"
                              if lattice_mib < 100 else f"the {lattice_mib:.0f} MiB lattice exceeds the 126 MB L2: every launch streams it from HBM")}
     return roofline, roofline_hbm
 
@@ -395,7 +396,8 @@ def other_workloads(lsm, torch, skip, sm_count, sm_max_mhz):
     out = {}
     for name, sweeps in (("cfg1", 1000), ("cfg2_T2.0", 100), ("cfg2_T2.6", 100), ("cfg3", 40), ("cfg4", 100),
                          ("cfg5_c0.10", 100), ("cfg5_c0.20", 100), ("cfg5_c0.30", 100), ("hbm3d_1024", 6),
-                         ("cold2d_T0.30", 100)):
+                         ("cold2d_T0.30", 100), ("mid2d_512", 2000), ("mid2d_1024", 1000), ("mid2d_2048", 400),
+                         ("mid2d_4096", 100), ("mid3d_128", 400)):
         if name == skip:
             continue
         w = W.by_name(name)
@@ -419,7 +421,9 @@ def other_workloads(lsm, torch, skip, sm_count, sm_max_mhz):
             gf = w.N * sweeps * reps / s / 1e9
             out[name] = {"gflips": gf, "alg_GBps": gf * BYTES_PER_UPDATE, "us_per_sweep": s / (sweeps * reps) * 1e6,
                          "kernel_family": KERNEL_FAMILY.get(lat.kernel, "?")}
-            if lat.kernel == 2:           # one launch per half-sweep: the per-launch rooflines apply
+            if lat.kernel == 5:
+                out[name]["temporal_depth"] = lat.temporal_depth
+            if lat.kernel in (2, 5):      # per half-sweep: one launch (tiled) or that share of one launch (slab)
                 r, rh = rooflines(w, lat.kernel, s / (2 * sweeps * reps), sm_count, sm_max_mhz)
                 out[name]["roofline"] = {k: r[k] for k in ("bound", "achieved", "peak", "unit", "frac", "traffic",
                                                            "traffic_source", "binding_bound", "avg_launch_us")}

@@ -80,6 +80,13 @@ def extras() -> dict[str, Workload]:
                                   note="2D Ising spin-1/2 32768^2 (1 GiB of spins)")
     out["cold2d_T0.30"] = Workload("cold2d_T0.30", 7, 2, 8192, T=0.30, seed=seed_of(7), sweeps=100,
                                    note="2D Ising spin-1/2 8192^2 at T = 0.30: thresholds with never-accepted entries")
+    # mid-size lattices (between the paper's own 32^2 ... 512^2, and BASELINE.json's 8192^2): a
+    # half-sweep is shorter than a kernel launch, the regime of the slab family (lattice resident in shared memory)
+    for L, n in ((512, 2000), (1024, 1000), (2048, 400), (4096, 100)):
+        out[f"mid2d_{L}"] = Workload(f"mid2d_{L}", 8, 2, L, T=2.269, seed=seed_of(8, L // 512), sweeps=n,
+                                     note=f"2D Ising spin-1/2 {L}^2 near Tc, (E, M) after every sweep")
+    out["mid3d_128"] = Workload("mid3d_128", 8, 3, 128, T=4.5115, seed=seed_of(8, 9), sweeps=400,
+                                note="3D Ising spin-1/2 128^3 near the 3D Tc")
     return out
 
 
