@@ -33,7 +33,7 @@ INT_SLOTS_PER_UPDATE_SPIN1 = 22
 # dram__bytes_read.sum + dram__bytes_write.sum per half-sweep launch, from the `ncu --set full` captures summarised
 # under profiles/ (caches flushed by ncu before the launch): workload -> (bytes, summary file)
 NCU_DRAM_BYTES_PER_LAUNCH = {
-    "cfg2_T2.269": (67.18e6 + 0.83e6, "profiles/r1_tiled_ncu_full.md"),
+    "cfg2_T2.269": (67.17e6 + 0.84e6, "profiles/r2_cfg2_final.md"),
     "cfg3": (138.46e6 + 28.19e6, "profiles/r2_tiled_variants_ncu.md"),
     "cfg4": (16.86e6 + 0.0e6, "profiles/r2_tiled_variants_ncu.md"),
     "cfg5_c0.10": (67.19e6 + 1.22e6, "profiles/r2_tiled_variants_ncu.md"),
