@@ -509,8 +509,11 @@ bool small_plan(const Lat &lat, int model, const TiledTables &t, SmallPlan *out,
         const long long nlanes = lat.half / 4;
         // thread blocks of the cluster: >= 128 lanes (4 warps) each, at most 16 (B200 schedules 16-block clusters;
         // measured: profiles/r1_small_family.md) -- a half-sweep of a small lattice is bound by latency, not issue
+        // ... except up to 512 lanes (64^2, 16^3): one block of <= 512 threads with bar.sync between the colours beats any
+        // cluster and its barrier (64^2: 1.00 us per sweep against 1.15-1.29 for 2-16 blocks; 32^2: 0.60 against 1.16)
         int c = 1;
-        while (c < small_max_cluster() && nlanes / (2 * c) >= 128 && 2 * c <= lat.L) c *= 2;
+        if (nlanes > 512)
+            while (c < small_max_cluster() && nlanes / (2 * c) >= 128 && 2 * c <= lat.L) c *= 2;
         if (N / c <= 196608) {                          // the slab must fit shared memory
             out->lane = 1;
             out->cluster = c;
