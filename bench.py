@@ -397,13 +397,13 @@ def other_workloads(lsm, torch, skip, sm_count, sm_max_mhz):
     for name, sweeps in (("cfg1", 1000), ("cfg2_T2.0", 100), ("cfg2_T2.6", 100), ("cfg3", 40), ("cfg4", 100),
                          ("cfg5_c0.10", 100), ("cfg5_c0.20", 100), ("cfg5_c0.30", 100), ("hbm3d_1024", 6),
                          ("cold2d_T0.30", 100), ("mid2d_512", 2000), ("mid2d_1024", 1000), ("mid2d_2048", 400),
-                         ("mid2d_4096", 100), ("mid3d_128", 400)):
+                         ("mid2d_4096", 100), ("mid3d_128", 400), ("ea2d_8192", 100), ("ea3d_512", 40), ("potts2d_q3_4096", 20)):
         if name == skip:
             continue
         w = W.by_name(name)
         try:
             lat = lsm.Lattice(**w.create_args())
-            if w.model == lsm.ISING:
+            if w.model in (lsm.ISING, lsm.EA, lsm.POTTS):
                 lat.set_tracking(False)
             obs = torch.empty((sweeps, 2), dtype=torch.int64, device="cuda")
             lat.sweep_record(sweeps, out=obs)
@@ -413,7 +413,7 @@ def other_workloads(lsm, torch, skip, sm_count, sm_max_mhz):
             e0.record()
             for _ in range(reps):
                 lat.sweep_record(sweeps, out=obs)
-                if w.model != lsm.ISING:
+                if w.model in (lsm.NE_HEATBATH, lsm.NE_METROPOLIS):
                     lat.persistence()
             e1.record()
             torch.cuda.synchronize()

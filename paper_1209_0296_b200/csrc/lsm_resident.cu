@@ -236,7 +236,7 @@ bool resident_plan(const Lat &lat, int model, int track, const TiledTables &t, R
     ResidentPlan p;
     memset(&p, 0, sizeof(p));
     if (!tiled_supported(lat, model, t)) return false;
-    if (model == M_EA) return false;                       // no resident instantiation for the NEXT-4 models
+    if (model == M_EA || model == M_POTTS) return false;   // no resident instantiation for the NEXT-4 models
     if (t.has_never) return false;                         // two-compare kernels exist in the tiled family only
     int coop = 0, dev = 0;
     if (cudaGetDevice(&dev) != cudaSuccess) return false;

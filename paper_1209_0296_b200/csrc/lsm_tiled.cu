@@ -53,7 +53,7 @@ k_sweep_tiled(const __grid_constant__ TiledGeom g, const __grid_constant__ Philo
     } sm;
     // two-stage per-thread ring of the asynchronous copies (March::step_pf): N, O [, Yp, Yn] words and the edge lane
     // (spin-1 keeps the direct loads: its rule needs the registers the copies' addresses would take)
-    constexpr bool PF = LSM_TILED_PF_ONE || MODEL != M_ISING_ONE;
+    constexpr bool PF = LSM_TILED_PF_ONE || (MODEL != M_ISING_ONE && MODEL != M_POTTS);
     __shared__ __align__(16) uint4 ring[PF ? ((DIMS == 3 ? 8 : 4) + (MODEL == M_EA ? 2 : 0)) * 256 : 1];
     __shared__ uint32_t ringE[PF ? 2 * 256 : 1];
     // Programmatic dependent launch: the next half-sweep's CTAs may be scheduled as soon as SM resources
@@ -67,7 +67,8 @@ k_sweep_tiled(const __grid_constant__ TiledGeom g, const __grid_constant__ Philo
     M.ne_t32 = 0;
     M.ne_always = 0;
     M.ne_all4 = false;
-    if constexpr (MODEL == M_ISING_HALF || MODEL == M_EA) {
+    M.potts_qm1 = (uint32_t)g.qm1;
+    if constexpr (MODEL == M_ISING_HALF || MODEL == M_EA || MODEL == M_POTTS) {
         if (threadIdx.x < 16) sm.t[threadIdx.x] = tab.t[threadIdx.x];
         if (NEV && threadIdx.x < 16) sm.t[16 + threadIdx.x] = ytab.y[threadIdx.x];
     } else if constexpr (MODEL == M_ISING_ONE) {
@@ -93,7 +94,7 @@ k_sweep_tiled(const __grid_constant__ TiledGeom g, const __grid_constant__ Philo
         const int col = (int)(gt - (long long)seg * g.ncol);
         const int n = march_init(M, g, g.own, g.oth, g.half, seg, col, true);
         nsites = 16 * n;
-        if constexpr (MODEL == M_ISING_ONE && LSM_TILED_ONE_UNROLL1 && !PF) {
+        if constexpr ((MODEL == M_ISING_ONE || MODEL == M_POTTS) && LSM_TILED_ONE_UNROLL1 && !PF) {
             M.template run1<true>(n, pc);
         } else
         if (g.parity_rows) {            // warp-uniform branch: q is a constant inside each loop
@@ -123,7 +124,14 @@ void build_tiled_tables(int model, int dims, double J, double h, const uint64_t 
     const int d = dims;
     (void)J; (void)h; (void)nthr;
     if (model == M_POTTS) {
-        t.usable = 0;                                       // scalar family only
+        // reading D26: thr[dn + 2d], 4d + 1 <= 13 entries, indexed directly
+        t.usable = 1;
+        for (int j = 0; j <= 4 * d; ++j) {
+            const uint64_t v = thr[j];
+            if (v == 0) t.has_never = 1;
+            t.t32[j] = v == 0 ? 0u : (uint32_t)(v - 1);
+            t.y32[j] = v == 0 ? 1u : 0u;
+        }
     } else if (model == M_ISING_HALF || model == M_EA) {
         t.usable = 1;
         for (int b = 0; b < 2; ++b)
@@ -165,10 +173,9 @@ void build_tiled_tables(int model, int dims, double J, double h, const uint64_t 
 bool tiled_supported(const Lat &lat, int model, const TiledTables &t)
 {
     if (!t.usable) return false;
-    if (model == M_POTTS) return false;                    // scalar family only
     if (lat.Lh % 16 != 0) return false;                    // whole 16-byte words per compact row
     if (lat.half / 4 > 0xFFFFFFFFll) return false;         // Philox group must fit c0 (c1 = 0 is hoisted)
-    if (model == M_ISING_ONE && lat.half / 2 > 0xFFFFFFFFll) return false;
+    if ((model == M_ISING_ONE || model == M_POTTS) && lat.half / 2 > 0xFFFFFFFFll) return false;
     return true;
 }
 
@@ -214,7 +221,7 @@ static cudaError_t launch_track(bool track, int obs_mode, dim3 grid, cudaStream_
 {
     NevTab yt;
     memset(&yt, 0, sizeof(yt));
-    constexpr bool CAN_NEV = MODEL == M_ISING_HALF || MODEL == M_ISING_ONE || MODEL == M_EA;
+    constexpr bool CAN_NEV = MODEL == M_ISING_HALF || MODEL == M_ISING_ONE || MODEL == M_EA || MODEL == M_POTTS;
     if constexpr (CAN_NEV) {
         if (nev && nev->has_never) {                       // a table with a "never" entry: the two-compare kernels
             for (int i = 0; i < 64; ++i) yt.y[i] = nev->y32[i];
@@ -239,6 +246,7 @@ cudaError_t launch_sweep_tiled(const SweepArgs &a, const TiledTables &t, cudaStr
     g.obs = a.obs;
     g.one = 1;
     g.bnd = a.model == M_EA ? (a.half ? a.lat.bnd[1] : a.lat.bnd[0]) : nullptr;
+    g.qm1 = a.model == M_POTTS ? a.lat.q - 1 : 0;
     // q = (march + y + colour) & 1 is warp-uniform if a warp sees one row parity only
     if (g.R == 1) g.parity_rows = 1;                                   // 2D: y = 0 for every thread
     else if (g.wpr % 32 == 0) g.parity_rows = 1;
@@ -275,6 +283,12 @@ cudaError_t launch_sweep_tiled(const SweepArgs &a, const TiledTables &t, cudaStr
         for (int i = 0; i < 64; ++i) ot.t[i] = t.s1[i];
         return d3 ? launch_track<M_ISING_ONE, 3>(track, obs_mode, grid, s, g, pc, ot, &t)
                   : launch_track<M_ISING_ONE, 2>(track, obs_mode, grid, s, g, pc, ot, &t);
+    }
+    case M_POTTS: {
+        HalfTab ht;
+        for (int i = 0; i < 16; ++i) ht.t[i] = t.t32[i];
+        return d3 ? launch_track<M_POTTS, 3>(track, obs_mode, grid, s, g, pc, ht, &t)
+                  : launch_track<M_POTTS, 2>(track, obs_mode, grid, s, g, pc, ht, &t);
     }
     case M_NE_HEATBATH: {
         NeTab nt = {t.ne_t32[0], 0, t.ne_all4};

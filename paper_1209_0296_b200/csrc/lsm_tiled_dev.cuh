@@ -30,7 +30,7 @@ namespace lsmk {
 
 constexpr int tiled_minblocks(int model)
 {
-    return model == M_ISING_ONE ? LSM_TILED_MINBLOCKS_ONE
+    return (model == M_ISING_ONE || model == M_POTTS) ? LSM_TILED_MINBLOCKS_ONE
          : (model == M_ISING_HALF || model == M_EA) ? LSM_TILED_MINBLOCKS_HALF : LSM_TILED_MINBLOCKS;
 }
 
@@ -127,6 +127,7 @@ struct TiledGeom {
     int one;               // the constant 1, kept opaque to the compiler (see rule_half)
     long long *obs;        // (B, M) accumulator or nullptr
     const uint8_t *bnd;    // M_EA: bond bytes of the colour being updated (same geometry as own); else nullptr
+    int qm1;               // M_POTTS: q - 1
 };
 
 struct HalfTab { uint32_t t[16]; };            // spin-1/2: t[n + 8*b] = thr - 1  (accept iff w <= t)
@@ -141,6 +142,7 @@ template <int MODEL> struct TabOf { using type = NeTab; };
 template <> struct TabOf<M_ISING_HALF> { using type = HalfTab; };
 template <> struct TabOf<M_ISING_ONE> { using type = OneTab; };
 template <> struct TabOf<M_EA> { using type = HalfTab; };     // reading D25: the Ising table on the bond-weighted up-count
+template <> struct TabOf<M_POTTS> { using type = HalfTab; };  // reading D26: t[dn + 2d] = thr - 1, 4d + 1 <= 13 entries
 
 __device__ __forceinline__ uint32_t bytesum(uint32_t v) { return __dp4a(v, 0x01010101u, 0u); }
 
@@ -303,6 +305,49 @@ __device__ __forceinline__ uint32_t rule_one(uint32_t own, uint32_t nsum, uint4 
     return nw;
 }
 
+// q-state Potts (reading D26), q <= 8, byte-parallel over the 4 sites of a lane.  Two words per site as for spin-1
+// (ra: sites 0, 1; rb: sites 2, 3; proposal word x / z, acceptance word y / w).
+//   proposal  s' = (s + 1 + mulhi32(w0, q-1)) mod q: the four r's packed into bytes, t = s + 1 + r <= 2q - 2 <= 14, and
+//             t >= q  <=>  bit 4 of t + (16 - q)  (no byte reaches 32): s' = t - q * that bit
+//   counts    "neighbour differs from x" = bit 3 of ((v ^ x) & 7) + 7  (a 3-bit value is non-zero iff adding 7 reaches 8);
+//             summed over the 2d neighbours in units of 8 (<= 48 per byte: no carry) for x = s and x = s'
+//   index     dn + 2d = (ne_old - ne_new) / 8 + 2d, so the table byte offset 4 (dn + 2d) = (ne_old + 16 d - ne_new) >> 1
+//   accept    iff w1 <= t[dn + 2d] (per site: extract, LDS, ISETP, predicated IMAD, as in rule_one)
+// Observables (raw sums in units of 8; march_observables converts): totNZ = sum of "final state != 0",
+// totNE = sum of "neighbours different from the final state".
+template <int DIMS, bool TRACK, int OBS, bool NEV = false>
+__device__ __forceinline__ uint32_t rule_potts(uint32_t own, const uint32_t (&nb)[2 * DIMS], uint4 ra, uint4 rb, uint32_t qm1,
+                                               uint32_t s_t, uint32_t one, int &totNZ, int &totNE)
+{
+    constexpr uint32_t M1 = 0x01010101u, M7 = 0x07070707u, M8 = 0x08080808u;
+    const uint32_t s = TRACK ? (own & M7) : own;
+    const uint32_t r = __umulhi(ra.x, qm1) | (__umulhi(ra.z, qm1) << 8) | (__umulhi(rb.x, qm1) << 16) | (__umulhi(rb.z, qm1) << 24);
+    const uint32_t t = s + r + M1;
+    const uint32_t ge = ((t + (15u - qm1) * M1) & 0x10101010u) >> 4;      // 16 - q = 15 - (q - 1)
+    const uint32_t prop = t - ge * (qm1 + 1u);
+    uint32_t ne_old = 0u, ne_new = 0u;
+#pragma unroll
+    for (int k = 0; k < 2 * DIMS; ++k) {
+        ne_old += (lop3<0x28>(nb[k], s, M7) + M7) & M8;
+        ne_new += (lop3<0x28>(nb[k], prop, M7) + M7) & M8;
+    }
+    const uint32_t adr = (ne_old + (uint32_t)(16 * DIMS) * M1 - ne_new) >> 1;
+    uint32_t acc = 0u;                                     // 0xFF in the byte of every accepted site
+    acc = accept_site<M_POTTS, NEV, 0x000000FFu>(acc, ra.y, s_t, adr & 0xFFu, one);
+    acc = accept_site<M_POTTS, NEV, 0x0000FF00u>(acc, ra.w, s_t, __byte_perm(adr, 0u, 0x4441), one);
+    acc = accept_site<M_POTTS, NEV, 0x00FF0000u>(acc, rb.y, s_t, __byte_perm(adr, 0u, 0x4442), one);
+    acc = accept_site<M_POTTS, NEV, 0xFF000000u>(acc, rb.w, s_t, adr >> 24, one);
+    const uint32_t fl = (s ^ prop) & acc;                  // change of the three state bits
+    uint32_t nw = own ^ fl;
+    if (TRACK) nw |= (fl + M7) & M8;                       // "ever changed" (0x08): the state bits changed
+    if (OBS >= 1) {
+        const uint32_t sn = s ^ fl;
+        totNZ = (int)__dp4a((sn + M7) & M8, M1, (uint32_t)totNZ);
+        if (OBS >= 2) totNE = (int)__dp4a(ne_old ^ ((ne_old ^ ne_new) & acc), M1, (uint32_t)totNE);
+    }
+    return nw;
+}
+
 // ------------------------------------------------------------------------------------------
 // One thread's march.  Q is the row parity bit q = (march + cross + colour) & 1 of the current step
 // when it is known at compile time (0 / 1: the side neighbour is the byte to the left / right), or
@@ -323,6 +368,7 @@ struct March {
     uint32_t ne_t32;
     int ne_always;
     bool ne_all4;
+    uint32_t potts_qm1;     // M_POTTS: q - 1
 
     // One step at march position m.  The march runs upwards (rowstride > 0, the tiled family and the even
     // half-sweeps of the resident family) or downwards (rowstride < 0): P is the row the march came
@@ -403,6 +449,19 @@ struct March {
                 uint4 ra = philox_sweep(2u * (grp + d), pc);
                 uint4 rb = philox_sweep(2u * (grp + d) + 1u, pc);
                 out[d] = rule_one<DIMS, TRACK, OBS, NEV>(o[d], ns, ra, rb, s_t, one, totU, totBN, totS);
+            }
+        } else if (MODEL == M_POTTS) {
+#pragma unroll
+            for (int d = 0; d < 4; ++d) {
+                uint4 ra = philox_sweep(2u * (grp + d), pc);
+                uint4 rb = philox_sweep(2u * (grp + d) + 1u, pc);
+                if constexpr (DIMS == 3) {
+                    const uint32_t nb[6] = {p[d], n[d], c[d], sd[d], yp[d], yn[d]};
+                    out[d] = rule_potts<3, TRACK, OBS, NEV>(o[d], nb, ra, rb, potts_qm1, s_t, one, totU, totBN);
+                } else {
+                    const uint32_t nb[4] = {p[d], n[d], c[d], sd[d]};
+                    out[d] = rule_potts<2, TRACK, OBS, NEV>(o[d], nb, ra, rb, potts_qm1, s_t, one, totU, totBN);
+                }
             }
         } else {
             uint32_t accU = 0;
@@ -747,6 +806,11 @@ __device__ __forceinline__ void march_observables(const March<MODEL, DIMS, TRACK
         // s' = a' - 1, nn = sum - 2d:  M = SA - n;  B = sum s' nn = SAS - 2d SA - SS + 2d n   (second colour only)
         cM = (long long)M.totU - nsites;
         if (second) cB = (long long)M.totBN - 2LL * DIMS * M.totU - M.totS + 2LL * DIMS * nsites;
+    } else if (MODEL == M_POTTS) {
+        // M = sites in state 0 = n - (non-zero sites); B = sum over the second colour of the neighbours equal to the final
+        // state = 2d n - (neighbours that differ); both raw sums are in units of 8
+        cM = (long long)nsites - M.totU / 8;
+        if (second) cB = 2LL * DIMS * nsites - M.totBN / 8;
     } else {
         cM = M.totU;
     }

@@ -9,7 +9,7 @@ from __future__ import annotations
 import math
 from dataclasses import dataclass, replace
 
-ISING, NE_HEATBATH, NE_METROPOLIS = 0, 1, 2
+ISING, NE_HEATBATH, NE_METROPOLIS, EA, POTTS = 0, 1, 2, 3, 4
 
 
 def seed_of(cfg: int, variant: int = 0) -> int:
@@ -85,6 +85,13 @@ def extras() -> dict[str, Workload]:
     for L, n in ((512, 2000), (1024, 1000), (2048, 400), (4096, 100)):
         out[f"mid2d_{L}"] = Workload(f"mid2d_{L}", 8, 2, L, T=2.269, seed=seed_of(8, L // 512), sweeps=n,
                                      note=f"2D Ising spin-1/2 {L}^2 near Tc, (E, M) after every sweep")
+    # SURVEY.md 8(f) NEXT-4 models (readings D25, D26): the +/-J Edwards-Anderson glass and the q-state Potts model
+    out["ea2d_8192"] = Workload("ea2d_8192", 9, 2, 8192, model=EA, T=1.0, seed=seed_of(9, 0), sweeps=100,
+                                note="2D Edwards-Anderson +/-J spin glass 8192^2, bonds from the seed")
+    out["ea3d_512"] = Workload("ea3d_512", 9, 3, 512, model=EA, T=1.1, seed=seed_of(9, 1), sweeps=40,
+                               note="3D Edwards-Anderson +/-J spin glass 512^3 near its glass temperature")
+    out["potts2d_q3_4096"] = Workload("potts2d_q3_4096", 9, 2, 4096, two_S=2, model=POTTS, T=0.995, seed=seed_of(9, 2),
+                                      sweeps=20, note="2D 3-state Potts 4096^2 at its transition T = 1/ln(1+sqrt 3)")
     out["mid3d_128"] = Workload("mid3d_128", 8, 3, 128, T=4.5115, seed=seed_of(8, 9), sweeps=400,
                                 note="3D Ising spin-1/2 128^3 near the 3D Tc")
     return out

@@ -126,13 +126,29 @@ POTTS_SHAPES = [
     (dict(dims=3, L=6, two_S=3, T=1.5), 12),
     (dict(dims=3, L=32, two_S=2, T=1.82), 6),
     (dict(dims=3, L=34, two_S=5, T=1.2), 4),
+    # whole 16-byte words per row: the vectorised rule of the tiled family (byte-parallel equal-neighbour counts)
+    (dict(dims=2, L=256, two_S=2, T=0.995), 12),
+    (dict(dims=2, L=96, two_S=1, T=1.1), 12),         # q = 2
+    (dict(dims=2, L=160, two_S=6, T=0.75, J=1.3), 10),  # q = 7
+    (dict(dims=2, L=1024, two_S=3, T=0.91), 5),
+    (dict(dims=3, L=64, two_S=7, T=1.0), 4),          # q = 8 in 3D
+    (dict(dims=3, L=96, two_S=2, T=0.05), 3),         # 3D, "never" thresholds
+    (dict(dims=3, L=32, two_S=4, T=1.4, J=-0.7), 6),
 ]
 
 
+@pytest.mark.parametrize("family", [lsm.KERNEL_AUTO, lsm.KERNEL_GENERIC, lsm.KERNEL_TILED])
 @pytest.mark.parametrize("kw,n", POTTS_SHAPES)
-def test_potts_parity(kw, n):
+def test_potts_parity(kw, n, family):
     kw = dict(kw, model=lsm.POTTS, seed=(0x9077 << 32) + 11 * kw["L"] + kw["two_S"])
     lat, orc = lsm.Lattice(**kw), O.Oracle(**kw)
+    try:
+        lat.set_kernel(family)
+    except lsm.LsmError as e:
+        assert e.code == lsm.ERR_UNSUPPORTED
+        pytest.skip("this family does not cover this lattice")
+    if family == lsm.KERNEL_AUTO and kw["L"] % 32 == 0:
+        assert lat.kernel == lsm.KERNEL_TILED
     assert lat.thresholds() == orc.thresholds()
     same_state(lat, orc)
     half = n // 2
