@@ -208,7 +208,7 @@ def run_ours(args, w):
 
     wl = replace(w, seed=replicas.rank_seed(w.seed, rank))  # replicas: independent seeds, no communication
     lat = lsm.Lattice(**wl.create_args(), device=f"cuda:{local}")
-    if wl.model == lsm.ISING:
+    if wl.model in (lsm.ISING, lsm.EA, lsm.POTTS):
         lat.set_tracking(False)  # persistence is not part of configs 1-4
     if args.kernel != "auto":
         lat.set_kernel({"generic": lsm.KERNEL_GENERIC, "tiled": lsm.KERNEL_TILED, "resident": lsm.KERNEL_RESIDENT,
