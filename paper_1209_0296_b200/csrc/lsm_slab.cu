@@ -18,7 +18,7 @@
 //     (of the colour updated in that step) into its mailbox in global memory (L2); the adjacent CTAs copy them into
 //     their halos at the start of the next epoch.  Mailbox lanes validate themselves: bit 31 of every 32-bit lane
 //     (bit 7 of a site byte is unused by every encoding, lsm_internal.cuh) carries one bit of the epoch number and the
-//     reader spins on each lane until it shows the expected one -- no flag, no fence.  One exchange costs about one
+//     reader spins on a 16-byte word until its four lanes show the expected one -- no flag, no fence.  One exchange costs about one
 //     microsecond of latency on B200 whatever its size, which is why it pays to make it once per D half-sweeps;
 //   * D = 1 is the plain scheme (one row of the colour just updated per half-sweep, no redundant update).
 // Mailboxes are double-buffered by epoch parity: a CTA rewrites buffer e & 1 in epoch e + 2, which it can only start
@@ -48,25 +48,9 @@ struct SlabArgs {
     uint32_t *mbox;              // [G][first, last][epoch parity][colour][dmax][lanes of a march row]
 };
 
-__device__ __forceinline__ uint32_t slab_ld_l2(const uint32_t *p)
-{
-    uint32_t v;
-    asm volatile("ld.relaxed.gpu.global.u32 %0, [%1];" : "=r"(v) : "l"(p) : "memory");
-    return v;
-}
-__device__ __forceinline__ void slab_st_l2(uint32_t *p, uint32_t v)
-{
-    asm volatile("st.relaxed.gpu.global.u32 [%0], %1;" ::"l"(p), "r"(v) : "memory");
-}
-// spin until the lane carries the expected epoch bit in bit 31; returns the lane without it
-__device__ __forceinline__ uint32_t slab_take(const uint32_t *p, uint32_t tag31)
-{
-    uint32_t v;
-    do { v = slab_ld_l2(p); } while (((v ^ tag31) & 0x80000000u) != 0u);
-    return v & 0x7FFFFFFFu;
-}
-
-// the same for the four lanes of a 16-byte word (each lane carries its own epoch bit, so a torn word is only retried)
+// L2-coherent 16-byte accesses to a mailbox word (relaxed, gpu scope: never served from or parked in this SM's L1)
+// spin until all four lanes of the word carry the expected epoch bit in bit 31 (each lane carries its own, so a torn
+// word is only retried); returns the word without the bits
 __device__ __forceinline__ uint4 slab_take4(const uint32_t *p, uint32_t tag31)
 {
     uint4 v;
