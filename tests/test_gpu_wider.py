@@ -134,6 +134,8 @@ POTTS_SHAPES = [
     (dict(dims=3, L=64, two_S=7, T=1.0), 4),          # q = 8 in 3D
     (dict(dims=3, L=96, two_S=2, T=0.05), 3),         # 3D, "never" thresholds
     (dict(dims=3, L=32, two_S=4, T=1.4, J=-0.7), 6),
+    (dict(dims=2, L=2048, two_S=2, T=0.995), 4),      # many CTAs, several march segments per word column
+    (dict(dims=3, L=128, two_S=2, T=1.82), 3),
 ]
 
 
