@@ -40,11 +40,11 @@ NCU_DRAM_BYTES_PER_LAUNCH = {
     "cfg5_c0.30": (67.18e6 + 0.75e6, "profiles/r2_tiled_variants_ncu.md"),
     "hbm3d_1024": (1083.86e6 + 497.63e6, "profiles/r2_tiled_variants_ncu.md"),
 }
-KERNEL_FAMILY = {1: "generic", 2: "tiled", 3: "resident", 4: "small", 5: "slab"}
+KERNEL_FAMILY = {1: "generic", 2: "tiled", 3: "resident", 4: "small", 5: "slab", 6: "bulk"}
 KERNEL_NAME = {1: "k_sweep_generic (half-sweep)", 2: "k_sweep_tiled (half-sweep)",
                3: "k_sweep_resident (per half-sweep share of one launch)",
                4: "k_sweep_small_lane (per half-sweep share of one launch)",
-               5: "k_sweep_slab (per half-sweep share of one launch)"}
+               5: "k_sweep_slab (per half-sweep share of one launch)", 6: "k_sweep_tiled_bulk (half-sweep)"}
 
 
 def parse():
@@ -61,7 +61,7 @@ def parse():
                     help="instead of the benchmark: us/sweep of the tiled and the small (cluster) family over lattice sizes")
     ap.add_argument("--pipe-probe", action="store_true",
                     help="instead of the benchmark: the integer-pipe microbenchmarks behind the 'alu' roofline (DESIGN.md 6)")
-    ap.add_argument("--kernel", default="auto", choices=["auto", "generic", "tiled", "resident", "small", "slab"],
+    ap.add_argument("--kernel", default="auto", choices=["auto", "generic", "tiled", "resident", "small", "slab", "bulk"],
                     help="kernel family (lsm_set_kernel); auto = the library's choice")
     return ap.parse_args()
 
@@ -212,7 +212,7 @@ def run_ours(args, w):
         lat.set_tracking(False)  # persistence is not part of configs 1-4
     if args.kernel != "auto":
         lat.set_kernel({"generic": lsm.KERNEL_GENERIC, "tiled": lsm.KERNEL_TILED, "resident": lsm.KERNEL_RESIDENT,
-                        "small": lsm.KERNEL_SMALL, "slab": lsm.KERNEL_SLAB}[args.kernel])
+                        "small": lsm.KERNEL_SMALL, "slab": lsm.KERNEL_SLAB, "bulk": lsm.KERNEL_BULK}[args.kernel])
     N = lat.N
     obs = torch.empty((S, 2), dtype=torch.int64, device=lat.device)
     flush = torch.empty(256 << 20, dtype=torch.uint8, device=lat.device)  # > 126 MB L2
@@ -423,7 +423,7 @@ def other_workloads(lsm, torch, skip, sm_count, sm_max_mhz):
                          "kernel_family": KERNEL_FAMILY.get(lat.kernel, "?")}
             if lat.kernel == 5:
                 out[name]["temporal_depth"] = lat.temporal_depth
-            if lat.kernel in (2, 5):      # per half-sweep: one launch (tiled) or that share of one launch (slab)
+            if lat.kernel in (2, 5, 6):      # per half-sweep: one launch (tiled) or that share of one launch (slab)
                 r, rh = rooflines(w, lat.kernel, s / (2 * sweeps * reps), sm_count, sm_max_mhz)
                 out[name]["roofline"] = {k: r[k] for k in ("bound", "achieved", "peak", "unit", "frac", "traffic",
                                                            "traffic_source", "binding_bound", "avg_launch_us")}

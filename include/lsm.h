@@ -92,10 +92,14 @@ enum {
  *           one CTA per SM: slabs of march rows, boundary rows exchanged through self-validating mailbox words in L2, one per
  *           CTA, several half-sweeps per exchange (lsm_set_temporal_depth); L a power of two, 512^2 ... 4096^2,
  *           64^3, 128^3, where AUTO chooses it;
+ *  BULK     the TILED half-sweep with its rows staged through shared memory by bulk asynchronous copies (TMA unit,
+ *           cp.async.bulk + mbarrier; one producer thread per CTA, 4-stage ring) instead of per-thread cp.async: 2D,
+ *           L a multiple of 8192, spin-1/2 and North-East.  Opt-in: measured 10 % slower than TILED on 8192^2
+ *           (profiles/r2_bulk_copy_variant.md);
  *  GENERIC  one thread per site, any even L >= 4, any table.
  * All families produce bit-identical results (same random-word map D2, same thresholds D3). */
 enum { LSM_KERNEL_AUTO = 0, LSM_KERNEL_GENERIC = 1, LSM_KERNEL_TILED = 2, LSM_KERNEL_RESIDENT = 3, LSM_KERNEL_SMALL = 4,
-       LSM_KERNEL_SLAB = 5 };
+       LSM_KERNEL_SLAB = 5, LSM_KERNEL_BULK = 6 };
 
 /* Device bytes lsm_create needs for this lattice (two colour arrays + small state). */
 int lsm_workspace_bytes(int dims, int L, int two_S, int model, size_t *bytes);

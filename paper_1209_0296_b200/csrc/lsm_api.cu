@@ -153,6 +153,8 @@ static void choose_kernel(lsm *o)
         want = tiled_ok ? LSM_KERNEL_TILED : LSM_KERNEL_GENERIC;
     if (want == LSM_KERNEL_SLAB && !slab_plan(o->lat, o->model, o->tiled, o->slab_depth, &o->slab))
         want = tiled_ok ? LSM_KERNEL_TILED : LSM_KERNEL_GENERIC;
+    if (want == LSM_KERNEL_BULK && !tiled_bulk_supported(o->lat, o->model, o->tiled))
+        want = tiled_ok ? LSM_KERNEL_TILED : LSM_KERNEL_GENERIC;
     o->kernel_in_use = want;
 }
 
@@ -235,7 +237,8 @@ static int enqueue_half(lsm *o, int half, long long *obs, int want_B, cudaStream
     a.lat = o->lat; a.model = o->model; a.half = half;
     a.key = make_sweep_key(o->seed, o->t, (uint32_t)half);
     a.track = o->tracking; a.obs = obs; a.want_B = want_B;
-    if (o->kernel_in_use == LSM_KERNEL_TILED) CU(launch_sweep_tiled(a, o->tiled, s));
+    a.bulk = o->kernel_in_use == LSM_KERNEL_BULK ? 1 : 0;
+    if (o->kernel_in_use == LSM_KERNEL_TILED || o->kernel_in_use == LSM_KERNEL_BULK) CU(launch_sweep_tiled(a, o->tiled, s));
     else CU(launch_sweep_generic(a, o->thr_param, s));
     o->launches += 1;
     return LSM_OK;
@@ -770,12 +773,13 @@ extern "C" int lsm_get_thresholds(lsm_t *o, uint64_t *out, int *count)
 
 extern "C" int lsm_set_kernel(lsm_t *o, int family)
 {
-    if (!o || family < LSM_KERNEL_AUTO || family > LSM_KERNEL_SLAB) return LSM_ERR_ARG;
+    if (!o || family < LSM_KERNEL_AUTO || family > LSM_KERNEL_BULK) return LSM_ERR_ARG;
     if (family == LSM_KERNEL_TILED && !tiled_supported(o->lat, o->model, o->tiled)) return LSM_ERR_UNSUPPORTED;
     if (family == LSM_KERNEL_RESIDENT && !resident_plan(o->lat, o->model, o->tracking, o->tiled, &o->plan))
         return LSM_ERR_UNSUPPORTED;
     if (family == LSM_KERNEL_SMALL && !small_plan(o->lat, o->model, o->tiled, &o->small, true)) return LSM_ERR_UNSUPPORTED;
     if (family == LSM_KERNEL_SLAB && !slab_plan(o->lat, o->model, o->tiled, o->slab_depth, &o->slab)) return LSM_ERR_UNSUPPORTED;
+    if (family == LSM_KERNEL_BULK && !tiled_bulk_supported(o->lat, o->model, o->tiled)) return LSM_ERR_UNSUPPORTED;
     o->kernel_pref = family;
     choose_kernel(o);
     return LSM_OK;

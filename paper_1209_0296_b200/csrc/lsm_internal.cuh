@@ -156,6 +156,7 @@ struct SweepArgs {
     int track;             // maintain "ever changed" bits
     long long *obs;        // device (B, M) accumulator of this sweep, or nullptr
     int want_B;            // add the bond sum (only meaningful after the second half)
+    int bulk;              // tiled family: rows staged by bulk copies (lsm_tiled_bulk.cu; LSM_KERNEL_BULK)
 };
 
 cudaError_t launch_init(const Lat &lat, int model, unsigned long long seed, unsigned long long thr_c,

@@ -31,6 +31,9 @@
 
 namespace lsmk {
 
+cudaError_t launch_sweep_tiled_bulk(int model, bool track, int obs_mode, TiledGeom g, const PhiloxSweepConsts &pc,
+                                    const TiledTables &t, cudaStream_t s);
+
 PhiloxSweepConsts make_philox_consts(const SweepKey &k)
 {
     PhiloxSweepConsts c;
@@ -264,6 +267,7 @@ cudaError_t launch_sweep_tiled(const SweepArgs &a, const TiledTables &t, cudaStr
     PhiloxSweepConsts pc = make_philox_consts(a.key);
     int obs_mode = a.obs ? (a.want_B ? 2 : 1) : 0;
     const bool track = a.track != 0;
+    if (a.bulk && tiled_bulk_supported(a.lat, a.model, t)) return launch_sweep_tiled_bulk(a.model, track, obs_mode, g, pc, t, s);
     const bool d3 = a.lat.dims == 3;
     switch (a.model) {
     case M_ISING_HALF: {

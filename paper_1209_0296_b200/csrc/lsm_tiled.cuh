@@ -27,6 +27,8 @@ struct TiledTables {
 void build_tiled_tables(int model, int dims, double J, double h, const uint64_t *thr, int nthr, TiledTables *out);
 bool tiled_supported(const Lat &lat, int model, const TiledTables &t);
 cudaError_t launch_sweep_tiled(const SweepArgs &a, const TiledTables &t, cudaStream_t s);
+// the same half-sweep with its rows staged through shared memory by bulk copies (lsm_tiled_bulk.cu; SweepArgs::bulk)
+bool tiled_bulk_supported(const Lat &lat, int model, const TiledTables &t);
 
 // Resident family (lsm_resident.cu): one cooperative launch runs `nsweeps` whole sweeps; CTAs
 // synchronise with the owners of the adjacent slabs only.  plan.grid CTAs must be co-resident.

@@ -15,7 +15,7 @@ _PKG = os.path.dirname(os.path.abspath(__file__))
 _LIB_PATH = os.path.join(_PKG, "liblsm.so")
 
 ISING, NE_HEATBATH, NE_METROPOLIS, EA, POTTS = 0, 1, 2, 3, 4
-KERNEL_AUTO, KERNEL_GENERIC, KERNEL_TILED, KERNEL_RESIDENT, KERNEL_SMALL, KERNEL_SLAB = 0, 1, 2, 3, 4, 5
+KERNEL_AUTO, KERNEL_GENERIC, KERNEL_TILED, KERNEL_RESIDENT, KERNEL_SMALL, KERNEL_SLAB, KERNEL_BULK = 0, 1, 2, 3, 4, 5, 6
 OK, ERR_ARG, ERR_UNSUPPORTED, ERR_CUDA, ERR_WORKSPACE, ERR_STATE = 0, -1, -2, -3, -4, -5
 
 # name -> (restype, argtypes); every symbol include/lsm.h declares

@@ -7,6 +7,7 @@ import math
 
 import numpy as np
 import pytest
+import torch
 
 from oracle import lsm_oracle as O
 from paper_1209_0296_b200 import build as B
@@ -88,7 +89,7 @@ SHAPES = [
     (dict(dims=2, L=1024, model=lsm.NE_HEATBATH, J=0.0, T=W.ne_temperature(0.3)), 16),
     (dict(dims=2, L=3072, model=lsm.NE_METROPOLIS, J=0.0, T=W.ne_temperature(0.2)), 6),
 ]
-FAMILIES = [lsm.KERNEL_GENERIC, lsm.KERNEL_TILED, lsm.KERNEL_RESIDENT, lsm.KERNEL_SMALL, lsm.KERNEL_SLAB]
+FAMILIES = [lsm.KERNEL_GENERIC, lsm.KERNEL_TILED, lsm.KERNEL_RESIDENT, lsm.KERNEL_SMALL, lsm.KERNEL_SLAB]   # + BULK: below
 
 
 def test_device_philox_known_answers_and_random():
@@ -193,6 +194,47 @@ def test_slab_temporal_blocking_parity(kw, depths):
     with pytest.raises(lsm.LsmError):
         lat.set_temporal_depth(5)
     lat.close()
+
+
+BULK_CASES = [
+    dict(dims=2, L=8192, T=2.269, h=0.05),
+    dict(dims=2, L=8192, T=0.3),                                   # "never" thresholds: the two-compare kernels
+    dict(dims=2, L=8192, model=lsm.NE_HEATBATH, J=0.0, T=W.ne_temperature(0.3)),
+    dict(dims=2, L=16384, model=lsm.NE_METROPOLIS, J=0.0, T=W.ne_temperature(0.1)),   # two 256-word chunks per row
+]
+
+
+@pytest.mark.parametrize("kw", BULK_CASES)
+def test_bulk_copy_family_parity(kw):
+    """LSM_KERNEL_BULK: the tiled half-sweep fed by bulk asynchronous copies (cp.async.bulk + mbarrier, one producer
+    thread per CTA).  Against the oracle for the first sweeps (every (B, M), configuration, persistence), then against
+    the tiled family for a longer run with tracking switched: bit-identical."""
+    seed = W.seed_of(12, kw["L"] // 8192)
+    lat = lsm.Lattice(seed=seed, **kw)
+    lat.set_kernel(lsm.KERNEL_BULK)
+    assert lat.kernel == lsm.KERNEL_BULK
+    n = 3 if kw["L"] == 8192 else 1
+    orc = O.Oracle(seed=seed, **kw)
+    assert np.array_equal(lat.sweep_record(n).cpu().numpy(), orc.sweep_record(n))
+    assert_same_state(lat, orc)
+    ref = lsm.Lattice(seed=seed, **kw)
+    ref.set_kernel(lsm.KERNEL_TILED)
+    ref.sweep(n)
+    for track in (False, True):
+        lat.set_tracking(track)
+        ref.set_tracking(track)
+        assert torch.equal(lat.sweep_record(7), ref.sweep_record(7))
+        lat.sweep(2)
+        ref.sweep(2)
+        assert torch.equal(lat.get_spins(), ref.get_spins())
+        assert lat.measure_int() == ref.measure_int() and lat.measure_full() == lat.measure_int()[:2]
+    assert lat.persistence() == ref.persistence()
+    small = lsm.Lattice(dims=2, L=4096, T=2.0, seed=1)
+    with pytest.raises(lsm.LsmError) as e:
+        small.set_kernel(lsm.KERNEL_BULK)
+    assert e.value.code == lsm.ERR_UNSUPPORTED
+    for x in (lat, ref, small):
+        x.close()
 
 
 @pytest.mark.parametrize("family", FAMILIES)
