@@ -405,6 +405,8 @@ k_sweep_small_lane_batch(const __grid_constant__ SmallBatchArgs a, const int lg_
         pk.rk1[r] = sd.y + (uint32_t)r * PHILOX_W1;
     }
     pk.x1 = pk.y2 = pk.z2 = pk.w3 = 0u;
+    pk.m0 = PHILOX_M0;
+    pk.m1 = PHILOX_M1;
     const unsigned long long seed = ((unsigned long long)sd.y << 32) | sd.x;
     long long *obs = (OBS >= 1 && a.obs) ? a.obs + a.obs_stride * (a.r0 + ci) : nullptr;
     small_lane_body<MODEL, DIMS, TRACK, OBS, LPT>(d.col[0], d.col[1], pk, seed, a.t0, a.nsweeps, obs,

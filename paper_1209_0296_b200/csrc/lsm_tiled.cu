@@ -42,6 +42,8 @@ PhiloxSweepConsts make_philox_consts(const SweepKey &k)
         c.rk1[r] = k.k1 + (uint32_t)r * PHILOX_W1;
     }
     philox_half_consts(k, c.rk0, c.rk1, c.x1, c.y2, c.z2, c.w3);
+    c.m0 = PHILOX_M0;
+    c.m1 = PHILOX_M1;
     return c;
 }
 
