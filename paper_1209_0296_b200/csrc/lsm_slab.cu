@@ -40,7 +40,7 @@ struct SlabArgs {
     int lg_lpr;                  // log2(lanes per compact row) = log2(L) - 3
     int lg_R;                    // log2(cross rows per march row): 0 in 2D, log2(L) in 3D
     int rows_max;                // most march rows of any slab (shared-memory stride)
-    int D;                       // temporal depth: half-sweeps per exchange; every slab has >= 2 D rows
+    int D;                       // temporal depth: half-sweeps per exchange; every slab has >= 2 D rows (3D: >= 1)
     int dmax;                    // mailbox rows reserved per slot
     int early;                   // D = 1, long steps: copy the halo behind the step instead of before the next one
     int one;
@@ -180,7 +180,9 @@ k_sweep_slab(const __grid_constant__ SlabArgs a, const __grid_constant__ PhiloxS
             // Row order: the 2 D rows the neighbours wait for first (first D and last D own rows), then the others.
             // A thread takes one 16-byte word (16 sites, four independent Philox calls) at a time: the update of a
             // word is the tiled family's (March::update_word), fed from shared memory.
-            const uint32_t nA = publish ? 2u * D : 0u, nrows = rows + 2u * ext;
+            // (a one-row slab -- 3D, D = 1: one plane per CTA -- has a row that is the first and the last at once and goes
+            // to both mailboxes)
+            const uint32_t nA = publish ? (DIMS == 3 && rows == 1u ? 1u : 2u * D) : 0u, nrows = rows + 2u * ext;
             const uint32_t total = nrows << lg_wrow;
             March<MODEL, DIMS, TRACK, OBS, NEV> W;
             W.s_t = s_t;
@@ -222,8 +224,13 @@ k_sweep_slab(const __grid_constant__ SlabArgs a, const __grid_constant__ PhiloxS
                 const uint4 out = W.template update_word<2, true>(pc, N, O, edge, Yp, Yn);
                 reinterpret_cast<uint4 *>(own)[wi] = out;
                 if (s < nA) {
-                    uint32_t *const dst = mbox_row(g, s < D ? 0 : 1, e_par, half, s < D ? s : s - D) + (wr << 2);
-                    slab_st4_l2(dst, make_uint4(out.x | wtag, out.y | wtag, out.z | wtag, out.w | wtag));
+                    const uint4 tagged = make_uint4(out.x | wtag, out.y | wtag, out.z | wtag, out.w | wtag);
+                    if (DIMS == 3 && rows == 1u) {
+                        slab_st4_l2(mbox_row(g, 0, e_par, half, 0u) + (wr << 2), tagged);
+                        slab_st4_l2(mbox_row(g, 1, e_par, half, 0u) + (wr << 2), tagged);
+                    } else {
+                        slab_st4_l2(mbox_row(g, s < D ? 0 : 1, e_par, half, s < D ? s : s - D) + (wr << 2), tagged);
+                    }
                 }
                 if (OBS >= 1 && own_row) {
                     totU += W.totU;
@@ -319,7 +326,9 @@ bool slab_plan(const Lat &lat, int model, const TiledTables &t, int depth, SlabP
     if (cudaDeviceGetAttribute(&coop, cudaDevAttrCooperativeLaunch, dev) != cudaSuccess || !coop) return false;
     int G = sm_count();                                               // one CTA per SM, all co-resident
     if (G > SLAB_MAX_CTAS) G = SLAB_MAX_CTAS;
-    if (G > lat.L / (2 * D)) G = lat.L / (2 * D);                     // every slab: >= 2 D rows (disjoint first / last D)
+    // every slab: >= 2 D rows (disjoint first / last D); in 3D (D = 1) a slab may be a single plane
+    const int gmax = lat.dims == 3 ? lat.L : lat.L / (2 * D);
+    if (G > gmax) G = gmax;
     if (G < 2) return false;
     const int rows_max = (lat.L + G - 1) / G;
     const long long rowl = (lat.dims == 3 ? (long long)lat.L : 1) * (lat.L / 8);   // lanes per march row and colour
