@@ -593,7 +593,8 @@ int small_batch_cluster(const Lat &lat, int R)
 {
     const long long nlanes = lat.half / 4, N = 2 * lat.half;
     int cmax = 1;
-    while (cmax < small_max_cluster() && nlanes / (2 * cmax) >= 128 && 2 * cmax <= lat.L) cmax *= 2;
+    if (nlanes > 512)                                  // up to 512 lanes one block beats any cluster (see small_plan)
+        while (cmax < small_max_cluster() && nlanes / (2 * cmax) >= 128 && 2 * cmax <= lat.L) cmax *= 2;
     int c = cmax;
     while (c > 1 && (long long)R * c > (long long)sm_count()) c >>= 1;   // measured: one block per SM beats two (32 x 128^2: c = 4)
     while (N / c > 196608 && c < 16) c <<= 1;          // the slab must fit shared memory
