@@ -29,6 +29,10 @@
 #define LSM_NE_ALL4_C 0.25
 #endif
 
+#ifndef LSM_TILED_THREADS
+#define LSM_TILED_THREADS 256            // threads per CTA (<= 256: the ring has 256 slots per stage)
+#endif
+
 namespace lsmk {
 
 cudaError_t launch_sweep_tiled_bulk(int model, bool track, int obs_mode, TiledGeom g, const PhiloxSweepConsts &pc,
@@ -48,7 +52,7 @@ PhiloxSweepConsts make_philox_consts(const SweepKey &k)
 }
 
 template <int MODEL, int DIMS, bool TRACK, int OBS, bool NEV>
-__global__ void __launch_bounds__(256, tiled_minblocks(MODEL))
+__global__ void __launch_bounds__(LSM_TILED_THREADS, tiled_minblocks(MODEL))
 k_sweep_tiled(const __grid_constant__ TiledGeom g, const __grid_constant__ PhiloxSweepConsts pc,
               const __grid_constant__ typename TabOf<MODEL>::type tab, const __grid_constant__ NevTab ytab)
 {
@@ -193,6 +197,9 @@ bool tiled_supported(const Lat &lat, int model, const TiledTables &t)
 #ifndef LSM_TILED_WAVES_X4
 #define LSM_TILED_WAVES_X4 4             // waves in quarters
 #endif
+#ifndef LSM_TILED_THREADS
+#define LSM_TILED_THREADS 256            // threads per CTA (<= 256: the ring has 256 slots)
+#endif
 #ifndef LSM_TILED_PDL
 #define LSM_TILED_PDL 1                  // programmatic dependent launch
 #endif
@@ -207,7 +214,7 @@ static cudaError_t launch_obs(int obs_mode, dim3 grid, cudaStream_t s, const Til
     cudaLaunchConfig_t cfg;
     memset(&cfg, 0, sizeof(cfg));
     cfg.gridDim = grid;
-    cfg.blockDim = dim3(256);
+    cfg.blockDim = dim3(LSM_TILED_THREADS);
     cfg.stream = s;
     cudaLaunchAttribute at[1];
     at[0].id = cudaLaunchAttributeProgrammaticStreamSerialization;
@@ -258,13 +265,13 @@ cudaError_t launch_sweep_tiled(const SweepArgs &a, const TiledTables &t, cudaStr
     else if (g.wpr < 32 && 32 % g.wpr == 0 && g.R % (2 * (32 / g.wpr)) == 0) g.parity_rows = 1;
     else g.parity_rows = 0;
     const int per_sm = g_tiled_ctas_per_sm > 0 ? g_tiled_ctas_per_sm : tiled_minblocks(a.model);
-    long long target = (long long)sm_count() * per_sm * 256 * g_tiled_waves_x4 / 4;
+    long long target = (long long)sm_count() * per_sm * LSM_TILED_THREADS * g_tiled_waves_x4 / 4;
     long long S = target / g.ncol;
     if (S < 1) S = 1;
     if (S > g.L) S = g.L;
     g.S = (int)S;
     long long threads = (long long)g.ncol * g.S;
-    dim3 grid((unsigned)((threads + 255) / 256));
+    dim3 grid((unsigned)((threads + LSM_TILED_THREADS - 1) / LSM_TILED_THREADS));
 
     PhiloxSweepConsts pc = make_philox_consts(a.key);
     int obs_mode = a.obs ? (a.want_B ? 2 : 1) : 0;
