@@ -34,6 +34,7 @@ namespace lsmk {
 
 struct SlabArgs {
     uint32_t *col[2];            // colour arrays as 32-bit lanes
+    const uint32_t *bnd[2];      // M_EA: bond bytes of the two colours (same geometry; constant during a launch)
     unsigned long long seed, t0; // first sweep of this launch
     int nsweeps;
     int L;                       // march extent
@@ -80,7 +81,7 @@ k_sweep_slab(const __grid_constant__ SlabArgs a, const __grid_constant__ PhiloxS
     uint32_t ne_t32 = 0;
     int ne_always = 0;
     bool ne_all4 = false;
-    if constexpr (MODEL == M_ISING_HALF || MODEL == M_ISING_ONE) {
+    if constexpr (MODEL == M_ISING_HALF || MODEL == M_ISING_ONE || MODEL == M_EA) {
         for (int i = threadIdx.x; i < NT; i += blockDim.x) {
             sm.t[i] = tab.t[i];
             if (NEV) sm.t[NT + i] = ytab.y[i];
@@ -104,6 +105,7 @@ k_sweep_slab(const __grid_constant__ SlabArgs a, const __grid_constant__ PhiloxS
     const uint32_t rows = (uint32_t)(m1 - m0);
     const uint32_t colstride = ((uint32_t)a.rows_max + 2u * D) << lg_row;       // shared lanes per colour
     uint32_t *const s_col[2] = {s_lat, s_lat + colstride};
+    uint32_t *const s_bnd[2] = {s_lat + 2u * colstride, s_lat + 3u * colstride};   // M_EA only (the launch sizes for it)
     const int g_below = g == 0 ? G - 1 : g - 1, g_above = g + 1 == G ? 0 : g + 1;
     // local march row lr <-> global march row (m0 - D + lr) mod L: 0 ... D-1 halo below, D ... D+rows-1 own rows,
     // D+rows ... rows+2D-1 halo above
@@ -115,6 +117,10 @@ k_sweep_slab(const __grid_constant__ SlabArgs a, const __grid_constant__ PhiloxS
         const uint32_t src = (((mbase + lr) & Lm) << lg_row) + r;
         s_col[0][i] = a.col[0][src];
         s_col[1][i] = a.col[1][src];
+        if (MODEL == M_EA) {                                   // the bonds of the halo rows too: their redundant updates need them
+            s_bnd[0][i] = a.bnd[0][src];
+            s_bnd[1][i] = a.bnd[1][src];
+        }
     }
     __syncthreads();
     // No CTA may write its slab back (end of the kernel) before the adjacent CTAs have read their initial halos; with
@@ -221,7 +227,9 @@ k_sweep_slab(const __grid_constant__ SlabArgs a, const __grid_constant__ PhiloxS
                 W.q = (int)qq;
                 W.grp = ((m << lg_wrow) + wr) << 2;                 // Philox group of the word's first lane (D2)
                 W.totU = W.totBN = W.totS = 0;                      // this word's sums: counted for own rows only
-                const uint4 out = W.template update_word<2, true>(pc, N, O, edge, Yp, Yn);
+                uint4 BW = make_uint4(0u, 0u, 0u, 0u);
+                if (MODEL == M_EA) BW = reinterpret_cast<const uint4 *>(s_bnd[half])[wi];
+                const uint4 out = W.template update_word<2, true>(pc, N, O, edge, Yp, Yn, BW);
                 reinterpret_cast<uint4 *>(own)[wi] = out;
                 if (s < nA) {
                     const uint4 tagged = make_uint4(out.x | wtag, out.y | wtag, out.z | wtag, out.w | wtag);
@@ -294,7 +302,8 @@ static int slab_ilog2(long long v)
 // where a half-sweep is shorter than an exchange (~1 us): the smaller 2D lattices.
 int slab_depth_max(int dims, int L, int model)
 {
-    if (model != M_ISING_HALF && model != M_ISING_ONE && model != M_NE_HEATBATH && model != M_NE_METROPOLIS) return 0;
+    if (model != M_ISING_HALF && model != M_ISING_ONE && model != M_NE_HEATBATH && model != M_NE_METROPOLIS && model != M_EA)
+        return 0;
     if ((L & (L - 1)) != 0) return 0;                                 // lane index math by shifts
     if (dims == 2 ? (L < 512 || L > 4096) : (L < 64 || L > 128)) return 0;   // below: the small family; above: does not fit
     if (dims == 3) return 1;
@@ -332,7 +341,7 @@ bool slab_plan(const Lat &lat, int model, const TiledTables &t, int depth, SlabP
     if (G < 2) return false;
     const int rows_max = (lat.L + G - 1) / G;
     const long long rowl = (lat.dims == 3 ? (long long)lat.L : 1) * (lat.L / 8);   // lanes per march row and colour
-    const long long smem = 2ll * (rows_max + 2 * D) * rowl * 4;
+    const long long smem = (model == M_EA ? 4ll : 2ll) * (rows_max + 2 * D) * rowl * 4;    // EA: the bond bytes as well
     if (smem > LSM_SLAB_SMEM_MAX) return false;
     long long per = (long long)(rows_max + 2 * (D - 1)) * rowl / 4;   // words of the largest step of the largest slab
     int threads = (int)(per < 512 ? ((per + 31) / 32) * 32 : 512);
@@ -361,7 +370,7 @@ static cudaError_t slab_launch_to(bool track, bool obs, const SlabPlan &plan, cu
         return cudaLaunchCooperativeKernel((const void *)kern, dim3((unsigned)plan.G), dim3((unsigned)plan.threads), params,
                                            (size_t)plan.smem, s);
     };
-    constexpr bool CAN_NEV = MODEL == M_ISING_HALF || MODEL == M_ISING_ONE;
+    constexpr bool CAN_NEV = MODEL == M_ISING_HALF || MODEL == M_ISING_ONE || MODEL == M_EA;
     if constexpr (CAN_NEV) {
         if (t.has_never) {
             if (track) return obs ? go(k_sweep_slab<MODEL, DIMS, true, 2, true>) : go(k_sweep_slab<MODEL, DIMS, true, 0, true>);
@@ -381,6 +390,8 @@ cudaError_t launch_sweep_slab(const Lat &lat, int model, int track, unsigned lon
     memset(&a, 0, sizeof(a));
     a.col[0] = reinterpret_cast<uint32_t *>(lat.col[0]);
     a.col[1] = reinterpret_cast<uint32_t *>(lat.col[1]);
+    a.bnd[0] = reinterpret_cast<const uint32_t *>(lat.bnd[0]);
+    a.bnd[1] = reinterpret_cast<const uint32_t *>(lat.bnd[1]);
     a.seed = seed;
     a.t0 = t0;
     a.nsweeps = nsweeps;
@@ -403,6 +414,12 @@ cudaError_t launch_sweep_slab(const Lat &lat, int model, int track, unsigned lon
         for (int i = 0; i < 16; ++i) ht.t[i] = t.t32[i];
         return lat.dims == 3 ? slab_launch_to<M_ISING_HALF, 3>(tr, obs, plan, s, a, pk, ht, t)
                              : slab_launch_to<M_ISING_HALF, 2>(tr, obs, plan, s, a, pk, ht, t);
+    }
+    case M_EA: {
+        HalfTab ht;
+        for (int i = 0; i < 16; ++i) ht.t[i] = t.t32[i];
+        return lat.dims == 3 ? slab_launch_to<M_EA, 3>(tr, obs, plan, s, a, pk, ht, t)
+                             : slab_launch_to<M_EA, 2>(tr, obs, plan, s, a, pk, ht, t);
     }
     case M_ISING_ONE: {
         OneTab ot;

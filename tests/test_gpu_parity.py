@@ -160,6 +160,9 @@ SLAB_DEPTH_CASES = [
     (dict(dims=2, L=4096, T=2.6), (1,)),
     (dict(dims=3, L=64, T=4.5115), (1,)),
     (dict(dims=3, L=128, two_S=2, T=3.0, h=0.01), (1,)),
+    (dict(dims=2, L=512, model=lsm.EA, T=1.1, h=0.05), (1, 2, 3)),      # +/-J bonds resident beside the spins
+    (dict(dims=2, L=2048, model=lsm.EA, T=0.2), (2,)),                  # "never" thresholds
+    (dict(dims=3, L=64, model=lsm.EA, T=1.2), (1,)),
 ]
 
 
