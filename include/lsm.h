@@ -91,7 +91,8 @@ enum {
  *  SLAB     one cooperative launch for all sweeps of a call with the whole lattice resident in the shared memory of
  *           one CTA per SM: slabs of march rows, boundary rows exchanged through self-validating mailbox words in L2, one per
  *           CTA, several half-sweeps per exchange (lsm_set_temporal_depth); L a power of two, 512^2 ... 4096^2,
- *           64^3, 128^3, where AUTO chooses it;
+ *           64^3, 128^3 and every model (Edwards-Anderson up to 2048^2: its bond bytes are resident too), where AUTO
+ *           chooses it;
  *  BULK     the TILED half-sweep with its rows staged through shared memory by bulk asynchronous copies (TMA unit,
  *           cp.async.bulk + mbarrier; one producer thread per CTA, 4-stage ring) instead of per-thread cp.async: 2D,
  *           L a multiple of 8192, spin-1/2 and North-East.  Opt-in: measured 10 % slower than TILED on 8192^2

@@ -45,6 +45,7 @@ struct SlabArgs {
     int dmax;                    // mailbox rows reserved per slot
     int early;                   // D = 1, long steps: copy the halo behind the step instead of before the next one
     int one;
+    int qm1;                     // M_POTTS: q - 1
     long long *obs;              // [nsweeps][2] (B, M) slots zeroed by the host, or nullptr
     uint32_t *mbox;              // [G][first, last][epoch parity][colour][dmax][lanes of a march row]
 };
@@ -81,7 +82,7 @@ k_sweep_slab(const __grid_constant__ SlabArgs a, const __grid_constant__ PhiloxS
     uint32_t ne_t32 = 0;
     int ne_always = 0;
     bool ne_all4 = false;
-    if constexpr (MODEL == M_ISING_HALF || MODEL == M_ISING_ONE || MODEL == M_EA) {
+    if constexpr (MODEL == M_ISING_HALF || MODEL == M_ISING_ONE || MODEL == M_EA || MODEL == M_POTTS) {
         for (int i = threadIdx.x; i < NT; i += blockDim.x) {
             sm.t[i] = tab.t[i];
             if (NEV) sm.t[NT + i] = ytab.y[i];
@@ -196,6 +197,7 @@ k_sweep_slab(const __grid_constant__ SlabArgs a, const __grid_constant__ PhiloxS
             W.ne_t32 = ne_t32;
             W.ne_always = ne_always;
             W.ne_all4 = ne_all4;
+            W.potts_qm1 = (uint32_t)a.qm1;
 #pragma unroll 1
             for (uint32_t i = tid; i < total; i += nthr) {
                 const uint32_t s = i >> lg_wrow, wr = i & (wrow - 1);
@@ -302,7 +304,8 @@ static int slab_ilog2(long long v)
 // where a half-sweep is shorter than an exchange (~1 us): the smaller 2D lattices.
 int slab_depth_max(int dims, int L, int model)
 {
-    if (model != M_ISING_HALF && model != M_ISING_ONE && model != M_NE_HEATBATH && model != M_NE_METROPOLIS && model != M_EA)
+    if (model != M_ISING_HALF && model != M_ISING_ONE && model != M_NE_HEATBATH && model != M_NE_METROPOLIS && model != M_EA &&
+        model != M_POTTS)
         return 0;
     if ((L & (L - 1)) != 0) return 0;                                 // lane index math by shifts
     if (dims == 2 ? (L < 512 || L > 4096) : (L < 64 || L > 128)) return 0;   // below: the small family; above: does not fit
@@ -370,7 +373,7 @@ static cudaError_t slab_launch_to(bool track, bool obs, const SlabPlan &plan, cu
         return cudaLaunchCooperativeKernel((const void *)kern, dim3((unsigned)plan.G), dim3((unsigned)plan.threads), params,
                                            (size_t)plan.smem, s);
     };
-    constexpr bool CAN_NEV = MODEL == M_ISING_HALF || MODEL == M_ISING_ONE || MODEL == M_EA;
+    constexpr bool CAN_NEV = MODEL == M_ISING_HALF || MODEL == M_ISING_ONE || MODEL == M_EA || MODEL == M_POTTS;
     if constexpr (CAN_NEV) {
         if (t.has_never) {
             if (track) return obs ? go(k_sweep_slab<MODEL, DIMS, true, 2, true>) : go(k_sweep_slab<MODEL, DIMS, true, 0, true>);
@@ -404,6 +407,7 @@ cudaError_t launch_sweep_slab(const Lat &lat, int model, int track, unsigned lon
     a.dmax = plan.dmax;
     a.early = plan.early;
     a.one = 1;
+    a.qm1 = model == M_POTTS ? lat.q - 1 : 0;
     a.obs = d_obs;
     a.mbox = d_mbox;
     PhiloxSweepConsts pk = make_philox_consts(make_sweep_key(seed, t0, 0u));   // only the round keys are used
@@ -414,6 +418,12 @@ cudaError_t launch_sweep_slab(const Lat &lat, int model, int track, unsigned lon
         for (int i = 0; i < 16; ++i) ht.t[i] = t.t32[i];
         return lat.dims == 3 ? slab_launch_to<M_ISING_HALF, 3>(tr, obs, plan, s, a, pk, ht, t)
                              : slab_launch_to<M_ISING_HALF, 2>(tr, obs, plan, s, a, pk, ht, t);
+    }
+    case M_POTTS: {
+        HalfTab ht;
+        for (int i = 0; i < 16; ++i) ht.t[i] = t.t32[i];
+        return lat.dims == 3 ? slab_launch_to<M_POTTS, 3>(tr, obs, plan, s, a, pk, ht, t)
+                             : slab_launch_to<M_POTTS, 2>(tr, obs, plan, s, a, pk, ht, t);
     }
     case M_EA: {
         HalfTab ht;

@@ -163,6 +163,8 @@ SLAB_DEPTH_CASES = [
     (dict(dims=2, L=512, model=lsm.EA, T=1.1, h=0.05), (1, 2, 3)),      # +/-J bonds resident beside the spins
     (dict(dims=2, L=2048, model=lsm.EA, T=0.2), (2,)),                  # "never" thresholds
     (dict(dims=3, L=64, model=lsm.EA, T=1.2), (1,)),
+    (dict(dims=2, L=1024, two_S=2, model=lsm.POTTS, T=0.995), (1, 2, 4)),   # 3-state Potts
+    (dict(dims=3, L=64, two_S=7, model=lsm.POTTS, T=0.9), (1,)),           # q = 8
 ]
 
 
