@@ -142,7 +142,9 @@ static void choose_kernel(lsm *o)
     bool tiled_ok = tiled_supported(o->lat, o->model, o->tiled);
     if (want == LSM_KERNEL_AUTO) {
         // 512^2 ... 4096^2, 64^3, 128^3: the lattice lives in the SMs' shared memory (profiles/r2_slab_family.md)
-        if (o->N >= 262144 && slab_plan(o->lat, o->model, o->tiled, o->slab_depth, &o->slab)) want = LSM_KERNEL_SLAB;
+        // (Edwards-Anderson / Potts have no small-family kernels: the slab family from 128^2 / 32^3)
+        if ((o->N >= 262144 || o->model == M_EA || o->model == M_POTTS) &&
+            slab_plan(o->lat, o->model, o->tiled, o->slab_depth, &o->slab)) want = LSM_KERNEL_SLAB;
         else want = small_plan(o->lat, o->model, o->tiled, &o->small, false) ? LSM_KERNEL_SMALL
                   : tiled_ok ? LSM_KERNEL_TILED : LSM_KERNEL_GENERIC;
     }

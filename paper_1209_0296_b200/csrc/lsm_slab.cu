@@ -308,7 +308,9 @@ int slab_depth_max(int dims, int L, int model)
         model != M_POTTS)
         return 0;
     if ((L & (L - 1)) != 0) return 0;                                 // lane index math by shifts
-    if (dims == 2 ? (L < 512 || L > 4096) : (L < 64 || L > 128)) return 0;   // below: the small family; above: does not fit
+    // above: does not fit; below: the small family (cluster barrier) is faster -- for the models it covers
+    const bool wider = model == M_EA || model == M_POTTS;
+    if (dims == 2 ? (L < (wider ? 128 : 512) || L > 4096) : (L < (wider ? 32 : 64) || L > 128)) return 0;
     if (dims == 3) return 1;
     return L <= 1024 ? 4 : L == 2048 ? 2 : 1;
 }

@@ -165,6 +165,8 @@ SLAB_DEPTH_CASES = [
     (dict(dims=3, L=64, model=lsm.EA, T=1.2), (1,)),
     (dict(dims=2, L=1024, two_S=2, model=lsm.POTTS, T=0.995), (1, 2, 4)),   # 3-state Potts
     (dict(dims=3, L=64, two_S=7, model=lsm.POTTS, T=0.9), (1,)),           # q = 8
+    (dict(dims=2, L=128, model=lsm.EA, T=0.9), (1, 2, 3, 4)),              # small lattices of the models without a small family
+    (dict(dims=3, L=32, two_S=3, model=lsm.POTTS, T=1.5), (1,)),
 ]
 
 
