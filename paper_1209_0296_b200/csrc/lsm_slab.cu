@@ -1,4 +1,5 @@
-// lsm_slab.cu -- the slab family for mid-size lattices (512^2 ... 4096^2, 64^3, 128^3): ONE launch runs many sweeps,
+// lsm_slab.cu -- the slab family for mid-size lattices (512^2 ... 4096^2, 64^3, 128^3; from 128^2 / 32^3 for the
+// Edwards-Anderson and Potts models, which have no small-family kernels): ONE launch runs many sweeps,
 // the whole lattice lives in the shared memory of the SMs, and several half-sweeps run between two exchanges
 // (temporal blocking with redundant halo updates).
 //
@@ -16,10 +17,11 @@
 //     the own rows are exact and the halo is used up;
 //   * exchange: while it makes the last two steps of an epoch a CTA stores the first and the last D of its own rows
 //     (of the colour updated in that step) into its mailbox in global memory (L2); the adjacent CTAs copy them into
-//     their halos at the start of the next epoch.  Mailbox lanes validate themselves: bit 31 of every 32-bit lane
+//     their halos behind the epoch's last step.  Mailbox lanes validate themselves: bit 31 of every 32-bit lane
 //     (bit 7 of a site byte is unused by every encoding, lsm_internal.cuh) carries one bit of the epoch number and the
-//     reader spins on a 16-byte word until its four lanes show the expected one -- no flag, no fence.  One exchange costs about one
-//     microsecond of latency on B200 whatever its size, which is why it pays to make it once per D half-sweeps;
+//     reader spins on a 16-byte word until its four lanes show the expected one -- no flag, no fence.  One exchange
+//     costs about one microsecond of latency on B200 whatever its size, which is why it pays to make it once per D
+//     half-sweeps;
 //   * D = 1 is the plain scheme (one row of the colour just updated per half-sweep, no redundant update).
 // Mailboxes are double-buffered by epoch parity: a CTA rewrites buffer e & 1 in epoch e + 2, which it can only start
 // after it has read the neighbours' rows of epoch e + 1, and those were computed from this CTA's rows of epoch e.
