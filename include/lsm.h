@@ -90,7 +90,7 @@ enum {
  *  RESIDENT one cooperative launch for all sweeps with neighbour-flag synchronisation (opt-in, large lattices);
  *  SLAB     one cooperative launch for all sweeps of a call with the whole lattice resident in the shared memory of
  *           one CTA per SM: slabs of march rows, boundary rows exchanged through self-validating mailbox words in L2, one per
- *           CTA, several half-sweeps per exchange (lsm_set_temporal_depth); L a power of two, 512^2 ... 4096^2,
+ *           CTA, several half-sweeps per exchange (lsm_set_temporal_depth); L a multiple of 32, 512^2 ... 4096^2,
  *           64^3, 128^3 and every model (Edwards-Anderson up to 2048^2: its bond bytes are resident too), where AUTO
  *           chooses it;
  *  BULK     the TILED half-sweep with its rows staged through shared memory by bulk asynchronous copies (TMA unit,

@@ -49,7 +49,7 @@ cudaError_t launch_sweep_small(const Lat &lat, int model, int track, unsigned lo
 
 // Slab family (lsm_slab.cu): one cooperative launch runs `nsweeps` whole sweeps with the lattice resident in the
 // shared memory of G CTAs (one per SM); boundary rows travel through self-validating mailbox words in L2.
-struct SlabPlan { int G, rows_max, threads, smem, D, dmax, early; };   // D: temporal depth (half-sweeps per exchange)
+struct SlabPlan { int G, rows_max, threads, smem, D, dmax, early; uint32_t magic_wrow, magic_wpr; };   // D: temporal depth (half-sweeps per exchange)
 constexpr int SLAB_MAX_CTAS = 160;                                   // mailbox rows reserved in the workspace
 size_t slab_mailbox_bytes(int dims, int L, int model);               // internal Model id; 0: shape not covered
 int slab_depth_max(int dims, int L, int model);                      // largest temporal depth of this shape

@@ -167,6 +167,13 @@ SLAB_DEPTH_CASES = [
     (dict(dims=3, L=64, two_S=7, model=lsm.POTTS, T=0.9), (1,)),           # q = 8
     (dict(dims=2, L=128, model=lsm.EA, T=0.9), (1, 2, 3, 4)),              # small lattices of the models without a small family
     (dict(dims=3, L=32, two_S=3, model=lsm.POTTS, T=1.5), (1,)),
+    # L not a power of two: the index arithmetic divides by multiplication
+    (dict(dims=2, L=1536, T=2.269), (1, 2)),
+    (dict(dims=2, L=1056, two_S=2, T=1.5, h=0.01), (2,)),
+    (dict(dims=2, L=736, T=2.0), (3, 4)),
+    (dict(dims=2, L=3072, model=lsm.NE_HEATBATH, J=0.0, T=W.ne_temperature(0.2)), (1,)),
+    (dict(dims=3, L=96, T=4.5115, h=0.05), (1,)),
+    (dict(dims=2, L=160, model=lsm.EA, T=1.0), (1, 2)),
 ]
 
 
