@@ -92,7 +92,8 @@ enum {
  *           one CTA per SM: slabs of march rows, boundary rows exchanged through self-validating mailbox words in L2, one per
  *           CTA, several half-sweeps per exchange (lsm_set_temporal_depth); L a multiple of 32, 512^2 ... 4096^2,
  *           64^3, 128^3 and every model (Edwards-Anderson up to 2048^2: its bond bytes are resident too), where AUTO
- *           chooses it;
+ *           chooses it; also from 128^2 / 32^3 where the small family has no lane kernel (Edwards-Anderson, Potts,
+ *           edges that are not powers of two);
  *  BULK     the TILED half-sweep with its rows staged through shared memory by bulk asynchronous copies (TMA unit,
  *           cp.async.bulk + mbarrier; one producer thread per CTA, 4-stage ring) instead of per-thread cp.async: 2D,
  *           L a multiple of 8192, spin-1/2 and North-East.  Opt-in: measured 10 % slower than TILED on 8192^2

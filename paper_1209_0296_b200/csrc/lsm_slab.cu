@@ -325,9 +325,10 @@ int slab_depth_max(int dims, int L, int model)
         model != M_POTTS)
         return 0;
     if (L % 32 != 0) return 0;                                        // whole 16-byte words per compact row
-    // above: does not fit; below: the small family (cluster barrier) is faster -- for the models it covers
-    const bool wider = model == M_EA || model == M_POTTS;
-    if (dims == 2 ? (L < (wider ? 128 : 512) || L > 4096) : (L < (wider ? 32 : 64) || L > 128)) return 0;
+    // above: does not fit; below: the small family's lane kernel (cluster barrier) is faster -- for the models and the
+    // power-of-two edges it covers
+    const bool low = model == M_EA || model == M_POTTS || (L & (L - 1)) != 0;
+    if (dims == 2 ? (L < (low ? 128 : 512) || L > 4096) : (L < (low ? 32 : 64) || L > 128)) return 0;
     if (dims == 3) return 1;
     return L <= 1024 ? 4 : L <= 2048 ? 2 : 1;
 }

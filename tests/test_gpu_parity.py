@@ -174,6 +174,8 @@ SLAB_DEPTH_CASES = [
     (dict(dims=2, L=3072, model=lsm.NE_HEATBATH, J=0.0, T=W.ne_temperature(0.2)), (1,)),
     (dict(dims=3, L=96, T=4.5115, h=0.05), (1,)),
     (dict(dims=2, L=160, model=lsm.EA, T=1.0), (1, 2)),
+    (dict(dims=2, L=320, T=2.269), (1, 3)),
+    (dict(dims=2, L=224, model=lsm.NE_METROPOLIS, J=0.0, T=W.ne_temperature(0.3)), (4,)),
 ]
 
 
