@@ -237,14 +237,14 @@ extern "C" int lsm_destroy(lsm_t *o)
 }
 
 // ---------------------------------------------------------------------------- sweeps (a2-a7)
-static int enqueue_half(lsm *o, int half, long long *obs, int want_B, cudaStream_t s)
+static int enqueue_half(lsm *o, int family, int half, long long *obs, int want_B, cudaStream_t s)
 {
     SweepArgs a;
     a.lat = o->lat; a.model = o->model; a.half = half;
     a.key = make_sweep_key(o->seed, o->t, (uint32_t)half);
     a.track = o->tracking; a.obs = obs; a.want_B = want_B;
-    a.bulk = o->kernel_in_use == LSM_KERNEL_BULK ? 1 : 0;
-    if (o->kernel_in_use == LSM_KERNEL_TILED || o->kernel_in_use == LSM_KERNEL_BULK) CU(launch_sweep_tiled(a, o->tiled, s));
+    a.bulk = family == LSM_KERNEL_BULK ? 1 : 0;
+    if (family == LSM_KERNEL_TILED || family == LSM_KERNEL_BULK) CU(launch_sweep_tiled(a, o->tiled, s));
     else CU(launch_sweep_generic(a, o->thr_param, s));
     o->launches += 1;
     return LSM_OK;
@@ -296,15 +296,21 @@ static int sweep_impl(lsm *o, int64_t n, long long *d_obs, cudaStream_t s)
 {
     o->last_stream = s;
     if (n == 0) return LSM_OK;
-    if (o->kernel_in_use == LSM_KERNEL_RESIDENT || o->kernel_in_use == LSM_KERNEL_SMALL || o->kernel_in_use == LSM_KERNEL_SLAB)
+    // A slab launch reads and writes the whole lattice once: on the largest slab lattices (4096^2: 2 x 16 MB, ~19 us) a
+    // call of a few sweeps is cheaper as launches per half-sweep (measured: break-even at 8 sweeps; same results).
+    const bool short_call = o->kernel_in_use == LSM_KERNEL_SLAB && o->kernel_pref == LSM_KERNEL_AUTO && n < 8 &&
+                            o->N >= ((int64_t)1 << 24) && tiled_supported(o->lat, o->model, o->tiled);
+    if (!short_call &&
+        (o->kernel_in_use == LSM_KERNEL_RESIDENT || o->kernel_in_use == LSM_KERNEL_SMALL || o->kernel_in_use == LSM_KERNEL_SLAB))
         return sweep_resident(o, n, d_obs, s);
+    const int family = short_call ? LSM_KERNEL_TILED : o->kernel_in_use;
     if (d_obs) CU(cudaMemsetAsync(d_obs, 0, (size_t)n * 16, s));
     else CU(cudaMemsetAsync(o->d_run, 0, 16, s));
     for (int64_t k = 0; k < n; ++k) {
         long long *obs = d_obs ? d_obs + 2 * k : (k == n - 1 ? o->d_run : nullptr);
-        int rc = enqueue_half(o, 0, obs, 0, s);
+        int rc = enqueue_half(o, family, 0, obs, 0, s);
         if (rc != LSM_OK) return rc;
-        rc = enqueue_half(o, 1, obs, 1, s);
+        rc = enqueue_half(o, family, 1, obs, 1, s);
         if (rc != LSM_OK) return rc;
         o->t += 1;
     }

@@ -212,6 +212,23 @@ def test_slab_temporal_blocking_parity(kw, depths):
     lat.close()
 
 
+def test_auto_mixes_short_and_long_calls_on_the_largest_slab_lattice():
+    """4096^2 under AUTO: calls of fewer than 8 sweeps run as launches per half-sweep, longer ones as one slab launch
+    (the slab launch reads and writes the whole lattice once); the results must not show the seam."""
+    kw = dict(dims=2, L=4096, T=2.269, h=0.02)
+    seed = W.seed_of(13, 0)
+    lat, orc = lsm.Lattice(seed=seed, **kw), O.Oracle(seed=seed, **kw)
+    assert lat.kernel == lsm.KERNEL_SLAB
+    for n, rec in ((3, True), (9, True), (2, False), (1, True)):
+        if rec:
+            assert np.array_equal(lat.sweep_record(n).cpu().numpy(), orc.sweep_record(n)), n
+        else:
+            lat.sweep(n)
+            orc.sweep(n)
+        assert_same_state(lat, orc)
+    lat.close()
+
+
 BULK_CASES = [
     dict(dims=2, L=8192, T=2.269, h=0.05),
     dict(dims=2, L=8192, T=0.3),                                   # "never" thresholds: the two-compare kernels
