@@ -212,6 +212,30 @@ def test_slab_temporal_blocking_parity(kw, depths):
     lat.close()
 
 
+@pytest.mark.parametrize("kw,depth,n", [
+    (dict(dims=2, L=512, T=2.269), 3, 60000),
+    (dict(dims=2, L=1024, T=2.0, h=0.1), 2, 40000),
+    (dict(dims=3, L=128, T=4.5115), 1, 10000),
+    (dict(dims=2, L=1536, model=lsm.NE_HEATBATH, J=0.0, T=W.ne_temperature(0.3)), 2, 20000),
+])
+def test_slab_long_run_against_the_tiled_family(kw, depth, n):
+    """The mailbox protocol of the slab family over 10^4 ... 10^5 sweeps (2 x 10^4 ... 10^5 exchanges per CTA pair): the
+    configuration, the running sums and the persistence counts must equal those of the tiled family, which the other
+    tests hold to the oracle sweep by sweep."""
+    a, b = lsm.Lattice(seed=77, **kw), lsm.Lattice(seed=77, **kw)
+    a.set_kernel(lsm.KERNEL_SLAB)
+    a.set_temporal_depth(depth)
+    b.set_kernel(lsm.KERNEL_TILED)
+    for _ in range(2):
+        a.sweep(n // 2)
+        b.sweep(n // 2)
+        assert a.measure_int() == b.measure_int()
+    assert torch.equal(a.get_spins(), b.get_spins())
+    assert a.persistence() == b.persistence() and a.measure_full() == a.measure_int()[:2]
+    a.close()
+    b.close()
+
+
 def test_auto_mixes_short_and_long_calls_on_the_largest_slab_lattice():
     """4096^2 under AUTO: calls of fewer than 8 sweeps run as launches per half-sweep, longer ones as one slab launch
     (the slab launch reads and writes the whole lattice once); the results must not show the seam."""
