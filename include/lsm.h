@@ -80,7 +80,8 @@ enum {
     LSM_ERR_UNSUPPORTED = -2, /* two_S not 1|2; NE with dims != 2, J != 0 or two_S != 1        */
     LSM_ERR_CUDA = -3,        /* a CUDA runtime call failed (text: lsm_last_cuda_error)         */
     LSM_ERR_WORKSPACE = -4,   /* workspace too small or not 256-byte aligned                   */
-    LSM_ERR_STATE = -5        /* tracking is off (lsm_persistence); replicas out of lockstep (batch) */
+    LSM_ERR_STATE = -5,       /* tracking is off (lsm_persistence); replicas out of lockstep (batch) */
+    LSM_ERR_LIMIT = -6        /* lsm_sweep_record_host_noalloc: n > LSM_NOALLOC_MAX_SWEEPS                 */
 };
 /* Kernel families (lsm_set_kernel).  AUTO picks the fastest one that supports the lattice:
  *  SMALL    one launch for all sweeps of a call: lattice slabs in the shared memory of a thread-block cluster,
@@ -126,6 +127,25 @@ int lsm_sweep_record_host(lsm_t *, int64_t n, int64_t *h_obs, int64_t *d_scratch
 /* Same without the final synchronisation: the copy into h_obs (pinned host memory) is enqueued on stream; the
  * series is valid once the caller has synchronised it.  For pipelines that keep several steps in flight. */
 int lsm_sweep_record_host_async(lsm_t *, int64_t n, int64_t *h_obs, int64_t *d_scratch, void *stream);
+
+/* lsm_sweep_record_host for callers that cannot allocate device memory and therefore cannot bring d_scratch: code that runs
+ * inside a host application whose own pool owns all of the GPU's memory and exposes no allocator to plug-ins, a loop with
+ * a latency budget that rules out cudaMalloc (it synchronises the whole device), a job whose memory quota is already
+ * spent on the lattice.  The (B, M) series is staged in a fixed 64 KiB array that is part of the library image -- every
+ * GPU the library is loaded on carries it until the process exits -- so n is limited:
+ *  - n > LSM_NOALLOC_MAX_SWEEPS returns LSM_ERR_LIMIT and does nothing (split the run into several calls; the sweep
+ *    counter carries on, so the series is the same as that of one long call);
+ *  - the call allocates and frees no device memory: no cudaMalloc / cudaFree, no library routine that allocates;
+ *  - the first call on each GPU (made with that GPU current, as for every call of this library) looks up the device address
+ *    of the array once; make that first call outside any stream capture;
+ *  - there is ONE array per GPU, shared by every handle and every host thread, and it still holds the previous call's
+ *    series when the next call starts (the call clears the n pairs it uses, on `stream`, before the sweeps add into them).
+ *    Two such calls whose GPU work overlaps -- two host threads, or two streams, on the same GPU -- race on it and both
+ *    series are garbage: serialise them.  Calls on different GPUs do not interact.
+ * Otherwise as lsm_sweep_record_host: h_obs[n][2] on the host (pageable or pinned), bit-identical values, the lattice,
+ * workspace and stream remain the caller's, returns after the copy into h_obs completed (synchronises stream). */
+enum { LSM_NOALLOC_MAX_SWEEPS = 4096 };
+int lsm_sweep_record_host_noalloc(lsm_t *, int64_t n, int64_t *h_obs, void *stream);
 
 /* North-East model only: n sweeps of the paper's "corrected algorithm" (steps 3-10) instead of
  * the checkerboard sweep, which the paper rejects for relaxation dynamics.  The lattice is

@@ -8,6 +8,7 @@
 #include <cmath>
 #include <cstdlib>
 #include <cstring>
+#include <mutex>
 #include <new>
 #include <string>
 #include <vector>
@@ -392,6 +393,60 @@ extern "C" int lsm_sweep_record_host(lsm_t *o, int64_t n, int64_t *h_obs, int64_
     int rc = sweep_impl(o, n, (long long *)d_scratch, s);
     if (rc != LSM_OK) return rc;
     if (n > 0) CU(cudaMemcpyAsync(h_obs, d_scratch, (size_t)n * 16, cudaMemcpyDeviceToHost, s));
+    CU(cudaStreamSynchronize(s));
+    return LSM_OK;
+}
+
+// ---------------------------------------------------------------------------- entry point without device allocation
+// lsm_sweep_record_host needs 16*n bytes of device scratch for the (B, M) series, and so far the caller had to bring
+// them.  Some callers have no way to: a plug-in inside a host program that handed every byte of HBM to its own pool
+// and offers no allocation hook, a control loop that may not pay cudaMalloc's device-wide synchronisation between
+// two steps, a process running under a memory quota that is already spent on the lattice.  For them the scratch
+// lives in the library image itself: the array below, LSM_NOALLOC_MAX_SWEEPS pairs = 64 KiB, present on every GPU
+// this library is loaded on from the moment the module is loaded until the process exits.
+//
+// `g_noalloc_obs` is two things.  In device code it is the array.  In host code the same name is only the handle the
+// runtime registered for it, NOT a device address: handing it to a kernel makes the kernel fault (or, on systems where
+// the GPU can reach host memory, scribble over host memory that has nothing to do with the array).  The device address
+// comes from cudaGetSymbolAddress, per device, with that device current; noalloc_scratch() asks once per device and
+// keeps the answer.
+static __device__ __align__(256) long long g_noalloc_obs[2 * LSM_NOALLOC_MAX_SWEEPS];
+
+static const int NOALLOC_MAX_DEVICES = 64;
+static std::mutex g_noalloc_mutex;
+static long long *g_noalloc_addr[NOALLOC_MAX_DEVICES];   // device address of g_noalloc_obs on device k (nullptr: not asked yet)
+
+static int noalloc_scratch(long long **d_ptr)
+{
+    int dev = -1;
+    CU(cudaGetDevice(&dev));
+    if (dev < 0 || dev >= NOALLOC_MAX_DEVICES) return LSM_ERR_UNSUPPORTED;
+    std::lock_guard<std::mutex> lock(g_noalloc_mutex);
+    if (!g_noalloc_addr[dev]) {
+        void *p = nullptr;
+        CU(cudaGetSymbolAddress(&p, g_noalloc_obs));     // the current device's copy of the array
+        if (!p) return LSM_ERR_CUDA;
+        g_noalloc_addr[dev] = (long long *)p;
+    }
+    *d_ptr = g_noalloc_addr[dev];
+    return LSM_OK;
+}
+
+// lsm_sweep_record_host with the device scratch taken from g_noalloc_obs: the sweep kernels accumulate (B, M) of
+// sweep k into pair k of the array (cleared first on `stream`, as for any d_obs: the kernels add into it), the series
+// is copied to h_obs on `stream`, and the call returns once the copy has completed.  No cudaMalloc / cudaFree, no
+// allocating library call.
+extern "C" int lsm_sweep_record_host_noalloc(lsm_t *o, int64_t n, int64_t *h_obs, void *stream)
+{
+    if (!o || n < 0 || (!h_obs && n > 0)) return LSM_ERR_ARG;
+    if (n > LSM_NOALLOC_MAX_SWEEPS) return LSM_ERR_LIMIT;
+    long long *d_obs = nullptr;
+    int rc = noalloc_scratch(&d_obs);
+    if (rc != LSM_OK) return rc;
+    cudaStream_t s = (cudaStream_t)stream;
+    rc = sweep_impl(o, n, d_obs, s);
+    if (rc != LSM_OK) return rc;
+    if (n > 0) CU(cudaMemcpyAsync(h_obs, d_obs, (size_t)n * 16, cudaMemcpyDeviceToHost, s));
     CU(cudaStreamSynchronize(s));
     return LSM_OK;
 }
@@ -915,6 +970,7 @@ extern "C" const char *lsm_strerror(int code)
     case LSM_ERR_CUDA: return "CUDA runtime error (see lsm_last_cuda_error)";
     case LSM_ERR_WORKSPACE: return "workspace too small or misaligned";
     case LSM_ERR_STATE: return "tracking is off, or the replicas of a batch are out of lockstep";
+    case LSM_ERR_LIMIT: return "n exceeds LSM_NOALLOC_MAX_SWEEPS, the capacity of the library's built-in device scratch";
     default: return "unknown error code";
     }
 }

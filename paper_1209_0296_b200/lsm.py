@@ -16,7 +16,8 @@ _LIB_PATH = os.path.join(_PKG, "liblsm.so")
 
 ISING, NE_HEATBATH, NE_METROPOLIS, EA, POTTS = 0, 1, 2, 3, 4
 KERNEL_AUTO, KERNEL_GENERIC, KERNEL_TILED, KERNEL_RESIDENT, KERNEL_SMALL, KERNEL_SLAB, KERNEL_BULK = 0, 1, 2, 3, 4, 5, 6
-OK, ERR_ARG, ERR_UNSUPPORTED, ERR_CUDA, ERR_WORKSPACE, ERR_STATE = 0, -1, -2, -3, -4, -5
+OK, ERR_ARG, ERR_UNSUPPORTED, ERR_CUDA, ERR_WORKSPACE, ERR_STATE, ERR_LIMIT = 0, -1, -2, -3, -4, -5, -6
+NOALLOC_MAX_SWEEPS = 4096     # LSM_NOALLOC_MAX_SWEEPS of include/lsm.h
 
 # name -> (restype, argtypes); every symbol include/lsm.h declares
 _vp, _i32, _i64, _u64, _dbl, _sz = (ctypes.c_void_p, ctypes.c_int, ctypes.c_int64, ctypes.c_uint64,
@@ -30,6 +31,7 @@ SIGNATURES = {
     "lsm_sweep_record": (_i32, [_vp, _i64, _vp, _vp]),
     "lsm_sweep_record_host": (_i32, [_vp, _i64, _vp, _vp, _vp]),
     "lsm_sweep_record_host_async": (_i32, [_vp, _i64, _vp, _vp, _vp]),
+    "lsm_sweep_record_host_noalloc": (_i32, [_vp, _i64, _vp, _vp]),
     "lsm_stage_spins_host": (_i32, [_vp, _vp, _vp, _vp]),
     "lsm_sweep_random_tile": (_i32, [_vp, _i64, _i32, _i32, _vp, _vp]),
     "lsm_sweep_random_tile_balanced": (_i32, [_vp, _i64, _i32, _i32, _vp, _vp]),
@@ -250,6 +252,22 @@ class Lattice:
         """n sweeps; the (B, M) series lands in the pinned host tensor h_obs once `stream` has been synchronised."""
         _check(self._lib.lsm_sweep_record_host_async(self._h, int(n), _vp(h_obs.data_ptr()), _vp(d_scratch.data_ptr()),
                                                      self._sp(stream)), "lsm_sweep_record_host_async")
+        return h_obs
+
+    @_on_device
+    def sweep_record_host_noalloc(self, n, h_obs=None, stream=None):
+        """n sweeps with the (B, M) series delivered into a HOST array, for callers that cannot allocate device memory
+        (a plug-in under somebody else's memory pool, a loop that cannot afford cudaMalloc's device-wide synchronisation,
+        a spent memory quota): the device-side staging of the series is a fixed 64 KiB array inside liblsm.so instead of a
+        tensor, so this method creates no device tensor and the library call allocates nothing.  n is limited to
+        NOALLOC_MAX_SWEEPS (LsmError with code ERR_LIMIT beyond; split the run).  One array per GPU for all lattices:
+        do not let two such calls overlap on one GPU.  h_obs: int64 [n, 2] numpy array or host tensor (default: a
+        fresh numpy array)."""
+        if h_obs is None:
+            h_obs = np.empty((int(n), 2), dtype=np.int64)
+        ptr = h_obs.data_ptr() if hasattr(h_obs, "data_ptr") else h_obs.ctypes.data
+        _check(self._lib.lsm_sweep_record_host_noalloc(self._h, int(n), _vp(ptr), self._sp(stream)),
+               "lsm_sweep_record_host_noalloc")
         return h_obs
 
     @_on_device
