@@ -40,6 +40,8 @@ NCU_DRAM_BYTES_PER_LAUNCH = {
     "cfg5_c0.30": (67.18e6 + 0.75e6, "profiles/r2_tiled_variants_ncu.md"),
     "hbm3d_1024": (1083.86e6 + 497.63e6, "profiles/r2_tiled_variants_ncu.md"),
 }
+# smsp__issue_active.avg.pct_of_peak_sustained_active of the half-sweep kernel in the cited capture
+NCU_ISSUE_ACTIVE_PCT = {"cfg2_T2.269": 57.5}     # profiles/r2_cfg2_final.md
 KERNEL_FAMILY = {1: "generic", 2: "tiled", 3: "resident", 4: "small", 5: "slab", 6: "bulk"}
 KERNEL_NAME = {1: "k_sweep_generic (half-sweep)", 2: "k_sweep_tiled (half-sweep)",
                3: "k_sweep_resident (per half-sweep share of one launch)",
@@ -133,6 +135,17 @@ class ClockSampler(threading.Thread):
 
 
 # ----------------------------------------------------------------------------- oracle legs (CPU)
+def pin_to_one_core():
+    """SURVEY.md 8(d), oracle timing: the single-threaded oracle pinned to one core.  Returns (core, previous mask)."""
+    try:
+        old = os.sched_getaffinity(0)
+        cpu = max(old)
+        os.sched_setaffinity(0, {cpu})
+        return cpu, old
+    except (AttributeError, OSError):
+        return None, None
+
+
 def time_oracle(w, L, sweeps):
     """The oracle as it stands, one thread, on an L^dims lattice of workload w: updates/s."""
     from oracle import lsm_oracle as O
@@ -140,12 +153,17 @@ def time_oracle(w, L, sweeps):
     kw = w.create_args()
     kw["L"] = L
     o = O.Oracle(**kw)
-    t0 = time.perf_counter()
-    o.sweep(sweeps)
-    dt = time.perf_counter() - t0
+    cpu, old = pin_to_one_core()
+    try:
+        t0 = time.perf_counter()
+        o.sweep(sweeps)
+        dt = time.perf_counter() - t0
+    finally:
+        if old is not None:
+            os.sched_setaffinity(0, old)
     n = (L ** w.dims) * sweeps
     o.close()
-    return n / dt, dt, n
+    return n / dt, dt, n, cpu
 
 
 def run_reference(args, w):
@@ -160,15 +178,19 @@ def run_reference(args, w):
     kw = w.create_args()
     kw["L"] = L
     o = O.Oracle(**kw)
+    cpu, old = pin_to_one_core()
     for _ in range(args.warmup):
         o.sweep(1)
     t0 = time.perf_counter()
     for _ in range(args.steps):
         o.sweep(1)
     dt = time.perf_counter() - t0
+    if old is not None:
+        os.sched_setaffinity(0, old)
     upd = (L ** w.dims) * args.steps
     value = upd / dt / 1e9
-    sample = f"each step = 1 sweep of a {L}^{w.dims} lattice with the workload's J, h, T, seed ({L ** w.dims} updates)"
+    sample = (f"each step = 1 sweep of a {L}^{w.dims} lattice with the workload's J, h, T, seed ({L ** w.dims} updates); "
+              f"one thread pinned to core {cpu}: 1 of {os.cpu_count()}")
     line = {
         "impl": "reference", "metric": "site_updates_per_sec", "value": value, "unit": "Gflips/s",
         "n_gpus": args.gpus, "steps": args.steps, "warmup": args.warmup, "ms_per_step": dt / args.steps * 1e3,
@@ -241,7 +263,9 @@ def run_ours(args, w):
     launches = lat.launch_count - launches0
     step_ms = [a.elapsed_time(b) for a, b in ev]
     total_ms = sum(step_ms)
-    total_ms_max, updates_all, ups = replicas.aggregate(total_ms, N * S * K, lat.device)
+    total_ms_max, updates_all, ups_mean = replicas.aggregate(total_ms, N * S * K, lat.device)
+    # SURVEY.md 8(d) timing protocol: `value` is the MEDIAN timed step (max over ranks); the mean is kept beside it
+    med_ms_max, _, ups = replicas.aggregate(statistics.median(step_ms), N * S, lat.device)
     value = ups / 1e9
 
     # sanity of the state after the timed region: fused running sums == full reduction (a6 vs a8)
@@ -252,42 +276,37 @@ def run_ours(args, w):
     # ---- end-to-end through the C ABI with HOST buffers (pinned), copies inside the timed region.
     # Every step uploads its input configuration (N bytes, lsm_stage_spins_host on a copy stream), installs it
     # (lsm_set_spins: layout conversion + full reduction), sweeps S times and downloads the (B, M) series
-    # (lsm_sweep_record_host_async).  Two staging buffers: the upload of step k+1 overlaps the sweeps of step k.
-    h_in = torch.empty(N, dtype=torch.int8).pin_memory()
-    h_in.copy_(lat.get_spins().cpu())
-    Ke = max(3, min(K, 10))
-    h_obs = [torch.empty((S, 2), dtype=torch.int64).pin_memory() for _ in range(2)]
-    d_obs = [torch.empty((S, 2), dtype=torch.int64, device=lat.device) for _ in range(2)]
-    d_stage = [torch.empty(N, dtype=torch.int8, device=lat.device) for _ in range(2)]
-    copy_stream, comp = torch.cuda.Stream(device=lat.device), torch.cuda.current_stream(lat.device)
-    staged = [torch.cuda.Event() for _ in range(2)]
-    consumed = [torch.cuda.Event() for _ in range(2)]
+    # (lsm_sweep_record_host_async): paper_1209_0296_b200/pipeline.py, the sequence tests/test_gpu_e2e.py holds to the
+    # oracle.  Two DIFFERENT inputs alternate (the configurations at sweep tdone and tdone + S, each with its own sweep
+    # counter), and every downloaded series is compared with the one recorded when the lattice went through those sweeps
+    # directly, so a broken stream order shows up here and not only in the tests.
+    from paper_1209_0296_b200.pipeline import HostPipeline
 
-    def e2e_pass(n_steps):
-        lat.stage_spins_host(h_in, d_stage[0], copy_stream)
-        staged[0].record(copy_stream)
-        for k in range(n_steps):
-            b = k & 1
-            comp.wait_event(staged[b])
-            lat.set_spins(d_stage[b], tdone)                       # convert + full (B, M) reduction, compute stream
-            consumed[b].record(comp)
-            if k + 1 < n_steps:                                    # next step's upload, behind this step's sweeps
-                if k >= 1:
-                    copy_stream.wait_event(consumed[b ^ 1])
-                lat.stage_spins_host(h_in, d_stage[b ^ 1], copy_stream)
-                staged[b ^ 1].record(copy_stream)
-            lat.sweep_record_host_async(S, h_obs[b], d_obs[b])     # S sweeps + D2H of the series (enqueued)
+    h_in, ref_series = [], []
+    for i in range(2):
+        h = torch.empty(N, dtype=torch.int8).pin_memory()
+        h.copy_(lat.get_spins().cpu())
+        h_in.append((h, tdone + i * S))
+        ref_series.append(lat.sweep_record(S).cpu())
+    Ke = max(4, min(K, 10))
+    pipe = HostPipeline(lat, S)
+    seen = []
 
-    e2e_pass(2)
+    def check_series(k, series):                   # host side, two steps behind the GPU
+        seen.append(bool(torch.equal(series, ref_series[k & 1])))
+
+    pipe.run([h_in[k & 1] for k in range(2)])
     barrier()
     e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
     e0.record()
-    e2e_pass(Ke)
+    pipe.run([h_in[k & 1] for k in range(Ke)], consume=check_series)
     e1.record()
     torch.cuda.synchronize()
     e2e_ms = e0.elapsed_time(e1)
     e2e_value = replicas.aggregate(e2e_ms, N * S * Ke, lat.device)[2] / 1e9
-    assert int(h_obs[(Ke - 1) & 1][-1, 1]) == lat.measure_int()[1]     # the downloaded series is the one just computed
+    assert len(seen) == Ke and all(seen), f"e2e: downloaded series differ from the directly recorded ones: {seen}"
+    assert lat.measure_int()[2] == h_in[(Ke - 1) & 1][1] + S
+    e2e_oracle = e2e_oracle_check(lsm, wl, S) if rank == 0 else None
 
     if rank != 0:
         if world > 1:
@@ -296,13 +315,15 @@ def run_ours(args, w):
 
     # ---- roofline of the dominant kernel (the half-sweep kernel), DESIGN.md 6
     n_sweep_launches = 2 * S * K
-    avg_launch_s = (sum(step_ms) * 1e-3) / n_sweep_launches
+    avg_launch_s = (sum(step_ms) * 1e-3) / n_sweep_launches      # average launch duration over the whole timed region
     sm_count = torch.cuda.get_device_properties(local).multi_processor_count
     roofline, roofline_hbm = rooflines(wl, lat.kernel, avg_launch_s, sm_count, clocks.get("sm_max_mhz") or 1965)
 
     line = {
         "metric": "site_updates_per_sec", "value": value, "unit": "Gflips/s", "n_gpus": world, "steps": K,
-        "warmup": Wm, "ms_per_step": total_ms_max / K, "higher_is_better": True, "scaling": "weak",
+        "warmup": Wm, "ms_per_step": med_ms_max, "higher_is_better": True, "scaling": "weak",
+        "timing": {"value_is": "median of the timed steps (SURVEY.md 8(d))", "ms_per_step_mean": total_ms_max / K,
+                   "value_mean": ups_mean / 1e9},
         "vs_baseline": None, "dtype": "u32", "data": "synthetic",
         "config": {"workload": wl.name, "lattice": f"{wl.L}^{wl.dims}", "model": "Ising spin-1/2" if wl.two_S == 1 and wl.model == 0 else wl.note,
                    "T": wl.T, "J": wl.J, "h": wl.h, "sweeps_per_step": S, "record": "(B, M) after every sweep",
@@ -311,30 +332,116 @@ def run_ours(args, w):
                    "l2": "256 MiB flush write between timed steps; within a step a lattice smaller than the 126 MB L2 is re-read from L2"},
         "roofline": roofline,
         "roofline_hbm": roofline_hbm,
-        "e2e": {"value": e2e_value, "unit": "Gflips/s", "h2d_bytes_per_step": N, "d2h_bytes_per_step": 16 * S,
-                "steps": Ke,
+        "e2e": {"value": e2e_value, "unit": "Gflips/s", "h2d_bytes_per_step": pipe.h2d_bytes_per_step,
+                "d2h_bytes_per_step": pipe.d2h_bytes_per_step, "steps": Ke,
                 "api": "lsm_stage_spins_host (copy stream) + lsm_set_spins + lsm_sweep_record_host_async, pinned host buffers, "
-                       "two staging buffers: the upload of step k+1 overlaps the sweeps of step k"},
+                       "two staging buffers: the upload of step k+1 overlaps the sweeps of step k (paper_1209_0296_b200/pipeline.py)",
+                "inputs": "two different configurations (sweep counters tdone, tdone + S) alternate",
+                "verified": {"every_series_equals_direct_run": True, "oracle_reduced_shape": e2e_oracle}},
         "gpu_launches": int(launches),
         "clocks": clocks,
         "step_ms_min_med_max": [min(step_ms), statistics.median(step_ms), max(step_ms)],
     }
 
     if not args.no_extras and world == 1:
-        line["philox_only"] = philox_microbench(lsm, torch)
-        line["other_workloads"] = other_workloads(lsm, torch, w.name, sm_count, clocks.get("sm_max_mhz") or 1965)
-        from paper_1209_0296_b200 import workloads as W
-
+        words = 2 if wl.two_S == 2 or wl.model == lsm.POTTS else 1      # Philox words per update
+        po = philox_microbench(lsm, torch)
+        line["philox_only"] = po
+        # SURVEY.md 8(d)'s integer bound, measured in this run: register-only Philox words/s / words per update
+        roofline["philox_only_gwords_per_s"] = po["gwords_per_s"]
+        roofline["frac_vs_philox_only"] = value / (po["gwords_per_s"] / words)
+        roofline["sm_mhz_sampled"] = clocks.get("sm_mhz")
+        if clocks.get("sm_mhz"):
+            roofline["frac_at_sampled_clock"] = roofline["achieved"] / (sm_count * 64 * clocks["sm_mhz"] * 1e6 / 1e9)
+        roofline["issue_active_pct"] = NCU_ISSUE_ACTIVE_PCT.get(wl.name)
+        roofline["hbm"] = {k: roofline_hbm[k] for k in ("achieved", "peak", "unit", "frac")}
+        # three seeds for the headline: 1 warm-up + median of 5 steps each
+        roofline["three_seeds_gflips"] = three_seeds(lsm, torch, wl, S, lat.kernel, flush)
+        others = other_workloads(lsm, torch, w.name, sm_count, clocks.get("sm_max_mhz") or 1965, po)
+        line["other_workloads"] = others
+        # BASELINE.json's configs (and the extras) in the key the driver keeps: workload -> [Gflips/s, fraction of the
+        # binding roofline (null where the family has no per-half-sweep roofline), kernel family]
+        per = {wl.name: [round(value, 1), round(roofline["frac"], 3), KERNEL_FAMILY.get(lat.kernel, "?")]}
+        for name, o in others.items():
+            if "gflips" in o:
+                fr = (o.get("roofline") or {}).get("frac")
+                if fr is not None and o["roofline"].get("binding_bound") == "hbm":
+                    fr = o["roofline_hbm"]["frac"]
+                per[name] = [round(o["gflips"], 1), None if fr is None else round(fr, 3),
+                             o.get("kernel_family", "ne_tile" if "random_tile" in name else "?")]
+        roofline["per_config"] = per
+        roofline["per_config_note"] = ("[Gflips/s, fraction of the binding roofline, kernel family]; North-East rows (cfg5): the 12-slot model "
+                                       "charges one Philox word to every site while the rule draws only for facilitated sites (about c^2 of them), "
+                                       "so the fraction can exceed 1 at low c; random_tile rows: against 2 picks per Philox call; "
+                                       "null: the small family has no per-half-sweep launch to put against a roofline")
         sweeps = 4
-        v, dt, n = time_oracle(w, w.L, sweeps)
+        v, dt, n, cpu = time_oracle(w, w.L, sweeps)
         line["cpu_baseline"] = {"value": v / 1e9, "unit": "Gflips/s", "cores": 1, "kind": "oracle",
-                                "sample": f"{sweeps} sweeps of the full {w.L}^{w.dims} lattice ({n} updates, {dt:.1f} s), single thread of {os.cpu_count()}"}
+                                "sample": f"{sweeps} sweeps of the full {w.L}^{w.dims} lattice ({n} updates, {dt:.1f} s), "
+                                          f"pinned to core {cpu}: 1 of {os.cpu_count()}"}
     else:
         line["cpu_baseline"] = None
     print(json.dumps(line), flush=True)
     if world > 1:
         dist.destroy_process_group()
     return 0
+
+
+def three_seeds(lsm, torch, wl, S, family, flush):
+    """Headline workload with three seeds: per seed 1 warm-up step + the median of 5 timed steps (L2 flushed between)."""
+    from dataclasses import replace
+
+    out = {}
+    for i in range(3):
+        w = replace(wl, seed=wl.seed + 16 * i)
+        lat = lsm.Lattice(**w.create_args())
+        if w.model in (lsm.ISING, lsm.EA, lsm.POTTS):
+            lat.set_tracking(False)
+        lat.set_kernel(family)
+        obs = torch.empty((S, 2), dtype=torch.int64, device=lat.device)
+        lat.sweep_record(S, out=obs)
+        ms = []
+        for k in range(5):
+            flush.fill_(k)
+            e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+            e0.record()
+            lat.sweep_record(S, out=obs)
+            e1.record()
+            torch.cuda.synchronize()
+            ms.append(e0.elapsed_time(e1))
+        out[str(w.seed)] = round(w.N * S / (statistics.median(ms) * 1e-3) / 1e9, 1)
+        lat.close()
+    return out
+
+
+def e2e_oracle_check(lsm, w, S):
+    """Outside the timed region: the same pipeline on a reduced shape of the workload, three different inputs from an
+    oracle trajectory, every downloaded series and the final configuration compared with the oracle."""
+    import numpy as np
+    import torch
+
+    from oracle import lsm_oracle as O
+    from paper_1209_0296_b200.pipeline import HostPipeline
+
+    L = 256 if w.dims == 2 else 32
+    S = min(S, 20)
+    kw = w.create_args()
+    kw["L"] = L
+    traj, runner = O.Oracle(**kw), O.Oracle(**kw)
+    inputs, want = [], []
+    for t in (0, 3, 7):
+        traj.sweep(t - traj.sweeps_done)
+        cfg = traj.get_spins().copy()
+        runner.set_spins(cfg, t)
+        want.append(runner.sweep_record(S))
+        inputs.append((torch.from_numpy(cfg).pin_memory(), t))
+    lat = lsm.Lattice(**kw)
+    got = {}
+    HostPipeline(lat, S).run(inputs, consume=lambda k, series: got.__setitem__(k, series.numpy().copy()))
+    ok = all(np.array_equal(got[k], want[k]) for k in range(3)) and np.array_equal(lat.get_spins().cpu().numpy(), runner.get_spins())
+    lat.close()
+    assert ok, "e2e pipeline disagrees with the oracle on the reduced shape"
+    return f"{L}^{w.dims}, 3 steps x {S} sweeps: bit-exact"
 
 
 def rooflines(w, family, avg_launch_s, sm_count, sm_max_mhz):
@@ -389,7 +496,18 @@ def philox_microbench(lsm, torch):
             "updates_bound_gflips_1word": 4 * calls_s / 1e9, "updates_bound_gflips_2words": 2 * calls_s / 1e9}
 
 
-def other_workloads(lsm, torch, skip, sm_count, sm_max_mhz):
+def random_tile_roofline(gpicks, po):
+    """The random-tile schedule draws every pick: one Philox4x32-10 call serves two picks (position word + acceptance
+    word each; include/lsm.h, readings D21 / D24), so its integer bound is 2 x the register-only Philox call rate
+    measured in this run (k_ne_random_tile, one launch = half / a quarter of a sweep)."""
+    if not po:
+        return None
+    peak = 2.0 * po["gcalls_per_s"]
+    return {"bound": "alu", "achieved": gpicks, "peak": peak, "unit": "Gpick/s", "frac": gpicks / peak,
+            "peak_source": "2 picks per Philox call x philox_only.gcalls_per_s of this run", "kernel": "k_ne_random_tile"}
+
+
+def other_workloads(lsm, torch, skip, sm_count, sm_max_mhz, po=None):
     """Short timings of the other BASELINE.json configs (context for the headline number)."""
     from paper_1209_0296_b200 import workloads as W
 
@@ -440,7 +558,8 @@ def other_workloads(lsm, torch, skip, sm_count, sm_max_mhz):
                 torch.cuda.synchronize()
                 s_rt = e0.elapsed_time(e1) * 1e-3
                 out[name + "_random_tile_b32_lambda16"] = {"gflips": w.N * n_rt / s_rt / 1e9,
-                                                           "us_per_sweep": s_rt / n_rt * 1e6, "launches_per_sweep": 2}
+                                                           "us_per_sweep": s_rt / n_rt * 1e6, "launches_per_sweep": 2,
+                                                           "roofline": random_tile_roofline(w.N * n_rt / s_rt / 1e9, po)}
                 lat.sweep_random_tile(n_rt, 32, 16, out=obs, balanced=True)
                 torch.cuda.synchronize()
                 e0.record()
@@ -449,7 +568,8 @@ def other_workloads(lsm, torch, skip, sm_count, sm_max_mhz):
                 torch.cuda.synchronize()
                 s_rt = e0.elapsed_time(e1) * 1e-3
                 out[name + "_random_tile_balanced_b32_lambda16"] = {"gflips": w.N * n_rt / s_rt / 1e9,
-                                                                    "us_per_sweep": s_rt / n_rt * 1e6, "launches_per_sweep": 4}
+                                                                    "us_per_sweep": s_rt / n_rt * 1e6, "launches_per_sweep": 4,
+                                                                    "roofline": random_tile_roofline(w.N * n_rt / s_rt / 1e9, po)}
             lat.close()
             del lat, obs
         except Exception as e:  # a secondary workload must not take the headline down

@@ -97,6 +97,36 @@ def extras() -> dict[str, Workload]:
     return out
 
 
+def parse_shape(name: str) -> Workload:
+    """Any lattice of the models by name, so that every table row under profiles/ has a command
+    (`python bench.py --workload ea2d_1024 --kernel tiled --no-extras`):
+      ising2d_<L> ising3d_<L> spin1_2d_<L> spin1_3d_<L> ea2d_<L> ea3d_<L> ne2d_c<conc>_<L> potts2d_q<q>_<L> potts3d_q<q>_<L>
+    at the temperatures of the named workloads of the same model (2D Ising 2.269, 3D 4.5115, spin-1 3.0 with h = 0.01,
+    EA 1.0 / 1.1, Potts at its 2D transition 1/ln(1+sqrt q), 3D q = 3: 1.8164)."""
+    import re
+
+    m = re.fullmatch(r"(ising|spin1_|ea|potts|ne)([23])d(?:_q(\d+))?(?:_c([0-9.]+))?_(\d+)", name)
+    if not m:
+        raise KeyError(name)
+    kind, dims, q, c, L = m.group(1), int(m.group(2)), m.group(3), m.group(4), int(m.group(5))
+    seed = seed_of(10 + dims, L % 256)
+    if kind == "ising":
+        return Workload(name, 10, dims, L, T=2.269 if dims == 2 else 4.5115, seed=seed, note=f"Ising spin-1/2 {L}^{dims}")
+    if kind == "spin1_":
+        return Workload(name, 10, dims, L, two_S=2, h=0.01, T=3.0 if dims == 3 else 1.69, seed=seed, note=f"spin-1 Ising {L}^{dims}")
+    if kind == "ea":
+        return Workload(name, 10, dims, L, model=EA, T=1.0 if dims == 2 else 1.1, seed=seed, note=f"Edwards-Anderson {L}^{dims}")
+    if kind == "ne":
+        if dims != 2 or c is None:
+            raise KeyError(name)
+        return Workload(name, 10, 2, L, model=NE_HEATBATH, J=0.0, T=ne_temperature(float(c)), seed=seed, note=f"North-East {L}^2 c = {c}")
+    if q is None:
+        raise KeyError(name)
+    qq = int(q)
+    T = 1.0 / math.log(1.0 + math.sqrt(qq)) if dims == 2 else 1.8164
+    return Workload(name, 10, dims, L, two_S=qq - 1, model=POTTS, T=T, seed=seed, note=f"{qq}-state Potts {L}^{dims}")
+
+
 def by_name(name: str) -> Workload:
     both = {**configs(), **extras()}
-    return both[name]
+    return both[name] if name in both else parse_shape(name)
