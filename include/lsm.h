@@ -77,7 +77,8 @@ enum { LSM_ISING = 0, LSM_NE_HEATBATH = 1, LSM_NE_METROPOLIS = 2, LSM_EA = 3, LS
 enum {
     LSM_OK = 0,
     LSM_ERR_ARG = -1,         /* dims not 2|3, L odd or < 4, T <= 0 or non-finite, NULL, n < 0 */
-    LSM_ERR_UNSUPPORTED = -2, /* two_S not 1|2; NE with dims != 2, J != 0 or two_S != 1        */
+    LSM_ERR_UNSUPPORTED = -2, /* Ising two_S not 1|2; NE with dims != 2, J != 0 or two_S != 1; EA two_S != 1; Potts q = two_S + 1
+                                 outside [2, 8] or h != 0; a kernel family / tile / depth that cannot run this lattice */
     LSM_ERR_CUDA = -3,        /* a CUDA runtime call failed (text: lsm_last_cuda_error)         */
     LSM_ERR_WORKSPACE = -4,   /* workspace too small or not 256-byte aligned                   */
     LSM_ERR_STATE = -5,       /* tracking is off (lsm_persistence); replicas out of lockstep (batch) */
@@ -104,7 +105,11 @@ enum {
 enum { LSM_KERNEL_AUTO = 0, LSM_KERNEL_GENERIC = 1, LSM_KERNEL_TILED = 2, LSM_KERNEL_RESIDENT = 3, LSM_KERNEL_SMALL = 4,
        LSM_KERNEL_SLAB = 5, LSM_KERNEL_BULK = 6 };
 
-/* Device bytes lsm_create needs for this lattice (two colour arrays + small state). */
+/* Device bytes lsm_create needs for this lattice: the two colour arrays and a few hundred bytes of state, plus, where
+ * they apply, a second pair of colour arrays (North-East: the random-tile schedule), the bond bytes of both colours
+ * (Edwards-Anderson) and the boundary-row mailboxes of the SLAB family (shapes it covers: up to ~10 MB, e.g. 10.5 MB for
+ * 128^3, 2.6 MB for 1024^2, which for a 512^2 lattice is several times the lattice itself;
+ * lsm_batch_workspace_bytes is R times this plus a descriptor array). */
 int lsm_workspace_bytes(int dims, int L, int two_S, int model, size_t *bytes);
 
 /* Build the threshold table on the host (D3), draw the initial state from `seed` on the

@@ -39,12 +39,15 @@ struct lsm {
     uint32_t *d_mbox;   // slab family: mailbox rows at the end of the workspace (nullptr: shape not covered)
     size_t mbox_bytes;
     int slab_depth;     // requested temporal depth of the slab family (0: default)
+    int slab_refused;   // a cooperative slab launch did not fit this context (SM-limited MPS / green context): AUTO avoids the family
     uint8_t *alt[2];    // NE models: second lattice buffer of the random-tile schedule (reading D18)
 };
 
 static thread_local std::string g_cuda_err;
+static thread_local cudaError_t g_cuda_code = cudaSuccess;
 static int cuda_fail(cudaError_t e)
 {
+    g_cuda_code = e;
     g_cuda_err = std::string(cudaGetErrorName(e)) + ": " + cudaGetErrorString(e);
     return LSM_ERR_CUDA;
 }
@@ -141,7 +144,10 @@ static void choose_kernel(lsm *o)
 {
     int want = o->kernel_pref;
     bool tiled_ok = tiled_supported(o->lat, o->model, o->tiled);
-    if (want == LSM_KERNEL_AUTO) {
+    if (want == LSM_KERNEL_AUTO && o->slab_refused) {
+        if (small_plan(o->lat, o->model, o->tiled, &o->small, false)) want = LSM_KERNEL_SMALL;
+        else want = tiled_ok ? LSM_KERNEL_TILED : LSM_KERNEL_GENERIC;
+    } else if (want == LSM_KERNEL_AUTO) {
         // 512^2 ... 4096^2, 64^3, 128^3: the lattice lives in the SMs' shared memory (profiles/r2_slab_family.md)
         // (Edwards-Anderson / Potts have no small-family kernels: the slab family from 128^2 / 32^3)
         if ((o->N >= 262144 || o->model == M_EA || o->model == M_POTTS) &&
@@ -213,7 +219,7 @@ extern "C" int lsm_create(int dims, int L, int two_S, int model, double J, doubl
     o->d_mbox = o->mbox_bytes ? (uint32_t *)(base + need - align256(o->mbox_bytes)) : nullptr;
     o->lat.L = L; o->lat.Lh = L / 2; o->lat.dims = dims; o->lat.Lz = dims == 3 ? L : 1;
     o->lat.half = o->N / 2;
-    o->t = 0; o->tracking = 1; o->kernel_pref = LSM_KERNEL_AUTO; o->launches = 0; o->slab_depth = 0;
+    o->t = 0; o->tracking = 1; o->kernel_pref = LSM_KERNEL_AUTO; o->launches = 0; o->slab_depth = 0; o->slab_refused = 0;
     o->last_stream = (cudaStream_t)stream;
     build_tables(o);
     choose_kernel(o);
@@ -261,7 +267,12 @@ static int resident_launch(lsm *o, int64_t n, long long *obs, cudaStream_t s)
         if (o->kernel_in_use == LSM_KERNEL_SMALL) {
             CU(launch_sweep_small(o->lat, o->model, o->tracking, o->seed, o->t, k, obs, o->small, o->tiled, s));
         } else if (o->kernel_in_use == LSM_KERNEL_SLAB) {
-            CU(cudaMemsetAsync(o->d_mbox, 0x80, o->mbox_bytes, s));     // every mailbox lane: sweep parity 1 (lsm_slab.cu)
+            // every mailbox lane this launch can read: sweep parity 1 (lsm_slab.cu).  The layout puts the CTA outermost,
+            // so G slabs use the first G * 8 * dmax march rows of the reservation (which is sized for SLAB_MAX_CTAS).
+            const size_t rowbytes = (size_t)(o->L / 2) * (o->dims == 3 ? (size_t)o->L : 1);
+            size_t used = (size_t)o->slab.G * 8 * (size_t)o->slab.dmax * rowbytes;
+            if (used > o->mbox_bytes) used = o->mbox_bytes;
+            CU(cudaMemsetAsync(o->d_mbox, 0x80, used, s));
             CU(launch_sweep_slab(o->lat, o->model, o->tracking, o->seed, o->t, k, obs, o->d_mbox, o->slab, o->tiled, s));
         } else {
             CU(cudaMemsetAsync(o->d_flags, 0, 8 * (size_t)o->plan.grid, s));
@@ -302,8 +313,22 @@ static int sweep_impl(lsm *o, int64_t n, long long *d_obs, cudaStream_t s)
     const bool short_call = o->kernel_in_use == LSM_KERNEL_SLAB && o->kernel_pref == LSM_KERNEL_AUTO && n < 8 &&
                             o->N >= ((int64_t)1 << 24) && tiled_supported(o->lat, o->model, o->tiled);
     if (!short_call &&
-        (o->kernel_in_use == LSM_KERNEL_RESIDENT || o->kernel_in_use == LSM_KERNEL_SMALL || o->kernel_in_use == LSM_KERNEL_SLAB))
-        return sweep_resident(o, n, d_obs, s);
+        (o->kernel_in_use == LSM_KERNEL_RESIDENT || o->kernel_in_use == LSM_KERNEL_SMALL || o->kernel_in_use == LSM_KERNEL_SLAB)) {
+        const uint64_t t_before = o->t;
+        const int rc = sweep_resident(o, n, d_obs, s);
+        // One CTA per SM, all co-resident: under an SM-limited context (MPS active-thread percentage, green context) the
+        // cooperative slab launch is refused although the launch-per-half-sweep families run the lattice.  AUTO then
+        // gives the family up for this handle and finishes the call with the next best one (same results).
+        if (rc == LSM_ERR_CUDA && g_cuda_code == cudaErrorCooperativeLaunchTooLarge && o->kernel_in_use == LSM_KERNEL_SLAB &&
+            o->kernel_pref == LSM_KERNEL_AUTO) {
+            (void)cudaGetLastError();
+            o->slab_refused = 1;
+            choose_kernel(o);
+            const int64_t done = (int64_t)(o->t - t_before);
+            return sweep_impl(o, n - done, d_obs ? d_obs + 2 * done : nullptr, s);
+        }
+        return rc;
+    }
     const int family = short_call ? LSM_KERNEL_TILED : o->kernel_in_use;
     if (d_obs) CU(cudaMemsetAsync(d_obs, 0, (size_t)n * 16, s));
     else CU(cudaMemsetAsync(o->d_run, 0, 16, s));
@@ -336,7 +361,6 @@ extern "C" int lsm_sweep_record(lsm_t *o, int64_t n, int64_t *d_obs, void *strea
 static int random_tile_impl(lsm_t *o, int64_t n, int tile_edge, int lambda, int64_t *d_obs, void *stream, bool balanced)
 {
     if (!o || n < 0) return LSM_ERR_ARG;
-    if (o->model != M_NE_HEATBATH && o->model != M_NE_METROPOLIS) return LSM_ERR_UNSUPPORTED;
     if (o->model != M_NE_HEATBATH && o->model != M_NE_METROPOLIS) return LSM_ERR_UNSUPPORTED;
     if (!ne_tile_supported(o->lat, tile_edge, lambda, balanced)) return LSM_ERR_UNSUPPORTED;
     cudaStream_t s = (cudaStream_t)stream;
@@ -388,12 +412,9 @@ extern "C" int lsm_sweep_record_host_async(lsm_t *o, int64_t n, int64_t *h_obs, 
 
 extern "C" int lsm_sweep_record_host(lsm_t *o, int64_t n, int64_t *h_obs, int64_t *d_scratch, void *stream)
 {
-    if (!o || n < 0 || ((!h_obs || !d_scratch) && n > 0)) return LSM_ERR_ARG;
-    cudaStream_t s = (cudaStream_t)stream;
-    int rc = sweep_impl(o, n, (long long *)d_scratch, s);
+    int rc = lsm_sweep_record_host_async(o, n, h_obs, d_scratch, stream);
     if (rc != LSM_OK) return rc;
-    if (n > 0) CU(cudaMemcpyAsync(h_obs, d_scratch, (size_t)n * 16, cudaMemcpyDeviceToHost, s));
-    CU(cudaStreamSynchronize(s));
+    CU(cudaStreamSynchronize((cudaStream_t)stream));
     return LSM_OK;
 }
 
@@ -658,7 +679,11 @@ extern "C" int lsm_batch_measure_int(lsm_batch_t *b, int64_t *B, int64_t *M)
     if (!b) return LSM_ERR_ARG;
     std::vector<long long> v(2 * (size_t)b->R);
     cudaStream_t s = b->rep[0]->last_stream;
-    for (int r = 0; r < b->R; ++r) CU(cudaMemcpyAsync(&v[2 * r], b->rep[r]->d_run, 16, cudaMemcpyDeviceToHost, s));
+    // the replicas' running pairs sit rep_bytes apart in the batch workspace: one strided copy instead of R small ones
+    if (b->R > 1 && b->rep_bytes <= ((size_t)1 << 30))
+        CU(cudaMemcpy2DAsync(v.data(), 16, b->rep[0]->d_run, b->rep_bytes, 16, (size_t)b->R, cudaMemcpyDeviceToHost, s));
+    else
+        for (int r = 0; r < b->R; ++r) CU(cudaMemcpyAsync(&v[2 * r], b->rep[r]->d_run, 16, cudaMemcpyDeviceToHost, s));
     CU(cudaStreamSynchronize(s));
     for (int r = 0; r < b->R; ++r) {
         if (B) B[r] = v[2 * r];

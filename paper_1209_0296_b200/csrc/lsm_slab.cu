@@ -25,7 +25,15 @@
 //   * D = 1 is the plain scheme (one row of the colour just updated per half-sweep, no redundant update).
 // Mailboxes are double-buffered by epoch parity: a CTA rewrites buffer e & 1 in epoch e + 2, which it can only start
 // after it has read the neighbours' rows of epoch e + 1, and those were computed from this CTA's rows of epoch e.
-// The host sets every mailbox lane to 0x80808080 before a launch; epoch e writes bit 31 = (e >> 1) & 1.
+// What the reuse argument rests on (there is no fence anywhere in the protocol): a reader's load of a mailbox word has
+// COMPLETED by the time the reader acts on it -- the loop in slab_take4 consumes the loaded value in its exit test, and
+// the value is stored to shared memory before the CTA's bar.sync -- so once a CTA's rows of epoch e + 1 are visible to
+// its neighbour (which the neighbour's tag check establishes by data dependence), every load the CTA made from the
+// neighbour's buffer of epoch e is over and the neighbour may overwrite that buffer.  With the "early" exchange
+// (SlabArgs::early: depth 1, long steps) the polling loads are issued before the CTA barrier instead of after it;
+// the argument is the same, and that path has its own long-run cases in tests/test_gpu_parity.py
+// (test_slab_long_run_against_the_tiled_family: 2048^2 and 4096^2 at depth 1).
+// The host sets every mailbox lane the launch can read to 0x80808080 before a launch; epoch e writes bit 31 = (e >> 1) & 1.
 // Only own rows count for the per-sweep (B, M).  Bit-identical to every other family.
 #include "lsm_tiled_dev.cuh"
 

@@ -217,11 +217,16 @@ def test_slab_temporal_blocking_parity(kw, depths):
     (dict(dims=2, L=1024, T=2.0, h=0.1), 2, 40000),
     (dict(dims=3, L=128, T=4.5115), 1, 10000),
     (dict(dims=2, L=1536, model=lsm.NE_HEATBATH, J=0.0, T=W.ne_temperature(0.3)), 2, 20000),
+    # depth 1 with at least 768 words per step: the "early" exchange, which polls the neighbours' mailbox words before
+    # the CTA barrier (slab_plan: 2048^2, 3072^2, 4096^2 at depth 1)
+    (dict(dims=2, L=2048, T=2.269), 1, 12000),
+    (dict(dims=2, L=4096, T=2.269), 1, 10000),
 ])
 def test_slab_long_run_against_the_tiled_family(kw, depth, n):
     """The mailbox protocol of the slab family over 10^4 ... 10^5 sweeps (2 x 10^4 ... 10^5 exchanges per CTA pair): the
     configuration, the running sums and the persistence counts must equal those of the tiled family, which the other
-    tests hold to the oracle sweep by sweep."""
+    tests hold to the oracle sweep by sweep; at the end the oracle itself checks one more slab sweep from the late state
+    (the random words are a pure function of (seed, sweep, half, site))."""
     a, b = lsm.Lattice(seed=77, **kw), lsm.Lattice(seed=77, **kw)
     a.set_kernel(lsm.KERNEL_SLAB)
     a.set_temporal_depth(depth)
@@ -232,6 +237,14 @@ def test_slab_long_run_against_the_tiled_family(kw, depth, n):
         assert a.measure_int() == b.measure_int()
     assert torch.equal(a.get_spins(), b.get_spins())
     assert a.persistence() == b.persistence() and a.measure_full() == a.measure_int()[:2]
+    # late one-step spot check against the oracle: its state := the slab family's at sweep n, one sweep on either side
+    orc = O.Oracle(seed=77, **kw)
+    orc.set_spins(a.get_spins_host(), n)
+    assert orc.measure_int() == a.measure_int()[:2]
+    series = a.sweep_record(1).cpu().numpy()
+    orc.sweep(1)
+    assert np.array_equal(a.get_spins_host(), orc.get_spins())
+    assert tuple(series[0]) == orc.measure_int() and a.measure_int()[2] == n + 1
     a.close()
     b.close()
 
