@@ -61,6 +61,8 @@ def parse():
     ap.add_argument("--batch-scan", action="store_true", help="instead of the benchmark: lsm_batch_sweep_record over R and cluster size")
     ap.add_argument("--size-scan", action="store_true",
                     help="instead of the benchmark: us/sweep of the tiled and the small (cluster) family over lattice sizes")
+    ap.add_argument("--ne-scan", action="store_true",
+                    help="instead of the benchmark: the North-East model at the paper's sizes (checkerboard / random-tile / balanced)")
     ap.add_argument("--pipe-probe", action="store_true",
                     help="instead of the benchmark: the integer-pipe microbenchmarks behind the 'alu' roofline (DESIGN.md 6)")
     ap.add_argument("--kernel", default="auto", choices=["auto", "generic", "tiled", "resident", "small", "slab", "bulk"],
@@ -706,6 +708,67 @@ PROBE_MODES = [
 ]
 
 
+def ne_scan():
+    """The North-East model at the paper's own sizes (128^2 and 512^2, 30 realisations per concentration)
+    and upwards: us per sweep of the checkerboard sweep, of the paper's corrected algorithm (32 x 32 tiles, lambda = 16,
+    PAPER.md:128-140,155; two dependent launches per sweep) and of its balance-preserving variant (four launches), for one
+    lattice; then 30 realisations one after the other on one stream and on 30 streams."""
+    import torch
+
+    from paper_1209_0296_b200 import build, lsm, workloads as W
+
+    build.build()
+    T = W.ne_temperature(0.30)
+
+    def timed(fn, n):
+        fn(n)
+        torch.cuda.synchronize()
+        e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        e0.record()
+        fn(n)
+        e1.record()
+        torch.cuda.synchronize()
+        return e0.elapsed_time(e1) * 1e3 / n
+
+    for L in (128, 512, 2048, 8192):
+        n = 200 if L <= 512 else 20
+        lat = lsm.Lattice(dims=2, L=L, model=lsm.NE_HEATBATH, J=0.0, T=T, seed=7)
+        row = {"L": L, "c": 0.30, "auto_family": KERNEL_FAMILY.get(lat.kernel),
+               "checkerboard_us_per_sweep": timed(lambda k: lat.sweep(k), n),
+               "random_tile_b32_l16_us_per_sweep": timed(lambda k: lat.sweep_random_tile(k, 32, 16), n),
+               "balanced_b32_l16_us_per_sweep": timed(lambda k: lat.sweep_random_tile(k, 32, 16, balanced=True), n)}
+        for key in ("checkerboard", "random_tile_b32_l16", "balanced_b32_l16"):
+            row[key + "_gflips"] = lat.N / row[key + "_us_per_sweep"] / 1e3
+        lat.close()
+        print(json.dumps(row), flush=True)
+    for L in (128, 512):
+        R, n = 30, 200
+        lats = [lsm.Lattice(dims=2, L=L, model=lsm.NE_HEATBATH, J=0.0, T=T, seed=100 + r) for r in range(R)]
+        streams = [torch.cuda.Stream() for _ in range(R)]
+        torch.cuda.synchronize()
+
+        def serial(k):
+            for lat in lats:
+                lat.sweep_random_tile(k, 32, 16)
+
+        def parallel(k):
+            cur = torch.cuda.current_stream()
+            for lat, st in zip(lats, streams):
+                st.wait_stream(cur)                       # fork from / join into the stream the timing events are on
+                lat.sweep_random_tile(k, 32, 16, stream=st)
+            for st in streams:
+                cur.wait_stream(st)
+
+        row = {"L": L, "realisations": R, "one_stream_us_per_sweep_of_all": timed(serial, n),
+               "streams_us_per_sweep_of_all": timed(parallel, n)}
+        row["one_stream_gflips"] = R * L * L / row["one_stream_us_per_sweep_of_all"] / 1e3
+        row["streams_gflips"] = R * L * L / row["streams_us_per_sweep_of_all"] / 1e3
+        for lat in lats:
+            lat.close()
+        print(json.dumps(row), flush=True)
+    return 0
+
+
 def pipe_probe(blocks_per_sm=8, iters=1024):
     """Register-only integer instruction streams (csrc/probe/pipe_probe.cu, its own libpipe_probe.so): cycles per loop
     iteration and warp against the issue law of DESIGN.md 6 -- every 16-lane math instruction (ALU or FMA-heavy pipe)
@@ -754,6 +817,8 @@ def main():
     args = parse()
     if args.pipe_probe:
         return pipe_probe()
+    if args.ne_scan:
+        return ne_scan()
     if args.batch_scan:
         return batch_scan()
     if args.size_scan:
