@@ -765,6 +765,12 @@ def ne_scan():
         row["streams_gflips"] = R * L * L / row["streams_us_per_sweep_of_all"] / 1e3
         for lat in lats:
             lat.close()
+        # the same 30 realisations as ONE batch: every launch of the schedule covers the tiles of all of them
+        batch = lsm.Batch(T=[T] * R, seeds=[100 + r for r in range(R)], dims=2, L=L, model=lsm.NE_HEATBATH, J=0.0)
+        row["batch_us_per_sweep_of_all"] = timed(lambda k: batch.sweep_random_tile(k, 32, 16), n)
+        row["batch_balanced_us_per_sweep_of_all"] = timed(lambda k: batch.sweep_random_tile(k, 32, 16, balanced=True), n)
+        row["batch_gflips"] = R * L * L / row["batch_us_per_sweep_of_all"] / 1e3
+        batch.close()
         print(json.dumps(row), flush=True)
     return 0
 

@@ -197,6 +197,13 @@ int lsm_batch_size(lsm_batch_t *, int *R);
 int lsm_batch_replica(lsm_batch_t *, int r, lsm_t **borrowed_handle);
 int lsm_batch_sweep(lsm_batch_t *, int64_t n, void *stream);
 int lsm_batch_sweep_record(lsm_batch_t *, int64_t n, int64_t *d_obs, void *stream);
+/* North-East batches: n sweeps of lsm_sweep_random_tile (balanced = 0) or lsm_sweep_random_tile_balanced (balanced != 0) on
+ * every replica, each launch of the schedule covering the tiles of ALL replicas -- the paper averages 30 realisations of
+ * 128^2 and 512^2 lattices per concentration, and one 128^2 lattice is 16 tiles = one thread block.
+ * Same arguments and restrictions as the single-lattice calls; d_obs: NULL, or device int64 [R][n][2] = (0, M) of replica r
+ * after sweep k.  Replica r ends bit-identical to a single handle swept with the same call.  LSM_ERR_STATE if the replicas'
+ * sweep counters or tracking states differ.  Asynchronous. */
+int lsm_batch_sweep_random_tile(lsm_batch_t *, int64_t n, int tile_edge, int lambda, int balanced, int64_t *d_obs, void *stream);
 int lsm_batch_set_temperatures(lsm_batch_t *, const double *T);
 int lsm_batch_set_tracking(lsm_batch_t *, int on, void *stream);
 int lsm_batch_set_cluster(lsm_batch_t *, int blocks_per_replica);

@@ -674,6 +674,69 @@ extern "C" int lsm_batch_sweep_record(lsm_batch_t *b, int64_t n, int64_t *d_obs,
     return batch_sweep_impl(b, n, (long long *)d_obs, (cudaStream_t)stream);
 }
 
+// The random-tile schedules for a whole batch (30 realisations per concentration; a 128^2 lattice is 16
+// tiles, one CTA): every launch of the schedule handles the tiles of ALL replicas, so a sweep of the batch costs the two
+// (four) launches a single lattice pays.  Bit-identical to lsm_sweep_random_tile[_balanced] on every replica.
+static int batch_random_tile_impl(lsm_batch *b, int64_t n, int tile_edge, int lambda, long long *d_obs, cudaStream_t s,
+                                  bool balanced)
+{
+    lsm *o0 = b->rep[0];
+    if (o0->model != M_NE_HEATBATH && o0->model != M_NE_METROPOLIS) return LSM_ERR_UNSUPPORTED;
+    if (!ne_tile_supported(o0->lat, tile_edge, lambda, balanced)) return LSM_ERR_UNSUPPORTED;
+    if ((size_t)b->R * 2 * sizeof(NeBatchDesc) > batch_desc_bytes(b->R)) return LSM_ERR_UNSUPPORTED;
+    const uint64_t t0 = o0->t;
+    for (lsm *o : b->rep) {
+        if (o->t != t0 || o->tracking != o0->tracking) return LSM_ERR_STATE;
+        o->last_stream = s;
+    }
+    if (n == 0) return LSM_OK;
+    const uint64_t ALWAYS = (uint64_t)1 << 32;
+    // descriptors of both launch directions (colour arrays -> second buffer and back), the checkerboard batch's
+    // descriptors share the region and are uploaded again when it runs next
+    std::vector<NeBatchDesc> d(2 * (size_t)b->R);
+    for (int dir = 0; dir < 2; ++dir)
+        for (int r = 0; r < b->R; ++r) {
+            const lsm *o = b->rep[r];
+            NeBatchDesc &e = d[(size_t)dir * b->R + r];
+            std::memset(&e, 0, sizeof(e));
+            for (int c = 0; c < 2; ++c) {
+                e.src[c] = dir ? o->alt[c] : o->lat.col[c];
+                e.dst[c] = dir ? o->lat.col[c] : o->alt[c];
+            }
+            e.obs = d_obs ? d_obs + 2 * n * r : o->d_run;
+            e.k0 = (uint32_t)o->seed;
+            e.k1 = (uint32_t)(o->seed >> 32);
+            e.thr_c = o->thr[0] >= ALWAYS ? 0xFFFFFFFFu : (uint32_t)o->thr[0];
+            e.thr_up = o->thr[1] >= ALWAYS ? 0xFFFFFFFFu : (uint32_t)o->thr[1];
+            e.up_always = o->thr[1] >= ALWAYS ? 1 : 0;
+        }
+    NeBatchDesc *d_desc = (NeBatchDesc *)b->d_desc;
+    CU(cudaMemcpyAsync(d_desc, d.data(), d.size() * sizeof(NeBatchDesc), cudaMemcpyHostToDevice, s));   // pageable: staged before return
+    b->h_desc.clear();
+    if (d_obs) CU(cudaMemsetAsync(d_obs, 0, (size_t)n * 16 * (size_t)b->R, s));
+    else CU(cudaMemset2DAsync(o0->d_run, b->rep_bytes, 0, 16, (size_t)b->R, s));
+    const int nlaunch = balanced ? 4 : 2;                           // reading D23 / D17: an even number, so the buffers end where they began
+    for (int64_t k = 0; k < n; ++k) {
+        for (int launch = 0; launch < nlaunch; ++launch) {
+            const long long off = launch != nlaunch - 1 ? -1 : d_obs ? 2 * k : (k == n - 1 ? 0 : -1);
+            CU(launch_ne_random_tile_batch(o0->lat, d_desc + (size_t)(launch & 1) * b->R, b->R, o0->model == M_NE_METROPOLIS,
+                                           balanced, tile_edge, lambda, t0 + (uint64_t)k, launch, o0->tracking, off, s));
+            b->launches += 1;
+        }
+    }
+    for (lsm *o : b->rep) o->t = t0 + (uint64_t)n;
+    if (d_obs)      // running pairs := last recorded pairs (rows 16 n bytes apart -> pairs rep_bytes apart)
+        CU(cudaMemcpy2DAsync(o0->d_run, b->rep_bytes, d_obs + 2 * (n - 1), (size_t)n * 16, 16, (size_t)b->R, cudaMemcpyDeviceToDevice, s));
+    return LSM_OK;
+}
+
+extern "C" int lsm_batch_sweep_random_tile(lsm_batch_t *b, int64_t n, int tile_edge, int lambda, int balanced, int64_t *d_obs,
+                                           void *stream)
+{
+    if (!b || n < 0) return LSM_ERR_ARG;
+    return batch_random_tile_impl(b, n, tile_edge, lambda, (long long *)d_obs, (cudaStream_t)stream, balanced != 0);
+}
+
 extern "C" int lsm_batch_measure_int(lsm_batch_t *b, int64_t *B, int64_t *M)
 {
     if (!b) return LSM_ERR_ARG;

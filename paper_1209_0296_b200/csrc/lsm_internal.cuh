@@ -180,6 +180,19 @@ cudaError_t launch_ne_random_tile(const Lat &lat, uint8_t *const dst[2], bool me
                                   unsigned long long seed, unsigned long long t, int launch, uint32_t thr_c,
                                   uint32_t thr_up, int up_always, int track, long long *obs, cudaStream_t s);
 
+// Batch form (lsm_batch_sweep_random_tile): one descriptor per lattice and launch direction, in device memory.
+struct NeBatchDesc {
+    const uint8_t *src[2];   // lattice at launch start
+    uint8_t *dst[2];         // lattice after the launch
+    long long *obs;          // base of the lattice's (B, M) slots (a recorded series or the running pair)
+    uint32_t k0, k1;         // Philox key = the lattice's seed
+    uint32_t thr_c, thr_up;  // its thresholds
+    int up_always;
+    int pad;
+};
+cudaError_t launch_ne_random_tile_batch(const Lat &lat, const NeBatchDesc *d_desc, int R, bool metropolis, bool balanced, int b,
+                                        int lam, unsigned long long t, int launch, int track, long long obs_off, cudaStream_t s);
+
 int sm_count();
 
 }  // namespace lsmk

@@ -35,6 +35,12 @@ struct NeTileArgs {
     int up_always;           // Metropolis: exp(-1/T) rounds to 2^32
     int track;
     long long *obs;          // (B, M) slot receiving the up-count after the launch, or nullptr
+    // BATCH instantiations (lsm_batch_sweep_random_tile): R lattices of this shape in one launch, tile index
+    // rep * ntiles + T.  Buffers, key, thresholds and the observable slot come from desc[rep]; obs_off is the offset (in
+    // int64) of this launch's (B, M) slot behind desc[rep].obs, or -1 for a launch that records nothing.
+    const NeBatchDesc *desc;
+    int R;
+    long long obs_off;
 };
 
 __device__ __forceinline__ uint32_t lds_u8(uint32_t a)
@@ -46,6 +52,12 @@ __device__ __forceinline__ uint32_t lds_u8(uint32_t a)
 __device__ __forceinline__ void sts_u8(uint32_t a, uint32_t v)
 {
     asm volatile("st.shared.u8 [%0], %1;" ::"r"(a), "r"(v) : "memory");
+}
+
+// The same with the key in registers (batch: every lattice has its own seed): two more additions per round.
+__device__ __forceinline__ uint4 philox_k(uint32_t c0, uint32_t c1, uint32_t c2, uint32_t c3, uint32_t k0, uint32_t k1)
+{
+    return philox4x32_10(c0, c1, c2, c3, k0, k1);
 }
 
 // Philox4x32-10 on counter (c0, c1, a.c2, a.c3) with the round keys read from the kernel parameters.
@@ -67,7 +79,7 @@ __device__ __forceinline__ uint4 philox_rk(uint32_t c0, uint32_t c1, const NeTil
 #ifndef LSM_NE_TILE_MINBLOCKS
 #define LSM_NE_TILE_MINBLOCKS 4
 #endif
-template <bool METRO, bool BAL>
+template <bool METRO, bool BAL, bool BATCH = false>
 __global__ void __launch_bounds__(256, LSM_NE_TILE_MINBLOCKS)
 k_ne_random_tile(const __grid_constant__ NeTileArgs a)
 {
@@ -90,14 +102,33 @@ k_ne_random_tile(const __grid_constant__ NeTileArgs a)
     // 32-bit shared-space addresses for the pick loop (no generic-address conversion per access)
     const uint32_t s_tile = (uint32_t)__cvta_generic_to_shared(tile), s_east = s_tile + 2u * (uint32_t)col_bytes,
                    s_claim = s_east + (uint32_t)b;
-    const uint32_t chg = a.track ? 0x08u : 0u, thr_c = a.thr_c, thr_up = a.thr_up;
-    const bool up_always = a.up_always != 0;
+    const uint32_t chg = a.track ? 0x08u : 0u;
+    uint32_t thr_c = a.thr_c, thr_up = a.thr_up;
+    bool up_always = a.up_always != 0;
+    const int ntiles_all = BATCH ? a.ntiles * a.R : a.ntiles;
+    const uint8_t *src0 = a.src[0], *src1 = a.src[1];
+    uint8_t *dst0 = a.dst[0], *dst1 = a.dst[1];
+    uint32_t bk0 = 0u, bk1 = 0u;                                      // BATCH: Philox key of the tile's lattice
+    long long *bobs = nullptr;
     const int q = BAL ? P >> (a.lg_lam + 3) : P >> (a.lg_lam + 1), calls = (lam + 1) >> 1;   // D23 / D17
     int ups = 0;
 
-    for (int base = warp_global * grp_per_warp; base < a.ntiles; base += nwarps * grp_per_warp) {
-        const int T = base + grp_in_warp;
-        const bool live = has_tile && T < a.ntiles;                    // tail groups idle but keep the warp converged
+    for (int base = warp_global * grp_per_warp; base < ntiles_all; base += nwarps * grp_per_warp) {
+        int T = base + grp_in_warp;
+        const bool live = has_tile && T < ntiles_all;                  // tail groups idle but keep the warp converged
+        if (BATCH) {
+            const int rep = live ? T / a.ntiles : 0;
+            T -= rep * a.ntiles;
+            const NeBatchDesc &dsc = a.desc[rep];
+            src0 = dsc.src[0]; src1 = dsc.src[1]; dst0 = dsc.dst[0]; dst1 = dsc.dst[1];
+            bk0 = dsc.k0; bk1 = dsc.k1;
+            thr_c = dsc.thr_c; thr_up = dsc.thr_up; up_always = dsc.up_always != 0;
+            bobs = dsc.obs;
+        }
+        auto philox = [&](const uint32_t c0, const uint32_t c1) {
+            if (BATCH) return philox_k(c0, c1, a.c2, a.c3, bk0, bk1);
+            return philox_rk(c0, c1, a);
+        };
         const int ty = live ? T / a.ntx : 0, tx = live ? T - ty * a.ntx : 0;   // one division per tile
         const int x0 = tx << a.lg_b, y0 = ty << a.lg_b;
         const uint32_t key_hi = ((uint32_t)grp_in_warp << 16) | (live ? 0u : 0x80000000u);
@@ -111,7 +142,7 @@ k_ne_random_tile(const __grid_constant__ NeTileArgs a)
                 const int rr = i >> (lg_cr + 1), c = (i >> lg_cr) & 1, u = i & ((1 << lg_cr) - 1);
                 int yy = y0 + rr;
                 if (yy >= a.L) yy -= a.L;
-                const uint8_t *g = (c ? a.src[1] : a.src[0]) + (size_t)yy * a.Lh + (x0 >> 1) + (u << lg_cw);
+                const uint8_t *g = (c ? src1 : src0) + (size_t)yy * a.Lh + (x0 >> 1) + (u << lg_cw);
                 const uint32_t d = s_tile + (uint32_t)(c * col_bytes + rr * rowb + (u << lg_cw));
                 if (lg_cw == 4) asm volatile("cp.async.ca.shared.global [%0], [%1], 16;" ::"r"(d), "l"(g) : "memory");
                 else asm volatile("cp.async.ca.shared.global [%0], [%1], 4;" ::"r"(d), "l"(g) : "memory");
@@ -120,7 +151,7 @@ k_ne_random_tile(const __grid_constant__ NeTileArgs a)
             if (xe >= a.L) xe -= a.L;
             for (int py = j; py < b; py += lam) {
                 const int yy = y0 + py;
-                east[py] = (((xe + yy) & 1) ? a.src[1] : a.src[0])[(size_t)yy * a.Lh + (xe >> 1)];
+                east[py] = (((xe + yy) & 1) ? src1 : src0)[(size_t)yy * a.Lh + (xe >> 1)];
             }
         }
         asm volatile("cp.async.commit_group;\n\tcp.async.wait_group 0;" ::: "memory");
@@ -159,7 +190,7 @@ k_ne_random_tile(const __grid_constant__ NeTileArgs a)
             // ---- balance-preserving variant (readings D22-D24): lambda red picks, barrier, lambda
             // white picks, barrier; one Philox call per lane and sub-step (words 0, 1: red pick; 2, 3: white pick)
             for (int k = 0; k < q; ++k) {
-                const uint4 w = philox_rk((uint32_t)T, (uint32_t)(k * lam + j), a);
+                const uint4 w = philox((uint32_t)T, (uint32_t)(k * lam + j));
 #pragma unroll
                 for (int c = 0; c < 2; ++c) {
                     const int r = (int)__umulhi(c ? w.z : w.x, (uint32_t)(P >> 1));   // r-th site of colour c, row-major
@@ -176,7 +207,7 @@ k_ne_random_tile(const __grid_constant__ NeTileArgs a)
             };
             if (lam == 1) {
                 for (int k = 0; k < q; ++k) {
-                    const uint4 w = philox_rk((uint32_t)T, (uint32_t)k, a);
+                    const uint4 w = philox((uint32_t)T, (uint32_t)k);
                     go(w.x, w.y);
                 }
             } else {
@@ -186,7 +217,7 @@ k_ne_random_tile(const __grid_constant__ NeTileArgs a)
                 for (int k = 0; k < q; k += 2) {
                     const int kk = k + (j & 1);                        // the odd lane works one sub-step ahead
                     uint4 w = make_uint4(0, 0, 0, 0);
-                    if (kk < q) w = philox_rk((uint32_t)T, (uint32_t)(kk * calls + (j >> 1)), a);
+                    if (kk < q) w = philox((uint32_t)T, (uint32_t)(kk * calls + (j >> 1)));
                     {                                                  // sub-step k: the even lane's call
                         const uint32_t pz = __shfl_xor_sync(0xffffffffu, w.z, 1), pw = __shfl_xor_sync(0xffffffffu, w.w, 1);
                         go((j & 1) ? pz : w.x, (j & 1) ? pw : w.y);
@@ -205,7 +236,7 @@ k_ne_random_tile(const __grid_constant__ NeTileArgs a)
                 for (int i = j; i < (b << (lg_cr + 1)); i += lam) {
                     const int rr = i >> (lg_cr + 1), c = (i >> lg_cr) & 1, u = i & ((1 << lg_cr) - 1);
                     const uint4 v = *reinterpret_cast<const uint4 *>((tile + c * col_bytes) + rr * rowb + 16 * u);
-                    *reinterpret_cast<uint4 *>((c ? a.dst[1] : a.dst[0]) + (size_t)(y0 + rr) * a.Lh + (x0 >> 1) + 16 * u) = v;
+                    *reinterpret_cast<uint4 *>((c ? dst1 : dst0) + (size_t)(y0 + rr) * a.Lh + (x0 >> 1) + 16 * u) = v;
                     ups += (int)__dp4a((v.x & 0x01010101u) + (v.y & 0x01010101u) + (v.z & 0x01010101u) + (v.w & 0x01010101u),
                                        0x01010101u, 0u);
                 }
@@ -214,14 +245,18 @@ k_ne_random_tile(const __grid_constant__ NeTileArgs a)
                 for (int i = j; i < (b << (lg_lr + 1)); i += lam) {
                     const int rr = i >> (lg_lr + 1), c = (i >> lg_lr) & 1, u = i & ((1 << lg_lr) - 1);
                     const uint32_t v = *reinterpret_cast<const uint32_t *>((tile + c * col_bytes) + rr * rowb + 4 * u);
-                    *reinterpret_cast<uint32_t *>((c ? a.dst[1] : a.dst[0]) + (size_t)(y0 + rr) * a.Lh + (x0 >> 1) + 4 * u) = v;
+                    *reinterpret_cast<uint32_t *>((c ? dst1 : dst0) + (size_t)(y0 + rr) * a.Lh + (x0 >> 1) + 4 * u) = v;
                     ups += (int)__dp4a(v & 0x01010101u, 0x01010101u, 0u);
                 }
             }
         }
+        if (BATCH) {                                                   // the warp's groups may sit in different lattices
+            if (live && a.obs_off >= 0 && ups != 0) atomicAdd((unsigned long long *)&bobs[a.obs_off + 1], (unsigned long long)ups);
+            ups = 0;
+        }
         __syncwarp();
     }
-    if (a.obs) {
+    if (!BATCH && a.obs) {
         const int s = __reduce_add_sync(0xffffffffu, ups);
         if (lane == 0 && s != 0) atomicAdd((unsigned long long *)&a.obs[1], (unsigned long long)s);
     }
@@ -301,6 +336,43 @@ cudaError_t launch_ne_random_tile(const Lat &lat, uint8_t *const dst[2], bool me
         if (e != cudaSuccess) return e;
     }
     kern<<<grid, threads, smem, s>>>(a);
+    return cudaGetLastError();
+}
+
+// R lattices of one shape in one launch (lsm_batch_sweep_random_tile): d_desc[r] names lattice r's buffers of this launch.
+cudaError_t launch_ne_random_tile_batch(const Lat &lat, const NeBatchDesc *d_desc, int R, bool metropolis, bool balanced, int b,
+                                        int lam, unsigned long long t, int launch, int track, long long obs_off, cudaStream_t s)
+{
+    NeTileArgs a;
+    memset(&a, 0, sizeof(a));
+    a.L = lat.L;
+    a.Lh = lat.Lh;
+    while ((1 << a.lg_b) < b) ++a.lg_b;
+    while ((1 << a.lg_lam) < lam) ++a.lg_lam;
+    a.ntx = lat.L / b;
+    a.ntiles = a.ntx * a.ntx;
+    a.c2 = (uint32_t)t;
+    a.c3 = ((balanced ? 8u : 4u) + (uint32_t)launch) | ((uint32_t)(t >> 32) << 4);
+    a.track = track;
+    a.desc = d_desc;
+    a.R = R;
+    a.obs_off = obs_off;
+    const int threads = ne_tile_threads(b, lam);
+    a.gpw = ne_tile_gpw(b, lam);
+    const int tiles_per_cta = (threads / 32) * a.gpw;
+    const size_t smem = tiles_per_cta * ne_tile_bytes(b, lam);
+    const long long total = (long long)a.ntiles * R;
+    if (total > 0x7fffffffLL) return cudaErrorInvalidValue;
+    long long grid = (total + tiles_per_cta - 1) / tiles_per_cta;
+    const int cap = sm_count() * 8;
+    if (grid > cap) grid = cap;
+    auto kern = balanced ? (metropolis ? k_ne_random_tile<true, true, true> : k_ne_random_tile<false, true, true>)
+                         : (metropolis ? k_ne_random_tile<true, false, true> : k_ne_random_tile<false, false, true>);
+    if (smem > 48 * 1024) {
+        cudaError_t e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+        if (e != cudaSuccess) return e;
+    }
+    kern<<<(unsigned)grid, threads, smem, s>>>(a);
     return cudaGetLastError();
 }
 

@@ -42,6 +42,7 @@ SIGNATURES = {
     "lsm_batch_replica": (_i32, [_vp, _i32, _P(_vp)]),
     "lsm_batch_sweep": (_i32, [_vp, _i64, _vp]),
     "lsm_batch_sweep_record": (_i32, [_vp, _i64, _vp, _vp]),
+    "lsm_batch_sweep_random_tile": (_i32, [_vp, _i64, _i32, _i32, _i32, _vp, _vp]),
     "lsm_batch_set_temperatures": (_i32, [_vp, _vp]),
     "lsm_batch_set_tracking": (_i32, [_vp, _i32, _vp]),
     "lsm_batch_set_cluster": (_i32, [_vp, _i32]),
@@ -497,6 +498,20 @@ class Batch:
         assert out.is_cuda and out.dtype == torch.int64 and out.is_contiguous() and out.numel() >= 2 * int(n) * self.R
         _check(self._lib.lsm_batch_sweep_record(self._h, int(n), _vp(out.data_ptr()), self._sp(stream)),
                "lsm_batch_sweep_record")
+        return out
+
+    @_on_device
+    def sweep_random_tile(self, n=1, b=32, lam=16, record=False, out=None, stream=None, balanced=False):
+        """North-East batches: n sweeps of the paper's corrected algorithm (balanced=True: its
+        balance-preserving variant) on every replica, each launch covering the tiles of all replicas.
+        record=True returns the device [R, n, 2] series (0, M)."""
+        import torch
+
+        if record and out is None:
+            out = torch.empty((self.R, int(n), 2), dtype=torch.int64, device=self.device)
+        ptr = _vp(out.data_ptr()) if out is not None else None
+        _check(self._lib.lsm_batch_sweep_random_tile(self._h, int(n), int(b), int(lam), 1 if balanced else 0, ptr,
+                                                     self._sp(stream)), "lsm_batch_sweep_random_tile")
         return out
 
     @_on_device

@@ -152,3 +152,60 @@ def test_batch_lockstep_and_argument_errors():
     batch.close()
     with pytest.raises(lsm.LsmError):
         lsm.Batch(dims=2, L=33, T=[2.0], seeds=[1])
+
+
+@pytest.mark.parametrize("model", [lsm.NE_HEATBATH, lsm.NE_METROPOLIS])
+@pytest.mark.parametrize("L,R,b,lam,balanced", [
+    (128, 30, 32, 16, False),          # the paper's case: 30 realisations of 128^2, 32 x 32 tiles, lambda = 16
+    (128, 30, 32, 16, True),
+    (64, 7, 8, 32, False),             # collisions in almost every sub-step; R * tiles is odd per warp pair
+    (64, 5, 16, 4, True),
+    (96, 3, 32, 1, False),             # lambda = 1: one lane per tile, 9 tiles per lattice (groups of a warp in different lattices)
+    (512, 4, 32, 16, False),
+    (256, 3, 128, 4, False),           # tiles too large for every group of a warp to hold one
+])
+def test_batch_random_tile_matches_independent_oracles(model, L, R, b, lam, balanced):
+    """lsm_batch_sweep_random_tile (SURVEY.md 8(f) NEXT-1 x NEXT-3): every replica must end exactly as the
+    oracle's random-tile schedule leaves a single lattice with its temperature and seed -- recorded series, unrecorded
+    sweeps, mixed with checkerboard batch sweeps, persistence included."""
+    kw = dict(dims=2, L=L, model=model, J=0.0)
+    T = [W.ne_temperature(0.2 + 0.25 * r / R) for r in range(R)]
+    seeds = [W.seed_of(12, 1) + 13 * r for r in range(R)]
+    batch = lsm.Batch(T=T, seeds=seeds, **kw)
+    orcs = oracles(kw, T, seeds)
+    rec = (lambda o, n: o.sweep_random_tile_balanced_record(n, b, lam)) if balanced else (lambda o, n: o.sweep_random_tile_record(n, b, lam))
+    n = 4
+    l0 = batch.launch_count
+    got = batch.sweep_random_tile(n, b, lam, record=True, balanced=balanced).cpu().numpy()
+    assert batch.launch_count - l0 == n * (4 if balanced else 2)            # launches do not grow with R
+    for r, o in enumerate(orcs):
+        assert np.array_equal(got[r], rec(o, n)), r
+    check_all(batch, orcs)
+    batch.sweep_random_tile(3, b, lam, balanced=balanced)                   # only the last sweep is measured
+    batch.sweep(2)                                                          # checkerboard sweeps of the same batch in between
+    got = batch.sweep_random_tile(1, b, lam, record=True, balanced=balanced).cpu().numpy()
+    for r, o in enumerate(orcs):
+        rec(o, 3)
+        o.sweep(2)
+        assert np.array_equal(got[r], rec(o, 1)), r
+    check_all(batch, orcs)
+    # a replica swept on its own puts the batch out of lockstep
+    batch.replica(1).sweep_random_tile(1, b, lam, balanced=balanced)
+    with pytest.raises(lsm.LsmError) as e:
+        batch.sweep_random_tile(1, b, lam, balanced=balanced)
+    assert e.value.code == lsm.ERR_STATE
+    batch.close()
+
+
+def test_batch_random_tile_argument_checks():
+    batch = lsm.Batch(T=[2.0, 2.1], seeds=[1, 2], dims=2, L=64)
+    with pytest.raises(lsm.LsmError) as e:
+        batch.sweep_random_tile(1, 32, 16)                                  # Ising batch
+    assert e.value.code == lsm.ERR_UNSUPPORTED
+    batch.close()
+    batch = lsm.Batch(T=[1.0, 1.1], seeds=[1, 2], dims=2, L=64, model=lsm.NE_HEATBATH, J=0.0)
+    with pytest.raises(lsm.LsmError) as e:
+        batch.sweep_random_tile(1, 24, 16)                                  # tile edge not a power of two
+    assert e.value.code == lsm.ERR_UNSUPPORTED
+    assert batch.sweep_random_tile(0, 32, 16) is None
+    batch.close()
