@@ -25,15 +25,18 @@ def phi_curves(L, c, schedules, times, realisations, seed0=1209, model=lsm.NE_ME
     out = {}
     for (b, lam) in schedules:
         acc = [[] for _ in times]
-        for r in range(realisations):
-            lat = lsm.Lattice(dims=2, L=L, model=model, J=0.0, T=T, seed=seed0 + r, device=device)
-            t_now = 0
-            for k, t in enumerate(times):
-                lat.sweep_random_tile(t - t_now, b, lam)
-                t_now = t
-                _, ov = lat.persistence()
-                acc[k].append(lsm.phi(ov, lat.N, c_lib))
-            lat.close()
+        # all realisations of a schedule as one batch: every launch of the schedule covers the tiles of all of them
+        # (lsm_batch_sweep_random_tile; replica r is bit-identical to a single lattice with seed seed0 + r)
+        batch = lsm.Batch(T=[T] * realisations, seeds=[seed0 + r for r in range(realisations)], dims=2, L=L, model=model,
+                          J=0.0, device=device)
+        t_now = 0
+        for k, t in enumerate(times):
+            batch.sweep_random_tile(t - t_now, b, lam)
+            t_now = t
+            for r in range(realisations):
+                _, ov = batch.replica(r).persistence()
+                acc[k].append(lsm.phi(ov, batch.N, c_lib))
+        batch.close()
         mean = [sum(a) / len(a) for a in acc]
         se = [math.sqrt(sum((x - m) ** 2 for x in a) / max(len(a) - 1, 1) / len(a)) for a, m in zip(acc, mean)]
         out[(b, lam)] = {"phi": mean, "se": se}
@@ -48,13 +51,19 @@ def main(argv=None) -> int:
     ap.add_argument("--times", type=int, nargs="+", default=[10, 30, 100, 300, 1000])
     a = ap.parse_args(argv)
     sched = [(a.L, 1), (32, 1), (32, 4), (32, 16), (32, 32), (16, 32), (8, 32)]
+    import time
+
+    t0 = time.perf_counter()
     res = phi_curves(a.L, a.c, sched, a.times, a.realisations)
+    wall = time.perf_counter() - t0
     ref = res[(a.L, 1)]
     for (b, lam), v in res.items():
         dev = max(abs(x - y) for x, y in zip(v["phi"], ref["phi"]))
         print(json.dumps({"tile_edge": b, "lambda": lam, "lambda_over_P": lam / (b * b), "times": a.times,
                           "phi": [round(x, 4) for x in v["phi"]], "se": [round(x, 4) for x in v["se"]],
                           "max_abs_dev_from_serial": round(dev, 4)}))
+    print(json.dumps({"wall_s": round(wall, 2), "L": a.L, "realisations": a.realisations, "schedules": len(sched),
+                      "sweeps_per_realisation_and_schedule": max(a.times)}))
     return 0
 
 
