@@ -42,9 +42,8 @@ NCU_DRAM_BYTES_PER_LAUNCH = {
 }
 # smsp__issue_active.avg.pct_of_peak_sustained_active of the half-sweep kernel in the cited capture
 NCU_ISSUE_ACTIVE_PCT = {"cfg2_T2.269": 57.5}     # profiles/r2_cfg2_final.md
-KERNEL_FAMILY = {1: "generic", 2: "tiled", 3: "resident", 4: "small", 5: "slab", 6: "bulk"}
+KERNEL_FAMILY = {1: "generic", 2: "tiled", 4: "small", 5: "slab", 6: "bulk"}
 KERNEL_NAME = {1: "k_sweep_generic (half-sweep)", 2: "k_sweep_tiled (half-sweep)",
-               3: "k_sweep_resident (per half-sweep share of one launch)",
                4: "k_sweep_small_lane (per half-sweep share of one launch)",
                5: "k_sweep_slab (per half-sweep share of one launch)", 6: "k_sweep_tiled_bulk (half-sweep)"}
 
@@ -65,7 +64,7 @@ def parse():
                     help="instead of the benchmark: the North-East model at the paper's sizes (checkerboard / random-tile / balanced)")
     ap.add_argument("--pipe-probe", action="store_true",
                     help="instead of the benchmark: the integer-pipe microbenchmarks behind the 'alu' roofline (DESIGN.md 6)")
-    ap.add_argument("--kernel", default="auto", choices=["auto", "generic", "tiled", "resident", "small", "slab", "bulk"],
+    ap.add_argument("--kernel", default="auto", choices=["auto", "generic", "tiled", "small", "slab", "bulk"],
                     help="kernel family (lsm_set_kernel); auto = the library's choice")
     return ap.parse_args()
 
@@ -235,7 +234,7 @@ def run_ours(args, w):
     if wl.model in (lsm.ISING, lsm.EA, lsm.POTTS):
         lat.set_tracking(False)  # persistence is not part of configs 1-4
     if args.kernel != "auto":
-        lat.set_kernel({"generic": lsm.KERNEL_GENERIC, "tiled": lsm.KERNEL_TILED, "resident": lsm.KERNEL_RESIDENT,
+        lat.set_kernel({"generic": lsm.KERNEL_GENERIC, "tiled": lsm.KERNEL_TILED,
                         "small": lsm.KERNEL_SMALL, "slab": lsm.KERNEL_SLAB, "bulk": lsm.KERNEL_BULK}[args.kernel])
     N = lat.N
     obs = torch.empty((S, 2), dtype=torch.int64, device=lat.device)

@@ -89,7 +89,8 @@ enum {
  *           cluster barrier between the colours (L a power of two >= 8; other L with L % 32 == 0 up to 32 768
  *           sites); chosen below 262 144 sites (up to 256^2, 32^3);
  *  TILED    one launch per half-sweep, 16 sites per 128-bit word (L % 32 == 0, no "never" threshold);
- *  RESIDENT one cooperative launch for all sweeps with neighbour-flag synchronisation (opt-in, large lattices);
+ *  RESIDENT removed in round 3 (one cooperative launch with neighbour-flag synchronisation: measured 18 % slower than TILED,
+ *           superseded by SLAB); the value stays reserved and lsm_set_kernel answers LSM_ERR_UNSUPPORTED;
  *  SLAB     one cooperative launch for all sweeps of a call with the whole lattice resident in the shared memory of
  *           one CTA per SM: slabs of march rows, boundary rows exchanged through self-validating mailbox words in L2, one per
  *           CTA, several half-sweeps per exchange (lsm_set_temporal_depth); L a multiple of 32, 512^2 ... 4096^2,
@@ -233,7 +234,9 @@ int lsm_get_spins(lsm_t *, int8_t *d_out, void *stream);
 int lsm_get_spins_host(lsm_t *, int8_t *h_out, int8_t *d_scratch /* N bytes */, void *stream);
 /* Replace configuration and sweep counter (LSM_ERR_ARG unless sweep_counter < 2^60), recompute (B, M);
  * snapshot and flags untouched.
- * Values outside the model's set give LSM_ERR_ARG only for NULL; they are not range-checked. */
+ * Values outside the model's set are not an error: the conversion maps every byte into the set (Ising spin-1/2 and EA:
+ * > 0 -> +1, else -1; spin-1: clamped to [-1, +1]; North-East: non-zero -> 1; Potts: clamped to [0, q-1]), so no input
+ * can corrupt the packed neighbour sums or the flag bits.  LSM_ERR_ARG for NULL. */
 int lsm_set_spins(lsm_t *, const int8_t *d_in, uint64_t sweep_counter, void *stream);
 int lsm_set_spins_host(lsm_t *, const int8_t *h_in, int8_t *d_scratch /* N bytes */,
                        uint64_t sweep_counter, void *stream);

@@ -13,7 +13,7 @@ import sys
 PKG = os.path.dirname(os.path.abspath(__file__))
 CSRC = os.path.join(PKG, "csrc")
 LIB = os.path.join(PKG, "liblsm.so")
-SOURCES = ["lsm_api.cu", "lsm_generic.cu", "lsm_tiled.cu", "lsm_tiled_bulk.cu", "lsm_resident.cu", "lsm_small.cu", "lsm_slab.cu", "lsm_ne_tile.cu"]
+SOURCES = ["lsm_api.cu", "lsm_generic.cu", "lsm_tiled.cu", "lsm_tiled_bulk.cu", "lsm_small.cu", "lsm_slab.cu", "lsm_ne_tile.cu"]
 NVCC_FLAGS = [
     "-gencode", "arch=compute_100a,code=sm_100a",
     "-lineinfo", "-O3", "-std=c++17",

@@ -32,8 +32,7 @@ struct lsm {
     int nthr;
     Thr64 thr_param;
     TiledTables tiled;
-    unsigned *d_flags;  // resident family: one progress word per CTA
-    ResidentPlan plan;
+    unsigned *d_flags;  // reserved words of the workspace state block (the removed resident family's progress flags)
     SmallPlan small;
     SlabPlan slab;
     uint32_t *d_mbox;   // slab family: mailbox rows at the end of the workspace (nullptr: shape not covered)
@@ -162,8 +161,7 @@ static void choose_kernel(lsm *o)
     if (want == LSM_KERNEL_SMALL && !small_plan(o->lat, o->model, o->tiled, &o->small, true))
         want = tiled_ok ? LSM_KERNEL_TILED : LSM_KERNEL_GENERIC;
     if (want == LSM_KERNEL_TILED && !tiled_ok) want = LSM_KERNEL_GENERIC;
-    if (want == LSM_KERNEL_RESIDENT && !resident_plan(o->lat, o->model, o->tracking, o->tiled, &o->plan))
-        want = tiled_ok ? LSM_KERNEL_TILED : LSM_KERNEL_GENERIC;
+    if (want == LSM_KERNEL_RESIDENT) want = tiled_ok ? LSM_KERNEL_TILED : LSM_KERNEL_GENERIC;   // family removed (lsm_set_kernel refuses it)
     if (want == LSM_KERNEL_SLAB && !slab_plan(o->lat, o->model, o->tiled, o->slab_depth, &o->slab))
         want = tiled_ok ? LSM_KERNEL_TILED : LSM_KERNEL_GENERIC;
     if (want == LSM_KERNEL_BULK && !tiled_bulk_supported(o->lat, o->model, o->tiled))
@@ -257,7 +255,7 @@ static int enqueue_half(lsm *o, int family, int half, long long *obs, int want_B
     return LSM_OK;
 }
 
-// Resident family: whole sweeps per launch.  Without a per-sweep record only the last sweep is
+// Families that run whole sweeps per launch (small, slab).  Without a per-sweep record only the last sweep is
 // measured (into the running pair), so it gets a launch of its own.
 static int resident_launch(lsm *o, int64_t n, long long *obs, cudaStream_t s)
 {
@@ -275,9 +273,7 @@ static int resident_launch(lsm *o, int64_t n, long long *obs, cudaStream_t s)
             CU(cudaMemsetAsync(o->d_mbox, 0x80, used, s));
             CU(launch_sweep_slab(o->lat, o->model, o->tracking, o->seed, o->t, k, obs, o->d_mbox, o->slab, o->tiled, s));
         } else {
-            CU(cudaMemsetAsync(o->d_flags, 0, 8 * (size_t)o->plan.grid, s));
-            CU(launch_sweep_resident(o->lat, o->model, o->tracking, o->seed, o->t, k, obs, o->d_flags, 0u, o->plan,
-                                     o->tiled, s));
+            return LSM_ERR_UNSUPPORTED;
         }
         o->launches += 1;
         o->t += (uint64_t)k;
@@ -313,7 +309,7 @@ static int sweep_impl(lsm *o, int64_t n, long long *d_obs, cudaStream_t s)
     const bool short_call = o->kernel_in_use == LSM_KERNEL_SLAB && o->kernel_pref == LSM_KERNEL_AUTO && n < 8 &&
                             o->N >= ((int64_t)1 << 24) && tiled_supported(o->lat, o->model, o->tiled);
     if (!short_call &&
-        (o->kernel_in_use == LSM_KERNEL_RESIDENT || o->kernel_in_use == LSM_KERNEL_SMALL || o->kernel_in_use == LSM_KERNEL_SLAB)) {
+        (o->kernel_in_use == LSM_KERNEL_SMALL || o->kernel_in_use == LSM_KERNEL_SLAB)) {
         const uint64_t t_before = o->t;
         const int rc = sweep_resident(o, n, d_obs, s);
         // One CTA per SM, all co-resident: under an SM-limited context (MPS active-thread percentage, green context) the
@@ -834,7 +830,7 @@ extern "C" int lsm_set_tracking(lsm_t *o, int on, void *stream)
     CU(launch_reset_reference(o->lat, o->model, on ? 1 : 0, s));
     o->launches += 1;
     o->tracking = on ? 1 : 0;
-    choose_kernel(o);          // the resident family's grid depends on the instantiation's occupancy
+    choose_kernel(o);
     return LSM_OK;
 }
 
@@ -930,8 +926,7 @@ extern "C" int lsm_set_kernel(lsm_t *o, int family)
 {
     if (!o || family < LSM_KERNEL_AUTO || family > LSM_KERNEL_BULK) return LSM_ERR_ARG;
     if (family == LSM_KERNEL_TILED && !tiled_supported(o->lat, o->model, o->tiled)) return LSM_ERR_UNSUPPORTED;
-    if (family == LSM_KERNEL_RESIDENT && !resident_plan(o->lat, o->model, o->tracking, o->tiled, &o->plan))
-        return LSM_ERR_UNSUPPORTED;
+    if (family == LSM_KERNEL_RESIDENT) return LSM_ERR_UNSUPPORTED;      // removed in round 3: superseded by the slab family
     if (family == LSM_KERNEL_SMALL && !small_plan(o->lat, o->model, o->tiled, &o->small, true)) return LSM_ERR_UNSUPPORTED;
     if (family == LSM_KERNEL_SLAB && !slab_plan(o->lat, o->model, o->tiled, o->slab_depth, &o->slab)) return LSM_ERR_UNSUPPORTED;
     if (family == LSM_KERNEL_BULK && !tiled_bulk_supported(o->lat, o->model, o->tiled)) return LSM_ERR_UNSUPPORTED;

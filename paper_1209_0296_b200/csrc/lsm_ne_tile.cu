@@ -76,9 +76,7 @@ __device__ __forceinline__ uint4 philox_rk(uint32_t c0, uint32_t c1, const NeTil
     return make_uint4(c0, c1, c2, c3);
 }
 
-#ifndef LSM_NE_TILE_MINBLOCKS
 #define LSM_NE_TILE_MINBLOCKS 4
-#endif
 template <bool METRO, bool BAL, bool BATCH = false>
 __global__ void __launch_bounds__(256, LSM_NE_TILE_MINBLOCKS)
 k_ne_random_tile(const __grid_constant__ NeTileArgs a)

@@ -321,9 +321,7 @@ k_sweep_slab(const __grid_constant__ SlabArgs a, const __grid_constant__ PhiloxS
 // ------------------------------------------------------------------------------------------
 PhiloxSweepConsts make_philox_consts(const SweepKey &k);   // lsm_tiled.cu
 
-#ifndef LSM_SLAB_SMEM_MAX
 #define LSM_SLAB_SMEM_MAX (220 * 1024)     // dynamic shared memory per CTA (227 KB opt-in minus the static part)
-#endif
 
 // Largest temporal depth the mailboxes of this shape are sized for (0: the slab family never runs it).  Deep halos pay
 // where a half-sweep is shorter than an exchange (~1 us): the smaller 2D lattices.

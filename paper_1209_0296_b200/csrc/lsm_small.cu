@@ -478,12 +478,8 @@ static cudaError_t small_launch_to(bool track, bool obs, int threads, cudaStream
 }
 
 // Compile-time knobs for tuning experiments; the library reads no environment variables.
-#ifndef LSM_SMALL_MAX_CLUSTER
 #define LSM_SMALL_MAX_CLUSTER 16         // B200 schedules 16-block clusters
-#endif
-#ifndef LSM_SMALL_MAX_SITES
 #define LSM_SMALL_MAX_SITES 262144       // above 512^2 / 64^3 the tiled family wins (profiles/r1_small_family.md)
-#endif
 static int small_max_cluster() { return LSM_SMALL_MAX_CLUSTER; }
 static int small_max_sites() { return LSM_SMALL_MAX_SITES; }
 

@@ -25,13 +25,9 @@
 #include <cstring>
 
 // up-concentration from which the North-East rule runs the four Philox calls of a word together (see update_word)
-#ifndef LSM_NE_ALL4_C
 #define LSM_NE_ALL4_C 0.25
-#endif
 
-#ifndef LSM_TILED_THREADS
 #define LSM_TILED_THREADS 256            // threads per CTA (<= 256: the ring has 256 slots per stage)
-#endif
 
 namespace lsmk {
 
@@ -62,7 +58,7 @@ k_sweep_tiled(const __grid_constant__ TiledGeom g, const __grid_constant__ Philo
     } sm;
     // two-stage per-thread ring of the asynchronous copies (March::step_pf): N, O [, Yp, Yn] words and the edge lane
     // (spin-1 keeps the direct loads: its rule needs the registers the copies' addresses would take)
-    constexpr bool PF = LSM_TILED_PF_ONE || (MODEL != M_ISING_ONE && MODEL != M_POTTS);
+    constexpr bool PF = MODEL != M_ISING_ONE && MODEL != M_POTTS;   // two-word rules load directly (the ring measured slower there)
     __shared__ __align__(16) uint4 ring[PF ? ((DIMS == 3 ? 8 : 4) + (MODEL == M_EA ? 2 : 0)) * 256 : 1];
     __shared__ uint32_t ringE[PF ? 2 * 256 : 1];
     // Programmatic dependent launch: the next half-sweep's CTAs may be scheduled as soon as SM resources
@@ -103,7 +99,7 @@ k_sweep_tiled(const __grid_constant__ TiledGeom g, const __grid_constant__ Philo
         const int col = (int)(gt - (long long)seg * g.ncol);
         const int n = march_init(M, g, g.own, g.oth, g.half, seg, col, true);
         nsites = 16 * n;
-        if constexpr ((MODEL == M_ISING_ONE || MODEL == M_POTTS) && LSM_TILED_ONE_UNROLL1 && !PF) {
+        if constexpr (!PF) {
             M.template run1<true>(n, pc);
         } else
         if (g.parity_rows) {            // warp-uniform branch: q is a constant inside each loop
@@ -191,18 +187,9 @@ bool tiled_supported(const Lat &lat, int model, const TiledTables &t)
 // Launch shape: threads = word columns x march segments, one wave of CTAS_PER_SM resident CTAs per
 // SM (finer segments do not help: measured, profiles/).  Compile-time knobs for tuning experiments
 // (-DLSM_TILED_...); the library reads no environment variables.
-#ifndef LSM_TILED_CTAS_PER_SM
 #define LSM_TILED_CTAS_PER_SM 0          // 0: tiled_minblocks(model)
-#endif
-#ifndef LSM_TILED_WAVES_X4
 #define LSM_TILED_WAVES_X4 4             // waves in quarters
-#endif
-#ifndef LSM_TILED_THREADS
-#define LSM_TILED_THREADS 256            // threads per CTA (<= 256: the ring has 256 slots)
-#endif
-#ifndef LSM_TILED_PDL
 #define LSM_TILED_PDL 1                  // programmatic dependent launch
-#endif
 static const int g_tiled_ctas_per_sm = LSM_TILED_CTAS_PER_SM;
 static const int g_tiled_waves_x4 = LSM_TILED_WAVES_X4;
 static const int g_tiled_pdl = LSM_TILED_PDL;

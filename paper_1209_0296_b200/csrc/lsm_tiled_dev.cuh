@@ -1,32 +1,19 @@
 // lsm_tiled_dev.cuh -- device code of the vectorised half-sweep, shared by
-// the one-launch-per-half-sweep kernel (lsm_tiled.cu) and the resident multi-sweep kernel
-// (lsm_resident.cu): hoisted Philox, per-lane update rules, the register march of one thread.
+// the one-launch-per-half-sweep kernel (lsm_tiled.cu), its bulk-copy form and the slab / small families: hoisted Philox,
+// per-lane update rules, the register march of one thread.
 #pragma once
 #include "lsm_tiled.cuh"
 
 #include <type_traits>
 
-#ifndef LSM_TILED_MINBLOCKS
 #define LSM_TILED_MINBLOCKS 4
-#endif
 
 // spin-1 needs two Philox calls per lane; measured 2/3/4 CTAs per SM: 518/478/414 Gflips/s on cfg4
-#ifndef LSM_TILED_MINBLOCKS_ONE
 #define LSM_TILED_MINBLOCKS_ONE 2
-#endif
 // spin-1/2 Ising: the march is bound by pipe issue, not by latency (4 independent Philox chains per thread), and runs
 // fastest with 2 CTAs per SM and up to 128 registers (measured 1/2/3/4/5/6 CTAs: 1132/1163/1141/1120/1027/970
 // Gflips/s on cfg2); the North-East rule, which skips Philox for most lanes, prefers 4.
-#ifndef LSM_TILED_MINBLOCKS_HALF
 #define LSM_TILED_MINBLOCKS_HALF 2
-#endif
-#ifndef LSM_TILED_PF_ONE
-#define LSM_TILED_PF_ONE 0
-#endif
-// spin-1: one step per loop iteration instead of the 2x-unrolled, parity-specialised loop
-#ifndef LSM_TILED_ONE_UNROLL1
-#define LSM_TILED_ONE_UNROLL1 1
-#endif
 
 namespace lsmk {
 
@@ -705,26 +692,6 @@ struct March {
     {
 #pragma unroll 1
         for (int k = 0; k < n; ++k) step<2, UP>(pc);
-    }
-
-    // The same with the resident family's hooks: h.after_first() once the first row is stored,
-    // h.before_last() before the last row is loaded (lsm_resident.cu).
-    template <int Q0, bool UP, class PC, class H>
-    __device__ __forceinline__ void run_hooked(int n, const PC &pc, H &h)
-    {
-        constexpr int Q1 = Q0 == 2 ? 2 : 1 - Q0;
-        int k = 0;
-        for (; k + 1 < n; k += 2) {
-            step<Q0, UP>(pc);
-            if (k == 0) h.after_first();
-            if (k + 2 == n) h.before_last();
-            step<Q1, UP>(pc);
-        }
-        if (k < n) {
-            h.before_last();
-            step<Q0, UP>(pc);
-            if (k == 0) h.after_first();
-        }
     }
 };
 

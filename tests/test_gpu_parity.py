@@ -80,7 +80,7 @@ SHAPES = [
     (dict(dims=2, L=256, model=lsm.NE_HEATBATH, J=0.0, T=W.ne_temperature(0.3)), 40),
     (dict(dims=2, L=64, model=lsm.NE_METROPOLIS, J=0.0, T=W.ne_temperature(0.3)), 60),
     (dict(dims=2, L=160, model=lsm.NE_METROPOLIS, J=0.0, T=W.ne_temperature(0.2)), 30),
-    # large enough for the resident family (whole CTAs of word columns, several march segments)
+    # larger lattices: several march segments per word column (tiled), many rows per slab
     (dict(dims=2, L=1024, T=2.269), 12),
     (dict(dims=2, L=2048, T=2.0, h=0.02), 7),
     (dict(dims=3, L=128, T=4.5115), 5),
@@ -89,7 +89,7 @@ SHAPES = [
     (dict(dims=2, L=1024, model=lsm.NE_HEATBATH, J=0.0, T=W.ne_temperature(0.3)), 16),
     (dict(dims=2, L=3072, model=lsm.NE_METROPOLIS, J=0.0, T=W.ne_temperature(0.2)), 6),
 ]
-FAMILIES = [lsm.KERNEL_GENERIC, lsm.KERNEL_TILED, lsm.KERNEL_RESIDENT, lsm.KERNEL_SMALL, lsm.KERNEL_SLAB]   # + BULK: below
+FAMILIES = [lsm.KERNEL_GENERIC, lsm.KERNEL_TILED, lsm.KERNEL_SMALL, lsm.KERNEL_SLAB]   # + BULK: below
 
 
 def test_device_philox_known_answers_and_random():
@@ -314,8 +314,8 @@ def test_cfg1_full_length(family):
     try:
         lat, orc = make_pair(family, **w.create_args())
     except lsm.LsmError as e:
-        if e.code == lsm.ERR_UNSUPPORTED and family in (lsm.KERNEL_RESIDENT, lsm.KERNEL_SLAB):
-            pytest.skip("64 x 64 has fewer word columns than one CTA of the resident family / is below the slab family's sizes")
+        if e.code == lsm.ERR_UNSUPPORTED and family == lsm.KERNEL_SLAB:
+            pytest.skip("64 x 64 is below the slab family's sizes")
         raise
     got = lat.sweep_record(w.sweeps).cpu().numpy()
     want = orc.sweep_record(w.sweeps)
@@ -459,7 +459,7 @@ FULL = [
 ]
 
 
-@pytest.mark.parametrize("family", [lsm.KERNEL_AUTO, lsm.KERNEL_RESIDENT])
+@pytest.mark.parametrize("family", [lsm.KERNEL_AUTO, lsm.KERNEL_TILED])
 @pytest.mark.parametrize("name,k_first,t_late", FULL)
 def test_full_size_prefix_and_late_spot_check(name, k_first, t_late, family):
     """BASELINE.json's full sizes in the launch configuration bench.py times (AUTO kernel family,
