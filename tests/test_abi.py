@@ -76,7 +76,14 @@ def test_workspace_and_argument_errors(lib):
     assert not h.value
     assert lib.lsm_sweep(None, 1, None) == lsm.ERR_ARG
     assert lib.lsm_destroy(None) == lsm.ERR_ARG
-    for code in (0, -1, -2, -3, -4, -5, -99):
+    # entry points added in round 3: argument errors are found before any CUDA call
+    buf = ctypes.c_void_p(8)
+    assert lib.lsm_sweep_record_host_noalloc(None, 1, buf, None) == lsm.ERR_ARG
+    assert lib.lsm_batch_sweep_random_tile(None, 1, 32, 16, 0, None, None) == lsm.ERR_ARG
+    assert b"LSM_NOALLOC_MAX_SWEEPS" in lib.lsm_strerror(lsm.ERR_LIMIT)
+    text = open(os.path.join(ROOT, "include", "lsm.h")).read()
+    assert f"LSM_NOALLOC_MAX_SWEEPS = {lsm.NOALLOC_MAX_SWEEPS}" in text and "LSM_ERR_LIMIT = -6" in text
+    for code in (0, -1, -2, -3, -4, -5, -6, -99):
         assert len(lib.lsm_strerror(code)) > 0
 
 
