@@ -41,7 +41,8 @@ NCU_DRAM_BYTES_PER_LAUNCH = {
     "hbm3d_1024": (1083.86e6 + 497.63e6, "profiles/r2_tiled_variants_ncu.md"),
 }
 # smsp__issue_active.avg.pct_of_peak_sustained_active of the half-sweep kernel in the cited capture
-NCU_ISSUE_ACTIVE_PCT = {"cfg2_T2.269": 57.5}     # profiles/r2_cfg2_final.md
+NCU_ISSUE_ACTIVE_PCT = {"cfg2_T2.269": 57.5,     # profiles/r2_cfg2_final.md
+                        "cfg4": 52.9}            # profiles/r3_cfg4.md
 KERNEL_FAMILY = {1: "generic", 2: "tiled", 4: "small", 5: "slab", 6: "bulk"}
 KERNEL_NAME = {1: "k_sweep_generic (half-sweep)", 2: "k_sweep_tiled (half-sweep)",
                4: "k_sweep_small_lane (per half-sweep share of one launch)",
